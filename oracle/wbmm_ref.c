@@ -1,0 +1,277 @@
+/*
+ * wbmm_ref.c -- CPU ORACLE for the WBMM operator.  TEST INFRASTRUCTURE ONLY.
+ *
+ * This file is the plain, slow, obviously-correct statement of what the GPU
+ * library must compute.  Only tests/, __graft_entry__.smoke() and bench.py's
+ * cpu_baseline / --impl reference legs may build, load or call it.  It shares
+ * no code, header, table or helper with paper_2607_02097_b200/csrc.
+ *
+ * Everything is fp64 (inputs, accumulation, outputs).  Callers round their
+ * inputs to the case dtype BEFORE widening to double; the oracle never rounds.
+ *
+ * What it follows (PAPER.md = /root/reference/PAPER.md at authoring time):
+ *   - relative position index I[i,j]            PAPER.md:188-193  (Eq. 6-7)
+ *   - weight construction  M = R[:, I]          PAPER.md:195-198  (Eq. 8)
+ *   - zero padding to a multiple of w, crop     PAPER.md:176-182  (Eq. 4-5)
+ *   - window partition / bmm / inverse reshape  PAPER.md:157-173  (Alg. 1)
+ *   - backward "gradients flow through R"
+ * Readings:
+ *   A1 orientation y = W_c . x with W_c[i,j] = T[c, rel(i,j)], i = OUTPUT
+ *      position, j = INPUT position (BASELINE.json north_star); the paper's
+ *      X.M form is the same operator with the table reversed.
+ *   A2 in-window order is row-major i = r*w + c.
+ *   A4 padding is on the bottom and right.
+ *   A6 shift: x^[h,v] = x~[(h+s_h) mod H', (v+s_w) mod W'] over the PADDED
+ *      extent, inverse roll on the output, then crop.
+ *   A11 dy is zero outside HxW; dx is cropped.
+ *
+ * Parity pins: tests/test_oracle_pins.py (closed forms for the index, delta /
+ * one-hot / all-ones tables, Theorem 3.2 against a library conv2d, adjoint
+ * identities, finite differences, brute force).  No value printed by the
+ * paper exists for the operator, so numerical parity with the AUTHORS' code is
+ * unpinned; parity with the paper's DEFINITION is pinned.
+ *
+ * Layout codes: 0 = NCHW, 1 = NHWC.  T is [C][(2w-1)^2] row-major.
+ */
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+int wbmm_ref_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+void wbmm_ref_set_threads(int n)
+{
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
+/* Eq. 6-7: i, j are row-major in-window positions, i = r*w + c. */
+int64_t wbmm_ref_rel_index(int w, int i, int j)
+{
+    int ri = i / w, ci = i % w;
+    int rj = j / w, cj = j % w;
+    int dh = ri - rj;                 /* Eq. 6 */
+    int dw = ci - cj;
+    return (int64_t)(dh + w - 1) * (2 * w - 1) + (dw + w - 1);   /* Eq. 7 */
+}
+
+/* I as a dense [N][N] buffer (the paper's "precomputed buffer"). */
+void wbmm_ref_index_matrix(int w, int64_t *I)
+{
+    int N = w * w;
+    for (int i = 0; i < N; ++i)
+        for (int j = 0; j < N; ++j)
+            I[(size_t)i * N + j] = wbmm_ref_rel_index(w, i, j);
+}
+
+/* Eq. 8: M[c,i,j] = T[c, I[i,j]]. */
+void wbmm_ref_weight_matrix(int C, int w, const double *T, double *M)
+{
+    int N = w * w;
+    int nb = (2 * w - 1) * (2 * w - 1);
+    int64_t *I = (int64_t *)malloc(sizeof(int64_t) * (size_t)N * N);
+    wbmm_ref_index_matrix(w, I);
+    for (int c = 0; c < C; ++c)
+        for (int i = 0; i < N; ++i)
+            for (int j = 0; j < N; ++j)
+                M[((size_t)c * N + i) * N + j] = T[(size_t)c * nb + I[(size_t)i * N + j]];
+    free(I);
+}
+
+static inline size_t elem_off(int layout, int B, int C, int H, int W,
+                              int b, int c, int h, int v)
+{
+    (void)B;
+    if (layout == 0)
+        return (((size_t)b * C + c) * H + h) * W + v;       /* NCHW */
+    return (((size_t)b * H + h) * W + v) * C + c;           /* NHWC */
+}
+
+static inline int padded(int n, int w)
+{
+    int pad = (w - n % w) % w;        /* Eq. 4-5 */
+    return n + pad;
+}
+
+static inline int modp(int a, int m)
+{
+    int r = a % m;
+    return r < 0 ? r + m : r;
+}
+
+/* x^ : zero-extended (A4) then cyclically shifted (A6) view of a tensor. */
+static inline double load_hat(const double *x, int layout, int B, int C, int H, int W,
+                              int Hp, int Wp, int sh, int sw, int b, int c, int h, int v)
+{
+    int hs = modp(h + sh, Hp);
+    int vs = modp(v + sw, Wp);
+    if (hs >= H || vs >= W)
+        return 0.0;
+    return x[elem_off(layout, B, C, H, W, b, c, hs, vs)];
+}
+
+/*
+ * Forward, MATRIX form (Alg. 1): build I, build W_c = T[c, I], gather each
+ * window into a length-N vector, y_win = W_c . x_win, scatter back, un-shift,
+ * crop.
+ */
+int wbmm_ref_forward_matrix(int B, int C, int H, int W, int w, int sh, int sw, int layout,
+                            const double *x, const double *T, double *y)
+{
+    if (B < 0 || C < 0 || H < 1 || W < 1 || w < 1 || sh < 0 || sw < 0 || sh >= w || sw >= w)
+        return 1;
+    const int N = w * w;
+    const int nb = (2 * w - 1) * (2 * w - 1);
+    const int Hp = padded(H, w), Wp = padded(W, w);
+    const int nwh = Hp / w, nww = Wp / w;
+    int64_t *I = (int64_t *)malloc(sizeof(int64_t) * (size_t)N * N);
+    if (!I) return 2;
+    wbmm_ref_index_matrix(w, I);
+
+#pragma omp parallel
+    {
+        double *Wc = (double *)malloc(sizeof(double) * (size_t)N * N);
+        double *xw = (double *)malloc(sizeof(double) * (size_t)N);
+        double *yw = (double *)malloc(sizeof(double) * (size_t)N);
+#pragma omp for schedule(static)
+        for (int c = 0; c < C; ++c) {
+            for (int i = 0; i < N; ++i)
+                for (int j = 0; j < N; ++j)
+                    Wc[(size_t)i * N + j] = T[(size_t)c * nb + I[(size_t)i * N + j]];
+            for (int b = 0; b < B; ++b)
+                for (int wy = 0; wy < nwh; ++wy)
+                    for (int wx = 0; wx < nww; ++wx) {
+                        for (int j = 0; j < N; ++j)
+                            xw[j] = load_hat(x, layout, B, C, H, W, Hp, Wp, sh, sw, b, c,
+                                             wy * w + j / w, wx * w + j % w);
+                        for (int i = 0; i < N; ++i) {
+                            double acc = 0.0;
+                            for (int j = 0; j < N; ++j)
+                                acc += Wc[(size_t)i * N + j] * xw[j];
+                            yw[i] = acc;
+                        }
+                        for (int i = 0; i < N; ++i) {
+                            /* y^ at (h,v) goes to y~ at ((h+sh) mod H', (v+sw) mod W') */
+                            int h = modp(wy * w + i / w + sh, Hp);
+                            int v = modp(wx * w + i % w + sw, Wp);
+                            if (h < H && v < W)
+                                y[elem_off(layout, B, C, H, W, b, c, h, v)] = yw[i];
+                        }
+                    }
+        }
+        free(Wc); free(xw); free(yw);
+    }
+    free(I);
+    return 0;
+}
+
+/*
+ * Forward, DIRECT form: for every output pixel, the windowed depthwise sum
+ *   y^[h,v] = sum_{(h',v') in win(h,v)} T[c, (h-h'+w-1)(2w-1) + (v-v'+w-1)] x^[h',v'].
+ * No index matrix, no weight matrix: structurally independent of the matrix form.
+ */
+int wbmm_ref_forward_direct(int B, int C, int H, int W, int w, int sh, int sw, int layout,
+                            const double *x, const double *T, double *y)
+{
+    if (B < 0 || C < 0 || H < 1 || W < 1 || w < 1 || sh < 0 || sw < 0 || sh >= w || sw >= w)
+        return 1;
+    const int tw = 2 * w - 1;
+    const int Hp = padded(H, w), Wp = padded(W, w);
+    const long planes = (long)B * C;
+
+#pragma omp parallel for schedule(static)
+    for (long pc = 0; pc < planes; ++pc) {
+        int b = (int)(pc / C), c = (int)(pc % C);
+        const double *Tc = T + (size_t)c * tw * tw;
+        for (int ho = 0; ho < H; ++ho)
+            for (int vo = 0; vo < W; ++vo) {
+                /* output pixel (ho,vo) of y~ is y^ at (h,v) = (ho - sh, vo - sw) mod padded */
+                int h = modp(ho - sh, Hp), v = modp(vo - sw, Wp);
+                int h0 = (h / w) * w, v0 = (v / w) * w;
+                double acc = 0.0;
+                for (int hq = h0; hq < h0 + w; ++hq)
+                    for (int vq = v0; vq < v0 + w; ++vq)
+                        acc += Tc[(h - hq + w - 1) * tw + (v - vq + w - 1)] *
+                               load_hat(x, layout, B, C, H, W, Hp, Wp, sh, sw, b, c, hq, vq);
+                y[elem_off(layout, B, C, H, W, b, c, ho, vo)] = acc;
+            }
+    }
+    return 0;
+}
+
+/*
+ * Backward (autograd of Alg. 1):
+ *   dx^_win = W_c^T . dy^_win
+ *   dT[c,k] = sum_{b,windows} sum_{(i,j): I[i,j]=k} dy^_win[i] * x^_win[j]
+ * dy is zero outside HxW (A11); dx is un-shifted and cropped.  Either output
+ * may be NULL.  dT is overwritten.
+ */
+int wbmm_ref_backward(int B, int C, int H, int W, int w, int sh, int sw, int layout,
+                      const double *x, const double *T, const double *dy,
+                      double *dx, double *dT)
+{
+    if (B < 0 || C < 0 || H < 1 || W < 1 || w < 1 || sh < 0 || sw < 0 || sh >= w || sw >= w)
+        return 1;
+    const int N = w * w;
+    const int nb = (2 * w - 1) * (2 * w - 1);
+    const int Hp = padded(H, w), Wp = padded(W, w);
+    const int nwh = Hp / w, nww = Wp / w;
+    int64_t *I = (int64_t *)malloc(sizeof(int64_t) * (size_t)N * N);
+    if (!I) return 2;
+    wbmm_ref_index_matrix(w, I);
+
+#pragma omp parallel
+    {
+        double *Wc = (double *)malloc(sizeof(double) * (size_t)N * N);
+        double *xw = (double *)malloc(sizeof(double) * (size_t)N);
+        double *gw = (double *)malloc(sizeof(double) * (size_t)N);
+#pragma omp for schedule(static)
+        for (int c = 0; c < C; ++c) {
+            for (int i = 0; i < N; ++i)
+                for (int j = 0; j < N; ++j)
+                    Wc[(size_t)i * N + j] = T[(size_t)c * nb + I[(size_t)i * N + j]];
+            if (dT)
+                for (int k = 0; k < nb; ++k) dT[(size_t)c * nb + k] = 0.0;
+            for (int b = 0; b < B; ++b)
+                for (int wy = 0; wy < nwh; ++wy)
+                    for (int wx = 0; wx < nww; ++wx) {
+                        for (int j = 0; j < N; ++j) {
+                            int h = wy * w + j / w, v = wx * w + j % w;
+                            xw[j] = load_hat(x, layout, B, C, H, W, Hp, Wp, sh, sw, b, c, h, v);
+                            gw[j] = load_hat(dy, layout, B, C, H, W, Hp, Wp, sh, sw, b, c, h, v);
+                        }
+                        if (dT)
+                            for (int i = 0; i < N; ++i)
+                                for (int j = 0; j < N; ++j)
+                                    dT[(size_t)c * nb + I[(size_t)i * N + j]] += gw[i] * xw[j];
+                        if (dx)
+                            for (int j = 0; j < N; ++j) {
+                                double acc = 0.0;
+                                for (int i = 0; i < N; ++i)
+                                    acc += Wc[(size_t)i * N + j] * gw[i];
+                                int h = modp(wy * w + j / w + sh, Hp);
+                                int v = modp(wx * w + j % w + sw, Wp);
+                                if (h < H && v < W)
+                                    dx[elem_off(layout, B, C, H, W, b, c, h, v)] = acc;
+                            }
+                    }
+        }
+        free(Wc); free(xw); free(gw);
+    }
+    free(I);
+    return 0;
+}

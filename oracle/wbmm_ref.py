@@ -1,0 +1,137 @@
+"""ctypes wrapper around oracle/wbmm_ref.c -- the CPU ORACLE.  TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+legs may import this module.  It never imports the product package and shares no
+code with it.  All arrays are float64 numpy arrays (callers round to the case
+dtype first, then widen); see the header of wbmm_ref.c for citations and readings.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "wbmm_ref.c")
+_LIB = os.path.join(_HERE, "libwbmm_ref.so")
+
+NCHW, NHWC = 0, 1
+
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (-O2, no fast-math, OpenMP).  Returns the .so path."""
+    stale = (not os.path.exists(_LIB)) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC)
+    if force or stale:
+        cmd = ["gcc", "-O2", "-std=c99", "-fopenmp", "-fPIC", "-shared", "-Wall", "-Wextra",
+               "-o", _LIB, _SRC]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is not None:
+        return _lib
+    lib = ctypes.CDLL(build())
+    dp = ctypes.POINTER(ctypes.c_double)
+    ip = ctypes.POINTER(ctypes.c_int64)
+    i = ctypes.c_int
+    lib.wbmm_ref_rel_index.restype = ctypes.c_int64
+    lib.wbmm_ref_rel_index.argtypes = [i, i, i]
+    lib.wbmm_ref_index_matrix.restype = None
+    lib.wbmm_ref_index_matrix.argtypes = [i, ip]
+    lib.wbmm_ref_weight_matrix.restype = None
+    lib.wbmm_ref_weight_matrix.argtypes = [i, i, dp, dp]
+    for name in ("wbmm_ref_forward_matrix", "wbmm_ref_forward_direct"):
+        f = getattr(lib, name)
+        f.restype = i
+        f.argtypes = [i] * 8 + [dp, dp, dp]
+    lib.wbmm_ref_backward.restype = i
+    lib.wbmm_ref_backward.argtypes = [i] * 8 + [dp, dp, dp, dp, dp]
+    lib.wbmm_ref_num_threads.restype = i
+    lib.wbmm_ref_set_threads.argtypes = [i]
+    _lib = lib
+    return lib
+
+
+def _d(a):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    return a, a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+
+def num_threads() -> int:
+    return int(_load().wbmm_ref_num_threads())
+
+
+def set_threads(n: int) -> None:
+    _load().wbmm_ref_set_threads(int(n))
+
+
+def rel_index(w: int, i: int, j: int) -> int:
+    """Eq. 7."""
+    return int(_load().wbmm_ref_rel_index(w, i, j))
+
+
+def index_matrix(w: int) -> np.ndarray:
+    n = w * w
+    out = np.empty((n, n), dtype=np.int64)
+    _load().wbmm_ref_index_matrix(w, out.ctypes.data_as(ctypes.POINTER(ctypes.c_int64)))
+    return out
+
+
+def weight_matrix(T: np.ndarray, w: int) -> np.ndarray:
+    """Eq. 8: M[c] = T[c, I]."""
+    T, tp = _d(T)
+    C = T.shape[0]
+    assert T.shape[1] == (2 * w - 1) ** 2
+    n = w * w
+    M = np.empty((C, n, n), dtype=np.float64)
+    _load().wbmm_ref_weight_matrix(C, w, tp, M.ctypes.data_as(ctypes.POINTER(ctypes.c_double)))
+    return M
+
+
+def _dims(x: np.ndarray, layout: int):
+    if layout == NCHW:
+        B, C, H, W = x.shape
+    else:
+        B, H, W, C = x.shape
+    return B, C, H, W
+
+
+def forward(x, T, w, shift=(0, 0), layout=NCHW, form="direct") -> np.ndarray:
+    """y = WBMM(x; T, w).  form = "direct" | "matrix" (two independent evaluations)."""
+    x, xp = _d(x)
+    T, tp = _d(T)
+    B, C, H, W = _dims(x, layout)
+    assert T.shape == (C, (2 * w - 1) ** 2), (T.shape, C, w)
+    y = np.zeros_like(x)
+    fn = {"direct": _load().wbmm_ref_forward_direct, "matrix": _load().wbmm_ref_forward_matrix}[form]
+    rc = fn(B, C, H, W, w, int(shift[0]), int(shift[1]), layout, xp, tp,
+            y.ctypes.data_as(ctypes.POINTER(ctypes.c_double)))
+    if rc != 0:
+        raise ValueError(f"oracle rejected arguments (rc={rc})")
+    return y
+
+
+def backward(x, T, dy, w, shift=(0, 0), layout=NCHW, need_dx=True, need_dT=True):
+    """Returns (dx, dT) in float64; either is None when not requested."""
+    x, xp = _d(x)
+    T, tp = _d(T)
+    dy, gp = _d(dy)
+    assert dy.shape == x.shape
+    B, C, H, W = _dims(x, layout)
+    assert T.shape == (C, (2 * w - 1) ** 2)
+    null = ctypes.POINTER(ctypes.c_double)()
+    dx = np.zeros_like(x) if need_dx else None
+    dT = np.zeros_like(T) if need_dT else None
+    rc = _load().wbmm_ref_backward(
+        B, C, H, W, w, int(shift[0]), int(shift[1]), layout, xp, tp, gp,
+        dx.ctypes.data_as(ctypes.POINTER(ctypes.c_double)) if need_dx else null,
+        dT.ctypes.data_as(ctypes.POINTER(ctypes.c_double)) if need_dT else null)
+    if rc != 0:
+        raise ValueError(f"oracle rejected arguments (rc={rc})")
+    return dx, dT

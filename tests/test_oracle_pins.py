@@ -1,0 +1,408 @@
+"""Pins for the CPU oracle (oracle/wbmm_ref.c): every function is checked against something
+other than itself -- closed forms, invariants, special cases that reduce to a library routine
+(torch conv2d, Theorem 3.2), exact adjoint identities, finite differences, pure-Python brute
+force, and the sizes the paper prints (tests/golden/paper_sizes.txt).
+
+Each pin names the mistake it would catch.  CPU only (-m "not gpu").
+"""
+import os
+
+import numpy as np
+import pytest
+import torch
+import torch.nn.functional as F
+
+NCHW, NHWC = 0, 1
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden", "paper_sizes.txt")
+
+
+def rng(seed):
+    return np.random.default_rng(seed)
+
+
+def golden():
+    out = {}
+    with open(GOLDEN) as f:
+        for line in f:
+            line = line.split("#")[0].strip()
+            if line:
+                k, v = line.split("=")
+                out[k.strip()] = float(v)
+    return out
+
+
+# ----------------------------------------------------------------------------- a1: index
+@pytest.mark.parametrize("w", [1, 2, 3, 4, 7, 14])
+def test_index_closed_form_properties(oracle, w):
+    """Eq. 6-7.  Catches: swapped i/j, wrong stride (2w vs 2w-1), off-by-one."""
+    I = oracle.index_matrix(w)
+    N, tw = w * w, 2 * w - 1
+    nb = tw * tw
+    assert I.shape == (N, N)
+    assert I.min() == 0 and I.max() == nb - 1              # Theorem 3.1: exactly (2w-1)^2 offsets
+    assert np.array_equal(I.T, nb - 1 - I)                 # rel(j,i) = nb-1-rel(i,j)
+    centre = (w - 1) * tw + (w - 1)
+    assert np.all(np.diag(I) == centre)                    # zero offset -> centre bin
+    # bin multiplicity (w-|dr|)(w-|dc|)
+    counts = np.bincount(I.ravel(), minlength=nb).reshape(tw, tw)
+    d = np.abs(np.arange(tw) - (w - 1))
+    assert np.array_equal(counts, np.outer(w - d, w - d))
+    # independent construction from coordinate grids (broadcast, no loops)
+    r, c = np.divmod(np.arange(N), w)
+    I2 = (r[:, None] - r[None, :] + w - 1) * tw + (c[:, None] - c[None, :] + w - 1)
+    assert np.array_equal(I, I2)
+    # scalar entry point agrees with the matrix
+    for (i, j) in [(0, 0), (0, N - 1), (N - 1, 0), (N // 2, N // 3)]:
+        assert oracle.rel_index(w, i, j) == I[i, j]
+
+
+def test_index_paper_sizes(oracle):
+    """Sizes the paper prints (golden file, each with its citation)."""
+    g = golden()
+    assert (2 * 7 - 1) ** 2 == g["table_entries_w7"]
+    assert 2 * 7 - 1 == g["table_side_w7"] and 2 * 14 - 1 == g["table_side_w14"]
+    assert oracle.index_matrix(7).shape[0] == g["matrix_side_w7"]
+    assert oracle.index_matrix(14).shape[0] == g["matrix_side_w14"]
+    assert oracle.index_matrix(7).max() + 1 == g["table_entries_w7"]
+    assert oracle.index_matrix(14).max() + 1 == g["table_side_w14"] ** 2
+    # centre bins quoted in SURVEY 8(c): 84 (w=7), 364 (w=14)
+    assert oracle.rel_index(7, 0, 0) == 84 and oracle.rel_index(14, 5, 5) == 364
+    M = oracle.weight_matrix(np.zeros((256, 27 * 27)), 14)
+    assert abs(M.size * 4 / 2 ** 20 - g["m_footprint_mib_c256_w14_fp32"]) < 0.1   # fp32 bytes
+    assert abs(196 / 25 - g["rf_ratio_w14_vs_k5"]) < 0.05
+
+
+def test_weight_matrix_is_gather(oracle):
+    """Eq. 8: values copied, no arithmetic.  Table = its own bin index makes M == I."""
+    for w in (3, 7):
+        nb = (2 * w - 1) ** 2
+        T = np.tile(np.arange(nb, dtype=np.float64), (2, 1))
+        T[1] += 1000
+        M = oracle.weight_matrix(T, w)
+        I = oracle.index_matrix(w)
+        assert np.array_equal(M[0], I) and np.array_equal(M[1], I + 1000)
+
+
+# ----------------------------------------------------------------------------- forward
+CASES = [
+    # B, C, H, W, w, shift
+    (2, 3, 6, 6, 3, (0, 0)),
+    (1, 2, 8, 12, 4, (0, 0)),
+    (2, 2, 7, 10, 3, (0, 0)),        # ragged both axes
+    (2, 2, 9, 6, 3, (1, 2)),         # shift, odd w
+    (1, 3, 10, 7, 4, (2, 2)),        # shift + ragged, even w
+    (1, 2, 14, 14, 7, (3, 3)),
+]
+
+
+def _to_layout(a, layout):
+    return np.ascontiguousarray(a.transpose(0, 2, 3, 1)) if layout == NHWC else a
+
+
+def _from_layout(a, layout):
+    return a.transpose(0, 3, 1, 2) if layout == NHWC else a
+
+
+@pytest.mark.parametrize("case", CASES)
+@pytest.mark.parametrize("layout", [NCHW, NHWC])
+def test_matrix_form_equals_direct_form(oracle, case, layout):
+    """Two structurally different evaluations (Alg. 1 vs windowed depthwise sum) must agree."""
+    B, C, H, W, w, s = case
+    r = rng(11)
+    x = r.standard_normal((B, C, H, W))
+    T = r.standard_normal((C, (2 * w - 1) ** 2))
+    ym = oracle.forward(_to_layout(x, layout), T, w, s, layout, "matrix")
+    yd = oracle.forward(_to_layout(x, layout), T, w, s, layout, "direct")
+    assert np.allclose(ym, yd, rtol=0, atol=1e-12)
+    # layouts: NHWC result == NCHW result on permuted copies
+    y0 = oracle.forward(x, T, w, s, NCHW, "direct")
+    assert np.array_equal(_from_layout(yd, layout), y0)
+
+
+def brute_force(x, T, w, s=(0, 0)):
+    """Pure-Python restatement of the DEFINITION, NCHW, tiny inputs only."""
+    B, C, H, W = x.shape
+    Hp, Wp = -(-H // w) * w, -(-W // w) * w
+    tw = 2 * w - 1
+    xt = np.zeros((B, C, Hp, Wp))
+    xt[:, :, :H, :W] = x
+    xh = np.zeros_like(xt)
+    for h in range(Hp):
+        for v in range(Wp):
+            xh[:, :, h, v] = xt[:, :, (h + s[0]) % Hp, (v + s[1]) % Wp]
+    yh = np.zeros_like(xt)
+    for b in range(B):
+        for c in range(C):
+            for h in range(Hp):
+                for v in range(Wp):
+                    h0, v0 = (h // w) * w, (v // w) * w
+                    acc = 0.0
+                    for hq in range(h0, h0 + w):
+                        for vq in range(v0, v0 + w):
+                            acc += T[c, (h - hq + w - 1) * tw + (v - vq + w - 1)] * xh[b, c, hq, vq]
+                    yh[b, c, h, v] = acc
+    yt = np.zeros_like(xt)
+    for h in range(Hp):
+        for v in range(Wp):
+            yt[:, :, h, v] = yh[:, :, (h - s[0]) % Hp, (v - s[1]) % Wp]
+    return yt[:, :, :H, :W]
+
+
+@pytest.mark.parametrize("case", CASES[:5])
+def test_brute_force_tiny(oracle, case):
+    B, C, H, W, w, s = case
+    r = rng(5)
+    x = r.standard_normal((B, C, H, W))
+    T = r.standard_normal((C, (2 * w - 1) ** 2))
+    ref = brute_force(x, T, w, s)
+    for form in ("direct", "matrix"):
+        assert np.allclose(oracle.forward(x, T, w, s, NCHW, form), ref, rtol=0, atol=1e-12)
+
+
+def test_brute_force_config1(oracle):
+    """BASELINE.json config 1: B=1, C=4, 14x14, w=7, fp32 inputs, seed 0."""
+    import synth_inputs as si
+    d = si.make(si.CFG1)
+    x, T = d["x"].double().numpy(), d["T"].double().numpy()
+    ref = brute_force(x, T, 7)
+    assert np.allclose(oracle.forward(x, T, 7, form="direct"), ref, rtol=0, atol=1e-13)
+    assert np.allclose(oracle.forward(x, T, 7, form="matrix"), ref, rtol=0, atol=1e-13)
+
+
+@pytest.mark.parametrize("form", ["direct", "matrix"])
+@pytest.mark.parametrize("w,s", [(3, (0, 0)), (4, (0, 0)), (3, (2, 1)), (4, (2, 2))])
+def test_delta_table_is_identity(oracle, form, w, s):
+    """Delta at the zero-offset bin => y == x exactly.  With a shift this also pins
+    shift o inverse-roll == identity."""
+    r = rng(2)
+    x = r.standard_normal((2, 3, 3 * w - 1, 2 * w + 1))      # ragged
+    tw = 2 * w - 1
+    T = np.zeros((3, tw * tw))
+    T[:, (w - 1) * tw + (w - 1)] = 1.0
+    assert np.array_equal(oracle.forward(x, T, w, s, NCHW, form), x)
+
+
+@pytest.mark.parametrize("form", ["direct", "matrix"])
+@pytest.mark.parametrize("w", [3, 4])
+def test_one_hot_table_all_bins(oracle, form, w):
+    """One-hot table at bin (dr,dc): y[r,c] = x[r-dr, c-dc] if that lies in the same window
+    else 0 (north_star orientation: offset = out - in).  Exact.  Catches a transposed W_c,
+    a wrong sign, a wrong row stride -- for EVERY bin."""
+    r = rng(3)
+    H = W = 2 * w
+    x = r.standard_normal((1, 1, H, W))
+    tw = 2 * w - 1
+    for dr in range(-(w - 1), w):
+        for dc in range(-(w - 1), w):
+            T = np.zeros((1, tw * tw))
+            T[0, (dr + w - 1) * tw + (dc + w - 1)] = 1.0
+            y = oracle.forward(x, T, w, (0, 0), NCHW, form)
+            exp = np.zeros_like(x)
+            for wy in range(2):
+                for wx in range(2):
+                    win = x[0, 0, wy * w:(wy + 1) * w, wx * w:(wx + 1) * w]
+                    out = np.zeros((w, w))
+                    # out[r, c] = win[r-dr, c-dc] where valid
+                    r0, r1 = max(0, dr), min(w, w + dr)
+                    c0, c1 = max(0, dc), min(w, w + dc)
+                    out[r0:r1, c0:c1] = win[r0 - dr:r1 - dr, c0 - dc:c1 - dc]
+                    exp[0, 0, wy * w:(wy + 1) * w, wx * w:(wx + 1) * w] = out
+            assert np.array_equal(y, exp), (dr, dc)
+
+
+@pytest.mark.parametrize("form", ["direct", "matrix"])
+def test_all_ones_table_gives_window_sums(oracle, form):
+    """Pins partition + bottom/right zero padding (A4): small-integer x, exact."""
+    w, H, W = 4, 10, 7
+    r = rng(4)
+    x = r.integers(-3, 4, size=(2, 2, H, W)).astype(np.float64)
+    T = np.ones((2, (2 * w - 1) ** 2))
+    y = oracle.forward(x, T, w, (0, 0), NCHW, form)
+    for h in range(H):
+        for v in range(W):
+            h0, v0 = (h // w) * w, (v // w) * w
+            s = x[:, :, h0:min(h0 + w, H), v0:min(v0 + w, W)].sum(axis=(2, 3))
+            assert np.array_equal(y[:, :, h, v], s)
+
+
+def test_linearity(oracle):
+    r = rng(6)
+    w = 3
+    x1, x2 = r.standard_normal((2, 2, 2, 7, 8))
+    T1, T2 = r.standard_normal((2, 2, 25))
+    f = lambda x, T: oracle.forward(x, T, w, (1, 2))
+    assert np.allclose(f(2 * x1 - 3 * x2, T1), 2 * f(x1, T1) - 3 * f(x2, T1), atol=1e-12)
+    assert np.allclose(f(x1, 2 * T1 - 3 * T2), 2 * f(x1, T1) - 3 * f(x1, T2), atol=1e-12)
+
+
+@pytest.mark.parametrize("w", [3, 4, 7, 14])
+def test_theorem_3_2_single_window_is_depthwise_conv(oracle, w):
+    """Theorem 3.2: on a single window (H=W=w) the operator is a zero-padded
+    depthwise conv with a (2w-1)^2 kernel -- a LIBRARY routine (torch conv2d, cross-correlation).
+    north_star orientation (offset = out - in) is a true convolution => flipped kernel;
+    the paper's orientation (offset = in - out) is the table reversed (reading A1)."""
+    r = rng(7)
+    C = 3
+    tw = 2 * w - 1
+    x = r.standard_normal((2, C, w, w))
+    T = r.standard_normal((C, tw * tw))
+    y = oracle.forward(x, T, w)
+    K = torch.from_numpy(T.reshape(C, 1, tw, tw))
+    conv_flipped = F.conv2d(torch.from_numpy(x), torch.flip(K, dims=(2, 3)), padding=w - 1, groups=C)
+    assert np.allclose(y, conv_flipped.numpy(), rtol=0, atol=1e-12)
+    # paper convention: WBMM_ns(x; reversed(R)) == conv2d(x, R) (cross-correlation, no flip)
+    R = T[:, ::-1].copy()
+    conv_paper = F.conv2d(torch.from_numpy(x), torch.from_numpy(R.reshape(C, 1, tw, tw)),
+                          padding=w - 1, groups=C)
+    assert np.allclose(y, conv_paper.numpy(), rtol=0, atol=1e-12)
+
+
+def test_multi_window_is_per_window_conv(oracle):
+    """Windows do not interact: each window equals the conv on its isolated crop."""
+    r = rng(8)
+    w, C = 4, 2
+    tw = 2 * w - 1
+    x = r.standard_normal((1, C, 8, 12))
+    T = r.standard_normal((C, tw * tw))
+    y = oracle.forward(x, T, w)
+    K = torch.flip(torch.from_numpy(T.reshape(C, 1, tw, tw)), dims=(2, 3))
+    for wy in range(2):
+        for wx in range(3):
+            crop = x[:, :, wy * w:(wy + 1) * w, wx * w:(wx + 1) * w]
+            ref = F.conv2d(torch.from_numpy(crop.copy()), K, padding=w - 1, groups=C).numpy()
+            assert np.allclose(y[:, :, wy * w:(wy + 1) * w, wx * w:(wx + 1) * w], ref, atol=1e-12)
+
+
+def test_padding_equals_explicit_pad_then_crop(oracle):
+    """Eq. 4-5, 'padding is removed'."""
+    r = rng(9)
+    w = 4
+    x = r.standard_normal((2, 2, 10, 7))
+    T = r.standard_normal((2, 49))
+    xp = np.zeros((2, 2, 12, 8))
+    xp[:, :, :10, :7] = x
+    assert np.array_equal(oracle.forward(x, T, w), oracle.forward(xp, T, w)[:, :, :10, :7])
+
+
+@pytest.mark.parametrize("w,s,H,W", [(3, (1, 2), 9, 6), (4, (2, 2), 8, 8), (3, (2, 2), 7, 8), (7, (3, 3), 14, 21)])
+def test_shift_equals_explicit_roll(oracle, w, s, H, W):
+    """A6: pad, roll by -s over the padded extent, WBMM, roll back by +s, crop."""
+    r = rng(10)
+    x = r.standard_normal((2, 2, H, W))
+    T = r.standard_normal((2, (2 * w - 1) ** 2))
+    Hp, Wp = -(-H // w) * w, -(-W // w) * w
+    xp = np.zeros((2, 2, Hp, Wp))
+    xp[:, :, :H, :W] = x
+    xr = np.roll(xp, shift=(-s[0], -s[1]), axis=(2, 3))       # x^[h] = x~[(h+s) mod H']
+    yr = oracle.forward(xr, T, w)
+    ref = np.roll(yr, shift=(s[0], s[1]), axis=(2, 3))[:, :, :H, :W]
+    assert np.allclose(oracle.forward(x, T, w, s), ref, rtol=0, atol=1e-13)
+    assert np.array_equal(oracle.forward(x, T, w, (0, 0)), oracle.forward(x, T, w))
+
+
+def test_shift_direction_pinned_by_odd_w_not_by_even_w(oracle):
+    """For even w and s = w/2 the roll direction is immaterial (+s and -s differ by a whole
+    window); for odd w it is not -- so the direction is pinned by w=3/7 cases above."""
+    r = rng(12)
+    for w, s, same in ((4, 2, True), (3, 1, False)):
+        x = r.standard_normal((1, 1, 2 * w, 2 * w))
+        T = r.standard_normal((1, (2 * w - 1) ** 2))
+        y_plus = oracle.forward(x, T, w, (s, s))
+        y_minus = oracle.forward(x, T, w, (w - s, w - s))       # -s mod w
+        assert np.allclose(y_plus, y_minus, atol=1e-13) == same
+
+
+# ----------------------------------------------------------------------------- backward
+BWD_CASES = [(2, 3, 6, 6, 3, (0, 0)), (2, 2, 7, 10, 3, (1, 2)), (1, 2, 10, 7, 4, (2, 2)), (1, 2, 14, 14, 7, (3, 3))]
+
+
+@pytest.mark.parametrize("case", BWD_CASES)
+@pytest.mark.parametrize("layout", [NCHW, NHWC])
+def test_dx_adjoint_identity(oracle, case, layout):
+    """<dy, WBMM(x2;T)> == <dX(dy;T), x2> exactly (the operator is linear in x)."""
+    B, C, H, W, w, s = case
+    r = rng(13)
+    x, x2, dy = (_to_layout(a, layout) for a in r.standard_normal((3, B, C, H, W)))
+    T = r.standard_normal((C, (2 * w - 1) ** 2))
+    dx, _ = oracle.backward(x, T, dy, w, s, layout, need_dT=False)
+    lhs = np.vdot(dy, oracle.forward(x2, T, w, s, layout))
+    rhs = np.vdot(dx, x2)
+    assert abs(lhs - rhs) <= 1e-11 * (1 + abs(lhs))
+
+
+@pytest.mark.parametrize("case", BWD_CASES)
+def test_dx_is_forward_with_reversed_table(oracle, case):
+    """W_c^T[i,j] = T[rel(j,i)] = T[nb-1-rel(i,j)]."""
+    B, C, H, W, w, s = case
+    r = rng(14)
+    x, dy = r.standard_normal((2, B, C, H, W))
+    T = r.standard_normal((C, (2 * w - 1) ** 2))
+    dx, _ = oracle.backward(x, T, dy, w, s, need_dT=False)
+    assert np.allclose(dx, oracle.forward(dy, T[:, ::-1].copy(), w, s), rtol=0, atol=1e-12)
+
+
+@pytest.mark.parametrize("case", BWD_CASES)
+@pytest.mark.parametrize("layout", [NCHW, NHWC])
+def test_dT_adjoint_identity(oracle, case, layout):
+    """<dT, T2> == <dy, WBMM(x;T2)> for any T2 (the operator is linear in T): exact."""
+    B, C, H, W, w, s = case
+    r = rng(15)
+    x, dy = (_to_layout(a, layout) for a in r.standard_normal((2, B, C, H, W)))
+    T, T2 = r.standard_normal((2, C, (2 * w - 1) ** 2))
+    _, dT = oracle.backward(x, T, dy, w, s, layout, need_dx=False)
+    lhs = np.vdot(dT, T2)
+    rhs = np.vdot(dy, oracle.forward(x, T2, w, s, layout))
+    assert abs(lhs - rhs) <= 1e-11 * (1 + abs(lhs))
+
+
+def test_dT_and_dx_finite_difference(oracle):
+    """Central finite difference of L = <dy, WBMM(x;T)> on tiny inputs in fp64 (north_star)."""
+    r = rng(16)
+    B, C, H, W, w, s = 1, 2, 5, 7, 3, (1, 1)
+    x, dy = r.standard_normal((2, B, C, H, W))
+    T = r.standard_normal((C, 25))
+    dx, dT = oracle.backward(x, T, dy, w, s)
+    L = lambda x_, T_: np.vdot(dy, oracle.forward(x_, T_, w, s))
+    eps = 1e-4
+    for (c, k) in [(0, 0), (0, 12), (1, 24), (1, 7), (0, 18)]:
+        Tp, Tm = T.copy(), T.copy()
+        Tp[c, k] += eps
+        Tm[c, k] -= eps
+        fd = (L(x, Tp) - L(x, Tm)) / (2 * eps)
+        assert abs(fd - dT[c, k]) <= 1e-8 * (1 + abs(fd))
+    for idx in [(0, 0, 0, 0), (0, 1, 4, 6), (0, 0, 2, 3), (0, 1, 3, 0)]:
+        xp_, xm_ = x.copy(), x.copy()
+        xp_[idx] += eps
+        xm_[idx] -= eps
+        fd = (L(xp_, T) - L(xm_, T)) / (2 * eps)
+        assert abs(fd - dx[idx]) <= 1e-8 * (1 + abs(fd))
+
+
+def test_dT_one_hot_pairs_land_in_one_bin(oracle):
+    """One-hot dy at output position p and one-hot x at input position q of the same window
+    => dT has a single 1 at bin rel(p,q); different windows => dT == 0."""
+    w, tw = 3, 5
+    for (p, q) in [((0, 0), (2, 2)), ((1, 2), (1, 0)), ((2, 1), (0, 1)), ((4, 4), (3, 5)), ((0, 0), (0, 3))]:
+        x = np.zeros((1, 1, 6, 6))
+        dy = np.zeros((1, 1, 6, 6))
+        x[0, 0, q[0], q[1]] = 1.0
+        dy[0, 0, p[0], p[1]] = 1.0
+        _, dT = oracle.backward(x, np.zeros((1, 25)), dy, w, need_dx=False)
+        exp = np.zeros((1, 25))
+        if p[0] // w == q[0] // w and p[1] // w == q[1] // w:
+            exp[0, (p[0] - q[0] + w - 1) * tw + (p[1] - q[1] + w - 1)] = 1.0
+        assert np.array_equal(dT, exp), (p, q)
+
+
+def test_backward_ignores_padded_region(oracle):
+    """A11: dy is zero outside HxW; padded x zeros contribute nothing to dT."""
+    r = rng(17)
+    w = 4
+    x, dy = r.standard_normal((2, 1, 2, 6, 7))
+    T = r.standard_normal((2, 49))
+    xp, dyp = np.zeros((2, 1, 2, 8, 8)), np.zeros((2, 1, 2, 8, 8))
+    xp[0][..., :6, :7] = x
+    xp[1][..., :6, :7] = dy
+    dx, dT = oracle.backward(x, T, dy, w)
+    dx2, dT2 = oracle.backward(xp[0], T, xp[1], w)
+    assert np.allclose(dT, dT2, atol=1e-13) and np.allclose(dx, dx2[..., :6, :7], atol=1e-13)
