@@ -1,0 +1,412 @@
+#!/usr/bin/env python
+"""bench.py -- WBMM forward on the headline workload (BASELINE.json config 3:
+B=128, C=96, 56x56, w=14, bf16 in / fp32 accumulate / bf16 out, NCHW), one B200 per rank.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl wbmm|reference]
+
+A "step" is one pass of the whole hot path (relative index -> W_c in shared memory -> window
+loads -> contraction -> un-partition/store) over one batch, i.e. one
+wbmm_forward call through the C ABI.  Prints ONE JSON line (rank 0).
+
+  value      TFLOP/s = algorithmic FLOPs (2*N per activation element, N=w*w=196, unpadded) of all
+             ranks / max-over-ranks device time, inputs resident in HBM.
+  e2e        the same metric through wbmm_forward_host (pinned HOST buffers; H2D + kernels + D2H
+             inside the timed region).
+  roofline   HBM-bound: algorithmic bytes (read x once + write y once + the table) / kernel time,
+             against MEASURED_PEAKS.json (else the profiling guide's fallback 6650 GB/s).
+  cpu_baseline  the CPU oracle (oracle/wbmm_ref.c, direct form, fp64, OpenMP) on a bounded sample
+             of the same workload, on this box's host cores.  A baseline, not the target.
+  train_step    config 5 (B=128, C=192, 28x28, w=14, shift 7: forward + dX + dT) ms, as context.
+
+`--impl reference` times the oracle itself (there is no reference code).
+Multi-GPU: the operator shards by batch with no exchange in the forward pass -> weak scaling,
+each rank runs the full config-3 batch on its own GPU.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import torch  # noqa: E402
+
+import synth_inputs as si  # noqa: E402
+
+METRIC = "wbmm_fwd_tflops_B128_C96_56x56_w14_bf16"
+UNIT = "TFLOP/s"
+FALLBACK_HBM_GBS = 6650.0      # /opt/skills/guides/B200_PROFILING.md fallback
+L2_BYTES = 126e6
+
+
+def flops_of(case: si.Case) -> float:
+    Hp = -(-case.H // case.w) * case.w
+    Wp = -(-case.W // case.w) * case.w
+    return 2.0 * case.w * case.w * case.B * case.C * Hp * Wp
+
+
+def bytes_of(case: si.Case) -> float:
+    es = 4 if case.dtype == "f32" else 2
+    return 2.0 * es * case.n_elem + es * case.C * case.bins
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), float(d.get("bf16_tflops", 1590.0)), "measured"
+    return FALLBACK_HBM_GBS, 1590.0, "fallback"
+
+
+def ncu_traffic_bytes():
+    """dram bytes per launch of the headline kernel from the committed ncu capture, or None."""
+    p = os.path.join(ROOT, "profiles", "headline_traffic.txt")
+    if not os.path.exists(p):
+        return None
+    for line in open(p):
+        line = line.split("#")[0].strip()
+        if line.startswith("dram_bytes_per_launch"):
+            return float(line.split("=")[1])
+    return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons, sampled while the GPU is under load."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.rows = []
+        self.proc = None
+        self.thread = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                 "--format=csv,noheader,nounits", "-lms", "50"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._read, daemon=True)
+        self.thread.start()
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0: float, t1: float):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        for ts, line in self.rows:
+            if ts < t0 or ts > t1 + 0.06:
+                continue
+            f = [s.strip() for s in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def dist_setup(n_gpus: int):
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl" if torch.cuda.is_available() else "gloo")
+    return rank, world, local
+
+
+def barrier(world):
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+
+
+def max_over_ranks(v: float, world: int, device) -> float:
+    if world == 1:
+        return v
+    import torch.distributed as dist
+    t = torch.tensor([v], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+# ------------------------------------------------------------------------------- oracle timing
+def oracle_probe(case: si.Case):
+    """Seconds per image of the oracle (direct form) on this box, measured on 2 images."""
+    from oracle import wbmm_ref
+    d = si.make(si.with_(case, B=2))
+    x2, T = d["x"].double().numpy(), d["T"].double().numpy()
+    wbmm_ref.forward(x2[:1], T, case.w, case.shift, case.layout, "direct")     # page-in, thread pool
+    t0 = time.perf_counter()
+    wbmm_ref.forward(x2, T, case.w, case.shift, case.layout, "direct")
+    return (time.perf_counter() - t0) / 2, T
+
+
+def oracle_sample(case: si.Case, target_s: float, per_image: float):
+    nb = int(max(1, min(case.B, target_s / max(per_image, 1e-6))))
+    sub = si.with_(case, B=nb)
+    return sub, si.make(sub)["x"].double().numpy(), \
+        f"first {nb} of {case.B} images, all {case.C} channels, direct form fp64"
+
+
+def time_oracle(case: si.Case, target_s: float = 12.0):
+    """The oracle as it stands (direct form, fp64, OpenMP over (b,c) planes) on a bounded sample
+    of `case`.  Returns (TFLOP/s, cores, sample, seconds)."""
+    from oracle import wbmm_ref
+    per_image, T = oracle_probe(case)
+    sub, xs, sample = oracle_sample(case, target_s, per_image)
+    t0 = time.perf_counter()
+    wbmm_ref.forward(xs, T, case.w, case.shift, case.layout, "direct")
+    dt = time.perf_counter() - t0
+    return flops_of(sub) / dt / 1e12, wbmm_ref.num_threads(), sample, dt
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the paper ships no code, so the reference arm is the CPU oracle, timed as
+    it stands on this box's host cores; each step is a bounded sample of config 3."""
+    if rank != 0:
+        return
+    from oracle import wbmm_ref
+    case = si.CFG3
+    per_image, T = oracle_probe(case)
+    per_step = max(0.05, min(15.0, 100.0 / max(1, args.steps + args.warmup)))
+    sub, xs, sample = oracle_sample(case, per_step, per_image)
+    times = []
+    for i in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        wbmm_ref.forward(xs, T, case.w, case.shift, case.layout, "direct")
+        if i >= args.warmup:
+            times.append(time.perf_counter() - t0)
+    dt = sum(times) / len(times)
+    value = flops_of(sub) / dt / 1e12
+    cores = wbmm_ref.num_threads()
+    out = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "cfg3: B=128 C=96 H=W=56 w=14 NCHW (bounded sample per step)", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(out), flush=True)
+
+
+# ------------------------------------------------------------------------------- GPU timing
+def time_steps(fn, n, stream):
+    """n calls of fn(i), each bracketed by CUDA events on `stream`; returns per-step ms list."""
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n)]
+    for i in range(n):
+        evs[i][0].record(stream)
+        fn(i)
+        evs[i][1].record(stream)
+    torch.cuda.synchronize()
+    return [a.elapsed_time(b) for a, b in evs]
+
+
+def conv_context(case: si.Case, x):
+    """Same-run torch depthwise conv (cuDNN as shipped) at k=5/7/13: context only."""
+    out = {}
+    try:
+        for k in (5, 7, 13):
+            wgt = torch.randn(case.C, 1, k, k, device=x.device, dtype=x.dtype) * 0.02
+            f = lambda: torch.nn.functional.conv2d(x, wgt, padding=k // 2, groups=case.C)
+            for _ in range(3):
+                f()
+            torch.cuda.synchronize()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            for _ in range(5):
+                f()
+            b.record()
+            torch.cuda.synchronize()
+            out[f"torch_dwconv_k{k}_ms"] = round(a.elapsed_time(b) / 5, 4)
+    except Exception as e:  # context only
+        out["error"] = str(e)[:100]
+    return out
+
+
+def run_wbmm(args, rank, world, local):
+    import paper_2607_02097_b200 as wb
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: libwbmm has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    stream = torch.cuda.current_stream()
+    case = si.CFG3
+    fl, by = flops_of(case), bytes_of(case)
+
+    # rotating buffer sets so that consecutive steps never find their inputs in L2
+    nsets = 3
+    d0 = si.make(case, device=dev)
+    xs = [d0["x"]] + [d0["x"].roll(i + 1, 0).contiguous() for i in range(nsets - 1)]
+    ys = [torch.empty_like(d0["x"]) for _ in range(nsets)]
+    T = d0["T"]
+    footprint = nsets * 2 * d0["x"].numel() * 2
+
+    def step(i):
+        wb.wbmm_forward(xs[i % nsets], T, case.w, case.shift, case.layout, out=ys[i % nsets])
+
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    warm = max(3, args.warmup)
+    for i in range(warm):
+        step(i)
+    torch.cuda.synchronize()
+    path = wb.wbmm_path_string(wb.wbmm_last_path())
+    # keep the GPU under load long enough for nvidia-smi to sample clocks under this kernel
+    t_load0 = time.time()
+    i = 0
+    while time.time() - t_load0 < 0.6:
+        for _ in range(50):
+            step(i); i += 1
+        torch.cuda.synchronize()
+
+    barrier(world)
+    torch.cuda.synchronize()
+    n0 = wb.wbmm_launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for i in range(args.steps):
+        step(i)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    barrier(world)
+    t_load1 = time.time()
+    launches = wb.wbmm_launch_count() - n0
+    ms_total = max_over_ranks(e0.elapsed_time(e1), world, dev)
+    ms_step = ms_total / args.steps
+    clocks = sampler.stop(t_load0, t_load1) if rank == 0 else None
+
+    # per-launch statistics (same kernel, each launch bracketed by events on its stream)
+    per = time_steps(step, max(args.steps, 20), stream)
+    ms_med, ms_min = statistics.median(per), min(per)
+    # hot-L2 number for contrast: same buffers every step
+    hot = time_steps(lambda i: wb.wbmm_forward(xs[0], T, case.w, out=ys[0]), 20, stream)
+
+    value = world * fl / (ms_step * 1e-3) / 1e12
+
+    # end to end through the C ABI with pinned host buffers
+    e2e = None
+    if True:
+        h = si.make(case, pin=True)
+        yh = torch.empty_like(h["x"]).pin_memory()
+        for _ in range(2):
+            wb.wbmm_forward_host(h["x"], h["T"], case.w, out=yh)
+        barrier(world)
+        n_e2e = max(3, min(args.steps, 10))
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            wb.wbmm_forward_host(h["x"], h["T"], case.w, out=yh)
+        dt = (time.perf_counter() - t0) / n_e2e
+        dt = max_over_ranks(dt, world, dev)
+        e2e = {"value": world * fl / dt / 1e12, "unit": UNIT, "ms_per_step": dt * 1e3,
+               "h2d_bytes_per_step": h["x"].numel() * 2 + h["T"].numel() * 2,
+               "d2h_bytes_per_step": yh.numel() * 2, "steps": n_e2e,
+               "api": "wbmm_forward_host (pinned host buffers)"}
+
+    if rank != 0:
+        return
+
+    hbm_peak, tc_peak, peak_kind = measured_peaks()
+    achieved = by / (ms_med * 1e-3) / 1e9
+    t_roof = max(fl / (tc_peak * 1e12), by / (hbm_peak * 1e9))
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s",
+                "frac": achieved / hbm_peak, "traffic": ncu_traffic_bytes(),
+                "peak_kind": f"{peak_kind} (MEASURED_PEAKS.json hbm_gbs)" if peak_kind == "measured" else "fallback (B200_PROFILING.md)",
+                "kernel": path, "kernel_ms_median": ms_med, "kernel_ms_min": ms_min,
+                "algorithmic_bytes_per_launch": by, "algorithmic_flops_per_launch": fl,
+                "t_roof_ms": t_roof * 1e3, "frac_of_roofline_time": t_roof * 1e3 / ms_med,
+                "tensor_tflops_at_median": fl / (ms_med * 1e-3) / 1e12,
+                "hot_l2_ms_median": statistics.median(hot)}
+
+    # training step (config 5) as context: forward + dX + dT
+    c5 = si.CFG5
+    d5 = si.make(c5, device=dev)
+    y5 = torch.empty_like(d5["x"])
+
+    def train(i):
+        wb.wbmm_forward(d5["x"], d5["T"], c5.w, c5.shift, out=y5)
+        wb.wbmm_backward(d5["x"], d5["T"], d5["dy"], c5.w, c5.shift)
+
+    for i in range(3):
+        train(i)
+    t5 = time_steps(train, 10, stream)
+    train_path = wb.wbmm_path_string(wb.wbmm_last_path())
+    by5 = 2 * c5.n_elem * 2 * 2 + 2 * c5.n_elem * 2 + c5.C * c5.bins * 4   # x,y; dy,dx; x,dy; dT
+    train_step = {"workload": "cfg5 B128 C192 28x28 w14 shift7 fwd+dX+dT", "ms_median": statistics.median(t5),
+                  "ms_min": min(t5), "last_path": train_path, "flops": 3 * flops_of(c5),
+                  "hbm_frac_at_median": by5 / (statistics.median(t5) * 1e-3) / 1e9 / hbm_peak,
+                  "note": "working set fits L2 (232 MB algorithmic traffic, 126 MB L2): hot-ish number"}
+
+    tfl_cpu, cores, sample, dt_cpu = time_oracle(case)
+    cpu = {"value": tfl_cpu, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+           "seconds": dt_cpu}
+
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": warm, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+        "config": {"workload": "cfg3: B=128 C=96 H=W=56 w=14 NCHW bf16 in/fp32 acc/bf16 out (BASELINE.json configs[2], the headline)",
+                   "per_gpu_batch": case.B, "path": path,
+                   "l2": f"rotating {nsets} buffer sets, footprint {footprint / 1e6:.0f} MB > 2x L2 (cold-L2 numbers)"},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
+        "roofline": roofline, "cpu_baseline": cpu, "train_step": train_step,
+        "context": conv_context(case, d0["x"]),
+    }
+    print(json.dumps(out), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="wbmm", choices=["wbmm", "reference"])
+    args = ap.parse_args()
+    if args.impl == "reference":
+        rank = int(os.environ.get("RANK", "0"))
+        run_reference(args, rank, int(os.environ.get("WORLD_SIZE", "1")))
+        return
+    rank, world, local = dist_setup(args.gpus)
+    try:
+        run_wbmm(args, rank, world, local)
+    finally:
+        if world > 1:
+            import torch.distributed as dist
+            dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,140 @@
+/*
+ * wbmm.h -- C ABI of libwbmm.so: the WBMM operator (Windowed Batch Matrix Multiplication,
+ * arxiv/paper_2607_02097) as hand-written CUDA kernels for NVIDIA B200 (sm_100a).
+ *
+ * Citations are to the paper text and to DESIGN.md ("Readings").
+ *
+ * The operator (Algorithm 1, Eq. 4-8; orientation per DESIGN.md reading A1):
+ *   the activation x[B,C,H,W] is zero-padded (bottom/right) to multiples of w, cut into
+ *   non-overlapping w x w windows of N = w*w positions (row-major inside a window), and every
+ *   window of channel c is multiplied by that channel's N x N matrix
+ *       W_c[i,j] = T[c, rel(i,j)],   rel(i,j) = (r_i - r_j + w-1)*(2w-1) + (c_i - c_j + w-1)
+ *   (Eq. 6-8), i = output position, j = input position:  y_win = W_c * x_win.  W_c is never
+ *   written to HBM.  The padding is cropped from the output (Eq. 4-5).
+ *   Optional cyclic shift (reading A6):  x^[h,v] = x~[(h+s_h) mod H', (v+s_w) mod W']
+ *   on the padded extent before partitioning, inverse roll on the output.
+ *   Backward (autograd of Alg. 1):  dX_win = W_c^T * dY_win,
+ *       dT[c,k] = sum over images, windows and pairs (i,j) with rel(i,j)=k of dY_win[i]*X_win[j].
+ *
+ * Conventions for every entry point
+ *   - Pointers named x, T, y, dy, dx, dT, Wout are DEVICE pointers unless the function name ends
+ *     in _host.  Tensors are dense and contiguous.  The caller owns all buffers and the stream.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *     Calls are asynchronous on that stream; the library never synchronises (the _host variants
+ *     do: they return after the result is in host memory).
+ *   - Return value: a wbmm_status_t.  Nothing throws or aborts across the ABI.  On a non-zero
+ *     status no output buffer has been written.
+ *   - There is no CPU fallback.  Without a CUDA device of compute capability 10.x every compute
+ *     entry point returns WBMM_STATUS_NO_DEVICE.
+ */
+#ifndef WBMM_H_
+#define WBMM_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define WBMM_VERSION 100 /* major*10000 + minor*100 + patch */
+
+#if defined(__GNUC__)
+#define WBMM_API __attribute__((visibility("default")))
+#else
+#define WBMM_API
+#endif
+
+typedef enum {
+    WBMM_STATUS_OK = 0,
+    WBMM_STATUS_INVALID_ARGUMENT = 1, /* null pointer, non-positive size, shift not in [0,w), bad enum, y aliases x */
+    WBMM_STATUS_UNSUPPORTED = 2,      /* window too large for shared memory, or dtype/path combination not built */
+    WBMM_STATUS_NO_DEVICE = 3,        /* no CUDA device, or the device is not sm_100 */
+    WBMM_STATUS_CUDA_ERROR = 4,       /* a CUDA runtime/driver call failed; see wbmm_last_error_string() */
+    WBMM_STATUS_MISALIGNED = 5        /* a pointer is not aligned to its element size */
+} wbmm_status_t;
+
+typedef enum { WBMM_DTYPE_F32 = 0, WBMM_DTYPE_BF16 = 1, WBMM_DTYPE_F16 = 2 } wbmm_dtype_t;
+typedef enum { WBMM_LAYOUT_NCHW = 0, WBMM_LAYOUT_NHWC = 1 } wbmm_layout_t;
+
+/* Which kernel family served the last call on this host thread (wbmm_last_path()). */
+typedef enum {
+    WBMM_PATH_NONE = 0,
+    WBMM_PATH_SIMT = 1,      /* general fp32-FFMA kernels: any w, dtype, layout, shift, ragged size */
+    WBMM_PATH_TC_TMA = 2,    /* tcgen05/TMEM tensor-core kernels fed by TMA window loads (bf16/fp16) */
+    WBMM_PATH_TC_GATHER = 3  /* tcgen05/TMEM kernels fed by a predicated gather loader (bf16/fp16) */
+} wbmm_path_t;
+
+enum {
+    WBMM_FLAG_ACCUMULATE_DT = 1u, /* wbmm_backward: add into dT instead of overwriting it */
+    WBMM_FLAG_FORCE_SIMT = 2u     /* never take a tensor-core path (testing / cross-checks) */
+};
+
+/* Problem descriptor (plain data, passed by pointer, read during the call only). */
+typedef struct wbmm_desc {
+    int32_t B, C, H, W;       /* logical activation sizes; H, W need not be multiples of w */
+    int32_t w;                /* square window side, w >= 1; N = w*w; the table has (2w-1)^2 bins per channel */
+    int32_t shift_h, shift_w; /* cyclic shift in [0, w); 0 = none */
+    int32_t dtype;            /* wbmm_dtype_t of x, y, dy, dx AND of T.  dT is always float32. */
+    int32_t layout;           /* wbmm_layout_t of x, y, dy, dx.  T and dT are [C][(2w-1)^2] row-major. */
+    uint32_t flags;           /* WBMM_FLAG_* */
+} wbmm_desc_t;
+
+/*
+ * Forward, Algorithm 1:  y = WBMM(x; T, w).
+ *   x  [in]  B*C*H*W elements of desc->dtype in desc->layout.            Read-only.
+ *   T  [in]  C*(2w-1)^2 elements of desc->dtype.                         Read-only.
+ *   y  [out] same shape/dtype/layout as x; every element is overwritten, nothing outside it.
+ *            Accumulation is fp32; the result is rounded to desc->dtype (RNE).  y must not alias x.
+ * bf16/fp16 tensor-core paths multiply some padding lanes by exact zero weights: inputs are
+ * assumed finite (a non-finite x may turn neighbouring outputs of the same row strip into NaN).
+ */
+WBMM_API int wbmm_forward(const wbmm_desc_t *desc, const void *x, const void *T, void *y, void *cuda_stream);
+
+/*
+ * Backward of wbmm_forward:
+ *   dx [out, nullable] dX = W_c^T * dY per window, shape/dtype/layout of x, fully overwritten.
+ *   dT [out, nullable] float32 [C][(2w-1)^2]; overwritten (zeroed on the stream first) unless
+ *                      WBMM_FLAG_ACCUMULATE_DT.  Summation order over windows is not fixed
+ *                      (atomics): results are reproducible to rounding, not bitwise.
+ *   x, T, dy [in] as in wbmm_forward; dy is treated as zero outside H x W (A11).
+ *   x may be NULL when dT is NULL; T may be NULL when dx is NULL.
+ */
+WBMM_API int wbmm_backward(const wbmm_desc_t *desc, const void *x, const void *T, const void *dy,
+                  void *dx, float *dT, void *cuda_stream);
+
+/*
+ * Eq. 6-8 on their own (test/debug and the WBMM-C "cached M" mode):
+ *   Wout [out] [C][N][N] elements of desc->dtype, Wout[c,i,j] = T[c, rel(i,j)] copied bit-exactly.
+ * Only C, w and dtype of the descriptor are used.
+ */
+WBMM_API int wbmm_materialize_weight(const wbmm_desc_t *desc, const void *T, void *Wout, void *cuda_stream);
+
+/*
+ * End-to-end variants with HOST buffers (pageable or pinned).  Each call copies its inputs to
+ * device scratch owned by the library (grown on demand, reused between calls, freed by
+ * wbmm_release()), runs the same kernels as the device entry points on an internal stream,
+ * copies the results back and returns when they are in host memory.
+ */
+WBMM_API int wbmm_forward_host(const wbmm_desc_t *desc, const void *x_host, const void *T_host, void *y_host);
+WBMM_API int wbmm_backward_host(const wbmm_desc_t *desc, const void *x_host, const void *T_host,
+                       const void *dy_host, void *dx_host /*nullable*/, float *dT_host /*nullable*/);
+
+/* Frees the scratch and cached state held by the library (host-variant buffers, tensor maps). */
+WBMM_API void wbmm_release(void);
+
+/* wbmm_path_t of the most recent compute call made by the calling host thread. */
+WBMM_API int wbmm_last_path(void);
+/* Number of kernels this library has launched since it was loaded (all threads). */
+WBMM_API uint64_t wbmm_launch_count(void);
+/* Static strings; never NULL. */
+WBMM_API const char *wbmm_status_string(int status);
+WBMM_API const char *wbmm_path_string(int path);
+/* Text of the last CUDA error seen by the calling host thread ("" if none). */
+WBMM_API const char *wbmm_last_error_string(void);
+WBMM_API int wbmm_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* WBMM_H_ */

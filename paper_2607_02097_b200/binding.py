@@ -1,0 +1,208 @@
+"""Thin ctypes binding over libwbmm.so (include/wbmm.h).  Argument marshalling only: every step
+of the WBMM path runs in the CUDA kernels behind the C ABI.  torch is used for device memory and
+the current stream.  There is no CPU fallback: a missing library or device raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Tuple
+
+import torch
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libwbmm.so")
+
+NCHW, NHWC = 0, 1
+DTYPE_F32, DTYPE_BF16, DTYPE_F16 = 0, 1, 2
+PATH_NONE, PATH_SIMT, PATH_TC_TMA, PATH_TC_GATHER = 0, 1, 2, 3
+FLAG_ACCUMULATE_DT, FLAG_FORCE_SIMT = 1, 2
+STATUS_OK = 0
+
+_DTYPES = {torch.float32: DTYPE_F32, torch.bfloat16: DTYPE_BF16, torch.float16: DTYPE_F16}
+
+# every symbol include/wbmm.h declares
+EXPORTS = (
+    "wbmm_forward", "wbmm_backward", "wbmm_materialize_weight", "wbmm_forward_host",
+    "wbmm_backward_host", "wbmm_release", "wbmm_last_path", "wbmm_launch_count",
+    "wbmm_status_string", "wbmm_path_string", "wbmm_last_error_string", "wbmm_version",
+)
+
+
+class WbmmDesc(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_int32) for n in
+                ("B", "C", "H", "W", "w", "shift_h", "shift_w", "dtype", "layout")] + [("flags", ctypes.c_uint32)]
+
+
+class WbmmError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(msg)
+        self.status = status
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """Loads libwbmm.so (built in-tree by paper_2607_02097_b200.build).  Raises if it is absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_2607_02097_b200.build` "
+                          "(there is no CPU fallback)")
+    L = ctypes.CDLL(LIB_PATH)
+    vp, dp, i = ctypes.c_void_p, ctypes.POINTER(WbmmDesc), ctypes.c_int
+    L.wbmm_forward.argtypes = [dp, vp, vp, vp, vp]
+    L.wbmm_backward.argtypes = [dp, vp, vp, vp, vp, vp, vp]
+    L.wbmm_materialize_weight.argtypes = [dp, vp, vp, vp]
+    L.wbmm_forward_host.argtypes = [dp, vp, vp, vp]
+    L.wbmm_backward_host.argtypes = [dp, vp, vp, vp, vp, vp]
+    for n in ("wbmm_forward", "wbmm_backward", "wbmm_materialize_weight", "wbmm_forward_host",
+              "wbmm_backward_host", "wbmm_last_path", "wbmm_version"):
+        getattr(L, n).restype = i
+    L.wbmm_release.restype = None
+    L.wbmm_launch_count.restype = ctypes.c_uint64
+    for n in ("wbmm_status_string", "wbmm_path_string", "wbmm_last_error_string"):
+        getattr(L, n).restype = ctypes.c_char_p
+    L.wbmm_status_string.argtypes = [i]
+    L.wbmm_path_string.argtypes = [i]
+    _lib = L
+    return L
+
+
+def _check(st: int) -> None:
+    if st != STATUS_OK:
+        L = lib()
+        msg = L.wbmm_status_string(st).decode()
+        err = L.wbmm_last_error_string().decode()
+        raise WbmmError(st, f"libwbmm: {msg}" + (f" ({err})" if st == 4 and err else ""))
+
+
+def _dims(t: torch.Tensor, layout: int):
+    if t.dim() != 4:
+        raise ValueError("activation must be 4-D")
+    if layout == NCHW:
+        B, C, H, W = t.shape
+    else:
+        B, H, W, C = t.shape
+    return B, C, H, W
+
+
+def make_desc(x: torch.Tensor, w: int, shift=(0, 0), layout: int = NCHW, flags: int = 0) -> WbmmDesc:
+    B, C, H, W = _dims(x, layout)
+    if x.dtype not in _DTYPES:
+        raise TypeError(f"unsupported dtype {x.dtype}")
+    return WbmmDesc(B, C, H, W, int(w), int(shift[0]), int(shift[1]), _DTYPES[x.dtype], int(layout), int(flags))
+
+
+def _stream(t: torch.Tensor) -> int:
+    return torch.cuda.current_stream(t.device).cuda_stream
+
+
+def _dev(t: Optional[torch.Tensor], name: str) -> Optional[int]:
+    if t is None:
+        return None
+    if not t.is_cuda:
+        raise ValueError(f"{name} must be a CUDA tensor (no CPU fallback)")
+    if not t.is_contiguous():
+        raise ValueError(f"{name} must be contiguous")
+    return t.data_ptr()
+
+
+def wbmm_forward(x: torch.Tensor, T: torch.Tensor, w: int, shift=(0, 0), layout: int = NCHW,
+                 flags: int = 0, out: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """y = WBMM(x; T, w) on the current CUDA stream (include/wbmm.h: wbmm_forward)."""
+    d = make_desc(x, w, shift, layout, flags)
+    if T.dtype != x.dtype or tuple(T.shape) != (d.C, (2 * w - 1) ** 2):
+        raise ValueError("T must be [C,(2w-1)^2] in the dtype of x")
+    y = torch.empty_like(x) if out is None else out
+    with torch.cuda.device(x.device):
+        _check(lib().wbmm_forward(ctypes.byref(d), _dev(x, "x"), _dev(T, "T"), _dev(y, "y"), _stream(x)))
+    return y
+
+
+def wbmm_backward(x: Optional[torch.Tensor], T: Optional[torch.Tensor], dy: torch.Tensor, w: int,
+                  shift=(0, 0), layout: int = NCHW, flags: int = 0, need_dx: bool = True,
+                  need_dT: bool = True, dT: Optional[torch.Tensor] = None
+                  ) -> Tuple[Optional[torch.Tensor], Optional[torch.Tensor]]:
+    """(dx, dT) of wbmm_forward; dT is float32 [C,(2w-1)^2] (include/wbmm.h: wbmm_backward)."""
+    d = make_desc(dy, w, shift, layout, flags)
+    dx = torch.empty_like(dy) if need_dx else None
+    if need_dT and dT is None:
+        dT = torch.empty((d.C, (2 * w - 1) ** 2), dtype=torch.float32, device=dy.device)
+    if not need_dT:
+        dT = None
+    with torch.cuda.device(dy.device):
+        _check(lib().wbmm_backward(ctypes.byref(d), _dev(x, "x") if need_dT else None,
+                                   _dev(T, "T") if need_dx else None, _dev(dy, "dy"),
+                                   _dev(dx, "dx"), _dev(dT, "dT"), _stream(dy)))
+    return dx, dT
+
+
+def wbmm_materialize_weight(T: torch.Tensor, w: int) -> torch.Tensor:
+    """Eq. 8: W[c,i,j] = T[c, rel(i,j)] as a [C,N,N] tensor (bit-exact copy of table entries)."""
+    C = T.shape[0]
+    d = WbmmDesc(0, C, 1, 1, int(w), 0, 0, _DTYPES[T.dtype], NCHW, 0)
+    W = torch.empty((C, w * w, w * w), dtype=T.dtype, device=T.device)
+    with torch.cuda.device(T.device):
+        _check(lib().wbmm_materialize_weight(ctypes.byref(d), _dev(T, "T"), _dev(W, "W"), _stream(T)))
+    return W
+
+
+def _host(t: Optional[torch.Tensor], name: str) -> Optional[int]:
+    if t is None:
+        return None
+    if t.is_cuda or not t.is_contiguous():
+        raise ValueError(f"{name} must be a contiguous host tensor")
+    return t.data_ptr()
+
+
+def wbmm_forward_host(x: torch.Tensor, T: torch.Tensor, w: int, shift=(0, 0), layout: int = NCHW,
+                      flags: int = 0, out: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """Host-buffer forward: H2D copies, kernels and the D2H copy all happen inside the C call."""
+    d = make_desc(x, w, shift, layout, flags)
+    y = torch.empty_like(x) if out is None else out
+    _check(lib().wbmm_forward_host(ctypes.byref(d), _host(x, "x"), _host(T, "T"), _host(y, "y")))
+    return y
+
+
+def wbmm_backward_host(x, T, dy, w, shift=(0, 0), layout: int = NCHW, flags: int = 0,
+                       need_dx: bool = True, need_dT: bool = True, dx=None, dT=None):
+    d = make_desc(dy, w, shift, layout, flags)
+    if need_dx and dx is None:
+        dx = torch.empty_like(dy)
+    if need_dT and dT is None:
+        dT = torch.empty((d.C, (2 * w - 1) ** 2), dtype=torch.float32)
+    _check(lib().wbmm_backward_host(ctypes.byref(d), _host(x, "x") if need_dT else None,
+                                    _host(T, "T") if need_dx else None, _host(dy, "dy"),
+                                    _host(dx, "dx") if need_dx else None, _host(dT, "dT") if need_dT else None))
+    return (dx if need_dx else None), (dT if need_dT else None)
+
+
+def wbmm_release() -> None:
+    lib().wbmm_release()
+
+
+def wbmm_last_path() -> int:
+    return int(lib().wbmm_last_path())
+
+
+def wbmm_path_string(path: int) -> str:
+    return lib().wbmm_path_string(int(path)).decode()
+
+
+def wbmm_status_string(status: int) -> str:
+    return lib().wbmm_status_string(int(status)).decode()
+
+
+def wbmm_last_error_string() -> str:
+    return lib().wbmm_last_error_string().decode()
+
+
+def wbmm_launch_count() -> int:
+    return int(lib().wbmm_launch_count())
+
+
+def wbmm_version() -> int:
+    return int(lib().wbmm_version())

@@ -1,0 +1,322 @@
+// C ABI of libwbmm.so (include/wbmm.h): argument validation, path selection, host-buffer variants.
+// No compute happens here and nothing here can fall back to a CPU implementation.
+#include <atomic>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+
+#include "wbmm_common.cuh"
+#include "wbmm_tc.cuh"
+
+namespace {
+
+thread_local int t_last_path = WBMM_PATH_NONE;
+thread_local char t_last_error[256] = "";
+std::atomic<uint64_t> g_launches{0};
+
+int set_cuda_error(cudaError_t e, const char* where)
+{
+    snprintf(t_last_error, sizeof(t_last_error), "%s: %s", where, cudaGetErrorString(e));
+    return WBMM_STATUS_CUDA_ERROR;
+}
+
+size_t elem_size(int dtype) { return dtype == WBMM_DTYPE_F32 ? 4 : 2; }
+
+// 0 = not probed, 1 = sm_100 present, -1 = absent
+int device_state()
+{
+    static std::atomic<int> state{0};
+    int s = state.load();
+    if (s != 0) return s;
+    int dev = 0, major = 0, count = 0;
+    if (cudaGetDeviceCount(&count) != cudaSuccess || count == 0) {
+        cudaGetLastError();
+        state.store(-1);
+        return -1;
+    }
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) {
+        cudaGetLastError();
+        state.store(-1);
+        return -1;
+    }
+    s = major == 10 ? 1 : -1;
+    state.store(s);
+    return s;
+}
+
+int validate(const wbmm_desc_t* d)
+{
+    if (!d) return WBMM_STATUS_INVALID_ARGUMENT;
+    if (d->B < 0 || d->C < 0 || d->H < 1 || d->W < 1 || d->w < 1) return WBMM_STATUS_INVALID_ARGUMENT;
+    if (d->shift_h < 0 || d->shift_w < 0 || d->shift_h >= d->w || d->shift_w >= d->w)
+        return WBMM_STATUS_INVALID_ARGUMENT;
+    if (d->dtype != WBMM_DTYPE_F32 && d->dtype != WBMM_DTYPE_BF16 && d->dtype != WBMM_DTYPE_F16)
+        return WBMM_STATUS_INVALID_ARGUMENT;
+    if (d->layout != WBMM_LAYOUT_NCHW && d->layout != WBMM_LAYOUT_NHWC) return WBMM_STATUS_INVALID_ARGUMENT;
+    if (d->w > 1024) return WBMM_STATUS_UNSUPPORTED;
+    // index arithmetic is 64-bit for elements, 32-bit for per-axis sizes
+    long long n = (long long)d->B * d->C;
+    if (n > (1ll << 40) / ((long long)d->H * d->W)) return WBMM_STATUS_UNSUPPORTED;
+    return WBMM_STATUS_OK;
+}
+
+bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
+
+// One operator application y = op(x; T) with op = W_c (reverse=false) or W_c^T (reverse=true).
+int apply(const wbmm_desc_t* d, const wbmm::Geom& g, const void* x, const void* T, void* y,
+          bool reverse, cudaStream_t stream)
+{
+    int launches = 0;
+    cudaError_t e;
+    if (!(d->flags & WBMM_FLAG_FORCE_SIMT) && wbmm::tc_forward_supported(g, d->dtype, x, y)) {
+        int path = WBMM_PATH_NONE;
+        e = wbmm::tc_forward(g, d->dtype, x, T, y, reverse, stream, &launches, &path);
+        g_launches += launches;
+        if (e != cudaSuccess) return set_cuda_error(e, "tc_forward");
+        t_last_path = path;
+        return WBMM_STATUS_OK;
+    }
+    if (!wbmm::simt_supported(g)) return WBMM_STATUS_UNSUPPORTED;
+    e = wbmm::simt_forward(g, d->dtype, x, T, y, reverse, stream, &launches);
+    g_launches += launches;
+    if (e != cudaSuccess) return set_cuda_error(e, "simt_forward");
+    t_last_path = WBMM_PATH_SIMT;
+    return WBMM_STATUS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int wbmm_forward(const wbmm_desc_t* desc, const void* x, const void* T, void* y, void* cuda_stream)
+{
+    int st = validate(desc);
+    if (st != WBMM_STATUS_OK) return st;
+    if (desc->B == 0 || desc->C == 0) return WBMM_STATUS_OK;   // empty problem: nothing to read or write
+    if (!x || !T || !y || x == y) return WBMM_STATUS_INVALID_ARGUMENT;
+    const size_t es = elem_size(desc->dtype);
+    if (!aligned(x, es) || !aligned(T, es) || !aligned(y, es)) return WBMM_STATUS_MISALIGNED;
+    if (device_state() < 0) return WBMM_STATUS_NO_DEVICE;
+    wbmm::Geom g = wbmm::make_geom(*desc);
+    return apply(desc, g, x, T, y, false, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int wbmm_backward(const wbmm_desc_t* desc, const void* x, const void* T, const void* dy,
+                  void* dx, float* dT, void* cuda_stream)
+{
+    int st = validate(desc);
+    if (st != WBMM_STATUS_OK) return st;
+    if (desc->C == 0) return WBMM_STATUS_OK;
+    if (desc->B == 0) {   // no windows: dT is all zero, dx is empty
+        if (dT && !(desc->flags & WBMM_FLAG_ACCUMULATE_DT)) {
+            if (device_state() < 0) return WBMM_STATUS_NO_DEVICE;
+            size_t n = sizeof(float) * (size_t)desc->C * (2 * desc->w - 1) * (2 * desc->w - 1);
+            cudaError_t e = cudaMemsetAsync(dT, 0, n, static_cast<cudaStream_t>(cuda_stream));
+            if (e != cudaSuccess) return set_cuda_error(e, "memset dT");
+        }
+        return WBMM_STATUS_OK;
+    }
+    if (!dy || (dx && !T) || (dT && !x) || (dx && dx == dy)) return WBMM_STATUS_INVALID_ARGUMENT;
+    const size_t es = elem_size(desc->dtype);
+    if (!aligned(dy, es) || (x && !aligned(x, es)) || (T && !aligned(T, es)) || (dx && !aligned(dx, es)) ||
+        (dT && !aligned(dT, 4)))
+        return WBMM_STATUS_MISALIGNED;
+    if (device_state() < 0) return WBMM_STATUS_NO_DEVICE;
+    wbmm::Geom g = wbmm::make_geom(*desc);
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    if (dx) {
+        // dX = W_c^T dY: the forward operator with the table index reversed (k -> nb-1-k)
+        st = apply(desc, g, dy, T, dx, true, stream);
+        if (st != WBMM_STATUS_OK) return st;
+    }
+    if (dT) {
+        if (!(desc->flags & WBMM_FLAG_ACCUMULATE_DT) && g.C > 0) {
+            cudaError_t e = cudaMemsetAsync(dT, 0, sizeof(float) * (size_t)g.C * g.nb, stream);
+            if (e != cudaSuccess) return set_cuda_error(e, "memset dT");
+        }
+        int launches = 0;
+        cudaError_t e;
+        if (!(desc->flags & WBMM_FLAG_FORCE_SIMT) && wbmm::tc_grad_table_supported(g, desc->dtype, x, dy)) {
+            int path = WBMM_PATH_NONE;
+            e = wbmm::tc_grad_table(g, desc->dtype, x, dy, dT, stream, &launches, &path);
+            g_launches += launches;
+            if (e != cudaSuccess) return set_cuda_error(e, "tc_grad_table");
+            t_last_path = path;
+        } else {
+            if (!wbmm::simt_supported(g)) return WBMM_STATUS_UNSUPPORTED;
+            e = wbmm::simt_grad_table(g, desc->dtype, x, dy, dT, stream, &launches);
+            g_launches += launches;
+            if (e != cudaSuccess) return set_cuda_error(e, "simt_grad_table");
+            t_last_path = WBMM_PATH_SIMT;
+        }
+    }
+    return WBMM_STATUS_OK;
+}
+
+int wbmm_materialize_weight(const wbmm_desc_t* desc, const void* T, void* Wout, void* cuda_stream)
+{
+    if (!desc || desc->C < 0 || desc->w < 1 || desc->w > 64) return WBMM_STATUS_INVALID_ARGUMENT;
+    if (desc->dtype != WBMM_DTYPE_F32 && desc->dtype != WBMM_DTYPE_BF16 && desc->dtype != WBMM_DTYPE_F16)
+        return WBMM_STATUS_INVALID_ARGUMENT;
+    if (!T || !Wout) return WBMM_STATUS_INVALID_ARGUMENT;
+    if (!aligned(T, elem_size(desc->dtype)) || !aligned(Wout, elem_size(desc->dtype))) return WBMM_STATUS_MISALIGNED;
+    if (device_state() < 0) return WBMM_STATUS_NO_DEVICE;
+    int launches = 0;
+    cudaError_t e = wbmm::simt_materialize(desc->C, desc->w, desc->dtype, T, Wout,
+                                           static_cast<cudaStream_t>(cuda_stream), &launches);
+    g_launches += launches;
+    if (e != cudaSuccess) return set_cuda_error(e, "materialize");
+    t_last_path = WBMM_PATH_SIMT;
+    return WBMM_STATUS_OK;
+}
+
+}  // extern "C"
+
+// ---------------------------------------------------------------------------------------------
+// Host-buffer variants: device scratch owned by the library, one internal stream.
+namespace {
+
+struct Scratch {
+    void* p = nullptr;
+    size_t cap = 0;
+    cudaError_t reserve(size_t n)
+    {
+        if (n <= cap) return cudaSuccess;
+        if (p) cudaFree(p);
+        p = nullptr; cap = 0;
+        cudaError_t e = cudaMalloc(&p, n);
+        if (e == cudaSuccess) cap = n;
+        return e;
+    }
+    void release() { if (p) cudaFree(p); p = nullptr; cap = 0; }
+};
+
+std::mutex g_host_mutex;
+Scratch g_sx, g_sT, g_sy, g_sdy, g_sdT;
+cudaStream_t g_host_stream = nullptr;
+
+cudaError_t host_stream(cudaStream_t* s)
+{
+    if (!g_host_stream) {
+        cudaError_t e = cudaStreamCreateWithFlags(&g_host_stream, cudaStreamNonBlocking);
+        if (e != cudaSuccess) return e;
+    }
+    *s = g_host_stream;
+    return cudaSuccess;
+}
+
+#define WBMM_TRY(expr, where)                                   \
+    do {                                                        \
+        cudaError_t e_ = (expr);                                \
+        if (e_ != cudaSuccess) return set_cuda_error(e_, where); \
+    } while (0)
+
+}  // namespace
+
+extern "C" {
+
+int wbmm_forward_host(const wbmm_desc_t* desc, const void* x_host, const void* T_host, void* y_host)
+{
+    int st = validate(desc);
+    if (st != WBMM_STATUS_OK) return st;
+    if (!x_host || !T_host || !y_host) return WBMM_STATUS_INVALID_ARGUMENT;
+    if (device_state() < 0) return WBMM_STATUS_NO_DEVICE;
+    std::lock_guard<std::mutex> lock(g_host_mutex);
+    wbmm::Geom g = wbmm::make_geom(*desc);
+    const size_t es = elem_size(desc->dtype);
+    const size_t nact = (size_t)g.B * g.C * g.H * g.W * es, ntab = (size_t)g.C * g.nb * es;
+    cudaStream_t s;
+    WBMM_TRY(host_stream(&s), "stream");
+    if (nact == 0) return WBMM_STATUS_OK;
+    WBMM_TRY(g_sx.reserve(nact), "cudaMalloc x");
+    WBMM_TRY(g_sy.reserve(nact), "cudaMalloc y");
+    WBMM_TRY(g_sT.reserve(ntab), "cudaMalloc T");
+    WBMM_TRY(cudaMemcpyAsync(g_sx.p, x_host, nact, cudaMemcpyHostToDevice, s), "H2D x");
+    WBMM_TRY(cudaMemcpyAsync(g_sT.p, T_host, ntab, cudaMemcpyHostToDevice, s), "H2D T");
+    st = apply(desc, g, g_sx.p, g_sT.p, g_sy.p, false, s);
+    if (st != WBMM_STATUS_OK) return st;
+    WBMM_TRY(cudaMemcpyAsync(y_host, g_sy.p, nact, cudaMemcpyDeviceToHost, s), "D2H y");
+    WBMM_TRY(cudaStreamSynchronize(s), "sync");
+    return WBMM_STATUS_OK;
+}
+
+int wbmm_backward_host(const wbmm_desc_t* desc, const void* x_host, const void* T_host,
+                       const void* dy_host, void* dx_host, float* dT_host)
+{
+    int st = validate(desc);
+    if (st != WBMM_STATUS_OK) return st;
+    if (!dy_host || (dx_host && !T_host) || (dT_host && !x_host)) return WBMM_STATUS_INVALID_ARGUMENT;
+    if (device_state() < 0) return WBMM_STATUS_NO_DEVICE;
+    std::lock_guard<std::mutex> lock(g_host_mutex);
+    wbmm::Geom g = wbmm::make_geom(*desc);
+    const size_t es = elem_size(desc->dtype);
+    const size_t nact = (size_t)g.B * g.C * g.H * g.W * es, ntab = (size_t)g.C * g.nb * es;
+    const size_t ngrad = (size_t)g.C * g.nb * sizeof(float);
+    cudaStream_t s;
+    WBMM_TRY(host_stream(&s), "stream");
+    if (nact == 0 || (!dx_host && !dT_host)) {
+        if (dT_host && !(desc->flags & WBMM_FLAG_ACCUMULATE_DT)) memset(dT_host, 0, ngrad);
+        return WBMM_STATUS_OK;
+    }
+    WBMM_TRY(g_sdy.reserve(nact), "cudaMalloc dy");
+    WBMM_TRY(cudaMemcpyAsync(g_sdy.p, dy_host, nact, cudaMemcpyHostToDevice, s), "H2D dy");
+    if (dT_host) {
+        WBMM_TRY(g_sx.reserve(nact), "cudaMalloc x");
+        WBMM_TRY(g_sdT.reserve(ngrad), "cudaMalloc dT");
+        WBMM_TRY(cudaMemcpyAsync(g_sx.p, x_host, nact, cudaMemcpyHostToDevice, s), "H2D x");
+        if (desc->flags & WBMM_FLAG_ACCUMULATE_DT)
+            WBMM_TRY(cudaMemcpyAsync(g_sdT.p, dT_host, ngrad, cudaMemcpyHostToDevice, s), "H2D dT");
+    }
+    if (dx_host) {
+        WBMM_TRY(g_sT.reserve(ntab), "cudaMalloc T");
+        WBMM_TRY(g_sy.reserve(nact), "cudaMalloc dx");
+        WBMM_TRY(cudaMemcpyAsync(g_sT.p, T_host, ntab, cudaMemcpyHostToDevice, s), "H2D T");
+    }
+    st = wbmm_backward(desc, dT_host ? g_sx.p : nullptr, dx_host ? g_sT.p : nullptr, g_sdy.p,
+                       dx_host ? g_sy.p : nullptr, dT_host ? (float*)g_sdT.p : nullptr, s);
+    if (st != WBMM_STATUS_OK) return st;
+    if (dx_host) WBMM_TRY(cudaMemcpyAsync(dx_host, g_sy.p, nact, cudaMemcpyDeviceToHost, s), "D2H dx");
+    if (dT_host) WBMM_TRY(cudaMemcpyAsync(dT_host, g_sdT.p, ngrad, cudaMemcpyDeviceToHost, s), "D2H dT");
+    WBMM_TRY(cudaStreamSynchronize(s), "sync");
+    return WBMM_STATUS_OK;
+}
+
+void wbmm_release(void)
+{
+    std::lock_guard<std::mutex> lock(g_host_mutex);
+    g_sx.release(); g_sT.release(); g_sy.release(); g_sdy.release(); g_sdT.release();
+    if (g_host_stream) { cudaStreamDestroy(g_host_stream); g_host_stream = nullptr; }
+    wbmm::tc_release();
+}
+
+int wbmm_last_path(void) { return t_last_path; }
+uint64_t wbmm_launch_count(void) { return g_launches.load(); }
+const char* wbmm_last_error_string(void) { return t_last_error; }
+int wbmm_version(void) { return WBMM_VERSION; }
+
+const char* wbmm_status_string(int status)
+{
+    switch (status) {
+    case WBMM_STATUS_OK: return "ok";
+    case WBMM_STATUS_INVALID_ARGUMENT: return "invalid argument";
+    case WBMM_STATUS_UNSUPPORTED: return "unsupported configuration";
+    case WBMM_STATUS_NO_DEVICE: return "no sm_100 CUDA device";
+    case WBMM_STATUS_CUDA_ERROR: return "CUDA error";
+    case WBMM_STATUS_MISALIGNED: return "misaligned pointer";
+    default: return "unknown status";
+    }
+}
+
+const char* wbmm_path_string(int path)
+{
+    switch (path) {
+    case WBMM_PATH_NONE: return "none";
+    case WBMM_PATH_SIMT: return "simt";
+    case WBMM_PATH_TC_TMA: return "tcgen05+tma";
+    case WBMM_PATH_TC_GATHER: return "tcgen05+gather";
+    default: return "unknown path";
+    }
+}
+
+}  // extern "C"

@@ -1,0 +1,68 @@
+// Shared host/device declarations for the WBMM kernels (not part of the C ABI).
+#pragma once
+
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "wbmm.h"
+
+namespace wbmm {
+
+// Geometry derived once on the host from wbmm_desc_t (Eq. 4-5: bottom/right zero padding).
+struct Geom {
+    int B, C, H, W, w;
+    int sh, sw;          // cyclic shift (reading A6), 0 = none
+    int layout;          // WBMM_LAYOUT_*
+    int Hp, Wp;          // padded extents H', W'
+    int nwh, nww;        // windows per column / row
+    int N;               // positions per window
+    int tw, nb;          // table side 2w-1 and bins (2w-1)^2
+    long long nwin;      // windows per channel L = B*nwh*nww
+};
+
+inline Geom make_geom(const wbmm_desc_t& d)
+{
+    Geom g;
+    g.B = d.B; g.C = d.C; g.H = d.H; g.W = d.W; g.w = d.w;
+    g.sh = d.shift_h; g.sw = d.shift_w; g.layout = d.layout;
+    g.Hp = (d.H + d.w - 1) / d.w * d.w;
+    g.Wp = (d.W + d.w - 1) / d.w * d.w;
+    g.nwh = g.Hp / d.w; g.nww = g.Wp / d.w;
+    g.N = d.w * d.w;
+    g.tw = 2 * d.w - 1; g.nb = g.tw * g.tw;
+    g.nwin = (long long)d.B * g.nwh * g.nww;
+    return g;
+}
+
+__device__ __forceinline__ float to_f32(float v) { return v; }
+__device__ __forceinline__ float to_f32(__nv_bfloat16 v) { return __bfloat162float(v); }
+__device__ __forceinline__ float to_f32(__half v) { return __half2float(v); }
+
+template <typename E> __device__ __forceinline__ E from_f32(float v);
+template <> __device__ __forceinline__ float from_f32<float>(float v) { return v; }
+template <> __device__ __forceinline__ __nv_bfloat16 from_f32<__nv_bfloat16>(float v) { return __float2bfloat16_rn(v); }
+template <> __device__ __forceinline__ __half from_f32<__half>(float v) { return __float2half_rn(v); }
+
+// Element offset of logical (b,c,h,v) in the activation tensor.
+__device__ __forceinline__ long long act_offset(const Geom& g, int b, int c, int h, int v)
+{
+    if (g.layout == WBMM_LAYOUT_NCHW)
+        return (((long long)b * g.C + c) * g.H + h) * g.W + v;
+    return (((long long)b * g.H + h) * g.W + v) * g.C + c;
+}
+
+// Launchers (defined in the .cu files).  All are asynchronous on `stream` and return the
+// cudaGetLastError() of their launches.  `reverse` selects the transposed operator W_c^T
+// (table index k -> nb-1-k), which is dX.
+cudaError_t simt_forward(const Geom& g, int dtype, const void* x, const void* T, void* y,
+                         bool reverse, cudaStream_t stream, int* launches);
+cudaError_t simt_grad_table(const Geom& g, int dtype, const void* x, const void* dy, float* dT,
+                            cudaStream_t stream, int* launches);
+cudaError_t simt_materialize(int C, int w, int dtype, const void* T, void* Wout,
+                             cudaStream_t stream, int* launches);
+// Largest window the SIMT kernels can stage in shared memory for this layout.
+bool simt_supported(const Geom& g);
+
+}  // namespace wbmm

@@ -1,0 +1,328 @@
+// General WBMM kernels on the fp32 ALUs (FFMA): any window side, dtype, layout, shift and ragged
+// size.  They are the fp32 path (BASELINE.json config 1), the route for shapes the tensor-core
+// kernels do not cover, and the on-GPU cross-check for them.  Window partition, zero padding,
+// cyclic shift and un-partition are index arithmetic in the loads and stores (Alg. 1 l.1-4, l.17;
+// PAPER.md:157-173); W_c is never formed: each thread walks the (2w-1)^2 table staged in shared
+// memory with the Eq. 7 index.
+#include "wbmm_common.cuh"
+
+namespace wbmm {
+
+namespace {
+
+constexpr int kThreads = 256;
+
+// One block works on CB channels x G windows.  Shared memory (floats):
+//   Ts[CB][nbp]      table rows (reversed for the transposed operator), nbp = nb rounded up to 4
+//   xs[CB][N][G]     input windows, window index fastest (float4 broadcast loads)
+//   ys[CB][N][G]     output windows (forward) / dY windows (table gradient)
+struct TileIndex {
+    int cb, g, q;
+};
+
+// Flat staging index -> (cb, g, q).  NCHW: q fastest (runs of w contiguous elements);
+// NHWC: cb fastest (contiguous channels).
+template <int G>
+__device__ __forceinline__ TileIndex decode(const Geom& g, int idx, int CB)
+{
+    TileIndex t;
+    if (g.layout == WBMM_LAYOUT_NCHW) {
+        t.q = idx % g.N;
+        int r = idx / g.N;
+        t.g = r % G;
+        t.cb = r / G;
+    } else {
+        t.cb = idx % CB;
+        int r = idx / CB;
+        t.q = r % g.N;
+        t.g = r / g.N;
+    }
+    return t;
+}
+
+// Source/destination element of window `win`, in-window position q, after zero padding and the
+// cyclic shift: returns -1 when the position lies in the padding.
+__device__ __forceinline__ long long window_elem(const Geom& g, long long win, int q, int c)
+{
+    int per_img = g.nwh * g.nww;
+    int b = (int)(win / per_img);
+    int r = (int)(win % per_img);
+    int wy = r / g.nww, wx = r % g.nww;
+    int h = wy * g.w + q / g.w + g.sh;
+    int v = wx * g.w + q % g.w + g.sw;
+    if (h >= g.Hp) h -= g.Hp;
+    if (v >= g.Wp) v -= g.Wp;
+    if (h >= g.H || v >= g.W) return -1;
+    return act_offset(g, b, c, h, v);
+}
+
+template <typename E, int G>
+__device__ __forceinline__ void stage_windows(const Geom& g, const E* __restrict__ src, float* dst,
+                                              long long win0, int c0, int CB)
+{
+    const int total = CB * G * g.N;
+    for (int idx = threadIdx.x; idx < total; idx += kThreads) {
+        TileIndex t = decode<G>(g, idx, CB);
+        long long win = win0 + t.g;
+        int c = c0 + t.cb;
+        float val = 0.f;
+        if (win < g.nwin && c < g.C) {
+            long long off = window_elem(g, win, t.q, c);
+            if (off >= 0) val = to_f32(src[off]);
+        }
+        dst[(t.cb * g.N + t.q) * G + t.g] = val;
+    }
+}
+
+template <typename E, int G>
+__global__ void __launch_bounds__(kThreads)
+simt_forward_kernel(Geom g, const E* __restrict__ x, const E* __restrict__ T, E* __restrict__ y,
+                    int CB, int reverse)
+{
+    extern __shared__ __align__(16) float smem[];
+    const int nbp = (g.nb + 3) & ~3;
+    float* Ts = smem;
+    float* xs = Ts + CB * nbp;
+    float* ys = xs + CB * g.N * G;
+    const int c0 = blockIdx.y * CB;
+    const long long win0 = (long long)blockIdx.x * G;
+
+    for (int idx = threadIdx.x; idx < CB * g.nb; idx += kThreads) {
+        int cb = idx / g.nb, k = idx % g.nb;
+        int c = c0 + cb;
+        int ks = reverse ? g.nb - 1 - k : k;
+        Ts[cb * nbp + k] = c < g.C ? to_f32(T[(long long)c * g.nb + ks]) : 0.f;
+    }
+    stage_windows<E, G>(g, x, xs, win0, c0, CB);
+    __syncthreads();
+
+    const int w = g.w, tw = g.tw;
+    for (int cb = 0; cb < CB; ++cb) {
+        const float* xc = xs + cb * g.N * G;
+        for (int p = threadIdx.x; p < g.N; p += kThreads) {
+            const int rp = p / w, cp = p % w;
+            // Eq. 7 with i = p (output), j = q (input): idx = (rp-rq+w-1)*tw + (cp-cq+w-1)
+            const float* Tc = Ts + cb * nbp + (rp + w - 1) * tw + cp + w - 1;
+            float acc[G];
+#pragma unroll
+            for (int k = 0; k < G; ++k) acc[k] = 0.f;
+            for (int rq = 0; rq < w; ++rq) {
+                const float* Tr = Tc - rq * tw;
+                const float4* xr = reinterpret_cast<const float4*>(xc + rq * w * G);
+                for (int cq = 0; cq < w; ++cq) {
+                    const float t = Tr[-cq];
+#pragma unroll
+                    for (int k4 = 0; k4 < G / 4; ++k4) {
+                        float4 xv = xr[cq * (G / 4) + k4];
+                        acc[4 * k4 + 0] = fmaf(t, xv.x, acc[4 * k4 + 0]);
+                        acc[4 * k4 + 1] = fmaf(t, xv.y, acc[4 * k4 + 1]);
+                        acc[4 * k4 + 2] = fmaf(t, xv.z, acc[4 * k4 + 2]);
+                        acc[4 * k4 + 3] = fmaf(t, xv.w, acc[4 * k4 + 3]);
+                    }
+                }
+            }
+            float4* yo = reinterpret_cast<float4*>(ys + (cb * g.N + p) * G);
+#pragma unroll
+            for (int k4 = 0; k4 < G / 4; ++k4)
+                yo[k4] = make_float4(acc[4 * k4], acc[4 * k4 + 1], acc[4 * k4 + 2], acc[4 * k4 + 3]);
+        }
+    }
+    __syncthreads();
+
+    // Un-partition: an output of the shifted frame returns to the element its input came from.
+    const int total = CB * G * g.N;
+    for (int idx = threadIdx.x; idx < total; idx += kThreads) {
+        TileIndex t = decode<G>(g, idx, CB);
+        long long win = win0 + t.g;
+        int c = c0 + t.cb;
+        if (win < g.nwin && c < g.C) {
+            long long off = window_elem(g, win, t.q, c);
+            if (off >= 0) y[off] = from_f32<E>(ys[(t.cb * g.N + t.q) * G + t.g]);
+        }
+    }
+}
+
+// dT[c,k] = sum over windows and pairs (p,q) with rel(p,q)=k of dY[p]*X[q].  One thread per bin:
+// for bin (dr,dc) the pairs are p=(rp,cp), q=(rp-dr,cp-dc) with both inside the window.
+template <typename E, int G>
+__global__ void __launch_bounds__(kThreads)
+simt_grad_table_kernel(Geom g, const E* __restrict__ x, const E* __restrict__ dy, float* __restrict__ dT,
+                       int CB, int groups_per_block)
+{
+    extern __shared__ __align__(16) float smem[];
+    const int nbp = (g.nb + 3) & ~3;
+    float* Ds = smem;                    // per-block partial table gradient
+    float* xs = Ds + CB * nbp;
+    float* gs = xs + CB * g.N * G;
+    const int c0 = blockIdx.y * CB;
+    const long long ngroups = (g.nwin + G - 1) / G;
+    const long long grp0 = (long long)blockIdx.x * groups_per_block;
+
+    for (int idx = threadIdx.x; idx < CB * nbp; idx += kThreads) Ds[idx] = 0.f;
+
+    const int w = g.w, tw = g.tw;
+    for (long long grp = grp0; grp < grp0 + groups_per_block && grp < ngroups; ++grp) {
+        __syncthreads();
+        stage_windows<E, G>(g, x, xs, grp * G, c0, CB);
+        stage_windows<E, G>(g, dy, gs, grp * G, c0, CB);
+        __syncthreads();
+        for (int cb = 0; cb < CB; ++cb) {
+            const float* xc = xs + cb * g.N * G;
+            const float* gc = gs + cb * g.N * G;
+            for (int k = threadIdx.x; k < g.nb; k += kThreads) {
+                const int dr = k / tw - (w - 1), dc = k % tw - (w - 1);
+                const int r0 = max(0, dr), r1 = min(w, w + dr);
+                const int q0 = max(0, dc), q1 = min(w, w + dc);
+                float acc = 0.f;
+                for (int rp = r0; rp < r1; ++rp)
+                    for (int cp = q0; cp < q1; ++cp) {
+                        const float4* gv = reinterpret_cast<const float4*>(gc + (rp * w + cp) * G);
+                        const float4* xv = reinterpret_cast<const float4*>(xc + ((rp - dr) * w + cp - dc) * G);
+#pragma unroll
+                        for (int k4 = 0; k4 < G / 4; ++k4) {
+                            float4 a = gv[k4], b = xv[k4];
+                            acc = fmaf(a.x, b.x, acc);
+                            acc = fmaf(a.y, b.y, acc);
+                            acc = fmaf(a.z, b.z, acc);
+                            acc = fmaf(a.w, b.w, acc);
+                        }
+                    }
+                Ds[cb * nbp + k] += acc;      // each (cb,k) is owned by one thread
+            }
+        }
+    }
+    __syncthreads();
+    for (int idx = threadIdx.x; idx < CB * g.nb; idx += kThreads) {
+        int cb = idx / g.nb, k = idx % g.nb;
+        if (c0 + cb < g.C) atomicAdd(&dT[(long long)(c0 + cb) * g.nb + k], Ds[cb * nbp + k]);
+    }
+}
+
+template <typename E>
+__global__ void materialize_kernel(int C, int w, const E* __restrict__ T, E* __restrict__ Wout)
+{
+    const int N = w * w, tw = 2 * w - 1, nb = tw * tw;
+    const long long total = (long long)C * N * N;
+    for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
+         idx += (long long)gridDim.x * blockDim.x) {
+        int j = (int)(idx % N);
+        long long r = idx / N;
+        int i = (int)(r % N);
+        int c = (int)(r / N);
+        int rel = (i / w - j / w + w - 1) * tw + (i % w - j % w + w - 1);   // Eq. 6-7
+        Wout[idx] = T[(long long)c * nb + rel];                              // Eq. 8: a copy
+    }
+}
+
+struct TileCfg {
+    int CB, G;
+    size_t smem_fwd, smem_dt;
+};
+
+TileCfg tile_cfg(const Geom& g)
+{
+    TileCfg t;
+    const size_t nbp = (g.nb + 3) & ~3;
+    if (g.layout == WBMM_LAYOUT_NCHW) { t.CB = 1; t.G = 8; }
+    else { t.CB = 8; t.G = 4; }
+    t.smem_fwd = sizeof(float) * t.CB * (nbp + 2ull * g.N * t.G);
+    t.smem_dt = t.smem_fwd;
+    return t;
+}
+
+constexpr size_t kMaxSmem = 227 * 1024;
+
+template <typename E>
+cudaError_t forward_t(const Geom& g, const E* x, const E* T, E* y, bool reverse, cudaStream_t s)
+{
+    TileCfg t = tile_cfg(g);
+    dim3 grid((unsigned)((g.nwin + t.G - 1) / t.G), (unsigned)((g.C + t.CB - 1) / t.CB));
+    cudaError_t e;
+    if (t.G == 8) {
+        auto k = simt_forward_kernel<E, 8>;
+        e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t.smem_fwd);
+        if (e != cudaSuccess) return e;
+        k<<<grid, kThreads, t.smem_fwd, s>>>(g, x, T, y, t.CB, reverse ? 1 : 0);
+    } else {
+        auto k = simt_forward_kernel<E, 4>;
+        e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t.smem_fwd);
+        if (e != cudaSuccess) return e;
+        k<<<grid, kThreads, t.smem_fwd, s>>>(g, x, T, y, t.CB, reverse ? 1 : 0);
+    }
+    return cudaGetLastError();
+}
+
+template <typename E>
+cudaError_t grad_table_t(const Geom& g, const E* x, const E* dy, float* dT, cudaStream_t s)
+{
+    TileCfg t = tile_cfg(g);
+    const long long ngroups = (g.nwin + t.G - 1) / t.G;
+    const int cblocks = (g.C + t.CB - 1) / t.CB;
+    // about 8 waves of blocks; each block folds its windows into one set of atomics
+    long long want = (8ll * 148 + cblocks - 1) / cblocks;
+    if (want < 1) want = 1;
+    long long nsplit = ngroups < want ? ngroups : want;
+    int gpb = (int)((ngroups + nsplit - 1) / nsplit);
+    nsplit = (ngroups + gpb - 1) / gpb;
+    dim3 grid((unsigned)nsplit, (unsigned)cblocks);
+    cudaError_t e;
+    if (t.G == 8) {
+        auto k = simt_grad_table_kernel<E, 8>;
+        e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t.smem_dt);
+        if (e != cudaSuccess) return e;
+        k<<<grid, kThreads, t.smem_dt, s>>>(g, x, dy, dT, t.CB, gpb);
+    } else {
+        auto k = simt_grad_table_kernel<E, 4>;
+        e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t.smem_dt);
+        if (e != cudaSuccess) return e;
+        k<<<grid, kThreads, t.smem_dt, s>>>(g, x, dy, dT, t.CB, gpb);
+    }
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+bool simt_supported(const Geom& g)
+{
+    TileCfg t = tile_cfg(g);
+    return t.smem_fwd <= kMaxSmem && g.C <= 65535ll * t.CB && (g.nwin + t.G - 1) / t.G <= 0x7fffffffll;
+}
+
+cudaError_t simt_forward(const Geom& g, int dtype, const void* x, const void* T, void* y,
+                         bool reverse, cudaStream_t s, int* launches)
+{
+    if (g.nwin == 0 || g.C == 0) return cudaSuccess;
+    *launches += 1;
+    switch (dtype) {
+    case WBMM_DTYPE_F32: return forward_t<float>(g, (const float*)x, (const float*)T, (float*)y, reverse, s);
+    case WBMM_DTYPE_BF16: return forward_t<__nv_bfloat16>(g, (const __nv_bfloat16*)x, (const __nv_bfloat16*)T, (__nv_bfloat16*)y, reverse, s);
+    default: return forward_t<__half>(g, (const __half*)x, (const __half*)T, (__half*)y, reverse, s);
+    }
+}
+
+cudaError_t simt_grad_table(const Geom& g, int dtype, const void* x, const void* dy, float* dT,
+                            cudaStream_t s, int* launches)
+{
+    if (g.nwin == 0 || g.C == 0) return cudaSuccess;
+    *launches += 1;
+    switch (dtype) {
+    case WBMM_DTYPE_F32: return grad_table_t<float>(g, (const float*)x, (const float*)dy, dT, s);
+    case WBMM_DTYPE_BF16: return grad_table_t<__nv_bfloat16>(g, (const __nv_bfloat16*)x, (const __nv_bfloat16*)dy, dT, s);
+    default: return grad_table_t<__half>(g, (const __half*)x, (const __half*)dy, dT, s);
+    }
+}
+
+cudaError_t simt_materialize(int C, int w, int dtype, const void* T, void* Wout, cudaStream_t s, int* launches)
+{
+    const long long total = (long long)C * w * w * w * w;
+    if (total == 0) return cudaSuccess;
+    int blocks = (int)((total + 255) / 256 < 148 * 16 ? (total + 255) / 256 : 148 * 16);
+    *launches += 1;
+    if (dtype == WBMM_DTYPE_F32)
+        materialize_kernel<uint32_t><<<blocks, 256, 0, s>>>(C, w, (const uint32_t*)T, (uint32_t*)Wout);
+    else
+        materialize_kernel<uint16_t><<<blocks, 256, 0, s>>>(C, w, (const uint16_t*)T, (uint16_t*)Wout);
+    return cudaGetLastError();
+}
+
+}  // namespace wbmm

@@ -1,0 +1,248 @@
+"""GPU parity: libwbmm.so (through the C ABI, via the ctypes binding) against the CPU oracle,
+element by element on the same seeded inputs.  Bar (BASELINE.json north_star):
+|got - ref| <= tol*(1+|ref|), tol = 1e-2 for bf16/fp16 (fp32 accumulate), 1e-4 for fp32;
+relative-position indexing and data movement bit-exact.
+"""
+import numpy as np
+import pytest
+import torch
+
+import synth_inputs as si
+from parity import TOL, max_err_over_tol, plane_subset, take_planes, widen
+
+pytestmark = pytest.mark.gpu
+
+NCHW, NHWC = si.NCHW, si.NHWC
+
+
+@pytest.fixture(scope="module")
+def wb():
+    import paper_2607_02097_b200 as wb
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    wb.wbmm_version()          # loads libwbmm.so or raises: no silent fallback
+    return wb
+
+
+def run_forward(wb, oracle, case, flags=0, sample=None, expect_path=None):
+    d = si.make(case, device="cuda")
+    y = wb.wbmm_forward(d["x"], d["T"], case.w, case.shift, case.layout, flags)
+    torch.cuda.synchronize()
+    path = wb.wbmm_last_path()
+    if expect_path is not None:
+        assert path == expect_path, wb.wbmm_path_string(path)
+    bs = cs = None
+    if sample:
+        bs, cs = plane_subset(case, *sample)
+    xs = take_planes(d["x"], case.layout, bs, cs)
+    Ts = d["T"].cpu() if cs is None else d["T"].cpu().index_select(0, cs)
+    ref = oracle.forward(widen(xs), widen(Ts), case.w, case.shift, case.layout, "direct")
+    err = max_err_over_tol(take_planes(y, case.layout, bs, cs), ref, TOL[case.dtype])
+    return err, path
+
+
+def run_backward(wb, oracle, case, flags=0, sample_c=None):
+    d = si.make(case, device="cuda")
+    dx, dT = wb.wbmm_backward(d["x"], d["T"], d["dy"], case.w, case.shift, case.layout, flags)
+    torch.cuda.synchronize()
+    cs = None
+    if sample_c:
+        _, cs = plane_subset(case, case.B, sample_c)
+    xs, gs = (take_planes(d[k], case.layout, None, cs) for k in ("x", "dy"))
+    Ts = d["T"].cpu() if cs is None else d["T"].cpu().index_select(0, cs)
+    rdx, rdT = oracle.backward(widen(xs), widen(Ts), widen(gs), case.w, case.shift, case.layout)
+    e_dx = max_err_over_tol(take_planes(dx, case.layout, None, cs), rdx, TOL[case.dtype])
+    dTs = dT.cpu() if cs is None else dT.cpu().index_select(0, cs)
+    e_dT = max_err_over_tol(dTs, rdT, TOL[case.dtype])
+    return e_dx, e_dT
+
+
+# ------------------------------------------------------------------ small cases, every variant
+SMALL = [
+    si.Case("s_w3", 2, 3, 6, 9, 3, dtype="f32"),
+    si.Case("s_w4_ragged", 3, 5, 10, 7, 4, dtype="f32"),
+    si.Case("s_w7_shift", 2, 4, 14, 21, 7, dtype="f32", shift=(3, 2)),
+    si.Case("s_w14", 3, 5, 28, 42, 14, dtype="bf16"),
+    si.Case("s_w14_ragged_shift", 2, 9, 30, 25, 14, dtype="bf16", shift=(7, 5)),
+    si.Case("s_w7_f16", 5, 17, 21, 28, 7, dtype="f16"),
+    si.Case("s_w1", 2, 3, 5, 4, 1, dtype="f32"),
+    si.Case("s_w16", 1, 2, 32, 16, 16, dtype="bf16"),
+    si.Case("s_w20", 1, 2, 20, 40, 20, dtype="f32"),
+    si.Case("s_many_windows", 33, 3, 28, 28, 7, dtype="bf16"),     # several blocks + ragged tail
+]
+
+
+@pytest.mark.parametrize("case", SMALL, ids=lambda c: c.name)
+@pytest.mark.parametrize("layout", [NCHW, NHWC])
+@pytest.mark.parametrize("force_simt", [True, False])
+def test_forward_small(wb, oracle, case, layout, force_simt):
+    case = si.with_(case, layout=layout)
+    err, _ = run_forward(wb, oracle, case, wb.FLAG_FORCE_SIMT if force_simt else 0)
+    assert err <= 1.0, err
+
+
+@pytest.mark.parametrize("case", SMALL, ids=lambda c: c.name)
+@pytest.mark.parametrize("layout", [NCHW, NHWC])
+@pytest.mark.parametrize("force_simt", [True, False])
+def test_backward_small(wb, oracle, case, layout, force_simt):
+    case = si.with_(case, layout=layout, backward=True)
+    e_dx, e_dT = run_backward(wb, oracle, case, wb.FLAG_FORCE_SIMT if force_simt else 0)
+    assert e_dx <= 1.0 and e_dT <= 1.0, (e_dx, e_dT)
+
+
+def test_config1_fp32_tiny(wb, oracle):
+    """BASELINE.json config 1: fp32 path, <= 1e-4."""
+    err, path = run_forward(wb, oracle, si.CFG1)
+    assert err <= 1.0, err
+    assert path == wb.PATH_SIMT
+
+
+# ------------------------------------------------------------------ exact structured tests
+@pytest.mark.parametrize("dtype", ["f32", "bf16", "f16"])
+@pytest.mark.parametrize("layout", [NCHW, NHWC])
+@pytest.mark.parametrize("w,shift,H,W", [(7, (0, 0), 14, 21), (14, (0, 0), 28, 56), (14, (7, 7), 28, 28),
+                                         (7, (3, 3), 15, 20), (14, (5, 9), 30, 60)])
+@pytest.mark.parametrize("force_simt", [True, False])
+def test_delta_table_is_identity_bitwise(wb, dtype, layout, w, shift, H, W, force_simt):
+    """Delta at the zero-offset bin => y == x bitwise (any dtype, any path)."""
+    case = si.Case("delta", 3, 6, H, W, w, dtype=dtype, layout=layout, shift=shift, seed=21)
+    d = si.make(case, device="cuda")
+    T = torch.zeros_like(d["T"])
+    tw = 2 * w - 1
+    T[:, (w - 1) * tw + (w - 1)] = 1.0
+    y = wb.wbmm_forward(d["x"], T, w, shift, layout, wb.FLAG_FORCE_SIMT if force_simt else 0)
+    assert torch.equal(y, d["x"])
+
+
+@pytest.mark.parametrize("w", [7, 14])
+@pytest.mark.parametrize("force_simt", [True, False])
+def test_one_hot_table_every_bin_bitwise(wb, oracle, w, force_simt):
+    """One-hot table at every bin k: the GPU result must equal the oracle's bitwise (a pure data
+    movement: y[r,c] = x[r-dr,c-dc] or 0).  Channel c carries bin (c mod nb): all (2w-1)^2 bins
+    are covered by C = nb channels in one launch.  This is the bit-exact indexing test."""
+    tw = 2 * w - 1
+    nb = tw * tw
+    case = si.Case("onehot", 2, nb, 2 * w, 4 * w, w, dtype="bf16", seed=22)
+    d = si.make(case, device="cuda")
+    T = torch.zeros_like(d["T"])
+    T[torch.arange(nb), torch.arange(nb)] = 1.0
+    y = wb.wbmm_forward(d["x"], T, w, flags=wb.FLAG_FORCE_SIMT if force_simt else 0)
+    ref = oracle.forward(widen(d["x"]), widen(T), w)
+    assert np.array_equal(widen(y), ref)
+    dx, _ = wb.wbmm_backward(None, T, d["x"], w, need_dT=False, flags=wb.FLAG_FORCE_SIMT if force_simt else 0)
+    rdx, _ = oracle.backward(widen(d["x"]), widen(T), widen(d["x"]), w, need_dT=False)
+    assert np.array_equal(widen(dx), rdx)
+
+
+@pytest.mark.parametrize("force_simt", [True, False])
+def test_all_ones_table_window_sums_exact(wb, force_simt):
+    """All-ones table => every output is its window's sum; small-integer x keeps bf16 exact.
+    Pins partition + zero padding on the GPU without the oracle."""
+    w, B, C, H, W = 14, 2, 3, 30, 60
+    g = torch.Generator().manual_seed(5)
+    x = torch.randint(-2, 3, (B, C, H, W), generator=g).to(torch.bfloat16).cuda()
+    T = torch.ones((C, 27 * 27), dtype=torch.bfloat16, device="cuda")
+    y = wb.wbmm_forward(x, T, w, flags=wb.FLAG_FORCE_SIMT if force_simt else 0).float().cpu()
+    xp = torch.zeros(B, C, 42, 70)
+    xp[:, :, :H, :W] = x.float().cpu()
+    sums = xp.reshape(B, C, 3, 14, 5, 14).sum(dim=(3, 5))
+    exp = sums[:, :, :, None, :, None].expand(B, C, 3, 14, 5, 14).reshape(B, C, 42, 70)[:, :, :H, :W]
+    assert torch.equal(y, exp)
+
+
+@pytest.mark.parametrize("dtype", ["f32", "bf16", "f16"])
+@pytest.mark.parametrize("w", [3, 7, 14])
+def test_materialize_weight_bitwise(wb, oracle, dtype, w):
+    """a1+a2: W[c,i,j] = T[c, rel(i,j)] must equal the oracle's gather bit for bit."""
+    case = si.Case("mat", 1, 5, w, w, w, dtype=dtype, seed=23)
+    T = si.make(case, device="cuda")["T"]
+    Wg = wb.wbmm_materialize_weight(T, w)
+    assert np.array_equal(widen(Wg), oracle.weight_matrix(widen(T), w))
+
+
+def test_output_is_fully_overwritten_and_nothing_else(wb):
+    """y is written exactly on its B*C*H*W elements: canary-filled, over-allocated buffer."""
+    case = si.Case("canary", 2, 3, 30, 25, 14, dtype="bf16", shift=(7, 3), seed=24)
+    d = si.make(case, device="cuda")
+    n = d["x"].numel()
+    for flags in (0, wb.FLAG_FORCE_SIMT):
+        buf = torch.full((n + 4096,), float("nan"), dtype=torch.bfloat16, device="cuda")
+        y = buf[2048:2048 + n].view_as(d["x"])
+        wb.wbmm_forward(d["x"], d["T"], 14, case.shift, out=y, flags=flags)
+        assert torch.isnan(buf[:2048]).all() and torch.isnan(buf[2048 + n:]).all()
+        assert not torch.isnan(y).any()
+
+
+def test_empty_inputs(wb):
+    for shape in ((0, 4, 14, 14), (2, 0, 14, 14)):
+        x = torch.zeros(shape, dtype=torch.bfloat16, device="cuda")
+        T = torch.zeros((shape[1], 169), dtype=torch.bfloat16, device="cuda")
+        y = wb.wbmm_forward(x, T, 7)
+        assert y.shape == x.shape
+        dx, dT = wb.wbmm_backward(x, T, x, 7)
+        assert dT.shape == (shape[1], 169) and torch.count_nonzero(dT) == 0
+
+
+def test_dT_accumulate_flag_and_run_to_run(wb, oracle):
+    case = si.Case("acc", 4, 6, 28, 28, 14, dtype="bf16", seed=25, backward=True)
+    d = si.make(case, device="cuda")
+    _, dT1 = wb.wbmm_backward(d["x"], d["T"], d["dy"], 14, need_dx=False)
+    _, dT2 = wb.wbmm_backward(d["x"], d["T"], d["dy"], 14, need_dx=False)
+    assert torch.all((dT1 - dT2).abs() <= 1e-5 * (1 + dT1.abs()))     # atomics: rounding only
+    acc = dT1.clone()
+    wb.wbmm_backward(d["x"], d["T"], d["dy"], 14, need_dx=False, dT=acc, flags=wb.FLAG_ACCUMULATE_DT)
+    assert torch.allclose(acc, 2 * dT1, rtol=1e-5, atol=1e-5)
+
+
+def test_host_entry_points(wb, oracle):
+    case = si.Case("host", 2, 5, 28, 30, 14, dtype="bf16", shift=(7, 7), seed=26, backward=True)
+    d = si.make(case)
+    y = wb.wbmm_forward_host(d["x"], d["T"], 14, case.shift)
+    ref = oracle.forward(widen(d["x"]), widen(d["T"]), 14, case.shift)
+    assert max_err_over_tol(y, ref, 1e-2) <= 1.0
+    dx, dT = wb.wbmm_backward_host(d["x"], d["T"], d["dy"], 14, case.shift)
+    rdx, rdT = oracle.backward(widen(d["x"]), widen(d["T"]), widen(d["dy"]), 14, case.shift)
+    assert max_err_over_tol(dx, rdx, 1e-2) <= 1.0 and max_err_over_tol(dT, rdT, 1e-2) <= 1.0
+
+
+def test_non_default_stream(wb, oracle):
+    case = si.Case("stream", 2, 4, 28, 28, 14, dtype="bf16", seed=27)
+    d = si.make(case, device="cuda")
+    s = torch.cuda.Stream()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(s):
+        y = wb.wbmm_forward(d["x"], d["T"], 14)
+    s.synchronize()
+    ref = oracle.forward(widen(d["x"]), widen(d["T"]), 14)
+    assert max_err_over_tol(y, ref, 1e-2) <= 1.0
+
+
+# ------------------------------------------------------------------ BASELINE.json configs, full size
+def test_config2_full_size(wb, oracle):
+    err, _ = run_forward(wb, oracle, si.CFG2, sample=(6, 8))
+    assert err <= 1.0, err
+
+
+def test_config3_headline_full_size(wb, oracle):
+    """The launch configuration bench.py times; sampled planes (8 images x 8 channels, full planes)."""
+    err, _ = run_forward(wb, oracle, si.CFG3, sample=(8, 8))
+    assert err <= 1.0, err
+    err, _ = run_forward(wb, oracle, si.with_(si.CFG3, table="structured"), sample=(4, 4))
+    assert err <= 1.0, err
+
+
+def test_config5_training_step_full_size(wb, oracle):
+    err, _ = run_forward(wb, oracle, si.CFG5, sample=(8, 8))
+    assert err <= 1.0, err
+    e_dx, e_dT = run_backward(wb, oracle, si.CFG5, sample_c=6)
+    assert e_dx <= 1.0 and e_dT <= 1.0, (e_dx, e_dT)
+
+
+SWEEP = [c for c in si.sweep_cases()]
+# every (layout, (C,H), w) at one small and one large batch, plus both ragged cases
+SWEEP_PICK = [c for c in SWEEP if c.B in (4, 64) or "ragged" in c.name]
+
+
+@pytest.mark.parametrize("case", SWEEP_PICK, ids=lambda c: c.name)
+def test_config4_sweep(wb, oracle, case):
+    err, _ = run_forward(wb, oracle, case, sample=(3, 4))
+    assert err <= 1.0, err
