@@ -1,12 +1,28 @@
-// Tensor-core (tcgen05 / TMEM / TMA) WBMM kernels for bf16 / fp16 -- host-side interface.
+// Tensor-core (tcgen05 / TMEM / bulk-copy) WBMM kernels for bf16 / fp16 -- host-side interface.
 #pragma once
 
 #include "wbmm_common.cuh"
 
 namespace wbmm {
 
-// True when the tcgen05 forward kernel can serve this problem (dtype, window, layout, strides
-// legal for the TMA tensor map, pointer alignment).
+// How the windows of one channel are cut into MMA tiles of at most 128 windows (= 128 TMEM lanes).
+// A tile is NP images x NSY window-rows x all nww windows across; its activation data sits in
+// shared memory as a "frame": [image][NSY*w rows][Wp columns] in the padded + shifted coordinate
+// system, image stride S bytes.  Window (wl, pl) (wl = wyl*nww + wx inside the frame, pl = image
+// inside the tile) is MMA row m = wl*NP + pl.
+struct TcTiles {
+    int NP, NSY;
+    int nstrips;       // strips per image = ceil(nwh / NSY); > 1 only when NP == 1
+    int ngb;           // image groups = ceil(B / NP)
+    int tiles_per_c;   // ngb * nstrips
+    int frame_rows;    // NSY * w
+    int S;             // frame image stride in bytes: 16 * odd
+    long long ntiles;  // C * tiles_per_c
+};
+
+bool tc_tiles(const Geom& g, TcTiles* t);
+
+// True when a tcgen05 forward kernel can serve this problem.
 bool tc_forward_supported(const Geom& g, int dtype, const void* x, const void* y);
 cudaError_t tc_forward(const Geom& g, int dtype, const void* x, const void* T, void* y, bool reverse,
                        cudaStream_t stream, int* launches, int* path);
