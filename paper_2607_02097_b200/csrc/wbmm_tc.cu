@@ -278,6 +278,296 @@ tc_generic_kernel(Geom g, TcTiles tl, const uint16_t* __restrict__ x, const uint
     if (warp == 0) ptx::tmem_dealloc(tmem, Cf::TMEM_COLS);
 }
 
+// ------------------------------------------------------------------------------------------------
+// Fast kernel ("tcgen05+tma"): NCHW, no shift, H and W multiples of w.  Every frame image is one
+// contiguous run of global memory, so the TMA engine moves it with 1-D bulk copies
+// (cp.async.bulk, completion on an mbarrier) and the whole path is a warp-specialised pipeline:
+//
+//   warp 0      producer   bulk loads  x -> ring of frame-image slots            (full/empty barriers)
+//   warp 1      MMA        KSTEPS tcgen05.mma per tile, A from TMEM, B = W_c     (a_full/a_empty, d_full/d_empty)
+//   warps 2-5   repack     slot -> registers -> tcgen05.st into A[buf] (2 buffers); build W_c on a channel change
+//   warps 6-9   epilogue   tcgen05.ld D -> RNE 16-bit -> output frame -> bulk stores to y
+//
+// Each 32-bit shared-memory access of the repack / epilogue warps is conflict-free for the
+// headline geometry: lanes are (4 adjacent windows) x (8 images) and the image stride is 16*odd bytes.
+int num_sms();
+constexpr int kThreadsB = 320;
+constexpr int kMaxSlots = 64;
+
+// W_c for w = 14 from two copies of the fully reversed table F[q] = T[NB-1-q] (F0 = F, F1 = F
+// shifted by one value), so that any pair (F[q], F[q+1]) is one aligned 32-bit load.  Row i of W_c
+// is, for every input row rj, the run F[q0 + 27*rj + cj], cj = 0..13, q0 = (13-ri)*27 + 13-ci
+// (Eq. 7 rewritten for the reversed table).  128 threads (the repack warps); rows >= N and chunk
+// 25 stay zero from the kernel prologue.
+__device__ __forceinline__ void build_weight14(const uint16_t* __restrict__ Tc, bool reverse, uint16_t* F0,
+                                               uint16_t* F1, uint8_t* Wc, int tid)
+{
+    using Cf = WinCfg<14>;
+    for (int q = tid; q < Cf::NB; q += 128) {
+        const uint16_t v = Tc[reverse ? q : Cf::NB - 1 - q];
+        F0[q] = v;
+        if (q >= 1) F1[q - 1] = v;
+    }
+    ptx::named_bar_sync(2, 128);
+    for (int i = tid; i < Cf::N; i += 128) {
+        const int ri = i / 14, ci = i % 14;
+        const int q0 = (13 - ri) * 27 + 13 - ci, p0 = q0 & 1;
+        const uint8_t* be = reinterpret_cast<const uint8_t*>(p0 ? F1 : F0) + (q0 - p0) * 2;   // even rj
+        const uint8_t* bo = reinterpret_cast<const uint8_t*>(p0 ? F0 : F1) + (q0 + p0) * 2;   // odd rj
+        uint8_t* dst = Wc + i * 16;
+#pragma unroll
+        for (int kc = 0; kc < 25; ++kc) {
+            uint32_t pk[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const int j = kc * 8 + 2 * e;
+                const int rj = j / 14, cj = j % 14;
+                if (j >= Cf::N) pk[e] = 0u;
+                else if (rj % 2 == 0) pk[e] = *reinterpret_cast<const uint32_t*>(be + (27 * rj + cj) * 2);
+                else pk[e] = *reinterpret_cast<const uint32_t*>(bo + (27 * rj - 1 + cj) * 2);
+            }
+            *reinterpret_cast<uint4*>(dst + kc * Cf::LBO) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+        }
+    }
+}
+
+template <int WS>
+struct BulkSmem {
+    using Cf = WinCfg<WS>;
+    static constexpr int TAB_ONE = ((Cf::NB + 2) * 2 + 15) / 16 * 16;
+    static constexpr int TAB_BYTES = 2 * TAB_ONE;                              // F0 and F1 (or Ts for the generic builder)
+    static constexpr int BAR_BYTES = (2 * kMaxSlots + 8) * 8;
+    static constexpr int FIXED = Cf::WC_BYTES + TAB_BYTES + BAR_BYTES;
+};
+
+template <int WS, bool BF16>
+__global__ void __launch_bounds__(kThreadsB, 1)
+tc_bulk_kernel(Geom g, TcTiles tl, int nslot, const uint16_t* __restrict__ x, const uint16_t* __restrict__ T,
+               uint16_t* __restrict__ y, int reverse)
+{
+    using Cf = WinCfg<WS>;
+    using Sm = BulkSmem<WS>;
+    extern __shared__ __align__(1024) uint8_t smem[];
+    uint8_t* Wc = smem;
+    uint16_t* tab = reinterpret_cast<uint16_t*>(smem + Cf::WC_BYTES);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + Cf::WC_BYTES + Sm::TAB_BYTES);
+    uint8_t* outf = smem + Sm::FIXED;
+    uint8_t* ring = outf + tl.NP * tl.S;
+    __shared__ uint32_t tmem_base_s;
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const uint32_t bar0 = ptx::smem_u32(bars);
+    auto FULL = [&](int s) { return bar0 + 8u * s; };
+    auto EMPTY = [&](int s) { return bar0 + 8u * (kMaxSlots + s); };
+    const uint32_t A_FULL = bar0 + 8u * (2 * kMaxSlots), A_EMPTY = A_FULL + 16, D_FULL = A_FULL + 32, D_EMPTY = A_FULL + 40;
+
+    const int wpf = tl.NSY * g.nww;   // windows per frame image
+    if (warp == 0) ptx::tmem_alloc(ptx::smem_u32(&tmem_base_s), 512);
+    if (tid == 32) {
+        for (int s = 0; s < nslot; ++s) {
+            ptx::mbar_init(FULL(s), 1);
+            ptx::mbar_init(EMPTY(s), wpf);
+        }
+        ptx::mbar_init(A_FULL, 128);
+        ptx::mbar_init(A_FULL + 8, 128);
+        ptx::mbar_init(A_EMPTY, 1);
+        ptx::mbar_init(A_EMPTY + 8, 1);
+        ptx::mbar_init(D_FULL, 1);
+        ptx::mbar_init(D_EMPTY, 128);
+        ptx::fence_mbar_init();
+    }
+    for (int i = tid; i < Cf::WC_BYTES / 16; i += kThreadsB) reinterpret_cast<uint4*>(Wc)[i] = make_uint4(0, 0, 0, 0);
+    for (int i = tid; i < Sm::TAB_BYTES / 4; i += kThreadsB) reinterpret_cast<uint32_t*>(tab)[i] = 0u;
+    ptx::fence_proxy_async_smem();
+    ptx::tc_fence_before_sync();
+    __syncthreads();
+    ptx::tc_fence_after_sync();
+    const uint32_t tmem = tmem_base_s;
+    constexpr uint32_t A_STRIDE = (Cf::A_COLS + 31) / 32 * 32;
+    const uint32_t tmem_d = tmem + 2 * A_STRIDE;
+    static_assert(2 * ((Cf::A_COLS + 31) / 32 * 32) + Cf::N_PAD <= 512, "TMEM budget");
+
+    const long long t0 = tl.ntiles * blockIdx.x / gridDim.x, t1 = tl.ntiles * (blockIdx.x + 1) / gridDim.x;
+    const int rowB = g.W * 2;
+    const long long plane_elems = (long long)g.H * g.W;
+
+    auto tile_decode = [&](long long t, int& c, int& b0, int& wy0, int& np_eff, int& rows_eff) {
+        c = (int)(t / tl.tiles_per_c);
+        const int rem = (int)(t % tl.tiles_per_c);
+        const int gb = rem / tl.nstrips, strip = rem % tl.nstrips;
+        b0 = gb * tl.NP;
+        wy0 = strip * tl.NSY;
+        np_eff = min(tl.NP, g.B - b0);
+        rows_eff = min(tl.frame_rows, g.H - wy0 * WS);
+    };
+
+    if (warp == 0) {
+        // ------------------------------------------------------------------ producer
+        if (lane == 0) {
+            uint32_t k = 0;
+            for (long long t = t0; t < t1; ++t) {
+                int c, b0, wy0, np_eff, rows_eff;
+                tile_decode(t, c, b0, wy0, np_eff, rows_eff);
+                const uint32_t bytes = (uint32_t)rows_eff * rowB;
+                for (int p = 0; p < np_eff; ++p, ++k) {
+                    const int slot = k % nslot;
+                    ptx::mbar_wait(EMPTY(slot), ((k / nslot) & 1) ^ 1);
+                    ptx::mbar_arrive_expect_tx(FULL(slot), bytes);
+                    const uint16_t* src = x + ((long long)(b0 + p) * g.C + c) * plane_elems + (long long)wy0 * WS * g.W;
+                    ptx::bulk_g2s(ptx::smem_u32(ring + (size_t)slot * tl.S), src, bytes, FULL(slot));
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ------------------------------------------------------------------ MMA issuer
+        if (lane == 0) {
+            constexpr uint32_t idesc = ptx::idesc_f16(BF16 ? 1 : 0, 128, Cf::N_PAD);
+            const uint32_t wc_addr = ptx::smem_u32(Wc);
+            uint32_t lt = 0;
+            for (long long t = t0; t < t1; ++t, ++lt) {
+                const uint32_t buf = lt & 1;
+                ptx::mbar_wait(A_FULL + 8 * buf, (lt >> 1) & 1);
+                ptx::mbar_wait(D_EMPTY, (lt & 1) ^ 1);
+                ptx::tc_fence_after_sync();
+                const uint32_t tmem_a = tmem + buf * A_STRIDE;
+#pragma unroll
+                for (int ks = 0; ks < Cf::KSTEPS; ++ks) {
+                    const uint64_t bdesc = ptx::smem_desc_kmajor_noswz(wc_addr + ks * 2 * Cf::LBO, Cf::LBO, 128);
+                    ptx::mma_ts(tmem_d, tmem_a + ks * 8, bdesc, idesc, ks > 0 ? 1u : 0u);
+                }
+                ptx::mma_commit(A_EMPTY + 8 * buf);
+                ptx::mma_commit(D_FULL);
+            }
+        }
+    } else if (warp < 6) {
+        // ------------------------------------------------------------------ repack (+ W_c builder)
+        const int q = warp & 3;
+        const int m = q * 32 + lane;
+        const int rt = (warp - 2) * 32 + lane;   // 0..127 among the repack threads
+        const int wl = m / tl.NP, pl = m % tl.NP;
+        const int wyl = wl / g.nww, wx = wl % g.nww;
+        const int win_off = ((wyl * WS) * g.W + wx * WS) * 2;
+        uint32_t k = 0, lt = 0;
+        int cur_c = -1;
+        for (long long t = t0; t < t1; ++t, ++lt) {
+            int c, b0, wy0, np_eff, rows_eff;
+            tile_decode(t, c, b0, wy0, np_eff, rows_eff);
+            const uint32_t buf = lt & 1;
+            ptx::mbar_wait(A_EMPTY + 8 * buf, ((lt >> 1) & 1) ^ 1);   // MMA(lt-2) has consumed A[buf]
+            if (c != cur_c) {
+                if (lt > 0) ptx::mbar_wait(A_EMPTY + 8 * ((lt - 1) & 1), ((lt - 1) >> 1) & 1);   // MMA(lt-1) done with W_c
+                const uint16_t* Tc = T + (long long)c * Cf::NB;
+                if constexpr (WS == 14) {
+                    build_weight14(Tc, reverse != 0, tab, tab + Sm::TAB_ONE / 2, Wc, rt);
+                } else {
+                    for (int kk = rt; kk < Cf::NB; kk += 128) tab[kk] = Tc[reverse ? Cf::NB - 1 - kk : kk];
+                    ptx::named_bar_sync(2, 128);
+                    constexpr int NCHUNK = (Cf::K_PAD / 8) * Cf::N_PAD;
+                    for (int id = rt; id < NCHUNK; id += 128) {
+                        const int kc = id / Cf::N_PAD, i = id % Cf::N_PAD;
+                        uint32_t pk[4] = {0u, 0u, 0u, 0u};
+                        if (i < Cf::N) {
+                            const int ri = i / WS, ci = i % WS;
+                            int j = kc * 8, rj = j / WS, cj = j % WS;
+#pragma unroll
+                            for (int e = 0; e < 8; ++e) {
+                                uint32_t v = 0;
+                                if (j < Cf::N) v = tab[(ri - rj + WS - 1) * Cf::TW + (ci - cj + WS - 1)];
+                                pk[e >> 1] |= v << ((e & 1) * 16);
+                                ++j;
+                                if (++cj == WS) { cj = 0; ++rj; }
+                            }
+                        }
+                        *reinterpret_cast<uint4*>(Wc + kc * Cf::LBO + i * 16) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+                    }
+                }
+                ptx::fence_proxy_async_smem();
+                cur_c = c;
+            }
+            const bool part = wl < wpf && pl < np_eff;               // this thread's frame image was loaded
+            const bool valid = part && wy0 + wyl < g.nwh;
+            const uint32_t kk = k + pl;
+            const int slot = kk % nslot;
+            if (part) ptx::mbar_wait(FULL(slot), (kk / nslot) & 1);
+            window_to_tmem<WS>(ring + (size_t)slot * tl.S + win_off, valid, rowB,
+                               tmem + buf * A_STRIDE + ((uint32_t)(q * 32) << 16));
+            ptx::tc_fence_before_sync();
+            ptx::mbar_arrive(A_FULL + 8 * buf);
+            if (part) ptx::mbar_arrive(EMPTY(slot));
+            k += np_eff;
+        }
+    } else {
+        // ------------------------------------------------------------------ epilogue
+        const int q = warp & 3;
+        const int m = q * 32 + lane;
+        const int et = (warp - 6) * 32 + lane;   // 0..127 among the epilogue threads
+        const int wl = m / tl.NP, pl = m % tl.NP;
+        const int wyl = wl / g.nww, wx = wl % g.nww;
+        uint8_t* win = outf + pl * tl.S + ((wyl * WS) * g.W + wx * WS) * 2;
+        uint32_t lt = 0;
+        for (long long t = t0; t < t1; ++t, ++lt) {
+            int c, b0, wy0, np_eff, rows_eff;
+            tile_decode(t, c, b0, wy0, np_eff, rows_eff);
+            const bool valid = wl < wpf && pl < np_eff && wy0 + wyl < g.nwh;
+            ptx::mbar_wait(D_FULL, lt & 1);
+            ptx::tc_fence_after_sync();
+            if (et == 0) ptx::bulk_wait_read<0>();     // the previous tile's stores have left the output frame
+            ptx::named_bar_sync(1, 128);
+            tmem_to_window<WS, BF16>(win, valid, rowB, tmem_d + ((uint32_t)(q * 32) << 16));
+            ptx::tc_fence_before_sync();
+            ptx::mbar_arrive(D_EMPTY);
+            ptx::fence_proxy_async_smem();
+            ptx::named_bar_sync(1, 128);
+            if (et == 0) {
+                const uint32_t bytes = (uint32_t)rows_eff * rowB;
+                for (int p = 0; p < np_eff; ++p) {
+                    uint16_t* dst = y + ((long long)(b0 + p) * g.C + c) * plane_elems + (long long)wy0 * WS * g.W;
+                    ptx::bulk_s2g(dst, ptx::smem_u32(outf + p * tl.S), bytes);
+                }
+                ptx::bulk_commit();
+            }
+        }
+        if (et == 0) ptx::bulk_wait_all<0>();
+    }
+    ptx::tc_fence_before_sync();
+    __syncthreads();
+    if (warp == 0) ptx::tmem_dealloc(tmem, 512);
+}
+
+template <int WS>
+int bulk_slots(const TcTiles& tl)
+{
+    const long long room = 227ll * 1024 - 1024 - BulkSmem<WS>::FIXED - (long long)tl.NP * tl.S;
+    long long n = room / tl.S;
+    if (n > 2 * tl.NP) n = 2 * tl.NP;
+    if (n > kMaxSlots) n = kMaxSlots;
+    return (int)n;
+}
+
+template <int WS>
+bool bulk_ok(const Geom& g, const TcTiles& tl, const void* x, const void* y)
+{
+    if (g.layout != WBMM_LAYOUT_NCHW || g.sh != 0 || g.sw != 0 || g.H != g.Hp || g.W != g.Wp) return false;
+    if ((tl.frame_rows * g.W * 2) % 16 != 0 || ((long long)g.H * g.W * 2) % 16 != 0) return false;
+    if (reinterpret_cast<uintptr_t>(x) % 16 != 0 || reinterpret_cast<uintptr_t>(y) % 16 != 0) return false;
+    if (tl.NP > kMaxSlots) return false;
+    return bulk_slots<WS>(tl) >= tl.NP + 1;
+}
+
+template <int WS, bool BF16>
+cudaError_t launch_bulk(const Geom& g, const TcTiles& tl, const void* x, const void* T, void* y, bool reverse,
+                        cudaStream_t s)
+{
+    auto k = tc_bulk_kernel<WS, BF16>;
+    const int nslot = bulk_slots<WS>(tl);
+    const size_t smem = (size_t)BulkSmem<WS>::FIXED + (size_t)(tl.NP + nslot) * tl.S;
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    const int grid = (int)(tl.ntiles < num_sms() ? tl.ntiles : num_sms());
+    k<<<grid, kThreadsB, smem, s>>>(g, tl, nslot, (const uint16_t*)x, (const uint16_t*)T, (uint16_t*)y, reverse ? 1 : 0);
+    return cudaGetLastError();
+}
+
 template <int WS>
 size_t generic_smem(const TcTiles& tl)
 {
@@ -351,8 +641,17 @@ cudaError_t tc_forward(const Geom& g, int dtype, const void* x, const void* T, v
     if (!tc_tiles(g, &tl)) return cudaErrorNotSupported;
     if (tl.ntiles == 0) return cudaSuccess;
     *launches += 1;
-    *path = WBMM_PATH_TC_GATHER;
     const bool bf = dtype == WBMM_DTYPE_BF16;
+    const bool bulk = g.w == 7 ? bulk_ok<7>(g, tl, x, y) : bulk_ok<14>(g, tl, x, y);
+    if (bulk) {
+        *path = WBMM_PATH_TC_TMA;
+        if (g.w == 7)
+            return bf ? launch_bulk<7, true>(g, tl, x, T, y, reverse, stream)
+                      : launch_bulk<7, false>(g, tl, x, T, y, reverse, stream);
+        return bf ? launch_bulk<14, true>(g, tl, x, T, y, reverse, stream)
+                  : launch_bulk<14, false>(g, tl, x, T, y, reverse, stream);
+    }
+    *path = WBMM_PATH_TC_GATHER;
     if (g.w == 7)
         return bf ? launch_generic<7, true>(g, tl, x, T, y, reverse, stream)
                   : launch_generic<7, false>(g, tl, x, T, y, reverse, stream);
