@@ -141,23 +141,24 @@ __device__ __forceinline__ void window_to_tmem(const uint8_t* win, bool valid, i
     ptx::tmem_wait_st();
 }
 
-// TMEM D -> rounded 16-bit values in the window's frame position.
+// TMEM D -> rounded 16-bit values in the window's frame position (32 columns per wait).
 template <int WS, bool BF16>
 __device__ __forceinline__ void tmem_to_window(uint8_t* win, bool valid, int rowB, uint32_t taddr)
 {
     using Cf = WinCfg<WS>;
+    constexpr int NCH = (Cf::NW + 7) / 8;     // 16-column chunks that hold real outputs
 #pragma unroll
-    for (int ch = 0; ch < Cf::N_PAD / 16; ++ch) {
-        if (ch * 8 < Cf::NW) {
-            uint32_t v[16];
-            ptx::tmem_ld16(taddr + ch * 16, v);
-            ptx::tmem_wait_ld();
-            if (valid) {
+    for (int ch = 0; ch < NCH; ch += 2) {
+        uint32_t v[32];
+        ptx::tmem_ld16(taddr + ch * 16, v);
+        if (ch + 1 < NCH) ptx::tmem_ld16(taddr + (ch + 1) * 16, v + 16);
+        ptx::tmem_wait_ld();
+        if (valid) {
 #pragma unroll
-                for (int e = 0; e < 8; ++e) {
-                    const int wi = ch * 8 + e;
-                    if (wi < Cf::NW) store_word<WS>(win, rowB, wi, pack2<BF16>(v[2 * e], v[2 * e + 1]));
-                }
+            for (int e = 0; e < 16; ++e) {
+                const int wi = ch * 8 + e;
+                if (wi < Cf::NW && (e < 8 || ch + 1 < NCH))
+                    store_word<WS>(win, rowB, wi, pack2<BF16>(v[2 * e], v[2 * e + 1]));
             }
         }
     }
@@ -286,27 +287,52 @@ tc_generic_kernel(Geom g, TcTiles tl, const uint16_t* __restrict__ x, const uint
 //   warp 0      producer   bulk loads  x -> ring of frame-image slots            (full/empty barriers)
 //   warp 1      MMA        KSTEPS tcgen05.mma per tile, A from TMEM, B = W_c     (a_full/a_empty, d_full/d_empty)
 //   warps 2-5   repack     slot -> registers -> tcgen05.st into A[buf] (2 buffers); build W_c on a channel change
-//   warps 6-9   epilogue   tcgen05.ld D -> RNE 16-bit -> output frame -> bulk stores to y
+//   warps 6-9   epilogue   tcgen05.ld D -> RNE 16-bit -> output frame                     (out_full/out_empty)
+//   warp 10     store      bulk stores output frame -> y
 //
 // Each 32-bit shared-memory access of the repack / epilogue warps is conflict-free for the
 // headline geometry: lanes are (4 adjacent windows) x (8 images) and the image stride is 16*odd bytes.
 int num_sms();
-constexpr int kThreadsB = 320;
+constexpr int kThreadsB = 352;
 constexpr int kMaxSlots = 64;
+
+
+#ifdef WBMM_TRACE
+// Debug build only: per-tile event timestamps of block 0 (read back with wbmm_debug_trace()).
+__device__ long long g_trace[16 * 16];
+#define TRACE(ev, lt) do { if (blockIdx.x == 1 && (lt) < 16) g_trace[(lt) * 16 + (ev)] = clock64(); } while (0)
+#else
+#define TRACE(ev, lt) do { } while (0)
+#endif
 
 // W_c for w = 14 from two copies of the fully reversed table F[q] = T[NB-1-q] (F0 = F, F1 = F
 // shifted by one value), so that any pair (F[q], F[q+1]) is one aligned 32-bit load.  Row i of W_c
 // is, for every input row rj, the run F[q0 + 27*rj + cj], cj = 0..13, q0 = (13-ri)*27 + 13-ci
 // (Eq. 7 rewritten for the reversed table).  128 threads (the repack warps); rows >= N and chunk
 // 25 stay zero from the kernel prologue.
-__device__ __forceinline__ void build_weight14(const uint16_t* __restrict__ Tc, bool reverse, uint16_t* F0,
-                                               uint16_t* F1, uint8_t* Wc, int tid)
+constexpr int kTabRegs = (WinCfg<14>::NB + 127) / 128;
+
+// The (reversed) table row of one channel, 128 threads -> registers (loads only; no use yet).
+__device__ __forceinline__ void table_to_regs14(const uint16_t* __restrict__ Tc, bool reverse, int tid, uint16_t* v)
 {
     using Cf = WinCfg<14>;
-    for (int q = tid; q < Cf::NB; q += 128) {
-        const uint16_t v = Tc[reverse ? q : Cf::NB - 1 - q];
-        F0[q] = v;
-        if (q >= 1) F1[q - 1] = v;
+#pragma unroll
+    for (int u = 0; u < kTabRegs; ++u) {
+        const int q = tid + u * 128;
+        v[u] = q < Cf::NB ? Tc[reverse ? q : Cf::NB - 1 - q] : (uint16_t)0;
+    }
+}
+
+__device__ __forceinline__ void build_weight14(const uint16_t* v, uint16_t* F0, uint16_t* F1, uint8_t* Wc, int tid)
+{
+    using Cf = WinCfg<14>;
+#pragma unroll
+    for (int u = 0; u < kTabRegs; ++u) {
+        const int q = tid + u * 128;
+        if (q < Cf::NB) {
+            F0[q] = v[u];
+            if (q >= 1) F1[q - 1] = v[u];
+        }
     }
     ptx::named_bar_sync(2, 128);
     for (int i = tid; i < Cf::N; i += 128) {
@@ -315,18 +341,25 @@ __device__ __forceinline__ void build_weight14(const uint16_t* __restrict__ Tc, 
         const uint8_t* be = reinterpret_cast<const uint8_t*>(p0 ? F1 : F0) + (q0 - p0) * 2;   // even rj
         const uint8_t* bo = reinterpret_cast<const uint8_t*>(p0 ? F0 : F1) + (q0 + p0) * 2;   // odd rj
         uint8_t* dst = Wc + i * 16;
+        constexpr int BATCH = 9;     // chunks whose loads are all issued before the first store
 #pragma unroll
-        for (int kc = 0; kc < 25; ++kc) {
-            uint32_t pk[4];
+        for (int k0 = 0; k0 < 25; k0 += BATCH) {
+            uint32_t pk[BATCH][4];
 #pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                const int j = kc * 8 + 2 * e;
-                const int rj = j / 14, cj = j % 14;
-                if (j >= Cf::N) pk[e] = 0u;
-                else if (rj % 2 == 0) pk[e] = *reinterpret_cast<const uint32_t*>(be + (27 * rj + cj) * 2);
-                else pk[e] = *reinterpret_cast<const uint32_t*>(bo + (27 * rj - 1 + cj) * 2);
+            for (int kb = 0; kb < BATCH; ++kb) {
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const int j = (k0 + kb) * 8 + 2 * e;
+                    const int rj = j / 14, cj = j % 14;
+                    if (k0 + kb >= 25 || j >= Cf::N) pk[kb][e] = 0u;
+                    else if (rj % 2 == 0) pk[kb][e] = *reinterpret_cast<const uint32_t*>(be + (27 * rj + cj) * 2);
+                    else pk[kb][e] = *reinterpret_cast<const uint32_t*>(bo + (27 * rj - 1 + cj) * 2);
+                }
             }
-            *reinterpret_cast<uint4*>(dst + kc * Cf::LBO) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+#pragma unroll
+            for (int kb = 0; kb < BATCH; ++kb)
+                if (k0 + kb < 25)
+                    *reinterpret_cast<uint4*>(dst + (k0 + kb) * Cf::LBO) = make_uint4(pk[kb][0], pk[kb][1], pk[kb][2], pk[kb][3]);
         }
     }
 }
@@ -336,7 +369,7 @@ struct BulkSmem {
     using Cf = WinCfg<WS>;
     static constexpr int TAB_ONE = ((Cf::NB + 2) * 2 + 15) / 16 * 16;
     static constexpr int TAB_BYTES = 2 * TAB_ONE;                              // F0 and F1 (or Ts for the generic builder)
-    static constexpr int BAR_BYTES = (2 * kMaxSlots + 8) * 8;
+    static constexpr int BAR_BYTES = (2 * kMaxSlots + 10) * 8;
     static constexpr int FIXED = Cf::WC_BYTES + TAB_BYTES + BAR_BYTES;
 };
 
@@ -351,15 +384,16 @@ tc_bulk_kernel(Geom g, TcTiles tl, int nslot, const uint16_t* __restrict__ x, co
     uint8_t* Wc = smem;
     uint16_t* tab = reinterpret_cast<uint16_t*>(smem + Cf::WC_BYTES);
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + Cf::WC_BYTES + Sm::TAB_BYTES);
-    uint8_t* outf = smem + Sm::FIXED;
-    uint8_t* ring = outf + tl.NP * tl.S;
+    uint8_t* outf = smem + Sm::FIXED;            // output frame: NP image slots
+    uint8_t* ring = outf + tl.NP * tl.S;         // input ring: nslot image slots
     __shared__ uint32_t tmem_base_s;
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const uint32_t bar0 = ptx::smem_u32(bars);
     auto FULL = [&](int s) { return bar0 + 8u * s; };
     auto EMPTY = [&](int s) { return bar0 + 8u * (kMaxSlots + s); };
-    const uint32_t A_FULL = bar0 + 8u * (2 * kMaxSlots), A_EMPTY = A_FULL + 16, D_FULL = A_FULL + 32, D_EMPTY = A_FULL + 40;
+    const uint32_t A_FULL = bar0 + 8u * (2 * kMaxSlots), A_EMPTY = A_FULL + 16, D_FULL = A_FULL + 32, D_EMPTY = A_FULL + 40,
+                   OUT_FULL = A_FULL + 48, OUT_EMPTY = A_FULL + 64;
 
     const int wpf = tl.NSY * g.nww;   // windows per frame image
     if (warp == 0) ptx::tmem_alloc(ptx::smem_u32(&tmem_base_s), 512);
@@ -374,6 +408,9 @@ tc_bulk_kernel(Geom g, TcTiles tl, int nslot, const uint16_t* __restrict__ x, co
         ptx::mbar_init(A_EMPTY + 8, 1);
         ptx::mbar_init(D_FULL, 1);
         ptx::mbar_init(D_EMPTY, 128);
+        ptx::mbar_init(OUT_FULL, 128);
+        ptx::mbar_init(OUT_FULL + 8, 128);
+        ptx::mbar_init(OUT_EMPTY, 1);
         ptx::fence_mbar_init();
     }
     for (int i = tid; i < Cf::WC_BYTES / 16; i += kThreadsB) reinterpret_cast<uint4*>(Wc)[i] = make_uint4(0, 0, 0, 0);
@@ -413,6 +450,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, int nslot, const uint16_t* __restrict__ x, co
                     const int slot = k % nslot;
                     ptx::mbar_wait(EMPTY(slot), ((k / nslot) & 1) ^ 1);
                     ptx::mbar_arrive_expect_tx(FULL(slot), bytes);
+                    if (p == 0) TRACE(0, (t - t0));
                     const uint16_t* src = x + ((long long)(b0 + p) * g.C + c) * plane_elems + (long long)wy0 * WS * g.W;
                     ptx::bulk_g2s(ptx::smem_u32(ring + (size_t)slot * tl.S), src, bytes, FULL(slot));
                 }
@@ -427,7 +465,9 @@ tc_bulk_kernel(Geom g, TcTiles tl, int nslot, const uint16_t* __restrict__ x, co
             for (long long t = t0; t < t1; ++t, ++lt) {
                 const uint32_t buf = lt & 1;
                 ptx::mbar_wait(A_FULL + 8 * buf, (lt >> 1) & 1);
+                TRACE(1, lt);
                 ptx::mbar_wait(D_EMPTY, (lt & 1) ^ 1);
+                TRACE(2, lt);
                 ptx::tc_fence_after_sync();
                 const uint32_t tmem_a = tmem + buf * A_STRIDE;
 #pragma unroll
@@ -437,6 +477,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, int nslot, const uint16_t* __restrict__ x, co
                 }
                 ptx::mma_commit(A_EMPTY + 8 * buf);
                 ptx::mma_commit(D_FULL);
+                TRACE(3, lt);
             }
         }
     } else if (warp < 6) {
@@ -449,16 +490,22 @@ tc_bulk_kernel(Geom g, TcTiles tl, int nslot, const uint16_t* __restrict__ x, co
         const int win_off = ((wyl * WS) * g.W + wx * WS) * 2;
         uint32_t k = 0, lt = 0;
         int cur_c = -1;
+        uint16_t tabv[kTabRegs];
+        bool tabv_ready = false;
         for (long long t = t0; t < t1; ++t, ++lt) {
             int c, b0, wy0, np_eff, rows_eff;
             tile_decode(t, c, b0, wy0, np_eff, rows_eff);
             const uint32_t buf = lt & 1;
             ptx::mbar_wait(A_EMPTY + 8 * buf, ((lt >> 1) & 1) ^ 1);   // MMA(lt-2) has consumed A[buf]
+            if (rt == 0) TRACE(4, lt);
             if (c != cur_c) {
                 if (lt > 0) ptx::mbar_wait(A_EMPTY + 8 * ((lt - 1) & 1), ((lt - 1) >> 1) & 1);   // MMA(lt-1) done with W_c
                 const uint16_t* Tc = T + (long long)c * Cf::NB;
+                if (rt == 0) TRACE(12, lt);
                 if constexpr (WS == 14) {
-                    build_weight14(Tc, reverse != 0, tab, tab + Sm::TAB_ONE / 2, Wc, rt);
+                    if (!tabv_ready) table_to_regs14(Tc, reverse != 0, rt, tabv);
+                    build_weight14(tabv, tab, tab + Sm::TAB_ONE / 2, Wc, rt);
+                    tabv_ready = false;
                 } else {
                     for (int kk = rt; kk < Cf::NB; kk += 128) tab[kk] = Tc[reverse ? Cf::NB - 1 - kk : kk];
                     ptx::named_bar_sync(2, 128);
@@ -484,23 +531,32 @@ tc_bulk_kernel(Geom g, TcTiles tl, int nslot, const uint16_t* __restrict__ x, co
                 ptx::fence_proxy_async_smem();
                 cur_c = c;
             }
+            if constexpr (WS == 14) {
+                // the next tile starts a new channel: have its table row in flight during this repack
+                if (t + 1 < t1 && (int)((t + 1) / tl.tiles_per_c) != c) {
+                    table_to_regs14(T + (long long)(c + 1) * Cf::NB, reverse != 0, rt, tabv);
+                    tabv_ready = true;
+                }
+            }
             const bool part = wl < wpf && pl < np_eff;               // this thread's frame image was loaded
             const bool valid = part && wy0 + wyl < g.nwh;
             const uint32_t kk = k + pl;
             const int slot = kk % nslot;
+            if (rt == 0) TRACE(5, lt);
             if (part) ptx::mbar_wait(FULL(slot), (kk / nslot) & 1);
+            if (rt == 0) TRACE(6, lt);
             window_to_tmem<WS>(ring + (size_t)slot * tl.S + win_off, valid, rowB,
                                tmem + buf * A_STRIDE + ((uint32_t)(q * 32) << 16));
             ptx::tc_fence_before_sync();
             ptx::mbar_arrive(A_FULL + 8 * buf);
-            if (part) ptx::mbar_arrive(EMPTY(slot));
+            if (part) ptx::mbar_arrive(EMPTY(slot));   // every window of this image is in TMEM
+            if (rt == 0) TRACE(7, lt);
             k += np_eff;
         }
-    } else {
+    } else if (warp < 10) {
         // ------------------------------------------------------------------ epilogue
         const int q = warp & 3;
         const int m = q * 32 + lane;
-        const int et = (warp - 6) * 32 + lane;   // 0..127 among the epilogue threads
         const int wl = m / tl.NP, pl = m % tl.NP;
         const int wyl = wl / g.nww, wx = wl % g.nww;
         uint8_t* win = outf + pl * tl.S + ((wyl * WS) * g.W + wx * WS) * 2;
@@ -510,24 +566,44 @@ tc_bulk_kernel(Geom g, TcTiles tl, int nslot, const uint16_t* __restrict__ x, co
             tile_decode(t, c, b0, wy0, np_eff, rows_eff);
             const bool valid = wl < wpf && pl < np_eff && wy0 + wyl < g.nwh;
             ptx::mbar_wait(D_FULL, lt & 1);
+            if (m == 0) TRACE(8, lt);
+            ptx::mbar_wait(OUT_EMPTY, (lt & 1) ^ 1);     // the previous tile's stores have left the output frame
             ptx::tc_fence_after_sync();
-            if (et == 0) ptx::bulk_wait_read<0>();     // the previous tile's stores have left the output frame
-            ptx::named_bar_sync(1, 128);
             tmem_to_window<WS, BF16>(win, valid, rowB, tmem_d + ((uint32_t)(q * 32) << 16));
             ptx::tc_fence_before_sync();
             ptx::mbar_arrive(D_EMPTY);
             ptx::fence_proxy_async_smem();
-            ptx::named_bar_sync(1, 128);
-            if (et == 0) {
+            ptx::mbar_arrive(OUT_FULL + 8 * (lt & 1));
+            if (m == 0) TRACE(9, lt);
+        }
+    } else {
+        // ------------------------------------------------------------------ store
+        if (lane > 0 && t1 > t0) {   // idle lanes: pull this CTA's table rows into L2 ahead of the W_c builds
+            const int c_first = (int)(t0 / tl.tiles_per_c), c_last = (int)((t1 - 1) / tl.tiles_per_c);
+            const char* base = reinterpret_cast<const char*>(T + (long long)c_first * Cf::NB);
+            const long long nbytes = (long long)(c_last - c_first + 1) * Cf::NB * 2;
+            for (long long off = (lane - 1) * 128ll; off < nbytes; off += 31 * 128)
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(base + off));
+        }
+        if (lane == 0) {
+            uint32_t lt = 0;
+            for (long long t = t0; t < t1; ++t, ++lt) {
+                int c, b0, wy0, np_eff, rows_eff;
+                tile_decode(t, c, b0, wy0, np_eff, rows_eff);
                 const uint32_t bytes = (uint32_t)rows_eff * rowB;
+                ptx::mbar_wait(OUT_FULL + 8 * (lt & 1), (lt >> 1) & 1);
+                TRACE(10, lt);
                 for (int p = 0; p < np_eff; ++p) {
                     uint16_t* dst = y + ((long long)(b0 + p) * g.C + c) * plane_elems + (long long)wy0 * WS * g.W;
                     ptx::bulk_s2g(dst, ptx::smem_u32(outf + p * tl.S), bytes);
                 }
                 ptx::bulk_commit();
+                ptx::bulk_wait_read<0>();
+                TRACE(11, lt);
+                ptx::mbar_arrive(OUT_EMPTY);
             }
+            ptx::bulk_wait_all<0>();
         }
-        if (et == 0) ptx::bulk_wait_all<0>();
     }
     ptx::tc_fence_before_sync();
     __syncthreads();
@@ -539,7 +615,7 @@ int bulk_slots(const TcTiles& tl)
 {
     const long long room = 227ll * 1024 - 1024 - BulkSmem<WS>::FIXED - (long long)tl.NP * tl.S;
     long long n = room / tl.S;
-    if (n > 2 * tl.NP) n = 2 * tl.NP;
+    if (n > 3 * tl.NP) n = 3 * tl.NP;
     if (n > kMaxSlots) n = kMaxSlots;
     return (int)n;
 }
@@ -665,5 +741,12 @@ cudaError_t tc_grad_table(const Geom&, int, const void*, const void*, float*, cu
     return cudaErrorNotSupported;
 }
 void tc_release() {}
+
+#ifdef WBMM_TRACE
+extern "C" __attribute__((visibility("default"))) int wbmm_debug_trace(long long* out)
+{
+    return (int)cudaMemcpyFromSymbol(out, g_trace, sizeof(long long) * 256);
+}
+#endif
 
 }  // namespace wbmm
