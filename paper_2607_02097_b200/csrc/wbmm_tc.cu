@@ -12,6 +12,8 @@
 //     l.17) are pure address arithmetic.
 #include "wbmm_tc.cuh"
 
+#include <mutex>
+
 #include "wbmm_ptx.cuh"
 
 namespace wbmm {
@@ -207,7 +209,7 @@ tc_generic_kernel(Geom g, TcTiles tl, const uint16_t* __restrict__ x, const uint
     const int wyl = wl / g.nww, wx = wl % g.nww;
     uint8_t* win = frame + pl * tl.S + ((wyl * WS) * g.Wp + wx * WS) * 2;
 
-    for (long long t = t0; t < t1; ++t) {
+    for (int t = t0; t < t1; ++t) {
         const int c = (int)(t / tl.tiles_per_c);
         const int rem = (int)(t % tl.tiles_per_c);
         const int gb = rem / tl.nstrips, strip = rem % tl.nstrips;
@@ -295,11 +297,20 @@ tc_generic_kernel(Geom g, TcTiles tl, const uint16_t* __restrict__ x, const uint
 int num_sms();
 constexpr int kThreadsB = 352;
 constexpr int kMaxSlots = 64;
+constexpr int kMaxGrid = 160;
+
+// Static tile schedule: CTA b owns tiles [start[b], start[b+1]) (channel-major, so W_c is rebuilt
+// at most once or twice per CTA).  The host balances tiles + the cost of mid-range W_c rebuilds.
+struct TilePart {
+    int start[kMaxGrid + 1];
+};
 
 
 #ifdef WBMM_TRACE
 // Debug build only: per-tile event timestamps of block 0 (read back with wbmm_debug_trace()).
 __device__ long long g_trace[16 * 16];
+__device__ long long g_blk[148 * 4];
+__device__ __forceinline__ long long gtime() { long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
 #define TRACE(ev, lt) do { if (blockIdx.x == 1 && (lt) < 16) g_trace[(lt) * 16 + (ev)] = clock64(); } while (0)
 #else
 #define TRACE(ev, lt) do { } while (0)
@@ -375,7 +386,7 @@ struct BulkSmem {
 
 template <int WS, bool BF16>
 __global__ void __launch_bounds__(kThreadsB, 1)
-tc_bulk_kernel(Geom g, TcTiles tl, int nslot, const uint16_t* __restrict__ x, const uint16_t* __restrict__ T,
+tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __restrict__ x, const uint16_t* __restrict__ T,
                uint16_t* __restrict__ y, int reverse)
 {
     using Cf = WinCfg<WS>;
@@ -389,6 +400,9 @@ tc_bulk_kernel(Geom g, TcTiles tl, int nslot, const uint16_t* __restrict__ x, co
     __shared__ uint32_t tmem_base_s;
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+#ifdef WBMM_TRACE
+    if (tid == 0 && blockIdx.x < 148) { g_blk[blockIdx.x * 4] = gtime(); unsigned sm; asm("mov.u32 %0, %smid;" : "=r"(sm)); g_blk[blockIdx.x * 4 + 3] = sm; }
+#endif
     const uint32_t bar0 = ptx::smem_u32(bars);
     auto FULL = [&](int s) { return bar0 + 8u * s; };
     auto EMPTY = [&](int s) { return bar0 + 8u * (kMaxSlots + s); };
@@ -396,8 +410,8 @@ tc_bulk_kernel(Geom g, TcTiles tl, int nslot, const uint16_t* __restrict__ x, co
                    OUT_FULL = A_FULL + 48, OUT_EMPTY = A_FULL + 64;
 
     const int wpf = tl.NSY * g.nww;   // windows per frame image
-    if (warp == 0) ptx::tmem_alloc(ptx::smem_u32(&tmem_base_s), 512);
-    if (tid == 32) {
+    if (warp == 1) ptx::tmem_alloc(ptx::smem_u32(&tmem_base_s), 512);
+    if (tid == 0) {
         for (int s = 0; s < nslot; ++s) {
             ptx::mbar_init(FULL(s), 1);
             ptx::mbar_init(EMPTY(s), wpf);
@@ -413,25 +427,35 @@ tc_bulk_kernel(Geom g, TcTiles tl, int nslot, const uint16_t* __restrict__ x, co
         ptx::mbar_init(OUT_EMPTY, 1);
         ptx::fence_mbar_init();
     }
-    for (int i = tid; i < Cf::WC_BYTES / 16; i += kThreadsB) reinterpret_cast<uint4*>(Wc)[i] = make_uint4(0, 0, 0, 0);
+    if constexpr (WS == 14) {
+        // build_weight14 writes rows < N of chunks 0..24 only: zero the padding rows and the last chunk once
+        constexpr int PADR = Cf::N_PAD - Cf::N;
+        for (int i = tid; i < PADR * 25 + Cf::N_PAD; i += kThreadsB) {
+            const int kc = i < PADR * 25 ? i / PADR : 25, row = i < PADR * 25 ? Cf::N + i % PADR : i - PADR * 25;
+            *reinterpret_cast<uint4*>(Wc + kc * Cf::LBO + row * 16) = make_uint4(0, 0, 0, 0);
+        }
+    }
     for (int i = tid; i < Sm::TAB_BYTES / 4; i += kThreadsB) reinterpret_cast<uint32_t*>(tab)[i] = 0u;
     ptx::fence_proxy_async_smem();
     ptx::tc_fence_before_sync();
     __syncthreads();
     ptx::tc_fence_after_sync();
+#ifdef WBMM_TRACE
+    if (tid == 0 && blockIdx.x < 148) g_blk[blockIdx.x * 4 + 1] = gtime();
+#endif
     const uint32_t tmem = tmem_base_s;
     constexpr uint32_t A_STRIDE = (Cf::A_COLS + 31) / 32 * 32;
     const uint32_t tmem_d = tmem + 2 * A_STRIDE;
     static_assert(2 * ((Cf::A_COLS + 31) / 32 * 32) + Cf::N_PAD <= 512, "TMEM budget");
 
-    const long long t0 = tl.ntiles * blockIdx.x / gridDim.x, t1 = tl.ntiles * (blockIdx.x + 1) / gridDim.x;
+    const int t0 = part_.start[blockIdx.x], t1 = part_.start[blockIdx.x + 1];
     const int rowB = g.W * 2;
     const long long plane_elems = (long long)g.H * g.W;
 
-    auto tile_decode = [&](long long t, int& c, int& b0, int& wy0, int& np_eff, int& rows_eff) {
-        c = (int)(t / tl.tiles_per_c);
-        const int rem = (int)(t % tl.tiles_per_c);
-        const int gb = rem / tl.nstrips, strip = rem % tl.nstrips;
+    auto tile_decode = [&](int t, int& c, int& b0, int& wy0, int& np_eff, int& rows_eff) {
+        c = t / tl.tiles_per_c;
+        const int rem = t - c * tl.tiles_per_c;
+        const int gb = rem / tl.nstrips, strip = rem - gb * tl.nstrips;
         b0 = gb * tl.NP;
         wy0 = strip * tl.NSY;
         np_eff = min(tl.NP, g.B - b0);
@@ -442,7 +466,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, int nslot, const uint16_t* __restrict__ x, co
         // ------------------------------------------------------------------ producer
         if (lane == 0) {
             uint32_t k = 0;
-            for (long long t = t0; t < t1; ++t) {
+            for (int t = t0; t < t1; ++t) {
                 int c, b0, wy0, np_eff, rows_eff;
                 tile_decode(t, c, b0, wy0, np_eff, rows_eff);
                 const uint32_t bytes = (uint32_t)rows_eff * rowB;
@@ -462,7 +486,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, int nslot, const uint16_t* __restrict__ x, co
             constexpr uint32_t idesc = ptx::idesc_f16(BF16 ? 1 : 0, 128, Cf::N_PAD);
             const uint32_t wc_addr = ptx::smem_u32(Wc);
             uint32_t lt = 0;
-            for (long long t = t0; t < t1; ++t, ++lt) {
+            for (int t = t0; t < t1; ++t, ++lt) {
                 const uint32_t buf = lt & 1;
                 ptx::mbar_wait(A_FULL + 8 * buf, (lt >> 1) & 1);
                 TRACE(1, lt);
@@ -492,7 +516,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, int nslot, const uint16_t* __restrict__ x, co
         int cur_c = -1;
         uint16_t tabv[kTabRegs];
         bool tabv_ready = false;
-        for (long long t = t0; t < t1; ++t, ++lt) {
+        for (int t = t0; t < t1; ++t, ++lt) {
             int c, b0, wy0, np_eff, rows_eff;
             tile_decode(t, c, b0, wy0, np_eff, rows_eff);
             const uint32_t buf = lt & 1;
@@ -533,7 +557,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, int nslot, const uint16_t* __restrict__ x, co
             }
             if constexpr (WS == 14) {
                 // the next tile starts a new channel: have its table row in flight during this repack
-                if (t + 1 < t1 && (int)((t + 1) / tl.tiles_per_c) != c) {
+                if (t + 1 < t1 && (t + 1) - c * tl.tiles_per_c == tl.tiles_per_c) {
                     table_to_regs14(T + (long long)(c + 1) * Cf::NB, reverse != 0, rt, tabv);
                     tabv_ready = true;
                 }
@@ -561,7 +585,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, int nslot, const uint16_t* __restrict__ x, co
         const int wyl = wl / g.nww, wx = wl % g.nww;
         uint8_t* win = outf + pl * tl.S + ((wyl * WS) * g.W + wx * WS) * 2;
         uint32_t lt = 0;
-        for (long long t = t0; t < t1; ++t, ++lt) {
+        for (int t = t0; t < t1; ++t, ++lt) {
             int c, b0, wy0, np_eff, rows_eff;
             tile_decode(t, c, b0, wy0, np_eff, rows_eff);
             const bool valid = wl < wpf && pl < np_eff && wy0 + wyl < g.nwh;
@@ -579,7 +603,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, int nslot, const uint16_t* __restrict__ x, co
     } else {
         // ------------------------------------------------------------------ store
         if (lane > 0 && t1 > t0) {   // idle lanes: pull this CTA's table rows into L2 ahead of the W_c builds
-            const int c_first = (int)(t0 / tl.tiles_per_c), c_last = (int)((t1 - 1) / tl.tiles_per_c);
+            const int c_first = t0 / tl.tiles_per_c, c_last = (t1 - 1) / tl.tiles_per_c;
             const char* base = reinterpret_cast<const char*>(T + (long long)c_first * Cf::NB);
             const long long nbytes = (long long)(c_last - c_first + 1) * Cf::NB * 2;
             for (long long off = (lane - 1) * 128ll; off < nbytes; off += 31 * 128)
@@ -587,7 +611,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, int nslot, const uint16_t* __restrict__ x, co
         }
         if (lane == 0) {
             uint32_t lt = 0;
-            for (long long t = t0; t < t1; ++t, ++lt) {
+            for (int t = t0; t < t1; ++t, ++lt) {
                 int c, b0, wy0, np_eff, rows_eff;
                 tile_decode(t, c, b0, wy0, np_eff, rows_eff);
                 const uint32_t bytes = (uint32_t)rows_eff * rowB;
@@ -607,7 +631,10 @@ tc_bulk_kernel(Geom g, TcTiles tl, int nslot, const uint16_t* __restrict__ x, co
     }
     ptx::tc_fence_before_sync();
     __syncthreads();
-    if (warp == 0) ptx::tmem_dealloc(tmem, 512);
+    if (warp == 1) ptx::tmem_dealloc(tmem, 512);
+#ifdef WBMM_TRACE
+    if (tid == 0 && blockIdx.x < 148) g_blk[blockIdx.x * 4 + 2] = gtime();
+#endif
 }
 
 template <int WS>
@@ -626,8 +653,43 @@ bool bulk_ok(const Geom& g, const TcTiles& tl, const void* x, const void* y)
     if (g.layout != WBMM_LAYOUT_NCHW || g.sh != 0 || g.sw != 0 || g.H != g.Hp || g.W != g.Wp) return false;
     if ((tl.frame_rows * g.W * 2) % 16 != 0 || ((long long)g.H * g.W * 2) % 16 != 0) return false;
     if (reinterpret_cast<uintptr_t>(x) % 16 != 0 || reinterpret_cast<uintptr_t>(y) % 16 != 0) return false;
-    if (tl.NP > kMaxSlots) return false;
+    if (tl.NP > kMaxSlots || tl.ntiles > 0x3fffffffll) return false;
     return bulk_slots<WS>(tl) >= tl.NP + 1;
+}
+
+// Greedy contiguous partition of the tile sequence over `grid` CTAs minimising the largest cost,
+// cost = tiles + kSwitchCost per channel boundary strictly inside a CTA's range.
+constexpr double kSwitchCost = 0.75;
+
+int partition_tiles(const TcTiles& tl, int grid, TilePart* part)
+{
+    const int n = (int)tl.ntiles, tpc = tl.tiles_per_c;
+    auto fill = [&](double cap, TilePart* out) {
+        int b = 0, t = 0;
+        if (out) out->start[0] = 0;
+        while (t < n) {
+            double cost = 0;
+            int first = t;
+            while (t < n) {
+                const double add = 1.0 + ((t > first && t % tpc == 0) ? kSwitchCost : 0.0);
+                if (cost + add > cap + 1e-9 && t > first) break;
+                cost += add;
+                ++t;
+            }
+            ++b;
+            if (out && b <= kMaxGrid) out->start[b] = t;
+            if (b > grid) return b;
+        }
+        return b;
+    };
+    double lo = (double)n / grid, hi = (double)n / grid * 2 + 4;
+    for (int it = 0; it < 40; ++it) {
+        const double mid = 0.5 * (lo + hi);
+        if (fill(mid, nullptr) <= grid) hi = mid; else lo = mid;
+    }
+    const int used = fill(hi, part);
+    for (int b = used; b < kMaxGrid; ++b) part->start[b + 1] = n;
+    return used;
 }
 
 template <int WS, bool BF16>
@@ -639,8 +701,24 @@ cudaError_t launch_bulk(const Geom& g, const TcTiles& tl, const void* x, const v
     const size_t smem = (size_t)BulkSmem<WS>::FIXED + (size_t)(tl.NP + nslot) * tl.S;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    const int grid = (int)(tl.ntiles < num_sms() ? tl.ntiles : num_sms());
-    k<<<grid, kThreadsB, smem, s>>>(g, tl, nslot, (const uint16_t*)x, (const uint16_t*)T, (uint16_t*)y, reverse ? 1 : 0);
+    int grid = (int)(tl.ntiles < num_sms() ? tl.ntiles : num_sms());
+    if (grid > kMaxGrid) grid = kMaxGrid;
+    // the schedule depends on (tiles, tiles per channel, grid) only: keep the last one
+    static std::mutex mu;
+    static TilePart cached;
+    static long long key_n = -1;
+    static int key_tpc = -1, key_grid = -1, cached_used = 0;
+    TilePart part;
+    {
+        std::lock_guard<std::mutex> lock(mu);
+        if (key_n != tl.ntiles || key_tpc != tl.tiles_per_c || key_grid != grid) {
+            cached_used = partition_tiles(tl, grid, &cached);
+            key_n = tl.ntiles; key_tpc = tl.tiles_per_c; key_grid = grid;
+        }
+        part = cached;
+        grid = cached_used;
+    }
+    k<<<grid, kThreadsB, smem, s>>>(g, tl, part, nslot, (const uint16_t*)x, (const uint16_t*)T, (uint16_t*)y, reverse ? 1 : 0);
     return cudaGetLastError();
 }
 
@@ -746,6 +824,10 @@ void tc_release() {}
 extern "C" __attribute__((visibility("default"))) int wbmm_debug_trace(long long* out)
 {
     return (int)cudaMemcpyFromSymbol(out, g_trace, sizeof(long long) * 256);
+}
+extern "C" __attribute__((visibility("default"))) int wbmm_debug_blocks(long long* out)
+{
+    return (int)cudaMemcpyFromSymbol(out, g_blk, sizeof(long long) * 148 * 4);
 }
 #endif
 
