@@ -310,8 +310,8 @@ struct TilePart {
 // Debug build only: per-tile event timestamps of block 0 (read back with wbmm_debug_trace()).
 __device__ long long g_trace[16 * 16];
 __device__ long long g_blk[148 * 4];
-__device__ __forceinline__ long long gtime() { long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
-#define TRACE(ev, lt) do { if (blockIdx.x == 1 && (lt) < 16) g_trace[(lt) * 16 + (ev)] = clock64(); } while (0)
+__device__ __forceinline__ long long gtime() { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
+#define TRACE(ev, lt) do { if (blockIdx.x == 1 && (lt) < 16) g_trace[(lt) * 16 + (ev)] = gtime(); } while (0)
 #else
 #define TRACE(ev, lt) do { } while (0)
 #endif
@@ -410,12 +410,14 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __
                    OUT_FULL = A_FULL + 48, OUT_EMPTY = A_FULL + 64;
 
     const int wpf = tl.NSY * g.nww;   // windows per frame image
-    if (warp == 1) ptx::tmem_alloc(ptx::smem_u32(&tmem_base_s), 512);
+    TRACE(0, 15);
+    if (warp == 1) { ptx::tmem_alloc(ptx::smem_u32(&tmem_base_s), 512); if (lane == 0) TRACE(1, 15); }
+    if (tid >= 64 && tid < 64 + nslot) {
+        ptx::mbar_init(FULL(tid - 64), 1);
+        ptx::mbar_init(EMPTY(tid - 64), wpf);
+        ptx::fence_mbar_init();
+    }
     if (tid == 0) {
-        for (int s = 0; s < nslot; ++s) {
-            ptx::mbar_init(FULL(s), 1);
-            ptx::mbar_init(EMPTY(s), wpf);
-        }
         ptx::mbar_init(A_FULL, 128);
         ptx::mbar_init(A_FULL + 8, 128);
         ptx::mbar_init(A_EMPTY, 1);
@@ -426,6 +428,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __
         ptx::mbar_init(OUT_FULL + 8, 128);
         ptx::mbar_init(OUT_EMPTY, 1);
         ptx::fence_mbar_init();
+        TRACE(2, 15);
     }
     if constexpr (WS == 14) {
         // build_weight14 writes rows < N of chunks 0..24 only: zero the padding rows and the last chunk once
@@ -438,8 +441,14 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __
     for (int i = tid; i < Sm::TAB_BYTES / 4; i += kThreadsB) reinterpret_cast<uint32_t*>(tab)[i] = 0u;
     ptx::fence_proxy_async_smem();
     ptx::tc_fence_before_sync();
+    if (tid == 64) TRACE(3, 15);
     __syncthreads();
+    if (tid == 64) TRACE(4, 15);
     ptx::tc_fence_after_sync();
+    // Programmatic dependent launch: everything above overlapped the previous kernel's tail; no
+    // global memory is touched before this point.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 #ifdef WBMM_TRACE
     if (tid == 0 && blockIdx.x < 148) g_blk[blockIdx.x * 4 + 1] = gtime();
 #endif
@@ -718,8 +727,18 @@ cudaError_t launch_bulk(const Geom& g, const TcTiles& tl, const void* x, const v
         part = cached;
         grid = cached_used;
     }
-    k<<<grid, kThreadsB, smem, s>>>(g, tl, part, nslot, (const uint16_t*)x, (const uint16_t*)T, (uint16_t*)y, reverse ? 1 : 0);
-    return cudaGetLastError();
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3(kThreadsB);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, k, g, tl, part, nslot, (const uint16_t*)x, (const uint16_t*)T, (uint16_t*)y,
+                              reverse ? 1 : 0);
 }
 
 template <int WS>
