@@ -166,6 +166,119 @@ __device__ __forceinline__ void tmem_to_window(uint8_t* win, bool valid, int row
     }
 }
 
+// General window addressing for whole-image frames held exactly as they sit in global memory
+// (row pitch W): the cyclic shift and the zero padding (Eq. 4-5; A6) become per-thread
+// row / column byte offsets plus validity bit masks (bit r / bit cc set = inside H x W).  Offsets
+// of padding rows / columns are clamped to 0 so every load address is legal; the value is masked.
+template <int WS>
+struct GenAddr {
+    int rowoff[WS], coloff[WS];
+    uint32_t rowmask, colmask;
+};
+
+template <int WS>
+__device__ __forceinline__ void gen_addr_init(GenAddr<WS>& a, const Geom& g, int wyl, int wx)
+{
+    a.rowmask = a.colmask = 0;
+#pragma unroll
+    for (int r = 0; r < WS; ++r) {
+        int h = wyl * WS + r + g.sh;
+        if (h >= g.Hp) h -= g.Hp;
+        a.rowoff[r] = h < g.H ? h * g.W * 2 : 0;
+        a.rowmask |= (h < g.H ? 1u : 0u) << r;
+    }
+#pragma unroll
+    for (int cc = 0; cc < WS; ++cc) {
+        int v = wx * WS + cc + g.sw;
+        if (v >= g.Wp) v -= g.Wp;
+        a.coloff[cc] = v < g.W ? v * 2 : 0;
+        a.colmask |= (v < g.W ? 1u : 0u) << cc;
+    }
+}
+
+// RAGGED = false: every window element lies inside H x W (no padding anywhere), masks unused.
+template <int WS, bool RAGGED>
+__device__ __forceinline__ uint32_t gen_load_word(const uint8_t* img, const GenAddr<WS>& a, uint32_t rm, int wi)
+{
+    const int e0 = 2 * wi, e1 = 2 * wi + 1;
+    uint32_t lo = *reinterpret_cast<const uint16_t*>(img + a.rowoff[e0 / WS] + a.coloff[e0 % WS]);
+    if (RAGGED && !((rm >> (e0 / WS)) & (a.colmask >> (e0 % WS)) & 1u)) lo = 0;
+    uint32_t hi = 0;
+    if (e1 < WS * WS) {
+        hi = *reinterpret_cast<const uint16_t*>(img + a.rowoff[e1 / WS] + a.coloff[e1 % WS]);
+        if (RAGGED && !((rm >> (e1 / WS)) & (a.colmask >> (e1 % WS)) & 1u)) hi = 0;
+    }
+    return lo | (hi << 16);
+}
+
+template <int WS, bool RAGGED>
+__device__ __forceinline__ void gen_store_word(uint8_t* img, const GenAddr<WS>& a, int wi, uint32_t v)
+{
+    const int e0 = 2 * wi, e1 = 2 * wi + 1;
+    if (!RAGGED || ((a.rowmask >> (e0 / WS)) & (a.colmask >> (e0 % WS)) & 1u))
+        *reinterpret_cast<uint16_t*>(img + a.rowoff[e0 / WS] + a.coloff[e0 % WS]) = (uint16_t)(v & 0xffffu);
+    if (e1 < WS * WS) {
+        if (!RAGGED || ((a.rowmask >> (e1 / WS)) & (a.colmask >> (e1 % WS)) & 1u))
+            *reinterpret_cast<uint16_t*>(img + a.rowoff[e1 / WS] + a.coloff[e1 % WS]) = (uint16_t)(v >> 16);
+    }
+}
+
+template <int WS, bool RAGGED>
+__device__ __forceinline__ void window_to_tmem_gen_t(const uint8_t* img, const GenAddr<WS>& a, uint32_t rm, uint32_t taddr)
+{
+    using Cf = WinCfg<WS>;
+#pragma unroll
+    for (int ch = 0; ch < (Cf::A_COLS + 15) / 16; ++ch) {
+        uint32_t v[16];
+#pragma unroll
+        for (int e = 0; e < 16; ++e) {
+            const int wi = ch * 16 + e;
+            v[e] = wi < Cf::NW ? gen_load_word<WS, RAGGED>(img, a, rm, wi) : 0u;
+        }
+        if (ch * 16 + 16 <= Cf::A_COLS) ptx::tmem_st16(taddr + ch * 16, v);
+        else ptx::tmem_st8(taddr + ch * 16, v);
+    }
+}
+
+// tcgen05.st is warp-collective: every lane runs the same instruction stream; a lane without a
+// window (or a ragged problem) takes the masked form, chosen warp-uniformly.
+template <int WS>
+__device__ __forceinline__ void window_to_tmem_gen(const uint8_t* img, const GenAddr<WS>& a, bool valid, bool ragged,
+                                                   uint32_t taddr)
+{
+    const bool masked = ragged || !__all_sync(0xffffffffu, valid);
+    if (masked) window_to_tmem_gen_t<WS, true>(img, a, valid ? a.rowmask : 0u, taddr);
+    else window_to_tmem_gen_t<WS, false>(img, a, 0u, taddr);
+    ptx::tmem_wait_st();
+}
+
+template <int WS, bool BF16, bool RAGGED>
+__device__ __forceinline__ void tmem_to_window_gen_t(uint8_t* img, const GenAddr<WS>& a, bool valid, uint32_t taddr)
+{
+    using Cf = WinCfg<WS>;
+    constexpr int NCH = (Cf::NW + 7) / 8;
+#pragma unroll
+    for (int ch = 0; ch < NCH; ++ch) {
+        uint32_t v[16];
+        ptx::tmem_ld16(taddr + ch * 16, v);
+        ptx::tmem_wait_ld();
+        if (valid) {
+#pragma unroll
+            for (int e = 0; e < 8; ++e) {
+                const int wi = ch * 8 + e;
+                if (wi < Cf::NW) gen_store_word<WS, RAGGED>(img, a, wi, pack2<BF16>(v[2 * e], v[2 * e + 1]));
+            }
+        }
+    }
+}
+
+template <int WS, bool BF16>
+__device__ __forceinline__ void tmem_to_window_gen(uint8_t* img, const GenAddr<WS>& a, bool valid, bool ragged, uint32_t taddr)
+{
+    if (ragged) tmem_to_window_gen_t<WS, BF16, true>(img, a, valid, taddr);
+    else tmem_to_window_gen_t<WS, BF16, false>(img, a, valid, taddr);
+}
+
 // ------------------------------------------------------------------------------------------------
 // Generic kernel ("tcgen05+gather"): any shift, ragged size, W and layout.  The frame is filled
 // and drained by plain predicated loads/stores (index arithmetic does padding, shift and layout),
@@ -352,7 +465,7 @@ __device__ __forceinline__ void build_weight14(const uint16_t* v, uint16_t* F0, 
         const uint8_t* be = reinterpret_cast<const uint8_t*>(p0 ? F1 : F0) + (q0 - p0) * 2;   // even rj
         const uint8_t* bo = reinterpret_cast<const uint8_t*>(p0 ? F0 : F1) + (q0 + p0) * 2;   // odd rj
         uint8_t* dst = Wc + i * 16;
-        constexpr int BATCH = 9;     // chunks whose loads are all issued before the first store
+        constexpr int BATCH = 5;     // chunks whose loads are all issued before the first store
 #pragma unroll
         for (int k0 = 0; k0 < 25; k0 += BATCH) {
             uint32_t pk[BATCH][4];
@@ -384,7 +497,7 @@ struct BulkSmem {
     static constexpr int FIXED = Cf::WC_BYTES + TAB_BYTES + BAR_BYTES;
 };
 
-template <int WS, bool BF16>
+template <int WS, bool BF16, bool GEN>
 __global__ void __launch_bounds__(kThreadsB, 1)
 tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __restrict__ x, const uint16_t* __restrict__ T,
                uint16_t* __restrict__ y, int reverse)
@@ -460,6 +573,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __
     const int t0 = part_.start[blockIdx.x], t1 = part_.start[blockIdx.x + 1];
     const int rowB = g.W * 2;
     const long long plane_elems = (long long)g.H * g.W;
+    const bool ragged = g.H != g.Hp || g.W != g.Wp;
 
     auto tile_decode = [&](int t, int& c, int& b0, int& wy0, int& np_eff, int& rows_eff) {
         c = t / tl.tiles_per_c;
@@ -468,26 +582,27 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __
         b0 = gb * tl.NP;
         wy0 = strip * tl.NSY;
         np_eff = min(tl.NP, g.B - b0);
-        rows_eff = min(tl.frame_rows, g.H - wy0 * WS);
+        rows_eff = GEN ? g.H : min(tl.frame_rows, g.H - wy0 * WS);   // GEN: whole images (nstrips == 1)
     };
 
     if (warp == 0) {
         // ------------------------------------------------------------------ producer
-        if (lane == 0) {
-            uint32_t k = 0;
-            for (int t = t0; t < t1; ++t) {
-                int c, b0, wy0, np_eff, rows_eff;
-                tile_decode(t, c, b0, wy0, np_eff, rows_eff);
-                const uint32_t bytes = (uint32_t)rows_eff * rowB;
-                for (int p = 0; p < np_eff; ++p, ++k) {
-                    const int slot = k % nslot;
-                    ptx::mbar_wait(EMPTY(slot), ((k / nslot) & 1) ^ 1);
-                    ptx::mbar_arrive_expect_tx(FULL(slot), bytes);
-                    if (p == 0) TRACE(0, (t - t0));
-                    const uint16_t* src = x + ((long long)(b0 + p) * g.C + c) * plane_elems + (long long)wy0 * WS * g.W;
-                    ptx::bulk_g2s(ptx::smem_u32(ring + (size_t)slot * tl.S), src, bytes, FULL(slot));
-                }
+        // lane p issues the copies of frame images p, p+32, ... of every tile
+        uint32_t k = 0;
+        for (int t = t0; t < t1; ++t) {
+            int c, b0, wy0, np_eff, rows_eff;
+            tile_decode(t, c, b0, wy0, np_eff, rows_eff);
+            const uint32_t bytes = (uint32_t)rows_eff * rowB;
+            for (int p = lane; p < np_eff; p += 32) {
+                const uint32_t kk = k + p;
+                const int slot = kk % nslot;
+                ptx::mbar_wait(EMPTY(slot), ((kk / nslot) & 1) ^ 1);
+                ptx::mbar_arrive_expect_tx(FULL(slot), bytes);
+                if (p == 0) TRACE(0, (t - t0));
+                const uint16_t* src = x + ((long long)(b0 + p) * g.C + c) * plane_elems + (long long)wy0 * WS * g.W;
+                ptx::bulk_g2s(ptx::smem_u32(ring + (size_t)slot * tl.S), src, bytes, FULL(slot));
             }
+            k += np_eff;
         }
     } else if (warp == 1) {
         // ------------------------------------------------------------------ MMA issuer
@@ -521,6 +636,8 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __
         const int wl = m / tl.NP, pl = m % tl.NP;
         const int wyl = wl / g.nww, wx = wl % g.nww;
         const int win_off = ((wyl * WS) * g.W + wx * WS) * 2;
+        GenAddr<GEN ? WS : 1> ga;
+        if constexpr (GEN) gen_addr_init<WS>(ga, g, wyl, wx);
         uint32_t k = 0, lt = 0;
         int cur_c = -1;
         uint16_t tabv[kTabRegs];
@@ -578,8 +695,11 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __
             if (rt == 0) TRACE(5, lt);
             if (part) ptx::mbar_wait(FULL(slot), (kk / nslot) & 1);
             if (rt == 0) TRACE(6, lt);
-            window_to_tmem<WS>(ring + (size_t)slot * tl.S + win_off, valid, rowB,
-                               tmem + buf * A_STRIDE + ((uint32_t)(q * 32) << 16));
+            if constexpr (GEN)
+                window_to_tmem_gen<WS>(ring + (size_t)slot * tl.S, ga, valid, ragged, tmem + buf * A_STRIDE + ((uint32_t)(q * 32) << 16));
+            else
+                window_to_tmem<WS>(ring + (size_t)slot * tl.S + win_off, valid, rowB,
+                                   tmem + buf * A_STRIDE + ((uint32_t)(q * 32) << 16));
             ptx::tc_fence_before_sync();
             ptx::mbar_arrive(A_FULL + 8 * buf);
             if (part) ptx::mbar_arrive(EMPTY(slot));   // every window of this image is in TMEM
@@ -593,6 +713,8 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __
         const int wl = m / tl.NP, pl = m % tl.NP;
         const int wyl = wl / g.nww, wx = wl % g.nww;
         uint8_t* win = outf + pl * tl.S + ((wyl * WS) * g.W + wx * WS) * 2;
+        GenAddr<GEN ? WS : 1> ga;
+        if constexpr (GEN) gen_addr_init<WS>(ga, g, wyl, wx);
         uint32_t lt = 0;
         for (int t = t0; t < t1; ++t, ++lt) {
             int c, b0, wy0, np_eff, rows_eff;
@@ -602,7 +724,10 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __
             if (m == 0) TRACE(8, lt);
             ptx::mbar_wait(OUT_EMPTY, (lt & 1) ^ 1);     // the previous tile's stores have left the output frame
             ptx::tc_fence_after_sync();
-            tmem_to_window<WS, BF16>(win, valid, rowB, tmem_d + ((uint32_t)(q * 32) << 16));
+            if constexpr (GEN)
+                tmem_to_window_gen<WS, BF16>(outf + pl * tl.S, ga, valid, ragged, tmem_d + ((uint32_t)(q * 32) << 16));
+            else
+                tmem_to_window<WS, BF16>(win, valid, rowB, tmem_d + ((uint32_t)(q * 32) << 16));
             ptx::tc_fence_before_sync();
             ptx::mbar_arrive(D_EMPTY);
             ptx::fence_proxy_async_smem();
@@ -611,29 +736,33 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __
         }
     } else {
         // ------------------------------------------------------------------ store
-        if (lane > 0 && t1 > t0) {   // idle lanes: pull this CTA's table rows into L2 ahead of the W_c builds
+        if (t1 > t0) {   // pull this CTA's table rows into L2 ahead of the W_c builds
             const int c_first = t0 / tl.tiles_per_c, c_last = (t1 - 1) / tl.tiles_per_c;
             const char* base = reinterpret_cast<const char*>(T + (long long)c_first * Cf::NB);
             const long long nbytes = (long long)(c_last - c_first + 1) * Cf::NB * 2;
-            for (long long off = (lane - 1) * 128ll; off < nbytes; off += 31 * 128)
+            for (long long off = lane * 128ll; off < nbytes; off += 32 * 128)
                 asm volatile("prefetch.global.L2 [%0];" ::"l"(base + off));
         }
-        if (lane == 0) {
+        {
+            // lane p stores frame images p, p+32, ... of every tile
             uint32_t lt = 0;
             for (int t = t0; t < t1; ++t, ++lt) {
                 int c, b0, wy0, np_eff, rows_eff;
                 tile_decode(t, c, b0, wy0, np_eff, rows_eff);
                 const uint32_t bytes = (uint32_t)rows_eff * rowB;
                 ptx::mbar_wait(OUT_FULL + 8 * (lt & 1), (lt >> 1) & 1);
-                TRACE(10, lt);
-                for (int p = 0; p < np_eff; ++p) {
+                if (lane == 0) TRACE(10, lt);
+                for (int p = lane; p < np_eff; p += 32) {
                     uint16_t* dst = y + ((long long)(b0 + p) * g.C + c) * plane_elems + (long long)wy0 * WS * g.W;
                     ptx::bulk_s2g(dst, ptx::smem_u32(outf + p * tl.S), bytes);
                 }
                 ptx::bulk_commit();
                 ptx::bulk_wait_read<0>();
-                TRACE(11, lt);
-                ptx::mbar_arrive(OUT_EMPTY);
+                __syncwarp();
+                if (lane == 0) {
+                    TRACE(11, lt);
+                    ptx::mbar_arrive(OUT_EMPTY);
+                }
             }
             ptx::bulk_wait_all<0>();
         }
@@ -656,14 +785,18 @@ int bulk_slots(const TcTiles& tl)
     return (int)n;
 }
 
+// 0 = not servable by the bulk kernel, 1 = aligned fast form, 2 = general form (shift / ragged).
 template <int WS>
-bool bulk_ok(const Geom& g, const TcTiles& tl, const void* x, const void* y)
+int bulk_mode(const Geom& g, const TcTiles& tl, const void* x, const void* y)
 {
-    if (g.layout != WBMM_LAYOUT_NCHW || g.sh != 0 || g.sw != 0 || g.H != g.Hp || g.W != g.Wp) return false;
-    if ((tl.frame_rows * g.W * 2) % 16 != 0 || ((long long)g.H * g.W * 2) % 16 != 0) return false;
-    if (reinterpret_cast<uintptr_t>(x) % 16 != 0 || reinterpret_cast<uintptr_t>(y) % 16 != 0) return false;
-    if (tl.NP > kMaxSlots || tl.ntiles > 0x3fffffffll) return false;
-    return bulk_slots<WS>(tl) >= tl.NP + 1;
+    if (g.layout != WBMM_LAYOUT_NCHW) return 0;
+    if (((long long)g.H * g.W * 2) % 16 != 0) return 0;
+    if (reinterpret_cast<uintptr_t>(x) % 16 != 0 || reinterpret_cast<uintptr_t>(y) % 16 != 0) return 0;
+    if (tl.NP > kMaxSlots || tl.ntiles > 0x3fffffffll) return 0;
+    if (bulk_slots<WS>(tl) < tl.NP + 1) return 0;
+    const bool plain = g.sh == 0 && g.sw == 0 && g.H == g.Hp && g.W == g.Wp;
+    if (plain) return (tl.frame_rows * g.W * 2) % 16 == 0 ? 1 : (tl.nstrips == 1 ? 2 : 0);
+    return tl.nstrips == 1 ? 2 : 0;
 }
 
 // Greedy contiguous partition of the tile sequence over `grid` CTAs minimising the largest cost,
@@ -701,11 +834,11 @@ int partition_tiles(const TcTiles& tl, int grid, TilePart* part)
     return used;
 }
 
-template <int WS, bool BF16>
+template <int WS, bool BF16, bool GEN>
 cudaError_t launch_bulk(const Geom& g, const TcTiles& tl, const void* x, const void* T, void* y, bool reverse,
                         cudaStream_t s)
 {
-    auto k = tc_bulk_kernel<WS, BF16>;
+    auto k = tc_bulk_kernel<WS, BF16, GEN>;
     const int nslot = bulk_slots<WS>(tl);
     const size_t smem = (size_t)BulkSmem<WS>::FIXED + (size_t)(tl.NP + nslot) * tl.S;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -815,14 +948,20 @@ cudaError_t tc_forward(const Geom& g, int dtype, const void* x, const void* T, v
     if (tl.ntiles == 0) return cudaSuccess;
     *launches += 1;
     const bool bf = dtype == WBMM_DTYPE_BF16;
-    const bool bulk = g.w == 7 ? bulk_ok<7>(g, tl, x, y) : bulk_ok<14>(g, tl, x, y);
-    if (bulk) {
+    const int mode = g.w == 7 ? bulk_mode<7>(g, tl, x, y) : bulk_mode<14>(g, tl, x, y);
+    if (mode != 0) {
         *path = WBMM_PATH_TC_TMA;
-        if (g.w == 7)
-            return bf ? launch_bulk<7, true>(g, tl, x, T, y, reverse, stream)
-                      : launch_bulk<7, false>(g, tl, x, T, y, reverse, stream);
-        return bf ? launch_bulk<14, true>(g, tl, x, T, y, reverse, stream)
-                  : launch_bulk<14, false>(g, tl, x, T, y, reverse, stream);
+        const int sel = (g.w == 7 ? 0 : 4) + (bf ? 2 : 0) + (mode == 2 ? 1 : 0);
+        switch (sel) {
+        case 0: return launch_bulk<7, false, false>(g, tl, x, T, y, reverse, stream);
+        case 1: return launch_bulk<7, false, true>(g, tl, x, T, y, reverse, stream);
+        case 2: return launch_bulk<7, true, false>(g, tl, x, T, y, reverse, stream);
+        case 3: return launch_bulk<7, true, true>(g, tl, x, T, y, reverse, stream);
+        case 4: return launch_bulk<14, false, false>(g, tl, x, T, y, reverse, stream);
+        case 5: return launch_bulk<14, false, true>(g, tl, x, T, y, reverse, stream);
+        case 6: return launch_bulk<14, true, false>(g, tl, x, T, y, reverse, stream);
+        default: return launch_bulk<14, true, true>(g, tl, x, T, y, reverse, stream);
+        }
     }
     *path = WBMM_PATH_TC_GATHER;
     if (g.w == 7)
