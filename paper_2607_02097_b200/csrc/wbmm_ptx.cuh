@@ -42,10 +42,33 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity)
         : "memory");
     return ok != 0;
 }
+#ifdef WBMM_WATCHDOG
+// Debug build only: a wait that gives up after ~2^22 probes and records who was stuck.
+__device__ unsigned long long g_watchdog[64];
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
 {
-    while (!mbar_try_wait(bar, parity)) {}
+    for (unsigned it = 0; it < (1u << 22); ++it)
+        if (mbar_try_wait(bar, parity)) return;
+    unsigned slot = atomicAdd((unsigned*)&g_watchdog[0], 1u);
+    if (slot < 60)
+        g_watchdog[2 + slot] = ((unsigned long long)blockIdx.x << 48) | ((unsigned long long)threadIdx.x << 36) |
+                               ((unsigned long long)(bar & 0xfffff) << 8) | parity;
 }
+#else
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n\t"
+        ".reg .pred P1;\n\t"
+        "WBMM_WAIT_LOOP:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n\t"
+        "@P1 bra WBMM_WAIT_DONE;\n\t"
+        "bra WBMM_WAIT_LOOP;\n\t"
+        "WBMM_WAIT_DONE:\n\t"
+        "}" ::"r"(bar), "r"(parity)
+        : "memory");
+}
+#endif
 
 // ------------------------------------------------------------------------------- proxies / fences
 // generic-proxy writes to shared memory -> visible to the async proxy (tcgen05.mma operand reads,

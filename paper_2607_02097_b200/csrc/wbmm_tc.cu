@@ -14,30 +14,15 @@
 
 #include <mutex>
 
-#include "wbmm_ptx.cuh"
+#include "wbmm_tc_dev.cuh"
 
 namespace wbmm {
+
+using namespace tcdev;
 
 namespace {
 
 constexpr int kThreadsG = 256;   // generic kernel: 8 warps; warps 0-3 own the 128 TMEM lanes
-
-template <int WS>
-struct WinCfg {
-    static constexpr int N = WS * WS;                    // positions per window
-    static constexpr int K_PAD = (N + 15) / 16 * 16;     // MMA K (16 per instruction)
-    static constexpr int N_PAD = (N + 15) / 16 * 16;     // MMA N (multiple of 16 for M = 128)
-    static constexpr int KSTEPS = K_PAD / 16;
-    static constexpr int NW = (N + 1) / 2;               // 32-bit words per window (A columns used)
-    static constexpr int A_COLS = K_PAD / 2;
-    static constexpr int TW = 2 * WS - 1;
-    static constexpr int NB = TW * TW;
-    static constexpr int LBO = N_PAD * 16;               // bytes between K chunks (8 values) of W_c
-    static constexpr int WC_BYTES = (K_PAD / 8) * LBO;
-    static constexpr int D_COL = (A_COLS + 31) / 32 * 32;
-    static constexpr int TMEM_COLS = (D_COL + N_PAD) <= 128 ? 128 : ((D_COL + N_PAD) <= 256 ? 256 : 512);
-    static constexpr int TS_BYTES = (NB * 2 + 15) / 16 * 16;
-};
 
 // Stage one channel's table row in shared memory (reversed for the transposed operator) and build
 // W_c[i][j] = T[c, rel(i,j)] in the K-major core-matrix layout: value (i, j) lives at byte
@@ -68,215 +53,6 @@ __device__ __forceinline__ void build_weight(const uint16_t* __restrict__ Tc, bo
         }
         *reinterpret_cast<uint4*>(Wc + kc * Cf::LBO + i * 16) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
     }
-}
-
-// Word wi (values 2wi, 2wi+1 in row-major in-window order) of the window whose top-left frame
-// element is at `win` (bytes), frame row pitch rowB bytes.
-template <int WS>
-__device__ __forceinline__ uint32_t load_word(const uint8_t* win, int rowB, int wi)
-{
-    if constexpr (WS % 2 == 0) {
-        const int r = (2 * wi) / WS, cc = (2 * wi) % WS;
-        return *reinterpret_cast<const uint32_t*>(win + r * rowB + cc * 2);
-    } else {
-        const int e0 = 2 * wi, e1 = 2 * wi + 1;
-        uint32_t lo = *reinterpret_cast<const uint16_t*>(win + (e0 / WS) * rowB + (e0 % WS) * 2);
-        uint32_t hi = 0;
-        if (e1 < WS * WS) hi = *reinterpret_cast<const uint16_t*>(win + (e1 / WS) * rowB + (e1 % WS) * 2);
-        return lo | (hi << 16);
-    }
-}
-
-template <int WS>
-__device__ __forceinline__ void store_word(uint8_t* win, int rowB, int wi, uint32_t v)
-{
-    if constexpr (WS % 2 == 0) {
-        const int r = (2 * wi) / WS, cc = (2 * wi) % WS;
-        *reinterpret_cast<uint32_t*>(win + r * rowB + cc * 2) = v;
-    } else {
-        const int e0 = 2 * wi, e1 = 2 * wi + 1;
-        *reinterpret_cast<uint16_t*>(win + (e0 / WS) * rowB + (e0 % WS) * 2) = (uint16_t)(v & 0xffffu);
-        if (e1 < WS * WS) *reinterpret_cast<uint16_t*>(win + (e1 / WS) * rowB + (e1 % WS) * 2) = (uint16_t)(v >> 16);
-    }
-}
-
-template <bool BF16>
-__device__ __forceinline__ uint32_t pack2(uint32_t a, uint32_t b)
-{
-    const float fa = __uint_as_float(a), fb = __uint_as_float(b);
-    if constexpr (BF16) {
-        __nv_bfloat162 h = __floats2bfloat162_rn(fa, fb);
-        return *reinterpret_cast<uint32_t*>(&h);
-    } else {
-        __half2 h = __floats2half2_rn(fa, fb);
-        return *reinterpret_cast<uint32_t*>(&h);
-    }
-}
-
-// Window -> TMEM A: all 32 lanes of the warp take part (tcgen05.st is warp-collective); lanes
-// without a window write zeros.
-template <int WS>
-__device__ __forceinline__ void window_to_tmem(const uint8_t* win, bool valid, int rowB, uint32_t taddr)
-{
-    using Cf = WinCfg<WS>;
-#pragma unroll
-    for (int ch = 0; ch < Cf::A_COLS / 16; ++ch) {
-        uint32_t v[16];
-#pragma unroll
-        for (int e = 0; e < 16; ++e) {
-            const int wi = ch * 16 + e;
-            v[e] = (wi < Cf::NW && valid) ? load_word<WS>(win, rowB, wi) : 0u;
-        }
-        ptx::tmem_st16(taddr + ch * 16, v);
-    }
-    if constexpr (Cf::A_COLS % 16 != 0) {
-        static_assert(Cf::A_COLS % 16 == 8, "A columns come in 8s");
-        constexpr int ch = Cf::A_COLS / 16;
-        uint32_t v[8];
-#pragma unroll
-        for (int e = 0; e < 8; ++e) {
-            const int wi = ch * 16 + e;
-            v[e] = (wi < Cf::NW && valid) ? load_word<WS>(win, rowB, wi) : 0u;
-        }
-        ptx::tmem_st8(taddr + ch * 16, v);
-    }
-    ptx::tmem_wait_st();
-}
-
-// TMEM D -> rounded 16-bit values in the window's frame position (32 columns per wait).
-template <int WS, bool BF16>
-__device__ __forceinline__ void tmem_to_window(uint8_t* win, bool valid, int rowB, uint32_t taddr)
-{
-    using Cf = WinCfg<WS>;
-    constexpr int NCH = (Cf::NW + 7) / 8;     // 16-column chunks that hold real outputs
-#pragma unroll
-    for (int ch = 0; ch < NCH; ch += 2) {
-        uint32_t v[32];
-        ptx::tmem_ld16(taddr + ch * 16, v);
-        if (ch + 1 < NCH) ptx::tmem_ld16(taddr + (ch + 1) * 16, v + 16);
-        ptx::tmem_wait_ld();
-        if (valid) {
-#pragma unroll
-            for (int e = 0; e < 16; ++e) {
-                const int wi = ch * 8 + e;
-                if (wi < Cf::NW && (e < 8 || ch + 1 < NCH))
-                    store_word<WS>(win, rowB, wi, pack2<BF16>(v[2 * e], v[2 * e + 1]));
-            }
-        }
-    }
-}
-
-// General window addressing for whole-image frames held exactly as they sit in global memory
-// (row pitch W): the cyclic shift and the zero padding (Eq. 4-5; A6) become per-thread
-// row / column byte offsets plus validity bit masks (bit r / bit cc set = inside H x W).  Offsets
-// of padding rows / columns are clamped to 0 so every load address is legal; the value is masked.
-template <int WS>
-struct GenAddr {
-    int rowoff[WS], coloff[WS];
-    uint32_t rowmask, colmask;
-};
-
-template <int WS>
-__device__ __forceinline__ void gen_addr_init(GenAddr<WS>& a, const Geom& g, int wyl, int wx)
-{
-    a.rowmask = a.colmask = 0;
-#pragma unroll
-    for (int r = 0; r < WS; ++r) {
-        int h = wyl * WS + r + g.sh;
-        if (h >= g.Hp) h -= g.Hp;
-        a.rowoff[r] = h < g.H ? h * g.W * 2 : 0;
-        a.rowmask |= (h < g.H ? 1u : 0u) << r;
-    }
-#pragma unroll
-    for (int cc = 0; cc < WS; ++cc) {
-        int v = wx * WS + cc + g.sw;
-        if (v >= g.Wp) v -= g.Wp;
-        a.coloff[cc] = v < g.W ? v * 2 : 0;
-        a.colmask |= (v < g.W ? 1u : 0u) << cc;
-    }
-}
-
-// RAGGED = false: every window element lies inside H x W (no padding anywhere), masks unused.
-template <int WS, bool RAGGED>
-__device__ __forceinline__ uint32_t gen_load_word(const uint8_t* img, const GenAddr<WS>& a, uint32_t rm, int wi)
-{
-    const int e0 = 2 * wi, e1 = 2 * wi + 1;
-    uint32_t lo = *reinterpret_cast<const uint16_t*>(img + a.rowoff[e0 / WS] + a.coloff[e0 % WS]);
-    if (RAGGED && !((rm >> (e0 / WS)) & (a.colmask >> (e0 % WS)) & 1u)) lo = 0;
-    uint32_t hi = 0;
-    if (e1 < WS * WS) {
-        hi = *reinterpret_cast<const uint16_t*>(img + a.rowoff[e1 / WS] + a.coloff[e1 % WS]);
-        if (RAGGED && !((rm >> (e1 / WS)) & (a.colmask >> (e1 % WS)) & 1u)) hi = 0;
-    }
-    return lo | (hi << 16);
-}
-
-template <int WS, bool RAGGED>
-__device__ __forceinline__ void gen_store_word(uint8_t* img, const GenAddr<WS>& a, int wi, uint32_t v)
-{
-    const int e0 = 2 * wi, e1 = 2 * wi + 1;
-    if (!RAGGED || ((a.rowmask >> (e0 / WS)) & (a.colmask >> (e0 % WS)) & 1u))
-        *reinterpret_cast<uint16_t*>(img + a.rowoff[e0 / WS] + a.coloff[e0 % WS]) = (uint16_t)(v & 0xffffu);
-    if (e1 < WS * WS) {
-        if (!RAGGED || ((a.rowmask >> (e1 / WS)) & (a.colmask >> (e1 % WS)) & 1u))
-            *reinterpret_cast<uint16_t*>(img + a.rowoff[e1 / WS] + a.coloff[e1 % WS]) = (uint16_t)(v >> 16);
-    }
-}
-
-template <int WS, bool RAGGED>
-__device__ __forceinline__ void window_to_tmem_gen_t(const uint8_t* img, const GenAddr<WS>& a, uint32_t rm, uint32_t taddr)
-{
-    using Cf = WinCfg<WS>;
-#pragma unroll
-    for (int ch = 0; ch < (Cf::A_COLS + 15) / 16; ++ch) {
-        uint32_t v[16];
-#pragma unroll
-        for (int e = 0; e < 16; ++e) {
-            const int wi = ch * 16 + e;
-            v[e] = wi < Cf::NW ? gen_load_word<WS, RAGGED>(img, a, rm, wi) : 0u;
-        }
-        if (ch * 16 + 16 <= Cf::A_COLS) ptx::tmem_st16(taddr + ch * 16, v);
-        else ptx::tmem_st8(taddr + ch * 16, v);
-    }
-}
-
-// tcgen05.st is warp-collective: every lane runs the same instruction stream; a lane without a
-// window (or a ragged problem) takes the masked form, chosen warp-uniformly.
-template <int WS>
-__device__ __forceinline__ void window_to_tmem_gen(const uint8_t* img, const GenAddr<WS>& a, bool valid, bool ragged,
-                                                   uint32_t taddr)
-{
-    const bool masked = ragged || !__all_sync(0xffffffffu, valid);
-    if (masked) window_to_tmem_gen_t<WS, true>(img, a, valid ? a.rowmask : 0u, taddr);
-    else window_to_tmem_gen_t<WS, false>(img, a, 0u, taddr);
-    ptx::tmem_wait_st();
-}
-
-template <int WS, bool BF16, bool RAGGED>
-__device__ __forceinline__ void tmem_to_window_gen_t(uint8_t* img, const GenAddr<WS>& a, bool valid, uint32_t taddr)
-{
-    using Cf = WinCfg<WS>;
-    constexpr int NCH = (Cf::NW + 7) / 8;
-#pragma unroll
-    for (int ch = 0; ch < NCH; ++ch) {
-        uint32_t v[16];
-        ptx::tmem_ld16(taddr + ch * 16, v);
-        ptx::tmem_wait_ld();
-        if (valid) {
-#pragma unroll
-            for (int e = 0; e < 8; ++e) {
-                const int wi = ch * 8 + e;
-                if (wi < Cf::NW) gen_store_word<WS, RAGGED>(img, a, wi, pack2<BF16>(v[2 * e], v[2 * e + 1]));
-            }
-        }
-    }
-}
-
-template <int WS, bool BF16>
-__device__ __forceinline__ void tmem_to_window_gen(uint8_t* img, const GenAddr<WS>& a, bool valid, bool ragged, uint32_t taddr)
-{
-    if (ragged) tmem_to_window_gen_t<WS, BF16, true>(img, a, valid, taddr);
-    else tmem_to_window_gen_t<WS, BF16, false>(img, a, valid, taddr);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -407,27 +183,6 @@ tc_generic_kernel(Geom g, TcTiles tl, const uint16_t* __restrict__ x, const uint
 //
 // Each 32-bit shared-memory access of the repack / epilogue warps is conflict-free for the
 // headline geometry: lanes are (4 adjacent windows) x (8 images) and the image stride is 16*odd bytes.
-int num_sms();
-constexpr int kThreadsB = 352;
-constexpr int kMaxSlots = 64;
-constexpr int kMaxGrid = 160;
-
-// Static tile schedule: CTA b owns tiles [start[b], start[b+1]) (channel-major, so W_c is rebuilt
-// at most once or twice per CTA).  The host balances tiles + the cost of mid-range W_c rebuilds.
-struct TilePart {
-    int start[kMaxGrid + 1];
-};
-
-
-#ifdef WBMM_TRACE
-// Debug build only: per-tile event timestamps of block 0 (read back with wbmm_debug_trace()).
-__device__ long long g_trace[16 * 16];
-__device__ long long g_blk[148 * 4];
-__device__ __forceinline__ long long gtime() { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
-#define TRACE(ev, lt) do { if (blockIdx.x == 1 && (lt) < 16) g_trace[(lt) * 16 + (ev)] = gtime(); } while (0)
-#else
-#define TRACE(ev, lt) do { } while (0)
-#endif
 
 // W_c for w = 14 from two copies of the fully reversed table F[q] = T[NB-1-q] (F0 = F, F1 = F
 // shifted by one value), so that any pair (F[q], F[q+1]) is one aligned 32-bit load.  Row i of W_c
@@ -603,6 +358,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __
                 ptx::bulk_g2s(ptx::smem_u32(ring + (size_t)slot * tl.S), src, bytes, FULL(slot));
             }
             k += np_eff;
+            __syncwarp();   // no lane starts the next tile's copies before every copy of this tile is issued (see the repack warps)
         }
     } else if (warp == 1) {
         // ------------------------------------------------------------------ MMA issuer
@@ -646,6 +402,11 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __
             int c, b0, wy0, np_eff, rows_eff;
             tile_decode(t, c, b0, wy0, np_eff, rows_eff);
             const uint32_t buf = lt & 1;
+            // Slot barriers are tested by phase PARITY, and successive fills of one slot are consumed by
+            // different threads: a thread may only test fill n once fill n-1 is known to have landed.
+            // After this barrier every repack thread has passed its waits of the previous tile, and a
+            // slot's previous fill always belongs to an earlier tile (nslot > images per tile).
+            ptx::named_bar_sync(2, 128);
             ptx::mbar_wait(A_EMPTY + 8 * buf, ((lt >> 1) & 1) ^ 1);   // MMA(lt-2) has consumed A[buf]
             if (rt == 0) TRACE(4, lt);
             if (c != cur_c) {
@@ -799,11 +560,82 @@ int bulk_mode(const Geom& g, const TcTiles& tl, const void* x, const void* y)
     return tl.nstrips == 1 ? 2 : 0;
 }
 
+template <int WS, bool BF16, bool GEN>
+cudaError_t launch_bulk(const Geom& g, const TcTiles& tl, const void* x, const void* T, void* y, bool reverse,
+                        cudaStream_t s)
+{
+    auto k = tc_bulk_kernel<WS, BF16, GEN>;
+    const int nslot = bulk_slots<WS>(tl);
+    const size_t smem = (size_t)BulkSmem<WS>::FIXED + (size_t)(tl.NP + nslot) * tl.S;
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    int grid = (int)(tl.ntiles < num_sms() ? tl.ntiles : num_sms());
+    if (grid > kMaxGrid) grid = kMaxGrid;
+    // the schedule depends on (tiles, tiles per channel, grid) only: keep the last one
+    static std::mutex mu;
+    static TilePart cached;
+    static long long key_n = -1;
+    static int key_tpc = -1, key_grid = -1, cached_used = 0;
+    TilePart part;
+    {
+        std::lock_guard<std::mutex> lock(mu);
+        if (key_n != tl.ntiles || key_tpc != tl.tiles_per_c || key_grid != grid) {
+            cached_used = partition_tiles(tl, grid, 0.75, &cached);
+            key_n = tl.ntiles; key_tpc = tl.tiles_per_c; key_grid = grid;
+        }
+        part = cached;
+        grid = cached_used;
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3(kThreadsB);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, k, g, tl, part, nslot, (const uint16_t*)x, (const uint16_t*)T, (uint16_t*)y,
+                              reverse ? 1 : 0);
+}
+
+template <int WS>
+size_t generic_smem(const TcTiles& tl)
+{
+    return (size_t)WinCfg<WS>::WC_BYTES + WinCfg<WS>::TS_BYTES + (size_t)tl.NP * tl.S;
+}
+
+template <int WS, bool BF16>
+cudaError_t launch_generic(const Geom& g, const TcTiles& tl, const void* x, const void* T, void* y, bool reverse,
+                           cudaStream_t s)
+{
+    auto k = tc_generic_kernel<WS, BF16>;
+    const size_t smem = generic_smem<WS>(tl);
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    const int grid = (int)(tl.ntiles < num_sms() ? tl.ntiles : num_sms());
+    k<<<grid, kThreadsG, smem, s>>>(g, tl, (const uint16_t*)x, (const uint16_t*)T, (uint16_t*)y, reverse ? 1 : 0);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+int num_sms()
+{
+    static int n = 0;
+    if (n == 0) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
+        if (n <= 0) n = 148;
+    }
+    return n;
+}
+
 // Greedy contiguous partition of the tile sequence over `grid` CTAs minimising the largest cost,
 // cost = tiles + kSwitchCost per channel boundary strictly inside a CTA's range.
-constexpr double kSwitchCost = 0.75;
-
-int partition_tiles(const TcTiles& tl, int grid, TilePart* part)
+int partition_tiles(const TcTiles& tl, int grid, double kSwitchCost, TilePart* part)
 {
     const int n = (int)tl.ntiles, tpc = tl.tiles_per_c;
     auto fill = [&](double cap, TilePart* out) {
@@ -833,79 +665,6 @@ int partition_tiles(const TcTiles& tl, int grid, TilePart* part)
     for (int b = used; b < kMaxGrid; ++b) part->start[b + 1] = n;
     return used;
 }
-
-template <int WS, bool BF16, bool GEN>
-cudaError_t launch_bulk(const Geom& g, const TcTiles& tl, const void* x, const void* T, void* y, bool reverse,
-                        cudaStream_t s)
-{
-    auto k = tc_bulk_kernel<WS, BF16, GEN>;
-    const int nslot = bulk_slots<WS>(tl);
-    const size_t smem = (size_t)BulkSmem<WS>::FIXED + (size_t)(tl.NP + nslot) * tl.S;
-    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    int grid = (int)(tl.ntiles < num_sms() ? tl.ntiles : num_sms());
-    if (grid > kMaxGrid) grid = kMaxGrid;
-    // the schedule depends on (tiles, tiles per channel, grid) only: keep the last one
-    static std::mutex mu;
-    static TilePart cached;
-    static long long key_n = -1;
-    static int key_tpc = -1, key_grid = -1, cached_used = 0;
-    TilePart part;
-    {
-        std::lock_guard<std::mutex> lock(mu);
-        if (key_n != tl.ntiles || key_tpc != tl.tiles_per_c || key_grid != grid) {
-            cached_used = partition_tiles(tl, grid, &cached);
-            key_n = tl.ntiles; key_tpc = tl.tiles_per_c; key_grid = grid;
-        }
-        part = cached;
-        grid = cached_used;
-    }
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((unsigned)grid);
-    cfg.blockDim = dim3(kThreadsB);
-    cfg.dynamicSmemBytes = smem;
-    cfg.stream = s;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = attr;
-    cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, k, g, tl, part, nslot, (const uint16_t*)x, (const uint16_t*)T, (uint16_t*)y,
-                              reverse ? 1 : 0);
-}
-
-template <int WS>
-size_t generic_smem(const TcTiles& tl)
-{
-    return (size_t)WinCfg<WS>::WC_BYTES + WinCfg<WS>::TS_BYTES + (size_t)tl.NP * tl.S;
-}
-
-int num_sms()
-{
-    static int n = 0;
-    if (n == 0) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
-        if (n <= 0) n = 148;
-    }
-    return n;
-}
-
-template <int WS, bool BF16>
-cudaError_t launch_generic(const Geom& g, const TcTiles& tl, const void* x, const void* T, void* y, bool reverse,
-                           cudaStream_t s)
-{
-    auto k = tc_generic_kernel<WS, BF16>;
-    const size_t smem = generic_smem<WS>(tl);
-    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    const int grid = (int)(tl.ntiles < num_sms() ? tl.ntiles : num_sms());
-    k<<<grid, kThreadsG, smem, s>>>(g, tl, (const uint16_t*)x, (const uint16_t*)T, (uint16_t*)y, reverse ? 1 : 0);
-    return cudaGetLastError();
-}
-
-}  // namespace
 
 bool tc_tiles(const Geom& g, TcTiles* t)
 {
@@ -971,11 +730,6 @@ cudaError_t tc_forward(const Geom& g, int dtype, const void* x, const void* T, v
               : launch_generic<14, false>(g, tl, x, T, y, reverse, stream);
 }
 
-bool tc_grad_table_supported(const Geom&, int, const void*, const void*) { return false; }
-cudaError_t tc_grad_table(const Geom&, int, const void*, const void*, float*, cudaStream_t, int*, int*)
-{
-    return cudaErrorNotSupported;
-}
 void tc_release() {}
 
 #ifdef WBMM_TRACE

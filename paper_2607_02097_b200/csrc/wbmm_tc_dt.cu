@@ -1,0 +1,352 @@
+// WBMM table gradient on the tensor cores (autograd of Alg. 1):
+//     S_c[i, j] = sum over windows n of dY[n, i] * X[n, j]          (tcgen05.mma, fp32 in TMEM)
+//     dT[c, k]  = sum over pairs (i, j) with rel(i, j) = k of S_c[i, j]   (Eq. 6-7 as a scatter)
+//
+// The contraction index of S is the WINDOW, so both operands are "MN-major": thread n writes its
+// window's N values as 16-byte vectors of 8 consecutive positions into the no-swizzle core-matrix
+// layout  addr(pos, n) = (pos/8)*SBO + (n/8)*128 + (n%8)*16 + (pos%8)*2  -- 32 lanes write 512
+// contiguous bytes.  One tile = 128 windows = MMA K of 128 (8 instructions per M-tile).  S stays in
+// TMEM while a CTA walks the tiles of one channel; at the end of the channel segment every warp
+// folds its 32 rows of S into a private copy of the (2w-1)^2 bins in shared memory (plain
+// read-add-write: within one column step the 32 rows of a warp hit 32 different bins), the copies
+// are summed and ONE pass of red.global.add.f32 per bin goes to dT.
+//
+//   warp 0      producer   bulk loads of the x and dy frame images of a tile into the slot ring
+//   warp 1      MMA        MT * 8 tcgen05.mma (SS form, both operands MN-major) per tile
+//   warps 2-5   x  -> B operand stage;  warps 6-9   dy -> A operand stage;  all eight: the bin epilogue
+#include "wbmm_tc_dev.cuh"
+
+#include <mutex>
+
+namespace wbmm {
+
+using namespace tcdev;
+
+namespace {
+
+constexpr int kThreadsD = 320;
+
+template <int WS>
+struct DtCfg {
+    using Cf = WinCfg<WS>;
+    static constexpr int MT = (Cf::N + 127) / 128;     // M tiles of 128 output positions
+    static constexpr int NV = (Cf::N + 7) / 8;         // 16-byte vectors a window fills
+    static constexpr int NVEC = Cf::N_PAD / 8;         // vectors per operand region
+    static constexpr int SBO = 128 * 16;               // bytes between position groups (128 windows x 16 B)
+    static constexpr int LBO = 128;                    // bytes between groups of 8 windows
+    static constexpr int OP_BYTES = NVEC * SBO;
+    static constexpr int STAGE = 2 * OP_BYTES;         // A region then B region; an M-tile's 16 vectors may run into B
+    static constexpr int BAR_BYTES = (2 * kMaxSlots + 8) * 8;
+    static constexpr int FIXED = STAGE + BAR_BYTES;
+    static_assert(MT * 16 <= 2 * NVEC, "an A M-tile must stay inside the stage");
+    static_assert(8 * Cf::NB * 4 <= STAGE, "per-warp bin copies alias the stage");
+};
+
+template <int WS, bool BF16, bool GEN>
+__global__ void __launch_bounds__(kThreadsD, 1)
+tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __restrict__ x,
+             const uint16_t* __restrict__ dy, float* __restrict__ dT)
+{
+    using Cf = WinCfg<WS>;
+    using Dc = DtCfg<WS>;
+    extern __shared__ __align__(1024) uint8_t smem[];
+    uint8_t* stage = smem;                                   // A (dy) region, then B (x) region
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + Dc::STAGE);
+    uint8_t* ring = smem + Dc::FIXED;
+    __shared__ uint32_t tmem_base_s;
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const uint32_t bar0 = ptx::smem_u32(bars);
+    auto FULL = [&](int s) { return bar0 + 8u * s; };
+    auto EMPTY = [&](int s) { return bar0 + 8u * (kMaxSlots + s); };
+    const uint32_t STAGE_FULL = bar0 + 8u * (2 * kMaxSlots), STAGE_EMPTY = STAGE_FULL + 8;
+    const int wpf = tl.NSY * g.nww;
+
+    if (warp == 1) ptx::tmem_alloc(ptx::smem_u32(&tmem_base_s), 512);
+    if (tid >= 64 && tid < 64 + nslot) {
+        ptx::mbar_init(FULL(tid - 64), 1);
+        ptx::mbar_init(EMPTY(tid - 64), wpf);
+        ptx::fence_mbar_init();
+    }
+    if (tid == 0) {
+        ptx::mbar_init(STAGE_FULL, 256);
+        ptx::mbar_init(STAGE_EMPTY, 1);
+        ptx::fence_mbar_init();
+    }
+    // vectors a window never writes (padding positions) must read as zero / finite
+    for (int i = tid; i < Dc::STAGE / 16; i += kThreadsD) reinterpret_cast<uint4*>(stage)[i] = make_uint4(0, 0, 0, 0);
+    ptx::fence_proxy_async_smem();
+    ptx::tc_fence_before_sync();
+    __syncthreads();
+    ptx::tc_fence_after_sync();
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    const uint32_t tmem = tmem_base_s;
+
+    const int t0 = part_.start[blockIdx.x], t1 = part_.start[blockIdx.x + 1];
+    const int rowB = g.W * 2;
+    const long long plane_elems = (long long)g.H * g.W;
+    const bool ragged = g.H != g.Hp || g.W != g.Wp;
+
+    auto tile_decode = [&](int t, int& c, int& b0, int& wy0, int& np_eff, int& rows_eff) {
+        c = t / tl.tiles_per_c;
+        const int rem = t - c * tl.tiles_per_c;
+        const int gb = rem / tl.nstrips, strip = rem - gb * tl.nstrips;
+        b0 = gb * tl.NP;
+        wy0 = strip * tl.NSY;
+        np_eff = min(tl.NP, g.B - b0);
+        rows_eff = GEN ? g.H : min(tl.frame_rows, g.H - wy0 * WS);
+    };
+
+    if (warp == 0) {
+        // ------------------------------------------------------------------ producer
+        // ring order per tile: x image 0, dy image 0, x image 1, dy image 1, ...
+        uint32_t k = 0;
+        for (int t = t0; t < t1; ++t) {
+            int c, b0, wy0, np_eff, rows_eff;
+            tile_decode(t, c, b0, wy0, np_eff, rows_eff);
+            const uint32_t bytes = (uint32_t)rows_eff * rowB;
+            for (int j = lane; j < 2 * np_eff; j += 32) {
+                const uint32_t kk = k + j;
+                const int slot = kk % nslot;
+                const int p = j >> 1;
+                ptx::mbar_wait(EMPTY(slot), ((kk / nslot) & 1) ^ 1);
+                ptx::mbar_arrive_expect_tx(FULL(slot), bytes);
+                const uint16_t* src = ((j & 1) ? dy : x) + ((long long)(b0 + p) * g.C + c) * plane_elems +
+                                      (long long)wy0 * WS * g.W;
+                ptx::bulk_g2s(ptx::smem_u32(ring + (size_t)slot * tl.S), src, bytes, FULL(slot));
+            }
+            k += 2 * np_eff;
+            __syncwarp();   // no lane starts the next tile's copies before every copy of this tile is issued (see the repack warps)
+        }
+    } else if (warp == 1) {
+        // ------------------------------------------------------------------ MMA issuer
+        if (lane == 0) {
+            constexpr uint32_t idesc = ptx::idesc_f16(BF16 ? 1 : 0, 128, Cf::N_PAD) | (1u << 15) | (1u << 16);   // A, B MN-major
+            const uint32_t a_addr = ptx::smem_u32(stage), b_addr = a_addr + Dc::OP_BYTES;
+            uint32_t lt = 0;
+            int cur_c = -1;
+            for (int t = t0; t < t1; ++t, ++lt) {
+                const int c = t / tl.tiles_per_c;
+                ptx::mbar_wait(STAGE_FULL, lt & 1);
+                ptx::tc_fence_after_sync();
+#pragma unroll
+                for (int mt = 0; mt < Dc::MT; ++mt) {
+#pragma unroll
+                    for (int ks = 0; ks < 8; ++ks) {
+                        const uint64_t ad = ptx::smem_desc_kmajor_noswz(a_addr + mt * 16 * Dc::SBO + ks * 2 * Dc::LBO, Dc::LBO, Dc::SBO);
+                        const uint64_t bd = ptx::smem_desc_kmajor_noswz(b_addr + ks * 2 * Dc::LBO, Dc::LBO, Dc::SBO);
+                        ptx::mma_ss(tmem + mt * 256, ad, bd, idesc, (c != cur_c && ks == 0) ? 0u : 1u);
+                    }
+                }
+                ptx::mma_commit(STAGE_EMPTY);
+                cur_c = c;
+            }
+        }
+    } else {
+        // ------------------------------------------------------------------ operand repack + bin epilogue
+        const int ot = tid - 64;            // 0..255
+        const int o = ot >> 7;              // 0: x -> B region, 1: dy -> A region
+        const int m = ot & 127;             // window of the tile = MMA K index (image-major)
+        const int pl = m / wpf, wl = m - pl * wpf;
+        const int wyl = wl / g.nww, wx = wl - wyl * g.nww;
+        const int win_off = ((wyl * WS) * g.W + wx * WS) * 2;
+        uint8_t* dst = stage + (o ? 0 : Dc::OP_BYTES) + m * 16;
+        GenAddr<GEN ? WS : 1> ga;
+        if constexpr (GEN) gen_addr_init<WS>(ga, g, wyl, wx);
+        float* bins = reinterpret_cast<float*>(stage);
+        float* bw = bins + (ot >> 5) * Cf::NB;          // this warp's private copy of the bins
+        const int ew = ot >> 5;                          // 0..7
+        const int emt = ew >> 2, eq = warp & 3;          // M-tile and TMEM lane quarter in the epilogue
+        const int erow = emt * 128 + eq * 32 + lane;     // row of S = output position i
+        const int eri = erow / WS, eci = erow - eri * WS;
+        uint32_t k = 0, lt = 0;
+        for (int t = t0; t < t1; ++t, ++lt) {
+            int c, b0, wy0, np_eff, rows_eff;
+            tile_decode(t, c, b0, wy0, np_eff, rows_eff);
+            // Slot barriers are tested by phase PARITY, and successive fills of one slot are consumed by
+            // different threads: a thread may only test fill n once fill n-1 is known to have landed.
+            // After this barrier every repack thread has passed its waits of the previous tile, and a
+            // slot's previous fill always belongs to an earlier tile (nslot > copies per tile).
+            ptx::named_bar_sync(1, 256);
+            const bool part = pl < tl.NP && pl < np_eff;
+            const bool valid = part && wy0 + wyl < g.nwh;
+            const uint32_t kk = k + 2 * pl + o;
+            const int slot = kk % nslot;
+            if (part) ptx::mbar_wait(FULL(slot), (kk / nslot) & 1);
+            ptx::mbar_wait(STAGE_EMPTY, (lt & 1) ^ 1);      // MMA(lt-1) has read the stage
+            const uint8_t* img = ring + (size_t)slot * tl.S;
+#pragma unroll
+            for (int v = 0; v < Dc::NV; ++v) {
+                uint32_t wv[4];
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const int wi = v * 4 + e;
+                    if (wi >= Cf::NW || !valid) wv[e] = 0u;
+                    else if constexpr (GEN) wv[e] = ragged ? gen_load_word<WS, true>(img, ga, ga.rowmask, wi)
+                                                           : gen_load_word<WS, false>(img, ga, 0u, wi);
+                    else wv[e] = load_word<WS>(img + win_off, rowB, wi);
+                }
+                *reinterpret_cast<uint4*>(dst + v * Dc::SBO) = make_uint4(wv[0], wv[1], wv[2], wv[3]);
+            }
+            ptx::fence_proxy_async_smem();
+            ptx::mbar_arrive(STAGE_FULL);
+            if (part) ptx::mbar_arrive(EMPTY(slot));
+            k += 2 * np_eff;
+
+            const bool seg_end = t + 1 == t1 || (t + 1) - c * tl.tiles_per_c == tl.tiles_per_c;
+            if (seg_end) {
+                // ---- S (TMEM) -> bins -> dT[c]
+                ptx::mbar_wait(STAGE_EMPTY, lt & 1);        // every MMA of this channel segment has completed
+                ptx::tc_fence_after_sync();
+                for (int b = lane; b < Cf::NB; b += 32) bw[b] = 0.f;
+                __syncwarp();
+                if (emt < Dc::MT) {
+                    const uint32_t taddr = tmem + emt * 256 + ((uint32_t)(eq * 32) << 16);
+                    const float* bbase = bw + (eri + WS - 1) * Cf::TW + eci + WS - 1;   // bin of (i, j) = base - rj*TW - cj
+#pragma unroll 1
+                    for (int ch = 0; ch < (Cf::N + 15) / 16; ++ch) {
+                        uint32_t v[16];
+                        ptx::tmem_ld16(taddr + ch * 16, v);
+                        ptx::tmem_wait_ld();
+                        int j = ch * 16;
+                        int rj = j / WS, cj = j - rj * WS;
+#pragma unroll
+                        for (int e = 0; e < 16; ++e) {
+                            if (j < Cf::N && erow < Cf::N) {
+                                float* pb = const_cast<float*>(bbase) - rj * Cf::TW - cj;
+                                *pb += __uint_as_float(v[e]);
+                            }
+                            __syncwarp();
+                            ++j;
+                            if (++cj == WS) { cj = 0; ++rj; }
+                        }
+                    }
+                }
+                ptx::tc_fence_before_sync();
+                ptx::named_bar_sync(1, 256);
+                for (int b = ot; b < Cf::NB; b += 256) {
+                    float sacc = 0.f;
+#pragma unroll
+                    for (int w8 = 0; w8 < 8; ++w8) sacc += bins[w8 * Cf::NB + b];
+                    atomicAdd(dT + (long long)c * Cf::NB + b, sacc);
+                }
+                ptx::named_bar_sync(1, 256);
+                // the bins aliased the operand stage: restore the zero padding vectors
+                for (int i = ot; i < 8 * Cf::NB * 4 / 16 + 1; i += 256)
+                    if (i * 16 < Dc::STAGE) reinterpret_cast<uint4*>(stage)[i] = make_uint4(0, 0, 0, 0);
+                ptx::fence_proxy_async_smem();
+                ptx::named_bar_sync(1, 256);
+            }
+        }
+    }
+    ptx::tc_fence_before_sync();
+    __syncthreads();
+    if (warp == 1) ptx::tmem_dealloc(tmem, 512);
+}
+
+template <int WS>
+int dt_slots(const TcTiles& tl)
+{
+    const long long room = 227ll * 1024 - 1024 - DtCfg<WS>::FIXED;
+    long long n = room / tl.S;
+    if (n > 6 * tl.NP) n = 6 * tl.NP;
+    if (n > kMaxSlots) n = kMaxSlots;
+    return (int)n;
+}
+
+// 0 = not servable, 1 = aligned form, 2 = general form (shift / ragged)
+template <int WS>
+int dt_mode(const Geom& g, const TcTiles& tl, const void* x, const void* dy)
+{
+    if (g.layout != WBMM_LAYOUT_NCHW) return 0;
+    if (((long long)g.H * g.W * 2) % 16 != 0) return 0;
+    if (reinterpret_cast<uintptr_t>(x) % 16 != 0 || reinterpret_cast<uintptr_t>(dy) % 16 != 0) return 0;
+    if (tl.ntiles > 0x3fffffffll) return 0;
+    if (dt_slots<WS>(tl) < 2 * tl.NP + 1) return 0;
+    const bool plain = g.sh == 0 && g.sw == 0 && g.H == g.Hp && g.W == g.Wp;
+    if (plain) return (tl.frame_rows * g.W * 2) % 16 == 0 ? 1 : (tl.nstrips == 1 ? 2 : 0);
+    return tl.nstrips == 1 ? 2 : 0;
+}
+
+template <int WS, bool BF16, bool GEN>
+cudaError_t launch_dt(const Geom& g, const TcTiles& tl, const void* x, const void* dy, float* dT, cudaStream_t s)
+{
+    auto k = tc_dt_kernel<WS, BF16, GEN>;
+    const int nslot = dt_slots<WS>(tl);
+    const size_t smem = (size_t)DtCfg<WS>::FIXED + (size_t)nslot * tl.S;
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    int grid = (int)(tl.ntiles < num_sms() ? tl.ntiles : num_sms());
+    if (grid > kMaxGrid) grid = kMaxGrid;
+    static std::mutex mu;
+    static TilePart cached;
+    static long long key_n = -1;
+    static int key_tpc = -1, key_grid = -1, cached_used = 0;
+    TilePart part;
+    {
+        std::lock_guard<std::mutex> lock(mu);
+        if (key_n != tl.ntiles || key_tpc != tl.tiles_per_c || key_grid != grid) {
+            cached_used = partition_tiles(tl, grid, 1.0, &cached);   // a channel boundary costs one bin epilogue
+            key_n = tl.ntiles; key_tpc = tl.tiles_per_c; key_grid = grid;
+        }
+        part = cached;
+        grid = cached_used;
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3(kThreadsD);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, k, g, tl, part, nslot, (const uint16_t*)x, (const uint16_t*)dy, dT);
+}
+
+}  // namespace
+
+bool tc_grad_table_supported(const Geom& g, int dtype, const void* x, const void* dy)
+{
+    if (dtype != WBMM_DTYPE_BF16 && dtype != WBMM_DTYPE_F16) return false;
+    if (g.w != 7 && g.w != 14) return false;
+    TcTiles tl;
+    if (!tc_tiles(g, &tl)) return false;
+    return (g.w == 7 ? dt_mode<7>(g, tl, x, dy) : dt_mode<14>(g, tl, x, dy)) != 0;
+}
+
+cudaError_t tc_grad_table(const Geom& g, int dtype, const void* x, const void* dy, float* dT, cudaStream_t stream,
+                          int* launches, int* path)
+{
+    TcTiles tl;
+    if (!tc_tiles(g, &tl)) return cudaErrorNotSupported;
+    if (tl.ntiles == 0) return cudaSuccess;
+    const int mode = g.w == 7 ? dt_mode<7>(g, tl, x, dy) : dt_mode<14>(g, tl, x, dy);
+    if (mode == 0) return cudaErrorNotSupported;
+    *launches += 1;
+    *path = WBMM_PATH_TC_TMA;
+    const bool bf = dtype == WBMM_DTYPE_BF16;
+    const int sel = (g.w == 7 ? 0 : 4) + (bf ? 2 : 0) + (mode == 2 ? 1 : 0);
+    switch (sel) {
+    case 0: return launch_dt<7, false, false>(g, tl, x, dy, dT, stream);
+    case 1: return launch_dt<7, false, true>(g, tl, x, dy, dT, stream);
+    case 2: return launch_dt<7, true, false>(g, tl, x, dy, dT, stream);
+    case 3: return launch_dt<7, true, true>(g, tl, x, dy, dT, stream);
+    case 4: return launch_dt<14, false, false>(g, tl, x, dy, dT, stream);
+    case 5: return launch_dt<14, false, true>(g, tl, x, dy, dT, stream);
+    case 6: return launch_dt<14, true, false>(g, tl, x, dy, dT, stream);
+    default: return launch_dt<14, true, true>(g, tl, x, dy, dT, stream);
+    }
+}
+
+
+#ifdef WBMM_WATCHDOG
+extern "C" __attribute__((visibility("default"))) int wbmm_debug_watchdog(unsigned long long* out)
+{
+    return (int)cudaMemcpyFromSymbol(out, ptx::g_watchdog, sizeof(unsigned long long) * 64);
+}
+#endif
+
+}  // namespace wbmm
