@@ -42,13 +42,30 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity)
         : "memory");
     return ok != 0;
 }
+// non-blocking probe
+__device__ __forceinline__ bool mbar_test_wait(uint32_t bar, uint32_t parity)
+{
+    uint32_t ok;
+    asm volatile(
+        "{ .reg .pred p; mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
 #ifdef WBMM_WATCHDOG
-// Debug build only: a wait that gives up after ~2^22 probes and records who was stuck.
+// Debug build only: a wait that gives up after 20 ms and records who was stuck.
 __device__ unsigned long long g_watchdog[64];
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
 {
-    for (unsigned it = 0; it < (1u << 22); ++it)
+    if (mbar_try_wait(bar, parity)) return;
+    long long t0, t1;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
+    for (;;) {
         if (mbar_try_wait(bar, parity)) return;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
+        if (t1 - t0 > 20000000ll) break;
+    }
     unsigned slot = atomicAdd((unsigned*)&g_watchdog[0], 1u);
     if (slot < 60)
         g_watchdog[2 + slot] = ((unsigned long long)blockIdx.x << 48) | ((unsigned long long)threadIdx.x << 36) |
@@ -57,16 +74,8 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
 #else
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
 {
-    asm volatile(
-        "{\n\t"
-        ".reg .pred P1;\n\t"
-        "WBMM_WAIT_LOOP:\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n\t"
-        "@P1 bra WBMM_WAIT_DONE;\n\t"
-        "bra WBMM_WAIT_LOOP;\n\t"
-        "WBMM_WAIT_DONE:\n\t"
-        "}" ::"r"(bar), "r"(parity)
-        : "memory");
+    while (!mbar_try_wait(bar, parity)) {
+    }
 }
 #endif
 

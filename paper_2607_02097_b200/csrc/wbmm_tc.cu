@@ -13,6 +13,7 @@
 #include "wbmm_tc.cuh"
 
 #include <mutex>
+#include <type_traits>
 
 #include "wbmm_tc_dev.cuh"
 
@@ -128,7 +129,7 @@ tc_generic_kernel(Geom g, TcTiles tl, const uint16_t* __restrict__ x, const uint
 
         const bool valid = wl < tl.NSY * g.nww && pl < np_eff && wy0 + wyl < g.nwh;
         if (warp < 4) {
-            window_to_tmem<WS>(win, valid, rowB, tmem_a + ((uint32_t)(warp * 32) << 16));
+            window_to_tmem<WS>(valid ? win : frame, valid, rowB, tmem_a + ((uint32_t)(warp * 32) << 16));
             ptx::tc_fence_before_sync();
         }
         __syncthreads();
@@ -178,8 +179,8 @@ tc_generic_kernel(Geom g, TcTiles tl, const uint16_t* __restrict__ x, const uint
 //   warp 0      producer   bulk loads  x -> ring of frame-image slots            (full/empty barriers)
 //   warp 1      MMA        KSTEPS tcgen05.mma per tile, A from TMEM, B = W_c     (a_full/a_empty, d_full/d_empty)
 //   warps 2-5   repack     slot -> registers -> tcgen05.st into A[buf] (2 buffers); build W_c on a channel change
-//   warps 6-9   epilogue   tcgen05.ld D -> RNE 16-bit -> output frame                     (out_full/out_empty)
-//   warp 10     store      bulk stores output frame -> y
+//   warps 6-9   epilogue   tcgen05.ld D -> RNE 16-bit -> back into the window's slot, in place  (out_full)
+//   warp 10     store      bulk stores slot -> y, then hands the slot back to the producer      (empty)
 //
 // Each 32-bit shared-memory access of the repack / epilogue warps is conflict-free for the
 // headline geometry: lanes are (4 adjacent windows) x (8 images) and the image stride is 16*odd bytes.
@@ -248,13 +249,13 @@ struct BulkSmem {
     using Cf = WinCfg<WS>;
     static constexpr int TAB_ONE = ((Cf::NB + 2) * 2 + 15) / 16 * 16;
     static constexpr int TAB_BYTES = 2 * TAB_ONE;                              // F0 and F1 (or Ts for the generic builder)
-    static constexpr int BAR_BYTES = (2 * kMaxSlots + 10) * 8;
+    static constexpr int BAR_BYTES = (2 * kMaxSlots + 8 + 2 * kMaxOutBufs) * 8;
     static constexpr int FIXED = Cf::WC_BYTES + TAB_BYTES + BAR_BYTES;
 };
 
 template <int WS, bool BF16, bool GEN>
 __global__ void __launch_bounds__(kThreadsB, 1)
-tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __restrict__ x, const uint16_t* __restrict__ T,
+tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const uint16_t* __restrict__ x, const uint16_t* __restrict__ T,
                uint16_t* __restrict__ y, int reverse)
 {
     using Cf = WinCfg<WS>;
@@ -263,8 +264,8 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __
     uint8_t* Wc = smem;
     uint16_t* tab = reinterpret_cast<uint16_t*>(smem + Cf::WC_BYTES);
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + Cf::WC_BYTES + Sm::TAB_BYTES);
-    uint8_t* outf = smem + Sm::FIXED;            // output frame: NP image slots
-    uint8_t* ring = outf + tl.NP * tl.S;         // input ring: nslot image slots
+    uint8_t* ring = smem + Sm::FIXED;                       // input ring: nslot frame-image slots
+    uint8_t* outb = ring + (size_t)nslot * tl.S;            // output ring: nout group buffers of og.images frame images
     __shared__ uint32_t tmem_base_s;
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -274,10 +275,15 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __
     const uint32_t bar0 = ptx::smem_u32(bars);
     auto FULL = [&](int s) { return bar0 + 8u * s; };
     auto EMPTY = [&](int s) { return bar0 + 8u * (kMaxSlots + s); };
-    const uint32_t A_FULL = bar0 + 8u * (2 * kMaxSlots), A_EMPTY = A_FULL + 16, D_FULL = A_FULL + 32, D_EMPTY = A_FULL + 40,
-                   OUT_FULL = A_FULL + 48, OUT_EMPTY = A_FULL + 64;
+    // A_FULL[2] A_EMPTY[2] D_FULL[2] D_EMPTY[2] OUT_FULL[nout] OUT_EMPTY[nout]
+    const uint32_t A_FULL = bar0 + 8u * (2 * kMaxSlots), A_EMPTY = A_FULL + 16, D_FULL = A_FULL + 32, D_EMPTY = A_FULL + 48,
+                   OUT_FULL = A_FULL + 64, OUT_EMPTY = OUT_FULL + 8 * kMaxOutBufs;
+    using Hs = HalfSplit<WS>;
 
     const int wpf = tl.NSY * g.nww;   // windows per frame image
+    // Output hand-off groups: the smallest runs of whole epilogue warps that cover whole frame images
+    // (lanes are image-major), so a group's images can be stored as soon as ITS warps are done.
+    const OutGroups og = out_groups(tl, wpf);
     TRACE(0, 15);
     if (warp == 1) { ptx::tmem_alloc(ptx::smem_u32(&tmem_base_s), 512); if (lane == 0) TRACE(1, 15); }
     if (tid >= 64 && tid < 64 + nslot) {
@@ -290,11 +296,14 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __
         ptx::mbar_init(A_FULL + 8, 128);
         ptx::mbar_init(A_EMPTY, 1);
         ptx::mbar_init(A_EMPTY + 8, 1);
-        ptx::mbar_init(D_FULL, 1);
-        ptx::mbar_init(D_EMPTY, 128);
-        ptx::mbar_init(OUT_FULL, 128);
-        ptx::mbar_init(OUT_FULL + 8, 128);
-        ptx::mbar_init(OUT_EMPTY, 1);
+        for (int h = 0; h < 2; ++h) {
+            ptx::mbar_init(D_FULL + 8 * h, 1);
+            ptx::mbar_init(D_EMPTY + 8 * h, 128);
+        }
+        for (int ob = 0; ob < nout; ++ob) {
+            ptx::mbar_init(OUT_FULL + 8 * ob, og.lanes);
+            ptx::mbar_init(OUT_EMPTY + 8 * ob, 1);
+        }
         ptx::fence_mbar_init();
         TRACE(2, 15);
     }
@@ -363,24 +372,27 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __
     } else if (warp == 1) {
         // ------------------------------------------------------------------ MMA issuer
         if (lane == 0) {
-            constexpr uint32_t idesc = ptx::idesc_f16(BF16 ? 1 : 0, 128, Cf::N_PAD);
             const uint32_t wc_addr = ptx::smem_u32(Wc);
             uint32_t lt = 0;
             for (int t = t0; t < t1; ++t, ++lt) {
                 const uint32_t buf = lt & 1;
                 ptx::mbar_wait(A_FULL + 8 * buf, (lt >> 1) & 1);
                 TRACE(1, lt);
-                ptx::mbar_wait(D_EMPTY, (lt & 1) ^ 1);
-                TRACE(2, lt);
-                ptx::tc_fence_after_sync();
                 const uint32_t tmem_a = tmem + buf * A_STRIDE;
 #pragma unroll
-                for (int ks = 0; ks < Cf::KSTEPS; ++ks) {
-                    const uint64_t bdesc = ptx::smem_desc_kmajor_noswz(wc_addr + ks * 2 * Cf::LBO, Cf::LBO, 128);
-                    ptx::mma_ts(tmem_d, tmem_a + ks * 8, bdesc, idesc, ks > 0 ? 1u : 0u);
+                for (int h = 0; h < Hs::NH; ++h) {
+                    ptx::mbar_wait(D_EMPTY + 8 * h, (lt & 1) ^ 1);      // the epilogue has drained this half of tile lt-1
+                    if (h == 0) TRACE(2, lt);
+                    ptx::tc_fence_after_sync();
+                    const uint32_t idesc = ptx::idesc_f16(BF16 ? 1 : 0, 128, Hs::ncols(h));
+#pragma unroll
+                    for (int ks = 0; ks < Cf::KSTEPS; ++ks) {
+                        const uint64_t bdesc = ptx::smem_desc_kmajor_noswz(wc_addr + ks * 2 * Cf::LBO + Hs::col0(h) * 16, Cf::LBO, 128);
+                        ptx::mma_ts(tmem_d + Hs::col0(h), tmem_a + ks * 8, bdesc, idesc, ks > 0 ? 1u : 0u);
+                    }
+                    ptx::mma_commit(D_FULL + 8 * h);
                 }
                 ptx::mma_commit(A_EMPTY + 8 * buf);
-                ptx::mma_commit(D_FULL);
                 TRACE(3, lt);
             }
         }
@@ -389,26 +401,16 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __
         const int q = warp & 3;
         const int m = q * 32 + lane;
         const int rt = (warp - 2) * 32 + lane;   // 0..127 among the repack threads
-        const int wl = m / tl.NP, pl = m % tl.NP;
+        const int pl = m / wpf, wl = m % wpf;   // image-major: a warp covers few images, so slots are consumed and released as they land
         const int wyl = wl / g.nww, wx = wl % g.nww;
-        const int win_off = ((wyl * WS) * g.W + wx * WS) * 2;
+        const int win_off = wl < wpf ? ((wyl * WS) * g.W + wx * WS) * 2 : 0;   // lanes without a window read a legal address
         GenAddr<GEN ? WS : 1> ga;
         if constexpr (GEN) gen_addr_init<WS>(ga, g, wyl, wx);
         uint32_t k = 0, lt = 0;
         int cur_c = -1;
         uint16_t tabv[kTabRegs];
         bool tabv_ready = false;
-        for (int t = t0; t < t1; ++t, ++lt) {
-            int c, b0, wy0, np_eff, rows_eff;
-            tile_decode(t, c, b0, wy0, np_eff, rows_eff);
-            const uint32_t buf = lt & 1;
-            // Slot barriers are tested by phase PARITY, and successive fills of one slot are consumed by
-            // different threads: a thread may only test fill n once fill n-1 is known to have landed.
-            // After this barrier every repack thread has passed its waits of the previous tile, and a
-            // slot's previous fill always belongs to an earlier tile (nslot > images per tile).
-            ptx::named_bar_sync(2, 128);
-            ptx::mbar_wait(A_EMPTY + 8 * buf, ((lt >> 1) & 1) ^ 1);   // MMA(lt-2) has consumed A[buf]
-            if (rt == 0) TRACE(4, lt);
+        auto rebuild_weight = [&](int c, uint32_t lt) {
             if (c != cur_c) {
                 if (lt > 0) ptx::mbar_wait(A_EMPTY + 8 * ((lt - 1) & 1), ((lt - 1) >> 1) & 1);   // MMA(lt-1) done with W_c
                 const uint16_t* Tc = T + (long long)c * Cf::NB;
@@ -442,17 +444,23 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __
                 ptx::fence_proxy_async_smem();
                 cur_c = c;
             }
-            if constexpr (WS == 14) {
-                // the next tile starts a new channel: have its table row in flight during this repack
-                if (t + 1 < t1 && (t + 1) - c * tl.tiles_per_c == tl.tiles_per_c) {
-                    table_to_regs14(T + (long long)(c + 1) * Cf::NB, reverse != 0, rt, tabv);
-                    tabv_ready = true;
-                }
-            }
+        };
+        for (int t = t0; t < t1; ++t, ++lt) {
+            int c, b0, wy0, np_eff, rows_eff;
+            tile_decode(t, c, b0, wy0, np_eff, rows_eff);
+            const uint32_t buf = lt & 1;
+            // Slot barriers are tested by phase PARITY, and successive fills of one slot are consumed by
+            // different threads: a thread may only test fill n once fill n-1 is known to have landed.
+            // After this barrier every repack thread has passed its waits of the previous tile, and a
+            // slot's previous fill always belongs to an earlier tile (nslot > images per tile).
+            ptx::named_bar_sync(2, 128);
+            ptx::mbar_wait(A_EMPTY + 8 * buf, ((lt >> 1) & 1) ^ 1);   // MMA(lt-2) has consumed A[buf]
+            if (rt == 0) TRACE(4, lt);
             const bool part = wl < wpf && pl < np_eff;               // this thread's frame image was loaded
             const bool valid = part && wy0 + wyl < g.nwh;
             const uint32_t kk = k + pl;
             const int slot = kk % nslot;
+            if (lt == 0) rebuild_weight(c, lt);   // first tile: build while its loads are in flight
             if (rt == 0) TRACE(5, lt);
             if (part) ptx::mbar_wait(FULL(slot), (kk / nslot) & 1);
             if (rt == 0) TRACE(6, lt);
@@ -461,38 +469,65 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __
             else
                 window_to_tmem<WS>(ring + (size_t)slot * tl.S + win_off, valid, rowB,
                                    tmem + buf * A_STRIDE + ((uint32_t)(q * 32) << 16));
+            if (part) ptx::mbar_arrive(EMPTY(slot));   // every window of this image is in TMEM
+            // W_c of a new channel is rebuilt AFTER this tile's windows are in TMEM, so the copy above
+            // overlaps the last MMA of the previous channel.
+            if (lt > 0) rebuild_weight(c, lt);
             ptx::tc_fence_before_sync();
             ptx::mbar_arrive(A_FULL + 8 * buf);
-            if (part) ptx::mbar_arrive(EMPTY(slot));   // every window of this image is in TMEM
             if (rt == 0) TRACE(7, lt);
             k += np_eff;
+            if constexpr (WS == 14) {
+                // the next tile starts a new channel: have its table row in flight during the next copy
+                if (t + 1 < t1 && (t + 1) - c * tl.tiles_per_c == tl.tiles_per_c) {
+                    table_to_regs14(T + (long long)(c + 1) * Cf::NB, reverse != 0, rt, tabv);
+                    tabv_ready = true;
+                }
+            }
         }
     } else if (warp < 10) {
         // ------------------------------------------------------------------ epilogue
         const int q = warp & 3;
         const int m = q * 32 + lane;
-        const int wl = m / tl.NP, pl = m % tl.NP;
+        const int pl = m / wpf, wl = m % wpf;
         const int wyl = wl / g.nww, wx = wl % g.nww;
-        uint8_t* win = outf + pl * tl.S + ((wyl * WS) * g.W + wx * WS) * 2;
+        const int win_off = ((wyl * WS) * g.W + wx * WS) * 2;
         GenAddr<GEN ? WS : 1> ga;
         if constexpr (GEN) gen_addr_init<WS>(ga, g, wyl, wx);
+        const int gq = m / og.lanes;                    // output group of this thread
+        const int pg = pl - gq * og.images;             // image inside the group
+        const uint32_t out_bytes = (uint32_t)og.images * tl.S;
         uint32_t lt = 0;
         for (int t = t0; t < t1; ++t, ++lt) {
             int c, b0, wy0, np_eff, rows_eff;
             tile_decode(t, c, b0, wy0, np_eff, rows_eff);
-            const bool valid = wl < wpf && pl < np_eff && wy0 + wyl < g.nwh;
-            ptx::mbar_wait(D_FULL, lt & 1);
-            if (m == 0) TRACE(8, lt);
-            ptx::mbar_wait(OUT_EMPTY, (lt & 1) ^ 1);     // the previous tile's stores have left the output frame
-            ptx::tc_fence_after_sync();
-            if constexpr (GEN)
-                tmem_to_window_gen<WS, BF16>(outf + pl * tl.S, ga, valid, ragged, tmem_d + ((uint32_t)(q * 32) << 16));
-            else
-                tmem_to_window<WS, BF16>(win, valid, rowB, tmem_d + ((uint32_t)(q * 32) << 16));
-            ptx::tc_fence_before_sync();
-            ptx::mbar_arrive(D_EMPTY);
-            ptx::fence_proxy_async_smem();
-            ptx::mbar_arrive(OUT_FULL + 8 * (lt & 1));
+            const bool valid = pl < np_eff && wy0 + wyl < g.nwh;
+            // group gq of tile lt is the j-th group this CTA produces; it goes to output buffer j mod nout
+            const uint32_t j = lt * og.n + gq, ob = j % nout, use = j / nout;
+            uint8_t* img = outb + (size_t)ob * out_bytes + (size_t)pg * tl.S;
+            auto drain_half = [&](auto hc) {
+                constexpr int h = decltype(hc)::value;
+                uint32_t pk[Hs::ncols(h) / 2];
+                ptx::mbar_wait(D_FULL + 8 * h, lt & 1);
+                if (m == 0 && h == 0) TRACE(8, lt);
+                ptx::tc_fence_after_sync();
+                tmem_cols_to_packed<BF16, Hs::ncols(h)>(tmem_d + Hs::col0(h) + ((uint32_t)(q * 32) << 16), pk);
+                ptx::tc_fence_before_sync();
+                ptx::mbar_arrive(D_EMPTY + 8 * h);                                 // the MMAs of the next tile may overwrite this half
+                if (h == 0) ptx::mbar_wait(OUT_EMPTY + 8 * ob, (use & 1) ^ 1);     // the buffer's previous contents have been read out
+                if (valid) {
+                    if constexpr (GEN) {
+                        if (ragged) packed_to_window_gen<WS, Hs::word0(h), Hs::word1(h), true>(img, ga, pk);
+                        else packed_to_window_gen<WS, Hs::word0(h), Hs::word1(h), false>(img, ga, pk);
+                    } else {
+                        packed_to_window<WS, Hs::word0(h), Hs::word1(h)>(img + win_off, rowB, pk);
+                    }
+                }
+            };
+            drain_half(std::integral_constant<int, 0>{});
+            if constexpr (Hs::NH > 1) drain_half(std::integral_constant<int, 1>{});
+            ptx::fence_proxy_async_smem();      // generic-proxy writes -> the bulk store's async-proxy reads
+            ptx::mbar_arrive(OUT_FULL + 8 * ob);
             if (m == 0) TRACE(9, lt);
         }
     } else {
@@ -504,26 +539,30 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __
             for (long long off = lane * 128ll; off < nbytes; off += 32 * 128)
                 asm volatile("prefetch.global.L2 [%0];" ::"l"(base + off));
         }
-        {
-            // lane p stores frame images p, p+32, ... of every tile
-            uint32_t lt = 0;
-            for (int t = t0; t < t1; ++t, ++lt) {
+        if (lane < nout) {
+            // Lane ob owns output buffer ob = output group ob of every tile (nout == og.n): it bulk-stores
+            // the group's images and releases the buffer once the copy engine has read it.  One lane per
+            // group, so waiting for the reads of one group never delays the stores of another.  The
+            // lanes always work on the same tile: lanes of one warp that spin on barriers several tiles
+            // apart starve one another (measured: a 5-buffer rotation hung), so nout is not made larger.
+            const uint32_t out_bytes = (uint32_t)og.images * tl.S;
+            const uint32_t ngroups = (uint32_t)(t1 - t0) * og.n;
+            for (uint32_t j = lane; j < ngroups; j += nout) {
+                const uint32_t lt = j / og.n, gq = j - lt * og.n;
                 int c, b0, wy0, np_eff, rows_eff;
-                tile_decode(t, c, b0, wy0, np_eff, rows_eff);
+                tile_decode(t0 + (int)lt, c, b0, wy0, np_eff, rows_eff);
                 const uint32_t bytes = (uint32_t)rows_eff * rowB;
-                ptx::mbar_wait(OUT_FULL + 8 * (lt & 1), (lt >> 1) & 1);
-                if (lane == 0) TRACE(10, lt);
-                for (int p = lane; p < np_eff; p += 32) {
+                ptx::mbar_wait(OUT_FULL + 8 * lane, (j / nout) & 1);
+                if (j == 0) TRACE(10, lt);
+                const int p_first = gq * og.images, p_end = min(p_first + og.images, np_eff);
+                for (int p = p_first; p < p_end; ++p) {
                     uint16_t* dst = y + ((long long)(b0 + p) * g.C + c) * plane_elems + (long long)wy0 * WS * g.W;
-                    ptx::bulk_s2g(dst, ptx::smem_u32(outf + p * tl.S), bytes);
+                    ptx::bulk_s2g(dst, ptx::smem_u32(outb + (size_t)lane * out_bytes + (size_t)(p - p_first) * tl.S), bytes);
                 }
                 ptx::bulk_commit();
                 ptx::bulk_wait_read<0>();
-                __syncwarp();
-                if (lane == 0) {
-                    TRACE(11, lt);
-                    ptx::mbar_arrive(OUT_EMPTY);
-                }
+                if (j == 0) TRACE(11, lt);
+                ptx::mbar_arrive(OUT_EMPTY + 8 * lane);
             }
             ptx::bulk_wait_all<0>();
         }
@@ -536,14 +575,22 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __
 #endif
 }
 
+// Shared memory left after W_c / tables / barriers is cut into frame-image slots: one output buffer
+// per output group (= one whole tile of output) and an input ring of `nslot` slots with the rest.
+// Returns false when a tile of output plus a tile + 1 of input does not fit.
 template <int WS>
-int bulk_slots(const TcTiles& tl)
+bool bulk_slots(const TcTiles& tl, int wpf, int* nslot, int* nout)
 {
-    const long long room = 227ll * 1024 - 1024 - BulkSmem<WS>::FIXED - (long long)tl.NP * tl.S;
-    long long n = room / tl.S;
-    if (n > 3 * tl.NP) n = 3 * tl.NP;
-    if (n > kMaxSlots) n = kMaxSlots;
-    return (int)n;
+    const OutGroups og = out_groups(tl, wpf);
+    const long long room = 227ll * 1024 - 1024 - BulkSmem<WS>::FIXED;
+    const long long total = room / tl.S;
+    long long ni = total - (long long)og.n * og.images;
+    if (ni > 3 * tl.NP) ni = 3 * tl.NP;
+    if (ni > kMaxSlots) ni = kMaxSlots;
+    if (ni < tl.NP + 1) return false;
+    *nslot = (int)ni;
+    *nout = og.n;
+    return true;
 }
 
 // 0 = not servable by the bulk kernel, 1 = aligned fast form, 2 = general form (shift / ragged).
@@ -554,7 +601,8 @@ int bulk_mode(const Geom& g, const TcTiles& tl, const void* x, const void* y)
     if (((long long)g.H * g.W * 2) % 16 != 0) return 0;
     if (reinterpret_cast<uintptr_t>(x) % 16 != 0 || reinterpret_cast<uintptr_t>(y) % 16 != 0) return 0;
     if (tl.NP > kMaxSlots || tl.ntiles > 0x3fffffffll) return 0;
-    if (bulk_slots<WS>(tl) < tl.NP + 1) return 0;
+    int nslot_, nout_;
+    if (!bulk_slots<WS>(tl, tl.NSY * g.nww, &nslot_, &nout_)) return 0;
     const bool plain = g.sh == 0 && g.sw == 0 && g.H == g.Hp && g.W == g.Wp;
     if (plain) return (tl.frame_rows * g.W * 2) % 16 == 0 ? 1 : (tl.nstrips == 1 ? 2 : 0);
     return tl.nstrips == 1 ? 2 : 0;
@@ -565,8 +613,10 @@ cudaError_t launch_bulk(const Geom& g, const TcTiles& tl, const void* x, const v
                         cudaStream_t s)
 {
     auto k = tc_bulk_kernel<WS, BF16, GEN>;
-    const int nslot = bulk_slots<WS>(tl);
-    const size_t smem = (size_t)BulkSmem<WS>::FIXED + (size_t)(tl.NP + nslot) * tl.S;
+    int nslot = 0, nout = 0;
+    const int wpf = tl.NSY * g.nww;
+    if (!bulk_slots<WS>(tl, wpf, &nslot, &nout)) return cudaErrorInvalidConfiguration;
+    const size_t smem = (size_t)BulkSmem<WS>::FIXED + (size_t)(nslot + nout * out_groups(tl, wpf).images) * tl.S;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     int grid = (int)(tl.ntiles < num_sms() ? tl.ntiles : num_sms());
@@ -596,7 +646,7 @@ cudaError_t launch_bulk(const Geom& g, const TcTiles& tl, const void* x, const v
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, k, g, tl, part, nslot, (const uint16_t*)x, (const uint16_t*)T, (uint16_t*)y,
+    return cudaLaunchKernelEx(&cfg, k, g, tl, part, nslot, nout, (const uint16_t*)x, (const uint16_t*)T, (uint16_t*)y,
                               reverse ? 1 : 0);
 }
 

@@ -70,11 +70,32 @@ __device__ __forceinline__ uint32_t pack2(uint32_t a, uint32_t b)
 }
 
 // Window -> TMEM A: all 32 lanes of the warp take part (tcgen05.st is warp-collective); lanes
-// without a window write zeros.
+// without a window write zeros (odd w) or whatever finite-or-not bytes `win` points at (even w:
+// unconditional loads -- the caller passes a legal address; row m of D depends on row m of A
+// only, and rows of lanes without a window are never stored).
 template <int WS>
 __device__ __forceinline__ void window_to_tmem(const uint8_t* win, bool valid, int rowB, uint32_t taddr)
 {
     using Cf = WinCfg<WS>;
+    if constexpr (WS % 2 == 0) {
+        // a window row is WS/2 aligned 32-bit words: one running row pointer, immediate offsets
+        constexpr int WPR = WS / 2;
+        uint32_t v[(Cf::A_COLS + 15) / 16 * 16];
+        const uint8_t* p = win;
+#pragma unroll
+        for (int r = 0; r < WS; ++r) {
+#pragma unroll
+            for (int k = 0; k < WPR; ++k) v[r * WPR + k] = *reinterpret_cast<const uint32_t*>(p + 4 * k);
+            p += rowB;
+        }
+#pragma unroll
+        for (int k = Cf::NW; k < (Cf::A_COLS + 15) / 16 * 16; ++k) v[k] = 0u;
+#pragma unroll
+        for (int ch = 0; ch < Cf::A_COLS / 16; ++ch) ptx::tmem_st16(taddr + ch * 16, v + ch * 16);
+        if constexpr (Cf::A_COLS % 16 != 0) ptx::tmem_st8(taddr + (Cf::A_COLS / 16) * 16, v + (Cf::A_COLS / 16) * 16);
+        ptx::tmem_wait_st();
+        return;
+    }
 #pragma unroll
     for (int ch = 0; ch < Cf::A_COLS / 16; ++ch) {
         uint32_t v[16];
@@ -119,6 +140,58 @@ __device__ __forceinline__ void tmem_to_window(uint8_t* win, bool valid, int row
                     store_word<WS>(win, rowB, wi, pack2<BF16>(v[2 * e], v[2 * e + 1]));
             }
         }
+    }
+}
+
+// The accumulator is drained in NH column ranges ("halves") so that the epilogue of one half
+// overlaps the MMAs of the other: w = 14 splits after output row 8 (112 | 84 positions), w = 7
+// is one range.  HalfCfg<WS, h>: first column, MMA N of the half, packed-word range.
+template <int WS>
+struct HalfSplit {
+    using Cf = WinCfg<WS>;
+    static constexpr int NH = (WS == 14) ? 2 : 1;
+    static constexpr int N0 = (WS == 14) ? 112 : Cf::N_PAD;                 // columns of half 0 (multiple of 16)
+    static constexpr int col0(int h) { return h == 0 ? 0 : N0; }
+    static constexpr int ncols(int h) { return h == 0 ? N0 : Cf::N_PAD - N0; }
+    static constexpr int word0(int h) { return col0(h) / 2; }
+    static constexpr int word1(int h) { return (col0(h) + ncols(h)) / 2 < Cf::NW ? (col0(h) + ncols(h)) / 2 : Cf::NW; }
+    static_assert(N0 % 16 == 0 && (Cf::N_PAD - N0) % 16 == 0, "halves are MMA-N legal");
+    static_assert(WS != 14 || N0 % (2 * WS) == 0, "the split falls on a window-row boundary");
+};
+
+// NCOLS fp32 accumulator columns (multiple of 16) -> NCOLS/2 packed 16-bit pairs (RNE).
+template <bool BF16, int NCOLS>
+__device__ __forceinline__ void tmem_cols_to_packed(uint32_t taddr, uint32_t* pk)
+{
+    static_assert(NCOLS % 16 == 0, "16-column chunks");
+#pragma unroll
+    for (int ch = 0; ch < NCOLS / 16; ch += 2) {
+        uint32_t v[32];
+        ptx::tmem_ld16(taddr + ch * 16, v);
+        if (ch + 1 < NCOLS / 16) ptx::tmem_ld16(taddr + (ch + 1) * 16, v + 16);
+        ptx::tmem_wait_ld();
+#pragma unroll
+        for (int e = 0; e < 16; ++e)
+            if (e < 8 || ch + 1 < NCOLS / 16) pk[ch * 8 + e] = pack2<BF16>(v[2 * e], v[2 * e + 1]);
+    }
+}
+
+// Packed words [W0, W1) of a window -> its frame position (aligned form).
+template <int WS, int W0, int W1>
+__device__ __forceinline__ void packed_to_window(uint8_t* win, int rowB, const uint32_t* pk)
+{
+    if constexpr (WS % 2 == 0) {
+        constexpr int WPR = WS / 2;
+        static_assert(W0 % WPR == 0, "starts on a window row");
+        uint8_t* p = win + (W0 / WPR) * rowB;
+#pragma unroll
+        for (int wi = W0; wi < W1; ++wi) {
+            *reinterpret_cast<uint32_t*>(p + 4 * (wi % WPR)) = pk[wi - W0];
+            if (wi % WPR == WPR - 1) p += rowB;
+        }
+    } else {
+#pragma unroll
+        for (int wi = W0; wi < W1; ++wi) store_word<WS>(win, rowB, wi, pk[wi - W0]);
     }
 }
 
@@ -228,6 +301,13 @@ __device__ __forceinline__ void tmem_to_window_gen_t(uint8_t* img, const GenAddr
     }
 }
 
+template <int WS, int W0, int W1, bool RAGGED>
+__device__ __forceinline__ void packed_to_window_gen(uint8_t* img, const GenAddr<WS>& a, const uint32_t* pk)
+{
+#pragma unroll
+    for (int wi = W0; wi < W1; ++wi) gen_store_word<WS, RAGGED>(img, a, wi, pk[wi - W0]);
+}
+
 template <int WS, bool BF16>
 __device__ __forceinline__ void tmem_to_window_gen(uint8_t* img, const GenAddr<WS>& a, bool valid, bool ragged, uint32_t taddr)
 {
@@ -238,6 +318,23 @@ __device__ __forceinline__ void tmem_to_window_gen(uint8_t* img, const GenAddr<W
 constexpr int kThreadsB = 352;
 constexpr int kMaxSlots = 96;
 constexpr int kMaxGrid = 160;
+constexpr int kMaxOutBufs = 16;  // output group buffers of the bulk kernel
+
+// Output hand-off groups of the bulk kernel: the smallest runs of whole epilogue warps that cover
+// whole frame images (MMA rows are image-major), so a group's images can be stored as soon as ITS
+// warps are done.  lanes per group, groups per tile, frame images per group.
+struct OutGroups { int lanes, n, images; };
+__host__ __device__ inline OutGroups out_groups(const TcTiles& tl, int wpf)
+{
+    OutGroups og;
+    og.lanes = 128;
+    for (int cand = 32; cand < 128; cand += cand)
+        if (cand % wpf == 0) { og.lanes = cand; break; }
+    og.n = 128 / og.lanes;
+    og.images = og.lanes % wpf == 0 ? og.lanes / wpf : tl.NP;
+    if (og.images > tl.NP) og.images = tl.NP;
+    return og;
+}
 
 // Static tile schedule: CTA b owns tiles [start[b], start[b+1]) (channel-major, so W_c is rebuilt
 // at most once or twice per CTA).  The host balances tiles + the cost of mid-range W_c rebuilds.
