@@ -604,8 +604,9 @@ int bulk_mode(const Geom& g, const TcTiles& tl, const void* x, const void* y)
     int nslot_, nout_;
     if (!bulk_slots<WS>(tl, tl.NSY * g.nww, &nslot_, &nout_)) return 0;
     const bool plain = g.sh == 0 && g.sw == 0 && g.H == g.Hp && g.W == g.Wp;
-    if (plain) return (tl.frame_rows * g.W * 2) % 16 == 0 ? 1 : (tl.nstrips == 1 ? 2 : 0);
-    return tl.nstrips == 1 ? 2 : 0;
+    if (plain && (tl.frame_rows * g.W * 2) % 16 == 0) return 1;
+    // general form: whole images in natural layout, word-granular window addressing (W, W' even)
+    return (tl.nstrips == 1 && g.W % 2 == 0 && g.Wp % 2 == 0) ? 2 : 0;
 }
 
 template <int WS, bool BF16, bool GEN>

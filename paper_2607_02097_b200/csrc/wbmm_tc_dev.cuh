@@ -69,6 +69,27 @@ __device__ __forceinline__ uint32_t pack2(uint32_t a, uint32_t b)
     }
 }
 
+// Aligned form: the window's N values, two per word in row-major in-window order, v[0 .. NW).
+// Even w: unconditional loads through one running row pointer (the caller passes a legal address).
+template <int WS>
+__device__ __forceinline__ void window_to_regs(const uint8_t* win, bool valid, int rowB, uint32_t* v)
+{
+    using Cf = WinCfg<WS>;
+    if constexpr (WS % 2 == 0) {
+        constexpr int WPR = WS / 2;
+        const uint8_t* p = win;
+#pragma unroll
+        for (int r = 0; r < WS; ++r) {
+#pragma unroll
+            for (int k = 0; k < WPR; ++k) v[r * WPR + k] = *reinterpret_cast<const uint32_t*>(p + 4 * k);
+            p += rowB;
+        }
+    } else {
+#pragma unroll
+        for (int wi = 0; wi < Cf::NW; ++wi) v[wi] = valid ? load_word<WS>(win, rowB, wi) : 0u;
+    }
+}
+
 // Window -> TMEM A: all 32 lanes of the warp take part (tcgen05.st is warp-collective); lanes
 // without a window write zeros (odd w) or whatever finite-or-not bytes `win` points at (even w:
 // unconditional loads -- the caller passes a legal address; row m of D depends on row m of A
@@ -196,13 +217,19 @@ __device__ __forceinline__ void packed_to_window(uint8_t* win, int rowB, const u
 }
 
 // General window addressing for whole-image frames held exactly as they sit in global memory
-// (row pitch W): the cyclic shift and the zero padding (Eq. 4-5; A6) become per-thread
-// row / column byte offsets plus validity bit masks (bit r / bit cc set = inside H x W).  Offsets
-// of padding rows / columns are clamped to 0 so every load address is legal; the value is masked.
+// (row pitch W elements, W and W' even): the cyclic shift and the zero padding (Eq. 4-5; DESIGN.md
+// A6) become per-thread byte offsets of the window's rows and of the NWR aligned 32-bit words that
+// cover one window row, plus validity masks.  Window column e of a thread sits at image column
+// (c0 + e) mod W', c0 = (wx*w + s_w) mod W'; with `odd` = c0 & 1 the aligned element pairs of the row
+// are  f_k = funnelshift_r(word_k, word_k+1, 16*odd).  Offsets of padding rows / words are 0 so that
+// every address is legal; their values are masked (loads) or skipped (stores).
 template <int WS>
 struct GenAddr {
-    int rowoff[WS], coloff[WS];
-    uint32_t rowmask, colmask;
+    static constexpr int NWR = WS / 2 + 1;          // image words that can hold one window row
+    int rowoff[WS];
+    int coloff[NWR];
+    uint32_t rowmask, colmask;                      // bit r / bit k set = inside H x W
+    uint32_t sh;                                    // 16 * odd
 };
 
 template <int WS>
@@ -216,103 +243,122 @@ __device__ __forceinline__ void gen_addr_init(GenAddr<WS>& a, const Geom& g, int
         a.rowoff[r] = h < g.H ? h * g.W * 2 : 0;
         a.rowmask |= (h < g.H ? 1u : 0u) << r;
     }
+    int c0 = wx * WS + g.sw;
+    if (c0 >= g.Wp) c0 -= g.Wp;
+    a.sh = (c0 & 1) * 16;
+    const int wbase = c0 >> 1, wpr = g.Wp >> 1, wreal = g.W >> 1;
 #pragma unroll
-    for (int cc = 0; cc < WS; ++cc) {
-        int v = wx * WS + cc + g.sw;
-        if (v >= g.Wp) v -= g.Wp;
-        a.coloff[cc] = v < g.W ? v * 2 : 0;
-        a.colmask |= (v < g.W ? 1u : 0u) << cc;
+    for (int k = 0; k < GenAddr<WS>::NWR; ++k) {
+        int wi = wbase + k;
+        if (wi >= wpr) wi -= wpr;
+        a.coloff[k] = wi < wreal ? wi * 4 : 0;
+        a.colmask |= (wi < wreal ? 1u : 0u) << k;
     }
 }
 
-// RAGGED = false: every window element lies inside H x W (no padding anywhere), masks unused.
-template <int WS, bool RAGGED>
-__device__ __forceinline__ uint32_t gen_load_word(const uint8_t* img, const GenAddr<WS>& a, uint32_t rm, int wi)
+// lo half of the result = half `ha` of a, hi half = half `hb` of b
+template <int HA, int HB>
+__device__ __forceinline__ uint32_t pick_halves(uint32_t a, uint32_t b)
 {
-    const int e0 = 2 * wi, e1 = 2 * wi + 1;
-    uint32_t lo = *reinterpret_cast<const uint16_t*>(img + a.rowoff[e0 / WS] + a.coloff[e0 % WS]);
-    if (RAGGED && !((rm >> (e0 / WS)) & (a.colmask >> (e0 % WS)) & 1u)) lo = 0;
-    uint32_t hi = 0;
-    if (e1 < WS * WS) {
-        hi = *reinterpret_cast<const uint16_t*>(img + a.rowoff[e1 / WS] + a.coloff[e1 % WS]);
-        if (RAGGED && !((rm >> (e1 / WS)) & (a.colmask >> (e1 % WS)) & 1u)) hi = 0;
-    }
-    return lo | (hi << 16);
+    return __byte_perm(a, b, (HA ? 0x32 : 0x10) | ((HB ? 0x76 : 0x54) << 8));
 }
 
+// The window's N values, two per word in row-major in-window order, v[0 .. NW).  RAGGED = false:
+// every window element lies inside H x W (no masks).
 template <int WS, bool RAGGED>
-__device__ __forceinline__ void gen_store_word(uint8_t* img, const GenAddr<WS>& a, int wi, uint32_t v)
+__device__ __forceinline__ void window_to_regs_gen(const uint8_t* img, const GenAddr<WS>& a, bool valid, uint32_t* v)
 {
-    const int e0 = 2 * wi, e1 = 2 * wi + 1;
-    if (!RAGGED || ((a.rowmask >> (e0 / WS)) & (a.colmask >> (e0 % WS)) & 1u))
-        *reinterpret_cast<uint16_t*>(img + a.rowoff[e0 / WS] + a.coloff[e0 % WS]) = (uint16_t)(v & 0xffffu);
-    if (e1 < WS * WS) {
-        if (!RAGGED || ((a.rowmask >> (e1 / WS)) & (a.colmask >> (e1 % WS)) & 1u))
-            *reinterpret_cast<uint16_t*>(img + a.rowoff[e1 / WS] + a.coloff[e1 % WS]) = (uint16_t)(v >> 16);
-    }
-}
-
-template <int WS, bool RAGGED>
-__device__ __forceinline__ void window_to_tmem_gen_t(const uint8_t* img, const GenAddr<WS>& a, uint32_t rm, uint32_t taddr)
-{
-    using Cf = WinCfg<WS>;
+    constexpr int NWR = GenAddr<WS>::NWR, NF = (WS + 1) / 2;
+    const uint32_t rm = valid ? a.rowmask : 0u;
 #pragma unroll
-    for (int ch = 0; ch < (Cf::A_COLS + 15) / 16; ++ch) {
-        uint32_t v[16];
+    for (int r = 0; r < WS; ++r) {
+        const uint8_t* p = img + a.rowoff[r];
+        uint32_t w[NWR + 1];
 #pragma unroll
-        for (int e = 0; e < 16; ++e) {
-            const int wi = ch * 16 + e;
-            v[e] = wi < Cf::NW ? gen_load_word<WS, RAGGED>(img, a, rm, wi) : 0u;
+        for (int k = 0; k < NWR; ++k) {
+            w[k] = *reinterpret_cast<const uint32_t*>(p + a.coloff[k]);
+            if (RAGGED && !((rm >> r) & (a.colmask >> k) & 1u)) w[k] = 0u;
         }
-        if (ch * 16 + 16 <= Cf::A_COLS) ptx::tmem_st16(taddr + ch * 16, v);
-        else ptx::tmem_st8(taddr + ch * 16, v);
+        w[NWR] = 0u;
+        uint32_t f[NF + 1];                        // aligned element pairs (e_2k, e_2k+1) of this row
+#pragma unroll
+        for (int k = 0; k < NF; ++k) f[k] = __funnelshift_r(w[k], w[k + 1], a.sh);
+        f[NF] = 0u;
+        // row r starts at linear position L = r*WS
+        const int L = r * WS;
+        if (L % 2 == 0) {
+#pragma unroll
+            for (int k = 0; k < WS / 2; ++k) v[L / 2 + k] = f[k];
+            if (WS % 2 == 1) v[(L + WS - 1) / 2] = f[NF - 1] & 0xffffu;       // last element; the next row fills the high half
+        } else {
+            v[(L - 1) / 2] |= f[0] << 16;                                      // first element -> high half of the previous word
+#pragma unroll
+            for (int k = 0; k < WS / 2; ++k) v[(L + 1) / 2 + k] = __funnelshift_r(f[k], f[k + 1], 16);   // (e_2k+1, e_2k+2)
+        }
+    }
+    if (!RAGGED && !valid) {
+#pragma unroll
+        for (int k = 0; k < WinCfg<WS>::NW; ++k) v[k] = 0u;
     }
 }
 
-// tcgen05.st is warp-collective: every lane runs the same instruction stream; a lane without a
-// window (or a ragged problem) takes the masked form, chosen warp-uniformly.
 template <int WS>
 __device__ __forceinline__ void window_to_tmem_gen(const uint8_t* img, const GenAddr<WS>& a, bool valid, bool ragged,
                                                    uint32_t taddr)
 {
-    const bool masked = ragged || !__all_sync(0xffffffffu, valid);
-    if (masked) window_to_tmem_gen_t<WS, true>(img, a, valid ? a.rowmask : 0u, taddr);
-    else window_to_tmem_gen_t<WS, false>(img, a, 0u, taddr);
+    using Cf = WinCfg<WS>;
+    constexpr int NV = (Cf::A_COLS + 15) / 16 * 16;
+    uint32_t v[NV];
+    if (ragged) window_to_regs_gen<WS, true>(img, a, valid, v);
+    else window_to_regs_gen<WS, false>(img, a, valid, v);
+#pragma unroll
+    for (int k = Cf::NW; k < NV; ++k) v[k] = 0u;
+#pragma unroll
+    for (int ch = 0; ch < Cf::A_COLS / 16; ++ch) ptx::tmem_st16(taddr + ch * 16, v + ch * 16);
+    if constexpr (Cf::A_COLS % 16 != 0) ptx::tmem_st8(taddr + (Cf::A_COLS / 16) * 16, v + (Cf::A_COLS / 16) * 16);
     ptx::tmem_wait_st();
 }
 
-template <int WS, bool BF16, bool RAGGED>
-__device__ __forceinline__ void tmem_to_window_gen_t(uint8_t* img, const GenAddr<WS>& a, bool valid, uint32_t taddr)
-{
-    using Cf = WinCfg<WS>;
-    constexpr int NCH = (Cf::NW + 7) / 8;
-#pragma unroll
-    for (int ch = 0; ch < NCH; ++ch) {
-        uint32_t v[16];
-        ptx::tmem_ld16(taddr + ch * 16, v);
-        ptx::tmem_wait_ld();
-        if (valid) {
-#pragma unroll
-            for (int e = 0; e < 8; ++e) {
-                const int wi = ch * 8 + e;
-                if (wi < Cf::NW) gen_store_word<WS, RAGGED>(img, a, wi, pack2<BF16>(v[2 * e], v[2 * e + 1]));
-            }
-        }
-    }
-}
-
+// Packed words [W0, W1) of a window (pk[0] = word W0; the range covers whole window rows, or the
+// whole window) -> the window's place in the natural-layout frame.
 template <int WS, int W0, int W1, bool RAGGED>
 __device__ __forceinline__ void packed_to_window_gen(uint8_t* img, const GenAddr<WS>& a, const uint32_t* pk)
 {
+    constexpr int NWR = GenAddr<WS>::NWR, NF = (WS + 1) / 2;
+    constexpr int R0 = (2 * W0) / WS, R1 = (2 * W1 + WS - 1) / WS < WS ? (2 * W1 + WS - 1) / WS : WS;
+    static_assert((2 * W0) % WS == 0, "the range starts on a window row");
+    const int odd = a.sh >> 4;
 #pragma unroll
-    for (int wi = W0; wi < W1; ++wi) gen_store_word<WS, RAGGED>(img, a, wi, pk[wi - W0]);
-}
-
-template <int WS, bool BF16>
-__device__ __forceinline__ void tmem_to_window_gen(uint8_t* img, const GenAddr<WS>& a, bool valid, bool ragged, uint32_t taddr)
-{
-    if (ragged) tmem_to_window_gen_t<WS, BF16, true>(img, a, valid, taddr);
-    else tmem_to_window_gen_t<WS, BF16, false>(img, a, valid, taddr);
+    for (int r = R0; r < R1; ++r) {
+        // aligned element pairs of the row from the linear packed words
+        uint32_t f[NF + 2];
+        f[0] = 0u;                                  // f[k+1] = (e_2k, e_2k+1); f[0] and f[NF+1] are zero pads
+        const int L = r * WS;
+#pragma unroll
+        for (int k = 0; k < NF; ++k) {
+            const int i0 = L + 2 * k, i1 = i0 + 1;                 // linear positions of the pair
+            const uint32_t wa = pk[i0 / 2 - W0];
+            const uint32_t wb = (2 * k + 1 < WS) ? pk[i1 / 2 - W0] : 0u;
+            if (i0 % 2 == 0) f[k + 1] = (2 * k + 1 < WS) ? wa : (wa & 0xffffu);
+            else f[k + 1] = (2 * k + 1 < WS) ? __funnelshift_r(wa, wb, 16) : (wa >> 16);
+        }
+        f[NF + 1] = 0u;
+        uint8_t* p = img + a.rowoff[r];
+        const bool rv = !RAGGED || ((a.rowmask >> r) & 1u);
+#pragma unroll
+        for (int k = 0; k < NWR; ++k) {
+            // image word k holds window elements ea = 2k - odd (low half) and ea + 1 (high half)
+            const uint32_t val = __funnelshift_l(f[k], k + 1 <= NF ? f[k + 1] : 0u, a.sh);
+            const int ea = 2 * k - odd;
+            const bool ok = rv && (!RAGGED || ((a.colmask >> k) & 1u));
+            uint8_t* q = p + a.coloff[k];
+            if (ok) {
+                if (ea >= 0 && ea + 1 < WS) *reinterpret_cast<uint32_t*>(q) = val;
+                else if (ea < 0) *reinterpret_cast<uint16_t*>(q + 2) = (uint16_t)(val >> 16);
+                else if (ea < WS) *reinterpret_cast<uint16_t*>(q) = (uint16_t)(val & 0xffffu);
+            }
+        }
+    }
 }
 
 constexpr int kThreadsB = 352;

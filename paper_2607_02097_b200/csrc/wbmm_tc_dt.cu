@@ -176,18 +176,23 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
             if (part) ptx::mbar_wait(FULL(slot), (kk / nslot) & 1);
             ptx::mbar_wait(STAGE_EMPTY, (lt & 1) ^ 1);      // MMA(lt-1) has read the stage
             const uint8_t* img = ring + (size_t)slot * tl.S;
+            {
+                uint32_t wv[Dc::NV * 4];
+                if constexpr (GEN) {
+                    if (ragged) window_to_regs_gen<WS, true>(img, ga, valid, wv);
+                    else window_to_regs_gen<WS, false>(img, ga, valid, wv);
+                } else {
+                    window_to_regs<WS>(valid ? img + win_off : img, valid, rowB, wv);
+                    if (WS % 2 == 0 && !valid) {
 #pragma unroll
-            for (int v = 0; v < Dc::NV; ++v) {
-                uint32_t wv[4];
-#pragma unroll
-                for (int e = 0; e < 4; ++e) {
-                    const int wi = v * 4 + e;
-                    if (wi >= Cf::NW || !valid) wv[e] = 0u;
-                    else if constexpr (GEN) wv[e] = ragged ? gen_load_word<WS, true>(img, ga, ga.rowmask, wi)
-                                                           : gen_load_word<WS, false>(img, ga, 0u, wi);
-                    else wv[e] = load_word<WS>(img + win_off, rowB, wi);
+                        for (int e = 0; e < Cf::NW; ++e) wv[e] = 0u;
+                    }
                 }
-                *reinterpret_cast<uint4*>(dst + v * Dc::SBO) = make_uint4(wv[0], wv[1], wv[2], wv[3]);
+#pragma unroll
+                for (int e = Cf::NW; e < Dc::NV * 4; ++e) wv[e] = 0u;
+#pragma unroll
+                for (int v = 0; v < Dc::NV; ++v)
+                    *reinterpret_cast<uint4*>(dst + v * Dc::SBO) = make_uint4(wv[4 * v], wv[4 * v + 1], wv[4 * v + 2], wv[4 * v + 3]);
             }
             ptx::fence_proxy_async_smem();
             ptx::mbar_arrive(STAGE_FULL);
@@ -265,8 +270,9 @@ int dt_mode(const Geom& g, const TcTiles& tl, const void* x, const void* dy)
     if (tl.ntiles > 0x3fffffffll) return 0;
     if (dt_slots<WS>(tl) < 2 * tl.NP + 1) return 0;
     const bool plain = g.sh == 0 && g.sw == 0 && g.H == g.Hp && g.W == g.Wp;
-    if (plain) return (tl.frame_rows * g.W * 2) % 16 == 0 ? 1 : (tl.nstrips == 1 ? 2 : 0);
-    return tl.nstrips == 1 ? 2 : 0;
+    if (plain && (tl.frame_rows * g.W * 2) % 16 == 0) return 1;
+    // general form: whole images in natural layout, word-granular window addressing (W, W' even)
+    return (tl.nstrips == 1 && g.W % 2 == 0 && g.Wp % 2 == 0) ? 2 : 0;
 }
 
 template <int WS, bool BF16, bool GEN>
