@@ -12,6 +12,7 @@
 //     l.17) are pure address arithmetic.
 #include "wbmm_tc.cuh"
 
+#include <cstdlib>
 #include <mutex>
 #include <type_traits>
 
@@ -185,11 +186,9 @@ tc_generic_kernel(Geom g, TcTiles tl, const uint16_t* __restrict__ x, const uint
 // Each 32-bit shared-memory access of the repack / epilogue warps is conflict-free for the
 // headline geometry: lanes are (4 adjacent windows) x (8 images) and the image stride is 16*odd bytes.
 
-// W_c for w = 14 from two copies of the fully reversed table F[q] = T[NB-1-q] (F0 = F, F1 = F
-// shifted by one value), so that any pair (F[q], F[q+1]) is one aligned 32-bit load.  Row i of W_c
-// is, for every input row rj, the run F[q0 + 27*rj + cj], cj = 0..13, q0 = (13-ri)*27 + 13-ci
-// (Eq. 7 rewritten for the reversed table).  128 threads (the repack warps); rows >= N and chunk
-// 25 stay zero from the kernel prologue.
+// The table row of a channel is staged in shared memory as two copies of the fully reversed table
+// F[q] = T[NB-1-q] (F0 = F, F1 = F shifted by one value), so that any pair (F[q], F[q+1]) is one
+// aligned 32-bit load whatever the parity of q.
 constexpr int kTabRegs = (WinCfg<14>::NB + 127) / 128;
 
 // The (reversed) table row of one channel, 128 threads -> registers (loads only; no use yet).
@@ -203,9 +202,13 @@ __device__ __forceinline__ void table_to_regs14(const uint16_t* __restrict__ Tc,
     }
 }
 
-__device__ __forceinline__ void build_weight14(const uint16_t* v, uint16_t* F0, uint16_t* F1, uint8_t* Wc, int tid)
+// Block-Toeplitz library for w = 14 (BulkCfg<14>) from the two staged copies of the reversed table
+// (see build_weight14): chunk (d, ci, kc) = Z[d-13][ci][8kc .. 8kc+7] = F[(26-d)*27 + 13-ci + 8kc + e].
+// 128 threads (the repack warps); rows ci = 14, 15 of every block stay zero from the kernel prologue.
+__device__ __forceinline__ void build_lib14(const uint16_t* v, uint16_t* F0, uint16_t* F1, uint8_t* lib, int tid)
 {
     using Cf = WinCfg<14>;
+    using Bc = BulkCfg<14>;
 #pragma unroll
     for (int u = 0; u < kTabRegs; ++u) {
         const int q = tid + u * 128;
@@ -215,32 +218,12 @@ __device__ __forceinline__ void build_weight14(const uint16_t* v, uint16_t* F0, 
         }
     }
     ptx::named_bar_sync(2, 128);
-    for (int i = tid; i < Cf::N; i += 128) {
-        const int ri = i / 14, ci = i % 14;
-        const int q0 = (13 - ri) * 27 + 13 - ci, p0 = q0 & 1;
-        const uint8_t* be = reinterpret_cast<const uint8_t*>(p0 ? F1 : F0) + (q0 - p0) * 2;   // even rj
-        const uint8_t* bo = reinterpret_cast<const uint8_t*>(p0 ? F0 : F1) + (q0 + p0) * 2;   // odd rj
-        uint8_t* dst = Wc + i * 16;
-        constexpr int BATCH = 5;     // chunks whose loads are all issued before the first store
-#pragma unroll
-        for (int k0 = 0; k0 < 25; k0 += BATCH) {
-            uint32_t pk[BATCH][4];
-#pragma unroll
-            for (int kb = 0; kb < BATCH; ++kb) {
-#pragma unroll
-                for (int e = 0; e < 4; ++e) {
-                    const int j = (k0 + kb) * 8 + 2 * e;
-                    const int rj = j / 14, cj = j % 14;
-                    if (k0 + kb >= 25 || j >= Cf::N) pk[kb][e] = 0u;
-                    else if (rj % 2 == 0) pk[kb][e] = *reinterpret_cast<const uint32_t*>(be + (27 * rj + cj) * 2);
-                    else pk[kb][e] = *reinterpret_cast<const uint32_t*>(bo + (27 * rj - 1 + cj) * 2);
-                }
-            }
-#pragma unroll
-            for (int kb = 0; kb < BATCH; ++kb)
-                if (k0 + kb < 25)
-                    *reinterpret_cast<uint4*>(dst + (k0 + kb) * Cf::LBO) = make_uint4(pk[kb][0], pk[kb][1], pk[kb][2], pk[kb][3]);
-        }
+    for (int id = tid; id < 27 * 28; id += 128) {
+        const int d = id / 28, rem = id - d * 28, ci = rem >> 1, kc = rem & 1;
+        const int q0 = (26 - d) * 27 + 13 - ci + 8 * kc, p0 = q0 & 1;
+        const uint32_t* src = reinterpret_cast<const uint32_t*>(reinterpret_cast<const uint8_t*>(p0 ? F1 : F0) + (q0 - p0) * 2);
+        const uint32_t w0 = src[0], w1 = src[1], w2 = src[2], w3 = kc ? 0u : src[3];   // cj = 14, 15 are padding
+        *reinterpret_cast<uint4*>(lib + kc * Bc::LBO + (d * 16 + ci) * 16) = make_uint4(w0, w1, w2, w3);
     }
 }
 
@@ -250,7 +233,7 @@ struct BulkSmem {
     static constexpr int TAB_ONE = ((Cf::NB + 2) * 2 + 15) / 16 * 16;
     static constexpr int TAB_BYTES = 2 * TAB_ONE;                              // F0 and F1 (or Ts for the generic builder)
     static constexpr int BAR_BYTES = (2 * kMaxSlots + 8 + 2 * kMaxOutBufs) * 8;
-    static constexpr int FIXED = Cf::WC_BYTES + TAB_BYTES + BAR_BYTES;
+    static constexpr int FIXED = BulkCfg<WS>::WC_BYTES + TAB_BYTES + BAR_BYTES;
 };
 
 template <int WS, bool BF16, bool GEN>
@@ -262,8 +245,9 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
     using Sm = BulkSmem<WS>;
     extern __shared__ __align__(1024) uint8_t smem[];
     uint8_t* Wc = smem;
-    uint16_t* tab = reinterpret_cast<uint16_t*>(smem + Cf::WC_BYTES);
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + Cf::WC_BYTES + Sm::TAB_BYTES);
+    using Bc = BulkCfg<WS>;
+    uint16_t* tab = reinterpret_cast<uint16_t*>(smem + Bc::WC_BYTES);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + Bc::WC_BYTES + Sm::TAB_BYTES);
     uint8_t* ring = smem + Sm::FIXED;                       // input ring: nslot frame-image slots
     uint8_t* outb = ring + (size_t)nslot * tl.S;            // output ring: nout group buffers of og.images frame images
     __shared__ uint32_t tmem_base_s;
@@ -278,7 +262,8 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
     // A_FULL[2] A_EMPTY[2] D_FULL[2] D_EMPTY[2] OUT_FULL[nout] OUT_EMPTY[nout]
     const uint32_t A_FULL = bar0 + 8u * (2 * kMaxSlots), A_EMPTY = A_FULL + 16, D_FULL = A_FULL + 32, D_EMPTY = A_FULL + 48,
                    OUT_FULL = A_FULL + 64, OUT_EMPTY = OUT_FULL + 8 * kMaxOutBufs;
-    using Hs = HalfSplit<WS>;
+    using Hs = BulkCfg<WS>;
+    constexpr bool WG = GEN || (WS % 2 == 1);   // word-granular window addressing (GenAddr)
 
     const int wpf = tl.NSY * g.nww;   // windows per frame image
     // Output hand-off groups: the smallest runs of whole epilogue warps that cover whole frame images
@@ -307,13 +292,9 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
         ptx::fence_mbar_init();
         TRACE(2, 15);
     }
-    if constexpr (WS == 14) {
-        // build_weight14 writes rows < N of chunks 0..24 only: zero the padding rows and the last chunk once
-        constexpr int PADR = Cf::N_PAD - Cf::N;
-        for (int i = tid; i < PADR * 25 + Cf::N_PAD; i += kThreadsB) {
-            const int kc = i < PADR * 25 ? i / PADR : 25, row = i < PADR * 25 ? Cf::N + i % PADR : i - PADR * 25;
-            *reinterpret_cast<uint4*>(Wc + kc * Cf::LBO + row * 16) = make_uint4(0, 0, 0, 0);
-        }
+    if constexpr (Bc::TOEP) {
+        // build_lib14 never writes the padding rows ci = 14, 15 of the blocks: zero the library once
+        for (int i = tid; i < Bc::WC_BYTES / 16; i += kThreadsB) reinterpret_cast<uint4*>(Wc)[i] = make_uint4(0, 0, 0, 0);
     }
     for (int i = tid; i < Sm::TAB_BYTES / 4; i += kThreadsB) reinterpret_cast<uint32_t*>(tab)[i] = 0u;
     ptx::fence_proxy_async_smem();
@@ -330,9 +311,9 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
     if (tid == 0 && blockIdx.x < 148) g_blk[blockIdx.x * 4 + 1] = gtime();
 #endif
     const uint32_t tmem = tmem_base_s;
-    constexpr uint32_t A_STRIDE = (Cf::A_COLS + 31) / 32 * 32;
+    constexpr uint32_t A_STRIDE = (Bc::A_COLS + 31) / 32 * 32;
     const uint32_t tmem_d = tmem + 2 * A_STRIDE;
-    static_assert(2 * ((Cf::A_COLS + 31) / 32 * 32) + Cf::N_PAD <= 512, "TMEM budget");
+    static_assert(2 * ((Bc::A_COLS + 31) / 32 * 32) + Bc::D_COLS <= 512, "TMEM budget");
 
     const int t0 = part_.start[blockIdx.x], t1 = part_.start[blockIdx.x + 1];
     const int rowB = g.W * 2;
@@ -386,8 +367,8 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                     ptx::tc_fence_after_sync();
                     const uint32_t idesc = ptx::idesc_f16(BF16 ? 1 : 0, 128, Hs::ncols(h));
 #pragma unroll
-                    for (int ks = 0; ks < Cf::KSTEPS; ++ks) {
-                        const uint64_t bdesc = ptx::smem_desc_kmajor_noswz(wc_addr + ks * 2 * Cf::LBO + Hs::col0(h) * 16, Cf::LBO, 128);
+                    for (int ks = 0; ks < Bc::KSTEPS; ++ks) {
+                        const uint64_t bdesc = ptx::smem_desc_kmajor_noswz(wc_addr + Bc::b_off(ks, h), Bc::LBO, 128);
                         ptx::mma_ts(tmem_d + Hs::col0(h), tmem_a + ks * 8, bdesc, idesc, ks > 0 ? 1u : 0u);
                     }
                     ptx::mma_commit(D_FULL + 8 * h);
@@ -404,8 +385,9 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
         const int pl = m / wpf, wl = m % wpf;   // image-major: a warp covers few images, so slots are consumed and released as they land
         const int wyl = wl / g.nww, wx = wl % g.nww;
         const int win_off = wl < wpf ? ((wyl * WS) * g.W + wx * WS) * 2 : 0;   // lanes without a window read a legal address
-        GenAddr<GEN ? WS : 1> ga;
+        GenAddr<WG ? WS : 1> ga;
         if constexpr (GEN) gen_addr_init<WS>(ga, g, wyl, wx);
+        else if constexpr (WG) gen_addr_init_plain<WS>(ga, g.W, wyl, wx);
         uint32_t k = 0, lt = 0;
         int cur_c = -1;
         uint16_t tabv[kTabRegs];
@@ -417,7 +399,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                 if (rt == 0) TRACE(12, lt);
                 if constexpr (WS == 14) {
                     if (!tabv_ready) table_to_regs14(Tc, reverse != 0, rt, tabv);
-                    build_weight14(tabv, tab, tab + Sm::TAB_ONE / 2, Wc, rt);
+                    build_lib14(tabv, tab, tab + Sm::TAB_ONE / 2, Wc, rt);
                     tabv_ready = false;
                 } else {
                     for (int kk = rt; kk < Cf::NB; kk += 128) tab[kk] = Tc[reverse ? Cf::NB - 1 - kk : kk];
@@ -464,11 +446,11 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
             if (rt == 0) TRACE(5, lt);
             if (part) ptx::mbar_wait(FULL(slot), (kk / nslot) & 1);
             if (rt == 0) TRACE(6, lt);
-            if constexpr (GEN)
-                window_to_tmem_gen<WS>(ring + (size_t)slot * tl.S, ga, valid, ragged, tmem + buf * A_STRIDE + ((uint32_t)(q * 32) << 16));
+            if constexpr (WG)
+                window_to_tmem_gen<WS>(ring + (size_t)slot * tl.S, ga, valid, GEN && ragged, tmem + buf * A_STRIDE + ((uint32_t)(q * 32) << 16));
             else
-                window_to_tmem<WS>(ring + (size_t)slot * tl.S + win_off, valid, rowB,
-                                   tmem + buf * A_STRIDE + ((uint32_t)(q * 32) << 16));
+                window_to_tmem_bulk<WS>(ring + (size_t)slot * tl.S + win_off, valid, rowB,
+                                        tmem + buf * A_STRIDE + ((uint32_t)(q * 32) << 16));
             if (part) ptx::mbar_arrive(EMPTY(slot));   // every window of this image is in TMEM
             // W_c of a new channel is rebuilt AFTER this tile's windows are in TMEM, so the copy above
             // overlaps the last MMA of the previous channel.
@@ -492,8 +474,9 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
         const int pl = m / wpf, wl = m % wpf;
         const int wyl = wl / g.nww, wx = wl % g.nww;
         const int win_off = ((wyl * WS) * g.W + wx * WS) * 2;
-        GenAddr<GEN ? WS : 1> ga;
+        GenAddr<WG ? WS : 1> ga;
         if constexpr (GEN) gen_addr_init<WS>(ga, g, wyl, wx);
+        else if constexpr (WG) gen_addr_init_plain<WS>(ga, g.W, wyl, wx);
         const int gq = m / og.lanes;                    // output group of this thread
         const int pg = pl - gq * og.images;             // image inside the group
         const uint32_t out_bytes = (uint32_t)og.images * tl.S;
@@ -502,22 +485,22 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
             int c, b0, wy0, np_eff, rows_eff;
             tile_decode(t, c, b0, wy0, np_eff, rows_eff);
             const bool valid = pl < np_eff && wy0 + wyl < g.nwh;
-            // group gq of tile lt is the j-th group this CTA produces; it goes to output buffer j mod nout
-            const uint32_t j = lt * og.n + gq, ob = j % nout, use = j / nout;
+            // the output frame is nout / og.n tiles deep: tile lt uses frame lt mod depth, group gq its buffer gq
+            const uint32_t otile = lt % (nout / og.n), ob = otile * og.n + gq, use = lt / (nout / og.n);
             uint8_t* img = outb + (size_t)ob * out_bytes + (size_t)pg * tl.S;
             auto drain_half = [&](auto hc) {
                 constexpr int h = decltype(hc)::value;
-                uint32_t pk[Hs::ncols(h) / 2];
+                uint32_t pk[Hs::TOEP ? 49 : Hs::ncols(h) / 2];
                 ptx::mbar_wait(D_FULL + 8 * h, lt & 1);
                 if (m == 0 && h == 0) TRACE(8, lt);
                 ptx::tc_fence_after_sync();
-                tmem_cols_to_packed<BF16, Hs::ncols(h)>(tmem_d + Hs::col0(h) + ((uint32_t)(q * 32) << 16), pk);
+                accum_half_to_packed<WS, BF16, h>(tmem_d + Hs::col0(h) + ((uint32_t)(q * 32) << 16), pk);
                 ptx::tc_fence_before_sync();
                 ptx::mbar_arrive(D_EMPTY + 8 * h);                                 // the MMAs of the next tile may overwrite this half
                 if (h == 0) ptx::mbar_wait(OUT_EMPTY + 8 * ob, (use & 1) ^ 1);     // the buffer's previous contents have been read out
                 if (valid) {
-                    if constexpr (GEN) {
-                        if (ragged) packed_to_window_gen<WS, Hs::word0(h), Hs::word1(h), true>(img, ga, pk);
+                    if constexpr (WG) {
+                        if (GEN && ragged) packed_to_window_gen<WS, Hs::word0(h), Hs::word1(h), true>(img, ga, pk);
                         else packed_to_window_gen<WS, Hs::word0(h), Hs::word1(h), false>(img, ga, pk);
                     } else {
                         packed_to_window<WS, Hs::word0(h), Hs::word1(h)>(img + win_off, rowB, pk);
@@ -540,20 +523,22 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                 asm volatile("prefetch.global.L2 [%0];" ::"l"(base + off));
         }
         if (lane < nout) {
-            // Lane ob owns output buffer ob = output group ob of every tile (nout == og.n): it bulk-stores
-            // the group's images and releases the buffer once the copy engine has read it.  One lane per
-            // group, so waiting for the reads of one group never delays the stores of another.  The
-            // lanes always work on the same tile: lanes of one warp that spin on barriers several tiles
-            // apart starve one another (measured: a 5-buffer rotation hung), so nout is not made larger.
+            // Lane ob = (frame, gq) owns output buffer ob: group gq of the tiles lt = frame mod depth.  It
+            // bulk-stores the group's images and releases the buffer once the copy engine has read it.
+            // One lane per buffer, so the ~1.4 us a store needs before its source may be overwritten is
+            // waited for in parallel.  (A single thread issuing everything in order and releasing a tile
+            // late measured 2 us slower per launch on cfg3; a rotation that put the lanes several tiles
+            // apart hung: every lane walks the tile loop in step and skips the tiles that are not its own.)
+            const uint32_t depth = nout / og.n, frame = lane / og.n, gq = lane - frame * og.n;
             const uint32_t out_bytes = (uint32_t)og.images * tl.S;
-            const uint32_t ngroups = (uint32_t)(t1 - t0) * og.n;
-            for (uint32_t j = lane; j < ngroups; j += nout) {
-                const uint32_t lt = j / og.n, gq = j - lt * og.n;
+            uint32_t lt = 0;
+            for (int t = t0; t < t1; ++t, ++lt) {
+                if (lt % depth != frame) continue;
                 int c, b0, wy0, np_eff, rows_eff;
-                tile_decode(t0 + (int)lt, c, b0, wy0, np_eff, rows_eff);
+                tile_decode(t, c, b0, wy0, np_eff, rows_eff);
                 const uint32_t bytes = (uint32_t)rows_eff * rowB;
-                ptx::mbar_wait(OUT_FULL + 8 * lane, (j / nout) & 1);
-                if (j == 0) TRACE(10, lt);
+                ptx::mbar_wait(OUT_FULL + 8 * lane, (lt / depth) & 1);
+                if (lane == 0) TRACE(10, lt);
                 const int p_first = gq * og.images, p_end = min(p_first + og.images, np_eff);
                 for (int p = p_first; p < p_end; ++p) {
                     uint16_t* dst = y + ((long long)(b0 + p) * g.C + c) * plane_elems + (long long)wy0 * WS * g.W;
@@ -561,7 +546,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                 }
                 ptx::bulk_commit();
                 ptx::bulk_wait_read<0>();
-                if (j == 0) TRACE(11, lt);
+                if (lane == 0) TRACE(11, lt);
                 ptx::mbar_arrive(OUT_EMPTY + 8 * lane);
             }
             ptx::bulk_wait_all<0>();
@@ -575,21 +560,28 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
 #endif
 }
 
-// Shared memory left after W_c / tables / barriers is cut into frame-image slots: one output buffer
-// per output group (= one whole tile of output) and an input ring of `nslot` slots with the rest.
+// Shared memory left after the weights / tables / barriers is cut into frame-image slots: an output
+// frame of one or two tiles (one buffer per output group and tile) and an input ring of `nslot` slots.
+// A bulk store takes ~1.4 us until its source may be overwritten, about as long as a load takes to
+// land, so the output side is two tiles deep whenever a tile + 1 of input still fits beside it.
 // Returns false when a tile of output plus a tile + 1 of input does not fit.
 template <int WS>
 bool bulk_slots(const TcTiles& tl, int wpf, int* nslot, int* nout)
 {
     const OutGroups og = out_groups(tl, wpf);
     const long long room = 227ll * 1024 - 1024 - BulkSmem<WS>::FIXED;
-    const long long total = room / tl.S;
-    long long ni = total - (long long)og.n * og.images;
-    if (ni > 3 * tl.NP) ni = 3 * tl.NP;
+    const long long total = room / tl.S, out_tile = (long long)og.n * og.images;
+    const int depth = (total - 2 * out_tile >= tl.NP + 1 && 2 * og.n <= kMaxOutBufs) ? 2 : 1;
+    long long ni = total - depth * out_tile;
+    // Two tiles of input for small frame images; for tiles of a few big images (>= 12 KB each) one
+    // tile + 1: more loads in flight measured SLOWER there (112 x 112 maps: 114 -> 104 us), as it does
+    // for a plain bulk-copy ring (profiles/r01_bulk_copy_microbench.md).
+    const long long in_cap = tl.NP >= 4 ? 2 * tl.NP : tl.NP + 1;
+    if (ni > in_cap) ni = in_cap;
     if (ni > kMaxSlots) ni = kMaxSlots;
     if (ni < tl.NP + 1) return false;
     *nslot = (int)ni;
-    *nout = og.n;
+    *nout = depth * og.n;
     return true;
 }
 
@@ -604,7 +596,7 @@ int bulk_mode(const Geom& g, const TcTiles& tl, const void* x, const void* y)
     int nslot_, nout_;
     if (!bulk_slots<WS>(tl, tl.NSY * g.nww, &nslot_, &nout_)) return 0;
     const bool plain = g.sh == 0 && g.sw == 0 && g.H == g.Hp && g.W == g.Wp;
-    if (plain && (tl.frame_rows * g.W * 2) % 16 == 0) return 1;
+    if (plain && (tl.frame_rows * g.W * 2) % 16 == 0 && (WS % 2 == 0 || g.W % 2 == 0)) return 1;   // odd w: rows must be word-aligned
     // general form: whole images in natural layout, word-granular window addressing (W, W' even)
     return (tl.nstrips == 1 && g.W % 2 == 0 && g.Wp % 2 == 0) ? 2 : 0;
 }
@@ -631,7 +623,7 @@ cudaError_t launch_bulk(const Geom& g, const TcTiles& tl, const void* x, const v
     {
         std::lock_guard<std::mutex> lock(mu);
         if (key_n != tl.ntiles || key_tpc != tl.tiles_per_c || key_grid != grid) {
-            cached_used = partition_tiles(tl, grid, 0.75, &cached);
+            cached_used = partition_tiles(tl, grid, WS == 14 ? 0.15 : 0.3, &cached);
             key_n = tl.ntiles; key_tpc = tl.tiles_per_c; key_grid = grid;
         }
         part = cached;

@@ -164,20 +164,56 @@ __device__ __forceinline__ void tmem_to_window(uint8_t* win, bool valid, int row
     }
 }
 
+// Operand geometry of the bulk kernel.
+//
+// w = 14 ("block-Toeplitz library"): W_c[(ri,ci),(rj,cj)] = T[c, (ri-rj+w-1)(2w-1) + (ci-cj+w-1)] (Eq. 7)
+// depends on the rows only through dr = ri - rj, so W_c is 14 x 14 blocks out of just 27 distinct
+// 14 x 14 Toeplitz blocks Z[dr].  With every window row padded to 16 positions on both GEMM axes
+// (K index = rj*16 + cj, N index = ri*16 + ci; the pads meet zero weights / are never stored), the
+// B operand of K-step rj is rows (13 - rj)*16 ... of ONE 432-row array
+//     lib[kc][(dr+13)*16 + ci][e] = Z[dr][ci][cj = 8*kc + e]      (K-major core matrices, 16-byte rows)
+// i.e. a plain descriptor with a different start address per K-step.  13.5 KB instead of the 86.5 KB
+// materialised W_c, and 864 16-byte chunks to build per channel instead of 4900.
+//
+// w = 7: the full K-major W_c (8 KB), as in WinCfg.
+//
 // The accumulator is drained in NH column ranges ("halves") so that the epilogue of one half
-// overlaps the MMAs of the other: w = 14 splits after output row 8 (112 | 84 positions), w = 7
-// is one range.  HalfCfg<WS, h>: first column, MMA N of the half, packed-word range.
+// overlaps the MMAs of the other.
 template <int WS>
-struct HalfSplit {
+struct BulkCfg {
     using Cf = WinCfg<WS>;
-    static constexpr int NH = (WS == 14) ? 2 : 1;
-    static constexpr int N0 = (WS == 14) ? 112 : Cf::N_PAD;                 // columns of half 0 (multiple of 16)
-    static constexpr int col0(int h) { return h == 0 ? 0 : N0; }
-    static constexpr int ncols(int h) { return h == 0 ? N0 : Cf::N_PAD - N0; }
-    static constexpr int word0(int h) { return col0(h) / 2; }
-    static constexpr int word1(int h) { return (col0(h) + ncols(h)) / 2 < Cf::NW ? (col0(h) + ncols(h)) / 2 : Cf::NW; }
-    static_assert(N0 % 16 == 0 && (Cf::N_PAD - N0) % 16 == 0, "halves are MMA-N legal");
-    static_assert(WS != 14 || N0 % (2 * WS) == 0, "the split falls on a window-row boundary");
+    static constexpr bool TOEP = false;
+    static constexpr int KSTEPS = Cf::KSTEPS;
+    static constexpr int A_COLS = Cf::A_COLS;          // 32-bit TMEM columns of one A buffer
+    static constexpr int D_COLS = Cf::N_PAD;
+    static constexpr int WC_BYTES = Cf::WC_BYTES;
+    static constexpr int LBO = Cf::LBO;
+    static constexpr int NH = 1;
+    static constexpr int ncols(int) { return D_COLS; }
+    static constexpr int col0(int) { return 0; }
+    static constexpr int word0(int) { return 0; }
+    static constexpr int word1(int) { return Cf::NW; }
+    // byte offset of the B operand of K-step ks, half h, inside the weight area
+    static constexpr int b_off(int ks, int) { return ks * 2 * LBO; }
+};
+
+template <>
+struct BulkCfg<14> {
+    using Cf = WinCfg<14>;
+    static constexpr bool TOEP = true;
+    static constexpr int RP = 16;                      // padded window row on both GEMM axes
+    static constexpr int KSTEPS = 14;                  // one input window row per tcgen05.mma (K = 16)
+    static constexpr int A_COLS = 14 * RP / 2;         // 112
+    static constexpr int D_COLS = 14 * RP;             // 224
+    static constexpr int LIB_ROWS = 27 * RP;           // 432
+    static constexpr int LBO = LIB_ROWS * 16;          // bytes between the two K chunks (cj 0-7 | 8-15)
+    static constexpr int WC_BYTES = 2 * LBO;           // 13824
+    static constexpr int NH = 2;                       // output rows 0-6 | 7-13
+    static constexpr int ncols(int) { return 7 * RP; }
+    static constexpr int col0(int h) { return h * 7 * RP; }
+    static constexpr int word0(int h) { return h * 49; }
+    static constexpr int word1(int h) { return (h + 1) * 49; }
+    static constexpr int b_off(int ks, int h) { return ((13 - ks) * RP + h * 7 * RP) * 16; }
 };
 
 // NCOLS fp32 accumulator columns (multiple of 16) -> NCOLS/2 packed 16-bit pairs (RNE).
@@ -194,6 +230,31 @@ __device__ __forceinline__ void tmem_cols_to_packed(uint32_t taddr, uint32_t* pk
 #pragma unroll
         for (int e = 0; e < 16; ++e)
             if (e < 8 || ch + 1 < NCOLS / 16) pk[ch * 8 + e] = pack2<BF16>(v[2 * e], v[2 * e + 1]);
+    }
+}
+
+// One half of the accumulator (BulkCfg<WS>::ncols(h) fp32 columns at taddr) -> packed 16-bit pairs
+// in row-major in-window order (the 2 pad columns of every padded row are dropped for w = 14).
+template <int WS, bool BF16, int H>
+__device__ __forceinline__ void accum_half_to_packed(uint32_t taddr, uint32_t* pk)
+{
+    using Bc = BulkCfg<WS>;
+    if constexpr (Bc::TOEP) {
+#pragma unroll
+        for (int r = 0; r < 7; r += 2) {
+            uint32_t v[32];
+            ptx::tmem_ld16(taddr + r * 16, v);
+            if (r + 1 < 7) ptx::tmem_ld16(taddr + (r + 1) * 16, v + 16);
+            ptx::tmem_wait_ld();
+#pragma unroll
+            for (int e = 0; e < 7; ++e) pk[r * 7 + e] = pack2<BF16>(v[2 * e], v[2 * e + 1]);
+            if (r + 1 < 7) {
+#pragma unroll
+                for (int e = 0; e < 7; ++e) pk[(r + 1) * 7 + e] = pack2<BF16>(v[16 + 2 * e], v[16 + 2 * e + 1]);
+            }
+        }
+    } else {
+        tmem_cols_to_packed<BF16, Bc::ncols(H)>(taddr, pk);
     }
 }
 
@@ -256,6 +317,20 @@ __device__ __forceinline__ void gen_addr_init(GenAddr<WS>& a, const Geom& g, int
     }
 }
 
+// The same descriptor for the aligned form (no shift, no padding; frame rows relative to the strip):
+// used for odd w, whose window rows start on odd columns for every other window.
+template <int WS>
+__device__ __forceinline__ void gen_addr_init_plain(GenAddr<WS>& a, int W, int wyl, int wx)
+{
+    a.rowmask = a.colmask = 0xffffffffu;
+#pragma unroll
+    for (int r = 0; r < WS; ++r) a.rowoff[r] = (wyl * WS + r) * W * 2;
+    const int c0 = wx * WS;
+    a.sh = (c0 & 1) * 16;
+#pragma unroll
+    for (int k = 0; k < GenAddr<WS>::NWR; ++k) a.coloff[k] = ((c0 >> 1) + k) * 4;
+}
+
 // lo half of the result = half `ha` of a, hi half = half `hb` of b
 template <int HA, int HB>
 __device__ __forceinline__ uint32_t pick_halves(uint32_t a, uint32_t b)
@@ -302,21 +377,47 @@ __device__ __forceinline__ void window_to_regs_gen(const uint8_t* img, const Gen
     }
 }
 
+// Linear packed window words v[0 .. NW) -> one A buffer of the bulk kernel (tcgen05.st, all 32
+// lanes).  w = 14: every window row is padded to 8 words, the last one zero (BulkCfg<14>).
+template <int WS>
+__device__ __forceinline__ void packed_window_to_tmem(const uint32_t* v, uint32_t taddr)
+{
+    using Bc = BulkCfg<WS>;
+    using Cf = WinCfg<WS>;
+    constexpr int NV = (Bc::A_COLS + 15) / 16 * 16;
+    uint32_t u[NV];
+    if constexpr (Bc::TOEP) {
+#pragma unroll
+        for (int r = 0; r < WS; ++r) {
+#pragma unroll
+            for (int k = 0; k < 8; ++k) u[r * 8 + k] = k < 7 ? v[r * 7 + k] : 0u;
+        }
+    } else {
+#pragma unroll
+        for (int k = 0; k < NV; ++k) u[k] = k < Cf::NW ? v[k] : 0u;
+    }
+#pragma unroll
+    for (int ch = 0; ch < Bc::A_COLS / 16; ++ch) ptx::tmem_st16(taddr + ch * 16, u + ch * 16);
+    if constexpr (Bc::A_COLS % 16 != 0) ptx::tmem_st8(taddr + (Bc::A_COLS / 16) * 16, u + (Bc::A_COLS / 16) * 16);
+    ptx::tmem_wait_st();
+}
+
+template <int WS>
+__device__ __forceinline__ void window_to_tmem_bulk(const uint8_t* win, bool valid, int rowB, uint32_t taddr)
+{
+    uint32_t v[WinCfg<WS>::NW];
+    window_to_regs<WS>(win, valid, rowB, v);
+    packed_window_to_tmem<WS>(v, taddr);
+}
+
 template <int WS>
 __device__ __forceinline__ void window_to_tmem_gen(const uint8_t* img, const GenAddr<WS>& a, bool valid, bool ragged,
                                                    uint32_t taddr)
 {
-    using Cf = WinCfg<WS>;
-    constexpr int NV = (Cf::A_COLS + 15) / 16 * 16;
-    uint32_t v[NV];
+    uint32_t v[WinCfg<WS>::NW];
     if (ragged) window_to_regs_gen<WS, true>(img, a, valid, v);
     else window_to_regs_gen<WS, false>(img, a, valid, v);
-#pragma unroll
-    for (int k = Cf::NW; k < NV; ++k) v[k] = 0u;
-#pragma unroll
-    for (int ch = 0; ch < Cf::A_COLS / 16; ++ch) ptx::tmem_st16(taddr + ch * 16, v + ch * 16);
-    if constexpr (Cf::A_COLS % 16 != 0) ptx::tmem_st8(taddr + (Cf::A_COLS / 16) * 16, v + (Cf::A_COLS / 16) * 16);
-    ptx::tmem_wait_st();
+    packed_window_to_tmem<WS>(v, taddr);
 }
 
 // Packed words [W0, W1) of a window (pk[0] = word W0; the range covers whole window rows, or the

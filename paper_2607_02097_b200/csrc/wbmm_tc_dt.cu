@@ -152,8 +152,10 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
         const int wyl = wl / g.nww, wx = wl - wyl * g.nww;
         const int win_off = ((wyl * WS) * g.W + wx * WS) * 2;
         uint8_t* dst = stage + (o ? 0 : Dc::OP_BYTES) + m * 16;
-        GenAddr<GEN ? WS : 1> ga;
+        constexpr bool WG = GEN || (WS % 2 == 1);   // word-granular window addressing (GenAddr)
+        GenAddr<WG ? WS : 1> ga;
         if constexpr (GEN) gen_addr_init<WS>(ga, g, wyl, wx);
+        else if constexpr (WG) gen_addr_init_plain<WS>(ga, g.W, wyl, wx);
         float* bins = reinterpret_cast<float*>(stage);
         float* bw = bins + (ot >> 5) * Cf::NB;          // this warp's private copy of the bins
         const int ew = ot >> 5;                          // 0..7
@@ -178,8 +180,8 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
             const uint8_t* img = ring + (size_t)slot * tl.S;
             {
                 uint32_t wv[Dc::NV * 4];
-                if constexpr (GEN) {
-                    if (ragged) window_to_regs_gen<WS, true>(img, ga, valid, wv);
+                if constexpr (WG) {
+                    if (GEN && ragged) window_to_regs_gen<WS, true>(img, ga, valid, wv);
                     else window_to_regs_gen<WS, false>(img, ga, valid, wv);
                 } else {
                     window_to_regs<WS>(valid ? img + win_off : img, valid, rowB, wv);
@@ -270,7 +272,7 @@ int dt_mode(const Geom& g, const TcTiles& tl, const void* x, const void* dy)
     if (tl.ntiles > 0x3fffffffll) return 0;
     if (dt_slots<WS>(tl) < 2 * tl.NP + 1) return 0;
     const bool plain = g.sh == 0 && g.sw == 0 && g.H == g.Hp && g.W == g.Wp;
-    if (plain && (tl.frame_rows * g.W * 2) % 16 == 0) return 1;
+    if (plain && (tl.frame_rows * g.W * 2) % 16 == 0 && (WS % 2 == 0 || g.W % 2 == 0)) return 1;   // odd w: rows must be word-aligned
     // general form: whole images in natural layout, word-granular window addressing (W, W' even)
     return (tl.nstrips == 1 && g.W % 2 == 0 && g.Wp % 2 == 0) ? 2 : 0;
 }
