@@ -129,6 +129,7 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
             for (int t = t0; t < t1; ++t, ++lt) {
                 const int c = t / tl.tiles_per_c;
                 ptx::mbar_wait(STAGE_FULL, lt & 1);
+                TRACE(1, lt);
                 ptx::tc_fence_after_sync();
 #pragma unroll
                 for (int mt = 0; mt < Dc::MT; ++mt) {
@@ -140,6 +141,7 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
                     }
                 }
                 ptx::mma_commit(STAGE_EMPTY);
+                TRACE(3, lt);
                 cur_c = c;
             }
         }
@@ -171,12 +173,15 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
             // After this barrier every repack thread has passed its waits of the previous tile, and a
             // slot's previous fill always belongs to an earlier tile (nslot > copies per tile).
             ptx::named_bar_sync(1, 256);
+            if (ot == 0) TRACE(4, lt);
             const bool part = pl < tl.NP && pl < np_eff;
             const bool valid = part && wy0 + wyl < g.nwh;
             const uint32_t kk = k + 2 * pl + o;
             const int slot = kk % nslot;
             if (part) ptx::mbar_wait(FULL(slot), (kk / nslot) & 1);
+            if (ot == 0) TRACE(5, lt);
             ptx::mbar_wait(STAGE_EMPTY, (lt & 1) ^ 1);      // MMA(lt-1) has read the stage
+            if (ot == 0) TRACE(6, lt);
             const uint8_t* img = ring + (size_t)slot * tl.S;
             {
                 uint32_t wv[Dc::NV * 4];
@@ -199,34 +204,45 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
             ptx::fence_proxy_async_smem();
             ptx::mbar_arrive(STAGE_FULL);
             if (part) ptx::mbar_arrive(EMPTY(slot));
+            if (ot == 0) TRACE(7, lt);
             k += 2 * np_eff;
 
             const bool seg_end = t + 1 == t1 || (t + 1) - c * tl.tiles_per_c == tl.tiles_per_c;
             if (seg_end) {
                 // ---- S (TMEM) -> bins -> dT[c]
                 ptx::mbar_wait(STAGE_EMPTY, lt & 1);        // every MMA of this channel segment has completed
+                if (ot == 0) TRACE(8, lt);
                 ptx::tc_fence_after_sync();
                 for (int b = lane; b < Cf::NB; b += 32) bw[b] = 0.f;
                 __syncwarp();
                 if (emt < Dc::MT) {
+                    // Row i = erow of S goes to bins base - rj*TW - cj.  For a fixed column j the 32 rows of
+                    // the warp hit 32 different bins; input rows rj and rj + RJ_STRIDE are RJ_STRIDE*w > 31
+                    // rows of S apart in bin space, so their updates are independent too: NU read-add-write
+                    // chains are in flight per step instead of one.
                     const uint32_t taddr = tmem + emt * 256 + ((uint32_t)(eq * 32) << 16);
-                    const float* bbase = bw + (eri + WS - 1) * Cf::TW + eci + WS - 1;   // bin of (i, j) = base - rj*TW - cj
+                    float* bbase = bw + (eri + WS - 1) * Cf::TW + eci + WS - 1;
+                    const bool rowok = erow < Cf::N;
+                    constexpr int RJ_STRIDE = 31 / WS + 1, NU = 3;
 #pragma unroll 1
-                    for (int ch = 0; ch < (Cf::N + 15) / 16; ++ch) {
-                        uint32_t v[16];
-                        ptx::tmem_ld16(taddr + ch * 16, v);
-                        ptx::tmem_wait_ld();
-                        int j = ch * 16;
-                        int rj = j / WS, cj = j - rj * WS;
+                    for (int g0 = 0; g0 < WS; g0 += (g0 % (NU * RJ_STRIDE) == RJ_STRIDE - 1) ? (NU - 1) * RJ_STRIDE + 1 : 1) {
+                        // rows rj = g0, g0 + RJ_STRIDE, g0 + 2*RJ_STRIDE of one pass
+                        uint32_t v[NU][16];
 #pragma unroll
-                        for (int e = 0; e < 16; ++e) {
-                            if (j < Cf::N && erow < Cf::N) {
-                                float* pb = const_cast<float*>(bbase) - rj * Cf::TW - cj;
-                                *pb += __uint_as_float(v[e]);
-                            }
+                        for (int u = 0; u < NU; ++u)
+                            if (g0 + u * RJ_STRIDE < WS) ptx::tmem_ld16(taddr + (g0 + u * RJ_STRIDE) * WS, v[u]);
+                        ptx::tmem_wait_ld();
+#pragma unroll
+                        for (int cj = 0; cj < WS; ++cj) {
+                            float old[NU];
+#pragma unroll
+                            for (int u = 0; u < NU; ++u)
+                                if (g0 + u * RJ_STRIDE < WS && rowok) old[u] = bbase[-(g0 + u * RJ_STRIDE) * Cf::TW - cj];
+#pragma unroll
+                            for (int u = 0; u < NU; ++u)
+                                if (g0 + u * RJ_STRIDE < WS && rowok)
+                                    bbase[-(g0 + u * RJ_STRIDE) * Cf::TW - cj] = old[u] + __uint_as_float(v[u][cj]);
                             __syncwarp();
-                            ++j;
-                            if (++cj == WS) { cj = 0; ++rj; }
                         }
                     }
                 }
@@ -244,6 +260,7 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
                     if (i * 16 < Dc::STAGE) reinterpret_cast<uint4*>(stage)[i] = make_uint4(0, 0, 0, 0);
                 ptx::fence_proxy_async_smem();
                 ptx::named_bar_sync(1, 256);
+                if (ot == 0) TRACE(9, lt);
             }
         }
     }
@@ -349,6 +366,13 @@ cudaError_t tc_grad_table(const Geom& g, int dtype, const void* x, const void* d
     }
 }
 
+
+#ifdef WBMM_TRACE
+extern "C" __attribute__((visibility("default"))) int wbmm_debug_trace_dt(long long* out)
+{
+    return (int)cudaMemcpyFromSymbol(out, tcdev::g_trace, sizeof(long long) * 256);
+}
+#endif
 
 #ifdef WBMM_WATCHDOG
 extern "C" __attribute__((visibility("default"))) int wbmm_debug_watchdog(unsigned long long* out)
