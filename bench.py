@@ -198,7 +198,7 @@ def run_reference(args, rank, world):
     from oracle import wbmm_ref
     case = si.CFG3
     per_image, T = oracle_probe(case)
-    per_step = max(0.05, min(15.0, 100.0 / max(1, args.steps + args.warmup)))
+    per_step = max(0.05, min(15.0, args.ref_seconds / max(1, args.steps + args.warmup)))
     sub, xs, sample = oracle_sample(case, per_step, per_image)
     times = []
     for i in range(args.warmup + args.steps):
@@ -340,16 +340,19 @@ def run_wbmm(args, rank, world, local):
         return
 
     hbm_peak, tc_peak, peak_kind = measured_peaks()
-    achieved = by / (ms_med * 1e-3) / 1e9
+    # one launch per step and nothing else on the stream: the average launch duration over the timed
+    # region (CUDA events on the launching stream) is ms_step
+    achieved = by / (ms_step * 1e-3) / 1e9
     t_roof = max(fl / (tc_peak * 1e12), by / (hbm_peak * 1e9))
     roofline = {"bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s",
                 "frac": achieved / hbm_peak, "traffic": ncu_traffic_bytes(),
                 "peak_kind": f"{peak_kind} (MEASURED_PEAKS.json hbm_gbs)" if peak_kind == "measured" else "fallback (B200_PROFILING.md)",
-                "kernel": path, "kernel_ms_median": ms_med, "kernel_ms_min": ms_min,
+                "kernel": path, "kernel_ms_avg_timed_region": ms_step,
+                "kernel_ms_median_event_pair_per_launch": ms_med, "kernel_ms_min_event_pair_per_launch": ms_min,
                 "algorithmic_bytes_per_launch": by, "algorithmic_flops_per_launch": fl,
-                "t_roof_ms": t_roof * 1e3, "frac_of_roofline_time": t_roof * 1e3 / ms_med,
-                "tensor_tflops_at_median": fl / (ms_med * 1e-3) / 1e12,
-                "hot_l2_ms_median": statistics.median(hot)}
+                "t_roof_ms": t_roof * 1e3, "frac_of_roofline_time": t_roof * 1e3 / ms_step,
+                "tensor_tflops": fl / (ms_step * 1e-3) / 1e12,
+                "hot_l2_ms_median_event_pair": statistics.median(hot)}
 
     # training step (config 5) as context: forward + dX + dT
     c5 = si.CFG5
@@ -360,15 +363,31 @@ def run_wbmm(args, rank, world, local):
         wb.wbmm_forward(d5["x"], d5["T"], c5.w, c5.shift, out=y5)
         wb.wbmm_backward(d5["x"], d5["T"], d5["dy"], c5.w, c5.shift)
 
+    def region_ms(fn, n=20):
+        for _ in range(3):
+            fn()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for _ in range(n):
+            fn()
+        b.record(stream)
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / n
+
     for i in range(3):
         train(i)
     t5 = time_steps(train, 10, stream)
     train_path = wb.wbmm_path_string(wb.wbmm_last_path())
+    parts = {
+        "fwd_ms": region_ms(lambda: wb.wbmm_forward(d5["x"], d5["T"], c5.w, c5.shift, out=y5)),
+        "dX_ms": region_ms(lambda: wb.wbmm_backward(None, d5["T"], d5["dy"], c5.w, c5.shift, need_dT=False)),
+        "dT_ms": region_ms(lambda: wb.wbmm_backward(d5["x"], None, d5["dy"], c5.w, c5.shift, need_dx=False)),
+    }
     by5 = 2 * c5.n_elem * 2 * 2 + 2 * c5.n_elem * 2 + c5.C * c5.bins * 4   # x,y; dy,dx; x,dy; dT
     train_step = {"workload": "cfg5 B128 C192 28x28 w14 shift7 fwd+dX+dT", "ms_median": statistics.median(t5),
-                  "ms_min": min(t5), "last_path": train_path, "flops": 3 * flops_of(c5),
+                  "ms_min": min(t5), "back_to_back": parts, "last_path": train_path, "flops": 3 * flops_of(c5),
                   "hbm_frac_at_median": by5 / (statistics.median(t5) * 1e-3) / 1e9 / hbm_peak,
-                  "note": "working set fits L2 (232 MB algorithmic traffic, 126 MB L2): hot-ish number"}
+                  "note": "x, y, dy, dx = 154 MB against a 126 MB L2: partly L2-resident between launches"}
 
     tfl_cpu, cores, sample, dt_cpu = time_oracle(case)
     cpu = {"value": tfl_cpu, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
@@ -388,13 +407,53 @@ def run_wbmm(args, rank, world, local):
     print(json.dumps(out), flush=True)
 
 
+def run_sweep(args):
+    """--sweep: BASELINE.json config 4 (82 forward cases) + configs 2 and 5, one JSON line per case.
+    Not the bench line; a table for profiles/ and BASELINE.md context."""
+    import paper_2607_02097_b200 as wb
+    torch.cuda.set_device(0)
+    stream = torch.cuda.current_stream()
+    hbm_peak, tc_peak, _ = measured_peaks()
+    cases = [si.CFG2, si.CFG3, si.with_(si.CFG5, backward=False)] + list(si.sweep_cases())
+    for case in cases:
+        d = si.make(case, device="cuda")
+        tensor_bytes = d["x"].numel() * 2
+        nsets = int(min(4, max(2, -(-2 * L2_BYTES // (2 * tensor_bytes)) + 1)))
+        xs = [d["x"]] + [d["x"].clone() for _ in range(nsets - 1)]
+        ys = [torch.empty_like(d["x"]) for _ in range(nsets)]
+        f = lambda i: wb.wbmm_forward(xs[i % nsets], d["T"], case.w, case.shift, case.layout, out=ys[i % nsets])
+        n = 30 if case.n_elem < 2e8 else 10
+        for i in range(3):
+            f(i)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for i in range(n):
+            f(i)
+        b.record(stream)
+        torch.cuda.synchronize()
+        ms = a.elapsed_time(b) / n
+        fl, by = flops_of(case), bytes_of(case)
+        t_roof = max(fl / (tc_peak * 1e12), by / (hbm_peak * 1e9))
+        print(json.dumps({"sweep_case": case.name, "layout": "NHWC" if case.layout else "NCHW", "B": case.B, "C": case.C,
+                          "H": case.H, "w": case.w, "shift": list(case.shift), "ms": round(ms, 5),
+                          "tflops": round(fl / ms / 1e9, 2), "gbs": round(by / ms / 1e6, 1),
+                          "frac_of_roofline": round(t_roof * 1e3 / ms, 4),
+                          "path": wb.wbmm_path_string(wb.wbmm_last_path()), "buffer_sets": nsets}), flush=True)
+        del xs, ys, d
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="wbmm", choices=["wbmm", "reference"])
+    ap.add_argument("--sweep", action="store_true", help="time the config-4 operator sweep instead (one JSON line per case)")
+    ap.add_argument("--ref-seconds", type=float, default=100.0, help="--impl reference: CPU seconds for the whole run")
     args = ap.parse_args()
+    if args.sweep:
+        run_sweep(args)
+        return
     if args.impl == "reference":
         rank = int(os.environ.get("RANK", "0"))
         run_reference(args, rank, int(os.environ.get("WORLD_SIZE", "1")))
