@@ -69,6 +69,13 @@ int apply(const wbmm_desc_t* d, const wbmm::Geom& g, const void* x, const void* 
 {
     int launches = 0;
     cudaError_t e;
+    if (!(d->flags & WBMM_FLAG_FORCE_SIMT) && wbmm::tc_nhwc_supported(g, d->dtype, x, y)) {
+        e = wbmm::tc_nhwc_forward(g, d->dtype, x, T, y, reverse, stream, &launches);
+        g_launches += launches;
+        if (e != cudaSuccess) return set_cuda_error(e, "tc_nhwc_forward");
+        t_last_path = WBMM_PATH_TC_GATHER;
+        return WBMM_STATUS_OK;
+    }
     if (!(d->flags & WBMM_FLAG_FORCE_SIMT) && wbmm::tc_forward_supported(g, d->dtype, x, y)) {
         int path = WBMM_PATH_NONE;
         e = wbmm::tc_forward(g, d->dtype, x, T, y, reverse, stream, &launches, &path);

@@ -26,37 +26,6 @@ namespace {
 
 constexpr int kThreadsG = 256;   // generic kernel: 8 warps; warps 0-3 own the 128 TMEM lanes
 
-// Stage one channel's table row in shared memory (reversed for the transposed operator) and build
-// W_c[i][j] = T[c, rel(i,j)] in the K-major core-matrix layout: value (i, j) lives at byte
-// (j/8)*LBO + i*16 + (j%8)*2.  Rows i >= N and columns j >= N are zero.
-template <int WS>
-__device__ __forceinline__ void build_weight(const uint16_t* __restrict__ Tc, bool reverse, uint16_t* Ts,
-                                             uint8_t* Wc, int tid, int nthreads)
-{
-    using Cf = WinCfg<WS>;
-    for (int k = tid; k < Cf::NB; k += nthreads) Ts[k] = Tc[reverse ? Cf::NB - 1 - k : k];
-    __syncthreads();
-    constexpr int NCHUNK = (Cf::K_PAD / 8) * Cf::N_PAD;
-    for (int id = tid; id < NCHUNK; id += nthreads) {
-        const int kc = id / Cf::N_PAD, i = id % Cf::N_PAD;
-        uint32_t pk[4] = {0u, 0u, 0u, 0u};
-        if (i < Cf::N) {
-            const int ri = i / WS, ci = i % WS;
-            int j = kc * 8;
-            int rj = j / WS, cj = j % WS;
-#pragma unroll
-            for (int e = 0; e < 8; ++e) {
-                uint32_t v = 0;
-                if (j < Cf::N) v = Ts[(ri - rj + WS - 1) * Cf::TW + (ci - cj + WS - 1)];   // Eq. 7
-                pk[e >> 1] |= v << ((e & 1) * 16);
-                ++j;
-                if (++cj == WS) { cj = 0; ++rj; }
-            }
-        }
-        *reinterpret_cast<uint4*>(Wc + kc * Cf::LBO + i * 16) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
-    }
-}
-
 // ------------------------------------------------------------------------------------------------
 // Generic kernel ("tcgen05+gather"): any shift, ragged size, W and layout.  The frame is filled
 // and drained by plain predicated loads/stores (index arithmetic does padding, shift and layout),
@@ -185,47 +154,6 @@ tc_generic_kernel(Geom g, TcTiles tl, const uint16_t* __restrict__ x, const uint
 //
 // Each 32-bit shared-memory access of the repack / epilogue warps is conflict-free for the
 // headline geometry: lanes are (4 adjacent windows) x (8 images) and the image stride is 16*odd bytes.
-
-// The table row of a channel is staged in shared memory as two copies of the fully reversed table
-// F[q] = T[NB-1-q] (F0 = F, F1 = F shifted by one value), so that any pair (F[q], F[q+1]) is one
-// aligned 32-bit load whatever the parity of q.
-constexpr int kTabRegs = (WinCfg<14>::NB + 127) / 128;
-
-// The (reversed) table row of one channel, 128 threads -> registers (loads only; no use yet).
-__device__ __forceinline__ void table_to_regs14(const uint16_t* __restrict__ Tc, bool reverse, int tid, uint16_t* v)
-{
-    using Cf = WinCfg<14>;
-#pragma unroll
-    for (int u = 0; u < kTabRegs; ++u) {
-        const int q = tid + u * 128;
-        v[u] = q < Cf::NB ? Tc[reverse ? q : Cf::NB - 1 - q] : (uint16_t)0;
-    }
-}
-
-// Block-Toeplitz library for w = 14 (BulkCfg<14>) from the two staged copies of the reversed table
-// (see build_weight14): chunk (d, ci, kc) = Z[d-13][ci][8kc .. 8kc+7] = F[(26-d)*27 + 13-ci + 8kc + e].
-// 128 threads (the repack warps); rows ci = 14, 15 of every block stay zero from the kernel prologue.
-__device__ __forceinline__ void build_lib14(const uint16_t* v, uint16_t* F0, uint16_t* F1, uint8_t* lib, int tid)
-{
-    using Cf = WinCfg<14>;
-    using Bc = BulkCfg<14>;
-#pragma unroll
-    for (int u = 0; u < kTabRegs; ++u) {
-        const int q = tid + u * 128;
-        if (q < Cf::NB) {
-            F0[q] = v[u];
-            if (q >= 1) F1[q - 1] = v[u];
-        }
-    }
-    ptx::named_bar_sync(2, 128);
-    for (int id = tid; id < 27 * 28; id += 128) {
-        const int d = id / 28, rem = id - d * 28, ci = rem >> 1, kc = rem & 1;
-        const int q0 = (26 - d) * 27 + 13 - ci + 8 * kc, p0 = q0 & 1;
-        const uint32_t* src = reinterpret_cast<const uint32_t*>(reinterpret_cast<const uint8_t*>(p0 ? F1 : F0) + (q0 - p0) * 2);
-        const uint32_t w0 = src[0], w1 = src[1], w2 = src[2], w3 = kc ? 0u : src[3];   // cj = 14, 15 are padding
-        *reinterpret_cast<uint4*>(lib + kc * Bc::LBO + (d * 16 + ci) * 16) = make_uint4(w0, w1, w2, w3);
-    }
-}
 
 template <int WS>
 struct BulkSmem {

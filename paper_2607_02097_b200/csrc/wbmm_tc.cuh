@@ -27,6 +27,11 @@ bool tc_forward_supported(const Geom& g, int dtype, const void* x, const void* y
 cudaError_t tc_forward(const Geom& g, int dtype, const void* x, const void* T, void* y, bool reverse,
                        cudaStream_t stream, int* launches, int* path);
 
+// NHWC forward / dX: 8-channel groups gathered with 16-byte cp.async (wbmm_tc_nhwc.cu).
+bool tc_nhwc_supported(const Geom& g, int dtype, const void* x, const void* y);
+cudaError_t tc_nhwc_forward(const Geom& g, int dtype, const void* x, const void* T, void* y, bool reverse,
+                            cudaStream_t stream, int* launches);
+
 bool tc_grad_table_supported(const Geom& g, int dtype, const void* x, const void* dy);
 cudaError_t tc_grad_table(const Geom& g, int dtype, const void* x, const void* dy, float* dT,
                           cudaStream_t stream, int* launches, int* path);
