@@ -248,14 +248,27 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
     const long long plane_elems = (long long)g.H * g.W;
     const bool ragged = g.H != g.Hp || g.W != g.Wp;
 
-    auto tile_decode = [&](int t, int& c, int& b0, int& wy0, int& np_eff, int& rows_eff) {
-        c = t / tl.tiles_per_c;
-        const int rem = t - c * tl.tiles_per_c;
-        const int gb = rem / tl.nstrips, strip = rem - gb * tl.nstrips;
-        b0 = gb * tl.NP;
-        wy0 = strip * tl.NSY;
+    // Every role walks the CTA's tiles in order: (channel, image group, strip) of the current tile, one
+    // division at the start and increments afterwards.  tile_decode() returns the current tile and advances.
+    int it_c = t0 / tl.tiles_per_c, it_gb, it_strip;
+    {
+        const int rem = t0 - it_c * tl.tiles_per_c;
+        it_gb = rem / tl.nstrips;
+        it_strip = rem - it_gb * tl.nstrips;
+    }
+    auto tile_decode = [&](int, int& c, int& b0, int& wy0, int& np_eff, int& rows_eff) {
+        c = it_c;
+        b0 = it_gb * tl.NP;
+        wy0 = it_strip * tl.NSY;
         np_eff = min(tl.NP, g.B - b0);
         rows_eff = GEN ? g.H : min(tl.frame_rows, g.H - wy0 * WS);   // GEN: whole images (nstrips == 1)
+        if (++it_strip == tl.nstrips) {
+            it_strip = 0;
+            if (++it_gb == tl.ngb) {
+                it_gb = 0;
+                ++it_c;
+            }
+        }
     };
 
     if (warp == 0) {
@@ -363,7 +376,9 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
             // different threads: a thread may only test fill n once fill n-1 is known to have landed.
             // After this barrier every repack thread has passed its waits of the previous tile, and a
             // slot's previous fill always belongs to an earlier tile (nslot > images per tile).
-            ptx::named_bar_sync(2, 128);
+            // With a ring of at least two tiles the wait below already implies it: MMA(lt-2) committed
+            // after every repack thread had finished tile lt-2, and the slot's previous fill is that old.
+            if (nslot < 2 * tl.NP) ptx::named_bar_sync(2, 128);
             ptx::mbar_wait(A_EMPTY + 8 * buf, ((lt >> 1) & 1) ^ 1);   // MMA(lt-2) has consumed A[buf]
             if (rt == 0) TRACE(4, lt);
             const bool part = wl < wpf && pl < np_eff;               // this thread's frame image was loaded
@@ -461,9 +476,9 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
             const uint32_t out_bytes = (uint32_t)og.images * tl.S;
             uint32_t lt = 0;
             for (int t = t0; t < t1; ++t, ++lt) {
-                if (lt % depth != frame) continue;
                 int c, b0, wy0, np_eff, rows_eff;
                 tile_decode(t, c, b0, wy0, np_eff, rows_eff);
+                if (lt % depth != frame) continue;
                 const uint32_t bytes = (uint32_t)rows_eff * rowB;
                 ptx::mbar_wait(OUT_FULL + 8 * lane, (lt / depth) & 1);
                 if (lane == 0) TRACE(10, lt);
@@ -477,7 +492,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                 if (lane == 0) TRACE(11, lt);
                 ptx::mbar_arrive(OUT_EMPTY + 8 * lane);
             }
-            ptx::bulk_wait_all<0>();
+            ptx::bulk_wait_read<0>();   // the sources are in this CTA's shared memory: reads must finish before it exits
         }
     }
     ptx::tc_fence_before_sync();
@@ -489,9 +504,12 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
 }
 
 // Shared memory left after the weights / tables / barriers is cut into frame-image slots: an output
-// frame of one or two tiles (one buffer per output group and tile) and an input ring of `nslot` slots.
-// A bulk store takes ~1.4 us until its source may be overwritten, about as long as a load takes to
-// land, so the output side is two tiles deep whenever a tile + 1 of input still fits beside it.
+// frame `depth` tiles deep (one buffer per output group and tile) and an input ring of `nslot` slots.
+// Both sides want about 96 KB: a bulk store takes ~1.4 us until its source may be overwritten and a
+// load ~1.5-2 us to land, i.e. ~50 KB in flight per SM each way at the ~35 GB/s per SM the copy engine
+// sustains, plus the tile being worked on.  More input in flight measured SLOWER (112 x 112 maps:
+// 4 slots of 25 KB 114 us, 3 slots 104 us; also for a plain bulk-copy ring,
+// profiles/r01_bulk_copy_microbench.md); less starves small tiles (w = 7: 12.5 KB per tile).
 // Returns false when a tile of output plus a tile + 1 of input does not fit.
 template <int WS>
 bool bulk_slots(const TcTiles& tl, int wpf, int* nslot, int* nout)
@@ -499,17 +517,19 @@ bool bulk_slots(const TcTiles& tl, int wpf, int* nslot, int* nout)
     const OutGroups og = out_groups(tl, wpf);
     const long long room = 227ll * 1024 - 1024 - BulkSmem<WS>::FIXED;
     const long long total = room / tl.S, out_tile = (long long)og.n * og.images;
-    const int depth = (total - 2 * out_tile >= tl.NP + 1 && 2 * og.n <= kMaxOutBufs) ? 2 : 1;
+    constexpr long long kSide = 96 * 1024;
+    long long depth = (kSide + out_tile * tl.S / 2) / (out_tile * tl.S);
+    if (depth > kMaxOutBufs / og.n) depth = kMaxOutBufs / og.n;
+    while (depth > 1 && total - depth * out_tile < tl.NP + 1) --depth;
+    if (depth < 1) return false;
     long long ni = total - depth * out_tile;
-    // Two tiles of input for small frame images; for tiles of a few big images (>= 12 KB each) one
-    // tile + 1: more loads in flight measured SLOWER there (112 x 112 maps: 114 -> 104 us), as it does
-    // for a plain bulk-copy ring (profiles/r01_bulk_copy_microbench.md).
-    const long long in_cap = tl.NP >= 4 ? 2 * tl.NP : tl.NP + 1;
+    long long in_cap = kSide / tl.S;
+    if (in_cap < tl.NP + 1) in_cap = tl.NP + 1;
     if (ni > in_cap) ni = in_cap;
     if (ni > kMaxSlots) ni = kMaxSlots;
     if (ni < tl.NP + 1) return false;
     *nslot = (int)ni;
-    *nout = depth * og.n;
+    *nout = (int)(depth * og.n);
     return true;
 }
 
