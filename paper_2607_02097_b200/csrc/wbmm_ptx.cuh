@@ -174,6 +174,34 @@ __device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t* v)
                  : "memory");
 }
 
+__device__ __forceinline__ void tmem_ld4(uint32_t taddr, uint32_t* v)
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3])
+                 : "r"(taddr)
+                 : "memory");
+}
+__device__ __forceinline__ void tmem_ld2(uint32_t taddr, uint32_t* v)
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0,%1}, [%2];" : "=r"(v[0]), "=r"(v[1]) : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_ld1(uint32_t taddr, uint32_t* v)
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x1.b32 {%0}, [%1];" : "=r"(v[0]) : "r"(taddr) : "memory");
+}
+// exactly N consecutive columns (N <= 16) with the fewest power-of-two loads
+template <int N>
+__device__ __forceinline__ void tmem_ld_n(uint32_t taddr, uint32_t* v)
+{
+    static_assert(N >= 1 && N <= 16, "1..16 columns");
+    int o = 0;
+    if constexpr (N >= 16) { tmem_ld16(taddr, v); return; }
+    if constexpr (N & 8) { tmem_ld8(taddr + o, v + o); o += 8; }
+    if constexpr (N & 4) { tmem_ld4(taddr + o, v + o); o += 4; }
+    if constexpr (N & 2) { tmem_ld2(taddr + o, v + o); o += 2; }
+    if constexpr (N & 1) { tmem_ld1(taddr + o, v + o); }
+}
+
 // ------------------------------------------------------------------------------- MMA
 // Shared-memory operand descriptor, K-major, no swizzle ("interleave"): 8-row x 16-byte core
 // matrices stored as 128 contiguous bytes; lbo = byte distance between the two core matrices an

@@ -223,14 +223,14 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
                     const uint32_t taddr = tmem + emt * 256 + ((uint32_t)(eq * 32) << 16);
                     float* bbase = bw + (eri + WS - 1) * Cf::TW + eci + WS - 1;
                     const bool rowok = erow < Cf::N;
-                    constexpr int RJ_STRIDE = 31 / WS + 1, NU = 3;
-#pragma unroll 1
-                    for (int g0 = 0; g0 < WS; g0 += (g0 % (NU * RJ_STRIDE) == RJ_STRIDE - 1) ? (NU - 1) * RJ_STRIDE + 1 : 1) {
-                        // rows rj = g0, g0 + RJ_STRIDE, g0 + 2*RJ_STRIDE of one pass
-                        uint32_t v[NU][16];
+                    constexpr int RJ_STRIDE = 31 / WS + 1, NU = (WS + RJ_STRIDE - 1) / RJ_STRIDE;
+#pragma unroll
+                    for (int g0 = 0; g0 < RJ_STRIDE; ++g0) {
+                        // rows rj = g0, g0 + RJ_STRIDE, ... of one pass: NU independent chains
+                        uint32_t v[NU][WS];
 #pragma unroll
                         for (int u = 0; u < NU; ++u)
-                            if (g0 + u * RJ_STRIDE < WS) ptx::tmem_ld16(taddr + (g0 + u * RJ_STRIDE) * WS, v[u]);
+                            if (g0 + u * RJ_STRIDE < WS) ptx::tmem_ld_n<WS>(taddr + (g0 + u * RJ_STRIDE) * WS, v[u]);
                         ptx::tmem_wait_ld();
 #pragma unroll
                         for (int cj = 0; cj < WS; ++cj) {
