@@ -652,7 +652,28 @@ int partition_tiles(const TcTiles& tl, int grid, double kSwitchCost, TilePart* p
         const double mid = 0.5 * (lo + hi);
         if (fill(mid, nullptr) <= grid) hi = mid; else lo = mid;
     }
-    const int used = fill(hi, part);
+    // `hi` is the smallest achievable maximum cost; packing every CTA up to it would leave the last CTAs
+    // idle (cfg5 dT: 128 of 148), and the kernels are bound by per-SM copy-engine throughput, so spread
+    // the tiles over ALL CTAs instead: each CTA takes its share of what is left, never more than `hi`.
+    const double cap = hi;
+    int t = 0, used = 0;
+    part->start[0] = 0;
+    for (int b = 0; b < grid && t < n; ++b) {
+        // cost of everything that is left if a CTA starts at tile t: tiles + channel boundaries inside (t, n)
+        const double rem = (n - t) + kSwitchCost * ((n - 1) / tpc - t / tpc);
+        const double target = rem / (grid - b);
+        double cost = 0;
+        const int first = t;
+        while (t < n) {
+            const double add = 1.0 + ((t > first && t % tpc == 0) ? kSwitchCost : 0.0);
+            if (t > first && (cost + add > cap + 1e-9 || cost + 0.5 * add > target)) break;
+            cost += add;
+            ++t;
+        }
+        part->start[b + 1] = t;
+        used = b + 1;
+    }
+    if (t < n) used = fill(hi, part);     // (rounding left tiles over: fall back to the packed schedule)
     for (int b = used; b < kMaxGrid; ++b) part->start[b + 1] = n;
     return used;
 }

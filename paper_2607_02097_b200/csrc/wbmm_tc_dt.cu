@@ -312,7 +312,7 @@ cudaError_t launch_dt(const Geom& g, const TcTiles& tl, const void* x, const voi
     {
         std::lock_guard<std::mutex> lock(mu);
         if (key_n != tl.ntiles || key_tpc != tl.tiles_per_c || key_grid != grid) {
-            cached_used = partition_tiles(tl, grid, 1.0, &cached);   // a channel boundary costs one bin epilogue
+            cached_used = partition_tiles(tl, grid, 1.5, &cached);   // a channel boundary costs one bin fold (~1.5 tiles)
             key_n = tl.ntiles; key_tpc = tl.tiles_per_c; key_grid = grid;
         }
         part = cached;
