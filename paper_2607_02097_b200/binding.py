@@ -117,8 +117,12 @@ def wbmm_forward(x: torch.Tensor, T: torch.Tensor, w: int, shift=(0, 0), layout:
     if T.dtype != x.dtype or tuple(T.shape) != (d.C, (2 * w - 1) ** 2):
         raise ValueError("T must be [C,(2w-1)^2] in the dtype of x")
     y = torch.empty_like(x) if out is None else out
-    with torch.cuda.device(x.device):
-        _check(lib().wbmm_forward(ctypes.byref(d), _dev(x, "x"), _dev(T, "T"), _dev(y, "y"), _stream(x)))
+    px, pT, py = _dev(x, "x"), _dev(T, "T"), _dev(y, "y")
+    if x.device.index == torch.cuda.current_device():      # the common case: no device switch
+        _check(lib().wbmm_forward(ctypes.byref(d), px, pT, py, _stream(x)))
+    else:
+        with torch.cuda.device(x.device):
+            _check(lib().wbmm_forward(ctypes.byref(d), px, pT, py, _stream(x)))
     return y
 
 

@@ -558,7 +558,8 @@ cudaError_t launch_bulk(const Geom& g, const TcTiles& tl, const void* x, const v
     const int wpf = tl.NSY * g.nww;
     if (!bulk_slots<WS>(tl, wpf, &nslot, &nout)) return cudaErrorInvalidConfiguration;
     const size_t smem = (size_t)BulkSmem<WS>::FIXED + (size_t)(nslot + nout * out_groups(tl, wpf).images) * tl.S;
-    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    static SmemOptIn smem_state = {0, 0};
+    cudaError_t e = ensure_dynamic_smem(reinterpret_cast<const void*>(k), smem, &smem_state);
     if (e != cudaSuccess) return e;
     int grid = (int)(tl.ntiles < num_sms() ? tl.ntiles : num_sms());
     if (grid > kMaxGrid) grid = kMaxGrid;
@@ -603,7 +604,8 @@ cudaError_t launch_generic(const Geom& g, const TcTiles& tl, const void* x, cons
 {
     auto k = tc_generic_kernel<WS, BF16>;
     const size_t smem = generic_smem<WS>(tl);
-    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    static SmemOptIn smem_state = {0, 0};
+    cudaError_t e = ensure_dynamic_smem(reinterpret_cast<const void*>(k), smem, &smem_state);
     if (e != cudaSuccess) return e;
     const int grid = (int)(tl.ntiles < num_sms() ? tl.ntiles : num_sms());
     k<<<grid, kThreadsG, smem, s>>>(g, tl, (const uint16_t*)x, (const uint16_t*)T, (uint16_t*)y, reverse ? 1 : 0);
@@ -611,6 +613,20 @@ cudaError_t launch_generic(const Geom& g, const TcTiles& tl, const void* x, cons
 }
 
 }  // namespace
+
+cudaError_t ensure_dynamic_smem(const void* kernel, size_t bytes, SmemOptIn* state)
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (state->dev_plus1 == dev + 1 && (size_t)state->bytes >= bytes) return cudaSuccess;
+    e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (e == cudaSuccess) {
+        state->dev_plus1 = dev + 1;
+        state->bytes = (int)bytes;
+    }
+    return e;
+}
 
 int num_sms()
 {

@@ -579,6 +579,10 @@ __device__ __forceinline__ long long gtime() { long long t; asm volatile("mov.u6
 
 // Host helpers defined in wbmm_tc.cu.
 int num_sms();
+// Opts a kernel in to `bytes` of dynamic shared memory unless an earlier call already allowed as much
+// on this device (`state`: one static per kernel instantiation, zero-initialised).
+struct SmemOptIn { int dev_plus1, bytes; };
+cudaError_t ensure_dynamic_smem(const void* kernel, size_t bytes, SmemOptIn* state);
 // Greedy contiguous partition of the tile sequence over `grid` CTAs minimising the largest cost,
 // cost = tiles + switch_cost per channel boundary strictly inside a CTA's range.  Returns the
 // number of CTAs used.

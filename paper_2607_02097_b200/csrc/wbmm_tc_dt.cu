@@ -300,7 +300,8 @@ cudaError_t launch_dt(const Geom& g, const TcTiles& tl, const void* x, const voi
     auto k = tc_dt_kernel<WS, BF16, GEN>;
     const int nslot = dt_slots<WS>(tl);
     const size_t smem = (size_t)DtCfg<WS>::FIXED + (size_t)nslot * tl.S;
-    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    static SmemOptIn smem_state = {0, 0};
+    cudaError_t e = ensure_dynamic_smem(reinterpret_cast<const void*>(k), smem, &smem_state);
     if (e != cudaSuccess) return e;
     int grid = (int)(tl.ntiles < num_sms() ? tl.ntiles : num_sms());
     if (grid > kMaxGrid) grid = kMaxGrid;

@@ -302,7 +302,8 @@ cudaError_t launch_nhwc(const Geom& g, const NhwcTiles& nt, const void* x, const
 {
     auto k = tc_nhwc_kernel<WS, BF16>;
     const size_t smem = (size_t)NhwcSmem<WS>::FIXED + (size_t)nt.NP * nt.frame_px * 16;
-    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    static SmemOptIn smem_state = {0, 0};
+    cudaError_t e = ensure_dynamic_smem(reinterpret_cast<const void*>(k), smem, &smem_state);
     if (e != cudaSuccess) return e;
     const int grid = (int)(nt.ntiles < num_sms() ? nt.ntiles : num_sms());
     k<<<grid, kThreadsN, smem, s>>>(g, nt, (const uint16_t*)x, (const uint16_t*)T, (uint16_t*)y, reverse ? 1 : 0);
