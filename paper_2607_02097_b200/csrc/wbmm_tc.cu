@@ -509,7 +509,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
 // load ~1.5-2 us to land, i.e. ~50 KB in flight per SM each way at the ~35 GB/s per SM the copy engine
 // sustains, plus the tile being worked on.  More input in flight measured SLOWER (112 x 112 maps:
 // 4 slots of 25 KB 114 us, 3 slots 104 us; also for a plain bulk-copy ring,
-// profiles/r01_bulk_copy_microbench.md); less starves small tiles (w = 7: 12.5 KB per tile).
+// DESIGN.md section 7.6); less starves small tiles (w = 7: 12.5 KB per tile).
 // Returns false when a tile of output plus a tile + 1 of input does not fit.
 template <int WS>
 bool bulk_slots(const TcTiles& tl, int wpf, int* nslot, int* nout)
