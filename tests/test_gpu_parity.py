@@ -89,6 +89,75 @@ def test_backward_small(wb, oracle, case, layout, force_simt):
     assert e_dx <= 1.0 and e_dT <= 1.0, (e_dx, e_dT)
 
 
+# ------------------------------------------------------------------ the pipelined kernels, every mode
+# Shapes chosen so that the warp-specialised bulk kernel (NCHW) / the 8-channel-group kernel (NHWC)
+# serve them -- asserted through wbmm_last_path() -- with ragged tails in every tiling dimension:
+# B not a multiple of the images per tile, several tiles and channels per CTA, strips of big maps,
+# shift with odd and even column offsets, padding, fp16.
+PIPE = [
+    si.Case("p_w14_plain", 19, 5, 56, 56, 14),                               # 8 images per tile, tail of 3
+    si.Case("p_w14_many_tiles", 40, 160, 28, 28, 14),                        # 32 images per tile, > 148 tiles
+    si.Case("p_w14_shift_odd", 9, 7, 28, 56, 14, shift=(7, 7)),              # odd column start: funnel shifts
+    si.Case("p_w14_shift_even", 9, 7, 28, 56, 14, shift=(3, 4)),
+    si.Case("p_w14_ragged", 7, 6, 60, 60, 14),                               # 25 windows per image, W' = 70
+    si.Case("p_w14_ragged_shift", 6, 5, 36, 40, 14, shift=(5, 9)),
+    si.Case("p_w14_strips", 3, 4, 168, 112, 14),                             # 96 windows per image: 2 images / tile
+    si.Case("p_w14_big_map", 2, 3, 224, 224, 14),                            # 256 windows per image: row strips
+    si.Case("p_w14_f16", 10, 9, 42, 56, 14, dtype="f16", shift=(0, 7)),
+    si.Case("p_w7_plain", 21, 6, 56, 56, 7),                                 # 64 windows per image
+    si.Case("p_w7_strips", 3, 5, 112, 112, 7),                               # 256 windows per image: strips
+    si.Case("p_w7_shift", 5, 7, 28, 28, 7, shift=(3, 2)),
+    si.Case("p_w7_ragged", 6, 4, 26, 30, 7, shift=(0, 3)),                   # W' = 35 is odd: generic path
+    si.Case("p_w7_f16", 33, 3, 28, 56, 7, dtype="f16"),
+]
+
+
+@pytest.mark.parametrize("case", PIPE, ids=lambda c: c.name)
+@pytest.mark.parametrize("layout", [NCHW, NHWC])
+def test_pipelined_kernels_forward_backward(wb, oracle, case, layout):
+    C = case.C if layout == NCHW else -(-case.C // 8) * 8                     # NHWC kernel: 8-channel groups
+    case = si.with_(case, layout=layout, C=C, backward=True)
+    d = si.make(case, device="cuda")
+    y = wb.wbmm_forward(d["x"], d["T"], case.w, case.shift, case.layout)
+    torch.cuda.synchronize()
+    path = wb.wbmm_last_path()
+    if case.name != "p_w7_ragged":
+        assert path == (wb.PATH_TC_TMA if layout == NCHW else wb.PATH_TC_GATHER), wb.wbmm_path_string(path)
+    dx, dT = wb.wbmm_backward(d["x"], d["T"], d["dy"], case.w, case.shift, case.layout)
+    torch.cuda.synchronize()
+    ry = oracle.forward(widen(d["x"]), widen(d["T"]), case.w, case.shift, case.layout, "direct")
+    rdx, rdT = oracle.backward(widen(d["x"]), widen(d["T"]), widen(d["dy"]), case.w, case.shift, case.layout)
+    tol = TOL[case.dtype]
+    errs = (max_err_over_tol(y, ry, tol), max_err_over_tol(dx, rdx, tol), max_err_over_tol(dT, rdT, tol))
+    assert max(errs) <= 1.0, errs
+
+
+@pytest.mark.parametrize("w,shift,H,W", [(14, (0, 0), 56, 56), (14, (7, 7), 28, 56), (14, (2, 5), 60, 60),
+                                         (7, (0, 0), 56, 56), (7, (3, 4), 28, 28)])
+@pytest.mark.parametrize("layout", [NCHW, NHWC])
+def test_pipelined_kernels_one_hot_bins_bitwise(wb, oracle, w, shift, H, W, layout):
+    """One-hot tables through the pipelined kernels (bulk / NHWC group kernel): pure data movement,
+    so the result must equal the oracle's bitwise -- the bit-exact indexing test of the Toeplitz
+    library, the word-granular shift / padding addressing and the NHWC transposition."""
+    tw = 2 * w - 1
+    nb = tw * tw
+    C = 64
+    case = si.Case("onehot_pipe", 9, C, H, W, w, dtype="bf16", layout=layout, shift=shift, seed=31)
+    d = si.make(case, device="cuda")
+    g = torch.Generator().manual_seed(w * 1000 + H)
+    bins = torch.randint(0, nb, (C,), generator=g)
+    bins[0], bins[1], bins[2] = 0, nb - 1, (w - 1) * tw + (w - 1)            # corners and the centre
+    T = torch.zeros_like(d["T"])
+    T[torch.arange(C), bins.to(T.device)] = 1.0
+    y = wb.wbmm_forward(d["x"], T, w, shift, layout)
+    assert wb.wbmm_last_path() == (wb.PATH_TC_TMA if layout == NCHW else wb.PATH_TC_GATHER)
+    ref = oracle.forward(widen(d["x"]), widen(T), w, shift, layout)
+    assert np.array_equal(widen(y), ref)
+    dx, _ = wb.wbmm_backward(None, T, d["x"], w, shift, layout, need_dT=False)
+    rdx, _ = oracle.backward(widen(d["x"]), widen(T), widen(d["x"]), w, shift, layout, need_dT=False)
+    assert np.array_equal(widen(dx), rdx)
+
+
 def test_config1_fp32_tiny(wb, oracle):
     """BASELINE.json config 1: fp32 path, <= 1e-4."""
     err, path = run_forward(wb, oracle, si.CFG1)
