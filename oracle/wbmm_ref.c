@@ -275,3 +275,131 @@ int wbmm_ref_backward(int B, int C, int H, int W, int w, int sh, int sw, int lay
     free(I);
     return 0;
 }
+
+/* ----------------------------------------------------------------------------------------------
+ * Hierarchical window reparameterisation (section 3.6, Eq. 9; PAPER.md:840-893
+ * Algorithms 2 and 3).  Global windows wg x wg (wg = 2 wl, wg = w), each a 2 x 2 grid of local
+ * wl x wl sub-windows; two tables Tg[C][(2wg-1)^2], Tl[C][(2wl-1)^2].  Same orientation (A1),
+ * padding (A4: to a multiple of wg) and shift (A6: over the wg-padded extent) as the single-scale
+ * operator.  transpose != 0 applies the transposed fused matrix (the dX of the operator).
+ *
+ * TRAIN form, Algorithm 2 line by line: per global window
+ *     y_w = Mg x_w + x_w  +  reshape( Ml x_sub + x_sub )          (identity shortcuts)
+ * with the local product taken per sub-window.  No fused matrix is ever formed.
+ */
+int wbmm_ref_hier_forward_train(int B, int C, int H, int W, int w, int sh, int sw, int layout, int transpose,
+                                const double *x, const double *Tg, const double *Tl, double *y)
+{
+    if (B < 0 || C < 0 || H < 1 || W < 1 || w < 2 || (w & 1) || sh < 0 || sw < 0 || sh >= w || sw >= w)
+        return 1;
+    const int wl = w / 2, N = w * w, Nl = wl * wl;
+    const int twg = 2 * w - 1, twl = 2 * wl - 1;
+    const int Hp = padded(H, w), Wp = padded(W, w);
+    const int nwh = Hp / w, nww = Wp / w;
+    const long planes = (long)B * C;
+
+#pragma omp parallel
+    {
+        double *xw = (double *)malloc(sizeof(double) * (size_t)N);
+        double *yw = (double *)malloc(sizeof(double) * (size_t)N);
+#pragma omp for schedule(static)
+        for (long pc = 0; pc < planes; ++pc) {
+            int b = (int)(pc / C), c = (int)(pc % C);
+            const double *Tgc = Tg + (size_t)c * twg * twg, *Tlc = Tl + (size_t)c * twl * twl;
+            for (int wy = 0; wy < nwh; ++wy)
+                for (int wx = 0; wx < nww; ++wx) {
+                    for (int j = 0; j < N; ++j)
+                        xw[j] = load_hat(x, layout, B, C, H, W, Hp, Wp, sh, sw, b, c, wy * w + j / w, wx * w + j % w);
+                    /* global scale with identity shortcut (Alg. 2 l.3-5) */
+                    for (int i = 0; i < N; ++i) {
+                        double acc = 0.0;
+                        for (int j = 0; j < N; ++j) {
+                            int64_t k = transpose ? wbmm_ref_rel_index(w, j, i) : wbmm_ref_rel_index(w, i, j);
+                            acc += Tgc[k] * xw[j];
+                        }
+                        yw[i] = acc + xw[i];
+                    }
+                    /* local scale: 2 x 2 sub-windows, each with its identity shortcut (Alg. 2 l.8-11) */
+                    for (int sr = 0; sr < 2; ++sr)
+                        for (int sc = 0; sc < 2; ++sc)
+                            for (int il = 0; il < Nl; ++il) {
+                                int io = (sr * wl + il / wl) * w + sc * wl + il % wl;     /* position in the global window */
+                                double acc = 0.0;
+                                for (int jl = 0; jl < Nl; ++jl) {
+                                    int jo = (sr * wl + jl / wl) * w + sc * wl + jl % wl;
+                                    int64_t k = transpose ? wbmm_ref_rel_index(wl, jl, il) : wbmm_ref_rel_index(wl, il, jl);
+                                    acc += Tlc[k] * xw[jo];
+                                }
+                                yw[io] += acc + xw[io];                                   /* additive fusion, l.14 */
+                            }
+                    for (int i = 0; i < N; ++i) {
+                        int h = modp(wy * w + i / w + sh, Hp), v = modp(wx * w + i % w + sw, Wp);
+                        if (h < H && v < W) y[elem_off(layout, B, C, H, W, b, c, h, v)] = yw[i];
+                    }
+                }
+        }
+        free(xw); free(yw);
+    }
+    return 0;
+}
+
+/*
+ * FUSED form, Algorithm 3: M_fused = M_g + diag_blocks(M_l + I_49) + I_196, built with the
+ * 9-axis view of the paper (l.8-16), then ONE matrix product per window (l.19-21).
+ * Mfused_out (nullable): [C][N][N], for inspection.
+ */
+int wbmm_ref_hier_forward_fused(int B, int C, int H, int W, int w, int sh, int sw, int layout, int transpose,
+                                const double *x, const double *Tg, const double *Tl, double *y, double *Mfused_out)
+{
+    if (B < 0 || C < 0 || H < 1 || W < 1 || w < 2 || (w & 1) || sh < 0 || sw < 0 || sh >= w || sw >= w)
+        return 1;
+    const int wl = w / 2, N = w * w, Nl = wl * wl;
+    const int nbg = (2 * w - 1) * (2 * w - 1), nbl = (2 * wl - 1) * (2 * wl - 1);
+    const int Hp = padded(H, w), Wp = padded(W, w);
+    const int nwh = Hp / w, nww = Wp / w;
+
+#pragma omp parallel
+    {
+        double *M = (double *)malloc(sizeof(double) * (size_t)N * N);
+        double *Ml = (double *)malloc(sizeof(double) * (size_t)Nl * Nl);
+        double *xw = (double *)malloc(sizeof(double) * (size_t)N);
+#pragma omp for schedule(static)
+        for (int c = 0; c < C; ++c) {
+            /* l.3-4: M_g, M_l by Eq. 8 */
+            for (int i = 0; i < N; ++i)
+                for (int j = 0; j < N; ++j)
+                    M[(size_t)i * N + j] = Tg[(size_t)c * nbg + wbmm_ref_rel_index(w, i, j)];
+            for (int i = 0; i < Nl; ++i)
+                for (int j = 0; j < Nl; ++j)
+                    Ml[(size_t)i * Nl + j] = Tl[(size_t)c * nbl + wbmm_ref_rel_index(wl, i, j)] + (i == j ? 1.0 : 0.0);   /* l.9 */
+            /* l.8, l.11-15: M viewed as (s_out_row, p_out_row, s_out_col, p_out_col, s_in_row, p_in_row, s_in_col, p_in_col);
+               only the blocks with s_out_row = s_in_row = a and s_out_col = s_in_col = e get M_l added */
+            for (int a = 0; a < 2; ++a)
+                for (int e = 0; e < 2; ++e)
+                    for (int por = 0; por < wl; ++por)
+                        for (int poc = 0; poc < wl; ++poc)
+                            for (int pir = 0; pir < wl; ++pir)
+                                for (int pic = 0; pic < wl; ++pic) {
+                                    int i = (a * wl + por) * w + e * wl + poc, j = (a * wl + pir) * w + e * wl + pic;
+                                    M[(size_t)i * N + j] += Ml[(size_t)(por * wl + poc) * Nl + pir * wl + pic];
+                                }
+            for (int i = 0; i < N; ++i) M[(size_t)i * N + i] += 1.0;                                                      /* l.16 */
+            if (Mfused_out) memcpy(Mfused_out + (size_t)c * N * N, M, sizeof(double) * (size_t)N * N);
+            for (int b = 0; b < B; ++b)
+                for (int wy = 0; wy < nwh; ++wy)
+                    for (int wx = 0; wx < nww; ++wx) {
+                        for (int j = 0; j < N; ++j)
+                            xw[j] = load_hat(x, layout, B, C, H, W, Hp, Wp, sh, sw, b, c, wy * w + j / w, wx * w + j % w);
+                        for (int i = 0; i < N; ++i) {
+                            double acc = 0.0;
+                            for (int j = 0; j < N; ++j)
+                                acc += (transpose ? M[(size_t)j * N + i] : M[(size_t)i * N + j]) * xw[j];
+                            int h = modp(wy * w + i / w + sh, Hp), v = modp(wx * w + i % w + sw, Wp);
+                            if (h < H && v < W) y[elem_off(layout, B, C, H, W, b, c, h, v)] = acc;
+                        }
+                    }
+        }
+        free(M); free(Ml); free(xw);
+    }
+    return 0;
+}

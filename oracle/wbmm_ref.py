@@ -52,6 +52,10 @@ def _load():
         f.argtypes = [i] * 8 + [dp, dp, dp]
     lib.wbmm_ref_backward.restype = i
     lib.wbmm_ref_backward.argtypes = [i] * 8 + [dp, dp, dp, dp, dp]
+    lib.wbmm_ref_hier_forward_train.restype = i
+    lib.wbmm_ref_hier_forward_train.argtypes = [i] * 9 + [dp, dp, dp, dp]
+    lib.wbmm_ref_hier_forward_fused.restype = i
+    lib.wbmm_ref_hier_forward_fused.argtypes = [i] * 9 + [dp, dp, dp, dp, dp]
     lib.wbmm_ref_num_threads.restype = i
     lib.wbmm_ref_set_threads.argtypes = [i]
     _lib = lib
@@ -135,3 +139,29 @@ def backward(x, T, dy, w, shift=(0, 0), layout=NCHW, need_dx=True, need_dT=True)
     if rc != 0:
         raise ValueError(f"oracle rejected arguments (rc={rc})")
     return dx, dT
+
+
+def hier_forward(x, Tg, Tl, w, shift=(0, 0), layout=NCHW, form="train", transpose=False, return_matrix=False):
+    """Hierarchical window reparameterisation: global w x w windows with
+    table Tg[C,(2w-1)^2] plus their 2 x 2 local sub-windows with table Tl[C,(w-1)^2], identity
+    shortcuts included.  form = "train" (Algorithm 2: the two scales evaluated separately) or
+    "fused" (Algorithm 3: one fused matrix per channel).  transpose=True applies the transposed
+    operator (dX)."""
+    x, xp = _d(x)
+    Tg, gp = _d(Tg)
+    Tl, lp = _d(Tl)
+    B, C, H, W = _dims(x, layout)
+    assert w % 2 == 0 and Tg.shape == (C, (2 * w - 1) ** 2) and Tl.shape == (C, (w - 1) ** 2)
+    y = np.zeros_like(x)
+    yp = y.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+    args = (B, C, H, W, w, int(shift[0]), int(shift[1]), layout, 1 if transpose else 0, xp, gp, lp, yp)
+    if form == "train":
+        rc = _load().wbmm_ref_hier_forward_train(*args)
+        M = None
+    else:
+        M = np.zeros((C, w * w, w * w)) if return_matrix else None
+        mp = M.ctypes.data_as(ctypes.POINTER(ctypes.c_double)) if return_matrix else ctypes.POINTER(ctypes.c_double)()
+        rc = _load().wbmm_ref_hier_forward_fused(*args, mp)
+    if rc != 0:
+        raise ValueError(f"oracle rejected arguments (rc={rc})")
+    return (y, M) if return_matrix else y

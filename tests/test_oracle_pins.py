@@ -406,3 +406,70 @@ def test_backward_ignores_padded_region(oracle):
     dx, dT = oracle.backward(x, T, dy, w)
     dx2, dT2 = oracle.backward(xp[0], T, xp[1], w)
     assert np.allclose(dT, dT2, atol=1e-13) and np.allclose(dx, dx2[..., :6, :7], atol=1e-13)
+
+
+# ------------------------------------------------------------------ hierarchical reparameterisation (Alg. 2 / 3)
+def _hier_inputs(seed, B, C, H, W, w):
+    r = rng(seed)
+    x = r.standard_normal((B, C, H, W))
+    Tg = 0.05 * r.standard_normal((C, (2 * w - 1) ** 2))
+    Tl = 0.05 * r.standard_normal((C, (w - 1) ** 2))
+    return x, Tg, Tl
+
+
+@pytest.mark.parametrize("w,H,W,s", [(4, 8, 12, (0, 0)), (6, 12, 12, (0, 0)), (4, 10, 7, (1, 3)), (14, 28, 14, (0, 0)), (14, 30, 20, (7, 5))])
+@pytest.mark.parametrize("layout", [NCHW, NHWC])
+def test_hier_training_form_equals_fused_form(oracle, w, H, W, s, layout):
+    """PAPER.md:891 "Algorithms 2 and 3 are functionally identical": the two structurally different
+    evaluations (two scales + shortcuts vs. one fused matrix) agree to round-off, also transposed."""
+    x, Tg, Tl = _hier_inputs(50 + w, 2, 3, H, W, w)
+    xl = _to_layout(x, layout)
+    for tr in (False, True):
+        a = oracle.hier_forward(xl, Tg, Tl, w, s, layout, "train", tr)
+        b = oracle.hier_forward(xl, Tg, Tl, w, s, layout, "fused", tr)
+        assert np.max(np.abs(a - b)) < 1e-12
+
+
+@pytest.mark.parametrize("w", [4, 14])
+def test_hier_is_sum_of_single_scale_operators_plus_two_x(oracle, w):
+    """On maps that are multiples of w the local sub-windows ARE the w/2 partition of the image, so
+    Y = WBMM(x; Tg, w) + WBMM(x; Tl, w/2) + 2x -- reduces the hierarchical oracle to
+    the single-scale one, which is pinned above."""
+    x, Tg, Tl = _hier_inputs(60 + w, 2, 3, 2 * w, 3 * w, w)
+    y = oracle.hier_forward(x, Tg, Tl, w, form="fused")
+    ref = oracle.forward(x, Tg, w) + oracle.forward(x, Tl, w // 2) + 2 * x
+    assert np.max(np.abs(y - ref)) < 1e-12
+
+
+def test_hier_fused_matrix_structure(oracle):
+    """Eq. 9 / Alg. 3: M_fused - M_g is I_196 everywhere plus (M_l + I_49) on the four diagonal
+    sub-window blocks and NOTHING on the cross-sub-window blocks."""
+    w, wl = 14, 7
+    x, Tg, Tl = _hier_inputs(70, 1, 2, w, w, w)
+    _, M = oracle.hier_forward(x, Tg, Tl, w, form="fused", return_matrix=True)
+    Mg = oracle.weight_matrix(Tg, w)
+    Ml = oracle.weight_matrix(Tl, wl)
+    D = (M - Mg).reshape(2, 2, wl, 2, wl, 2, wl, 2, wl)       # (c, s_or, p_or, s_oc, p_oc, s_ir, p_ir, s_ic, p_ic)
+    eye = np.eye(wl * wl).reshape(wl, wl, wl, wl)
+    for a in range(2):
+        for e in range(2):
+            for a2 in range(2):
+                for e2 in range(2):
+                    blk = D[:, a, :, e, :, a2, :, e2, :]      # (c, p_or, p_oc, p_ir, p_ic)
+                    if (a, e) == (a2, e2):
+                        exp = Ml.reshape(2, wl, wl, wl, wl) + 2 * eye[None]
+                        assert np.max(np.abs(blk - exp)) < 1e-14
+                    else:
+                        assert np.max(np.abs(blk)) == 0.0
+    # size printed by the paper: (C, 196, 196) for 14 x 14 windows (PAPER.md:867)
+    assert M.shape == (2, 196, 196)
+
+
+def test_hier_transpose_is_adjoint(oracle):
+    w = 6
+    x, Tg, Tl = _hier_inputs(80, 2, 2, 13, 9, w)
+    r = rng(81)
+    dy = r.standard_normal(x.shape)
+    y = oracle.hier_forward(x, Tg, Tl, w, (2, 5), form="train")
+    dx = oracle.hier_forward(dy, Tg, Tl, w, (2, 5), form="train", transpose=True)
+    assert abs(np.sum(dy * y) - np.sum(dx * x)) < 1e-10
