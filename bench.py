@@ -389,6 +389,12 @@ def run_wbmm(args, rank, world, local):
                   "hbm_frac_at_median": by5 / (statistics.median(t5) * 1e-3) / 1e9 / hbm_peak,
                   "note": "x, y, dy, dx = 154 MB against a 126 MB L2: partly L2-resident between launches"}
 
+    # hierarchical reparameterisation, fused forward on the headline shape: context
+    g_l = torch.Generator(device="cpu").manual_seed(77)
+    Tl = (torch.randn((case.C, (case.w - 1) ** 2), generator=g_l) * 0.02).to(T.dtype).to(dev)
+    hier_ms = region_ms(lambda: wb.wbmm_hier_forward(xs[0], T, Tl, case.w, out=ys[0]))
+    train_step["hier_forward_cfg3_ms"] = hier_ms
+
     tfl_cpu, cores, sample, dt_cpu = time_oracle(case)
     cpu = {"value": tfl_cpu, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
            "seconds": dt_cpu}

@@ -104,6 +104,24 @@ WBMM_API int wbmm_backward(const wbmm_desc_t *desc, const void *x, const void *T
                   void *dx, float *dT, void *cuda_stream);
 
 /*
+ * Hierarchical window reparameterisation, fused (section 3.6, Eq. 9; PAPER.md:862-887
+ * Algorithm 3; identical in value to the training form, Algorithm 2):
+ *     y_win = (M_g + diag_blocks(M_l) + 2 I) * x_win
+ * per global w x w window (desc->w, even), M_g[i,j] = Tg[c, rel_w(i,j)], M_l[i,j] = Tl[c, rel_{w/2}(i,j)]
+ * placed on the four diagonal blocks of the 2 x 2 local sub-windows, 2 I = the two identity shortcuts.
+ * The fused matrix is never formed: both tables are expanded into block-Toeplitz libraries in shared
+ * memory (27 KB instead of the C x 196 x 196 tensor of Algorithm 3).
+ *   Tg [in] C*(2w-1)^2, Tl [in] C*(w-1)^2 elements of desc->dtype.  x, y, padding, shift as wbmm_forward.
+ *   transpose != 0 applies the transposed fused matrix: dX of the operator for dy in `x`.
+ * The table gradients need no entry point of their own: on maps that are multiples of w (no shift)
+ * dTg = wbmm_backward(w) and dTl = wbmm_backward(w/2) of the same (x, dy).
+ * Supported where the pipelined tensor-core kernel is: w = 14, bf16/fp16, NCHW, 16-byte aligned planes
+ * (H*W even ... see wbmm_last_path); otherwise WBMM_STATUS_UNSUPPORTED.
+ */
+WBMM_API int wbmm_hier_forward(const wbmm_desc_t *desc, const void *x, const void *Tg, const void *Tl, void *y,
+                      int transpose, void *cuda_stream);
+
+/*
  * Eq. 6-8 on their own (test/debug and the WBMM-C "cached M" mode):
  *   Wout [out] [C][N][N] elements of desc->dtype, Wout[c,i,j] = T[c, rel(i,j)] copied bit-exactly.
  * Only C, w and dtype of the descriptor are used.

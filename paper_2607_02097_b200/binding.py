@@ -23,7 +23,7 @@ _DTYPES = {torch.float32: DTYPE_F32, torch.bfloat16: DTYPE_BF16, torch.float16: 
 
 # every symbol include/wbmm.h declares
 EXPORTS = (
-    "wbmm_forward", "wbmm_backward", "wbmm_materialize_weight", "wbmm_forward_host",
+    "wbmm_forward", "wbmm_backward", "wbmm_hier_forward", "wbmm_materialize_weight", "wbmm_forward_host",
     "wbmm_backward_host", "wbmm_release", "wbmm_last_path", "wbmm_launch_count",
     "wbmm_status_string", "wbmm_path_string", "wbmm_last_error_string", "wbmm_version",
 )
@@ -55,6 +55,8 @@ def lib() -> ctypes.CDLL:
     vp, dp, i = ctypes.c_void_p, ctypes.POINTER(WbmmDesc), ctypes.c_int
     L.wbmm_forward.argtypes = [dp, vp, vp, vp, vp]
     L.wbmm_backward.argtypes = [dp, vp, vp, vp, vp, vp, vp]
+    L.wbmm_hier_forward.argtypes = [dp, vp, vp, vp, vp, i, vp]
+    L.wbmm_hier_forward.restype = i
     L.wbmm_materialize_weight.argtypes = [dp, vp, vp, vp]
     L.wbmm_forward_host.argtypes = [dp, vp, vp, vp]
     L.wbmm_backward_host.argtypes = [dp, vp, vp, vp, vp, vp]
@@ -123,6 +125,21 @@ def wbmm_forward(x: torch.Tensor, T: torch.Tensor, w: int, shift=(0, 0), layout:
     else:
         with torch.cuda.device(x.device):
             _check(lib().wbmm_forward(ctypes.byref(d), px, pT, py, _stream(x)))
+    return y
+
+
+def wbmm_hier_forward(x: torch.Tensor, Tg: torch.Tensor, Tl: torch.Tensor, w: int, shift=(0, 0),
+                      layout: int = NCHW, transpose: bool = False, out: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """Fused hierarchical operator y = (M_g + diag_blocks(M_l) + 2I) x per w x w window
+    (include/wbmm.h: wbmm_hier_forward); transpose=True gives dX for dy passed as x."""
+    d = make_desc(x, w, shift, layout, 0)
+    if Tg.dtype != x.dtype or Tl.dtype != x.dtype or tuple(Tg.shape) != (d.C, (2 * w - 1) ** 2) \
+            or tuple(Tl.shape) != (d.C, (w - 1) ** 2):
+        raise ValueError("Tg must be [C,(2w-1)^2] and Tl [C,(w-1)^2] in the dtype of x")
+    y = torch.empty_like(x) if out is None else out
+    px, pg, pl, py = _dev(x, "x"), _dev(Tg, "Tg"), _dev(Tl, "Tl"), _dev(y, "y")
+    with torch.cuda.device(x.device):
+        _check(lib().wbmm_hier_forward(ctypes.byref(d), px, pg, pl, py, 1 if transpose else 0, _stream(x)))
     return y
 
 

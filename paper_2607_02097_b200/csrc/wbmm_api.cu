@@ -78,7 +78,7 @@ int apply(const wbmm_desc_t* d, const wbmm::Geom& g, const void* x, const void* 
     }
     if (!(d->flags & WBMM_FLAG_FORCE_SIMT) && wbmm::tc_forward_supported(g, d->dtype, x, y)) {
         int path = WBMM_PATH_NONE;
-        e = wbmm::tc_forward(g, d->dtype, x, T, y, reverse, stream, &launches, &path);
+        e = wbmm::tc_forward(g, d->dtype, x, T, nullptr, y, reverse, stream, &launches, &path);
         g_launches += launches;
         if (e != cudaSuccess) return set_cuda_error(e, "tc_forward");
         t_last_path = path;
@@ -158,6 +158,28 @@ int wbmm_backward(const wbmm_desc_t* desc, const void* x, const void* T, const v
             t_last_path = WBMM_PATH_SIMT;
         }
     }
+    return WBMM_STATUS_OK;
+}
+
+int wbmm_hier_forward(const wbmm_desc_t* desc, const void* x, const void* Tg, const void* Tl, void* y,
+                      int transpose, void* cuda_stream)
+{
+    int st = validate(desc);
+    if (st != WBMM_STATUS_OK) return st;
+    if (desc->w % 2 != 0) return WBMM_STATUS_INVALID_ARGUMENT;
+    if (desc->B == 0 || desc->C == 0) return WBMM_STATUS_OK;
+    if (!x || !Tg || !Tl || !y || x == y) return WBMM_STATUS_INVALID_ARGUMENT;
+    const size_t es = elem_size(desc->dtype);
+    if (!aligned(x, es) || !aligned(Tg, es) || !aligned(Tl, es) || !aligned(y, es)) return WBMM_STATUS_MISALIGNED;
+    if (device_state() < 0) return WBMM_STATUS_NO_DEVICE;
+    wbmm::Geom g = wbmm::make_geom(*desc);
+    if (!wbmm::tc_hier_supported(g, desc->dtype, x, y)) return WBMM_STATUS_UNSUPPORTED;
+    int launches = 0, path = WBMM_PATH_NONE;
+    cudaError_t e = wbmm::tc_forward(g, desc->dtype, x, Tg, Tl, y, transpose != 0, static_cast<cudaStream_t>(cuda_stream),
+                                     &launches, &path);
+    g_launches += launches;
+    if (e != cudaSuccess) return set_cuda_error(e, "tc_forward (hierarchical)");
+    t_last_path = path;
     return WBMM_STATUS_OK;
 }
 

@@ -161,21 +161,23 @@ struct BulkSmem {
     static constexpr int TAB_ONE = ((Cf::NB + 2) * 2 + 15) / 16 * 16;
     static constexpr int TAB_BYTES = 2 * TAB_ONE;                              // F0 and F1 (or Ts for the generic builder)
     static constexpr int BAR_BYTES = (2 * kMaxSlots + 8 + 2 * kMaxOutBufs) * 8;
-    static constexpr int FIXED = BulkCfg<WS>::WC_BYTES + TAB_BYTES + BAR_BYTES;
+    static constexpr int FIXED = BulkCfg<WS>::WC_BYTES + BulkCfg<WS>::HIER_BYTES + TAB_BYTES + BAR_BYTES;
 };
 
 template <int WS, bool BF16, bool GEN>
 __global__ void __launch_bounds__(kThreadsB, 1)
 tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const uint16_t* __restrict__ x, const uint16_t* __restrict__ T,
-               uint16_t* __restrict__ y, int reverse)
+               const uint16_t* __restrict__ Tl, uint16_t* __restrict__ y, int reverse)
 {
     using Cf = WinCfg<WS>;
     using Sm = BulkSmem<WS>;
     extern __shared__ __align__(1024) uint8_t smem[];
     uint8_t* Wc = smem;
     using Bc = BulkCfg<WS>;
-    uint16_t* tab = reinterpret_cast<uint16_t*>(smem + Bc::WC_BYTES);
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + Bc::WC_BYTES + Sm::TAB_BYTES);
+    uint8_t* hier = smem + Bc::WC_BYTES;                    // w = 14: libA | libI | local table (hierarchical operator)
+    uint16_t* tab = reinterpret_cast<uint16_t*>(smem + Bc::WC_BYTES + Bc::HIER_BYTES);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + Bc::WC_BYTES + Bc::HIER_BYTES + Sm::TAB_BYTES);
+    const bool is_hier = Bc::TOEP && Tl != nullptr;
     uint8_t* ring = smem + Sm::FIXED;                       // input ring: nslot frame-image slots
     uint8_t* outb = ring + (size_t)nslot * tl.S;            // output ring: nout group buffers of og.images frame images
     __shared__ uint32_t tmem_base_s;
@@ -222,7 +224,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
     }
     if constexpr (Bc::TOEP) {
         // build_lib14 never writes the padding rows ci = 14, 15 of the blocks: zero the library once
-        for (int i = tid; i < Bc::WC_BYTES / 16; i += kThreadsB) reinterpret_cast<uint4*>(Wc)[i] = make_uint4(0, 0, 0, 0);
+        for (int i = tid; i < (Bc::WC_BYTES + Bc::HIER_BYTES) / 16; i += kThreadsB) reinterpret_cast<uint4*>(Wc)[i] = make_uint4(0, 0, 0, 0);
     }
     for (int i = tid; i < Sm::TAB_BYTES / 4; i += kThreadsB) reinterpret_cast<uint32_t*>(tab)[i] = 0u;
     ptx::fence_proxy_async_smem();
@@ -309,8 +311,21 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                     const uint32_t idesc = ptx::idesc_f16(BF16 ? 1 : 0, 128, Hs::ncols(h));
 #pragma unroll
                     for (int ks = 0; ks < Bc::KSTEPS; ++ks) {
-                        const uint64_t bdesc = ptx::smem_desc_kmajor_noswz(wc_addr + Bc::b_off(ks, h), Bc::LBO, 128);
+                        uint64_t bdesc = ptx::smem_desc_kmajor_noswz(wc_addr + Bc::b_off(ks, h), Bc::LBO, 128);
+                        if constexpr (Bc::TOEP) {
+                            if (is_hier && ks / 7 == h)     // input and output rows in the same half: global + local blocks
+                                bdesc = ptx::smem_desc_kmajor_noswz(wc_addr + Bc::WC_BYTES + Bc::b_off_a(ks, h), Bc::LBO_A, 128);
+                        }
                         ptx::mma_ts(tmem_d + Hs::col0(h), tmem_a + ks * 8, bdesc, idesc, ks > 0 ? 1u : 0u);
+                    }
+                    if constexpr (Bc::TOEP) {
+                        if (is_hier) {      // + 2 x: output row ri takes input row ri through the 2*I block
+                            const uint32_t idesc_i = ptx::idesc_f16(BF16 ? 1 : 0, 128, 16);
+                            const uint64_t idn = ptx::smem_desc_kmajor_noswz(wc_addr + Bc::WC_BYTES + Bc::LIBA_BYTES, Bc::LBO_I, 128);
+#pragma unroll
+                            for (int ri = 7 * h; ri < 7 * h + 7; ++ri)
+                                ptx::mma_ts(tmem_d + ri * 16, tmem_a + ri * 8, idn, idesc_i, 1u);
+                        }
                     }
                     ptx::mma_commit(D_FULL + 8 * h);
                 }
@@ -342,6 +357,16 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                     if (!tabv_ready) table_to_regs14(Tc, reverse != 0, rt, tabv);
                     build_lib14(tabv, tab, tab + Sm::TAB_ONE / 2, Wc, rt);
                     tabv_ready = false;
+                    if (is_hier) {
+                        uint16_t* FL = reinterpret_cast<uint16_t*>(hier + Bc::LIBA_BYTES + Bc::LIBI_BYTES);
+                        const uint16_t* Tlc = Tl + (long long)c * 169;
+                        for (int qq = rt; qq < 169; qq += 128) FL[qq] = Tlc[reverse ? qq : 168 - qq];
+                        // libI = 2*I (the two identity shortcuts): 2.0 is 0x4000 in bf16 and in fp16
+                        if (rt < 14)
+                            *reinterpret_cast<uint16_t*>(hier + Bc::LIBA_BYTES + (rt >> 3) * Bc::LBO_I + rt * 16 + (rt & 7) * 2) = 0x4000;
+                        ptx::named_bar_sync(2, 128);          // the global library and FL are complete
+                        build_lib14_local<BF16>(Wc, FL, hier, rt);
+                    }
                 } else {
                     for (int kk = rt; kk < Cf::NB; kk += 128) tab[kk] = Tc[reverse ? Cf::NB - 1 - kk : kk];
                     ptx::named_bar_sync(2, 128);
@@ -509,7 +534,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
 // load ~1.5-2 us to land, i.e. ~50 KB in flight per SM each way at the ~35 GB/s per SM the copy engine
 // sustains, plus the tile being worked on.  More input in flight measured SLOWER (112 x 112 maps:
 // 4 slots of 25 KB 114 us, 3 slots 104 us; also for a plain bulk-copy ring,
-// DESIGN.md section 7.6); less starves small tiles (w = 7: 12.5 KB per tile).
+// DESIGN.md section 7.7); less starves small tiles (w = 7: 12.5 KB per tile).
 // Returns false when a tile of output plus a tile + 1 of input does not fit.
 template <int WS>
 bool bulk_slots(const TcTiles& tl, int wpf, int* nslot, int* nout)
@@ -550,8 +575,8 @@ int bulk_mode(const Geom& g, const TcTiles& tl, const void* x, const void* y)
 }
 
 template <int WS, bool BF16, bool GEN>
-cudaError_t launch_bulk(const Geom& g, const TcTiles& tl, const void* x, const void* T, void* y, bool reverse,
-                        cudaStream_t s)
+cudaError_t launch_bulk(const Geom& g, const TcTiles& tl, const void* x, const void* T, const void* Tl, void* y,
+                        bool reverse, cudaStream_t s)
 {
     auto k = tc_bulk_kernel<WS, BF16, GEN>;
     int nslot = 0, nout = 0;
@@ -588,7 +613,8 @@ cudaError_t launch_bulk(const Geom& g, const TcTiles& tl, const void* x, const v
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, k, g, tl, part, nslot, nout, (const uint16_t*)x, (const uint16_t*)T, (uint16_t*)y,
+    return cudaLaunchKernelEx(&cfg, k, g, tl, part, nslot, nout, (const uint16_t*)x, (const uint16_t*)T, (const uint16_t*)Tl,
+                              (uint16_t*)y,
                               reverse ? 1 : 0);
 }
 
@@ -727,7 +753,16 @@ bool tc_forward_supported(const Geom& g, int dtype, const void*, const void*)
     return smem <= 227 * 1024 - 64;
 }
 
-cudaError_t tc_forward(const Geom& g, int dtype, const void* x, const void* T, void* y, bool reverse,
+bool tc_hier_supported(const Geom& g, int dtype, const void* x, const void* y)
+{
+    if (dtype != WBMM_DTYPE_BF16 && dtype != WBMM_DTYPE_F16) return false;
+    if (g.w != 14) return false;
+    TcTiles tl;
+    if (!tc_tiles(g, &tl)) return false;
+    return bulk_mode<14>(g, tl, x, y) != 0;
+}
+
+cudaError_t tc_forward(const Geom& g, int dtype, const void* x, const void* T, const void* Tl, void* y, bool reverse,
                        cudaStream_t stream, int* launches, int* path)
 {
     TcTiles tl;
@@ -740,16 +775,17 @@ cudaError_t tc_forward(const Geom& g, int dtype, const void* x, const void* T, v
         *path = WBMM_PATH_TC_TMA;
         const int sel = (g.w == 7 ? 0 : 4) + (bf ? 2 : 0) + (mode == 2 ? 1 : 0);
         switch (sel) {
-        case 0: return launch_bulk<7, false, false>(g, tl, x, T, y, reverse, stream);
-        case 1: return launch_bulk<7, false, true>(g, tl, x, T, y, reverse, stream);
-        case 2: return launch_bulk<7, true, false>(g, tl, x, T, y, reverse, stream);
-        case 3: return launch_bulk<7, true, true>(g, tl, x, T, y, reverse, stream);
-        case 4: return launch_bulk<14, false, false>(g, tl, x, T, y, reverse, stream);
-        case 5: return launch_bulk<14, false, true>(g, tl, x, T, y, reverse, stream);
-        case 6: return launch_bulk<14, true, false>(g, tl, x, T, y, reverse, stream);
-        default: return launch_bulk<14, true, true>(g, tl, x, T, y, reverse, stream);
+        case 0: return launch_bulk<7, false, false>(g, tl, x, T, Tl, y, reverse, stream);
+        case 1: return launch_bulk<7, false, true>(g, tl, x, T, Tl, y, reverse, stream);
+        case 2: return launch_bulk<7, true, false>(g, tl, x, T, Tl, y, reverse, stream);
+        case 3: return launch_bulk<7, true, true>(g, tl, x, T, Tl, y, reverse, stream);
+        case 4: return launch_bulk<14, false, false>(g, tl, x, T, Tl, y, reverse, stream);
+        case 5: return launch_bulk<14, false, true>(g, tl, x, T, Tl, y, reverse, stream);
+        case 6: return launch_bulk<14, true, false>(g, tl, x, T, Tl, y, reverse, stream);
+        default: return launch_bulk<14, true, true>(g, tl, x, T, Tl, y, reverse, stream);
         }
     }
+    if (Tl) return cudaErrorNotSupported;      // the hierarchical operator exists in the bulk kernel only
     *path = WBMM_PATH_TC_GATHER;
     if (g.w == 7)
         return bf ? launch_generic<7, true>(g, tl, x, T, y, reverse, stream)

@@ -24,8 +24,10 @@ bool tc_tiles(const Geom& g, TcTiles* t);
 
 // True when a tcgen05 forward kernel can serve this problem.
 bool tc_forward_supported(const Geom& g, int dtype, const void* x, const void* y);
-cudaError_t tc_forward(const Geom& g, int dtype, const void* x, const void* T, void* y, bool reverse,
+// Tl != nullptr: the hierarchical operator (global table T, local table Tl; w = 14, bulk kernel only).
+cudaError_t tc_forward(const Geom& g, int dtype, const void* x, const void* T, const void* Tl, void* y, bool reverse,
                        cudaStream_t stream, int* launches, int* path);
+bool tc_hier_supported(const Geom& g, int dtype, const void* x, const void* y);
 
 // NHWC forward / dX: 8-channel groups gathered with 16-byte cp.async (wbmm_tc_nhwc.cu).
 bool tc_nhwc_supported(const Geom& g, int dtype, const void* x, const void* y);

@@ -195,6 +195,7 @@ struct BulkCfg {
     static constexpr int word1(int) { return Cf::NW; }
     // byte offset of the B operand of K-step ks, half h, inside the weight area
     static constexpr int b_off(int ks, int) { return ks * 2 * LBO; }
+    static constexpr int HIER_BYTES = 0;
 };
 
 template <>
@@ -214,6 +215,18 @@ struct BulkCfg<14> {
     static constexpr int word0(int h) { return h * 49; }
     static constexpr int word1(int h) { return (h + 1) * 49; }
     static constexpr int b_off(int ks, int h) { return ((13 - ks) * RP + h * 7 * RP) * 16; }
+    // Hierarchical reparameterisation (Eq. 9): inside one half of the window rows
+    // (ri/7 == rj/7) the block of the fused matrix is Z_g[dr] + Z_l'[dr], |dr| <= 6, where Z_l' holds the
+    // local table on its two 7 x 7 diagonal sub-blocks: a second library of 13 blocks; the two identity
+    // shortcuts are a 16 x 16 block 2*I applied by 14 extra N = 16 MMAs (kept out of the 16-bit sums).
+    static constexpr int LIBA_ROWS = 13 * RP;          // 208
+    static constexpr int LBO_A = LIBA_ROWS * 16;
+    static constexpr int LIBA_BYTES = 2 * LBO_A;       // 6656
+    static constexpr int LBO_I = RP * 16;
+    static constexpr int LIBI_BYTES = 2 * LBO_I;       // 512
+    static constexpr int TL_BYTES = 352;               // 13 x 13 local table, staged reversed
+    static constexpr int HIER_BYTES = LIBA_BYTES + LIBI_BYTES + TL_BYTES;
+    static constexpr int b_off_a(int ks, int h) { return (7 * h - ks + 6) * RP * 16; }   // valid when ks / 7 == h
 };
 
 // NCOLS fp32 accumulator columns (multiple of 16) -> NCOLS/2 packed 16-bit pairs (RNE).
@@ -536,6 +549,45 @@ __device__ __forceinline__ void build_lib14(const uint16_t* v, uint16_t* F0, uin
     }
 }
 
+
+// Second library of the hierarchical operator (BulkCfg<14>): libA[da] = lib[da + 7] + Z_l'[da - 6], da = 0..12,
+// Z_l'[dr][ci][cj] = [ci/7 == cj/7] * T_l[(dr+6)*13 + (ci-cj+6)]; FL = the local table staged reversed
+// (FL[q] = T_l[168 - q], or T_l[q] for the transposed operator).  Sums are rounded (RNE) to the 16-bit type.
+// 128 threads, after build_lib14 and a barrier among them.
+template <bool BF16>
+__device__ __forceinline__ uint32_t add_pairs(uint32_t a, uint32_t b)
+{
+    if constexpr (BF16) {
+        __nv_bfloat162 r = __hadd2(*reinterpret_cast<__nv_bfloat162*>(&a), *reinterpret_cast<__nv_bfloat162*>(&b));
+        return *reinterpret_cast<uint32_t*>(&r);
+    } else {
+        __half2 r = __hadd2(*reinterpret_cast<__half2*>(&a), *reinterpret_cast<__half2*>(&b));
+        return *reinterpret_cast<uint32_t*>(&r);
+    }
+}
+
+template <bool BF16>
+__device__ __forceinline__ void build_lib14_local(const uint8_t* lib, const uint16_t* FL, uint8_t* libA, int tid)
+{
+    using Bc = BulkCfg<14>;
+    for (int id = tid; id < 13 * 28; id += 128) {
+        const int da = id / 28, rem = id - da * 28, ci = rem >> 1, kc = rem & 1;
+        const uint4 g = *reinterpret_cast<const uint4*>(lib + kc * Bc::LBO + ((da + 7) * 16 + ci) * 16);
+        uint32_t l[4];
+#pragma unroll
+        for (int e2 = 0; e2 < 4; ++e2) {
+            uint32_t w = 0;
+#pragma unroll
+            for (int hh = 0; hh < 2; ++hh) {
+                const int cj = 8 * kc + 2 * e2 + hh;
+                if (cj < 14 && (ci >= 7) == (cj >= 7)) w |= (uint32_t)FL[(12 - da) * 13 + 6 - ci + cj] << (16 * hh);
+            }
+            l[e2] = w;
+        }
+        *reinterpret_cast<uint4*>(libA + kc * Bc::LBO_A + (da * 16 + ci) * 16) =
+            make_uint4(add_pairs<BF16>(g.x, l[0]), add_pairs<BF16>(g.y, l[1]), add_pairs<BF16>(g.z, l[2]), add_pairs<BF16>(g.w, l[3]));
+    }
+}
 
 constexpr int kThreadsB = 352;
 constexpr int kMaxSlots = 96;

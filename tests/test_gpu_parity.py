@@ -158,6 +158,74 @@ def test_pipelined_kernels_one_hot_bins_bitwise(wb, oracle, w, shift, H, W, layo
     assert np.array_equal(widen(dx), rdx)
 
 
+# ------------------------------------------------------------------ hierarchical reparameterisation (NEXT-1)
+def _hier_case(case):
+    d = si.make(case, device="cuda")
+    g = torch.Generator().manual_seed(case.seed + 7)
+    Tl = (torch.randn((case.C, (case.w - 1) ** 2), generator=g) * 0.02).to(d["T"].dtype).cuda()
+    return d, Tl
+
+
+@pytest.mark.parametrize("case", [
+    si.Case("h_plain", 19, 5, 56, 56, 14, seed=41),
+    si.Case("h_many", 40, 150, 28, 28, 14, seed=42),
+    si.Case("h_shift", 9, 7, 28, 56, 14, shift=(7, 3), seed=43),
+    si.Case("h_ragged", 7, 6, 60, 60, 14, seed=44),
+    si.Case("h_strips", 2, 3, 224, 224, 14, seed=45),
+    si.Case("h_f16", 10, 9, 42, 56, 14, dtype="f16", shift=(0, 7), seed=46),
+], ids=lambda c: c.name)
+@pytest.mark.parametrize("transpose", [False, True])
+def test_hier_forward_matches_oracle(wb, oracle, case, transpose):
+    """Fused hierarchical operator (Alg. 3) on the GPU against the oracle's TRAINING form (Alg. 2)."""
+    d, Tl = _hier_case(case)
+    y = wb.wbmm_hier_forward(d["x"], d["T"], Tl, case.w, case.shift, case.layout, transpose)
+    torch.cuda.synchronize()
+    assert wb.wbmm_last_path() == wb.PATH_TC_TMA
+    ref = oracle.hier_forward(widen(d["x"]), widen(d["T"]), widen(Tl), case.w, case.shift, case.layout, "train", transpose)
+    # |y| is ~2|x| here (two identity shortcuts): same bound form, |ref| carries the scale
+    assert max_err_over_tol(y, ref, TOL[case.dtype]) <= 1.0
+
+
+def test_hier_zero_tables_is_exactly_two_x(wb):
+    """Both tables zero => y = 2x bitwise: pins the identity blocks (14 extra N=16 MMAs) alone."""
+    case = si.Case("h_2x", 9, 6, 56, 56, 14, seed=47)
+    d, Tl = _hier_case(case)
+    y = wb.wbmm_hier_forward(d["x"], torch.zeros_like(d["T"]), torch.zeros_like(Tl), 14)
+    assert torch.equal(y, (2 * d["x"].float()).to(d["x"].dtype))
+
+
+@pytest.mark.parametrize("which", ["global", "local"])
+def test_hier_one_hot_tables_bitwise(wb, oracle, which):
+    """One-hot global table (local zero) and one-hot local table (global zero): y - 2x is a pure shift
+    inside the window / inside the 7 x 7 sub-window; small-integer x keeps every sum exact in bf16, so
+    the GPU result must equal the oracle bitwise.  Pins which library (global / global+local) serves
+    which (row-half, K-step) pair and the sub-window masks."""
+    C = 96
+    case = si.Case("h_onehot", 5, C, 28, 56, 14, seed=48)
+    gen = torch.Generator().manual_seed(49)
+    x = torch.randint(-3, 4, (case.B, C, case.H, case.W), generator=gen).to(torch.bfloat16).cuda()
+    Tg = torch.zeros((C, 729), dtype=torch.bfloat16, device="cuda")
+    Tl = torch.zeros((C, 169), dtype=torch.bfloat16, device="cuda")
+    if which == "global":
+        bins = torch.randint(0, 729, (C,), generator=gen)
+        Tg[torch.arange(C), bins.cuda()] = 1.0
+    else:
+        bins = torch.randint(0, 169, (C,), generator=gen)
+        bins[:4] = torch.tensor([0, 168, 84, 12])
+        Tl[torch.arange(C), bins.cuda()] = 1.0
+    for transpose in (False, True):
+        y = wb.wbmm_hier_forward(x, Tg, Tl, 14, transpose=transpose)
+        ref = oracle.hier_forward(widen(x), widen(Tg), widen(Tl), 14, form="fused", transpose=transpose)
+        assert np.array_equal(widen(y), ref)
+
+
+def test_hier_unsupported_shapes_fail_loudly(wb):
+    x = torch.zeros((2, 4, 14, 14), dtype=torch.bfloat16, device="cuda")
+    with pytest.raises(wb.WbmmError):       # w = 7 has no hierarchical tensor-core path
+        wb.wbmm_hier_forward(x, torch.zeros((4, 169), dtype=torch.bfloat16, device="cuda"),
+                             torch.zeros((4, 36), dtype=torch.bfloat16, device="cuda"), 7)
+
+
 def test_config1_fp32_tiny(wb, oracle):
     """BASELINE.json config 1: fp32 path, <= 1e-4."""
     err, path = run_forward(wb, oracle, si.CFG1)
