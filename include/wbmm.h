@@ -24,6 +24,10 @@
  *     do: they return after the result is in host memory).
  *   - Return value: a wbmm_status_t.  Nothing throws or aborts across the ABI.  On a non-zero
  *     status no output buffer has been written.
+ *   - NHWC activations (bf16/fp16, C and H*W multiples of 8) are served by transposing to NCHW and back around
+ *     the NCHW kernels; the two temporaries come from cudaMallocAsync / cudaFreeAsync on the caller's stream
+ *     (stream-ordered, capturable in CUDA graphs) and never outlive the call's work.  WBMM_FLAG_NO_SCRATCH
+ *     selects the scratch-free in-kernel NHWC path instead.  Every other path allocates nothing.
  *   - There is no CPU fallback.  Without a CUDA device of compute capability 10.x every compute
  *     entry point returns WBMM_STATUS_NO_DEVICE.
  */
@@ -62,12 +66,15 @@ typedef enum {
     WBMM_PATH_NONE = 0,
     WBMM_PATH_SIMT = 1,      /* general fp32-FFMA kernels: any w, dtype, layout, shift, ragged size */
     WBMM_PATH_TC_TMA = 2,    /* tcgen05/TMEM tensor-core kernels fed by TMA window loads (bf16/fp16) */
-    WBMM_PATH_TC_GATHER = 3  /* tcgen05/TMEM kernels fed by a predicated gather loader (bf16/fp16) */
+    WBMM_PATH_TC_GATHER = 3, /* tcgen05/TMEM kernels fed by a predicated gather loader (bf16/fp16) */
+    WBMM_PATH_TC_TRANSPOSED = 4 /* NHWC: transposition passes through stream-ordered scratch around the TC_TMA kernels */
 } wbmm_path_t;
 
 enum {
     WBMM_FLAG_ACCUMULATE_DT = 1u, /* wbmm_backward: add into dT instead of overwriting it */
-    WBMM_FLAG_FORCE_SIMT = 2u     /* never take a tensor-core path (testing / cross-checks) */
+    WBMM_FLAG_FORCE_SIMT = 2u,    /* never take a tensor-core path (testing / cross-checks) */
+    WBMM_FLAG_NO_SCRATCH = 4u     /* NHWC: never allocate transposition scratch (cudaMallocAsync on the stream); use the
+                                     in-kernel NHWC kernels, which are 2.5-20x slower */
 };
 
 /* Problem descriptor (plain data, passed by pointer, read during the call only). */

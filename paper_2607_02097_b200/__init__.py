@@ -5,8 +5,8 @@ thin Python binding with the same names.  Importing the package does not load th
 the first call does, and raises if it has not been built (no CPU fallback).
 """
 from .binding import (  # noqa: F401
-    NCHW, NHWC, FLAG_ACCUMULATE_DT, FLAG_FORCE_SIMT,
-    PATH_NONE, PATH_SIMT, PATH_TC_TMA, PATH_TC_GATHER,
+    NCHW, NHWC, FLAG_ACCUMULATE_DT, FLAG_FORCE_SIMT, FLAG_NO_SCRATCH,
+    PATH_NONE, PATH_SIMT, PATH_TC_TMA, PATH_TC_GATHER, PATH_TC_TRANSPOSED,
     WbmmDesc, WbmmError,
     wbmm_forward, wbmm_backward, wbmm_hier_forward, wbmm_materialize_weight,
     wbmm_forward_host, wbmm_backward_host, wbmm_release,

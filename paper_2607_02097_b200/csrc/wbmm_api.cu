@@ -63,12 +63,64 @@ int validate(const wbmm_desc_t* d)
 
 bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
 
+// NHWC through NCHW: stream-ordered temporaries.
+struct AsyncScratch {
+    void* p = nullptr;
+    cudaStream_t s;
+    explicit AsyncScratch(cudaStream_t stream) : s(stream) {}
+    cudaError_t alloc(size_t n)
+    {
+        // Keep freed blocks cached in the device's default pool (its default is to hand memory back to the
+        // driver at the next synchronisation, which makes every call pay a fresh allocation).
+        static std::once_flag once;
+        std::call_once(once, [] {
+            int dev = 0;
+            cudaMemPool_t pool;
+            if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+                uint64_t keep = ~0ull;
+                cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+            }
+            cudaGetLastError();
+        });
+        return cudaMallocAsync(&p, n, s);
+    }
+    ~AsyncScratch() { if (p) cudaFreeAsync(p, s); }
+};
+
+bool nhwc_scratch_candidate(const wbmm_desc_t* d, const wbmm::Geom& g)
+{
+    if (g.layout != WBMM_LAYOUT_NHWC || (d->flags & (WBMM_FLAG_FORCE_SIMT | WBMM_FLAG_NO_SCRATCH))) return false;
+    if (d->dtype != WBMM_DTYPE_BF16 && d->dtype != WBMM_DTYPE_F16) return false;
+    return g.C % 8 == 0 && ((long long)g.H * g.W) % 8 == 0;
+}
+
 // One operator application y = op(x; T) with op = W_c (reverse=false) or W_c^T (reverse=true).
 int apply(const wbmm_desc_t* d, const wbmm::Geom& g, const void* x, const void* T, void* y,
           bool reverse, cudaStream_t stream)
 {
     int launches = 0;
     cudaError_t e;
+    if (nhwc_scratch_candidate(d, g)) {
+        wbmm::Geom gn = g;
+        gn.layout = WBMM_LAYOUT_NCHW;
+        void* const aligned16 = reinterpret_cast<void*>(256);
+        if (wbmm::tc_bulk_supported(gn, d->dtype, aligned16, aligned16) &&
+            wbmm::transpose16_supported((long long)g.H * g.W, g.C, x, y)) {
+            const size_t nbytes = (size_t)g.B * g.C * g.H * g.W * 2;
+            AsyncScratch xt(stream), yt(stream);
+            if (xt.alloc(nbytes) == cudaSuccess && yt.alloc(nbytes) == cudaSuccess) {
+                int path = WBMM_PATH_NONE;
+                e = wbmm::transpose16(x, xt.p, g.B, g.H * g.W, g.C, stream, &launches);
+                if (e == cudaSuccess) e = wbmm::tc_forward(gn, d->dtype, xt.p, T, nullptr, yt.p, reverse, stream, &launches, &path);
+                if (e == cudaSuccess) e = wbmm::transpose16(yt.p, y, g.B, g.C, g.H * g.W, stream, &launches);
+                g_launches += launches;
+                if (e != cudaSuccess) return set_cuda_error(e, "NHWC via NCHW scratch");
+                t_last_path = WBMM_PATH_TC_TRANSPOSED;
+                return WBMM_STATUS_OK;
+            }
+            cudaGetLastError();      // no stream-ordered allocator / out of memory: in-kernel NHWC path below
+        }
+    }
     if (!(d->flags & WBMM_FLAG_FORCE_SIMT) && wbmm::tc_nhwc_supported(g, d->dtype, x, y)) {
         e = wbmm::tc_nhwc_forward(g, d->dtype, x, T, y, reverse, stream, &launches);
         g_launches += launches;
@@ -144,7 +196,30 @@ int wbmm_backward(const wbmm_desc_t* desc, const void* x, const void* T, const v
         }
         int launches = 0;
         cudaError_t e;
-        if (!(desc->flags & WBMM_FLAG_FORCE_SIMT) && wbmm::tc_grad_table_supported(g, desc->dtype, x, dy)) {
+        bool done = false;
+        if (nhwc_scratch_candidate(desc, g) && wbmm::transpose16_supported((long long)g.H * g.W, g.C, x, dy)) {
+            wbmm::Geom gn = g;
+            gn.layout = WBMM_LAYOUT_NCHW;
+            void* const aligned16 = reinterpret_cast<void*>(256);
+            if (wbmm::tc_grad_table_supported(gn, desc->dtype, aligned16, aligned16)) {
+                const size_t nbytes = (size_t)g.B * g.C * g.H * g.W * 2;
+                AsyncScratch xt(stream), gt(stream);
+                if (xt.alloc(nbytes) == cudaSuccess && gt.alloc(nbytes) == cudaSuccess) {
+                    int path = WBMM_PATH_NONE;
+                    e = wbmm::transpose16(x, xt.p, g.B, g.H * g.W, g.C, stream, &launches);
+                    if (e == cudaSuccess) e = wbmm::transpose16(dy, gt.p, g.B, g.H * g.W, g.C, stream, &launches);
+                    if (e == cudaSuccess) e = wbmm::tc_grad_table(gn, desc->dtype, xt.p, gt.p, dT, stream, &launches, &path);
+                    g_launches += launches;
+                    if (e != cudaSuccess) return set_cuda_error(e, "NHWC dT via NCHW scratch");
+                    t_last_path = WBMM_PATH_TC_TRANSPOSED;
+                    done = true;
+                } else {
+                    cudaGetLastError();
+                }
+            }
+        }
+        if (done) {
+        } else if (!(desc->flags & WBMM_FLAG_FORCE_SIMT) && wbmm::tc_grad_table_supported(g, desc->dtype, x, dy)) {
             int path = WBMM_PATH_NONE;
             e = wbmm::tc_grad_table(g, desc->dtype, x, dy, dT, stream, &launches, &path);
             g_launches += launches;
@@ -344,6 +419,7 @@ const char* wbmm_path_string(int path)
     case WBMM_PATH_SIMT: return "simt";
     case WBMM_PATH_TC_TMA: return "tcgen05+tma";
     case WBMM_PATH_TC_GATHER: return "tcgen05+gather";
+    case WBMM_PATH_TC_TRANSPOSED: return "tcgen05+tma via NCHW scratch";
     default: return "unknown path";
     }
 }

@@ -753,6 +753,15 @@ bool tc_forward_supported(const Geom& g, int dtype, const void*, const void*)
     return smem <= 227 * 1024 - 64;
 }
 
+bool tc_bulk_supported(const Geom& g, int dtype, const void* x, const void* y)
+{
+    if (dtype != WBMM_DTYPE_BF16 && dtype != WBMM_DTYPE_F16) return false;
+    if (g.w != 7 && g.w != 14) return false;
+    TcTiles tl;
+    if (!tc_tiles(g, &tl)) return false;
+    return (g.w == 7 ? bulk_mode<7>(g, tl, x, y) : bulk_mode<14>(g, tl, x, y)) != 0;
+}
+
 bool tc_hier_supported(const Geom& g, int dtype, const void* x, const void* y)
 {
     if (dtype != WBMM_DTYPE_BF16 && dtype != WBMM_DTYPE_F16) return false;

@@ -28,6 +28,8 @@ bool tc_forward_supported(const Geom& g, int dtype, const void* x, const void* y
 cudaError_t tc_forward(const Geom& g, int dtype, const void* x, const void* T, const void* Tl, void* y, bool reverse,
                        cudaStream_t stream, int* launches, int* path);
 bool tc_hier_supported(const Geom& g, int dtype, const void* x, const void* y);
+// True when the pipelined bulk kernel (not the gather fallback) serves this NCHW problem.
+bool tc_bulk_supported(const Geom& g, int dtype, const void* x, const void* y);
 
 // NHWC forward / dX: 8-channel groups gathered with 16-byte cp.async (wbmm_tc_nhwc.cu).
 bool tc_nhwc_supported(const Geom& g, int dtype, const void* x, const void* y);

@@ -112,18 +112,26 @@ PIPE = [
 ]
 
 
+def _nhwc_path(wb, case, flags):
+    """NHWC: transposition scratch around the NCHW kernels when C and H*W are multiples of 8, else (or with
+    FLAG_NO_SCRATCH) the in-kernel 8-channel-group kernels."""
+    via_scratch = not (flags & wb.FLAG_NO_SCRATCH) and case.C % 8 == 0 and (case.H * case.W) % 8 == 0
+    return wb.PATH_TC_TRANSPOSED if via_scratch else wb.PATH_TC_GATHER
+
+
 @pytest.mark.parametrize("case", PIPE, ids=lambda c: c.name)
-@pytest.mark.parametrize("layout", [NCHW, NHWC])
-def test_pipelined_kernels_forward_backward(wb, oracle, case, layout):
-    C = case.C if layout == NCHW else -(-case.C // 8) * 8                     # NHWC kernel: 8-channel groups
+@pytest.mark.parametrize("layout,no_scratch", [(NCHW, False), (NHWC, False), (NHWC, True)])
+def test_pipelined_kernels_forward_backward(wb, oracle, case, layout, no_scratch):
+    C = case.C if layout == NCHW else -(-case.C // 8) * 8                     # NHWC paths: 8-channel groups
     case = si.with_(case, layout=layout, C=C, backward=True)
+    flags = wb.FLAG_NO_SCRATCH if no_scratch else 0
     d = si.make(case, device="cuda")
-    y = wb.wbmm_forward(d["x"], d["T"], case.w, case.shift, case.layout)
+    y = wb.wbmm_forward(d["x"], d["T"], case.w, case.shift, case.layout, flags)
     torch.cuda.synchronize()
     path = wb.wbmm_last_path()
     if case.name != "p_w7_ragged":
-        assert path == (wb.PATH_TC_TMA if layout == NCHW else wb.PATH_TC_GATHER), wb.wbmm_path_string(path)
-    dx, dT = wb.wbmm_backward(d["x"], d["T"], d["dy"], case.w, case.shift, case.layout)
+        assert path == (wb.PATH_TC_TMA if layout == NCHW else _nhwc_path(wb, case, flags)), wb.wbmm_path_string(path)
+    dx, dT = wb.wbmm_backward(d["x"], d["T"], d["dy"], case.w, case.shift, case.layout, flags)
     torch.cuda.synchronize()
     ry = oracle.forward(widen(d["x"]), widen(d["T"]), case.w, case.shift, case.layout, "direct")
     rdx, rdT = oracle.backward(widen(d["x"]), widen(d["T"]), widen(d["dy"]), case.w, case.shift, case.layout)
@@ -134,8 +142,8 @@ def test_pipelined_kernels_forward_backward(wb, oracle, case, layout):
 
 @pytest.mark.parametrize("w,shift,H,W", [(14, (0, 0), 56, 56), (14, (7, 7), 28, 56), (14, (2, 5), 60, 60),
                                          (7, (0, 0), 56, 56), (7, (3, 4), 28, 28)])
-@pytest.mark.parametrize("layout", [NCHW, NHWC])
-def test_pipelined_kernels_one_hot_bins_bitwise(wb, oracle, w, shift, H, W, layout):
+@pytest.mark.parametrize("layout,no_scratch", [(NCHW, False), (NHWC, False), (NHWC, True)])
+def test_pipelined_kernels_one_hot_bins_bitwise(wb, oracle, w, shift, H, W, layout, no_scratch):
     """One-hot tables through the pipelined kernels (bulk / NHWC group kernel): pure data movement,
     so the result must equal the oracle's bitwise -- the bit-exact indexing test of the Toeplitz
     library, the word-granular shift / padding addressing and the NHWC transposition."""
@@ -149,11 +157,12 @@ def test_pipelined_kernels_one_hot_bins_bitwise(wb, oracle, w, shift, H, W, layo
     bins[0], bins[1], bins[2] = 0, nb - 1, (w - 1) * tw + (w - 1)            # corners and the centre
     T = torch.zeros_like(d["T"])
     T[torch.arange(C), bins.to(T.device)] = 1.0
-    y = wb.wbmm_forward(d["x"], T, w, shift, layout)
-    assert wb.wbmm_last_path() == (wb.PATH_TC_TMA if layout == NCHW else wb.PATH_TC_GATHER)
+    flags = wb.FLAG_NO_SCRATCH if no_scratch else 0
+    y = wb.wbmm_forward(d["x"], T, w, shift, layout, flags)
+    assert wb.wbmm_last_path() == (wb.PATH_TC_TMA if layout == NCHW else _nhwc_path(wb, case, flags))
     ref = oracle.forward(widen(d["x"]), widen(T), w, shift, layout)
     assert np.array_equal(widen(y), ref)
-    dx, _ = wb.wbmm_backward(None, T, d["x"], w, shift, layout, need_dT=False)
+    dx, _ = wb.wbmm_backward(None, T, d["x"], w, shift, layout, flags, need_dT=False)
     rdx, _ = oracle.backward(widen(d["x"]), widen(T), widen(d["x"]), w, shift, layout, need_dT=False)
     assert np.array_equal(widen(dx), rdx)
 
