@@ -32,11 +32,14 @@ struct DtCfg {
     static constexpr int MT = (Cf::N + 127) / 128;     // M tiles of 128 output positions
     static constexpr int NV = (Cf::N + 7) / 8;         // 16-byte vectors a window fills
     static constexpr int NVEC = Cf::N_PAD / 8;         // vectors per operand region
-    static constexpr int SBO = 128 * 16;               // bytes between position groups (128 windows x 16 B)
+    // The stage is two HALVES of 64 windows (K = 64 each): the repack of one half overlaps the MMAs of the other.
+    static constexpr int HW = 64;                      // windows per half
+    static constexpr int SBO = HW * 16;                // bytes between position groups (64 windows x 16 B)
     static constexpr int LBO = 128;                    // bytes between groups of 8 windows
-    static constexpr int OP_BYTES = NVEC * SBO;
-    static constexpr int STAGE = 2 * OP_BYTES;         // A region then B region; an M-tile's 16 vectors may run into B
-    static constexpr int BAR_BYTES = (2 * kMaxSlots + 8) * 8;
+    static constexpr int OP_BYTES = NVEC * SBO;        // one operand of one half
+    static constexpr int HALF = 2 * OP_BYTES;          // A region then B region; an M-tile's 16 vectors may run into B
+    static constexpr int STAGE = 2 * HALF;
+    static constexpr int BAR_BYTES = (2 * kMaxSlots + 8) * 8;   // slots + STAGE_FULL[2] + STAGE_EMPTY[2]
     static constexpr int FIXED = STAGE + BAR_BYTES;
     static_assert(MT * 16 <= 2 * NVEC, "an A M-tile must stay inside the stage");
     static_assert(8 * Cf::NB * 4 <= STAGE, "per-warp bin copies alias the stage");
@@ -59,7 +62,7 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
     const uint32_t bar0 = ptx::smem_u32(bars);
     auto FULL = [&](int s) { return bar0 + 8u * s; };
     auto EMPTY = [&](int s) { return bar0 + 8u * (kMaxSlots + s); };
-    const uint32_t STAGE_FULL = bar0 + 8u * (2 * kMaxSlots), STAGE_EMPTY = STAGE_FULL + 8;
+    const uint32_t STAGE_FULL = bar0 + 8u * (2 * kMaxSlots), STAGE_EMPTY = STAGE_FULL + 16;   // [2 halves] each
     const int wpf = tl.NSY * g.nww;
 
     if (warp == 1) ptx::tmem_alloc(ptx::smem_u32(&tmem_base_s), 512);
@@ -69,8 +72,10 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
         ptx::fence_mbar_init();
     }
     if (tid == 0) {
-        ptx::mbar_init(STAGE_FULL, 256);
-        ptx::mbar_init(STAGE_EMPTY, 1);
+        for (int hf = 0; hf < 2; ++hf) {
+            ptx::mbar_init(STAGE_FULL + 8 * hf, 2 * Dc::HW);      // 64 windows x (x, dy)
+            ptx::mbar_init(STAGE_EMPTY + 8 * hf, 1);
+        }
         ptx::fence_mbar_init();
     }
     // vectors a window never writes (padding positions) must read as zero / finite
@@ -123,24 +128,28 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
         // ------------------------------------------------------------------ MMA issuer
         if (lane == 0) {
             constexpr uint32_t idesc = ptx::idesc_f16(BF16 ? 1 : 0, 128, Cf::N_PAD) | (1u << 15) | (1u << 16);   // A, B MN-major
-            const uint32_t a_addr = ptx::smem_u32(stage), b_addr = a_addr + Dc::OP_BYTES;
+            const uint32_t stage_addr = ptx::smem_u32(stage);
             uint32_t lt = 0;
             int cur_c = -1;
             for (int t = t0; t < t1; ++t, ++lt) {
                 const int c = t / tl.tiles_per_c;
-                ptx::mbar_wait(STAGE_FULL, lt & 1);
-                TRACE(1, lt);
-                ptx::tc_fence_after_sync();
 #pragma unroll
-                for (int mt = 0; mt < Dc::MT; ++mt) {
+                for (int hf = 0; hf < 2; ++hf) {
+                    const uint32_t a_addr = stage_addr + hf * Dc::HALF, b_addr = a_addr + Dc::OP_BYTES;
+                    ptx::mbar_wait(STAGE_FULL + 8 * hf, lt & 1);
+                    if (hf == 0) TRACE(1, lt);
+                    ptx::tc_fence_after_sync();
 #pragma unroll
-                    for (int ks = 0; ks < 8; ++ks) {
-                        const uint64_t ad = ptx::smem_desc_kmajor_noswz(a_addr + mt * 16 * Dc::SBO + ks * 2 * Dc::LBO, Dc::LBO, Dc::SBO);
-                        const uint64_t bd = ptx::smem_desc_kmajor_noswz(b_addr + ks * 2 * Dc::LBO, Dc::LBO, Dc::SBO);
-                        ptx::mma_ss(tmem + mt * 256, ad, bd, idesc, (c != cur_c && ks == 0) ? 0u : 1u);
+                    for (int mt = 0; mt < Dc::MT; ++mt) {
+#pragma unroll
+                        for (int ks = 0; ks < Dc::HW / 16; ++ks) {
+                            const uint64_t ad = ptx::smem_desc_kmajor_noswz(a_addr + mt * 16 * Dc::SBO + ks * 2 * Dc::LBO, Dc::LBO, Dc::SBO);
+                            const uint64_t bd = ptx::smem_desc_kmajor_noswz(b_addr + ks * 2 * Dc::LBO, Dc::LBO, Dc::SBO);
+                            ptx::mma_ss(tmem + mt * 256, ad, bd, idesc, (c != cur_c && hf == 0 && ks == 0) ? 0u : 1u);
+                        }
                     }
+                    ptx::mma_commit(STAGE_EMPTY + 8 * hf);
                 }
-                ptx::mma_commit(STAGE_EMPTY);
                 TRACE(3, lt);
                 cur_c = c;
             }
@@ -153,7 +162,8 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
         const int pl = m / wpf, wl = m - pl * wpf;
         const int wyl = wl / g.nww, wx = wl - wyl * g.nww;
         const int win_off = ((wyl * WS) * g.W + wx * WS) * 2;
-        uint8_t* dst = stage + (o ? 0 : Dc::OP_BYTES) + m * 16;
+        const int hf = m >> 6;                                   // half of the stage this window goes to
+        uint8_t* dst = stage + hf * Dc::HALF + (o ? 0 : Dc::OP_BYTES) + (m & 63) * 16;
         constexpr bool WG = GEN || (WS % 2 == 1);   // word-granular window addressing (GenAddr)
         GenAddr<WG ? WS : 1> ga;
         if constexpr (GEN) gen_addr_init<WS>(ga, g, wyl, wx);
@@ -180,7 +190,7 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
             const int slot = kk % nslot;
             if (part) ptx::mbar_wait(FULL(slot), (kk / nslot) & 1);
             if (ot == 0) TRACE(5, lt);
-            ptx::mbar_wait(STAGE_EMPTY, (lt & 1) ^ 1);      // MMA(lt-1) has read the stage
+            ptx::mbar_wait(STAGE_EMPTY + 8 * hf, (lt & 1) ^ 1);      // the MMAs of tile lt-1 have read this half
             if (ot == 0) TRACE(6, lt);
             const uint8_t* img = ring + (size_t)slot * tl.S;
             {
@@ -202,7 +212,7 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
                     *reinterpret_cast<uint4*>(dst + v * Dc::SBO) = make_uint4(wv[4 * v], wv[4 * v + 1], wv[4 * v + 2], wv[4 * v + 3]);
             }
             ptx::fence_proxy_async_smem();
-            ptx::mbar_arrive(STAGE_FULL);
+            ptx::mbar_arrive(STAGE_FULL + 8 * hf);
             if (part) ptx::mbar_arrive(EMPTY(slot));
             if (ot == 0) TRACE(7, lt);
             k += 2 * np_eff;
@@ -211,6 +221,7 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
             if (seg_end) {
                 // ---- S (TMEM) -> bins -> dT[c]
                 ptx::mbar_wait(STAGE_EMPTY, lt & 1);        // every MMA of this channel segment has completed
+                ptx::mbar_wait(STAGE_EMPTY + 8, lt & 1);
                 if (ot == 0) TRACE(8, lt);
                 ptx::tc_fence_after_sync();
                 for (int b = lane; b < Cf::NB; b += 32) bw[b] = 0.f;
