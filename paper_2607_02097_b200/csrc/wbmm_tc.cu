@@ -415,7 +415,15 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
             if (part) ptx::mbar_wait(FULL(slot), (kk / nslot) & 1);
             if (rt == 0) TRACE(6, lt);
             if constexpr (WG)
-                window_to_tmem_gen<WS>(ring + (size_t)slot * tl.S, ga, valid, GEN && ragged, tmem + buf * A_STRIDE + ((uint32_t)(q * 32) << 16));
+            {
+                const uint32_t ta = tmem + buf * A_STRIDE + ((uint32_t)(q * 32) << 16);
+                if constexpr (GEN && WS % 2 == 0) {      // even w: every window starts on the parity of the column shift
+                    if (g.sw & 1) window_to_tmem_gen<WS, 1>(ring + (size_t)slot * tl.S, ga, valid, ragged, ta);
+                    else window_to_tmem_gen<WS, 0>(ring + (size_t)slot * tl.S, ga, valid, ragged, ta);
+                } else {
+                    window_to_tmem_gen<WS>(ring + (size_t)slot * tl.S, ga, valid, GEN && ragged, ta);
+                }
+            }
             else
                 window_to_tmem_bulk<WS>(ring + (size_t)slot * tl.S + win_off, valid, rowB,
                                         tmem + buf * A_STRIDE + ((uint32_t)(q * 32) << 16));
@@ -468,8 +476,19 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                 if (h == 0) ptx::mbar_wait(OUT_EMPTY + 8 * ob, (use & 1) ^ 1);     // the buffer's previous contents have been read out
                 if (valid) {
                     if constexpr (WG) {
-                        if (GEN && ragged) packed_to_window_gen<WS, Hs::word0(h), Hs::word1(h), true>(img, ga, pk);
-                        else packed_to_window_gen<WS, Hs::word0(h), Hs::word1(h), false>(img, ga, pk);
+                        if constexpr (GEN && WS % 2 == 0) {
+                            if (g.sw & 1) {
+                                if (ragged) packed_to_window_gen<WS, Hs::word0(h), Hs::word1(h), true, 1>(img, ga, pk);
+                                else packed_to_window_gen<WS, Hs::word0(h), Hs::word1(h), false, 1>(img, ga, pk);
+                            } else {
+                                if (ragged) packed_to_window_gen<WS, Hs::word0(h), Hs::word1(h), true, 0>(img, ga, pk);
+                                else packed_to_window_gen<WS, Hs::word0(h), Hs::word1(h), false, 0>(img, ga, pk);
+                            }
+                        } else if (GEN && ragged) {
+                            packed_to_window_gen<WS, Hs::word0(h), Hs::word1(h), true>(img, ga, pk);
+                        } else {
+                            packed_to_window_gen<WS, Hs::word0(h), Hs::word1(h), false>(img, ga, pk);
+                        }
                     } else {
                         packed_to_window<WS, Hs::word0(h), Hs::word1(h)>(img + win_off, rowB, pk);
                     }

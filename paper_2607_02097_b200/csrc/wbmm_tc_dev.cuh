@@ -353,7 +353,9 @@ __device__ __forceinline__ uint32_t pick_halves(uint32_t a, uint32_t b)
 
 // The window's N values, two per word in row-major in-window order, v[0 .. NW).  RAGGED = false:
 // every window element lies inside H x W (no masks).
-template <int WS, bool RAGGED>
+// PAR: parity of the window's first column when it is known to the caller (0 / 1; for even w it is the
+// parity of the column shift, the same for every window), -1 = per thread from a.sh.
+template <int WS, bool RAGGED, int PAR = -1>
 __device__ __forceinline__ void window_to_regs_gen(const uint8_t* img, const GenAddr<WS>& a, bool valid, uint32_t* v)
 {
     constexpr int NWR = GenAddr<WS>::NWR, NF = (WS + 1) / 2;
@@ -370,7 +372,8 @@ __device__ __forceinline__ void window_to_regs_gen(const uint8_t* img, const Gen
         w[NWR] = 0u;
         uint32_t f[NF + 1];                        // aligned element pairs (e_2k, e_2k+1) of this row
 #pragma unroll
-        for (int k = 0; k < NF; ++k) f[k] = __funnelshift_r(w[k], w[k + 1], a.sh);
+        for (int k = 0; k < NF; ++k)
+            f[k] = PAR == 0 ? w[k] : (PAR == 1 ? __funnelshift_r(w[k], w[k + 1], 16) : __funnelshift_r(w[k], w[k + 1], a.sh));
         f[NF] = 0u;
         // row r starts at linear position L = r*WS
         const int L = r * WS;
@@ -423,25 +426,26 @@ __device__ __forceinline__ void window_to_tmem_bulk(const uint8_t* win, bool val
     packed_window_to_tmem<WS>(v, taddr);
 }
 
-template <int WS>
+template <int WS, int PAR = -1>
 __device__ __forceinline__ void window_to_tmem_gen(const uint8_t* img, const GenAddr<WS>& a, bool valid, bool ragged,
                                                    uint32_t taddr)
 {
     uint32_t v[WinCfg<WS>::NW];
-    if (ragged) window_to_regs_gen<WS, true>(img, a, valid, v);
-    else window_to_regs_gen<WS, false>(img, a, valid, v);
+    if (ragged) window_to_regs_gen<WS, true, PAR>(img, a, valid, v);
+    else window_to_regs_gen<WS, false, PAR>(img, a, valid, v);
     packed_window_to_tmem<WS>(v, taddr);
 }
 
 // Packed words [W0, W1) of a window (pk[0] = word W0; the range covers whole window rows, or the
 // whole window) -> the window's place in the natural-layout frame.
-template <int WS, int W0, int W1, bool RAGGED>
+template <int WS, int W0, int W1, bool RAGGED, int PAR = -1>
 __device__ __forceinline__ void packed_to_window_gen(uint8_t* img, const GenAddr<WS>& a, const uint32_t* pk)
 {
     constexpr int NWR = GenAddr<WS>::NWR, NF = (WS + 1) / 2;
     constexpr int R0 = (2 * W0) / WS, R1 = (2 * W1 + WS - 1) / WS < WS ? (2 * W1 + WS - 1) / WS : WS;
     static_assert((2 * W0) % WS == 0, "the range starts on a window row");
-    const int odd = a.sh >> 4;
+    const int odd = PAR < 0 ? (int)(a.sh >> 4) : PAR;
+    const uint32_t sh = PAR < 0 ? a.sh : (uint32_t)PAR * 16u;
 #pragma unroll
     for (int r = R0; r < R1; ++r) {
         // aligned element pairs of the row from the linear packed words
@@ -462,7 +466,7 @@ __device__ __forceinline__ void packed_to_window_gen(uint8_t* img, const GenAddr
 #pragma unroll
         for (int k = 0; k < NWR; ++k) {
             // image word k holds window elements ea = 2k - odd (low half) and ea + 1 (high half)
-            const uint32_t val = __funnelshift_l(f[k], k + 1 <= NF ? f[k + 1] : 0u, a.sh);
+            const uint32_t val = PAR == 0 ? f[k + 1] : __funnelshift_l(f[k], f[k + 1], sh);
             const int ea = 2 * k - odd;
             const bool ok = rv && (!RAGGED || ((a.colmask >> k) & 1u));
             uint8_t* q = p + a.coloff[k];
