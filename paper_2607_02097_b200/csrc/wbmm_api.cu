@@ -300,6 +300,32 @@ std::mutex g_host_mutex;
 Scratch g_sx, g_sT, g_sy, g_sdy, g_sdT;
 cudaStream_t g_host_stream = nullptr;
 
+constexpr int kHostChunks = 8;
+cudaStream_t g_s_kernel = nullptr, g_s_out = nullptr;
+cudaEvent_t g_ev_in[kHostChunks] = {}, g_ev_k[kHostChunks] = {};
+
+cudaError_t host_pipeline_init()
+{
+    if (g_s_kernel) return cudaSuccess;
+    cudaError_t e = cudaStreamCreateWithFlags(&g_s_kernel, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&g_s_out, cudaStreamNonBlocking);
+    for (int i = 0; i < kHostChunks && e == cudaSuccess; ++i) {
+        e = cudaEventCreateWithFlags(&g_ev_in[i], cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&g_ev_k[i], cudaEventDisableTiming);
+    }
+    return e;
+}
+
+void host_pipeline_release()
+{
+    if (g_s_kernel) { cudaStreamDestroy(g_s_kernel); g_s_kernel = nullptr; }
+    if (g_s_out) { cudaStreamDestroy(g_s_out); g_s_out = nullptr; }
+    for (int i = 0; i < kHostChunks; ++i) {
+        if (g_ev_in[i]) { cudaEventDestroy(g_ev_in[i]); g_ev_in[i] = nullptr; }
+        if (g_ev_k[i]) { cudaEventDestroy(g_ev_k[i]); g_ev_k[i] = nullptr; }
+    }
+}
+
 cudaError_t host_stream(cudaStream_t* s)
 {
     if (!g_host_stream) {
@@ -336,11 +362,30 @@ int wbmm_forward_host(const wbmm_desc_t* desc, const void* x_host, const void* T
     WBMM_TRY(g_sx.reserve(nact), "cudaMalloc x");
     WBMM_TRY(g_sy.reserve(nact), "cudaMalloc y");
     WBMM_TRY(g_sT.reserve(ntab), "cudaMalloc T");
-    WBMM_TRY(cudaMemcpyAsync(g_sx.p, x_host, nact, cudaMemcpyHostToDevice, s), "H2D x");
+    // The batch is cut into chunks that flow through three streams -- H2D, kernels, D2H -- so that the
+    // upload of chunk i+1, the kernels of chunk i and the download of chunk i-1 overlap (PCIe is full
+    // duplex; with pinned host buffers the call takes about max(H2D, D2H) instead of their sum).
+    WBMM_TRY(host_pipeline_init(), "streams");
+    const int nchunk = nact >= (8u << 20) ? (g.B < kHostChunks ? g.B : kHostChunks) : 1;
+    const size_t per_image = nact / (size_t)g.B;
     WBMM_TRY(cudaMemcpyAsync(g_sT.p, T_host, ntab, cudaMemcpyHostToDevice, s), "H2D T");
-    st = apply(desc, g, g_sx.p, g_sT.p, g_sy.p, false, s);
-    if (st != WBMM_STATUS_OK) return st;
-    WBMM_TRY(cudaMemcpyAsync(y_host, g_sy.p, nact, cudaMemcpyDeviceToHost, s), "D2H y");
+    for (int i = 0; i < nchunk; ++i) {
+        const int b0 = (int)((long long)g.B * i / nchunk), b1 = (int)((long long)g.B * (i + 1) / nchunk);
+        if (b1 == b0) continue;
+        const size_t off = per_image * b0, len = per_image * (b1 - b0);
+        WBMM_TRY(cudaMemcpyAsync((char*)g_sx.p + off, (const char*)x_host + off, len, cudaMemcpyHostToDevice, s), "H2D x");
+        WBMM_TRY(cudaEventRecord(g_ev_in[i], s), "event");
+        WBMM_TRY(cudaStreamWaitEvent(g_s_kernel, g_ev_in[i], 0), "wait");
+        wbmm_desc_t dc = *desc;
+        dc.B = b1 - b0;
+        wbmm::Geom gc = wbmm::make_geom(dc);
+        st = apply(&dc, gc, (char*)g_sx.p + off, g_sT.p, (char*)g_sy.p + off, false, g_s_kernel);
+        if (st != WBMM_STATUS_OK) return st;
+        WBMM_TRY(cudaEventRecord(g_ev_k[i], g_s_kernel), "event");
+        WBMM_TRY(cudaStreamWaitEvent(g_s_out, g_ev_k[i], 0), "wait");
+        WBMM_TRY(cudaMemcpyAsync((char*)y_host + off, (char*)g_sy.p + off, len, cudaMemcpyDeviceToHost, g_s_out), "D2H y");
+    }
+    WBMM_TRY(cudaStreamSynchronize(g_s_out), "sync");
     WBMM_TRY(cudaStreamSynchronize(s), "sync");
     return WBMM_STATUS_OK;
 }
@@ -391,6 +436,7 @@ void wbmm_release(void)
     std::lock_guard<std::mutex> lock(g_host_mutex);
     g_sx.release(); g_sT.release(); g_sy.release(); g_sdy.release(); g_sdT.release();
     if (g_host_stream) { cudaStreamDestroy(g_host_stream); g_host_stream = nullptr; }
+    host_pipeline_release();
     wbmm::tc_release();
 }
 
