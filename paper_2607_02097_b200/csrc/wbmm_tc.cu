@@ -12,6 +12,10 @@
 //     l.17) are pure address arithmetic.
 #include "wbmm_tc.cuh"
 
+#include <cuda.h>
+
+#include <cstring>
+
 #include <cstdlib>
 #include <mutex>
 #include <type_traits>
@@ -161,13 +165,14 @@ struct BulkSmem {
     static constexpr int TAB_ONE = ((Cf::NB + 2) * 2 + 15) / 16 * 16;
     static constexpr int TAB_BYTES = 2 * TAB_ONE;                              // F0 and F1 (or Ts for the generic builder)
     static constexpr int BAR_BYTES = (2 * kMaxSlots + 8 + 2 * kMaxOutBufs) * 8;
-    static constexpr int FIXED = BulkCfg<WS>::WC_BYTES + BulkCfg<WS>::HIER_BYTES + TAB_BYTES + BAR_BYTES;
+    static constexpr int FIXED = (BulkCfg<WS>::WC_BYTES + BulkCfg<WS>::HIER_BYTES + TAB_BYTES + BAR_BYTES + 127) / 128 * 128;   // tensor-map boxes land 128-byte aligned
 };
 
 template <int WS, bool BF16, bool GEN>
 __global__ void __launch_bounds__(kThreadsB, 1)
 tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const uint16_t* __restrict__ x, const uint16_t* __restrict__ T,
-               const uint16_t* __restrict__ Tl, uint16_t* __restrict__ y, int reverse)
+               const uint16_t* __restrict__ Tl, uint16_t* __restrict__ y, int reverse, int box, int sbox,
+               const __grid_constant__ CUtensorMap mx, const __grid_constant__ CUtensorMap my)
 {
     using Cf = WinCfg<WS>;
     using Sm = BulkSmem<WS>;
@@ -203,7 +208,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
     if (warp == 1) { ptx::tmem_alloc(ptx::smem_u32(&tmem_base_s), 512); if (lane == 0) TRACE(1, 15); }
     if (tid >= 64 && tid < 64 + nslot) {
         ptx::mbar_init(FULL(tid - 64), 1);
-        ptx::mbar_init(EMPTY(tid - 64), wpf);
+        ptx::mbar_init(EMPTY(tid - 64), box ? box * wpf : wpf);   // box mode: one barrier pair per group of `box` images
         ptx::fence_mbar_init();
     }
     if (tid == 0) {
@@ -281,6 +286,17 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
             int c, b0, wy0, np_eff, rows_eff;
             tile_decode(t, c, b0, wy0, np_eff, rows_eff);
             const uint32_t bytes = (uint32_t)rows_eff * rowB;
+            if (box) {
+                // small images: ONE tensor-map box {a, b, 1 channel, box images} per group instead of `box` copies
+                for (int p = lane * box; p < np_eff; p += 32 * box) {
+                    const uint32_t kk = k + p;
+                    const int slot = kk % nslot;            // first slot of the group (nslot, k, p are multiples of box)
+                    ptx::mbar_wait(EMPTY(slot), ((kk / nslot) & 1) ^ 1);
+                    ptx::mbar_arrive_expect_tx(FULL(slot), bytes * box);
+                    if (p == 0) TRACE(0, (t - t0));
+                    ptx::tma_load_4d(ptx::smem_u32(ring + (size_t)slot * tl.S), &mx, 0, 0, c, b0 + p, FULL(slot));
+                }
+            } else
             for (int p = lane; p < np_eff; p += 32) {
                 const uint32_t kk = k + p;
                 const int slot = kk % nslot;
@@ -412,7 +428,8 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
             const int slot = kk % nslot;
             if (lt == 0) rebuild_weight(c, lt);   // first tile: build while its loads are in flight
             if (rt == 0) TRACE(5, lt);
-            if (part) ptx::mbar_wait(FULL(slot), (kk / nslot) & 1);
+            const int bslot = box ? slot - slot % box : slot;      // the barrier pair that covers this image
+            if (part) ptx::mbar_wait(FULL(bslot), (kk / nslot) & 1);
             if (rt == 0) TRACE(6, lt);
             if constexpr (WG)
             {
@@ -427,7 +444,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
             else
                 window_to_tmem_bulk<WS>(ring + (size_t)slot * tl.S + win_off, valid, rowB,
                                         tmem + buf * A_STRIDE + ((uint32_t)(q * 32) << 16));
-            if (part) ptx::mbar_arrive(EMPTY(slot));   // every window of this image is in TMEM
+            if (part) ptx::mbar_arrive(EMPTY(bslot));   // every window of this image is in TMEM
             // W_c of a new channel is rebuilt AFTER this tile's windows are in TMEM, so the copy above
             // overlaps the last MMA of the previous channel.
             if (lt > 0) rebuild_weight(c, lt);
@@ -527,6 +544,9 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                 ptx::mbar_wait(OUT_FULL + 8 * lane, (lt / depth) & 1);
                 if (lane == 0) TRACE(10, lt);
                 const int p_first = gq * og.images, p_end = min(p_first + og.images, np_eff);
+                if (sbox) {
+                    if (p_first < p_end) ptx::tma_store_4d(&my, 0, 0, c, b0 + p_first, ptx::smem_u32(outb + (size_t)lane * out_bytes));
+                } else
                 for (int p = p_first; p < p_end; ++p) {
                     uint16_t* dst = y + ((long long)(b0 + p) * g.C + c) * plane_elems + (long long)wy0 * WS * g.W;
                     ptx::bulk_s2g(dst, ptx::smem_u32(outb + (size_t)lane * out_bytes + (size_t)(p - p_first) * tl.S), bytes);
@@ -593,14 +613,87 @@ int bulk_mode(const Geom& g, const TcTiles& tl, const void* x, const void* y)
     return (tl.nstrips == 1 && g.W % 2 == 0 && g.Wp % 2 == 0) ? 2 : 0;
 }
 
+// cuTensorMapEncodeTiled through the runtime's driver entry point (libcuda is not linked).
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn bulk_encode_fn()
+{
+    static EncodeTiledFn fn = nullptr;
+    static std::once_flag once;
+    std::call_once(once, [] {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiledFn>(p);
+        else
+            cudaGetLastError();
+    });
+    return fn;
+}
+
+// Small frame images (28 x 28: 1568 bytes) make one bulk copy per image the bottleneck: 64 copy-engine
+// operations per tile.  When whole images are tiled (nstrips == 1) the images of one output group are
+// moved by ONE tensor-map box instead: the activation is viewed as (a, b, C, B) with a*b = H*W, a a
+// multiple of 8 elements and both <= 256, box {a, b, 1, group}.  Returns the group size (0 = not applicable).
+int bulk_box_mode(const Geom& g, const TcTiles& tl, int dtype, const void* x, const void* y, int* S, int* sbox,
+                  CUtensorMap* mx, CUtensorMap* my)
+{
+    *sbox = 0;
+    if (tl.nstrips != 1) return 0;
+    const long long hw = (long long)g.H * g.W, ib = hw * 2;
+    if (ib > 4096) return 0;
+    // load box: the largest group of images (a divisor of the tile and of the batch, at most 8: the repack
+    // warps start on a group as soon as it has landed) whose bytes are a multiple of 128
+    int LB = 0;
+    for (int cand = 8; cand >= 2; cand >>= 1)
+        if (tl.NP % cand == 0 && g.B % cand == 0 && (cand * ib) % 128 == 0) { LB = cand; break; }
+    if (LB == 0) return 0;
+    int a = 0;
+    for (int cand = 256; cand >= 8; cand -= 8)
+        if (hw % cand == 0 && hw / cand <= 256) { a = cand; break; }
+    EncodeTiledFn fn = bulk_encode_fn();
+    if (a == 0 || !fn) return 0;
+    // store box: one output group, when that is a legal box too
+    const int G = out_groups(tl, tl.NSY * g.nww).images;
+    const bool sb = G >= 2 && g.B % G == 0 && tl.NP % G == 0 && (G * ib) % 128 == 0;
+    const cuuint64_t dims[4] = {(cuuint64_t)a, (cuuint64_t)(hw / a), (cuuint64_t)g.C, (cuuint64_t)g.B};
+    const cuuint64_t strides[3] = {(cuuint64_t)a * 2, (cuuint64_t)ib, (cuuint64_t)ib * g.C};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    const CUtensorMapDataType dt = dtype == WBMM_DTYPE_BF16 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT16;
+    for (int i = 0; i < (sb ? 2 : 1); ++i) {
+        const cuuint32_t boxd[4] = {(cuuint32_t)a, (cuuint32_t)(hw / a), 1, (cuuint32_t)(i ? G : LB)};
+        const CUresult r = fn(i ? my : mx, dt, 4, const_cast<void*>(i ? y : x), dims, strides, boxd, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return 0;
+    }
+    *S = (int)ib;      // boxes land densely: the slot stride is exactly one image
+    *sbox = sb ? 1 : 0;
+    return LB;
+}
+
 template <int WS, bool BF16, bool GEN>
-cudaError_t launch_bulk(const Geom& g, const TcTiles& tl, const void* x, const void* T, const void* Tl, void* y,
+cudaError_t launch_bulk(const Geom& g, const TcTiles& tl_in, const void* x, const void* T, const void* Tl, void* y,
                         bool reverse, cudaStream_t s)
 {
     auto k = tc_bulk_kernel<WS, BF16, GEN>;
     int nslot = 0, nout = 0;
+    TcTiles tl = tl_in;
+    CUtensorMap mx, my;
+    memset(&mx, 0, sizeof(mx));
+    memset(&my, 0, sizeof(my));
+    int sbox = 0;
+    int box = bulk_box_mode(g, tl_in, BF16 ? WBMM_DTYPE_BF16 : WBMM_DTYPE_F16, x, y, &tl.S, &sbox, &mx, &my);
     const int wpf = tl.NSY * g.nww;
-    if (!bulk_slots<WS>(tl, wpf, &nslot, &nout)) return cudaErrorInvalidConfiguration;
+    if (box) {
+        if (bulk_slots<WS>(tl, wpf, &nslot, &nout)) nslot -= nslot % box;      // groups never wrap around the ring
+        if (nslot < tl.NP + box) {                                            // (does not fit: one copy per image)
+            box = sbox = 0;
+            tl = tl_in;
+        }
+    }
+    if (!box && !bulk_slots<WS>(tl, wpf, &nslot, &nout)) return cudaErrorInvalidConfiguration;
     const size_t smem = (size_t)BulkSmem<WS>::FIXED + (size_t)(nslot + nout * out_groups(tl, wpf).images) * tl.S;
     static SmemOptIn smem_state = {0, 0};
     cudaError_t e = ensure_dynamic_smem(reinterpret_cast<const void*>(k), smem, &smem_state);
@@ -633,8 +726,7 @@ cudaError_t launch_bulk(const Geom& g, const TcTiles& tl, const void* x, const v
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     return cudaLaunchKernelEx(&cfg, k, g, tl, part, nslot, nout, (const uint16_t*)x, (const uint16_t*)T, (const uint16_t*)Tl,
-                              (uint16_t*)y,
-                              reverse ? 1 : 0);
+                              (uint16_t*)y, reverse ? 1 : 0, box, sbox, mx, my);
 }
 
 template <int WS>
