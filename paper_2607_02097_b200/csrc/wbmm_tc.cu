@@ -637,6 +637,30 @@ EncodeTiledFn bulk_encode_fn()
 // operations per tile.  When whole images are tiled (nstrips == 1) the images of one output group are
 // moved by ONE tensor-map box instead: the activation is viewed as (a, b, C, B) with a*b = H*W, a a
 // multiple of 8 elements and both <= 256, box {a, b, 1, group}.  Returns the group size (0 = not applicable).
+}  // namespace
+
+// Tensor map over an NCHW activation viewed as (a, b, C, B), a*b = H*W, with box {a, b, 1, images}: `images`
+// whole frame images of one channel per copy.  False when H*W has no legal factorisation or the driver
+// entry point is missing.  `map` is a CUtensorMap.
+bool image_box_map(const Geom& g, int dtype, const void* base, int images, void* map)
+{
+    const long long hw = (long long)g.H * g.W, ib = hw * 2;
+    int a = 0;
+    for (int cand = 256; cand >= 8; cand -= 8)
+        if (hw % cand == 0 && hw / cand <= 256) { a = cand; break; }
+    EncodeTiledFn fn = bulk_encode_fn();
+    if (a == 0 || !fn || images < 1 || images > 256) return false;
+    const cuuint64_t dims[4] = {(cuuint64_t)a, (cuuint64_t)(hw / a), (cuuint64_t)g.C, (cuuint64_t)g.B};
+    const cuuint64_t strides[3] = {(cuuint64_t)a * 2, (cuuint64_t)ib, (cuuint64_t)ib * g.C};
+    const cuuint32_t boxd[4] = {(cuuint32_t)a, (cuuint32_t)(hw / a), 1, (cuuint32_t)images};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    const CUtensorMapDataType dt = dtype == WBMM_DTYPE_BF16 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT16;
+    return fn(static_cast<CUtensorMap*>(map), dt, 4, const_cast<void*>(base), dims, strides, boxd, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+namespace {
+
 int bulk_box_mode(const Geom& g, const TcTiles& tl, int dtype, const void* x, const void* y, int* S, int* sbox,
                   CUtensorMap* mx, CUtensorMap* my)
 {
@@ -650,24 +674,11 @@ int bulk_box_mode(const Geom& g, const TcTiles& tl, int dtype, const void* x, co
     for (int cand = 8; cand >= 2; cand >>= 1)
         if (tl.NP % cand == 0 && g.B % cand == 0 && (cand * ib) % 128 == 0) { LB = cand; break; }
     if (LB == 0) return 0;
-    int a = 0;
-    for (int cand = 256; cand >= 8; cand -= 8)
-        if (hw % cand == 0 && hw / cand <= 256) { a = cand; break; }
-    EncodeTiledFn fn = bulk_encode_fn();
-    if (a == 0 || !fn) return 0;
     // store box: one output group, when that is a legal box too
     const int G = out_groups(tl, tl.NSY * g.nww).images;
     const bool sb = G >= 2 && g.B % G == 0 && tl.NP % G == 0 && (G * ib) % 128 == 0;
-    const cuuint64_t dims[4] = {(cuuint64_t)a, (cuuint64_t)(hw / a), (cuuint64_t)g.C, (cuuint64_t)g.B};
-    const cuuint64_t strides[3] = {(cuuint64_t)a * 2, (cuuint64_t)ib, (cuuint64_t)ib * g.C};
-    const cuuint32_t estr[4] = {1, 1, 1, 1};
-    const CUtensorMapDataType dt = dtype == WBMM_DTYPE_BF16 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT16;
-    for (int i = 0; i < (sb ? 2 : 1); ++i) {
-        const cuuint32_t boxd[4] = {(cuuint32_t)a, (cuuint32_t)(hw / a), 1, (cuuint32_t)(i ? G : LB)};
-        const CUresult r = fn(i ? my : mx, dt, 4, const_cast<void*>(i ? y : x), dims, strides, boxd, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-        if (r != CUDA_SUCCESS) return 0;
-    }
+    if (!image_box_map(g, dtype, x, LB, mx)) return 0;
+    if (sb && !image_box_map(g, dtype, y, G, my)) return 0;
     *S = (int)ib;      // boxes land densely: the slot stride is exactly one image
     *sbox = sb ? 1 : 0;
     return LB;

@@ -40,6 +40,10 @@ bool tc_grad_table_supported(const Geom& g, int dtype, const void* x, const void
 cudaError_t tc_grad_table(const Geom& g, int dtype, const void* x, const void* dy, float* dT,
                           cudaStream_t stream, int* launches, int* path);
 
+// Tensor map (CUtensorMap behind the void*) over an NCHW activation with box = `images` whole frame images of
+// one channel (wbmm_tc.cu).
+bool image_box_map(const Geom& g, int dtype, const void* base, int images, void* map);
+
 void tc_release();
 
 }  // namespace wbmm

@@ -16,6 +16,9 @@
 //   warps 2-5   x  -> B operand stage;  warps 6-9   dy -> A operand stage;  all eight: the bin epilogue
 #include "wbmm_tc_dev.cuh"
 
+#include <cuda.h>
+
+#include <cstring>
 #include <mutex>
 
 namespace wbmm {
@@ -40,7 +43,7 @@ struct DtCfg {
     static constexpr int HALF = 2 * OP_BYTES;          // A region then B region; an M-tile's 16 vectors may run into B
     static constexpr int STAGE = 2 * HALF;
     static constexpr int BAR_BYTES = (2 * kMaxSlots + 8) * 8;   // slots + STAGE_FULL[2] + STAGE_EMPTY[2]
-    static constexpr int FIXED = STAGE + BAR_BYTES;
+    static constexpr int FIXED = (STAGE + BAR_BYTES + 127) / 128 * 128;   // tensor-map boxes land 128-byte aligned
     static_assert(MT * 16 <= 2 * NVEC, "an A M-tile must stay inside the stage");
     static_assert(8 * Cf::NB * 4 <= STAGE, "per-warp bin copies alias the stage");
 };
@@ -48,7 +51,8 @@ struct DtCfg {
 template <int WS, bool BF16, bool GEN>
 __global__ void __launch_bounds__(kThreadsD, 1)
 tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __restrict__ x,
-             const uint16_t* __restrict__ dy, float* __restrict__ dT)
+             const uint16_t* __restrict__ dy, float* __restrict__ dT, int box,
+             const __grid_constant__ CUtensorMap mx, const __grid_constant__ CUtensorMap mg)
 {
     using Cf = WinCfg<WS>;
     using Dc = DtCfg<WS>;
@@ -68,7 +72,7 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
     if (warp == 1) ptx::tmem_alloc(ptx::smem_u32(&tmem_base_s), 512);
     if (tid >= 64 && tid < 64 + nslot) {
         ptx::mbar_init(FULL(tid - 64), 1);
-        ptx::mbar_init(EMPTY(tid - 64), wpf);
+        ptx::mbar_init(EMPTY(tid - 64), box ? box * wpf : wpf);   // box mode: one barrier pair per group of `box` images
         ptx::fence_mbar_init();
     }
     if (tid == 0) {
@@ -111,6 +115,17 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
             int c, b0, wy0, np_eff, rows_eff;
             tile_decode(t, c, b0, wy0, np_eff, rows_eff);
             const uint32_t bytes = (uint32_t)rows_eff * rowB;
+            if (box) {
+                // small images: one tensor-map box per group of `box` images and operand; ring order per tile:
+                // x group 0, dy group 0, x group 1, dy group 1, ...
+                for (int j = lane; j < 2 * np_eff / box; j += 32) {
+                    const uint32_t kk = k + j * box;
+                    const int slot = kk % nslot;
+                    ptx::mbar_wait(EMPTY(slot), ((kk / nslot) & 1) ^ 1);
+                    ptx::mbar_arrive_expect_tx(FULL(slot), bytes * box);
+                    ptx::tma_load_4d(ptx::smem_u32(ring + (size_t)slot * tl.S), (j & 1) ? &mg : &mx, 0, 0, c, b0 + (j >> 1) * box, FULL(slot));
+                }
+            } else
             for (int j = lane; j < 2 * np_eff; j += 32) {
                 const uint32_t kk = k + j;
                 const int slot = kk % nslot;
@@ -186,9 +201,10 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
             if (ot == 0) TRACE(4, lt);
             const bool part = pl < tl.NP && pl < np_eff;
             const bool valid = part && wy0 + wyl < g.nwh;
-            const uint32_t kk = k + 2 * pl + o;
+            const uint32_t kk = box ? k + 2 * box * (pl / box) + box * o + pl % box : k + 2 * pl + o;
             const int slot = kk % nslot;
-            if (part) ptx::mbar_wait(FULL(slot), (kk / nslot) & 1);
+            const int bslot = box ? slot - slot % box : slot;      // the barrier pair that covers this image
+            if (part) ptx::mbar_wait(FULL(bslot), (kk / nslot) & 1);
             if (ot == 0) TRACE(5, lt);
             ptx::mbar_wait(STAGE_EMPTY + 8 * hf, (lt & 1) ^ 1);      // the MMAs of tile lt-1 have read this half
             if (ot == 0) TRACE(6, lt);
@@ -213,7 +229,7 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
             }
             ptx::fence_proxy_async_smem();
             ptx::mbar_arrive(STAGE_FULL + 8 * hf);
-            if (part) ptx::mbar_arrive(EMPTY(slot));
+            if (part) ptx::mbar_arrive(EMPTY(bslot));
             if (ot == 0) TRACE(7, lt);
             k += 2 * np_eff;
 
@@ -306,10 +322,33 @@ int dt_mode(const Geom& g, const TcTiles& tl, const void* x, const void* dy)
 }
 
 template <int WS, bool BF16, bool GEN>
-cudaError_t launch_dt(const Geom& g, const TcTiles& tl, const void* x, const void* dy, float* dT, cudaStream_t s)
+cudaError_t launch_dt(const Geom& g, const TcTiles& tl_in, const void* x, const void* dy, float* dT, cudaStream_t s)
 {
     auto k = tc_dt_kernel<WS, BF16, GEN>;
-    const int nslot = dt_slots<WS>(tl);
+    TcTiles tl = tl_in;
+    CUtensorMap mx, mg;
+    memset(&mx, 0, sizeof(mx));
+    memset(&mg, 0, sizeof(mg));
+    // small frame images: tensor-map boxes of 8 images per copy (see bulk_box_mode in wbmm_tc.cu)
+    int box = 0;
+    {
+        const long long ib = (long long)g.H * g.W * 2;
+        const int dtype = BF16 ? WBMM_DTYPE_BF16 : WBMM_DTYPE_F16;
+        if (tl.nstrips == 1 && ib <= 4096 && tl.NP % 8 == 0 && g.B % 8 == 0 && (8 * ib) % 128 == 0 &&
+            image_box_map(g, dtype, x, 8, &mx) && image_box_map(g, dtype, dy, 8, &mg)) {
+            box = 8;
+            tl.S = (int)ib;
+        }
+    }
+    int nslot = dt_slots<WS>(tl);
+    if (box) {
+        nslot -= nslot % (2 * box);
+        if (nslot < 2 * tl.NP) {
+            box = 0;
+            tl = tl_in;
+            nslot = dt_slots<WS>(tl);
+        }
+    }
     const size_t smem = (size_t)DtCfg<WS>::FIXED + (size_t)nslot * tl.S;
     static SmemOptIn smem_state = {0, 0};
     cudaError_t e = ensure_dynamic_smem(reinterpret_cast<const void*>(k), smem, &smem_state);
@@ -340,7 +379,7 @@ cudaError_t launch_dt(const Geom& g, const TcTiles& tl, const void* x, const voi
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, k, g, tl, part, nslot, (const uint16_t*)x, (const uint16_t*)dy, dT);
+    return cudaLaunchKernelEx(&cfg, k, g, tl, part, nslot, (const uint16_t*)x, (const uint16_t*)dy, dT, box, mx, mg);
 }
 
 }  // namespace
