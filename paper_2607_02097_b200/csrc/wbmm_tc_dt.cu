@@ -44,8 +44,13 @@ struct DtCfg {
     static constexpr int STAGE = 2 * HALF;
     static constexpr int BAR_BYTES = (2 * kMaxSlots + 8) * 8;   // slots + STAGE_FULL[2] + STAGE_EMPTY[2]
     static constexpr int FIXED = (STAGE + BAR_BYTES + 127) / 128 * 128;   // tensor-map boxes land 128-byte aligned
+    // Bin fold: a warp's private bins have row pitch BP = WS (mod 32), so the 32 consecutive rows of S a warp
+    // updates in one step (bin = ri*BP + ci + const) fall into 32 different banks.
+    static constexpr int BP = ((Cf::TW - WS + 31) / 32) * 32 + WS;
+    static constexpr int BN = Cf::TW * BP;             // floats per private copy
+    static_assert(BP >= Cf::TW && BP % 32 == WS % 32, "bin pitch");
     static_assert(MT * 16 <= 2 * NVEC, "an A M-tile must stay inside the stage");
-    static_assert(8 * Cf::NB * 4 <= STAGE, "per-warp bin copies alias the stage");
+    static_assert(8 * BN * 4 <= STAGE, "per-warp bin copies alias the stage");
 };
 
 template <int WS, bool BF16, bool GEN>
@@ -184,7 +189,7 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
         if constexpr (GEN) gen_addr_init<WS>(ga, g, wyl, wx);
         else if constexpr (WG) gen_addr_init_plain<WS>(ga, g.W, wyl, wx);
         float* bins = reinterpret_cast<float*>(stage);
-        float* bw = bins + (ot >> 5) * Cf::NB;          // this warp's private copy of the bins
+        float* bw = bins + (ot >> 5) * Dc::BN;          // this warp's private copy of the bins
         const int ew = ot >> 5;                          // 0..7
         const int emt = ew >> 2, eq = warp & 3;          // M-tile and TMEM lane quarter in the epilogue
         const int erow = emt * 128 + eq * 32 + lane;     // row of S = output position i
@@ -240,7 +245,7 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
                 ptx::mbar_wait(STAGE_EMPTY + 8, lt & 1);
                 if (ot == 0) TRACE(8, lt);
                 ptx::tc_fence_after_sync();
-                for (int b = lane; b < Cf::NB; b += 32) bw[b] = 0.f;
+                for (int b = lane; b < Dc::BN; b += 32) bw[b] = 0.f;
                 __syncwarp();
                 if (emt < Dc::MT) {
                     // Row i = erow of S goes to bins base - rj*TW - cj.  For a fixed column j the 32 rows of
@@ -248,7 +253,7 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
                     // rows of S apart in bin space, so their updates are independent too: NU read-add-write
                     // chains are in flight per step instead of one.
                     const uint32_t taddr = tmem + emt * 256 + ((uint32_t)(eq * 32) << 16);
-                    float* bbase = bw + (eri + WS - 1) * Cf::TW + eci + WS - 1;
+                    float* bbase = bw + (eri + WS - 1) * Dc::BP + eci + WS - 1;
                     const bool rowok = erow < Cf::N;
                     constexpr int RJ_STRIDE = 31 / WS + 1, NU = (WS + RJ_STRIDE - 1) / RJ_STRIDE;
 #pragma unroll
@@ -259,31 +264,37 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
                         for (int u = 0; u < NU; ++u)
                             if (g0 + u * RJ_STRIDE < WS) ptx::tmem_ld_n<WS>(taddr + (g0 + u * RJ_STRIDE) * WS, v[u]);
                         ptx::tmem_wait_ld();
+                        if (ot == 0 && g0 == 0) TRACE(13, lt);
 #pragma unroll
                         for (int cj = 0; cj < WS; ++cj) {
                             float old[NU];
 #pragma unroll
                             for (int u = 0; u < NU; ++u)
-                                if (g0 + u * RJ_STRIDE < WS && rowok) old[u] = bbase[-(g0 + u * RJ_STRIDE) * Cf::TW - cj];
+                                if (g0 + u * RJ_STRIDE < WS && rowok) old[u] = bbase[-(g0 + u * RJ_STRIDE) * Dc::BP - cj];
 #pragma unroll
                             for (int u = 0; u < NU; ++u)
                                 if (g0 + u * RJ_STRIDE < WS && rowok)
-                                    bbase[-(g0 + u * RJ_STRIDE) * Cf::TW - cj] = old[u] + __uint_as_float(v[u][cj]);
+                                    bbase[-(g0 + u * RJ_STRIDE) * Dc::BP - cj] = old[u] + __uint_as_float(v[u][cj]);
                             __syncwarp();
                         }
+                        if (ot == 0 && g0 == 0) TRACE(14, lt);
                     }
                 }
+                if (ot == 0) TRACE(10, lt);
                 ptx::tc_fence_before_sync();
                 ptx::named_bar_sync(1, 256);
+                if (ot == 0) TRACE(11, lt);
                 for (int b = ot; b < Cf::NB; b += 256) {
                     float sacc = 0.f;
+                    const int bp = (b / Cf::TW) * Dc::BP + b % Cf::TW;
 #pragma unroll
-                    for (int w8 = 0; w8 < 8; ++w8) sacc += bins[w8 * Cf::NB + b];
+                    for (int w8 = 0; w8 < 8; ++w8) sacc += bins[w8 * Dc::BN + bp];
                     atomicAdd(dT + (long long)c * Cf::NB + b, sacc);
                 }
                 ptx::named_bar_sync(1, 256);
+                if (ot == 0) TRACE(12, lt);
                 // the bins aliased the operand stage: restore the zero padding vectors
-                for (int i = ot; i < 8 * Cf::NB * 4 / 16 + 1; i += 256)
+                for (int i = ot; i < 8 * Dc::BN * 4 / 16 + 1; i += 256)
                     if (i * 16 < Dc::STAGE) reinterpret_cast<uint4*>(stage)[i] = make_uint4(0, 0, 0, 0);
                 ptx::fence_proxy_async_smem();
                 ptx::named_bar_sync(1, 256);
