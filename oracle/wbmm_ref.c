@@ -15,6 +15,8 @@
  *   - zero padding to a multiple of w, crop     PAPER.md:176-182  (Eq. 4-5)
  *   - window partition / bmm / inverse reshape  PAPER.md:157-173  (Alg. 1)
  *   - backward "gradients flow through R"
+ *   - hierarchical reparameterisation, training and fused forms, and the
+ *     gradients of its two tables              PAPER.md:216-227 (Eq. 9), 840-893 (Alg. 2-3)
  * Readings:
  *   A1 orientation y = W_c . x with W_c[i,j] = T[c, rel(i,j)], i = OUTPUT
  *      position, j = INPUT position (BASELINE.json north_star); the paper's
@@ -400,6 +402,59 @@ int wbmm_ref_hier_forward_fused(int B, int C, int H, int W, int w, int sh, int s
                     }
         }
         free(M); free(Ml); free(xw);
+    }
+    return 0;
+}
+
+/*
+ * Backward of the hierarchical operator with respect to its two tables (the gradient of Algorithm 2,
+ * PAPER.md:840-860, taken term by term; the identity shortcuts carry no parameter).  With
+ * y_w = Mg x_w + sum_sub Ml x_sub + 2 x_w  and  Mg[i,j] = Tg[rel_w(i,j)], Ml[il,jl] = Tl[rel_{w/2}(il,jl)]:
+ *     dTg[c,k] = sum over windows, (i,j) with rel_w(i,j) = k        of  dy_w[i] x_w[j]
+ *     dTl[c,k] = sum over windows, sub-windows, (il,jl) with rel_{w/2}(il,jl) = k  of  dy_sub[il] x_sub[jl]
+ * x and dy are read through the same pad / shift view as the forward (dy is zero outside H x W).
+ * dX is wbmm_ref_hier_forward_train(transpose = 1) applied to dy.  Outputs are overwritten.
+ */
+int wbmm_ref_hier_backward_tables(int B, int C, int H, int W, int w, int sh, int sw, int layout,
+                                  const double *x, const double *dy, double *dTg, double *dTl)
+{
+    if (B < 0 || C < 0 || H < 1 || W < 1 || w < 2 || (w & 1) || sh < 0 || sw < 0 || sh >= w || sw >= w)
+        return 1;
+    const int wl = w / 2, N = w * w, Nl = wl * wl;
+    const int nbg = (2 * w - 1) * (2 * w - 1), nbl = (2 * wl - 1) * (2 * wl - 1);
+    const int Hp = padded(H, w), Wp = padded(W, w);
+    const int nwh = Hp / w, nww = Wp / w;
+
+#pragma omp parallel
+    {
+        double *xw = (double *)malloc(sizeof(double) * (size_t)N);
+        double *gw = (double *)malloc(sizeof(double) * (size_t)N);
+#pragma omp for schedule(static)
+        for (int c = 0; c < C; ++c) {
+            double *dg = dTg + (size_t)c * nbg, *dl = dTl + (size_t)c * nbl;
+            for (int k = 0; k < nbg; ++k) dg[k] = 0.0;
+            for (int k = 0; k < nbl; ++k) dl[k] = 0.0;
+            for (int b = 0; b < B; ++b)
+                for (int wy = 0; wy < nwh; ++wy)
+                    for (int wx = 0; wx < nww; ++wx) {
+                        for (int j = 0; j < N; ++j) {
+                            xw[j] = load_hat(x, layout, B, C, H, W, Hp, Wp, sh, sw, b, c, wy * w + j / w, wx * w + j % w);
+                            gw[j] = load_hat(dy, layout, B, C, H, W, Hp, Wp, sh, sw, b, c, wy * w + j / w, wx * w + j % w);
+                        }
+                        for (int i = 0; i < N; ++i)
+                            for (int j = 0; j < N; ++j)
+                                dg[wbmm_ref_rel_index(w, i, j)] += gw[i] * xw[j];
+                        for (int sr = 0; sr < 2; ++sr)
+                            for (int sc = 0; sc < 2; ++sc)
+                                for (int il = 0; il < Nl; ++il)
+                                    for (int jl = 0; jl < Nl; ++jl) {
+                                        int io = (sr * wl + il / wl) * w + sc * wl + il % wl;
+                                        int jo = (sr * wl + jl / wl) * w + sc * wl + jl % wl;
+                                        dl[wbmm_ref_rel_index(wl, il, jl)] += gw[io] * xw[jo];
+                                    }
+                    }
+        }
+        free(xw); free(gw);
     }
     return 0;
 }

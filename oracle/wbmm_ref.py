@@ -56,6 +56,8 @@ def _load():
     lib.wbmm_ref_hier_forward_train.argtypes = [i] * 9 + [dp, dp, dp, dp]
     lib.wbmm_ref_hier_forward_fused.restype = i
     lib.wbmm_ref_hier_forward_fused.argtypes = [i] * 9 + [dp, dp, dp, dp, dp]
+    lib.wbmm_ref_hier_backward_tables.restype = i
+    lib.wbmm_ref_hier_backward_tables.argtypes = [i] * 8 + [dp, dp, dp, dp]
     lib.wbmm_ref_num_threads.restype = i
     lib.wbmm_ref_set_threads.argtypes = [i]
     _lib = lib
@@ -165,3 +167,22 @@ def hier_forward(x, Tg, Tl, w, shift=(0, 0), layout=NCHW, form="train", transpos
     if rc != 0:
         raise ValueError(f"oracle rejected arguments (rc={rc})")
     return (y, M) if return_matrix else y
+
+
+def hier_backward(x, Tg, Tl, dy, w, shift=(0, 0), layout=NCHW):
+    """Gradients of the hierarchical operator (the backward of Algorithm 2):
+    returns (dx, dTg, dTl).  dx is the transposed operator applied to dy (training form);
+    dTg[C,(2w-1)^2], dTl[C,(w-1)^2] are the table gradients by their definition."""
+    dx = hier_forward(dy, Tg, Tl, w, shift, layout, form="train", transpose=True)
+    x, xp = _d(x)
+    dy, gp = _d(dy)
+    B, C, H, W = _dims(x, layout)
+    assert w % 2 == 0 and x.shape == dy.shape
+    dTg = np.zeros((C, (2 * w - 1) ** 2))
+    dTl = np.zeros((C, (w - 1) ** 2))
+    rc = _load().wbmm_ref_hier_backward_tables(
+        B, C, H, W, w, int(shift[0]), int(shift[1]), layout, xp, gp,
+        dTg.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), dTl.ctypes.data_as(ctypes.POINTER(ctypes.c_double)))
+    if rc != 0:
+        raise ValueError(f"oracle rejected arguments (rc={rc})")
+    return dx, dTg, dTl

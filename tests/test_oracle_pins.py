@@ -473,3 +473,58 @@ def test_hier_transpose_is_adjoint(oracle):
     y = oracle.hier_forward(x, Tg, Tl, w, (2, 5), form="train")
     dx = oracle.hier_forward(dy, Tg, Tl, w, (2, 5), form="train", transpose=True)
     assert abs(np.sum(dy * y) - np.sum(dx * x)) < 1e-10
+
+
+# ------------------------------------------------------------------ hierarchical backward (tables)
+@pytest.mark.parametrize("w,H,W,s", [(4, 8, 12, (0, 0)), (4, 10, 7, (1, 3)), (6, 13, 9, (2, 5)), (14, 30, 20, (7, 5))])
+@pytest.mark.parametrize("layout", [NCHW, NHWC])
+def test_hier_table_gradients_are_directional_derivatives(oracle, w, H, W, s, layout):
+    """y is linear in (Tg, Tl): <dTg, dG> + <dTl, dL> must equal <dy, y(Tg+dG, Tl+dL) - y(Tg, Tl)> exactly
+    (to round-off) for ANY direction -- checks the table gradients against the pinned forward, not
+    against themselves; a wrong index, sign or a dropped sub-window fails it."""
+    x, Tg, Tl = _hier_inputs(90 + w, 2, 3, H, W, w)
+    r = rng(91 + w)
+    dy = r.standard_normal(x.shape)
+    dG = r.standard_normal(Tg.shape)
+    dL = r.standard_normal(Tl.shape)
+    xl, dyl = _to_layout(x, layout), _to_layout(dy, layout)
+    _, dTg, dTl = oracle.hier_backward(xl, Tg, Tl, dyl, w, s, layout)
+    for a, b_ in ((dG, 0 * dL), (0 * dG, dL), (dG, dL)):
+        y1 = oracle.hier_forward(xl, Tg + a, Tl + b_, w, s, layout, "fused")
+        y0 = oracle.hier_forward(xl, Tg, Tl, w, s, layout, "fused")
+        lhs = np.sum(dTg * a) + np.sum(dTl * b_)
+        rhs = np.sum(dyl * (y1 - y0))
+        assert abs(lhs - rhs) < 1e-9 * (1 + abs(rhs))
+
+
+@pytest.mark.parametrize("w", [4, 14])
+def test_hier_table_gradients_reduce_to_single_scale(oracle, w):
+    """On maps that are multiples of w (no shift) the local sub-windows are the w/2 partition of the
+    image: dTg, dTl are the single-scale table gradients at w and w/2 (pinned above)."""
+    x, Tg, Tl = _hier_inputs(100 + w, 2, 3, 2 * w, 3 * w, w)
+    dy = rng(101 + w).standard_normal(x.shape)
+    dx, dTg, dTl = oracle.hier_backward(x, Tg, Tl, dy, w)
+    _, rg = oracle.backward(x, Tg, dy, w, need_dx=False)
+    _, rl = oracle.backward(x, Tl, dy, w // 2, need_dx=False)
+    assert np.max(np.abs(dTg - rg)) < 1e-11
+    assert np.max(np.abs(dTl - rl)) < 1e-11
+    rdx, _ = oracle.backward(x, Tg, dy, w, need_dT=False)
+    rdl, _ = oracle.backward(x, Tl, dy, w // 2, need_dT=False)
+    assert np.max(np.abs(dx - (rdx + rdl + 2 * dy))) < 1e-11
+
+
+def test_hier_table_gradients_w2_closed_form(oracle):
+    """w = 2: the local windows are single pixels, Tl has one entry per channel and dTl = sum(dy * x);
+    the centre bin of dTg (rel = 4 of 9) is the same sum."""
+    r = rng(110)
+    x = r.standard_normal((3, 2, 4, 6))
+    dy = r.standard_normal(x.shape)
+    Tg = r.standard_normal((2, 9))
+    Tl = r.standard_normal((2, 1))
+    _, dTg, dTl = oracle.hier_backward(x, Tg, Tl, dy, 2)
+    s = np.sum(dy * x, axis=(0, 2, 3))
+    assert np.max(np.abs(dTl[:, 0] - s)) < 1e-12
+    assert np.max(np.abs(dTg[:, 4] - s)) < 1e-12
+    # the corner bin (dr, dc) = (+1, +1): output position (1,1) reads input position (0,0) of each 2 x 2 window
+    c = np.sum(dy[:, :, 1::2, 1::2] * x[:, :, 0::2, 0::2], axis=(0, 2, 3))
+    assert np.max(np.abs(dTg[:, 8] - c)) < 1e-12
