@@ -394,6 +394,14 @@ def run_wbmm(args, rank, world, local):
     Tl = (torch.randn((case.C, (case.w - 1) ** 2), generator=g_l) * 0.02).to(T.dtype).to(dev)
     hier_ms = region_ms(lambda: wb.wbmm_hier_forward(xs[0], T, Tl, case.w, out=ys[0]))
     train_step["hier_forward_cfg3_ms"] = hier_ms
+    # ... and its backward on the config-5 shape: dX (transposed fused operator) + both table gradients in one pass
+    g_l5 = torch.Generator(device="cpu").manual_seed(78)
+    Tl5 = (torch.randn((c5.C, (c5.w - 1) ** 2), generator=g_l5) * 0.02).to(d5["T"].dtype).to(dev)
+    train_step["hier_cfg5_ms"] = {
+        "fwd": region_ms(lambda: wb.wbmm_hier_forward(d5["x"], d5["T"], Tl5, c5.w, c5.shift, out=y5)),
+        "dX": region_ms(lambda: wb.wbmm_hier_backward(None, d5["T"], Tl5, d5["dy"], c5.w, c5.shift, need_dT=False)),
+        "dTg_dTl": region_ms(lambda: wb.wbmm_hier_backward(d5["x"], None, None, d5["dy"], c5.w, c5.shift, need_dx=False)),
+    }
 
     tfl_cpu, cores, sample, dt_cpu = time_oracle(case)
     cpu = {"value": tfl_cpu, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,

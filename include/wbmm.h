@@ -120,13 +120,29 @@ WBMM_API int wbmm_backward(const wbmm_desc_t *desc, const void *x, const void *T
  * memory (27 KB instead of the C x 196 x 196 tensor of Algorithm 3).
  *   Tg [in] C*(2w-1)^2, Tl [in] C*(w-1)^2 elements of desc->dtype.  x, y, padding, shift as wbmm_forward.
  *   transpose != 0 applies the transposed fused matrix: dX of the operator for dy in `x`.
- * The table gradients need no entry point of their own: on maps that are multiples of w (no shift)
- * dTg = wbmm_backward(w) and dTl = wbmm_backward(w/2) of the same (x, dy).
+ * Gradients: wbmm_hier_backward.
  * Supported where the pipelined tensor-core kernel is: w = 14, bf16/fp16, NCHW, 16-byte aligned planes
  * (H*W even ... see wbmm_last_path); otherwise WBMM_STATUS_UNSUPPORTED.
  */
 WBMM_API int wbmm_hier_forward(const wbmm_desc_t *desc, const void *x, const void *Tg, const void *Tl, void *y,
                       int transpose, void *cuda_stream);
+
+/*
+ * Backward of wbmm_hier_forward (the gradient of Algorithm 2, term by term; the identity
+ * shortcuts carry no parameter):
+ *   dx  [out, nullable] the transposed fused operator applied to dy (= wbmm_hier_forward(..., transpose = 1)).
+ *   dTg [out, nullable] float32 [C][(2w-1)^2]: sum over windows and pairs (i,j) with rel_w(i,j) = k of dy[i] x[j].
+ *   dTl [out, nullable] float32 [C][(w-1)^2]: the same sum restricted to pairs inside one of the 2 x 2 local
+ *                       sub-windows, binned by rel_{w/2}.  dTg and dTl are given together or not at all; both
+ *                       come from ONE pass over (x, dy): S = dY^T X is accumulated once in tensor memory and
+ *                       folded onto both sets of bins.  Overwritten unless WBMM_FLAG_ACCUMULATE_DT.
+ *   x may be NULL when the table gradients are not requested; Tg, Tl may be NULL when dx is NULL.
+ * Padding, shift and the zero extension of dy as in wbmm_backward.  Supported where the pipelined
+ * tensor-core kernels are (w = 14, bf16/fp16, NCHW, 16-byte aligned planes); otherwise
+ * WBMM_STATUS_UNSUPPORTED, with nothing launched.
+ */
+WBMM_API int wbmm_hier_backward(const wbmm_desc_t *desc, const void *x, const void *Tg, const void *Tl, const void *dy,
+                       void *dx, float *dTg, float *dTl, void *cuda_stream);
 
 /*
  * Eq. 6-8 on their own (test/debug and the WBMM-C "cached M" mode):

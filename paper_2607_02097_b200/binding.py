@@ -23,7 +23,7 @@ _DTYPES = {torch.float32: DTYPE_F32, torch.bfloat16: DTYPE_BF16, torch.float16: 
 
 # every symbol include/wbmm.h declares
 EXPORTS = (
-    "wbmm_forward", "wbmm_backward", "wbmm_hier_forward", "wbmm_materialize_weight", "wbmm_forward_host",
+    "wbmm_forward", "wbmm_backward", "wbmm_hier_forward", "wbmm_hier_backward", "wbmm_materialize_weight", "wbmm_forward_host",
     "wbmm_backward_host", "wbmm_release", "wbmm_last_path", "wbmm_launch_count",
     "wbmm_status_string", "wbmm_path_string", "wbmm_last_error_string", "wbmm_version",
 )
@@ -57,6 +57,8 @@ def lib() -> ctypes.CDLL:
     L.wbmm_backward.argtypes = [dp, vp, vp, vp, vp, vp, vp]
     L.wbmm_hier_forward.argtypes = [dp, vp, vp, vp, vp, i, vp]
     L.wbmm_hier_forward.restype = i
+    L.wbmm_hier_backward.argtypes = [dp, vp, vp, vp, vp, vp, vp, vp, vp]
+    L.wbmm_hier_backward.restype = i
     L.wbmm_materialize_weight.argtypes = [dp, vp, vp, vp]
     L.wbmm_forward_host.argtypes = [dp, vp, vp, vp]
     L.wbmm_backward_host.argtypes = [dp, vp, vp, vp, vp, vp]
@@ -141,6 +143,28 @@ def wbmm_hier_forward(x: torch.Tensor, Tg: torch.Tensor, Tl: torch.Tensor, w: in
     with torch.cuda.device(x.device):
         _check(lib().wbmm_hier_forward(ctypes.byref(d), px, pg, pl, py, 1 if transpose else 0, _stream(x)))
     return y
+
+
+def wbmm_hier_backward(x: Optional[torch.Tensor], Tg: Optional[torch.Tensor], Tl: Optional[torch.Tensor],
+                       dy: torch.Tensor, w: int, shift=(0, 0), layout: int = NCHW, flags: int = 0,
+                       need_dx: bool = True, need_dT: bool = True, dTg: Optional[torch.Tensor] = None,
+                       dTl: Optional[torch.Tensor] = None):
+    """(dx, dTg, dTl) of wbmm_hier_forward (include/wbmm.h: wbmm_hier_backward); the table gradients
+    are float32 [C,(2w-1)^2] and [C,(w-1)^2] and come from one pass over (x, dy)."""
+    d = make_desc(dy, w, shift, layout, flags)
+    dx = torch.empty_like(dy) if need_dx else None
+    if need_dT:
+        if dTg is None:
+            dTg = torch.empty((d.C, (2 * w - 1) ** 2), dtype=torch.float32, device=dy.device)
+        if dTl is None:
+            dTl = torch.empty((d.C, (w - 1) ** 2), dtype=torch.float32, device=dy.device)
+    else:
+        dTg = dTl = None
+    with torch.cuda.device(dy.device):
+        _check(lib().wbmm_hier_backward(ctypes.byref(d), _dev(x, "x") if need_dT else None,
+                                        _dev(Tg, "Tg") if need_dx else None, _dev(Tl, "Tl") if need_dx else None,
+                                        _dev(dy, "dy"), _dev(dx, "dx"), _dev(dTg, "dTg"), _dev(dTl, "dTl"), _stream(dy)))
+    return dx, dTg, dTl
 
 
 def wbmm_backward(x: Optional[torch.Tensor], T: Optional[torch.Tensor], dy: torch.Tensor, w: int,

@@ -258,6 +258,51 @@ int wbmm_hier_forward(const wbmm_desc_t* desc, const void* x, const void* Tg, co
     return WBMM_STATUS_OK;
 }
 
+int wbmm_hier_backward(const wbmm_desc_t* desc, const void* x, const void* Tg, const void* Tl, const void* dy,
+                       void* dx, float* dTg, float* dTl, void* cuda_stream)
+{
+    int st = validate(desc);
+    if (st != WBMM_STATUS_OK) return st;
+    if (desc->w % 2 != 0) return WBMM_STATUS_INVALID_ARGUMENT;
+    if ((dTg == nullptr) != (dTl == nullptr)) return WBMM_STATUS_INVALID_ARGUMENT;   // the two tables go together
+    if (desc->C == 0) return WBMM_STATUS_OK;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    const int wl = desc->w / 2;
+    const size_t ng = sizeof(float) * (size_t)desc->C * (2 * desc->w - 1) * (2 * desc->w - 1);
+    const size_t nl = sizeof(float) * (size_t)desc->C * (2 * wl - 1) * (2 * wl - 1);
+    if (dTg && !aligned(dTg, 4)) return WBMM_STATUS_MISALIGNED;
+    if (dTl && !aligned(dTl, 4)) return WBMM_STATUS_MISALIGNED;
+    if (dTg && !(desc->flags & WBMM_FLAG_ACCUMULATE_DT)) {
+        if (device_state() < 0) return WBMM_STATUS_NO_DEVICE;
+        cudaError_t e = cudaMemsetAsync(dTg, 0, ng, stream);
+        if (e == cudaSuccess) e = cudaMemsetAsync(dTl, 0, nl, stream);
+        if (e != cudaSuccess) return set_cuda_error(e, "memset dT (hierarchical)");
+    }
+    if (desc->B == 0) return WBMM_STATUS_OK;
+    if (!dy || (dx && (!Tg || !Tl)) || (dTg && !x) || (dx && dx == dy)) return WBMM_STATUS_INVALID_ARGUMENT;
+    const size_t es = elem_size(desc->dtype);
+    if (!aligned(dy, es) || (x && !aligned(x, es)) || (Tg && !aligned(Tg, es)) || (Tl && !aligned(Tl, es)) ||
+        (dx && !aligned(dx, es)))
+        return WBMM_STATUS_MISALIGNED;
+    if (device_state() < 0) return WBMM_STATUS_NO_DEVICE;
+    wbmm::Geom g = wbmm::make_geom(*desc);
+    // check both halves before launching either
+    if (dx && !wbmm::tc_hier_supported(g, desc->dtype, dy, dx)) return WBMM_STATUS_UNSUPPORTED;
+    if (dTg && (g.w != 14 || !wbmm::tc_grad_table_supported(g, desc->dtype, x, dy))) return WBMM_STATUS_UNSUPPORTED;
+    if (dx) {
+        st = wbmm_hier_forward(desc, dy, Tg, Tl, dx, 1, cuda_stream);
+        if (st != WBMM_STATUS_OK) return st;
+    }
+    if (dTg) {
+        int launches = 0, path = WBMM_PATH_NONE;
+        cudaError_t e = wbmm::tc_grad_table(g, desc->dtype, x, dy, dTg, stream, &launches, &path, dTl);
+        g_launches += launches;
+        if (e != cudaSuccess) return set_cuda_error(e, "tc_grad_table (hierarchical)");
+        t_last_path = path;
+    }
+    return WBMM_STATUS_OK;
+}
+
 int wbmm_materialize_weight(const wbmm_desc_t* desc, const void* T, void* Wout, void* cuda_stream)
 {
     if (!desc || desc->C < 0 || desc->w < 1 || desc->w > 64) return WBMM_STATUS_INVALID_ARGUMENT;

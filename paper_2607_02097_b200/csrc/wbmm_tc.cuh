@@ -37,8 +37,9 @@ cudaError_t tc_nhwc_forward(const Geom& g, int dtype, const void* x, const void*
                             cudaStream_t stream, int* launches);
 
 bool tc_grad_table_supported(const Geom& g, int dtype, const void* x, const void* dy);
+// dTl != nullptr (w = 14 only): also folds S onto the local (w/2) sub-window table of the hierarchical operator.
 cudaError_t tc_grad_table(const Geom& g, int dtype, const void* x, const void* dy, float* dT,
-                          cudaStream_t stream, int* launches, int* path);
+                          cudaStream_t stream, int* launches, int* path, float* dTl = nullptr);
 
 // Tensor map (CUtensorMap behind the void*) over an NCHW activation with box = `images` whole frame images of
 // one channel (wbmm_tc.cu).

@@ -50,13 +50,17 @@ struct DtCfg {
     static constexpr int BN = Cf::TW * BP;             // floats per private copy
     static_assert(BP >= Cf::TW && BP % 32 == WS % 32, "bin pitch");
     static_assert(MT * 16 <= 2 * NVEC, "an A M-tile must stay inside the stage");
-    static_assert(8 * BN * 4 <= STAGE, "per-warp bin copies alias the stage");
+    // Hierarchical variant: a second set of bins for the (w/2)-window table (row pitch WS: 2*(WS/2)-1 < WS).
+    static constexpr int WL = WS / 2, LTW = 2 * WL - 1, LP = WS, LBN = LTW * LP, LNB = LTW * LTW;
+    static_assert(8 * (BN + LBN) * 4 <= STAGE, "per-warp bin copies alias the stage");
 };
 
-template <int WS, bool BF16, bool GEN>
+// HIER: S is folded a second time, onto the bins of the local (w/2 x w/2) sub-window table -- only pairs
+// (i, j) inside the same sub-window count (Eq. 9: diag_blocks(M_l)).
+template <int WS, bool BF16, bool GEN, bool HIER>
 __global__ void __launch_bounds__(kThreadsD, 1)
 tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __restrict__ x,
-             const uint16_t* __restrict__ dy, float* __restrict__ dT, int box,
+             const uint16_t* __restrict__ dy, float* __restrict__ dT, float* __restrict__ dTl, int box,
              const __grid_constant__ CUtensorMap mx, const __grid_constant__ CUtensorMap mg)
 {
     using Cf = WinCfg<WS>;
@@ -194,6 +198,8 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
         const int emt = ew >> 2, eq = warp & 3;          // M-tile and TMEM lane quarter in the epilogue
         const int erow = emt * 128 + eq * 32 + lane;     // row of S = output position i
         const int eri = erow / WS, eci = erow - eri * WS;
+        float* lw = bins + 8 * Dc::BN + (ot >> 5) * Dc::LBN;   // HIER: this warp's private local-table bins
+        const int erh = eri / Dc::WL, ech = eci / Dc::WL;      // HIER: sub-window of output position i
         uint32_t k = 0, lt = 0;
         for (int t = t0; t < t1; ++t, ++lt) {
             int c, b0, wy0, np_eff, rows_eff;
@@ -246,6 +252,8 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
                 if (ot == 0) TRACE(8, lt);
                 ptx::tc_fence_after_sync();
                 for (int b = lane; b < Dc::BN; b += 32) bw[b] = 0.f;
+                if constexpr (HIER)
+                    for (int b = lane; b < Dc::LBN; b += 32) lw[b] = 0.f;
                 __syncwarp();
                 if (emt < Dc::MT) {
                     // Row i = erow of S goes to bins base - rj*TW - cj.  For a fixed column j the 32 rows of
@@ -255,6 +263,7 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
                     const uint32_t taddr = tmem + emt * 256 + ((uint32_t)(eq * 32) << 16);
                     float* bbase = bw + (eri + WS - 1) * Dc::BP + eci + WS - 1;
                     const bool rowok = erow < Cf::N;
+                    float* lbase = lw + (eri + Dc::WL - 1) * Dc::LP + eci + Dc::WL - 1;
                     constexpr int RJ_STRIDE = 31 / WS + 1, NU = (WS + RJ_STRIDE - 1) / RJ_STRIDE;
 #pragma unroll
                     for (int g0 = 0; g0 < RJ_STRIDE; ++g0) {
@@ -276,6 +285,19 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
                                 if (g0 + u * RJ_STRIDE < WS && rowok)
                                     bbase[-(g0 + u * RJ_STRIDE) * Dc::BP - cj] = old[u] + __uint_as_float(v[u][cj]);
                             __syncwarp();
+                            if constexpr (HIER) {
+                                // same S element, local bin (ri - rj + w/2 - 1, ci - cj + w/2 - 1), if j is in i's sub-window
+                                const bool colok = rowok && ech == cj / Dc::WL;
+#pragma unroll
+                                for (int u = 0; u < NU; ++u)
+                                    if (g0 + u * RJ_STRIDE < WS && colok && erh == (g0 + u * RJ_STRIDE) / Dc::WL)
+                                        old[u] = lbase[-(g0 + u * RJ_STRIDE) * Dc::LP - cj];
+#pragma unroll
+                                for (int u = 0; u < NU; ++u)
+                                    if (g0 + u * RJ_STRIDE < WS && colok && erh == (g0 + u * RJ_STRIDE) / Dc::WL)
+                                        lbase[-(g0 + u * RJ_STRIDE) * Dc::LP - cj] = old[u] + __uint_as_float(v[u][cj]);
+                                __syncwarp();
+                            }
                         }
                         if (ot == 0 && g0 == 0) TRACE(14, lt);
                     }
@@ -291,10 +313,20 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
                     for (int w8 = 0; w8 < 8; ++w8) sacc += bins[w8 * Dc::BN + bp];
                     atomicAdd(dT + (long long)c * Cf::NB + b, sacc);
                 }
+                if constexpr (HIER) {
+                    const float* lbins = bins + 8 * Dc::BN;
+                    for (int b = ot; b < Dc::LNB; b += 256) {
+                        float sacc = 0.f;
+                        const int bp = (b / Dc::LTW) * Dc::LP + b % Dc::LTW;
+#pragma unroll
+                        for (int w8 = 0; w8 < 8; ++w8) sacc += lbins[w8 * Dc::LBN + bp];
+                        atomicAdd(dTl + (long long)c * Dc::LNB + b, sacc);
+                    }
+                }
                 ptx::named_bar_sync(1, 256);
                 if (ot == 0) TRACE(12, lt);
                 // the bins aliased the operand stage: restore the zero padding vectors
-                for (int i = ot; i < 8 * Dc::BN * 4 / 16 + 1; i += 256)
+                for (int i = ot; i < 8 * (Dc::BN + Dc::LBN) * 4 / 16 + 1; i += 256)
                     if (i * 16 < Dc::STAGE) reinterpret_cast<uint4*>(stage)[i] = make_uint4(0, 0, 0, 0);
                 ptx::fence_proxy_async_smem();
                 ptx::named_bar_sync(1, 256);
@@ -332,10 +364,11 @@ int dt_mode(const Geom& g, const TcTiles& tl, const void* x, const void* dy)
     return (tl.nstrips == 1 && g.W % 2 == 0 && g.Wp % 2 == 0) ? 2 : 0;
 }
 
-template <int WS, bool BF16, bool GEN>
-cudaError_t launch_dt(const Geom& g, const TcTiles& tl_in, const void* x, const void* dy, float* dT, cudaStream_t s)
+template <int WS, bool BF16, bool GEN, bool HIER = false>
+cudaError_t launch_dt(const Geom& g, const TcTiles& tl_in, const void* x, const void* dy, float* dT, cudaStream_t s,
+                      float* dTl = nullptr)
 {
-    auto k = tc_dt_kernel<WS, BF16, GEN>;
+    auto k = tc_dt_kernel<WS, BF16, GEN, HIER>;
     TcTiles tl = tl_in;
     CUtensorMap mx, mg;
     memset(&mx, 0, sizeof(mx));
@@ -390,7 +423,7 @@ cudaError_t launch_dt(const Geom& g, const TcTiles& tl_in, const void* x, const 
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, k, g, tl, part, nslot, (const uint16_t*)x, (const uint16_t*)dy, dT, box, mx, mg);
+    return cudaLaunchKernelEx(&cfg, k, g, tl, part, nslot, (const uint16_t*)x, (const uint16_t*)dy, dT, dTl, box, mx, mg);
 }
 
 }  // namespace
@@ -405,7 +438,7 @@ bool tc_grad_table_supported(const Geom& g, int dtype, const void* x, const void
 }
 
 cudaError_t tc_grad_table(const Geom& g, int dtype, const void* x, const void* dy, float* dT, cudaStream_t stream,
-                          int* launches, int* path)
+                          int* launches, int* path, float* dTl)
 {
     TcTiles tl;
     if (!tc_tiles(g, &tl)) return cudaErrorNotSupported;
@@ -415,6 +448,14 @@ cudaError_t tc_grad_table(const Geom& g, int dtype, const void* x, const void* d
     *launches += 1;
     *path = WBMM_PATH_TC_TMA;
     const bool bf = dtype == WBMM_DTYPE_BF16;
+    if (dTl) {
+        // hierarchical: both table gradients from one pass over (x, dy)
+        if (g.w != 14) return cudaErrorNotSupported;
+        if (mode == 2) return bf ? launch_dt<14, true, true, true>(g, tl, x, dy, dT, stream, dTl)
+                                 : launch_dt<14, false, true, true>(g, tl, x, dy, dT, stream, dTl);
+        return bf ? launch_dt<14, true, false, true>(g, tl, x, dy, dT, stream, dTl)
+                  : launch_dt<14, false, false, true>(g, tl, x, dy, dT, stream, dTl);
+    }
     const int sel = (g.w == 7 ? 0 : 4) + (bf ? 2 : 0) + (mode == 2 ? 1 : 0);
     switch (sel) {
     case 0: return launch_dt<7, false, false>(g, tl, x, dy, dT, stream);

@@ -228,6 +228,46 @@ def test_hier_one_hot_tables_bitwise(wb, oracle, which):
         assert np.array_equal(widen(y), ref)
 
 
+@pytest.mark.parametrize("case", [
+    si.Case("hb_plain", 19, 5, 56, 56, 14, seed=51, backward=True),
+    si.Case("hb_many", 40, 150, 28, 28, 14, seed=52, backward=True),          # box mode, several segments per CTA
+    si.Case("hb_shift", 9, 7, 28, 56, 14, shift=(7, 3), seed=53, backward=True),
+    si.Case("hb_ragged_shift", 7, 6, 60, 60, 14, shift=(5, 9), seed=54, backward=True),
+    si.Case("hb_f16", 10, 9, 42, 56, 14, dtype="f16", shift=(0, 7), seed=56, backward=True),
+], ids=lambda c: c.name)
+def test_hier_backward_matches_oracle(wb, oracle, case):
+    """dx, dTg, dTl of the hierarchical operator: one transposed fused forward and ONE pass of the
+    table-gradient kernel that folds S onto both sets of bins."""
+    d, Tl = _hier_case(case)
+    dx, dTg, dTl = wb.wbmm_hier_backward(d["x"], d["T"], Tl, d["dy"], case.w, case.shift, case.layout)
+    torch.cuda.synchronize()
+    assert wb.wbmm_last_path() == wb.PATH_TC_TMA
+    rdx, rg, rl = oracle.hier_backward(widen(d["x"]), widen(d["T"]), widen(Tl), widen(d["dy"]), case.w, case.shift, case.layout)
+    tol = TOL[case.dtype]
+    errs = (max_err_over_tol(dx, rdx, tol), max_err_over_tol(dTg, rg, tol), max_err_over_tol(dTl, rl, tol))
+    assert max(errs) <= 1.0, errs
+    # the global table gradient is the single-scale one: same kernel, same bins
+    _, dT = wb.wbmm_backward(d["x"], None, d["dy"], case.w, case.shift, case.layout, need_dx=False)
+    assert max_err_over_tol(dTg, widen(dT), 1e-5) <= 1.0
+    # accumulate flag: a second call doubles both
+    wb.wbmm_hier_backward(d["x"], None, None, d["dy"], case.w, case.shift, case.layout, wb.FLAG_ACCUMULATE_DT,
+                          need_dx=False, dTg=dTg, dTl=dTl)
+    assert max_err_over_tol(dTg, 2 * rg, tol) <= 1.0 and max_err_over_tol(dTl, 2 * rl, tol) <= 1.0
+
+
+def test_hier_backward_local_bins_exact_on_integers(wb, oracle):
+    """Small-integer x and dy: every product and partial sum is an exact fp32 integer, so both table
+    gradients must equal the oracle exactly -- pins the sub-window predicate of the second fold."""
+    C = 20
+    gen = torch.Generator().manual_seed(57)
+    x = torch.randint(-2, 3, (8, C, 28, 28), generator=gen).to(torch.bfloat16).cuda()
+    dy = torch.randint(-2, 3, (8, C, 28, 28), generator=gen).to(torch.bfloat16).cuda()
+    _, dTg, dTl = wb.wbmm_hier_backward(x, None, None, dy, 14, (3, 8), need_dx=False)
+    z = np.zeros((C, 729)), np.zeros((C, 169))
+    _, rg, rl = oracle.hier_backward(widen(x), z[0], z[1], widen(dy), 14, (3, 8))
+    assert np.array_equal(widen(dTg), rg) and np.array_equal(widen(dTl), rl)
+
+
 def test_hier_unsupported_shapes_fail_loudly(wb):
     x = torch.zeros((2, 4, 14, 14), dtype=torch.bfloat16, device="cuda")
     with pytest.raises(wb.WbmmError):       # w = 7 has no hierarchical tensor-core path
