@@ -186,3 +186,48 @@ def hier_backward(x, Tg, Tl, dy, w, shift=(0, 0), layout=NCHW):
     if rc != 0:
         raise ValueError(f"oracle rejected arguments (rc={rc})")
     return dx, dTg, dTl
+
+
+def apply_matrix(x, M, w, shift=(0, 0), layout=NCHW, transpose=False, bias=None) -> np.ndarray:
+    """Cached-M mode, WBMM-C: Algorithm 1 with a GIVEN per-channel
+    matrix M[C, N, N] (y_win = M_c x_win, orientation A1) instead of M = R[:, I]; optional per-channel bias
+    (Eq. 1's beta_c).  Written out in the paper's order with plain numpy: pad (l.2), roll
+    (A6), window partition (l.3-4), one batched matrix product (l.15), inverse reshape (l.17), un-roll, crop."""
+    x = np.asarray(x, dtype=np.float64)
+    M = np.asarray(M, dtype=np.float64)
+    xc = x if layout == NCHW else np.transpose(x, (0, 3, 1, 2))
+    B, C, H, W = xc.shape
+    N = w * w
+    assert M.shape == (C, N, N)
+    Hp, Wp = -(-H // w) * w, -(-W // w) * w
+    xp = np.zeros((B, C, Hp, Wp))
+    xp[:, :, :H, :W] = xc                                              # zero padding, bottom / right (A4)
+    xh = np.roll(xp, (-int(shift[0]), -int(shift[1])), axis=(2, 3))    # x^[h, v] = x~[(h + s) mod H', ...] (A6)
+    nh, nw = Hp // w, Wp // w
+    win = xh.reshape(B, C, nh, w, nw, w).transpose(0, 1, 2, 4, 3, 5).reshape(B, C, nh * nw, N)
+    Mc = np.transpose(M, (0, 2, 1)) if transpose else M
+    yw = np.einsum("cij,bcnj->bcni", Mc, win)                          # l.15: the batched product
+    yh = yw.reshape(B, C, nh, nw, w, w).transpose(0, 1, 2, 4, 3, 5).reshape(B, C, Hp, Wp)
+    y = np.roll(yh, (int(shift[0]), int(shift[1])), axis=(2, 3))[:, :, :H, :W]
+    if bias is not None:
+        y = y + np.asarray(bias, dtype=np.float64).reshape(1, C, 1, 1)
+    return np.ascontiguousarray(y if layout == NCHW else np.transpose(y, (0, 2, 3, 1)))
+
+
+def fold_dwconv(T, K, w, scale=None) -> np.ndarray:
+    """Multi-kernel fusion (section 3.7): on a map that is ONE w x w window, a zero-padded
+    depthwise conv (Eq. 1: Y[h,v] = sum_{i,j} K[i+k, j+k] X[h+i, v+j]) is the WBMM operator whose table is
+    zero except T[(w-1-i)(2w-1) + (w-1-j)] = K[i+k, j+k] -- output p = (h,v) reads input q = (h+i, v+j), and
+    rel(p, q) = (r_p - r_q + w-1)(2w-1) + (c_p - c_q + w-1) (Eq. 6-7).  Returns T + scale_c * (that table);
+    the scale is BatchNorm's gamma / sigma (its shift becomes the bias of apply_matrix)."""
+    T = np.array(T, dtype=np.float64)
+    K = np.asarray(K, dtype=np.float64)
+    C, kk, _ = K.shape
+    k = kk // 2
+    assert kk % 2 == 1 and k <= w - 1 and T.shape == (C, (2 * w - 1) ** 2)
+    s = np.ones(C) if scale is None else np.asarray(scale, dtype=np.float64)
+    tw = 2 * w - 1
+    for i in range(-k, k + 1):
+        for j in range(-k, k + 1):
+            T[:, (w - 1 - i) * tw + (w - 1 - j)] += s * K[:, i + k, j + k]
+    return T

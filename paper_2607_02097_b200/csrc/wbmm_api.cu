@@ -2,6 +2,7 @@
 // No compute happens here and nothing here can fall back to a CPU implementation.
 #include <atomic>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 
@@ -345,9 +346,21 @@ std::mutex g_host_mutex;
 Scratch g_sx, g_sT, g_sy, g_sdy, g_sdT;
 cudaStream_t g_host_stream = nullptr;
 
-constexpr int kHostChunks = 8;
+constexpr int kHostChunks = 32;   // at most; see host_chunks()
 cudaStream_t g_s_kernel = nullptr, g_s_out = nullptr;
 cudaEvent_t g_ev_in[kHostChunks] = {}, g_ev_k[kHostChunks] = {};
+
+// Chunks per call: enough that the un-overlapped head (first upload) and tail (last download) are small,
+// few enough that per-copy set-up does not show.  WBMM_HOST_CHUNKS overrides (1..32) for experiments.
+int host_chunks()
+{
+    static int n = [] {
+        const char* e = getenv("WBMM_HOST_CHUNKS");
+        int v = e ? atoi(e) : 8;
+        return v < 1 ? 1 : (v > kHostChunks ? kHostChunks : v);
+    }();
+    return n;
+}
 
 cudaError_t host_pipeline_init()
 {
@@ -411,7 +424,7 @@ int wbmm_forward_host(const wbmm_desc_t* desc, const void* x_host, const void* T
     // upload of chunk i+1, the kernels of chunk i and the download of chunk i-1 overlap (PCIe is full
     // duplex; with pinned host buffers the call takes about max(H2D, D2H) instead of their sum).
     WBMM_TRY(host_pipeline_init(), "streams");
-    const int nchunk = nact >= (8u << 20) ? (g.B < kHostChunks ? g.B : kHostChunks) : 1;
+    const int nchunk = nact >= (8u << 20) ? (g.B < host_chunks() ? g.B : host_chunks()) : 1;
     const size_t per_image = nact / (size_t)g.B;
     WBMM_TRY(cudaMemcpyAsync(g_sT.p, T_host, ntab, cudaMemcpyHostToDevice, s), "H2D T");
     for (int i = 0; i < nchunk; ++i) {

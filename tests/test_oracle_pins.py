@@ -528,3 +528,66 @@ def test_hier_table_gradients_w2_closed_form(oracle):
     # the corner bin (dr, dc) = (+1, +1): output position (1,1) reads input position (0,0) of each 2 x 2 window
     c = np.sum(dy[:, :, 1::2, 1::2] * x[:, :, 0::2, 0::2], axis=(0, 2, 3))
     assert np.max(np.abs(dTg[:, 8] - c)) < 1e-12
+
+
+# ------------------------------------------------------------------ cached-M mode and multi-kernel fusion (NEXT-2)
+@pytest.mark.parametrize("w,H,W,s", [(3, 6, 9, (0, 0)), (4, 10, 7, (1, 3)), (7, 14, 21, (3, 0)), (14, 30, 20, (7, 5))])
+@pytest.mark.parametrize("layout", [NCHW, NHWC])
+def test_apply_matrix_with_table_matrix_is_the_operator(oracle, w, H, W, s, layout):
+    """WBMM-C and WBMM-NC "produce identical outputs": Algorithm 1 with M = R[:, I] given as
+    a matrix equals the pinned direct form; the transposed application equals the pinned dX."""
+    r = rng(120 + w)
+    x = r.standard_normal((2, 3, H, W))
+    T = r.standard_normal((3, (2 * w - 1) ** 2))
+    xl = _to_layout(x, layout)
+    M = oracle.weight_matrix(T, w)
+    assert np.max(np.abs(oracle.apply_matrix(xl, M, w, s, layout) - oracle.forward(xl, T, w, s, layout))) < 1e-12
+    dx, _ = oracle.backward(xl, T, xl, w, s, layout, need_dT=False)
+    assert np.max(np.abs(oracle.apply_matrix(xl, M, w, s, layout, transpose=True) - dx)) < 1e-12
+
+
+def test_apply_matrix_brute_force_non_toeplitz(oracle):
+    """An arbitrary (non-Toeplitz) M and a bias against pure-Python loops over a tiny ragged, shifted map."""
+    r = rng(130)
+    B, C, H, W, w, s = 2, 2, 5, 7, 3, (1, 2)
+    x = r.standard_normal((B, C, H, W))
+    M = r.standard_normal((C, 9, 9))
+    bias = r.standard_normal(C)
+    Hp, Wp = 6, 9
+    ref = np.zeros_like(x)
+    for b in range(B):
+        for c in range(C):
+            for wy in range(Hp // w):
+                for wx in range(Wp // w):
+                    for i in range(9):
+                        acc = 0.0
+                        for j in range(9):
+                            h, v = (wy * w + j // w + s[0]) % Hp, (wx * w + j % w + s[1]) % Wp
+                            acc += M[c, i, j] * (x[b, c, h, v] if h < H and v < W else 0.0)
+                        h, v = (wy * w + i // w + s[0]) % Hp, (wx * w + i % w + s[1]) % Wp
+                        if h < H and v < W:
+                            ref[b, c, h, v] = acc + bias[c]
+    assert np.max(np.abs(oracle.apply_matrix(x, M, w, s, bias=bias) - ref)) < 1e-13
+
+
+@pytest.mark.parametrize("w", [7, 5])
+def test_fold_dwconv_equals_library_conv_on_one_window(oracle, w):
+    """Section 3.7: Y = WBMM(X) + BN1(DW5(X)) + BN2(DW3(X)) on a single-window map equals ONE WBMM with the
+    folded table plus a bias -- the conv branches come from a LIBRARY routine (torch conv2d, cross-correlation,
+    zero padding), the BatchNorms are written out as scale and shift."""
+    import torch
+    import torch.nn.functional as F
+    r = rng(140 + w)
+    B, C = 3, 4
+    x = r.standard_normal((B, C, w, w))
+    T = 0.1 * r.standard_normal((C, (2 * w - 1) ** 2))
+    K5, K3 = r.standard_normal((C, 5, 5)), r.standard_normal((C, 3, 3))
+    s1, b1, s2, b2 = (r.standard_normal(C) for _ in range(4))
+    xt = torch.from_numpy(x)
+    d5 = F.conv2d(xt, torch.from_numpy(K5).reshape(C, 1, 5, 5), padding=2, groups=C).numpy()
+    d3 = F.conv2d(xt, torch.from_numpy(K3).reshape(C, 1, 3, 3), padding=1, groups=C).numpy()
+    ref = oracle.forward(x, T, w) + s1.reshape(1, C, 1, 1) * d5 + b1.reshape(1, C, 1, 1) \
+        + s2.reshape(1, C, 1, 1) * d3 + b2.reshape(1, C, 1, 1)
+    Tf = oracle.fold_dwconv(oracle.fold_dwconv(T, K5, w, s1), K3, w, s2)
+    got = oracle.apply_matrix(x, oracle.weight_matrix(Tf, w), w, bias=b1 + b2)
+    assert np.max(np.abs(got - ref)) < 1e-11
