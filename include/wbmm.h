@@ -152,6 +152,38 @@ WBMM_API int wbmm_hier_backward(const wbmm_desc_t *desc, const void *x, const vo
 WBMM_API int wbmm_materialize_weight(const wbmm_desc_t *desc, const void *T, void *Wout, void *cuda_stream);
 
 /*
+ * Cached-M inference mode, "WBMM-C": Algorithm 1 with GIVEN per-channel matrices,
+ *     y_win = M_c * x_win (+ bias_c),
+ *   M    [in] [C][N][N] elements of desc->dtype, row i = output position, column j = input position (the
+ *             layout wbmm_materialize_weight writes); any matrix, not only Eq. 8's.
+ *   bias [in, nullable] [C] elements of desc->dtype (Eq. 1's beta_c; the BatchNorm shifts of section 3.7), added
+ *             to the fp32 accumulator before the single rounding.
+ *   transpose != 0 applies M_c^T (the dX of the cached operator; the bias is still added if given).
+ * x, y, padding, shift, layout as wbmm_forward.  With M = wbmm_materialize_weight(T) and no bias the result is
+ * wbmm_forward's ("identical outputs") up to the fp32 summation order of the kernel that serves it
+ * (at most one 16-bit ulp).  Served by the gather tensor-core kernel
+ * (w in {7, 14}, bf16/fp16, any layout / shift / ragged size); otherwise WBMM_STATUS_UNSUPPORTED.  On this design
+ * the cached mode is NOT the fast one: the table path rebuilds its weights in shared memory from 1.4 KB per
+ * channel while M costs 75 KB per channel of HBM traffic -- it exists for matrices that are not table-generated.
+ */
+WBMM_API int wbmm_forward_matrix(const wbmm_desc_t *desc, const void *x, const void *M, const void *bias, void *y,
+                        int transpose, void *cuda_stream);
+
+/*
+ * Multi-kernel fusion for one-window maps (section 3.7): a zero-padded ksize x ksize depthwise
+ * conv (Eq. 1, cross-correlation) on an H = W = w map is the WBMM operator with the conv kernel written around
+ * the centre of the table, so  Y = WBMM(X) + BN1(DW5(X)) + BN2(DW3(X))  folds into ONE table plus a bias:
+ *     Tout[c, (w-1-i)(2w-1) + (w-1-j)] = T[c, same] + scale[c] * K[c, i+k, j+k],   -k <= i, j <= k = ksize/2,
+ * every other entry copied.  T, Tout [C][(2w-1)^2] and K [C][ksize][ksize] of desc->dtype (Tout may be T);
+ * scale [in, nullable = 1] float32 [C] (BatchNorm's gamma / sigma; its shift goes to wbmm_forward_matrix's bias,
+ * or is added by the caller).  fp32 arithmetic, one rounding.  Only C, w and dtype of the descriptor are used;
+ * ksize odd, ksize/2 <= w-1.  The fold is exact for maps of one window; on larger maps the conv would cross
+ * window borders and the identity does not hold.
+ */
+WBMM_API int wbmm_fold_dwconv(const wbmm_desc_t *desc, const void *T, const void *K, int ksize, const float *scale,
+                     void *Tout, void *cuda_stream);
+
+/*
  * End-to-end variants with HOST buffers (pageable or pinned).  Each call copies its inputs to
  * device scratch owned by the library (grown on demand, reused between calls, freed by
  * wbmm_release()), runs the same kernels as the device entry points on an internal stream,

@@ -23,7 +23,7 @@ _DTYPES = {torch.float32: DTYPE_F32, torch.bfloat16: DTYPE_BF16, torch.float16: 
 
 # every symbol include/wbmm.h declares
 EXPORTS = (
-    "wbmm_forward", "wbmm_backward", "wbmm_hier_forward", "wbmm_hier_backward", "wbmm_materialize_weight", "wbmm_forward_host",
+    "wbmm_forward", "wbmm_backward", "wbmm_hier_forward", "wbmm_hier_backward", "wbmm_forward_matrix", "wbmm_fold_dwconv", "wbmm_materialize_weight", "wbmm_forward_host",
     "wbmm_backward_host", "wbmm_release", "wbmm_last_path", "wbmm_launch_count",
     "wbmm_status_string", "wbmm_path_string", "wbmm_last_error_string", "wbmm_version",
 )
@@ -60,6 +60,10 @@ def lib() -> ctypes.CDLL:
     L.wbmm_hier_backward.argtypes = [dp, vp, vp, vp, vp, vp, vp, vp, vp]
     L.wbmm_hier_backward.restype = i
     L.wbmm_materialize_weight.argtypes = [dp, vp, vp, vp]
+    L.wbmm_forward_matrix.argtypes = [dp, vp, vp, vp, vp, i, vp]
+    L.wbmm_forward_matrix.restype = i
+    L.wbmm_fold_dwconv.argtypes = [dp, vp, vp, i, vp, vp, vp]
+    L.wbmm_fold_dwconv.restype = i
     L.wbmm_forward_host.argtypes = [dp, vp, vp, vp]
     L.wbmm_backward_host.argtypes = [dp, vp, vp, vp, vp, vp]
     for n in ("wbmm_forward", "wbmm_backward", "wbmm_materialize_weight", "wbmm_forward_host",
@@ -193,6 +197,40 @@ def wbmm_materialize_weight(T: torch.Tensor, w: int) -> torch.Tensor:
     with torch.cuda.device(T.device):
         _check(lib().wbmm_materialize_weight(ctypes.byref(d), _dev(T, "T"), _dev(W, "W"), _stream(T)))
     return W
+
+
+def wbmm_forward_matrix(x: torch.Tensor, M: torch.Tensor, w: int, shift=(0, 0), layout: int = NCHW,
+                        bias: Optional[torch.Tensor] = None, transpose: bool = False,
+                        out: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """Cached-M mode (WBMM-C): y_win = M_c x_win (+ bias_c) with M [C,N,N] given
+    (include/wbmm.h: wbmm_forward_matrix)."""
+    d = make_desc(x, w, shift, layout, 0)
+    if M.dtype != x.dtype or tuple(M.shape) != (d.C, w * w, w * w):
+        raise ValueError("M must be [C, w*w, w*w] in the dtype of x")
+    if bias is not None and (bias.dtype != x.dtype or tuple(bias.shape) != (d.C,)):
+        raise ValueError("bias must be [C] in the dtype of x")
+    y = torch.empty_like(x) if out is None else out
+    with torch.cuda.device(x.device):
+        _check(lib().wbmm_forward_matrix(ctypes.byref(d), _dev(x, "x"), _dev(M, "M"), _dev(bias, "bias"),
+                                         _dev(y, "y"), 1 if transpose else 0, _stream(x)))
+    return y
+
+
+def wbmm_fold_dwconv(T: torch.Tensor, K: torch.Tensor, w: int, scale: Optional[torch.Tensor] = None,
+                     out: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """T + scale_c * (table of the zero-padded depthwise conv K [C,k,k]) -- section 3.7's fold for
+    one-window maps (include/wbmm.h: wbmm_fold_dwconv)."""
+    C = T.shape[0]
+    if K.dtype != T.dtype or K.dim() != 3 or K.shape[0] != C or K.shape[1] != K.shape[2]:
+        raise ValueError("K must be [C, k, k] in the dtype of T")
+    if scale is not None and (scale.dtype != torch.float32 or tuple(scale.shape) != (C,)):
+        raise ValueError("scale must be float32 [C]")
+    d = WbmmDesc(0, C, 1, 1, int(w), 0, 0, _DTYPES[T.dtype], NCHW, 0)
+    Tout = torch.empty_like(T) if out is None else out
+    with torch.cuda.device(T.device):
+        _check(lib().wbmm_fold_dwconv(ctypes.byref(d), _dev(T, "T"), _dev(K, "K"), int(K.shape[1]),
+                                      _dev(scale, "scale"), _dev(Tout, "Tout"), _stream(T)))
+    return Tout
 
 
 def _host(t: Optional[torch.Tensor], name: str) -> Optional[int]:

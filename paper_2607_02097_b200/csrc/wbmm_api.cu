@@ -304,6 +304,48 @@ int wbmm_hier_backward(const wbmm_desc_t* desc, const void* x, const void* Tg, c
     return WBMM_STATUS_OK;
 }
 
+int wbmm_forward_matrix(const wbmm_desc_t* desc, const void* x, const void* M, const void* bias, void* y,
+                        int transpose, void* cuda_stream)
+{
+    int st = validate(desc);
+    if (st != WBMM_STATUS_OK) return st;
+    if (desc->B == 0 || desc->C == 0) return WBMM_STATUS_OK;
+    if (!x || !M || !y || x == y) return WBMM_STATUS_INVALID_ARGUMENT;
+    const size_t es = elem_size(desc->dtype);
+    if (!aligned(x, es) || !aligned(M, es) || !aligned(y, es) || (bias && !aligned(bias, es))) return WBMM_STATUS_MISALIGNED;
+    if (device_state() < 0) return WBMM_STATUS_NO_DEVICE;
+    wbmm::Geom g = wbmm::make_geom(*desc);
+    if (!wbmm::tc_forward_supported(g, desc->dtype, x, y)) return WBMM_STATUS_UNSUPPORTED;
+    int launches = 0, path = WBMM_PATH_NONE;
+    cudaError_t e = wbmm::tc_forward_matrix(g, desc->dtype, x, M, bias, y, transpose != 0,
+                                            static_cast<cudaStream_t>(cuda_stream), &launches, &path);
+    g_launches += launches;
+    if (e != cudaSuccess) return set_cuda_error(e, "tc_forward_matrix");
+    t_last_path = path;
+    return WBMM_STATUS_OK;
+}
+
+int wbmm_fold_dwconv(const wbmm_desc_t* desc, const void* T, const void* K, int ksize, const float* scale,
+                     void* Tout, void* cuda_stream)
+{
+    if (!desc || desc->C < 0 || desc->w < 1 || desc->w > 64) return WBMM_STATUS_INVALID_ARGUMENT;
+    if (desc->dtype != WBMM_DTYPE_F32 && desc->dtype != WBMM_DTYPE_BF16 && desc->dtype != WBMM_DTYPE_F16)
+        return WBMM_STATUS_INVALID_ARGUMENT;
+    if (ksize < 1 || ksize % 2 == 0 || ksize / 2 > desc->w - 1) return WBMM_STATUS_INVALID_ARGUMENT;
+    if (desc->C == 0) return WBMM_STATUS_OK;
+    if (!T || !K || !Tout) return WBMM_STATUS_INVALID_ARGUMENT;
+    const size_t es = elem_size(desc->dtype);
+    if (!aligned(T, es) || !aligned(K, es) || !aligned(Tout, es) || (scale && !aligned(scale, 4))) return WBMM_STATUS_MISALIGNED;
+    if (device_state() < 0) return WBMM_STATUS_NO_DEVICE;
+    int launches = 0;
+    cudaError_t e = wbmm::simt_fold_dwconv(desc->C, desc->w, ksize, desc->dtype, T, K, scale, Tout,
+                                           static_cast<cudaStream_t>(cuda_stream), &launches);
+    g_launches += launches;
+    if (e != cudaSuccess) return set_cuda_error(e, "fold_dwconv");
+    t_last_path = WBMM_PATH_SIMT;
+    return WBMM_STATUS_OK;
+}
+
 int wbmm_materialize_weight(const wbmm_desc_t* desc, const void* T, void* Wout, void* cuda_stream)
 {
     if (!desc || desc->C < 0 || desc->w < 1 || desc->w > 64) return WBMM_STATUS_INVALID_ARGUMENT;

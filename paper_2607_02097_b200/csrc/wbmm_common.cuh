@@ -62,6 +62,9 @@ cudaError_t simt_grad_table(const Geom& g, int dtype, const void* x, const void*
                             cudaStream_t stream, int* launches);
 cudaError_t simt_materialize(int C, int w, int dtype, const void* T, void* Wout,
                              cudaStream_t stream, int* launches);
+// Tout = T + scale_c * (the table of a zero-padded kk x kk depthwise conv); Tout may be T.
+cudaError_t simt_fold_dwconv(int C, int w, int kk, int dtype, const void* T, const void* K, const float* scale,
+                             void* Tout, cudaStream_t stream, int* launches);
 // Batched transposition of 16-bit elements in[b][R][Cc] -> out[b][Cc][R] (wbmm_transpose.cu).
 bool transpose16_supported(long long R, long long Cc, const void* in, const void* out);
 cudaError_t transpose16(const void* in, void* out, int batch, int R, int Cc, cudaStream_t stream, int* launches);

@@ -214,6 +214,26 @@ __global__ void materialize_kernel(int C, int w, const E* __restrict__ T, E* __r
     }
 }
 
+// Section 3.7: a zero-padded depthwise conv on a one-window map is the operator whose table
+// holds the conv kernel around the centre: Tout[c, (w-1-i)(2w-1) + (w-1-j)] = T[...] + scale_c * K[c, i+k, j+k]
+// (Eq. 1 read through Eq. 6-7: output p = (h, v) reads input q = (h+i, v+j)).  fp32 arithmetic, one RNE rounding.
+template <typename E>
+__global__ void fold_dwconv_kernel(int C, int w, int kk, const E* __restrict__ T, const E* __restrict__ K,
+                                   const float* __restrict__ scale, E* __restrict__ Tout)
+{
+    const int tw = 2 * w - 1, nb = tw * tw, k = kk / 2;
+    const long long total = (long long)C * nb;
+    for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total;
+         idx += (long long)gridDim.x * blockDim.x) {
+        const int c = (int)(idx / nb), b = (int)(idx % nb);
+        const int i = (w - 1) - b / tw, j = (w - 1) - b % tw;      // the conv tap this bin is
+        float v = to_f32(T[idx]);
+        if (i >= -k && i <= k && j >= -k && j <= k)
+            v = fmaf(scale ? scale[c] : 1.f, to_f32(K[((long long)c * kk + (i + k)) * kk + (j + k)]), v);
+        Tout[idx] = from_f32<E>(v);
+    }
+}
+
 struct TileCfg {
     int CB, G;
     size_t smem_fwd, smem_dt;
@@ -322,6 +342,21 @@ cudaError_t simt_materialize(int C, int w, int dtype, const void* T, void* Wout,
         materialize_kernel<uint32_t><<<blocks, 256, 0, s>>>(C, w, (const uint32_t*)T, (uint32_t*)Wout);
     else
         materialize_kernel<uint16_t><<<blocks, 256, 0, s>>>(C, w, (const uint16_t*)T, (uint16_t*)Wout);
+    return cudaGetLastError();
+}
+
+cudaError_t simt_fold_dwconv(int C, int w, int kk, int dtype, const void* T, const void* K, const float* scale,
+                             void* Tout, cudaStream_t s, int* launches)
+{
+    const long long total = (long long)C * (2 * w - 1) * (2 * w - 1);
+    if (total == 0) return cudaSuccess;
+    const int blocks = (int)((total + 255) / 256 < 148 * 4 ? (total + 255) / 256 : 148 * 4);
+    *launches += 1;
+    switch (dtype) {
+    case WBMM_DTYPE_F32: fold_dwconv_kernel<float><<<blocks, 256, 0, s>>>(C, w, kk, (const float*)T, (const float*)K, scale, (float*)Tout); break;
+    case WBMM_DTYPE_BF16: fold_dwconv_kernel<__nv_bfloat16><<<blocks, 256, 0, s>>>(C, w, kk, (const __nv_bfloat16*)T, (const __nv_bfloat16*)K, scale, (__nv_bfloat16*)Tout); break;
+    default: fold_dwconv_kernel<__half><<<blocks, 256, 0, s>>>(C, w, kk, (const __half*)T, (const __half*)K, scale, (__half*)Tout); break;
+    }
     return cudaGetLastError();
 }
 

@@ -37,7 +37,7 @@ constexpr int kThreadsG = 256;   // generic kernel: 8 warps; warps 0-3 own the 1
 template <int WS, bool BF16>
 __global__ void __launch_bounds__(kThreadsG, 1)
 tc_generic_kernel(Geom g, TcTiles tl, const uint16_t* __restrict__ x, const uint16_t* __restrict__ T,
-                  uint16_t* __restrict__ y, int reverse)
+                  uint16_t* __restrict__ y, int reverse, const uint16_t* __restrict__ Mfull, const uint16_t* __restrict__ bias)
 {
     using Cf = WinCfg<WS>;
     extern __shared__ __align__(1024) uint8_t smem[];
@@ -81,7 +81,9 @@ tc_generic_kernel(Geom g, TcTiles tl, const uint16_t* __restrict__ x, const uint
         const int np_eff = min(tl.NP, g.B - b0);
 
         if (c != cur_c) {   // (the previous tile's MMAs have completed: every thread waited on mma_bar)
-            build_weight<WS>(T + (long long)c * Cf::NB, reverse != 0, Ts, Wc, tid, kThreadsG);
+            // cached-M mode: the channel's matrix is given (reverse = apply its transpose); else Eq. 6-8 from the table
+            if (Mfull) load_weight<WS>(Mfull + (long long)c * Cf::N * Cf::N, reverse != 0, Wc, tid, kThreadsG);
+            else build_weight<WS>(T + (long long)c * Cf::NB, reverse != 0, Ts, Wc, tid, kThreadsG);
             cur_c = c;
         }
         // frame <- x (padded + shifted coordinates)
@@ -121,7 +123,9 @@ tc_generic_kernel(Geom g, TcTiles tl, const uint16_t* __restrict__ x, const uint
         phase ^= 1;
         ptx::tc_fence_after_sync();
         if (warp < 4) {
-            tmem_to_window<WS, BF16>(win, valid, rowB, tmem_d + ((uint32_t)(warp * 32) << 16));
+            float bc = 0.f;
+            if (bias) bc = BF16 ? __uint_as_float((uint32_t)bias[c] << 16) : __half2float(__ushort_as_half(bias[c]));
+            tmem_to_window<WS, BF16>(win, valid, rowB, tmem_d + ((uint32_t)(warp * 32) << 16), bc);
             ptx::tc_fence_before_sync();
         }
         __syncthreads();
@@ -748,7 +752,7 @@ size_t generic_smem(const TcTiles& tl)
 
 template <int WS, bool BF16>
 cudaError_t launch_generic(const Geom& g, const TcTiles& tl, const void* x, const void* T, void* y, bool reverse,
-                           cudaStream_t s)
+                           cudaStream_t s, const void* Mfull = nullptr, const void* bias = nullptr)
 {
     auto k = tc_generic_kernel<WS, BF16>;
     const size_t smem = generic_smem<WS>(tl);
@@ -756,7 +760,8 @@ cudaError_t launch_generic(const Geom& g, const TcTiles& tl, const void* x, cons
     cudaError_t e = ensure_dynamic_smem(reinterpret_cast<const void*>(k), smem, &smem_state);
     if (e != cudaSuccess) return e;
     const int grid = (int)(tl.ntiles < num_sms() ? tl.ntiles : num_sms());
-    k<<<grid, kThreadsG, smem, s>>>(g, tl, (const uint16_t*)x, (const uint16_t*)T, (uint16_t*)y, reverse ? 1 : 0);
+    k<<<grid, kThreadsG, smem, s>>>(g, tl, (const uint16_t*)x, (const uint16_t*)T, (uint16_t*)y, reverse ? 1 : 0,
+                                    (const uint16_t*)Mfull, (const uint16_t*)bias);
     return cudaGetLastError();
 }
 
@@ -923,6 +928,23 @@ cudaError_t tc_forward(const Geom& g, int dtype, const void* x, const void* T, c
                   : launch_generic<7, false>(g, tl, x, T, y, reverse, stream);
     return bf ? launch_generic<14, true>(g, tl, x, T, y, reverse, stream)
               : launch_generic<14, false>(g, tl, x, T, y, reverse, stream);
+}
+
+// Cached-M mode (WBMM-C): the per-channel matrices are given, nothing is built from a table.
+cudaError_t tc_forward_matrix(const Geom& g, int dtype, const void* x, const void* M, const void* bias, void* y,
+                              bool transpose, cudaStream_t stream, int* launches, int* path)
+{
+    TcTiles tl;
+    if (!tc_tiles(g, &tl)) return cudaErrorNotSupported;
+    if (tl.ntiles == 0) return cudaSuccess;
+    *launches += 1;
+    *path = WBMM_PATH_TC_GATHER;
+    const bool bf = dtype == WBMM_DTYPE_BF16;
+    if (g.w == 7)
+        return bf ? launch_generic<7, true>(g, tl, x, nullptr, y, transpose, stream, M, bias)
+                  : launch_generic<7, false>(g, tl, x, nullptr, y, transpose, stream, M, bias);
+    return bf ? launch_generic<14, true>(g, tl, x, nullptr, y, transpose, stream, M, bias)
+              : launch_generic<14, false>(g, tl, x, nullptr, y, transpose, stream, M, bias);
 }
 
 void tc_release() {}

@@ -28,6 +28,10 @@ bool tc_forward_supported(const Geom& g, int dtype, const void* x, const void* y
 cudaError_t tc_forward(const Geom& g, int dtype, const void* x, const void* T, const void* Tl, void* y, bool reverse,
                        cudaStream_t stream, int* launches, int* path);
 bool tc_hier_supported(const Geom& g, int dtype, const void* x, const void* y);
+// Cached-M forward through the gather kernel, wherever tc_forward_supported holds:
+// M [C][N][N] and bias [C] (nullable) in the activation dtype; transpose applies M_c^T.
+cudaError_t tc_forward_matrix(const Geom& g, int dtype, const void* x, const void* M, const void* bias, void* y,
+                              bool transpose, cudaStream_t stream, int* launches, int* path);
 // True when the pipelined bulk kernel (not the gather fallback) serves this NCHW problem.
 bool tc_bulk_supported(const Geom& g, int dtype, const void* x, const void* y);
 

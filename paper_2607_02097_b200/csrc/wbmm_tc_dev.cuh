@@ -143,7 +143,7 @@ __device__ __forceinline__ void window_to_tmem(const uint8_t* win, bool valid, i
 
 // TMEM D -> rounded 16-bit values in the window's frame position (32 columns per wait).
 template <int WS, bool BF16>
-__device__ __forceinline__ void tmem_to_window(uint8_t* win, bool valid, int rowB, uint32_t taddr)
+__device__ __forceinline__ void tmem_to_window(uint8_t* win, bool valid, int rowB, uint32_t taddr, float bias = 0.f)
 {
     using Cf = WinCfg<WS>;
     constexpr int NCH = (Cf::NW + 7) / 8;     // 16-column chunks that hold real outputs
@@ -158,9 +158,33 @@ __device__ __forceinline__ void tmem_to_window(uint8_t* win, bool valid, int row
             for (int e = 0; e < 16; ++e) {
                 const int wi = ch * 8 + e;
                 if (wi < Cf::NW && (e < 8 || ch + 1 < NCH))
-                    store_word<WS>(win, rowB, wi, pack2<BF16>(v[2 * e], v[2 * e + 1]));
+                    store_word<WS>(win, rowB, wi, pack2<BF16>(__float_as_uint(__uint_as_float(v[2 * e]) + bias),
+                                                               __float_as_uint(__uint_as_float(v[2 * e + 1]) + bias)));
             }
         }
+    }
+}
+
+// W_c from a GIVEN matrix M_c[N][N] (cached-M mode) into the K-major core-matrix layout of
+// build_weight: value (i, j) at byte (j/8)*LBO + i*16 + (j%8)*2; transpose: W_c = M_c^T.  Rows / columns >= N zero.
+template <int WS>
+__device__ __forceinline__ void load_weight(const uint16_t* __restrict__ Mc, bool transpose, uint8_t* Wc, int tid, int nthreads)
+{
+    using Cf = WinCfg<WS>;
+    constexpr int NCHUNK = (Cf::K_PAD / 8) * Cf::N_PAD;
+    for (int id = tid; id < NCHUNK; id += nthreads) {
+        const int kc = id / Cf::N_PAD, i = id % Cf::N_PAD;
+        uint32_t pk[4] = {0u, 0u, 0u, 0u};
+        if (i < Cf::N) {
+#pragma unroll
+            for (int e = 0; e < 8; ++e) {
+                const int j = kc * 8 + e;
+                uint32_t v = 0;
+                if (j < Cf::N) v = transpose ? Mc[j * Cf::N + i] : Mc[i * Cf::N + j];
+                pk[e >> 1] |= v << ((e & 1) * 16);
+            }
+        }
+        *reinterpret_cast<uint4*>(Wc + kc * Cf::LBO + i * 16) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
     }
 }
 

@@ -268,6 +268,81 @@ def test_hier_backward_local_bins_exact_on_integers(wb, oracle):
     assert np.array_equal(widen(dTg), rg) and np.array_equal(widen(dTl), rl)
 
 
+# ------------------------------------------------------------------ cached-M mode and multi-kernel fusion (NEXT-2)
+@pytest.mark.parametrize("case", [
+    si.Case("m_w14", 6, 5, 56, 56, 14, seed=61),
+    si.Case("m_w7_shift", 9, 7, 28, 42, 7, shift=(3, 4), seed=62),
+    si.Case("m_ragged_nhwc", 3, 8, 30, 45, 14, shift=(7, 2), layout=NHWC, seed=63),
+    si.Case("m_f16", 4, 3, 21, 21, 7, dtype="f16", seed=64),
+], ids=lambda c: c.name)
+def test_cached_matrix_mode_equals_the_table_mode(wb, oracle, case):
+    """WBMM-C and WBMM-NC "produce identical outputs": forward and dX through
+    wbmm_forward_matrix with M = materialize(T) against the oracle, and against the table path of the
+    library (another kernel, so another fp32 summation order: equal to within one 16-bit ulp)."""
+    d = si.make(case, device="cuda")
+    M = wb.wbmm_materialize_weight(d["T"], case.w)
+    for transpose in (False, True):
+        y = wb.wbmm_forward_matrix(d["x"], M, case.w, case.shift, case.layout, transpose=transpose)
+        assert wb.wbmm_last_path() == wb.PATH_TC_GATHER
+        if transpose:
+            ref, _ = wb.wbmm_backward(None, d["T"], d["x"], case.w, case.shift, case.layout, need_dT=False)
+            rdx, _ = oracle.backward(widen(d["x"]), widen(d["T"]), widen(d["x"]), case.w, case.shift, case.layout, need_dT=False)
+            assert max_err_over_tol(y, rdx, TOL[case.dtype]) <= 1.0
+        else:
+            ref = wb.wbmm_forward(d["x"], d["T"], case.w, case.shift, case.layout)
+            ry = oracle.forward(widen(d["x"]), widen(d["T"]), case.w, case.shift, case.layout)
+            assert max_err_over_tol(y, ry, TOL[case.dtype]) <= 1.0
+        ulp = 2.0 ** -7 if case.dtype == "bf16" else 2.0 ** -10
+        diff = (y.float() - ref.float()).abs()
+        assert bool((diff <= ulp * ref.float().abs() + 1e-6).all())
+
+
+def test_cached_matrix_mode_arbitrary_matrix_and_bias(wb, oracle):
+    """A matrix that is NOT table-generated, plus a bias, against the oracle's Algorithm 1."""
+    case = si.Case("m_any", 5, 6, 30, 44, 14, shift=(2, 9), seed=65)
+    d = si.make(case, device="cuda")
+    g = torch.Generator().manual_seed(66)
+    M = (torch.randn((case.C, 196, 196), generator=g) * 0.05).to(torch.bfloat16).cuda()
+    bias = torch.randn((case.C,), generator=g).to(torch.bfloat16).cuda()
+    for transpose in (False, True):
+        y = wb.wbmm_forward_matrix(d["x"], M, case.w, case.shift, case.layout, bias, transpose)
+        ref = oracle.apply_matrix(widen(d["x"]), widen(M), case.w, case.shift, case.layout, transpose, widen(bias))
+        assert max_err_over_tol(y, ref, TOL["bf16"]) <= 1.0
+
+
+@pytest.mark.parametrize("dtype", ["bf16", "f32"])
+def test_multi_kernel_fusion_on_a_one_window_map(wb, oracle, dtype):
+    """Section 3.7 on a 7 x 7 map: Y = WBMM(X) + BN1(DW5(X)) + BN2(DW3(X)) as ONE operator -- tables folded on
+    the device (wbmm_fold_dwconv), then the cached-M forward with the BatchNorm shifts as bias (16-bit) or the
+    table forward (fp32, bias added by the caller).  Reference: the oracle's fold + Algorithm 1, itself pinned
+    against a library conv2d."""
+    w, B, C = 7, 33, 24
+    td = {"bf16": torch.bfloat16, "f32": torch.float32}[dtype]
+    g = torch.Generator().manual_seed(67)
+    x = torch.randn((B, C, w, w), generator=g).to(td).cuda()
+    T = (torch.randn((C, 169), generator=g) * 0.02).to(td).cuda()
+    K5 = (torch.randn((C, 5, 5), generator=g) * 0.2).to(td).cuda()
+    K3 = (torch.randn((C, 3, 3), generator=g) * 0.3).to(td).cuda()
+    s1, s2 = torch.rand((C,), generator=g).cuda() + 0.5, torch.rand((C,), generator=g).cuda() + 0.5
+    bias = torch.randn((C,), generator=g).to(td).cuda()
+    Tf = wb.wbmm_fold_dwconv(wb.wbmm_fold_dwconv(T, K5, w, s1), K3, w, s2)
+    rTf = oracle.fold_dwconv(oracle.fold_dwconv(widen(T), widen(K5), w, widen(s1)), widen(K3), w, widen(s2))
+    tol = TOL[dtype]
+    assert max_err_over_tol(Tf, rTf, tol) <= 1.0
+    # entries the conv kernels do not touch are copied bit for bit
+    far = torch.ones(169, dtype=torch.bool)
+    for i in range(-2, 3):
+        for j in range(-2, 3):
+            far[(6 - i) * 13 + (6 - j)] = False
+    assert torch.equal(Tf[:, far], T[:, far])
+    if dtype == "bf16":
+        y = wb.wbmm_forward_matrix(x, wb.wbmm_materialize_weight(Tf, w), w, bias=bias)
+    else:
+        y = wb.wbmm_forward(x, Tf, w) + bias.view(1, C, 1, 1)
+    ref = oracle.apply_matrix(widen(x), oracle.weight_matrix(widen(Tf), w), w, bias=widen(bias))
+    assert max_err_over_tol(y, ref, tol) <= 1.0
+
+
 def test_hier_unsupported_shapes_fail_loudly(wb):
     x = torch.zeros((2, 4, 14, 14), dtype=torch.bfloat16, device="cuda")
     with pytest.raises(wb.WbmmError):       # w = 7 has no hierarchical tensor-core path
