@@ -364,6 +364,39 @@ int dt_mode(const Geom& g, const TcTiles& tl, const void* x, const void* dy)
     return (tl.nstrips == 1 && g.W % 2 == 0 && g.Wp % 2 == 0) ? 2 : 0;
 }
 
+// Tiling of the table-gradient kernel.  Its ring holds x AND dy and shares the SM with the 106 KB operand stage,
+// so whole frame images of large maps (112 x 112: 25 KB) do not fit 2 * NP + 1 times.  Window-multiple, unshifted
+// maps can be cut into strips of window rows instead (the aligned form reads any whole rows): more images per
+// tile, fewer rows per image, frame images of ~6 KB as on the 56 x 56 maps.
+template <int WS>
+bool dt_tiles(const Geom& g, TcTiles* t)
+{
+    if (!tc_tiles(g, t)) return false;
+    const bool plain = g.sh == 0 && g.sw == 0 && g.H == g.Hp && g.W == g.Wp;
+    if (!plain || t->nstrips != 1 || dt_slots<WS>(*t) >= 2 * t->NP + 1) return true;
+    for (int nsy = g.nwh / 2; nsy >= 1; --nsy) {
+        if (g.nwh % nsy != 0 || (nsy * g.w * g.W * 2) % 16 != 0) continue;
+        TcTiles c = *t;
+        c.NSY = nsy;
+        c.NP = 128 / (nsy * g.nww);
+        if (c.NP > g.B) c.NP = g.B;
+        if (c.NP < 1) continue;
+        c.nstrips = g.nwh / nsy;
+        c.ngb = (g.B + c.NP - 1) / c.NP;
+        c.tiles_per_c = c.ngb * c.nstrips;
+        c.frame_rows = nsy * g.w;
+        int s16 = (c.frame_rows * g.Wp * 2 + 15) / 16;
+        if (s16 % 2 == 0) ++s16;
+        c.S = s16 * 16;
+        c.ntiles = (long long)g.C * c.tiles_per_c;
+        if (c.S <= 8192 && dt_slots<WS>(c) >= 2 * c.NP + 1) {
+            *t = c;
+            return true;
+        }
+    }
+    return true;    // nothing fits: dt_mode() rejects the original tiling
+}
+
 template <int WS, bool BF16, bool GEN, bool HIER = false>
 cudaError_t launch_dt(const Geom& g, const TcTiles& tl_in, const void* x, const void* dy, float* dT, cudaStream_t s,
                       float* dTl = nullptr)
@@ -433,7 +466,7 @@ bool tc_grad_table_supported(const Geom& g, int dtype, const void* x, const void
     if (dtype != WBMM_DTYPE_BF16 && dtype != WBMM_DTYPE_F16) return false;
     if (g.w != 7 && g.w != 14) return false;
     TcTiles tl;
-    if (!tc_tiles(g, &tl)) return false;
+    if (!(g.w == 7 ? dt_tiles<7>(g, &tl) : dt_tiles<14>(g, &tl))) return false;
     return (g.w == 7 ? dt_mode<7>(g, tl, x, dy) : dt_mode<14>(g, tl, x, dy)) != 0;
 }
 
@@ -441,7 +474,7 @@ cudaError_t tc_grad_table(const Geom& g, int dtype, const void* x, const void* d
                           int* launches, int* path, float* dTl)
 {
     TcTiles tl;
-    if (!tc_tiles(g, &tl)) return cudaErrorNotSupported;
+    if (!(g.w == 7 ? dt_tiles<7>(g, &tl) : dt_tiles<14>(g, &tl))) return cudaErrorNotSupported;
     if (tl.ntiles == 0) return cudaSuccess;
     const int mode = g.w == 7 ? dt_mode<7>(g, tl, x, dy) : dt_mode<14>(g, tl, x, dy);
     if (mode == 0) return cudaErrorNotSupported;
