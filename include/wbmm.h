@@ -152,6 +152,24 @@ WBMM_API int wbmm_hier_backward(const wbmm_desc_t *desc, const void *x, const vo
 WBMM_API int wbmm_materialize_weight(const wbmm_desc_t *desc, const void *T, void *Wout, void *cuda_stream);
 
 /*
+ * Forward with the neighbouring elementwise steps fused (Eq. 1's beta_c,
+ * PAPER.md:848-852 identity shortcut):
+ *     y_win = W_c * x_win + identity * x_win + bias_c          (W_c from the table, Eq. 6-8)
+ *   bias     [in, nullable] [C] elements of desc->dtype (finite).  Costs nothing: it rides the contraction as one
+ *            more K index -- a column of ones in the padding of the A operand against a weight row holding bias_c --
+ *            so it is added in the fp32 accumulator, before the single rounding.
+ *   identity coefficient of the shortcut, rounded to desc->dtype (1.0 and 2.0 are exact); 0 = none.  Applied by the
+ *            16 x 16 block identity * I of the w = 14 weight library (14 extra N = 16 MMAs per tile), never summed
+ *            into the 16-bit table values.  w = 14 only.
+ *   transpose != 0 applies W_c^T + identity * I (the dX of the fused operator for dy in `x`; pass bias = NULL).
+ * Served by the pipelined tensor-core kernel only (bf16/fp16, w in {7, 14}, NCHW planes 16-byte aligned, or NHWC
+ * through the transposition scratch); otherwise WBMM_STATUS_UNSUPPORTED with nothing launched -- the caller then
+ * uses wbmm_forward and its own elementwise pass.
+ */
+WBMM_API int wbmm_forward_fused(const wbmm_desc_t *desc, const void *x, const void *T, const void *bias, float identity,
+                       void *y, int transpose, void *cuda_stream);
+
+/*
  * Cached-M inference mode, "WBMM-C": Algorithm 1 with GIVEN per-channel matrices,
  *     y_win = M_c * x_win (+ bias_c),
  *   M    [in] [C][N][N] elements of desc->dtype, row i = output position, column j = input position (the

@@ -23,7 +23,7 @@ _DTYPES = {torch.float32: DTYPE_F32, torch.bfloat16: DTYPE_BF16, torch.float16: 
 
 # every symbol include/wbmm.h declares
 EXPORTS = (
-    "wbmm_forward", "wbmm_backward", "wbmm_hier_forward", "wbmm_hier_backward", "wbmm_forward_matrix", "wbmm_fold_dwconv", "wbmm_materialize_weight", "wbmm_forward_host",
+    "wbmm_forward", "wbmm_backward", "wbmm_hier_forward", "wbmm_hier_backward", "wbmm_forward_matrix", "wbmm_fold_dwconv", "wbmm_forward_fused", "wbmm_materialize_weight", "wbmm_forward_host",
     "wbmm_backward_host", "wbmm_release", "wbmm_last_path", "wbmm_launch_count",
     "wbmm_status_string", "wbmm_path_string", "wbmm_last_error_string", "wbmm_version",
 )
@@ -64,6 +64,8 @@ def lib() -> ctypes.CDLL:
     L.wbmm_forward_matrix.restype = i
     L.wbmm_fold_dwconv.argtypes = [dp, vp, vp, i, vp, vp, vp]
     L.wbmm_fold_dwconv.restype = i
+    L.wbmm_forward_fused.argtypes = [dp, vp, vp, vp, ctypes.c_float, vp, i, vp]
+    L.wbmm_forward_fused.restype = i
     L.wbmm_forward_host.argtypes = [dp, vp, vp, vp]
     L.wbmm_backward_host.argtypes = [dp, vp, vp, vp, vp, vp]
     for n in ("wbmm_forward", "wbmm_backward", "wbmm_materialize_weight", "wbmm_forward_host",
@@ -197,6 +199,22 @@ def wbmm_materialize_weight(T: torch.Tensor, w: int) -> torch.Tensor:
     with torch.cuda.device(T.device):
         _check(lib().wbmm_materialize_weight(ctypes.byref(d), _dev(T, "T"), _dev(W, "W"), _stream(T)))
     return W
+
+
+def wbmm_forward_fused(x: torch.Tensor, T: torch.Tensor, w: int, shift=(0, 0), layout: int = NCHW,
+                       bias: Optional[torch.Tensor] = None, identity: float = 0.0, transpose: bool = False,
+                       out: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """y = WBMM(x; T) + identity * x + bias_c in one kernel (include/wbmm.h: wbmm_forward_fused)."""
+    d = make_desc(x, w, shift, layout, 0)
+    if T.dtype != x.dtype or tuple(T.shape) != (d.C, (2 * w - 1) ** 2):
+        raise ValueError("T must be [C,(2w-1)^2] in the dtype of x")
+    if bias is not None and (bias.dtype != x.dtype or tuple(bias.shape) != (d.C,)):
+        raise ValueError("bias must be [C] in the dtype of x")
+    y = torch.empty_like(x) if out is None else out
+    with torch.cuda.device(x.device):
+        _check(lib().wbmm_forward_fused(ctypes.byref(d), _dev(x, "x"), _dev(T, "T"), _dev(bias, "bias"),
+                                        ctypes.c_float(identity), _dev(y, "y"), 1 if transpose else 0, _stream(x)))
+    return y
 
 
 def wbmm_forward_matrix(x: torch.Tensor, M: torch.Tensor, w: int, shift=(0, 0), layout: int = NCHW,

@@ -304,6 +304,59 @@ int wbmm_hier_backward(const wbmm_desc_t* desc, const void* x, const void* Tg, c
     return WBMM_STATUS_OK;
 }
 
+int wbmm_forward_fused(const wbmm_desc_t* desc, const void* x, const void* T, const void* bias, float identity,
+                       void* y, int transpose, void* cuda_stream)
+{
+    int st = validate(desc);
+    if (st != WBMM_STATUS_OK) return st;
+    if (desc->B == 0 || desc->C == 0) return WBMM_STATUS_OK;
+    if (!x || !T || !y || x == y) return WBMM_STATUS_INVALID_ARGUMENT;
+    if (!(identity == identity) || identity - identity != 0.f) return WBMM_STATUS_INVALID_ARGUMENT;   // NaN / inf
+    const size_t es = elem_size(desc->dtype);
+    if (!aligned(x, es) || !aligned(T, es) || !aligned(y, es) || (bias && !aligned(bias, es))) return WBMM_STATUS_MISALIGNED;
+    if (device_state() < 0) return WBMM_STATUS_NO_DEVICE;
+    if (desc->dtype != WBMM_DTYPE_BF16 && desc->dtype != WBMM_DTYPE_F16) return WBMM_STATUS_UNSUPPORTED;
+    uint32_t ident_bits = 0;
+    if (identity != 0.f) {
+        if (desc->w != 14) return WBMM_STATUS_UNSUPPORTED;            // the identity block exists in the w = 14 library only
+        if (desc->dtype == WBMM_DTYPE_BF16) { __nv_bfloat16 h = __float2bfloat16_rn(identity); memcpy(&ident_bits, &h, 2); }
+        else { __half h = __float2half_rn(identity); memcpy(&ident_bits, &h, 2); }
+    }
+    wbmm::Geom g = wbmm::make_geom(*desc);
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    int launches = 0, path = WBMM_PATH_NONE;
+    cudaError_t e;
+    if (g.layout == WBMM_LAYOUT_NHWC) {
+        // the transposition route of wbmm_forward around the same fused kernel
+        wbmm::Geom gn = g;
+        gn.layout = WBMM_LAYOUT_NCHW;
+        void* const aligned16 = reinterpret_cast<void*>(256);
+        if (!nhwc_scratch_candidate(desc, g) || !wbmm::tc_bulk_supported(gn, desc->dtype, aligned16, aligned16) ||
+            !wbmm::transpose16_supported((long long)g.H * g.W, g.C, x, y))
+            return WBMM_STATUS_UNSUPPORTED;
+        const size_t nbytes = (size_t)g.B * g.C * g.H * g.W * 2;
+        AsyncScratch xt(stream), yt(stream);
+        if (xt.alloc(nbytes) != cudaSuccess || yt.alloc(nbytes) != cudaSuccess) {
+            cudaGetLastError();
+            return WBMM_STATUS_UNSUPPORTED;
+        }
+        e = wbmm::transpose16(x, xt.p, g.B, g.H * g.W, g.C, stream, &launches);
+        if (e == cudaSuccess)
+            e = wbmm::tc_forward(gn, desc->dtype, xt.p, T, nullptr, yt.p, transpose != 0, stream, &launches, &path, bias, ident_bits);
+        if (e == cudaSuccess) e = wbmm::transpose16(yt.p, y, g.B, g.C, g.H * g.W, stream, &launches);
+        g_launches += launches;
+        if (e != cudaSuccess) return set_cuda_error(e, "fused forward, NHWC via NCHW scratch");
+        t_last_path = WBMM_PATH_TC_TRANSPOSED;
+        return WBMM_STATUS_OK;
+    }
+    if (!wbmm::tc_bulk_supported(g, desc->dtype, x, y)) return WBMM_STATUS_UNSUPPORTED;
+    e = wbmm::tc_forward(g, desc->dtype, x, T, nullptr, y, transpose != 0, stream, &launches, &path, bias, ident_bits);
+    g_launches += launches;
+    if (e != cudaSuccess) return set_cuda_error(e, "tc_forward (fused)");
+    t_last_path = path;
+    return WBMM_STATUS_OK;
+}
+
 int wbmm_forward_matrix(const wbmm_desc_t* desc, const void* x, const void* M, const void* bias, void* y,
                         int transpose, void* cuda_stream)
 {

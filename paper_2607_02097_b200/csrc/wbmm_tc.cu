@@ -176,7 +176,8 @@ template <int WS, bool BF16, bool GEN>
 __global__ void __launch_bounds__(kThreadsB, 1)
 tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const uint16_t* __restrict__ x, const uint16_t* __restrict__ T,
                const uint16_t* __restrict__ Tl, uint16_t* __restrict__ y, int reverse, int box, int sbox,
-               const __grid_constant__ CUtensorMap mx, const __grid_constant__ CUtensorMap my)
+               const __grid_constant__ CUtensorMap mx, const __grid_constant__ CUtensorMap my,
+               const uint16_t* __restrict__ bias, uint32_t ident_bits)
 {
     using Cf = WinCfg<WS>;
     using Sm = BulkSmem<WS>;
@@ -187,6 +188,11 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
     uint16_t* tab = reinterpret_cast<uint16_t*>(smem + Bc::WC_BYTES + Bc::HIER_BYTES);
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + Bc::WC_BYTES + Bc::HIER_BYTES + Sm::TAB_BYTES);
     const bool is_hier = Bc::TOEP && Tl != nullptr;
+    // Epilogue fusions without an epilogue: y = W_c x + ident * x + bias_c.  The identity term is the 16 x 16 block
+    // ident * I applied by 14 extra N = 16 MMAs (w = 14; 2 * I for the hierarchical operator); the bias is one more
+    // K index: a column of ones in the A operand's padding against a weight row that holds bias_c.
+    const bool use_I = Bc::TOEP && (is_hier || ident_bits != 0u);
+    const uint32_t pad0 = bias ? (BF16 ? 0x3F80u : 0x3C00u) : 0u;     // 1.0
     uint8_t* ring = smem + Sm::FIXED;                       // input ring: nslot frame-image slots
     uint8_t* outb = ring + (size_t)nslot * tl.S;            // output ring: nout group buffers of og.images frame images
     __shared__ uint32_t tmem_base_s;
@@ -339,7 +345,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                         ptx::mma_ts(tmem_d + Hs::col0(h), tmem_a + ks * 8, bdesc, idesc, ks > 0 ? 1u : 0u);
                     }
                     if constexpr (Bc::TOEP) {
-                        if (is_hier) {      // + 2 x: output row ri takes input row ri through the 2*I block
+                        if (use_I) {        // + ident * x: output row ri takes input row ri through the ident*I block
                             const uint32_t idesc_i = ptx::idesc_f16(BF16 ? 1 : 0, 128, 16);
                             const uint64_t idn = ptx::smem_desc_kmajor_noswz(wc_addr + Bc::WC_BYTES + Bc::LIBA_BYTES, Bc::LBO_I, 128);
 #pragma unroll
@@ -375,15 +381,16 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                 if (rt == 0) TRACE(12, lt);
                 if constexpr (WS == 14) {
                     if (!tabv_ready) table_to_regs14(Tc, reverse != 0, rt, tabv);
-                    build_lib14(tabv, tab, tab + Sm::TAB_ONE / 2, Wc, rt);
+                    build_lib14(tabv, tab, tab + Sm::TAB_ONE / 2, Wc, rt, bias ? (uint32_t)bias[c] : 0u);
                     tabv_ready = false;
+                    // libI = ident * I (hierarchical: the two identity shortcuts, 2.0 = 0x4000 in bf16 and in fp16)
+                    if (use_I && rt < 14)
+                        *reinterpret_cast<uint16_t*>(hier + Bc::LIBA_BYTES + (rt >> 3) * Bc::LBO_I + rt * 16 + (rt & 7) * 2) =
+                            (uint16_t)(is_hier ? 0x4000u : ident_bits);
                     if (is_hier) {
                         uint16_t* FL = reinterpret_cast<uint16_t*>(hier + Bc::LIBA_BYTES + Bc::LIBI_BYTES);
                         const uint16_t* Tlc = Tl + (long long)c * 169;
                         for (int qq = rt; qq < 169; qq += 128) FL[qq] = Tlc[reverse ? qq : 168 - qq];
-                        // libI = 2*I (the two identity shortcuts): 2.0 is 0x4000 in bf16 and in fp16
-                        if (rt < 14)
-                            *reinterpret_cast<uint16_t*>(hier + Bc::LIBA_BYTES + (rt >> 3) * Bc::LBO_I + rt * 16 + (rt & 7) * 2) = 0x4000;
                         ptx::named_bar_sync(2, 128);          // the global library and FL are complete
                         build_lib14_local<BF16>(Wc, FL, hier, rt);
                     }
@@ -401,6 +408,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                             for (int e = 0; e < 8; ++e) {
                                 uint32_t v = 0;
                                 if (j < Cf::N) v = tab[(ri - rj + WS - 1) * Cf::TW + (ci - cj + WS - 1)];
+                                else if (j == Cf::N + 1 && bias) v = bias[c];      // K index of the column of ones
                                 pk[e >> 1] |= v << ((e & 1) * 16);
                                 ++j;
                                 if (++cj == WS) { cj = 0; ++rj; }
@@ -439,15 +447,15 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
             {
                 const uint32_t ta = tmem + buf * A_STRIDE + ((uint32_t)(q * 32) << 16);
                 if constexpr (GEN && WS % 2 == 0) {      // even w: every window starts on the parity of the column shift
-                    if (g.sw & 1) window_to_tmem_gen<WS, 1>(ring + (size_t)slot * tl.S, ga, valid, ragged, ta);
-                    else window_to_tmem_gen<WS, 0>(ring + (size_t)slot * tl.S, ga, valid, ragged, ta);
+                    if (g.sw & 1) window_to_tmem_gen<WS, 1>(ring + (size_t)slot * tl.S, ga, valid, ragged, ta, pad0);
+                    else window_to_tmem_gen<WS, 0>(ring + (size_t)slot * tl.S, ga, valid, ragged, ta, pad0);
                 } else {
-                    window_to_tmem_gen<WS>(ring + (size_t)slot * tl.S, ga, valid, GEN && ragged, ta);
+                    window_to_tmem_gen<WS>(ring + (size_t)slot * tl.S, ga, valid, GEN && ragged, ta, pad0);
                 }
             }
             else
                 window_to_tmem_bulk<WS>(ring + (size_t)slot * tl.S + win_off, valid, rowB,
-                                        tmem + buf * A_STRIDE + ((uint32_t)(q * 32) << 16));
+                                        tmem + buf * A_STRIDE + ((uint32_t)(q * 32) << 16), pad0);
             if (part) ptx::mbar_arrive(EMPTY(bslot));   // every window of this image is in TMEM
             // W_c of a new channel is rebuilt AFTER this tile's windows are in TMEM, so the copy above
             // overlaps the last MMA of the previous channel.
@@ -690,7 +698,7 @@ int bulk_box_mode(const Geom& g, const TcTiles& tl, int dtype, const void* x, co
 
 template <int WS, bool BF16, bool GEN>
 cudaError_t launch_bulk(const Geom& g, const TcTiles& tl_in, const void* x, const void* T, const void* Tl, void* y,
-                        bool reverse, cudaStream_t s)
+                        bool reverse, cudaStream_t s, const void* bias, uint32_t ident_bits)
 {
     auto k = tc_bulk_kernel<WS, BF16, GEN>;
     int nslot = 0, nout = 0;
@@ -741,7 +749,7 @@ cudaError_t launch_bulk(const Geom& g, const TcTiles& tl_in, const void* x, cons
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     return cudaLaunchKernelEx(&cfg, k, g, tl, part, nslot, nout, (const uint16_t*)x, (const uint16_t*)T, (const uint16_t*)Tl,
-                              (uint16_t*)y, reverse ? 1 : 0, box, sbox, mx, my);
+                              (uint16_t*)y, reverse ? 1 : 0, box, sbox, mx, my, (const uint16_t*)bias, ident_bits);
 }
 
 template <int WS>
@@ -899,7 +907,7 @@ bool tc_hier_supported(const Geom& g, int dtype, const void* x, const void* y)
 }
 
 cudaError_t tc_forward(const Geom& g, int dtype, const void* x, const void* T, const void* Tl, void* y, bool reverse,
-                       cudaStream_t stream, int* launches, int* path)
+                       cudaStream_t stream, int* launches, int* path, const void* bias, uint32_t ident_bits)
 {
     TcTiles tl;
     if (!tc_tiles(g, &tl)) return cudaErrorNotSupported;
@@ -911,17 +919,17 @@ cudaError_t tc_forward(const Geom& g, int dtype, const void* x, const void* T, c
         *path = WBMM_PATH_TC_TMA;
         const int sel = (g.w == 7 ? 0 : 4) + (bf ? 2 : 0) + (mode == 2 ? 1 : 0);
         switch (sel) {
-        case 0: return launch_bulk<7, false, false>(g, tl, x, T, Tl, y, reverse, stream);
-        case 1: return launch_bulk<7, false, true>(g, tl, x, T, Tl, y, reverse, stream);
-        case 2: return launch_bulk<7, true, false>(g, tl, x, T, Tl, y, reverse, stream);
-        case 3: return launch_bulk<7, true, true>(g, tl, x, T, Tl, y, reverse, stream);
-        case 4: return launch_bulk<14, false, false>(g, tl, x, T, Tl, y, reverse, stream);
-        case 5: return launch_bulk<14, false, true>(g, tl, x, T, Tl, y, reverse, stream);
-        case 6: return launch_bulk<14, true, false>(g, tl, x, T, Tl, y, reverse, stream);
-        default: return launch_bulk<14, true, true>(g, tl, x, T, Tl, y, reverse, stream);
+        case 0: return launch_bulk<7, false, false>(g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
+        case 1: return launch_bulk<7, false, true>(g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
+        case 2: return launch_bulk<7, true, false>(g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
+        case 3: return launch_bulk<7, true, true>(g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
+        case 4: return launch_bulk<14, false, false>(g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
+        case 5: return launch_bulk<14, false, true>(g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
+        case 6: return launch_bulk<14, true, false>(g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
+        default: return launch_bulk<14, true, true>(g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
         }
     }
-    if (Tl) return cudaErrorNotSupported;      // the hierarchical operator exists in the bulk kernel only
+    if (Tl || bias || ident_bits) return cudaErrorNotSupported;      // hierarchical / fused variants exist in the bulk kernel only
     *path = WBMM_PATH_TC_GATHER;
     if (g.w == 7)
         return bf ? launch_generic<7, true>(g, tl, x, T, y, reverse, stream)

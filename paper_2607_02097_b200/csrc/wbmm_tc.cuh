@@ -25,8 +25,10 @@ bool tc_tiles(const Geom& g, TcTiles* t);
 // True when a tcgen05 forward kernel can serve this problem.
 bool tc_forward_supported(const Geom& g, int dtype, const void* x, const void* y);
 // Tl != nullptr: the hierarchical operator (global table T, local table Tl; w = 14, bulk kernel only).
+// bias [C] (activation dtype, nullable) and ident_bits (16-bit pattern of the identity coefficient, 0 = none;
+// w = 14 only) are fused into the pipelined kernel; with either set the call fails where that kernel cannot serve.
 cudaError_t tc_forward(const Geom& g, int dtype, const void* x, const void* T, const void* Tl, void* y, bool reverse,
-                       cudaStream_t stream, int* launches, int* path);
+                       cudaStream_t stream, int* launches, int* path, const void* bias = nullptr, uint32_t ident_bits = 0);
 bool tc_hier_supported(const Geom& g, int dtype, const void* x, const void* y);
 // Cached-M forward through the gather kernel, wherever tc_forward_supported holds:
 // M [C][N][N] and bias [C] (nullable) in the activation dtype; transpose applies M_c^T.

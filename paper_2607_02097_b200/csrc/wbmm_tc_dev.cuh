@@ -419,8 +419,10 @@ __device__ __forceinline__ void window_to_regs_gen(const uint8_t* img, const Gen
 
 // Linear packed window words v[0 .. NW) -> one A buffer of the bulk kernel (tcgen05.st, all 32
 // lanes).  w = 14: every window row is padded to 8 words, the last one zero (BulkCfg<14>).
+// pad0: the first padding word of the window's K range -- (row 0, columns 14-15) at w = 14, elements N+1, N+2
+// otherwise; 1.0 in its low half turns that K index into a column of ones (the fused bias, see build_lib14).
 template <int WS>
-__device__ __forceinline__ void packed_window_to_tmem(const uint32_t* v, uint32_t taddr)
+__device__ __forceinline__ void packed_window_to_tmem(const uint32_t* v, uint32_t taddr, uint32_t pad0 = 0u)
 {
     using Bc = BulkCfg<WS>;
     using Cf = WinCfg<WS>;
@@ -430,11 +432,11 @@ __device__ __forceinline__ void packed_window_to_tmem(const uint32_t* v, uint32_
 #pragma unroll
         for (int r = 0; r < WS; ++r) {
 #pragma unroll
-            for (int k = 0; k < 8; ++k) u[r * 8 + k] = k < 7 ? v[r * 7 + k] : 0u;
+            for (int k = 0; k < 8; ++k) u[r * 8 + k] = k < 7 ? v[r * 7 + k] : (r == 0 ? pad0 : 0u);
         }
     } else {
 #pragma unroll
-        for (int k = 0; k < NV; ++k) u[k] = k < Cf::NW ? v[k] : 0u;
+        for (int k = 0; k < NV; ++k) u[k] = k < Cf::NW ? v[k] : (k == Cf::NW ? pad0 : 0u);
     }
 #pragma unroll
     for (int ch = 0; ch < Bc::A_COLS / 16; ++ch) ptx::tmem_st16(taddr + ch * 16, u + ch * 16);
@@ -443,21 +445,21 @@ __device__ __forceinline__ void packed_window_to_tmem(const uint32_t* v, uint32_
 }
 
 template <int WS>
-__device__ __forceinline__ void window_to_tmem_bulk(const uint8_t* win, bool valid, int rowB, uint32_t taddr)
+__device__ __forceinline__ void window_to_tmem_bulk(const uint8_t* win, bool valid, int rowB, uint32_t taddr, uint32_t pad0 = 0u)
 {
     uint32_t v[WinCfg<WS>::NW];
     window_to_regs<WS>(win, valid, rowB, v);
-    packed_window_to_tmem<WS>(v, taddr);
+    packed_window_to_tmem<WS>(v, taddr, pad0);
 }
 
 template <int WS, int PAR = -1>
 __device__ __forceinline__ void window_to_tmem_gen(const uint8_t* img, const GenAddr<WS>& a, bool valid, bool ragged,
-                                                   uint32_t taddr)
+                                                   uint32_t taddr, uint32_t pad0 = 0u)
 {
     uint32_t v[WinCfg<WS>::NW];
     if (ragged) window_to_regs_gen<WS, true, PAR>(img, a, valid, v);
     else window_to_regs_gen<WS, false, PAR>(img, a, valid, v);
-    packed_window_to_tmem<WS>(v, taddr);
+    packed_window_to_tmem<WS>(v, taddr, pad0);
 }
 
 // Packed words [W0, W1) of a window (pk[0] = word W0; the range covers whole window rows, or the
@@ -555,7 +557,7 @@ __device__ __forceinline__ void table_to_regs14(const uint16_t* __restrict__ Tc,
 // Block-Toeplitz library for w = 14 (BulkCfg<14>) from the two staged copies of the reversed table
 // (see build_weight14): chunk (d, ci, kc) = Z[d-13][ci][8kc .. 8kc+7] = F[(26-d)*27 + 13-ci + 8kc + e].
 // 128 threads (the repack warps); rows ci = 14, 15 of every block stay zero from the kernel prologue.
-__device__ __forceinline__ void build_lib14(const uint16_t* v, uint16_t* F0, uint16_t* F1, uint8_t* lib, int tid)
+__device__ __forceinline__ void build_lib14(const uint16_t* v, uint16_t* F0, uint16_t* F1, uint8_t* lib, int tid, uint32_t bias_bits = 0u)
 {
     using Cf = WinCfg<14>;
     using Bc = BulkCfg<14>;
@@ -572,7 +574,9 @@ __device__ __forceinline__ void build_lib14(const uint16_t* v, uint16_t* F0, uin
         const int d = id / 28, rem = id - d * 28, ci = rem >> 1, kc = rem & 1;
         const int q0 = (26 - d) * 27 + 13 - ci + 8 * kc, p0 = q0 & 1;
         const uint32_t* src = reinterpret_cast<const uint32_t*>(reinterpret_cast<const uint8_t*>(p0 ? F1 : F0) + (q0 - p0) * 2);
-        const uint32_t w0 = src[0], w1 = src[1], w2 = src[2], w3 = kc ? 0u : src[3];   // cj = 14, 15 are padding
+        // cj = 14, 15 are padding; the fused bias sits at cj = 14 of every block row and meets the column of ones the
+        // repack puts at K index (row 0, cj 14) -- the other rows' pads are zero, so it is added exactly once
+        const uint32_t w0 = src[0], w1 = src[1], w2 = src[2], w3 = kc ? bias_bits : src[3];
         *reinterpret_cast<uint4*>(lib + kc * Bc::LBO + (d * 16 + ci) * 16) = make_uint4(w0, w1, w2, w3);
     }
 }

@@ -356,6 +356,55 @@ def test_multi_kernel_fusion_on_a_one_window_map(wb, oracle, dtype):
     assert max_err_over_tol(y, ref, tol) <= 1.0
 
 
+# ------------------------------------------------------------------ fused bias / identity shortcut (NEXT-3)
+@pytest.mark.parametrize("case,identity", [
+    (si.Case("f_w14", 19, 5, 56, 56, 14, seed=81), 1.0),
+    (si.Case("f_w14_box", 40, 150, 28, 28, 14, seed=82), 0.0),
+    (si.Case("f_w14_shift", 9, 7, 28, 56, 14, shift=(7, 3), seed=83), 2.0),
+    (si.Case("f_w14_ragged", 7, 6, 60, 60, 14, shift=(5, 8), seed=84), 0.5),
+    (si.Case("f_w14_f16_nhwc", 6, 8, 42, 56, 14, dtype="f16", layout=NHWC, seed=85), 1.0),
+    (si.Case("f_w7", 21, 6, 56, 56, 7, seed=86), 0.0),
+    (si.Case("f_w7_shift", 5, 7, 28, 28, 7, shift=(3, 2), seed=87), 0.0),
+], ids=lambda v: v.name if hasattr(v, "name") else str(v))
+def test_fused_bias_and_identity(wb, oracle, case, identity):
+    """y = W_c x + identity x + bias_c in the pipelined kernel (bias as one more K index, identity as the
+    identity block of the library) against the oracle's Algorithm 1 with M = R[:, I] + identity I and a bias;
+    transposed application without the bias."""
+    d = si.make(case, device="cuda")
+    td = d["x"].dtype
+    bias = torch.randn((case.C,), generator=torch.Generator().manual_seed(case.seed)).to(td).cuda()
+    M = oracle.weight_matrix(widen(d["T"]), case.w) + identity * np.eye(case.w ** 2)[None]
+    y = wb.wbmm_forward_fused(d["x"], d["T"], case.w, case.shift, case.layout, bias, identity)
+    assert wb.wbmm_last_path() == (wb.PATH_TC_TMA if case.layout == NCHW else wb.PATH_TC_TRANSPOSED)
+    ref = oracle.apply_matrix(widen(d["x"]), M, case.w, case.shift, case.layout, bias=widen(bias))
+    assert max_err_over_tol(y, ref, TOL[case.dtype]) <= 1.0
+    dx = wb.wbmm_forward_fused(d["x"], d["T"], case.w, case.shift, case.layout, None, identity, transpose=True)
+    rdx = oracle.apply_matrix(widen(d["x"]), M, case.w, case.shift, case.layout, transpose=True)
+    assert max_err_over_tol(dx, rdx, TOL[case.dtype]) <= 1.0
+
+
+def test_fused_bias_exact_with_zero_table(wb):
+    """Zero table: y = identity * x + bias_c must be exact (one rounding of an fp32 sum of two 16-bit values)
+    -- pins that the bias is added exactly once and to every output position, the identity to its own."""
+    case = si.Case("f_exact", 9, 12, 28, 56, 14, shift=(7, 7), seed=88)
+    d = si.make(case, device="cuda")
+    bias = torch.randn((case.C,), generator=torch.Generator().manual_seed(89)).to(torch.bfloat16).cuda()
+    y = wb.wbmm_forward_fused(d["x"], torch.zeros_like(d["T"]), 14, case.shift, bias=bias, identity=1.0)
+    ref = (d["x"].float() + bias.float().view(1, -1, 1, 1)).to(torch.bfloat16)
+    assert torch.equal(y, ref)
+    y7 = wb.wbmm_forward_fused(d["x"], torch.zeros((case.C, 169), dtype=torch.bfloat16, device="cuda"), 7, bias=bias)
+    assert torch.equal(y7, bias.view(1, -1, 1, 1).expand_as(d["x"]).contiguous())
+
+
+def test_fused_unsupported_combinations_fail_loudly(wb):
+    x = torch.zeros((2, 4, 14, 14), dtype=torch.bfloat16, device="cuda")
+    T7 = torch.zeros((4, 169), dtype=torch.bfloat16, device="cuda")
+    with pytest.raises(wb.WbmmError):       # the identity block exists in the w = 14 library only
+        wb.wbmm_forward_fused(x, T7, 7, identity=1.0)
+    with pytest.raises(wb.WbmmError):       # fp32 has no pipelined kernel
+        wb.wbmm_forward_fused(x.float(), T7.float(), 7, bias=torch.zeros(4, device="cuda"))
+
+
 def test_hier_unsupported_shapes_fail_loudly(wb):
     x = torch.zeros((2, 4, 14, 14), dtype=torch.bfloat16, device="cuda")
     with pytest.raises(wb.WbmmError):       # w = 7 has no hierarchical tensor-core path
