@@ -475,6 +475,39 @@ def run_sweep(args):
                           "path": wb.wbmm_path_string(wb.wbmm_last_path()), "buffer_sets": nsets}), flush=True)
         del xs, ys, d
 
+    # backward (rows a7, a8 of SURVEY.md 8(a)) on the named configs and the large sweep shapes: dX and dT timed
+    # apart, back to back on one buffer set (x + dy + dx of these shapes exceed L2 except where noted by the size)
+    bwd = [si.with_(si.CFG2, backward=True), si.with_(si.CFG3, backward=True), si.CFG5,
+           si.with_(si.CFG5, shift=(0, 0), name="cfg5_shape_no_shift")]
+    for (C, H) in ((96, 56), (192, 28), (384, 28), (96, 112)):
+        for w in (7, 14):
+            bwd.append(si.Case(f"bwd_B128_C{C}_H{H}_w{w}", 128, C, H, H, w, backward=True, seed=200 + C + H + w))
+    bwd.append(si.Case("bwd_ragged_B64_C96_H60_w14", 64, 96, 60, 60, 14, backward=True, seed=299))
+    for case in bwd:
+        d = si.make(case, device="cuda")
+        dx = torch.empty_like(d["x"])
+        dT = torch.empty((case.C, case.bins), dtype=torch.float32, device="cuda")
+        out = {}
+        for key, fn in (("dX", lambda: wb.wbmm_backward(None, d["T"], d["dy"], case.w, case.shift, case.layout, need_dT=False)),
+                        ("dT", lambda: wb.wbmm_backward(d["x"], None, d["dy"], case.w, case.shift, case.layout, need_dx=False, dT=dT))):
+            for _ in range(3):
+                fn()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            n = 20
+            a.record(stream)
+            for _ in range(n):
+                fn()
+            b.record(stream)
+            torch.cuda.synchronize()
+            out[key] = (a.elapsed_time(b) / n, wb.wbmm_path_string(wb.wbmm_last_path()))
+        by = bytes_of(case)          # dX: dy in, dx out; dT: x and dy in -- the same 2 x tensor bytes (+ table)
+        print(json.dumps({"sweep_case": "backward_" + case.name, "layout": "NCHW", "B": case.B, "C": case.C, "H": case.H,
+                          "w": case.w, "shift": list(case.shift), "dX_ms": round(out["dX"][0], 5), "dT_ms": round(out["dT"][0], 5),
+                          "dX_frac_of_hbm_roofline": round(by / (hbm_peak * 1e9) * 1e3 / out["dX"][0], 4),
+                          "dT_frac_of_hbm_roofline": round(by / (hbm_peak * 1e9) * 1e3 / out["dT"][0], 4),
+                          "dX_path": out["dX"][1], "dT_path": out["dT"][1]}), flush=True)
+        del d, dx, dT
+
 
 def main():
     ap = argparse.ArgumentParser()
