@@ -59,6 +59,29 @@ def test_argument_validation_without_gpu(wb):
     assert L.wbmm_backward(ctypes.byref(d), p, None, p + 64, p + 128, None, None) == 1  # dx needs T
 
 
+def test_argument_validation_of_the_extended_entry_points(wb):
+    """Hierarchical / cached-M / fused / fold entry points: argument errors are reported before any device work."""
+    from paper_2607_02097_b200 import binding
+    L = binding.lib()
+    buf = (ctypes.c_float * 4096)()
+    p = ctypes.addressof(buf)
+    d14 = wb.WbmmDesc(1, 1, 14, 14, 14, 0, 0, 1, 0, 0)
+    odd = wb.WbmmDesc(1, 1, 14, 14, 7, 0, 0, 1, 0, 0)
+    assert L.wbmm_hier_forward(ctypes.byref(odd), p, p + 64, p + 128, p + 4096, 0, None) == 1        # w must be even
+    assert L.wbmm_hier_forward(ctypes.byref(d14), p, None, p + 128, p + 4096, 0, None) == 1
+    assert L.wbmm_hier_backward(ctypes.byref(d14), p, p + 64, p + 128, p + 256, None, p + 512, None, None) == 1   # dTg without dTl
+    assert L.wbmm_hier_backward(ctypes.byref(odd), p, p + 64, p + 128, p + 256, p + 4096, None, None, None) == 1
+    assert L.wbmm_forward_matrix(ctypes.byref(d14), p, None, None, p + 4096, 0, None) == 1
+    assert L.wbmm_forward_matrix(ctypes.byref(d14), p, p + 64, None, p, 0, None) == 1                # y aliases x
+    assert L.wbmm_forward_fused(ctypes.byref(d14), p, None, None, ctypes.c_float(0.0), p + 4096, 0, None) == 1
+    assert L.wbmm_forward_fused(ctypes.byref(d14), p, p + 64, None, ctypes.c_float(float("nan")), p + 4096, 0, None) == 1
+    assert L.wbmm_forward_fused(ctypes.byref(d14), p + 1, p + 64, None, ctypes.c_float(0.0), p + 4096, 0, None) == 5
+    for ks in (0, 4, 29):                                                                            # even / too large
+        assert L.wbmm_fold_dwconv(ctypes.byref(d14), p, p + 64, ks, None, p + 128, None) == 1, ks
+    assert L.wbmm_fold_dwconv(ctypes.byref(d14), p, None, 3, None, p + 128, None) == 1
+    assert L.wbmm_fold_dwconv(None, p, p + 64, 3, None, p + 128, None) == 1
+
+
 @pytest.mark.skipif(torch.cuda.is_available(), reason="checks the no-GPU behaviour")
 def test_no_cpu_fallback(wb):
     """Without a device every compute entry point fails loudly."""
