@@ -192,8 +192,10 @@ int wbmm_backward(const wbmm_desc_t* desc, const void* x, const void* T, const v
     }
     if (dT) {
         if (!(desc->flags & WBMM_FLAG_ACCUMULATE_DT) && g.C > 0) {
-            cudaError_t e = cudaMemsetAsync(dT, 0, sizeof(float) * (size_t)g.C * g.nb, stream);
-            if (e != cudaSuccess) return set_cuda_error(e, "memset dT");
+            int zl = 0;
+            cudaError_t e = wbmm::simt_zero_f32(dT, (long long)g.C * g.nb, stream, &zl);
+            g_launches += zl;
+            if (e != cudaSuccess) return set_cuda_error(e, "zero dT");
         }
         int launches = 0;
         cudaError_t e;
@@ -275,9 +277,11 @@ int wbmm_hier_backward(const wbmm_desc_t* desc, const void* x, const void* Tg, c
     if (dTl && !aligned(dTl, 4)) return WBMM_STATUS_MISALIGNED;
     if (dTg && !(desc->flags & WBMM_FLAG_ACCUMULATE_DT)) {
         if (device_state() < 0) return WBMM_STATUS_NO_DEVICE;
-        cudaError_t e = cudaMemsetAsync(dTg, 0, ng, stream);
-        if (e == cudaSuccess) e = cudaMemsetAsync(dTl, 0, nl, stream);
-        if (e != cudaSuccess) return set_cuda_error(e, "memset dT (hierarchical)");
+        int zl = 0;
+        cudaError_t e = wbmm::simt_zero_f32(dTg, (long long)(ng / sizeof(float)), stream, &zl);
+        if (e == cudaSuccess) e = wbmm::simt_zero_f32(dTl, (long long)(nl / sizeof(float)), stream, &zl);
+        g_launches += zl;
+        if (e != cudaSuccess) return set_cuda_error(e, "zero dT (hierarchical)");
     }
     if (desc->B == 0) return WBMM_STATUS_OK;
     if (!dy || (dx && (!Tg || !Tl)) || (dTg && !x) || (dx && dx == dy)) return WBMM_STATUS_INVALID_ARGUMENT;

@@ -62,6 +62,8 @@ cudaError_t simt_grad_table(const Geom& g, int dtype, const void* x, const void*
                             cudaStream_t stream, int* launches);
 cudaError_t simt_materialize(int C, int w, int dtype, const void* T, void* Wout,
                              cudaStream_t stream, int* launches);
+// p[0..n) = 0 (stream-ordered; programmatic dependent launch on both sides).
+cudaError_t simt_zero_f32(float* p, long long n, cudaStream_t stream, int* launches);
 // Tout = T + scale_c * (the table of a zero-padded kk x kk depthwise conv); Tout may be T.
 cudaError_t simt_fold_dwconv(int C, int w, int kk, int dtype, const void* T, const void* K, const float* scale,
                              void* Tout, cudaStream_t stream, int* launches);
