@@ -373,7 +373,18 @@ bool dt_tiles(const Geom& g, TcTiles* t)
 {
     if (!tc_tiles(g, t)) return false;
     const bool plain = g.sh == 0 && g.sw == 0 && g.H == g.Hp && g.W == g.Wp;
-    if (!plain || t->nstrips != 1 || dt_slots<WS>(*t) >= 2 * t->NP + 1) return true;
+    if (t->nstrips != 1 || dt_slots<WS>(*t) >= 2 * t->NP + 1) return true;
+    if (!plain) {
+        // shifted / ragged maps need whole images (general addressing): fewer images per tile instead; the
+        // windows a tile then lacks are zero columns of the contraction
+        TcTiles c = *t;
+        while (c.NP > 1 && dt_slots<WS>(c) < 2 * c.NP + 1) c.NP /= 2;
+        c.ngb = (g.B + c.NP - 1) / c.NP;
+        c.tiles_per_c = c.ngb * c.nstrips;
+        c.ntiles = (long long)g.C * c.tiles_per_c;
+        if (dt_slots<WS>(c) >= 2 * c.NP + 1) *t = c;
+        return true;
+    }
     for (int nsy = g.nwh / 2; nsy >= 1; --nsy) {
         if (g.nwh % nsy != 0 || (nsy * g.w * g.W * 2) % 16 != 0) continue;
         TcTiles c = *t;

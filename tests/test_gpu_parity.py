@@ -167,6 +167,19 @@ def test_pipelined_kernels_one_hot_bins_bitwise(wb, oracle, w, shift, H, W, layo
     assert np.array_equal(widen(dx), rdx)
 
 
+@pytest.mark.parametrize("H,W,shift", [(112, 112, (7, 7)), (112, 112, (3, 8)), (106, 112, (0, 0))])
+def test_table_gradient_of_large_shifted_maps_stays_on_the_tensor_cores(wb, oracle, H, W, shift):
+    """Shifted / ragged 112-row maps need whole frame images (general addressing): the dT kernel then takes one
+    image per tile (half the MMA K is zero windows) instead of falling back to SIMT."""
+    case = si.Case("dt_big_shift", 5, 4, H, W, 14, shift=shift, seed=72, backward=True)
+    d = si.make(case, device="cuda")
+    _, dT = wb.wbmm_backward(d["x"], None, d["dy"], 14, shift, need_dx=False)
+    torch.cuda.synchronize()
+    assert wb.wbmm_last_path() == wb.PATH_TC_TMA, wb.wbmm_path_string(wb.wbmm_last_path())
+    _, rdT = oracle.backward(widen(d["x"]), widen(d["T"]), widen(d["dy"]), 14, shift, need_dx=False)
+    assert max_err_over_tol(dT, rdT, TOL["bf16"]) <= 1.0
+
+
 @pytest.mark.parametrize("B,C,H,W", [(5, 6, 112, 112), (9, 3, 112, 56), (3, 4, 112, 224)])
 def test_table_gradient_of_large_maps_stays_on_the_tensor_cores(wb, oracle, B, C, H, W):
     """112-row maps at w = 14: whole frame images (25 KB) of x and dy do not fit beside the operand stage, so
