@@ -622,7 +622,8 @@ int bulk_mode(const Geom& g, const TcTiles& tl, const void* x, const void* y)
     const bool plain = g.sh == 0 && g.sw == 0 && g.H == g.Hp && g.W == g.Wp;
     if (plain && (tl.frame_rows * g.W * 2) % 16 == 0 && (WS % 2 == 0 || g.W % 2 == 0)) return 1;   // odd w: rows must be word-aligned
     // general form: whole images in natural layout, word-granular window addressing (W, W' even)
-    return (tl.nstrips == 1 && g.W % 2 == 0 && g.Wp % 2 == 0) ? 2 : 0;
+    // (an odd W' -- ragged maps at odd w -- is fine without a column shift: nothing wraps)
+    return (tl.nstrips == 1 && g.W % 2 == 0 && (g.Wp % 2 == 0 || g.sw == 0)) ? 2 : 0;
 }
 
 // cuTensorMapEncodeTiled through the runtime's driver entry point (libcuda is not linked).

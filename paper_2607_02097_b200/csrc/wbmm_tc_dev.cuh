@@ -348,7 +348,7 @@ __device__ __forceinline__ void gen_addr_init(GenAddr<WS>& a, const Geom& g, int
 #pragma unroll
     for (int k = 0; k < GenAddr<WS>::NWR; ++k) {
         int wi = wbase + k;
-        if (wi >= wpr) wi -= wpr;
+        if (g.sw != 0 && wi >= wpr) wi -= wpr;      // columns wrap only under a shift (then W' is even: whole words wrap)
         a.coloff[k] = wi < wreal ? wi * 4 : 0;
         a.colmask |= (wi < wreal ? 1u : 0u) << k;
     }

@@ -361,7 +361,8 @@ int dt_mode(const Geom& g, const TcTiles& tl, const void* x, const void* dy)
     const bool plain = g.sh == 0 && g.sw == 0 && g.H == g.Hp && g.W == g.Wp;
     if (plain && (tl.frame_rows * g.W * 2) % 16 == 0 && (WS % 2 == 0 || g.W % 2 == 0)) return 1;   // odd w: rows must be word-aligned
     // general form: whole images in natural layout, word-granular window addressing (W, W' even)
-    return (tl.nstrips == 1 && g.W % 2 == 0 && g.Wp % 2 == 0) ? 2 : 0;
+    // (an odd W' -- ragged maps at odd w -- is fine without a column shift: nothing wraps)
+    return (tl.nstrips == 1 && g.W % 2 == 0 && (g.Wp % 2 == 0 || g.sw == 0)) ? 2 : 0;
 }
 
 // Tiling of the table-gradient kernel.  Its ring holds x AND dy and shares the SM with the 106 KB operand stage,
@@ -373,8 +374,9 @@ bool dt_tiles(const Geom& g, TcTiles* t)
 {
     if (!tc_tiles(g, t)) return false;
     const bool plain = g.sh == 0 && g.sw == 0 && g.H == g.Hp && g.W == g.Wp;
-    if (t->nstrips != 1 || dt_slots<WS>(*t) >= 2 * t->NP + 1) return true;
+    if (dt_slots<WS>(*t) >= 2 * t->NP + 1) return true;
     if (!plain) {
+        if (t->nstrips != 1) return true;
         // shifted / ragged maps need whole images (general addressing): fewer images per tile instead; the
         // windows a tile then lacks are zero columns of the contraction
         TcTiles c = *t;
@@ -385,7 +387,7 @@ bool dt_tiles(const Geom& g, TcTiles* t)
         if (dt_slots<WS>(c) >= 2 * c.NP + 1) *t = c;
         return true;
     }
-    for (int nsy = g.nwh / 2; nsy >= 1; --nsy) {
+    for (int nsy = t->NSY - 1; nsy >= 1; --nsy) {
         if (g.nwh % nsy != 0 || (nsy * g.w * g.W * 2) % 16 != 0) continue;
         TcTiles c = *t;
         c.NSY = nsy;

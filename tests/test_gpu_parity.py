@@ -107,7 +107,9 @@ PIPE = [
     si.Case("p_w7_plain", 21, 6, 56, 56, 7),                                 # 64 windows per image
     si.Case("p_w7_strips", 3, 5, 112, 112, 7),                               # 256 windows per image: strips
     si.Case("p_w7_shift", 5, 7, 28, 28, 7, shift=(3, 2)),
-    si.Case("p_w7_ragged", 6, 4, 26, 30, 7, shift=(0, 3)),                   # W' = 35 is odd: generic path
+    si.Case("p_w7_ragged", 6, 4, 26, 30, 7, shift=(0, 3)),                   # W' = 35 is odd and columns wrap: generic path
+    si.Case("p_w7_ragged_noshift", 6, 4, 30, 60, 7),                         # W' = 63 is odd, nothing wraps: pipelined
+    si.Case("p_w7_ragged_rowshift", 5, 3, 60, 60, 7, shift=(3, 0)),          # rows wrap, columns do not
     si.Case("p_w7_f16", 33, 3, 28, 56, 7, dtype="f16"),
 ]
 
@@ -180,7 +182,7 @@ def test_table_gradient_of_large_shifted_maps_stays_on_the_tensor_cores(wb, orac
     assert max_err_over_tol(dT, rdT, TOL["bf16"]) <= 1.0
 
 
-@pytest.mark.parametrize("B,C,H,W", [(5, 6, 112, 112), (9, 3, 112, 56), (3, 4, 112, 224)])
+@pytest.mark.parametrize("B,C,H,W", [(5, 6, 112, 112), (9, 3, 112, 56), (3, 4, 112, 224), (2, 3, 224, 224)])
 def test_table_gradient_of_large_maps_stays_on_the_tensor_cores(wb, oracle, B, C, H, W):
     """112-row maps at w = 14: whole frame images (25 KB) of x and dy do not fit beside the operand stage, so
     the dT kernel tiles them in strips of window rows (more images per tile); it must not fall back to SIMT."""
