@@ -295,7 +295,9 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
         for (int t = t0; t < t1; ++t) {
             int c, b0, wy0, np_eff, rows_eff;
             tile_decode(t, c, b0, wy0, np_eff, rows_eff);
-            const uint32_t bytes = (uint32_t)rows_eff * rowB;
+            // sbox == 2 ("plane boxes"): planes whose byte size is not a multiple of 16 (14 x 14: 392 B) -- the map is over
+            // [B][C*H*W], a box is box images x (H*W rounded up to 8) elements from element c*H*W: slot pitch tl.S
+            const uint32_t bytes = sbox == 2 ? (uint32_t)tl.S : (uint32_t)rows_eff * rowB;
             if (box) {
                 // small images: ONE tensor-map box {a, b, 1 channel, box images} per group instead of `box` copies
                 for (int p = lane * box; p < np_eff; p += 32 * box) {
@@ -304,7 +306,9 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                     ptx::mbar_wait(EMPTY(slot), ((kk / nslot) & 1) ^ 1);
                     ptx::mbar_arrive_expect_tx(FULL(slot), bytes * box);
                     if (p == 0) TRACE(0, (t - t0));
-                    ptx::tma_load_4d(ptx::smem_u32(ring + (size_t)slot * tl.S), &mx, 0, 0, c, b0 + p, FULL(slot));
+                    // (the box starts on a 16-byte boundary at or below the plane: the plane sits poff bytes into the slot)
+                    ptx::tma_load_4d(ptx::smem_u32(ring + (size_t)slot * tl.S), &mx, sbox == 2 ? (c * (int)plane_elems) & ~7 : 0, 0,
+                                     sbox == 2 ? 0 : c, b0 + p, FULL(slot));
                 }
             } else
             for (int p = lane; p < np_eff; p += 32) {
@@ -438,6 +442,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
             const bool valid = part && wy0 + wyl < g.nwh;
             const uint32_t kk = k + pl;
             const int slot = kk % nslot;
+            const int poff = sbox == 2 ? ((c * (int)plane_elems) & 7) * 2 : 0;    // plane boxes: offset of the plane in its slot
             if (lt == 0) rebuild_weight(c, lt);   // first tile: build while its loads are in flight
             if (rt == 0) TRACE(5, lt);
             const int bslot = box ? slot - slot % box : slot;      // the barrier pair that covers this image
@@ -447,14 +452,14 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
             {
                 const uint32_t ta = tmem + buf * A_STRIDE + ((uint32_t)(q * 32) << 16);
                 if constexpr (GEN && WS % 2 == 0) {      // even w: every window starts on the parity of the column shift
-                    if (g.sw & 1) window_to_tmem_gen<WS, 1>(ring + (size_t)slot * tl.S, ga, valid, ragged, ta, pad0);
-                    else window_to_tmem_gen<WS, 0>(ring + (size_t)slot * tl.S, ga, valid, ragged, ta, pad0);
+                    if (g.sw & 1) window_to_tmem_gen<WS, 1>(ring + (size_t)slot * tl.S + poff, ga, valid, ragged, ta, pad0);
+                    else window_to_tmem_gen<WS, 0>(ring + (size_t)slot * tl.S + poff, ga, valid, ragged, ta, pad0);
                 } else {
-                    window_to_tmem_gen<WS>(ring + (size_t)slot * tl.S, ga, valid, GEN && ragged, ta, pad0);
+                    window_to_tmem_gen<WS>(ring + (size_t)slot * tl.S + poff, ga, valid, GEN && ragged, ta, pad0);
                 }
             }
             else
-                window_to_tmem_bulk<WS>(ring + (size_t)slot * tl.S + win_off, valid, rowB,
+                window_to_tmem_bulk<WS>(ring + (size_t)slot * tl.S + poff + win_off, valid, rowB,
                                         tmem + buf * A_STRIDE + ((uint32_t)(q * 32) << 16), pad0);
             if (part) ptx::mbar_arrive(EMPTY(bslot));   // every window of this image is in TMEM
             // W_c of a new channel is rebuilt AFTER this tile's windows are in TMEM, so the copy above
@@ -538,7 +543,30 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
             for (long long off = lane * 128ll; off < nbytes; off += 32 * 128)
                 asm volatile("prefetch.global.L2 [%0];" ::"l"(base + off));
         }
-        if (lane < nout) {
+        if (sbox == 2) {
+            // plane boxes: a plane is not a multiple of 16 bytes, so no bulk store can write it -- the whole warp
+            // copies the group's planes with 8-byte stores (these maps are small: a few KB per tile)
+            const uint32_t depth = nout / og.n;
+            const uint32_t out_bytes = (uint32_t)og.images * tl.S;
+            const int chunks = (int)(plane_elems * 2 / 8);
+            uint32_t lt = 0;
+            for (int t = t0; t < t1; ++t, ++lt) {
+                int c, b0, wy0, np_eff, rows_eff;
+                tile_decode(t, c, b0, wy0, np_eff, rows_eff);
+                for (int gq = 0; gq < og.n; ++gq) {
+                    const uint32_t ob = (lt % depth) * og.n + gq;
+                    ptx::mbar_wait(OUT_FULL + 8 * ob, (lt / depth) & 1);
+                    const int p_first = gq * og.images, p_end = min(p_first + og.images, np_eff);
+                    for (int idx = lane; idx < (p_end - p_first) * chunks; idx += 32) {
+                        const int p = idx / chunks, ch = idx - p * chunks;
+                        const uint2 v = *reinterpret_cast<const uint2*>(outb + (size_t)ob * out_bytes + (size_t)p * tl.S + ch * 8);
+                        *reinterpret_cast<uint2*>(reinterpret_cast<uint8_t*>(y + ((long long)(b0 + p_first + p) * g.C + c) * plane_elems) + ch * 8) = v;
+                    }
+                    __syncwarp();
+                    if (lane == 0) ptx::mbar_arrive(OUT_EMPTY + 8 * ob);
+                }
+            }
+        } else if (lane < nout) {
             // Lane ob = (frame, gq) owns output buffer ob: group gq of the tiles lt = frame mod depth.  It
             // bulk-stores the group's images and releases the buffer once the copy engine has read it.
             // One lane per buffer, so the ~1.4 us a store needs before its source may be overwritten is
@@ -614,13 +642,14 @@ template <int WS>
 int bulk_mode(const Geom& g, const TcTiles& tl, const void* x, const void* y)
 {
     if (g.layout != WBMM_LAYOUT_NCHW) return 0;
-    if (((long long)g.H * g.W * 2) % 16 != 0) return 0;
+    const bool pb = ((long long)g.H * g.W * 2) % 16 != 0;       // planes no bulk copy can move: tensor-map "plane boxes"
+    if (pb && plane_box_images(g, tl) == 0) return 0;
     if (reinterpret_cast<uintptr_t>(x) % 16 != 0 || reinterpret_cast<uintptr_t>(y) % 16 != 0) return 0;
     if (tl.NP > kMaxSlots || tl.ntiles > 0x3fffffffll) return 0;
     int nslot_, nout_;
     if (!bulk_slots<WS>(tl, tl.NSY * g.nww, &nslot_, &nout_)) return 0;
     const bool plain = g.sh == 0 && g.sw == 0 && g.H == g.Hp && g.W == g.Wp;
-    if (plain && (tl.frame_rows * g.W * 2) % 16 == 0 && (WS % 2 == 0 || g.W % 2 == 0)) return 1;   // odd w: rows must be word-aligned
+    if (plain && (pb || (tl.frame_rows * g.W * 2) % 16 == 0) && (WS % 2 == 0 || g.W % 2 == 0)) return 1;   // odd w: rows must be word-aligned
     // general form: whole images in natural layout, word-granular window addressing (W, W' even)
     // (an odd W' -- ragged maps at odd w -- is fine without a column shift: nothing wraps)
     return (tl.nstrips == 1 && g.W % 2 == 0 && (g.Wp % 2 == 0 || g.sw == 0)) ? 2 : 0;
@@ -655,6 +684,35 @@ EncodeTiledFn bulk_encode_fn()
 // Tensor map over an NCHW activation viewed as (a, b, C, B), a*b = H*W, with box {a, b, 1, images}: `images`
 // whole frame images of one channel per copy.  False when H*W has no legal factorisation or the driver
 // entry point is missing.  `map` is a CUtensorMap.
+// Plane boxes: when H*W*2 is not a multiple of 16 (14 x 14 maps: 392 B) neither a bulk copy nor a tensor map with a
+// channel dimension can address one plane, but a map over [B][C*H*W] can: a box of `images` rows x (H*W + 7 rounded up
+// to 8) elements starting at the 16-byte boundary at or below element c*H*W (it also reads a few elements of the
+// neighbouring planes; the slot pitch is the padded size and the plane sits (c*H*W mod 8) elements into its slot).  Returns the images per box (8, 4 or 2), 0 when the shape does not allow it.
+int plane_box_images(const Geom& g, const TcTiles& tl)
+{
+    const long long hw = (long long)g.H * g.W;
+    const long long hwp = (hw + 14) / 8 * 8;       // the box starts up to 7 elements before the plane (16-byte boundary)
+    if (tl.nstrips != 1 || hw % 2 != 0 || hwp > 256 || (g.C * hw * 2) % 16 != 0 || g.C * hw > 0x7fffffffll) return 0;
+    for (int cand = 8; cand >= 2; cand >>= 1)
+        if (tl.NP % cand == 0 && g.B % cand == 0 && (cand * hwp * 2) % 128 == 0) return cand;
+    return 0;
+}
+
+bool plane_box_map(const Geom& g, int dtype, const void* base, int images, void* map)
+{
+    const long long hw = (long long)g.H * g.W, hwp = (hw + 14) / 8 * 8;
+    EncodeTiledFn fn = bulk_encode_fn();
+    if (!fn || images < 1 || images > 256 || hwp > 256) return false;
+    const cuuint64_t row = (cuuint64_t)g.C * hw;
+    const cuuint64_t dims[4] = {row, 1, 1, (cuuint64_t)g.B};
+    const cuuint64_t strides[3] = {row * 2, row * 2, row * 2};
+    const cuuint32_t boxd[4] = {(cuuint32_t)hwp, 1, 1, (cuuint32_t)images};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    const CUtensorMapDataType dt = dtype == WBMM_DTYPE_BF16 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT16;
+    return fn(static_cast<CUtensorMap*>(map), dt, 4, const_cast<void*>(base), dims, strides, boxd, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 bool image_box_map(const Geom& g, int dtype, const void* base, int images, void* map)
 {
     const long long hw = (long long)g.H * g.W, ib = hw * 2;
@@ -707,14 +765,25 @@ cudaError_t launch_bulk(const Geom& g, const TcTiles& tl_in, const void* x, cons
     CUtensorMap mx, my;
     memset(&mx, 0, sizeof(mx));
     memset(&my, 0, sizeof(my));
-    int sbox = 0;
-    int box = bulk_box_mode(g, tl_in, BF16 ? WBMM_DTYPE_BF16 : WBMM_DTYPE_F16, x, y, &tl.S, &sbox, &mx, &my);
+    int sbox = 0, box = 0;
     const int wpf = tl.NSY * g.nww;
-    if (box) {
-        if (bulk_slots<WS>(tl, wpf, &nslot, &nout)) nslot -= nslot % box;      // groups never wrap around the ring
-        if (nslot < tl.NP + box) {                                            // (does not fit: one copy per image)
-            box = sbox = 0;
-            tl = tl_in;
+    if (((long long)g.H * g.W * 2) % 16 != 0) {
+        // plane boxes (see plane_box_images): loads by tensor map, stores by the store warp's own 8-byte stores
+        box = plane_box_images(g, tl_in);
+        if (box == 0 || !plane_box_map(g, BF16 ? WBMM_DTYPE_BF16 : WBMM_DTYPE_F16, x, box, &mx)) return cudaErrorInvalidConfiguration;
+        sbox = 2;
+        tl.S = (int)(((long long)g.H * g.W + 14) / 8 * 8 * 2);
+        if (!bulk_slots<WS>(tl, wpf, &nslot, &nout)) return cudaErrorInvalidConfiguration;
+        nslot -= nslot % box;
+        if (nslot < tl.NP + box) return cudaErrorInvalidConfiguration;
+    } else {
+        box = bulk_box_mode(g, tl_in, BF16 ? WBMM_DTYPE_BF16 : WBMM_DTYPE_F16, x, y, &tl.S, &sbox, &mx, &my);
+        if (box) {
+            if (bulk_slots<WS>(tl, wpf, &nslot, &nout)) nslot -= nslot % box;      // groups never wrap around the ring
+            if (nslot < tl.NP + box) {                                            // (does not fit: one copy per image)
+                box = sbox = 0;
+                tl = tl_in;
+            }
         }
     }
     if (!box && !bulk_slots<WS>(tl, wpf, &nslot, &nout)) return cudaErrorInvalidConfiguration;
@@ -863,6 +932,8 @@ bool tc_tiles(const Geom& g, TcTiles* t)
     if (wpp <= 128) {
         t->NSY = g.nwh;
         t->NP = 128 / wpp;
+        if (t->NP > 64) t->NP = 64;      // one window per image (14 x 14 at w = 14): half-filled tiles, so that the ring's
+                                         // slot count (one frame image each) stays within kMaxSlots
         if (t->NP > g.B) t->NP = g.B;
     } else {
         t->NP = 1;

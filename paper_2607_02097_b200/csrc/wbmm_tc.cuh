@@ -50,6 +50,10 @@ cudaError_t tc_grad_table(const Geom& g, int dtype, const void* x, const void* d
 // Tensor map (CUtensorMap behind the void*) over an NCHW activation with box = `images` whole frame images of
 // one channel (wbmm_tc.cu).
 bool image_box_map(const Geom& g, int dtype, const void* base, int images, void* map);
+// Plane boxes for planes whose byte size is not a multiple of 16 (wbmm_tc.cu): images per box (0 = not possible) and
+// the tensor map over [B][C*H*W] (box = images x (H*W rounded up to 8) elements; inner coordinate c*H*W).
+int plane_box_images(const Geom& g, const TcTiles& tl);
+bool plane_box_map(const Geom& g, int dtype, const void* base, int images, void* map);
 
 void tc_release();
 

@@ -60,7 +60,7 @@ struct DtCfg {
 template <int WS, bool BF16, bool GEN, bool HIER>
 __global__ void __launch_bounds__(kThreadsD, 1)
 tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __restrict__ x,
-             const uint16_t* __restrict__ dy, float* __restrict__ dT, float* __restrict__ dTl, int box,
+             const uint16_t* __restrict__ dy, float* __restrict__ dT, float* __restrict__ dTl, int box, int pbox,
              const __grid_constant__ CUtensorMap mx, const __grid_constant__ CUtensorMap mg)
 {
     using Cf = WinCfg<WS>;
@@ -123,7 +123,8 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
         for (int t = t0; t < t1; ++t) {
             int c, b0, wy0, np_eff, rows_eff;
             tile_decode(t, c, b0, wy0, np_eff, rows_eff);
-            const uint32_t bytes = (uint32_t)rows_eff * rowB;
+            // pbox ("plane boxes", wbmm_tc.cu): the maps are over [B][C*H*W], inner coordinate c*H*W, slot pitch tl.S
+            const uint32_t bytes = pbox ? (uint32_t)tl.S : (uint32_t)rows_eff * rowB;
             if (box) {
                 // small images: one tensor-map box per group of `box` images and operand; ring order per tile:
                 // x group 0, dy group 0, x group 1, dy group 1, ...
@@ -132,7 +133,8 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
                     const int slot = kk % nslot;
                     ptx::mbar_wait(EMPTY(slot), ((kk / nslot) & 1) ^ 1);
                     ptx::mbar_arrive_expect_tx(FULL(slot), bytes * box);
-                    ptx::tma_load_4d(ptx::smem_u32(ring + (size_t)slot * tl.S), (j & 1) ? &mg : &mx, 0, 0, c, b0 + (j >> 1) * box, FULL(slot));
+                    ptx::tma_load_4d(ptx::smem_u32(ring + (size_t)slot * tl.S), (j & 1) ? &mg : &mx, pbox ? (c * (int)plane_elems) & ~7 : 0, 0,
+                                     pbox ? 0 : c, b0 + (j >> 1) * box, FULL(slot));
                 }
             } else
             for (int j = lane; j < 2 * np_eff; j += 32) {
@@ -219,7 +221,7 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
             if (ot == 0) TRACE(5, lt);
             ptx::mbar_wait(STAGE_EMPTY + 8 * hf, (lt & 1) ^ 1);      // the MMAs of tile lt-1 have read this half
             if (ot == 0) TRACE(6, lt);
-            const uint8_t* img = ring + (size_t)slot * tl.S;
+            const uint8_t* img = ring + (size_t)slot * tl.S + (pbox ? ((c * (int)plane_elems) & 7) * 2 : 0);
             {
                 uint32_t wv[Dc::NV * 4];
                 if constexpr (WG) {
@@ -354,12 +356,13 @@ template <int WS>
 int dt_mode(const Geom& g, const TcTiles& tl, const void* x, const void* dy)
 {
     if (g.layout != WBMM_LAYOUT_NCHW) return 0;
-    if (((long long)g.H * g.W * 2) % 16 != 0) return 0;
+    const bool pb = ((long long)g.H * g.W * 2) % 16 != 0;       // plane boxes (wbmm_tc.cu), 8 images per box here
+    if (pb && (plane_box_images(g, tl) != 8)) return 0;
     if (reinterpret_cast<uintptr_t>(x) % 16 != 0 || reinterpret_cast<uintptr_t>(dy) % 16 != 0) return 0;
     if (tl.ntiles > 0x3fffffffll) return 0;
     if (dt_slots<WS>(tl) < 2 * tl.NP + 1) return 0;
     const bool plain = g.sh == 0 && g.sw == 0 && g.H == g.Hp && g.W == g.Wp;
-    if (plain && (tl.frame_rows * g.W * 2) % 16 == 0 && (WS % 2 == 0 || g.W % 2 == 0)) return 1;   // odd w: rows must be word-aligned
+    if (plain && (pb || (tl.frame_rows * g.W * 2) % 16 == 0) && (WS % 2 == 0 || g.W % 2 == 0)) return 1;   // odd w: rows must be word-aligned
     // general form: whole images in natural layout, word-granular window addressing (W, W' even)
     // (an odd W' -- ragged maps at odd w -- is fine without a column shift: nothing wraps)
     return (tl.nstrips == 1 && g.W % 2 == 0 && (g.Wp % 2 == 0 || g.sw == 0)) ? 2 : 0;
@@ -375,10 +378,11 @@ bool dt_tiles(const Geom& g, TcTiles* t)
     if (!tc_tiles(g, t)) return false;
     const bool plain = g.sh == 0 && g.sw == 0 && g.H == g.Hp && g.W == g.Wp;
     if (dt_slots<WS>(*t) >= 2 * t->NP + 1) return true;
-    if (!plain) {
+    if (!plain || (t->nstrips == 1 && t->S <= 8192)) {
         if (t->nstrips != 1) return true;
-        // shifted / ragged maps need whole images (general addressing): fewer images per tile instead; the
-        // windows a tile then lacks are zero columns of the contraction
+        // shifted / ragged maps need whole images (general addressing), and tiny maps have more images per tile than
+        // the ring has slots for x and dy: fewer images per tile instead; the windows a tile then lacks are zero
+        // columns of the contraction
         TcTiles c = *t;
         while (c.NP > 1 && dt_slots<WS>(c) < 2 * c.NP + 1) c.NP /= 2;
         c.ngb = (g.B + c.NP - 1) / c.NP;
@@ -420,8 +424,15 @@ cudaError_t launch_dt(const Geom& g, const TcTiles& tl_in, const void* x, const 
     memset(&mx, 0, sizeof(mx));
     memset(&mg, 0, sizeof(mg));
     // small frame images: tensor-map boxes of 8 images per copy (see bulk_box_mode in wbmm_tc.cu)
-    int box = 0;
-    {
+    int box = 0, pbox = 0;
+    if (((long long)g.H * g.W * 2) % 16 != 0) {
+        const int dtype = BF16 ? WBMM_DTYPE_BF16 : WBMM_DTYPE_F16;
+        if (plane_box_images(g, tl) != 8 || !plane_box_map(g, dtype, x, 8, &mx) || !plane_box_map(g, dtype, dy, 8, &mg))
+            return cudaErrorInvalidConfiguration;
+        box = 8;
+        pbox = 1;
+        tl.S = (int)(((long long)g.H * g.W + 14) / 8 * 8 * 2);
+    } else {
         const long long ib = (long long)g.H * g.W * 2;
         const int dtype = BF16 ? WBMM_DTYPE_BF16 : WBMM_DTYPE_F16;
         if (tl.nstrips == 1 && ib <= 4096 && tl.NP % 8 == 0 && g.B % 8 == 0 && (8 * ib) % 128 == 0 &&
@@ -434,6 +445,7 @@ cudaError_t launch_dt(const Geom& g, const TcTiles& tl_in, const void* x, const 
     if (box) {
         nslot -= nslot % (2 * box);
         if (nslot < 2 * tl.NP) {
+            if (pbox) return cudaErrorInvalidConfiguration;
             box = 0;
             tl = tl_in;
             nslot = dt_slots<WS>(tl);
@@ -469,7 +481,7 @@ cudaError_t launch_dt(const Geom& g, const TcTiles& tl_in, const void* x, const 
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, k, g, tl, part, nslot, (const uint16_t*)x, (const uint16_t*)dy, dT, dTl, box, mx, mg);
+    return cudaLaunchKernelEx(&cfg, k, g, tl, part, nslot, (const uint16_t*)x, (const uint16_t*)dy, dT, dTl, box, pbox, mx, mg);
 }
 
 }  // namespace

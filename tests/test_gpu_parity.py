@@ -195,6 +195,31 @@ def test_table_gradient_of_large_maps_stays_on_the_tensor_cores(wb, oracle, B, C
     assert max_err_over_tol(dT, rdT, TOL["bf16"]) <= 1.0
 
 
+@pytest.mark.parametrize("case", [
+    si.Case("pb_14_w7", 16, 6, 14, 14, 7, seed=91, backward=True),                   # 392-byte planes, 4 windows per image
+    si.Case("pb_14_w7_shift", 24, 6, 14, 14, 7, shift=(3, 0), seed=92, backward=True),
+    si.Case("pb_14_w14", 72, 4, 14, 14, 14, seed=93, backward=True),                 # one window per image
+    si.Case("pb_14_w14_shift", 16, 6, 14, 14, 14, shift=(7, 4), seed=94, backward=True),
+    si.Case("pb_14_f16", 8, 10, 14, 14, 14, dtype="f16", seed=95, backward=True),
+    si.Case("pb_7x28_w7", 16, 4, 7, 28, 7, seed=96, backward=True),                  # 392-byte planes again, 1 x 4 windows
+], ids=lambda c: c.name)
+def test_planes_that_are_not_multiples_of_16_bytes(wb, oracle, case):
+    """14 x 14 and 7 x 7 maps: neither a bulk copy nor a tensor map with a channel dimension can address one plane;
+    the pipelined kernels load them as boxes of a map over [B][C*H*W] and store them with 8-byte stores."""
+    d = si.make(case, device="cuda")
+    y = wb.wbmm_forward(d["x"], d["T"], case.w, case.shift)
+    torch.cuda.synchronize()
+    assert wb.wbmm_last_path() == wb.PATH_TC_TMA, wb.wbmm_path_string(wb.wbmm_last_path())
+    dx, dT = wb.wbmm_backward(d["x"], d["T"], d["dy"], case.w, case.shift)
+    torch.cuda.synchronize()
+    assert wb.wbmm_last_path() == wb.PATH_TC_TMA, wb.wbmm_path_string(wb.wbmm_last_path())
+    ry = oracle.forward(widen(d["x"]), widen(d["T"]), case.w, case.shift)
+    rdx, rdT = oracle.backward(widen(d["x"]), widen(d["T"]), widen(d["dy"]), case.w, case.shift)
+    tol = TOL[case.dtype]
+    errs = (max_err_over_tol(y, ry, tol), max_err_over_tol(dx, rdx, tol), max_err_over_tol(dT, rdT, tol))
+    assert max(errs) <= 1.0, errs
+
+
 # ------------------------------------------------------------------ hierarchical reparameterisation (NEXT-1)
 def _hier_case(case):
     d = si.make(case, device="cuda")
