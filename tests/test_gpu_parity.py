@@ -556,6 +556,63 @@ def test_dT_accumulate_flag_and_run_to_run(wb, oracle):
     assert torch.allclose(acc, 2 * dT1, rtol=1e-5, atol=1e-5)
 
 
+def test_calls_from_two_threads_on_two_streams(wb, oracle):
+    """The library keeps per-process caches (tile schedules, shared-memory opt-ins, tensor-map encoder): calls from
+    two host threads on two streams, different shapes interleaved, must each give their own correct result."""
+    import threading
+    cases = [si.Case("mt_a", 24, 12, 56, 56, 14, seed=111, backward=True),
+             si.Case("mt_b", 40, 20, 28, 28, 14, shift=(7, 7), seed=112, backward=True)]
+    data = [si.make(c, device="cuda") for c in cases]
+    out = [None, None]
+
+    def work(i):
+        c, d = cases[i], data[i]
+        st = torch.cuda.Stream()
+        with torch.cuda.stream(st):
+            for _ in range(20):
+                y = wb.wbmm_forward(d["x"], d["T"], c.w, c.shift)
+                dx, dT = wb.wbmm_backward(d["x"], d["T"], d["dy"], c.w, c.shift)
+        st.synchronize()
+        out[i] = (y, dx, dT)
+
+    th = [threading.Thread(target=work, args=(i,)) for i in range(2)]
+    for t in th:
+        t.start()
+    for t in th:
+        t.join()
+    for c, d, (y, dx, dT) in zip(cases, data, out):
+        ry = oracle.forward(widen(d["x"]), widen(d["T"]), c.w, c.shift)
+        rdx, rdT = oracle.backward(widen(d["x"]), widen(d["T"]), widen(d["dy"]), c.w, c.shift)
+        tol = TOL[c.dtype]
+        assert max(max_err_over_tol(y, ry, tol), max_err_over_tol(dx, rdx, tol), max_err_over_tol(dT, rdT, tol)) <= 1.0
+
+
+def test_training_step_replays_from_a_cuda_graph(wb, oracle):
+    """Forward + backward (incl. the dT zeroing kernel, the NHWC scratch allocations and their programmatic
+    dependent launches) captured once and replayed: the replay must reproduce the oracle on NEW input values."""
+    for layout in (NCHW, NHWC):
+        case = si.Case("graph", 16, 16, 28, 56, 14, shift=(7, 7), layout=layout, seed=113, backward=True)
+        d = si.make(case, device="cuda")
+        x, dy = d["x"].clone(), d["dy"].clone()
+        y, dx = torch.empty_like(x), None
+        dT = torch.empty((case.C, case.bins), dtype=torch.float32, device="cuda")
+        wb.wbmm_forward(x, d["T"], case.w, case.shift, layout, out=y)            # warm-up outside the capture
+        wb.wbmm_backward(x, d["T"], dy, case.w, case.shift, layout, dT=dT)
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            wb.wbmm_forward(x, d["T"], case.w, case.shift, layout, out=y)
+            dx, _ = wb.wbmm_backward(x, d["T"], dy, case.w, case.shift, layout, dT=dT)
+        x.copy_(torch.flip(d["x"], dims=(0,)))                                   # new values in the captured buffers
+        dy.copy_(torch.flip(d["dy"], dims=(0,)))
+        g.replay()
+        torch.cuda.synchronize()
+        ry = oracle.forward(widen(x), widen(d["T"]), case.w, case.shift, layout)
+        rdx, rdT = oracle.backward(widen(x), widen(d["T"]), widen(dy), case.w, case.shift, layout)
+        tol = TOL[case.dtype]
+        assert max(max_err_over_tol(y, ry, tol), max_err_over_tol(dx, rdx, tol), max_err_over_tol(dT, rdT, tol)) <= 1.0
+
+
 def test_host_entry_points(wb, oracle):
     case = si.Case("host", 2, 5, 28, 30, 14, dtype="bf16", shift=(7, 7), seed=26, backward=True)
     d = si.make(case)
