@@ -278,7 +278,8 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
         b0 = it_gb * tl.NP;
         wy0 = it_strip * tl.NSY;
         np_eff = min(tl.NP, g.B - b0);
-        rows_eff = GEN ? g.H : min(tl.frame_rows, g.H - wy0 * WS);   // GEN: whole images (nstrips == 1)
+        // GEN: whole images (nstrips == 1), or the rolled rows of a strip (gstrip)
+        rows_eff = GEN ? (tl.nstrips == 1 ? g.H : min(tl.frame_rows, g.Hp - wy0 * WS)) : min(tl.frame_rows, g.H - wy0 * WS);
         if (++it_strip == tl.nstrips) {
             it_strip = 0;
             if (++it_gb == tl.ngb) {
@@ -315,6 +316,17 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                 const uint32_t kk = k + p;
                 const int slot = kk % nslot;
                 ptx::mbar_wait(EMPTY(slot), ((kk / nslot) & 1) ^ 1);
+                if (GEN && tl.nstrips > 1) {
+                    // strip of a shifted / ragged map: the rolled rows are up to two runs of image rows (none at all
+                    // when the strip lies in the padding: the barrier then completes on the arrival alone)
+                    const StripRuns sr = strip_runs(g, wy0 * WS, rows_eff);
+                    const uint16_t* pl0 = x + ((long long)(b0 + p) * g.C + c) * plane_elems;
+                    const uint32_t dst0 = ptx::smem_u32(ring + (size_t)slot * tl.S);
+                    ptx::mbar_arrive_expect_tx(FULL(slot), (uint32_t)(sr.nA + sr.nB) * rowB);
+                    if (sr.nA > 0) ptx::bulk_g2s(dst0, pl0 + (long long)sr.a0 * g.W, (uint32_t)sr.nA * rowB, FULL(slot));
+                    if (sr.nB > 0) ptx::bulk_g2s(dst0 + sr.n1 * rowB, pl0, (uint32_t)sr.nB * rowB, FULL(slot));
+                    continue;
+                }
                 ptx::mbar_arrive_expect_tx(FULL(slot), bytes);
                 if (p == 0) TRACE(0, (t - t0));
                 const uint16_t* src = x + ((long long)(b0 + p) * g.C + c) * plane_elems + (long long)wy0 * WS * g.W;
@@ -372,7 +384,11 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
         const int wyl = wl / g.nww, wx = wl % g.nww;
         const int win_off = wl < wpf ? ((wyl * WS) * g.W + wx * WS) * 2 : 0;   // lanes without a window read a legal address
         GenAddr<WG ? WS : 1> ga;
-        if constexpr (GEN) gen_addr_init<WS>(ga, g, wyl, wx);
+        const bool gstrip = GEN && tl.nstrips > 1;
+        if constexpr (GEN) {
+            if (gstrip) gen_addr_init_strip<WS>(ga, g, wyl, wx);
+            else gen_addr_init<WS>(ga, g, wyl, wx);
+        }
         else if constexpr (WG) gen_addr_init_plain<WS>(ga, g.W, wyl, wx);
         uint32_t k = 0, lt = 0;
         int cur_c = -1;
@@ -440,6 +456,9 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
             if (rt == 0) TRACE(4, lt);
             const bool part = wl < wpf && pl < np_eff;               // this thread's frame image was loaded
             const bool valid = part && wy0 + wyl < g.nwh;
+            if constexpr (GEN) {
+                if (gstrip && ragged) ga.rowmask = gen_strip_rowmask<WS>(g, wy0 + wyl);
+            }
             const uint32_t kk = k + pl;
             const int slot = kk % nslot;
             const int poff = sbox == 2 ? ((c * (int)plane_elems) & 7) * 2 : 0;    // plane boxes: offset of the plane in its slot
@@ -485,7 +504,11 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
         const int wyl = wl / g.nww, wx = wl % g.nww;
         const int win_off = ((wyl * WS) * g.W + wx * WS) * 2;
         GenAddr<WG ? WS : 1> ga;
-        if constexpr (GEN) gen_addr_init<WS>(ga, g, wyl, wx);
+        const bool gstrip = GEN && tl.nstrips > 1;
+        if constexpr (GEN) {
+            if (gstrip) gen_addr_init_strip<WS>(ga, g, wyl, wx);
+            else gen_addr_init<WS>(ga, g, wyl, wx);
+        }
         else if constexpr (WG) gen_addr_init_plain<WS>(ga, g.W, wyl, wx);
         const int gq = m / og.lanes;                    // output group of this thread
         const int pg = pl - gq * og.images;             // image inside the group
@@ -495,6 +518,9 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
             int c, b0, wy0, np_eff, rows_eff;
             tile_decode(t, c, b0, wy0, np_eff, rows_eff);
             const bool valid = pl < np_eff && wy0 + wyl < g.nwh;
+            if constexpr (GEN) {
+                if (gstrip && ragged) ga.rowmask = gen_strip_rowmask<WS>(g, wy0 + wyl);
+            }
             // the output frame is nout / og.n tiles deep: tile lt uses frame lt mod depth, group gq its buffer gq
             const uint32_t otile = lt % (nout / og.n), ob = otile * og.n + gq, use = lt / (nout / og.n);
             uint8_t* img = outb + (size_t)ob * out_bytes + (size_t)pg * tl.S;
@@ -600,8 +626,16 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                     if (p_first < p_end) ptx::tma_store_4d(&my, 0, 0, c, b0 + p_first, ptx::smem_u32(outb + (size_t)lane * out_bytes));
                 } else
                 for (int p = p_first; p < p_end; ++p) {
+                    const uint32_t src = ptx::smem_u32(outb + (size_t)lane * out_bytes + (size_t)(p - p_first) * tl.S);
+                    if (GEN && tl.nstrips > 1) {     // strip in rolled row order: up to two runs of image rows
+                        const StripRuns sr = strip_runs(g, wy0 * WS, rows_eff);
+                        uint16_t* pl0 = y + ((long long)(b0 + p) * g.C + c) * plane_elems;
+                        if (sr.nA > 0) ptx::bulk_s2g(pl0 + (long long)sr.a0 * g.W, src, (uint32_t)sr.nA * rowB);
+                        if (sr.nB > 0) ptx::bulk_s2g(pl0, src + sr.n1 * rowB, (uint32_t)sr.nB * rowB);
+                        continue;
+                    }
                     uint16_t* dst = y + ((long long)(b0 + p) * g.C + c) * plane_elems + (long long)wy0 * WS * g.W;
-                    ptx::bulk_s2g(dst, ptx::smem_u32(outb + (size_t)lane * out_bytes + (size_t)(p - p_first) * tl.S), bytes);
+                    ptx::bulk_s2g(dst, src, bytes);
                 }
                 ptx::bulk_commit();
                 ptx::bulk_wait_read<0>();
@@ -664,7 +698,8 @@ int bulk_mode(const Geom& g, const TcTiles& tl, const void* x, const void* y)
     if (plain && (pb || (tl.frame_rows * g.W * 2) % 16 == 0) && (WS % 2 == 0 || g.W % 2 == 0)) return 1;   // odd w: rows must be word-aligned
     // general form: whole images in natural layout, word-granular window addressing (W, W' even)
     // (an odd W' -- ragged maps at odd w -- is fine without a column shift: nothing wraps)
-    return (tl.nstrips == 1 && g.W % 2 == 0 && (g.Wp % 2 == 0 || g.sw == 0)) ? 2 : 0;
+    // maps cut into strips of window rows (more than 128 windows per image): rolled-order frames, rows of 16-byte multiples
+    return ((tl.nstrips == 1 || (g.W * 2) % 16 == 0) && g.W % 2 == 0 && (g.Wp % 2 == 0 || g.sw == 0)) ? 2 : 0;
 }
 
 // cuTensorMapEncodeTiled through the runtime's driver entry point (libcuda is not linked).

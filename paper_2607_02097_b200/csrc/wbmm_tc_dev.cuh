@@ -354,6 +354,44 @@ __device__ __forceinline__ void gen_addr_init(GenAddr<WS>& a, const Geom& g, int
     }
 }
 
+// General addressing on a STRIP of window rows (maps with more than 128 windows per image): the frame holds the
+// strip's rows in ROLLED order (frame row i = rolled row wy0*w + i, loaded as up to two runs of image rows), so the
+// row offsets are plain and only the columns wrap.  rowmask is per tile (gen_strip_rowmask).
+template <int WS>
+__device__ __forceinline__ void gen_addr_init_strip(GenAddr<WS>& a, const Geom& g, int wyl, int wx)
+{
+    gen_addr_init<WS>(a, g, 0, wx);                  // columns as in the whole-image form
+#pragma unroll
+    for (int r = 0; r < WS; ++r) a.rowoff[r] = (wyl * WS + r) * g.W * 2;
+    a.rowmask = 0xffffffffu;
+}
+template <int WS>
+__device__ __forceinline__ uint32_t gen_strip_rowmask(const Geom& g, int wy)
+{
+    uint32_t m = 0;
+#pragma unroll
+    for (int r = 0; r < WS; ++r) {
+        int h = wy * WS + r + g.sh;
+        if (h >= g.Hp) h -= g.Hp;
+        m |= (h < g.H ? 1u : 0u) << r;
+    }
+    return m;
+}
+// The (at most two) runs of image rows behind the n rolled rows that start at rolled row R0: run A = image rows
+// [a0, a0 + nA) -> frame row 0, run B = image rows [0, nB) -> frame row n1.  Rows at or beyond H (padding) are in
+// neither run.
+struct StripRuns { int a0, nA, n1, nB; };
+__device__ __forceinline__ StripRuns strip_runs(const Geom& g, int R0, int n)
+{
+    StripRuns s;
+    s.a0 = R0 + g.sh;
+    if (s.a0 >= g.Hp) s.a0 -= g.Hp;
+    s.n1 = min(n, g.Hp - s.a0);
+    s.nA = max(0, min(s.a0 + s.n1, g.H) - s.a0);
+    s.nB = min(n - s.n1, g.H);
+    return s;
+}
+
 // The same descriptor for the aligned form (no shift, no padding; frame rows relative to the strip):
 // used for odd w, whose window rows start on odd columns for every other window.
 template <int WS>

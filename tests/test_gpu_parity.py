@@ -104,6 +104,9 @@ PIPE = [
     si.Case("p_w14_strips", 3, 4, 168, 112, 14),                             # 96 windows per image: 2 images / tile
     si.Case("p_w14_big_map", 2, 3, 224, 224, 14),                            # 256 windows per image: row strips
     si.Case("p_w14_f16", 10, 9, 42, 56, 14, dtype="f16", shift=(0, 7)),
+    si.Case("p_w14_big_map_shift", 2, 3, 224, 224, 14, shift=(7, 7)),        # row strips in rolled order: two row runs
+    si.Case("p_w7_strips_shift", 3, 5, 112, 112, 7, shift=(3, 4)),
+    si.Case("p_w7_strips_ragged", 2, 4, 108, 112, 7, shift=(2, 0)),          # last strip partly in the padding
     si.Case("p_w7_plain", 21, 6, 56, 56, 7),                                 # 64 windows per image
     si.Case("p_w7_strips", 3, 5, 112, 112, 7),                               # 256 windows per image: strips
     si.Case("p_w7_shift", 5, 7, 28, 28, 7, shift=(3, 2)),
