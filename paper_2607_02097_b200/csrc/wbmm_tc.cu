@@ -172,7 +172,9 @@ struct BulkSmem {
     static constexpr int FIXED = (BulkCfg<WS>::WC_BYTES + BulkCfg<WS>::HIER_BYTES + TAB_BYTES + BAR_BYTES + 127) / 128 * 128;   // tensor-map boxes land 128-byte aligned
 };
 
-template <int WS, bool BF16, bool GEN>
+// STRIP (with GEN): general addressing on strips of window rows in rolled row order (maps with more than 128
+// windows per image); a template flag so that the whole-image general form pays nothing for it.
+template <int WS, bool BF16, bool GEN, bool STRIP>
 __global__ void __launch_bounds__(kThreadsB, 1)
 tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const uint16_t* __restrict__ x, const uint16_t* __restrict__ T,
                const uint16_t* __restrict__ Tl, uint16_t* __restrict__ y, int reverse, int box, int sbox,
@@ -279,7 +281,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
         wy0 = it_strip * tl.NSY;
         np_eff = min(tl.NP, g.B - b0);
         // GEN: whole images (nstrips == 1), or the rolled rows of a strip (gstrip)
-        rows_eff = GEN ? (tl.nstrips == 1 ? g.H : min(tl.frame_rows, g.Hp - wy0 * WS)) : min(tl.frame_rows, g.H - wy0 * WS);
+        rows_eff = GEN ? (!STRIP ? g.H : min(tl.frame_rows, g.Hp - wy0 * WS)) : min(tl.frame_rows, g.H - wy0 * WS);
         if (++it_strip == tl.nstrips) {
             it_strip = 0;
             if (++it_gb == tl.ngb) {
@@ -316,7 +318,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                 const uint32_t kk = k + p;
                 const int slot = kk % nslot;
                 ptx::mbar_wait(EMPTY(slot), ((kk / nslot) & 1) ^ 1);
-                if (GEN && tl.nstrips > 1) {
+                if constexpr (STRIP) {
                     // strip of a shifted / ragged map: the rolled rows are up to two runs of image rows (none at all
                     // when the strip lies in the padding: the barrier then completes on the arrival alone)
                     const StripRuns sr = strip_runs(g, wy0 * WS, rows_eff);
@@ -384,11 +386,8 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
         const int wyl = wl / g.nww, wx = wl % g.nww;
         const int win_off = wl < wpf ? ((wyl * WS) * g.W + wx * WS) * 2 : 0;   // lanes without a window read a legal address
         GenAddr<WG ? WS : 1> ga;
-        const bool gstrip = GEN && tl.nstrips > 1;
-        if constexpr (GEN) {
-            if (gstrip) gen_addr_init_strip<WS>(ga, g, wyl, wx);
-            else gen_addr_init<WS>(ga, g, wyl, wx);
-        }
+        if constexpr (STRIP) gen_addr_init_strip<WS>(ga, g, wyl, wx);
+        else if constexpr (GEN) gen_addr_init<WS>(ga, g, wyl, wx);
         else if constexpr (WG) gen_addr_init_plain<WS>(ga, g.W, wyl, wx);
         uint32_t k = 0, lt = 0;
         int cur_c = -1;
@@ -456,8 +455,8 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
             if (rt == 0) TRACE(4, lt);
             const bool part = wl < wpf && pl < np_eff;               // this thread's frame image was loaded
             const bool valid = part && wy0 + wyl < g.nwh;
-            if constexpr (GEN) {
-                if (gstrip && ragged) ga.rowmask = gen_strip_rowmask<WS>(g, wy0 + wyl);
+            if constexpr (STRIP) {
+                if (ragged) ga.rowmask = gen_strip_rowmask<WS>(g, wy0 + wyl);
             }
             const uint32_t kk = k + pl;
             const int slot = kk % nslot;
@@ -504,11 +503,8 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
         const int wyl = wl / g.nww, wx = wl % g.nww;
         const int win_off = ((wyl * WS) * g.W + wx * WS) * 2;
         GenAddr<WG ? WS : 1> ga;
-        const bool gstrip = GEN && tl.nstrips > 1;
-        if constexpr (GEN) {
-            if (gstrip) gen_addr_init_strip<WS>(ga, g, wyl, wx);
-            else gen_addr_init<WS>(ga, g, wyl, wx);
-        }
+        if constexpr (STRIP) gen_addr_init_strip<WS>(ga, g, wyl, wx);
+        else if constexpr (GEN) gen_addr_init<WS>(ga, g, wyl, wx);
         else if constexpr (WG) gen_addr_init_plain<WS>(ga, g.W, wyl, wx);
         const int gq = m / og.lanes;                    // output group of this thread
         const int pg = pl - gq * og.images;             // image inside the group
@@ -518,8 +514,8 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
             int c, b0, wy0, np_eff, rows_eff;
             tile_decode(t, c, b0, wy0, np_eff, rows_eff);
             const bool valid = pl < np_eff && wy0 + wyl < g.nwh;
-            if constexpr (GEN) {
-                if (gstrip && ragged) ga.rowmask = gen_strip_rowmask<WS>(g, wy0 + wyl);
+            if constexpr (STRIP) {
+                if (ragged) ga.rowmask = gen_strip_rowmask<WS>(g, wy0 + wyl);
             }
             // the output frame is nout / og.n tiles deep: tile lt uses frame lt mod depth, group gq its buffer gq
             const uint32_t otile = lt % (nout / og.n), ob = otile * og.n + gq, use = lt / (nout / og.n);
@@ -627,7 +623,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                 } else
                 for (int p = p_first; p < p_end; ++p) {
                     const uint32_t src = ptx::smem_u32(outb + (size_t)lane * out_bytes + (size_t)(p - p_first) * tl.S);
-                    if (GEN && tl.nstrips > 1) {     // strip in rolled row order: up to two runs of image rows
+                    if constexpr (STRIP) {           // strip in rolled row order: up to two runs of image rows
                         const StripRuns sr = strip_runs(g, wy0 * WS, rows_eff);
                         uint16_t* pl0 = y + ((long long)(b0 + p) * g.C + c) * plane_elems;
                         if (sr.nA > 0) ptx::bulk_s2g(pl0 + (long long)sr.a0 * g.W, src, (uint32_t)sr.nA * rowB);
@@ -802,11 +798,11 @@ int bulk_box_mode(const Geom& g, const TcTiles& tl, int dtype, const void* x, co
     return LB;
 }
 
-template <int WS, bool BF16, bool GEN>
+template <int WS, bool BF16, bool GEN, bool STRIP = false>
 cudaError_t launch_bulk(const Geom& g, const TcTiles& tl_in, const void* x, const void* T, const void* Tl, void* y,
                         bool reverse, cudaStream_t s, const void* bias, uint32_t ident_bits)
 {
-    auto k = tc_bulk_kernel<WS, BF16, GEN>;
+    auto k = tc_bulk_kernel<WS, BF16, GEN, STRIP>;
     int nslot = 0, nout = 0;
     TcTiles tl = tl_in;
     CUtensorMap mx, my;
@@ -1036,6 +1032,12 @@ cudaError_t tc_forward(const Geom& g, int dtype, const void* x, const void* T, c
     const int mode = g.w == 7 ? bulk_mode<7>(g, tl, x, y) : bulk_mode<14>(g, tl, x, y);
     if (mode != 0) {
         *path = WBMM_PATH_TC_TMA;
+        if (mode == 2 && tl.nstrips > 1) {      // general addressing on strips of window rows
+            if (g.w == 7) return bf ? launch_bulk<7, true, true, true>(g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits)
+                                    : launch_bulk<7, false, true, true>(g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
+            return bf ? launch_bulk<14, true, true, true>(g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits)
+                      : launch_bulk<14, false, true, true>(g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
+        }
         const int sel = (g.w == 7 ? 0 : 4) + (bf ? 2 : 0) + (mode == 2 ? 1 : 0);
         switch (sel) {
         case 0: return launch_bulk<7, false, false>(g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
