@@ -76,6 +76,8 @@ def ncu_traffic_bytes():
         line = line.split("#")[0].strip()
         if line.startswith("dram_bytes_per_launch"):
             return float(line.split("=")[1])
+        if line.isdigit():  # a bare number is the same figure
+            return float(line)
     return None
 
 
