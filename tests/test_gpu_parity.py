@@ -669,3 +669,14 @@ SWEEP_PICK = [c for c in SWEEP if c.B in (4, 64) or "ragged" in c.name]
 def test_config4_sweep(wb, oracle, case):
     err, _ = run_forward(wb, oracle, case, sample=(3, 4))
     assert err <= 1.0, err
+
+
+# the largest batch of the sweep (up to 308 M elements, 616 MB per tensor): sampled planes, both layouts
+SWEEP_MAX = [c for c in SWEEP if c.B == 256]
+
+
+@pytest.mark.parametrize("case", SWEEP_MAX, ids=lambda c: c.name)
+def test_config4_sweep_largest_batch(wb, oracle, case):
+    err, _ = run_forward(wb, oracle, case, sample=(4, 4))
+    assert err <= 1.0, err
+    torch.cuda.empty_cache()
