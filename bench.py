@@ -391,6 +391,21 @@ def run_wbmm(args, rank, world, local):
                   "hbm_frac_at_median": by5 / (statistics.median(t5) * 1e-3) / 1e9 / hbm_peak,
                   "note": "x, y, dy, dx = 154 MB against a 126 MB L2: partly L2-resident between launches"}
 
+    # the same step (forward, dX, dT zeroing, dT) replayed from one CUDA graph: device-side time, no host gaps
+    try:
+        dT5 = torch.empty((c5.C, c5.bins), dtype=torch.float32, device=dev)
+        torch.cuda.synchronize()
+        g5 = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g5):
+            wb.wbmm_forward(d5["x"], d5["T"], c5.w, c5.shift, out=y5)
+            wb.wbmm_backward(d5["x"], d5["T"], d5["dy"], c5.w, c5.shift, dT=dT5)
+        train_step["ms_graph"] = region_ms(g5.replay)
+        del g5
+    except Exception as e:  # capture not possible: the eager numbers stand
+        sys.stderr.write(f"train-step graph capture failed: {str(e)[:80]}\n")
+        torch.cuda.synchronize()
+        train_step["ms_graph"] = None
+
     # hierarchical reparameterisation, fused forward on the headline shape: context
     g_l = torch.Generator(device="cpu").manual_seed(77)
     Tl = (torch.randn((case.C, (case.w - 1) ** 2), generator=g_l) * 0.02).to(T.dtype).to(dev)
