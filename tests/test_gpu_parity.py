@@ -667,7 +667,9 @@ SWEEP_PICK = [c for c in SWEEP if c.B in (4, 64) or "ragged" in c.name]
 
 @pytest.mark.parametrize("case", SWEEP_PICK, ids=lambda c: c.name)
 def test_config4_sweep(wb, oracle, case):
-    err, _ = run_forward(wb, oracle, case, sample=(3, 4))
+    """Parity, and the dispatch: every sweep shape runs on the pipelined tcgen05 + TMA kernel (NHWC around it)."""
+    err, _ = run_forward(wb, oracle, case, sample=(3, 4),
+                         expect_path=wb.PATH_TC_TRANSPOSED if case.layout == NHWC else wb.PATH_TC_TMA)
     assert err <= 1.0, err
 
 
@@ -677,6 +679,7 @@ SWEEP_MAX = [c for c in SWEEP if c.B == 256]
 
 @pytest.mark.parametrize("case", SWEEP_MAX, ids=lambda c: c.name)
 def test_config4_sweep_largest_batch(wb, oracle, case):
-    err, _ = run_forward(wb, oracle, case, sample=(4, 4))
+    err, _ = run_forward(wb, oracle, case, sample=(4, 4),
+                         expect_path=wb.PATH_TC_TRANSPOSED if case.layout == NHWC else wb.PATH_TC_TMA)
     assert err <= 1.0, err
     torch.cuda.empty_cache()
