@@ -526,6 +526,71 @@ def run_sweep(args):
         del d, dx, dT
 
 
+# The paper's operator benchmark, Table 13 B=128 block: single A800, FP32,
+# 256 channels, kFPS read as 10^3 [256,H,W] maps per second.  Context, not the target: another machine, another
+# precision for the bf16 rows.  {w: {map side: (WBMM-C kFPS, WBMM-NC kFPS)}}
+PAPER_TABLE13_B128 = {
+    7: {7: (2016, 1582), 14: (566, 525), 28: (165, 161), 56: (42, 42), 112: (10.5, 10.5), 224: (2.66, 2.67)},
+    14: {14: (1276, 641), 28: (242, 199), 56: (63, 60), 112: (15.1, 14.9), 224: (3.83, 3.84)},
+}
+
+
+def run_paper_shapes(args):
+    """--paper-shapes: wbmm_forward on the shapes of the paper's own operator benchmark (B=128, C=256, maps 7^2 ..
+    224^2, windows 7 and 14), in bf16 and in fp32, one JSON line per case with kFPS = B / ms next to the paper's
+    A800 FP32 figures.  Values are drawn on the device (timing only; parity lives in tests/)."""
+    import paper_2607_02097_b200 as wb
+    torch.cuda.set_device(0)
+    stream = torch.cuda.current_stream()
+    hbm_peak, tc_peak, _ = measured_peaks()
+    B, C = 128, 256
+    gen = torch.Generator(device="cuda").manual_seed(1313)
+    for dtype, tdt in (("bf16", torch.bfloat16), ("f32", torch.float32)):
+        for w, maps in PAPER_TABLE13_B128.items():
+            for H, (kfps_c, kfps_nc) in maps.items():
+                x = torch.randn((B, C, H, H), generator=gen, device="cuda", dtype=torch.float32).to(tdt)
+                T = (torch.randn((C, (2 * w - 1) ** 2), generator=gen, device="cuda") * 0.02).to(tdt)
+                y = torch.empty_like(x)
+                f = lambda: wb.wbmm_forward(x, T, w, (0, 0), si.NCHW, out=y)
+                for _ in range(2):
+                    f()
+                torch.cuda.synchronize()
+                n = 3 if dtype == "f32" and H >= 112 else 10
+                ms = None
+                try:        # from a CUDA graph: device-side time (the small maps are host-bound when called eagerly)
+                    gr = torch.cuda.CUDAGraph()
+                    with torch.cuda.graph(gr):
+                        for _ in range(n):
+                            f()
+                    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    a.record(stream)
+                    gr.replay()
+                    b.record(stream)
+                    torch.cuda.synchronize()
+                    ms = a.elapsed_time(b) / n
+                    del gr
+                except Exception as e:
+                    sys.stderr.write(f"graph capture failed for H={H} w={w} {dtype}: {str(e)[:80]}\n")
+                    torch.cuda.synchronize()
+                    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    a.record(stream)
+                    for _ in range(n):
+                        f()
+                    b.record(stream)
+                    torch.cuda.synchronize()
+                    ms = a.elapsed_time(b) / n
+                es = 2 if dtype == "bf16" else 4
+                by = 2.0 * x.numel() * es + T.numel() * es
+                fl = 2.0 * w * w * x.numel()
+                print(json.dumps({"paper_case": f"B{B}_C{C}_H{H}_w{w}_{dtype}", "B": B, "C": C, "H": H, "w": w, "dtype": dtype,
+                                  "ms": round(ms, 5), "kfps": round(B / ms, 2), "tflops": round(fl / ms / 1e9, 2),
+                                  "gbs": round(by / ms / 1e6, 1), "frac_of_hbm_roofline": round(by / (hbm_peak * 1e9) * 1e3 / ms, 4),
+                                  "path": wb.wbmm_path_string(wb.wbmm_last_path()),
+                                  "paper_A800_fp32_kfps_cached": kfps_c, "paper_A800_fp32_kfps_not_cached": kfps_nc}), flush=True)
+                del x, y, T
+                torch.cuda.empty_cache()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -534,9 +599,14 @@ def main():
     ap.add_argument("--impl", default="wbmm", choices=["wbmm", "reference"])
     ap.add_argument("--sweep", action="store_true", help="time the config-4 operator sweep instead (one JSON line per case)")
     ap.add_argument("--ref-seconds", type=float, default=100.0, help="--impl reference: CPU seconds for the whole run")
+    ap.add_argument("--paper-shapes", action="store_true",
+                    help="time the shapes of the paper's Table 13 (B=128, C=256) in bf16 and fp32 (one JSON line per case)")
     args = ap.parse_args()
     if args.sweep:
         run_sweep(args)
+        return
+    if args.paper_shapes:
+        run_paper_shapes(args)
         return
     if args.impl == "reference":
         rank = int(os.environ.get("RANK", "0"))

@@ -74,7 +74,67 @@ __device__ __forceinline__ void stage_windows(const Geom& g, const E* __restrict
     }
 }
 
-template <typename E, int G>
+// Forward / dX staging without per-element 64-bit divisions: the G windows of a block are located once
+// (image, first row and column in the padded + shifted frame), an element then costs one division by the window side.
+struct WinBase {
+    int b, h0, v0;      // b = -1: beyond the last window
+};
+
+template <int G>
+__device__ __forceinline__ void window_bases(const Geom& g, long long win0, WinBase* wb)
+{
+    if (threadIdx.x < G) {
+        const long long win = win0 + threadIdx.x;
+        WinBase r;
+        r.b = -1;
+        r.h0 = r.v0 = 0;
+        if (win < g.nwin) {
+            const int per_img = g.nwh * g.nww;
+            r.b = (int)(win / per_img);
+            const int rr = (int)(win - (long long)r.b * per_img);
+            const int wy = rr / g.nww;
+            r.h0 = wy * g.w + g.sh;
+            r.v0 = (rr - wy * g.nww) * g.w + g.sw;
+        }
+        wb[threadIdx.x] = r;
+    }
+}
+
+// The element of window `b`, in-window position q (same result as window_elem).
+template <int WS>
+__device__ __forceinline__ long long window_elem_at(const Geom& g, const WinBase& b, int q, int c)
+{
+    const int w = WS ? WS : g.w;
+    const int qr = q / w;
+    int h = b.h0 + qr, v = b.v0 + (q - qr * w);
+    if (h >= g.Hp) h -= g.Hp;
+    if (v >= g.Wp) v -= g.Wp;
+    if (h >= g.H || v >= g.W) return -1;
+    return act_offset(g, b.b, c, h, v);
+}
+
+template <int G, int WS>
+__device__ __forceinline__ TileIndex decode_ws(const Geom& g, int idx, int CB)
+{
+    const int N = WS ? WS * WS : g.N;
+    TileIndex t;
+    if (g.layout == WBMM_LAYOUT_NCHW) {
+        const int r = idx / N;
+        t.q = idx - r * N;
+        t.cb = r / G;
+        t.g = r - t.cb * G;
+    } else {
+        const int r = idx / CB;
+        t.cb = idx - r * CB;
+        t.g = r / N;
+        t.q = r - t.g * N;
+    }
+    return t;
+}
+
+// WS: the window side when it is known at compile time (7, 14: the inner loop over a window row is unrolled, its
+// shared-memory loads issued ahead of the FFMAs), 0 = any side (read from g.w).
+template <typename E, int G, int WS>
 __global__ void __launch_bounds__(kThreads)
 simt_forward_kernel(Geom g, const E* __restrict__ x, const E* __restrict__ T, E* __restrict__ y,
                     int CB, int reverse)
@@ -93,50 +153,79 @@ simt_forward_kernel(Geom g, const E* __restrict__ x, const E* __restrict__ T, E*
         int ks = reverse ? g.nb - 1 - k : k;
         Ts[cb * nbp + k] = c < g.C ? to_f32(T[(long long)c * g.nb + ks]) : 0.f;
     }
-    stage_windows<E, G>(g, x, xs, win0, c0, CB);
+    __shared__ WinBase wbase[G];
+    window_bases<G>(g, win0, wbase);
+    __syncthreads();
+    const int total = CB * G * g.N;
+    for (int idx = threadIdx.x; idx < total; idx += kThreads) {
+        const TileIndex t = decode_ws<G, WS>(g, idx, CB);
+        const int c = c0 + t.cb;
+        float val = 0.f;
+        if (wbase[t.g].b >= 0 && c < g.C) {
+            const long long off = window_elem_at<WS>(g, wbase[t.g], t.q, c);
+            if (off >= 0) val = to_f32(x[off]);
+        }
+        xs[(t.cb * g.N + t.q) * G + t.g] = val;
+    }
     __syncthreads();
 
-    const int w = g.w, tw = g.tw;
-    for (int cb = 0; cb < CB; ++cb) {
+    // One unit = (channel of the block, pair of outputs p0 = pp and p1 = pp + ceil(N/2)): the two outputs share every
+    // broadcast load of the input windows (2 + G/4 shared-memory loads per 2G FFMA), and the units of all CB channels
+    // are spread over the threads, so that a 7 x 7 window (25 pairs) does not leave most of the block idle.
+    const int w = WS ? WS : g.w, tw = 2 * w - 1;
+    const int NH = (g.N + 1) / 2;
+    for (int u = threadIdx.x; u < CB * NH; u += kThreads) {
+        const int cb = u / NH, pp = u - cb * NH;
         const float* xc = xs + cb * g.N * G;
-        for (int p = threadIdx.x; p < g.N; p += kThreads) {
-            const int rp = p / w, cp = p % w;
-            // Eq. 7 with i = p (output), j = q (input): idx = (rp-rq+w-1)*tw + (cp-cq+w-1)
-            const float* Tc = Ts + cb * nbp + (rp + w - 1) * tw + cp + w - 1;
-            float acc[G];
+        const int p0 = pp, p1 = pp + NH;
+        const bool has1 = p1 < g.N;                    // odd N: the last pair has one output
+        const int p1c = has1 ? p1 : p0;
+        // Eq. 7 with i = p (output), j = q (input): idx = (rp-rq+w-1)*tw + (cp-cq+w-1)
+        const float* Tc0 = Ts + cb * nbp + (p0 / w + w - 1) * tw + p0 % w + w - 1;
+        const float* Tc1 = Ts + cb * nbp + (p1c / w + w - 1) * tw + p1c % w + w - 1;
+        float acc0[G], acc1[G];
 #pragma unroll
-            for (int k = 0; k < G; ++k) acc[k] = 0.f;
-            for (int rq = 0; rq < w; ++rq) {
-                const float* Tr = Tc - rq * tw;
-                const float4* xr = reinterpret_cast<const float4*>(xc + rq * w * G);
-                for (int cq = 0; cq < w; ++cq) {
-                    const float t = Tr[-cq];
+        for (int k = 0; k < G; ++k) acc0[k] = acc1[k] = 0.f;
+        for (int rq = 0; rq < w; ++rq) {
+            const float* Tr0 = Tc0 - rq * tw;
+            const float* Tr1 = Tc1 - rq * tw;
+            const float4* xr = reinterpret_cast<const float4*>(xc + rq * w * G);
+#pragma unroll (WS ? WS : 1)
+            for (int cq = 0; cq < w; ++cq) {
+                const float t0 = Tr0[-cq], t1 = Tr1[-cq];
 #pragma unroll
-                    for (int k4 = 0; k4 < G / 4; ++k4) {
-                        float4 xv = xr[cq * (G / 4) + k4];
-                        acc[4 * k4 + 0] = fmaf(t, xv.x, acc[4 * k4 + 0]);
-                        acc[4 * k4 + 1] = fmaf(t, xv.y, acc[4 * k4 + 1]);
-                        acc[4 * k4 + 2] = fmaf(t, xv.z, acc[4 * k4 + 2]);
-                        acc[4 * k4 + 3] = fmaf(t, xv.w, acc[4 * k4 + 3]);
-                    }
+                for (int k4 = 0; k4 < G / 4; ++k4) {
+                    float4 xv = xr[cq * (G / 4) + k4];
+                    acc0[4 * k4 + 0] = fmaf(t0, xv.x, acc0[4 * k4 + 0]);
+                    acc0[4 * k4 + 1] = fmaf(t0, xv.y, acc0[4 * k4 + 1]);
+                    acc0[4 * k4 + 2] = fmaf(t0, xv.z, acc0[4 * k4 + 2]);
+                    acc0[4 * k4 + 3] = fmaf(t0, xv.w, acc0[4 * k4 + 3]);
+                    acc1[4 * k4 + 0] = fmaf(t1, xv.x, acc1[4 * k4 + 0]);
+                    acc1[4 * k4 + 1] = fmaf(t1, xv.y, acc1[4 * k4 + 1]);
+                    acc1[4 * k4 + 2] = fmaf(t1, xv.z, acc1[4 * k4 + 2]);
+                    acc1[4 * k4 + 3] = fmaf(t1, xv.w, acc1[4 * k4 + 3]);
                 }
             }
-            float4* yo = reinterpret_cast<float4*>(ys + (cb * g.N + p) * G);
+        }
+        float4* yo0 = reinterpret_cast<float4*>(ys + (cb * g.N + p0) * G);
+#pragma unroll
+        for (int k4 = 0; k4 < G / 4; ++k4)
+            yo0[k4] = make_float4(acc0[4 * k4], acc0[4 * k4 + 1], acc0[4 * k4 + 2], acc0[4 * k4 + 3]);
+        if (has1) {
+            float4* yo1 = reinterpret_cast<float4*>(ys + (cb * g.N + p1) * G);
 #pragma unroll
             for (int k4 = 0; k4 < G / 4; ++k4)
-                yo[k4] = make_float4(acc[4 * k4], acc[4 * k4 + 1], acc[4 * k4 + 2], acc[4 * k4 + 3]);
+                yo1[k4] = make_float4(acc1[4 * k4], acc1[4 * k4 + 1], acc1[4 * k4 + 2], acc1[4 * k4 + 3]);
         }
     }
     __syncthreads();
 
     // Un-partition: an output of the shifted frame returns to the element its input came from.
-    const int total = CB * G * g.N;
     for (int idx = threadIdx.x; idx < total; idx += kThreads) {
-        TileIndex t = decode<G>(g, idx, CB);
-        long long win = win0 + t.g;
-        int c = c0 + t.cb;
-        if (win < g.nwin && c < g.C) {
-            long long off = window_elem(g, win, t.q, c);
+        const TileIndex t = decode_ws<G, WS>(g, idx, CB);
+        const int c = c0 + t.cb;
+        if (wbase[t.g].b >= 0 && c < g.C) {
+            const long long off = window_elem_at<WS>(g, wbase[t.g], t.q, c);
             if (off >= 0) y[off] = from_f32<E>(ys[(t.cb * g.N + t.q) * G + t.g]);
         }
     }
@@ -250,26 +339,49 @@ TileCfg tile_cfg(const Geom& g)
     return t;
 }
 
+// Forward / dX: channels per block chosen so that the (channel, output pair) units fill the 256 threads
+// (w = 7: 25 pairs, 10 channels = 250 units), within 48 KB of shared memory so that four or more blocks
+// stay resident (w = 14: 98 pairs, 2 channels = 196 units).  The table-gradient kernel keeps tile_cfg.
+TileCfg tile_cfg_fwd(const Geom& g)
+{
+    TileCfg t = tile_cfg(g);
+    if (g.layout != WBMM_LAYOUT_NCHW) return t;
+    const size_t per_c = t.smem_fwd / t.CB;
+    const int NH = (g.N + 1) / 2;
+    int best = 1;
+    double best_eff = 0.0;
+    for (int cb = 1; cb <= 16 && cb <= g.C; ++cb) {
+        if (cb > 1 && cb * per_c > 48 * 1024) break;
+        const int units = cb * NH;
+        const double eff = (double)units / (double)((units + kThreads - 1) / kThreads * kThreads);
+        if (eff > best_eff + 1e-9) { best_eff = eff; best = cb; }
+    }
+    t.CB = best;
+    t.smem_fwd = per_c * best;
+    return t;
+}
+
 constexpr size_t kMaxSmem = 227 * 1024;
 
 template <typename E>
 cudaError_t forward_t(const Geom& g, const E* x, const E* T, E* y, bool reverse, cudaStream_t s)
 {
-    TileCfg t = tile_cfg(g);
+    TileCfg t = tile_cfg_fwd(g);
     dim3 grid((unsigned)((g.nwin + t.G - 1) / t.G), (unsigned)((g.C + t.CB - 1) / t.CB));
-    cudaError_t e;
+    auto launch = [&](auto k) -> cudaError_t {
+        cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t.smem_fwd);
+        if (e != cudaSuccess) return e;
+        k<<<grid, kThreads, t.smem_fwd, s>>>(g, x, T, y, t.CB, reverse ? 1 : 0);
+        return cudaGetLastError();
+    };
     if (t.G == 8) {
-        auto k = simt_forward_kernel<E, 8>;
-        e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t.smem_fwd);
-        if (e != cudaSuccess) return e;
-        k<<<grid, kThreads, t.smem_fwd, s>>>(g, x, T, y, t.CB, reverse ? 1 : 0);
-    } else {
-        auto k = simt_forward_kernel<E, 4>;
-        e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)t.smem_fwd);
-        if (e != cudaSuccess) return e;
-        k<<<grid, kThreads, t.smem_fwd, s>>>(g, x, T, y, t.CB, reverse ? 1 : 0);
+        if (g.w == 14) return launch(simt_forward_kernel<E, 8, 14>);
+        if (g.w == 7) return launch(simt_forward_kernel<E, 8, 7>);
+        return launch(simt_forward_kernel<E, 8, 0>);
     }
-    return cudaGetLastError();
+    if (g.w == 14) return launch(simt_forward_kernel<E, 4, 14>);
+    if (g.w == 7) return launch(simt_forward_kernel<E, 4, 7>);
+    return launch(simt_forward_kernel<E, 4, 0>);
 }
 
 template <typename E>
@@ -304,7 +416,7 @@ cudaError_t grad_table_t(const Geom& g, const E* x, const E* dy, float* dT, cuda
 
 bool simt_supported(const Geom& g)
 {
-    TileCfg t = tile_cfg(g);
+    TileCfg t = tile_cfg(g);       // tile_cfg_fwd falls back to this size when more channels do not fit
     return t.smem_fwd <= kMaxSmem && g.C <= 65535ll * t.CB && (g.nwin + t.G - 1) / t.G <= 0x7fffffffll;
 }
 
