@@ -169,30 +169,31 @@ simt_forward_kernel(Geom g, const E* __restrict__ x, const E* __restrict__ T, E*
     }
     __syncthreads();
 
-    // One unit = (channel of the block, pair of outputs p0 = pp and p1 = pp + ceil(N/2)): the two outputs share every
-    // broadcast load of the input windows (2 + G/4 shared-memory loads per 2G FFMA), and the units of all CB channels
-    // are spread over the threads, so that a 7 x 7 window (25 pairs) does not leave most of the block idle.
+    // One unit = (channel of the block, two outputs side by side in a window row: p0 = (rp, cp0), p1 = (rp, cp0 + 1)).
+    // The two outputs share every broadcast load of the input windows, and the table entry p1 needs at input column
+    // cq is the one p0 used at cq - 1 (Eq. 7 depends on cp - cq only), so a row of the window costs w + 1 table loads
+    // for both outputs: (w + 1) + w * G/4 shared-memory loads per 2 * w * G FFMA.  The units of all CB channels are
+    // spread over the threads, so that a 7 x 7 window (28 units) does not leave most of the block idle.
     const int w = WS ? WS : g.w, tw = 2 * w - 1;
-    const int NH = (g.N + 1) / 2;
-    for (int u = threadIdx.x; u < CB * NH; u += kThreads) {
-        const int cb = u / NH, pp = u - cb * NH;
+    const int WH = (w + 1) / 2, NU = w * WH;
+    for (int u = threadIdx.x; u < CB * NU; u += kThreads) {
+        const int cb = u / NU, pp = u - cb * NU;
+        const int rp = pp / WH, cp0 = 2 * (pp - rp * WH);
+        const bool has1 = cp0 + 1 < w;                 // odd w: the last unit of a row has one output
+        const int p0 = rp * w + cp0;
         const float* xc = xs + cb * g.N * G;
-        const int p0 = pp, p1 = pp + NH;
-        const bool has1 = p1 < g.N;                    // odd N: the last pair has one output
-        const int p1c = has1 ? p1 : p0;
         // Eq. 7 with i = p (output), j = q (input): idx = (rp-rq+w-1)*tw + (cp-cq+w-1)
-        const float* Tc0 = Ts + cb * nbp + (p0 / w + w - 1) * tw + p0 % w + w - 1;
-        const float* Tc1 = Ts + cb * nbp + (p1c / w + w - 1) * tw + p1c % w + w - 1;
+        const float* Tc0 = Ts + cb * nbp + (rp + w - 1) * tw + cp0 + w - 1;
         float acc0[G], acc1[G];
 #pragma unroll
         for (int k = 0; k < G; ++k) acc0[k] = acc1[k] = 0.f;
         for (int rq = 0; rq < w; ++rq) {
             const float* Tr0 = Tc0 - rq * tw;
-            const float* Tr1 = Tc1 - rq * tw;
             const float4* xr = reinterpret_cast<const float4*>(xc + rq * w * G);
+            float t1 = has1 ? Tr0[1] : 0.f;            // p1 at cq = 0
 #pragma unroll (WS ? WS : 1)
             for (int cq = 0; cq < w; ++cq) {
-                const float t0 = Tr0[-cq], t1 = Tr1[-cq];
+                const float t0 = Tr0[-cq];
 #pragma unroll
                 for (int k4 = 0; k4 < G / 4; ++k4) {
                     float4 xv = xr[cq * (G / 4) + k4];
@@ -205,6 +206,7 @@ simt_forward_kernel(Geom g, const E* __restrict__ x, const E* __restrict__ T, E*
                     acc1[4 * k4 + 2] = fmaf(t1, xv.z, acc1[4 * k4 + 2]);
                     acc1[4 * k4 + 3] = fmaf(t1, xv.w, acc1[4 * k4 + 3]);
                 }
+                t1 = t0;                               // p1 at cq + 1 reads what p0 read at cq
             }
         }
         float4* yo0 = reinterpret_cast<float4*>(ys + (cb * g.N + p0) * G);
@@ -212,7 +214,7 @@ simt_forward_kernel(Geom g, const E* __restrict__ x, const E* __restrict__ T, E*
         for (int k4 = 0; k4 < G / 4; ++k4)
             yo0[k4] = make_float4(acc0[4 * k4], acc0[4 * k4 + 1], acc0[4 * k4 + 2], acc0[4 * k4 + 3]);
         if (has1) {
-            float4* yo1 = reinterpret_cast<float4*>(ys + (cb * g.N + p1) * G);
+            float4* yo1 = yo0 + G / 4;
 #pragma unroll
             for (int k4 = 0; k4 < G / 4; ++k4)
                 yo1[k4] = make_float4(acc1[4 * k4], acc1[4 * k4 + 1], acc1[4 * k4 + 2], acc1[4 * k4 + 3]);
@@ -340,14 +342,14 @@ TileCfg tile_cfg(const Geom& g)
 }
 
 // Forward / dX: channels per block chosen so that the (channel, output pair) units fill the 256 threads
-// (w = 7: 25 pairs, 10 channels = 250 units), within 48 KB of shared memory so that four or more blocks
+// (w = 7: 28 units per channel, 9 channels = 252 units), within 48 KB of shared memory so that four or more blocks
 // stay resident (w = 14: 98 pairs, 2 channels = 196 units).  The table-gradient kernel keeps tile_cfg.
 TileCfg tile_cfg_fwd(const Geom& g)
 {
     TileCfg t = tile_cfg(g);
     if (g.layout != WBMM_LAYOUT_NCHW) return t;
     const size_t per_c = t.smem_fwd / t.CB;
-    const int NH = (g.N + 1) / 2;
+    const int NH = g.w * ((g.w + 1) / 2);      // units per channel: pairs of neighbouring outputs, row by row
     int best = 1;
     double best_eff = 0.0;
     for (int cb = 1; cb <= 16 && cb <= g.C; ++cb) {
