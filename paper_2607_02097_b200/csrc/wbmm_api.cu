@@ -137,6 +137,13 @@ int apply(const wbmm_desc_t* d, const wbmm::Geom& g, const void* x, const void* 
         t_last_path = path;
         return WBMM_STATUS_OK;
     }
+    if (d->dtype == WBMM_DTYPE_F32 && !(d->flags & WBMM_FLAG_FORCE_SIMT) && wbmm::tc_f32_supported(g, x, y)) {
+        e = wbmm::tc_f32_forward(g, x, T, y, reverse, stream, &launches);
+        g_launches += launches;
+        if (e != cudaSuccess) return set_cuda_error(e, "tc_f32_forward");
+        t_last_path = WBMM_PATH_TC_TMA;
+        return WBMM_STATUS_OK;
+    }
     if (!wbmm::simt_supported(g)) return WBMM_STATUS_UNSUPPORTED;
     e = wbmm::simt_forward(g, d->dtype, x, T, y, reverse, stream, &launches);
     g_launches += launches;

@@ -339,42 +339,51 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
         }
     } else if (warp == 1) {
         // ------------------------------------------------------------------ MMA issuer
-        if (lane == 0) {
+        // The whole warp walks the loop and one elected lane issues: the compiler then keeps the operands in uniform
+        // registers and emits the tcgen05.mma of a half back to back (issued from inside `if (lane == 0)` every
+        // instruction sat in its own elect-and-retry loop behind a rebuilt descriptor, ~75 cycles per issue).  The
+        // descriptors differ from a base value by compile-time constants in their 14-bit address field.
+        {
             const uint32_t wc_addr = ptx::smem_u32(Wc);
+            const uint64_t bd0 = ptx::smem_desc_kmajor_noswz(wc_addr, Bc::LBO, 128);
+            const uint32_t b_hi = (uint32_t)(bd0 >> 32), b_lo = (uint32_t)bd0;
             uint32_t lt = 0;
             for (int t = t0; t < t1; ++t, ++lt) {
                 const uint32_t buf = lt & 1;
                 ptx::mbar_wait(A_FULL + 8 * buf, (lt >> 1) & 1);
-                TRACE(1, lt);
+                if (lane == 0) TRACE(1, lt);
                 const uint32_t tmem_a = tmem + buf * A_STRIDE;
 #pragma unroll
                 for (int h = 0; h < Hs::NH; ++h) {
                     ptx::mbar_wait(D_EMPTY + 8 * h, (lt & 1) ^ 1);      // the epilogue has drained this half of tile lt-1
-                    if (h == 0) TRACE(2, lt);
+                    if (h == 0 && lane == 0) TRACE(2, lt);
                     ptx::tc_fence_after_sync();
-                    const uint32_t idesc = ptx::idesc_f16(BF16 ? 1 : 0, 128, Hs::ncols(h));
+                    if (ptx::elect_one()) {
+                        const uint32_t idesc = ptx::idesc_f16(BF16 ? 1 : 0, 128, Hs::ncols(h));
 #pragma unroll
-                    for (int ks = 0; ks < Bc::KSTEPS; ++ks) {
-                        uint64_t bdesc = ptx::smem_desc_kmajor_noswz(wc_addr + Bc::b_off(ks, h), Bc::LBO, 128);
+                        for (int ks = 0; ks < Bc::KSTEPS; ++ks) {
+                            uint64_t bdesc = ((uint64_t)b_hi << 32) | (b_lo + (uint32_t)(Bc::b_off(ks, h) >> 4));
+                            if constexpr (Bc::TOEP) {
+                                if (is_hier && ks / 7 == h)     // input and output rows in the same half: global + local blocks
+                                    bdesc = ptx::smem_desc_kmajor_noswz(wc_addr + Bc::WC_BYTES + Bc::b_off_a(ks, h), Bc::LBO_A, 128);
+                            }
+                            ptx::mma_ts(tmem_d + Hs::col0(h), tmem_a + ks * 8, bdesc, idesc, ks > 0 ? 1u : 0u);
+                        }
                         if constexpr (Bc::TOEP) {
-                            if (is_hier && ks / 7 == h)     // input and output rows in the same half: global + local blocks
-                                bdesc = ptx::smem_desc_kmajor_noswz(wc_addr + Bc::WC_BYTES + Bc::b_off_a(ks, h), Bc::LBO_A, 128);
-                        }
-                        ptx::mma_ts(tmem_d + Hs::col0(h), tmem_a + ks * 8, bdesc, idesc, ks > 0 ? 1u : 0u);
-                    }
-                    if constexpr (Bc::TOEP) {
-                        if (use_I) {        // + ident * x: output row ri takes input row ri through the ident*I block
-                            const uint32_t idesc_i = ptx::idesc_f16(BF16 ? 1 : 0, 128, 16);
-                            const uint64_t idn = ptx::smem_desc_kmajor_noswz(wc_addr + Bc::WC_BYTES + Bc::LIBA_BYTES, Bc::LBO_I, 128);
+                            if (use_I) {        // + ident * x: output row ri takes input row ri through the ident*I block
+                                const uint32_t idesc_i = ptx::idesc_f16(BF16 ? 1 : 0, 128, 16);
+                                const uint64_t idn = ptx::smem_desc_kmajor_noswz(wc_addr + Bc::WC_BYTES + Bc::LIBA_BYTES, Bc::LBO_I, 128);
 #pragma unroll
-                            for (int ri = 7 * h; ri < 7 * h + 7; ++ri)
-                                ptx::mma_ts(tmem_d + ri * 16, tmem_a + ri * 8, idn, idesc_i, 1u);
+                                for (int ri = 7 * h; ri < 7 * h + 7; ++ri)
+                                    ptx::mma_ts(tmem_d + ri * 16, tmem_a + ri * 8, idn, idesc_i, 1u);
+                            }
                         }
+                        ptx::mma_commit(D_FULL + 8 * h);
+                        if (h == Hs::NH - 1) ptx::mma_commit(A_EMPTY + 8 * buf);
                     }
-                    ptx::mma_commit(D_FULL + 8 * h);
+                    __syncwarp();
                 }
-                ptx::mma_commit(A_EMPTY + 8 * buf);
-                TRACE(3, lt);
+                if (lane == 0) TRACE(3, lt);
             }
         }
     } else if (warp < 6) {

@@ -37,6 +37,11 @@ cudaError_t tc_forward_matrix(const Geom& g, int dtype, const void* x, const voi
 // True when the pipelined bulk kernel (not the gather fallback) serves this NCHW problem.
 bool tc_bulk_supported(const Geom& g, int dtype, const void* x, const void* y);
 
+// FP32 forward / dX on the tensor cores: exact 3-way bf16 splitting, six tcgen05 passes (wbmm_tc_f32.cu).  NCHW, w in {7, 14}.
+bool tc_f32_supported(const Geom& g, const void* x, const void* y);
+cudaError_t tc_f32_forward(const Geom& g, const void* x, const void* T, void* y, bool reverse, cudaStream_t stream,
+                           int* launches);
+
 // NHWC forward / dX: 8-channel groups gathered with 16-byte cp.async (wbmm_tc_nhwc.cu).
 bool tc_nhwc_supported(const Geom& g, int dtype, const void* x, const void* y);
 cudaError_t tc_nhwc_forward(const Geom& g, int dtype, const void* x, const void* T, void* y, bool reverse,

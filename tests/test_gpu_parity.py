@@ -473,10 +473,64 @@ def test_hier_unsupported_shapes_fail_loudly(wb):
 
 
 def test_config1_fp32_tiny(wb, oracle):
-    """BASELINE.json config 1: fp32 path, <= 1e-4."""
+    """BASELINE.json config 1: fp32 path, <= 1e-4 -- on the tensor cores (3-way bf16 split) and on the FFMA kernel."""
     err, path = run_forward(wb, oracle, si.CFG1)
     assert err <= 1.0, err
+    assert path == wb.PATH_TC_TMA
+    err, path = run_forward(wb, oracle, si.CFG1, wb.FLAG_FORCE_SIMT)
+    assert err <= 1.0, err
     assert path == wb.PATH_SIMT
+
+
+# ------------------------------------------------------------------ fp32 on the tensor cores (NEXT-4)
+F32_TC = [
+    si.Case("f32_w14_plain", 19, 5, 56, 56, 14, dtype="f32", seed=201),              # 8 images per tile, tail of 3
+    si.Case("f32_w14_many", 40, 150, 28, 28, 14, dtype="f32", seed=202),             # 32 images per tile, > 148 tiles
+    si.Case("f32_w14_shift", 9, 7, 28, 56, 14, dtype="f32", shift=(7, 5), seed=203),
+    si.Case("f32_w14_ragged", 7, 6, 60, 60, 14, dtype="f32", seed=204),              # 25 windows per image, W' = 70
+    si.Case("f32_w14_ragged_shift", 6, 5, 36, 40, 14, dtype="f32", shift=(5, 9), seed=205),
+    si.Case("f32_w14_two_images", 5, 4, 112, 112, 14, dtype="f32", seed=206),        # 64 windows per image
+    si.Case("f32_w14_strips", 2, 3, 224, 224, 14, dtype="f32", seed=207),            # 256 windows per image: row strips
+    si.Case("f32_w7_plain", 21, 6, 56, 56, 7, dtype="f32", seed=208),
+    si.Case("f32_w7_shift", 5, 7, 28, 28, 7, dtype="f32", shift=(3, 2), seed=209),
+    si.Case("f32_w7_ragged", 6, 4, 26, 30, 7, dtype="f32", shift=(0, 3), seed=210),
+    si.Case("f32_w7_strips", 3, 5, 112, 112, 7, dtype="f32", seed=211),
+    si.Case("f32_w7_tiny_maps", 70, 6, 14, 14, 7, dtype="f32", seed=212),            # 784-byte planes, 32 images per tile
+]
+
+
+@pytest.mark.parametrize("case", F32_TC, ids=lambda c: c.name)
+def test_fp32_tensor_core_path(wb, oracle, case):
+    """fp32 forward and dX through six bf16 tensor passes (exact 3-way splits of windows and table): the paper's
+    precision at the 1e-4 bar of BASELINE.json -- and far inside it: dropping any of the three
+    2^-16-weight cross terms would leave ~2e-6, the full expansion measures ~2.5e-7 (fp32 accumulation)."""
+    d = si.make(case, device="cuda")
+    y = wb.wbmm_forward(d["x"], d["T"], case.w, case.shift)
+    assert wb.wbmm_last_path() == wb.PATH_TC_TMA, wb.wbmm_path_string(wb.wbmm_last_path())
+    dx, _ = wb.wbmm_backward(None, d["T"], d["x"], case.w, case.shift, need_dT=False)
+    assert wb.wbmm_last_path() == wb.PATH_TC_TMA
+    ry = oracle.forward(widen(d["x"]), widen(d["T"]), case.w, case.shift)
+    rdx, _ = oracle.backward(widen(d["x"]), widen(d["T"]), widen(d["x"]), case.w, case.shift, need_dT=False)
+    assert max_err_over_tol(y, ry, 1e-6) <= 1.0 and max_err_over_tol(dx, rdx, 1e-6) <= 1.0
+
+
+def test_fp32_tensor_core_path_one_hot_bins_bitwise(wb, oracle):
+    """One-hot tables through the fp32 tensor-core kernel: x1 + x2 + x3 is x exactly and the only non-zero weight is
+    1.0, so the result must equal the oracle's bitwise at every bin -- indexing of the three libraries, of the
+    window splits and of the staged row-run stores."""
+    for w, H, W, shift in ((14, 28, 56, (0, 0)), (14, 30, 44, (5, 9)), (7, 28, 28, (0, 0)), (7, 26, 30, (3, 2))):
+        tw = 2 * w - 1
+        nb = tw * tw
+        C = 64
+        case = si.Case("f32_onehot", 9, C, H, W, w, dtype="f32", shift=shift, seed=213)
+        d = si.make(case, device="cuda")
+        bins = torch.randint(0, nb, (C,), generator=torch.Generator().manual_seed(w * 100 + H))
+        bins[0], bins[1], bins[2] = 0, nb - 1, (w - 1) * tw + (w - 1)
+        T = torch.zeros_like(d["T"])
+        T[torch.arange(C), bins.to(T.device)] = 1.0
+        y = wb.wbmm_forward(d["x"], T, w, shift)
+        assert wb.wbmm_last_path() == wb.PATH_TC_TMA
+        assert np.array_equal(widen(y), oracle.forward(widen(d["x"]), widen(T), w, shift))
 
 
 # ------------------------------------------------------------------ exact structured tests
