@@ -192,6 +192,48 @@ def time_oracle(case: si.Case, target_s: float = 12.0):
     return flops_of(sub) / dt / 1e12, wbmm_ref.num_threads(), sample, dt
 
 
+def oracle_legs(case3: si.Case, case5: si.Case, budget_s: float = 4.0):
+    """BASELINE.md section 3 context rows, each on a bounded sample: the oracle on ONE core, the matrix form
+    (Alg. 1 with a materialised M) on config 3, and the config-5 training step (forward + dX + dT)."""
+    from oracle import wbmm_ref
+    out = {}
+    ncores = wbmm_ref.num_threads()
+    per_image, T = oracle_probe(case3)           # all cores
+    # one core
+    nb1 = int(max(1, min(case3.B, budget_s / max(per_image * ncores, 1e-6))))
+    sub = si.with_(case3, B=nb1)
+    xs = si.make(sub)["x"].double().numpy()
+    wbmm_ref.set_threads(1)
+    t0 = time.perf_counter()
+    wbmm_ref.forward(xs, T, case3.w, case3.shift, case3.layout, "direct")
+    dt = time.perf_counter() - t0
+    wbmm_ref.set_threads(ncores)
+    out["cfg3_direct_1core"] = {"value": flops_of(sub) / dt / 1e12, "unit": UNIT, "cores": 1, "seconds": dt,
+                                "sample": f"first {nb1} of {case3.B} images, all {case3.C} channels"}
+    # matrix form, all cores
+    nbm = int(max(1, min(case3.B, budget_s / max(per_image, 1e-6))))
+    sub = si.with_(case3, B=nbm)
+    xs = si.make(sub)["x"].double().numpy()
+    t0 = time.perf_counter()
+    wbmm_ref.forward(xs, T, case3.w, case3.shift, case3.layout, "matrix")
+    dt = time.perf_counter() - t0
+    out["cfg3_matrix_form"] = {"value": flops_of(sub) / dt / 1e12, "unit": UNIT, "cores": ncores, "seconds": dt,
+                               "sample": f"first {nbm} of {case3.B} images, all {case3.C} channels"}
+    # config 5: forward + backward (dX, dT), all cores
+    per5, T5 = oracle_probe(case5)
+    nb5 = int(max(1, min(case5.B, budget_s / max(3 * per5, 1e-6))))
+    sub = si.with_(case5, B=nb5)
+    d = si.make(sub)
+    x5, g5 = d["x"].double().numpy(), d["dy"].double().numpy()
+    t0 = time.perf_counter()
+    wbmm_ref.forward(x5, T5, case5.w, case5.shift, case5.layout, "direct")
+    wbmm_ref.backward(x5, T5, g5, case5.w, case5.shift, case5.layout)
+    dt = time.perf_counter() - t0
+    out["cfg5_fwd_bwd"] = {"ms": dt * 1e3, "value": 3 * flops_of(sub) / dt / 1e12, "unit": UNIT, "cores": ncores,
+                           "sample": f"first {nb5} of {case5.B} images, all {case5.C} channels, forward + dX + dT"}
+    return out
+
+
 def run_reference(args, rank, world):
     """--impl reference: the paper ships no code, so the reference arm is the CPU oracle, timed as
     it stands on this box's host cores; each step is a bounded sample of config 3."""
@@ -254,6 +296,69 @@ def conv_context(case: si.Case, x):
             out[f"torch_dwconv_k{k}_ms"] = round(a.elapsed_time(b) / 5, 4)
     except Exception as e:  # context only
         out["error"] = str(e)[:100]
+    return out
+
+
+def region_ms_rot(fn, n, stream, warm=3):
+    """Average device ms of n back-to-back calls fn(i) (i rotates the buffer set), CUDA events on `stream`."""
+    for i in range(warm):
+        fn(i)
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(stream)
+    for i in range(n):
+        fn(warm + i)
+    b.record(stream)
+    torch.cuda.synchronize()
+    return a.elapsed_time(b) / n
+
+
+def buffer_sets(per_set_bytes: float, cap: int = 8) -> int:
+    """Enough buffer sets that the rotating footprint exceeds 2 x L2 (cold-L2 numbers)."""
+    return int(max(2, min(cap, -(-2 * L2_BYTES // per_set_bytes) + 1)))
+
+
+def other_rooflines(wb, dev, stream, hbm_peak):
+    """Roofline fractions of the other kernels / configs, measured in the same run with rotating buffers (cold L2):
+    algorithmic bytes (read the inputs once, write the outputs once, + the table) / average launch duration."""
+    out = {}
+
+    def fwd_row(name, case, n=30):
+        d = si.make(case, device=dev)
+        es = 4 if case.dtype == "f32" else 2
+        ns = buffer_sets(2.0 * case.n_elem * es)
+        xs = [d["x"]] + [d["x"].clone() for _ in range(ns - 1)]
+        ys = [torch.empty_like(d["x"]) for _ in range(ns)]
+        ms = region_ms_rot(lambda i: wb.wbmm_forward(xs[i % ns], d["T"], case.w, case.shift, case.layout, out=ys[i % ns]), n, stream)
+        by = bytes_of(case)
+        out[name] = {"ms": round(ms, 5), "gbs": round(by / ms / 1e6, 1), "frac": round(by / (hbm_peak * 1e9) * 1e3 / ms, 4),
+                     "path": wb.wbmm_path_string(wb.wbmm_last_path()), "buffer_sets": ns}
+        del xs, ys, d
+        torch.cuda.empty_cache()
+
+    fwd_row("cfg2_fwd_w7", si.CFG2)
+    fwd_row("cfg5_fwd_shift7", si.with_(si.CFG5, backward=False))
+    fwd_row("ragged_B64_C96_60x60_w14_fwd", si.Case("ragged", 64, 96, 60, 60, 14, seed=85))
+    fwd_row("nhwc_cfg3_shape_fwd", si.with_(si.CFG3, layout=si.NHWC))
+    fwd_row("nhwc_cfg2_shape_fwd_w7", si.with_(si.CFG2, layout=si.NHWC))
+    fwd_row("fp32_B128_C96_56x56_w14_fwd", si.with_(si.CFG3, dtype="f32"), n=10)
+    fwd_row("fp32_B128_C96_56x56_w7_fwd", si.Case("f32w7", 128, 96, 56, 56, 7, dtype="f32", seed=86), n=10)
+
+    # backward of config 5, each kernel alone, rotating (x, dy, dx) sets
+    c5 = si.CFG5
+    d = si.make(c5, device=dev)
+    ns = buffer_sets(3.0 * c5.n_elem * 2)
+    xs = [d["x"]] + [d["x"].clone() for _ in range(ns - 1)]
+    gs = [d["dy"]] + [d["dy"].clone() for _ in range(ns - 1)]
+    dxs = [torch.empty_like(d["x"]) for _ in range(ns)]
+    dT = torch.empty((c5.C, c5.bins), dtype=torch.float32, device=dev)
+    by = bytes_of(c5)
+    ms = region_ms_rot(lambda i: wb.wbmm_backward(None, d["T"], gs[i % ns], c5.w, c5.shift, need_dT=False, dx=dxs[i % ns]), 30, stream)
+    out["cfg5_dX"] = {"ms": round(ms, 5), "frac": round(by / (hbm_peak * 1e9) * 1e3 / ms, 4), "buffer_sets": ns}
+    ms = region_ms_rot(lambda i: wb.wbmm_backward(xs[i % ns], None, gs[i % ns], c5.w, c5.shift, need_dx=False, dT=dT), 30, stream)
+    out["cfg5_dT"] = {"ms": round(ms, 5), "frac": round(by / (hbm_peak * 1e9) * 1e3 / ms, 4), "buffer_sets": ns,
+                      "note": "includes the dT zeroing launch"}
+    del xs, gs, dxs, d
+    torch.cuda.empty_cache()
     return out
 
 
@@ -356,40 +461,40 @@ def run_wbmm(args, rank, world, local):
                 "tensor_tflops": fl / (ms_step * 1e-3) / 1e12,
                 "hot_l2_ms_median_event_pair": statistics.median(hot)}
 
-    # training step (config 5) as context: forward + dX + dT
+    # training step (config 5) as context: forward + dX + dT on rotating buffer sets (x, y, dy, dx of one set are
+    # 154 MB; three sets never find their inputs in the 126 MB L2)
     c5 = si.CFG5
     d5 = si.make(c5, device=dev)
-    y5 = torch.empty_like(d5["x"])
+    ns5 = 3
+    x5 = [d5["x"]] + [d5["x"].clone() for _ in range(ns5 - 1)]
+    g5s = [d5["dy"]] + [d5["dy"].clone() for _ in range(ns5 - 1)]
+    y5s = [torch.empty_like(d5["x"]) for _ in range(ns5)]
+    dx5 = [torch.empty_like(d5["x"]) for _ in range(ns5)]
+    dT5r = torch.empty((c5.C, c5.bins), dtype=torch.float32, device=dev)
+    y5 = y5s[0]
 
     def train(i):
-        wb.wbmm_forward(d5["x"], d5["T"], c5.w, c5.shift, out=y5)
-        wb.wbmm_backward(d5["x"], d5["T"], d5["dy"], c5.w, c5.shift)
+        j = i % ns5
+        wb.wbmm_forward(x5[j], d5["T"], c5.w, c5.shift, out=y5s[j])
+        wb.wbmm_backward(x5[j], d5["T"], g5s[j], c5.w, c5.shift, dT=dT5r, dx=dx5[j])
 
     def region_ms(fn, n=20):
-        for _ in range(3):
-            fn()
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record(stream)
-        for _ in range(n):
-            fn()
-        b.record(stream)
-        torch.cuda.synchronize()
-        return a.elapsed_time(b) / n
+        return region_ms_rot(lambda i: fn(), n, stream)
 
     for i in range(3):
         train(i)
-    t5 = time_steps(train, 10, stream)
+    t5 = time_steps(train, 12, stream)
     train_path = wb.wbmm_path_string(wb.wbmm_last_path())
     parts = {
-        "fwd_ms": region_ms(lambda: wb.wbmm_forward(d5["x"], d5["T"], c5.w, c5.shift, out=y5)),
-        "dX_ms": region_ms(lambda: wb.wbmm_backward(None, d5["T"], d5["dy"], c5.w, c5.shift, need_dT=False)),
-        "dT_ms": region_ms(lambda: wb.wbmm_backward(d5["x"], None, d5["dy"], c5.w, c5.shift, need_dx=False)),
+        "fwd_ms": region_ms_rot(lambda i: wb.wbmm_forward(x5[i % ns5], d5["T"], c5.w, c5.shift, out=y5s[i % ns5]), 30, stream),
+        "dX_ms": region_ms_rot(lambda i: wb.wbmm_backward(None, d5["T"], g5s[i % ns5], c5.w, c5.shift, need_dT=False, dx=dx5[i % ns5]), 30, stream),
+        "dT_ms": region_ms_rot(lambda i: wb.wbmm_backward(x5[i % ns5], None, g5s[i % ns5], c5.w, c5.shift, need_dx=False, dT=dT5r), 30, stream),
     }
     by5 = 2 * c5.n_elem * 2 * 2 + 2 * c5.n_elem * 2 + c5.C * c5.bins * 4   # x,y; dy,dx; x,dy; dT
     train_step = {"workload": "cfg5 B128 C192 28x28 w14 shift7 fwd+dX+dT", "ms_median": statistics.median(t5),
                   "ms_min": min(t5), "back_to_back": parts, "last_path": train_path, "flops": 3 * flops_of(c5),
                   "hbm_frac_at_median": by5 / (statistics.median(t5) * 1e-3) / 1e9 / hbm_peak,
-                  "note": "x, y, dy, dx = 154 MB against a 126 MB L2: partly L2-resident between launches"}
+                  "note": f"rotating {ns5} buffer sets of (x, y, dy, dx) = 462 MB: cold-L2 numbers; back_to_back = each kernel alone"}
 
     # the same step (forward, dX, dT zeroing, dT) replayed from one CUDA graph: device-side time, no host gaps
     try:
@@ -397,9 +502,10 @@ def run_wbmm(args, rank, world, local):
         torch.cuda.synchronize()
         g5 = torch.cuda.CUDAGraph()
         with torch.cuda.graph(g5):
-            wb.wbmm_forward(d5["x"], d5["T"], c5.w, c5.shift, out=y5)
-            wb.wbmm_backward(d5["x"], d5["T"], d5["dy"], c5.w, c5.shift, dT=dT5)
-        train_step["ms_graph"] = region_ms(g5.replay)
+            for j in range(ns5):
+                wb.wbmm_forward(x5[j], d5["T"], c5.w, c5.shift, out=y5s[j])
+                wb.wbmm_backward(x5[j], d5["T"], g5s[j], c5.w, c5.shift, dT=dT5, dx=dx5[j])
+        train_step["ms_graph"] = region_ms(g5.replay) / ns5       # the graph holds one step per buffer set
         del g5
     except Exception as e:  # capture not possible: the eager numbers stand
         sys.stderr.write(f"train-step graph capture failed: {str(e)[:80]}\n")
@@ -420,9 +526,13 @@ def run_wbmm(args, rank, world, local):
         "dTg_dTl": region_ms(lambda: wb.wbmm_hier_backward(d5["x"], None, None, d5["dy"], c5.w, c5.shift, need_dx=False)),
     }
 
+    del x5, g5s, y5s, dx5
+    torch.cuda.empty_cache()
+    others = other_rooflines(wb, dev, stream, hbm_peak)
+
     tfl_cpu, cores, sample, dt_cpu = time_oracle(case)
     cpu = {"value": tfl_cpu, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
-           "seconds": dt_cpu}
+           "seconds": dt_cpu, "legs": oracle_legs(case, c5)}
 
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -432,7 +542,7 @@ def run_wbmm(args, rank, world, local):
                    "per_gpu_batch": case.B, "path": path,
                    "l2": f"rotating {nsets} buffer sets, footprint {footprint / 1e6:.0f} MB > 2x L2 (cold-L2 numbers)"},
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
-        "roofline": roofline, "cpu_baseline": cpu, "train_step": train_step,
+        "roofline": roofline, "other_rooflines": others, "cpu_baseline": cpu, "train_step": train_step,
         "context": conv_context(case, d0["x"]),
     }
     print(json.dumps(out), flush=True)
@@ -493,7 +603,7 @@ def run_sweep(args):
         del xs, ys, d
 
     # backward (rows a7, a8 of SURVEY.md 8(a)) on the named configs and the large sweep shapes: dX and dT timed
-    # apart, back to back on one buffer set (x + dy + dx of these shapes exceed L2 except where noted by the size)
+    # apart, back to back on rotating buffer sets
     bwd = [si.with_(si.CFG2, backward=True), si.with_(si.CFG3, backward=True), si.CFG5,
            si.with_(si.CFG5, shift=(0, 0), name="cfg5_shape_no_shift")]
     for (C, H) in ((96, 56), (192, 28), (384, 28), (96, 112)):
@@ -502,28 +612,23 @@ def run_sweep(args):
     bwd.append(si.Case("bwd_ragged_B64_C96_H60_w14", 64, 96, 60, 60, 14, backward=True, seed=299))
     for case in bwd:
         d = si.make(case, device="cuda")
-        dx = torch.empty_like(d["x"])
+        ns = buffer_sets(3.0 * case.n_elem * 2, cap=6)       # rotating (x, dy, dx) sets: cold-L2 numbers
+        xs = [d["x"]] + [d["x"].clone() for _ in range(ns - 1)]
+        gs = [d["dy"]] + [d["dy"].clone() for _ in range(ns - 1)]
+        dxs = [torch.empty_like(d["x"]) for _ in range(ns)]
         dT = torch.empty((case.C, case.bins), dtype=torch.float32, device="cuda")
         out = {}
-        for key, fn in (("dX", lambda: wb.wbmm_backward(None, d["T"], d["dy"], case.w, case.shift, case.layout, need_dT=False)),
-                        ("dT", lambda: wb.wbmm_backward(d["x"], None, d["dy"], case.w, case.shift, case.layout, need_dx=False, dT=dT))):
-            for _ in range(3):
-                fn()
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            n = 20
-            a.record(stream)
-            for _ in range(n):
-                fn()
-            b.record(stream)
-            torch.cuda.synchronize()
-            out[key] = (a.elapsed_time(b) / n, wb.wbmm_path_string(wb.wbmm_last_path()))
+        for key, fn in (("dX", lambda i: wb.wbmm_backward(None, d["T"], gs[i % ns], case.w, case.shift, case.layout, need_dT=False, dx=dxs[i % ns])),
+                        ("dT", lambda i: wb.wbmm_backward(xs[i % ns], None, gs[i % ns], case.w, case.shift, case.layout, need_dx=False, dT=dT))):
+            out[key] = (region_ms_rot(fn, 20, stream), wb.wbmm_path_string(wb.wbmm_last_path()))
         by = bytes_of(case)          # dX: dy in, dx out; dT: x and dy in -- the same 2 x tensor bytes (+ table)
         print(json.dumps({"sweep_case": "backward_" + case.name, "layout": "NCHW", "B": case.B, "C": case.C, "H": case.H,
                           "w": case.w, "shift": list(case.shift), "dX_ms": round(out["dX"][0], 5), "dT_ms": round(out["dT"][0], 5),
                           "dX_frac_of_hbm_roofline": round(by / (hbm_peak * 1e9) * 1e3 / out["dX"][0], 4),
                           "dT_frac_of_hbm_roofline": round(by / (hbm_peak * 1e9) * 1e3 / out["dT"][0], 4),
-                          "dX_path": out["dX"][1], "dT_path": out["dT"][1]}), flush=True)
-        del d, dx, dT
+                          "dX_path": out["dX"][1], "dT_path": out["dT"][1], "buffer_sets": ns}), flush=True)
+        del d, xs, gs, dxs, dT
+        torch.cuda.empty_cache()
 
 
 # The paper's operator benchmark, Table 13 B=128 block: single A800, FP32,
@@ -612,6 +717,21 @@ def main():
         rank = int(os.environ.get("RANK", "0"))
         run_reference(args, rank, int(os.environ.get("WORLD_SIZE", "1")))
         return
+    if "WORLD_SIZE" not in os.environ and args.gpus > 1:
+        # plain `python bench.py --gpus N`: launch the N ranks ourselves (one process per GPU, replicas only)
+        if torch.cuda.device_count() < args.gpus:
+            sys.stderr.write(f"bench.py: --gpus {args.gpus} but {torch.cuda.device_count()} CUDA device(s) visible\n")
+            raise SystemExit(2)
+        import socket
+        with socket.socket() as sock:
+            sock.bind(("127.0.0.1", 0))
+            port = sock.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__), *sys.argv[1:]]
+        raise SystemExit(subprocess.call(cmd))
+    if int(os.environ.get("WORLD_SIZE", "1")) != args.gpus:
+        sys.stderr.write(f"bench.py: --gpus {args.gpus} does not match WORLD_SIZE={os.environ.get('WORLD_SIZE')}\n")
+        raise SystemExit(2)
     rank, world, local = dist_setup(args.gpus)
     try:
         run_wbmm(args, rank, world, local)

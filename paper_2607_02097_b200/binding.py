@@ -175,11 +175,14 @@ def wbmm_hier_backward(x: Optional[torch.Tensor], Tg: Optional[torch.Tensor], Tl
 
 def wbmm_backward(x: Optional[torch.Tensor], T: Optional[torch.Tensor], dy: torch.Tensor, w: int,
                   shift=(0, 0), layout: int = NCHW, flags: int = 0, need_dx: bool = True,
-                  need_dT: bool = True, dT: Optional[torch.Tensor] = None
+                  need_dT: bool = True, dT: Optional[torch.Tensor] = None, dx: Optional[torch.Tensor] = None
                   ) -> Tuple[Optional[torch.Tensor], Optional[torch.Tensor]]:
     """(dx, dT) of wbmm_forward; dT is float32 [C,(2w-1)^2] (include/wbmm.h: wbmm_backward)."""
     d = make_desc(dy, w, shift, layout, flags)
-    dx = torch.empty_like(dy) if need_dx else None
+    if need_dx and dx is None:
+        dx = torch.empty_like(dy)
+    if not need_dx:
+        dx = None
     if need_dT and dT is None:
         dT = torch.empty((d.C, (2 * w - 1) ** 2), dtype=torch.float32, device=dy.device)
     if not need_dT:

@@ -23,26 +23,26 @@ int set_cuda_error(cudaError_t e, const char* where)
 
 size_t elem_size(int dtype) { return dtype == WBMM_DTYPE_F32 ? 4 : 2; }
 
-// 0 = not probed, 1 = sm_100 present, -1 = absent
+constexpr int kMaxDevices = 64;
+
+// Is the CURRENT device an sm_100 part?  Cached per device: 0 = not probed, 1 = yes, -1 = no.
 int device_state()
 {
-    static std::atomic<int> state{0};
-    int s = state.load();
-    if (s != 0) return s;
+    static std::atomic<int> state[kMaxDevices];
     int dev = 0, major = 0, count = 0;
-    if (cudaGetDeviceCount(&count) != cudaSuccess || count == 0) {
+    if (cudaGetDeviceCount(&count) != cudaSuccess || count == 0 || cudaGetDevice(&dev) != cudaSuccess) {
         cudaGetLastError();
-        state.store(-1);
         return -1;
     }
-    if (cudaGetDevice(&dev) != cudaSuccess ||
-        cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) {
+    const bool cached = dev >= 0 && dev < kMaxDevices;
+    int s = cached ? state[dev].load(std::memory_order_relaxed) : 0;
+    if (s != 0) return s;
+    if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) {
         cudaGetLastError();
-        state.store(-1);
         return -1;
     }
     s = major == 10 ? 1 : -1;
-    state.store(s);
+    if (cached) state[dev].store(s, std::memory_order_relaxed);
     return s;
 }
 
@@ -64,26 +64,57 @@ int validate(const wbmm_desc_t* d)
 
 bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
 
-// NHWC through NCHW: stream-ordered temporaries.
+// NHWC through NCHW: stream-ordered temporaries from a memory pool the LIBRARY owns (one per device, created on
+// first use, destroyed by wbmm_release).  Freed blocks stay cached in that pool (release threshold = max), so a call
+// pays no fresh allocation after the first -- without touching the policy of the device's default pool, which
+// belongs to the application (a PyTorch process may run its own allocator on it).
+std::mutex g_pool_mutex;
+cudaMemPool_t g_pools[kMaxDevices] = {};
+
+cudaError_t scratch_pool(cudaMemPool_t* out)
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_pool_mutex);
+    if (!g_pools[dev]) {
+        cudaMemPoolProps props = {};
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        cudaMemPool_t pool;
+        e = cudaMemPoolCreate(&pool, &props);
+        if (e != cudaSuccess) return e;
+        uint64_t keep = ~0ull;
+        cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        g_pools[dev] = pool;
+    }
+    *out = g_pools[dev];
+    return cudaSuccess;
+}
+
+void scratch_pools_release()
+{
+    std::lock_guard<std::mutex> lock(g_pool_mutex);
+    for (int d = 0; d < kMaxDevices; ++d)
+        if (g_pools[d]) {
+            cudaMemPoolDestroy(g_pools[d]);
+            g_pools[d] = nullptr;
+        }
+}
+
 struct AsyncScratch {
     void* p = nullptr;
     cudaStream_t s;
     explicit AsyncScratch(cudaStream_t stream) : s(stream) {}
     cudaError_t alloc(size_t n)
     {
-        // Keep freed blocks cached in the device's default pool (its default is to hand memory back to the
-        // driver at the next synchronisation, which makes every call pay a fresh allocation).
-        static std::once_flag once;
-        std::call_once(once, [] {
-            int dev = 0;
-            cudaMemPool_t pool;
-            if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
-                uint64_t keep = ~0ull;
-                cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
-            }
-            cudaGetLastError();
-        });
-        return cudaMallocAsync(&p, n, s);
+        cudaMemPool_t pool;
+        cudaError_t e = scratch_pool(&pool);
+        if (e != cudaSuccess) return e;
+        return cudaMallocFromPoolAsync(&p, n, pool, s);
     }
     ~AsyncScratch() { if (p) cudaFreeAsync(p, s); }
 };
@@ -456,17 +487,9 @@ constexpr int kHostChunks = 32;   // at most; see host_chunks()
 cudaStream_t g_s_kernel = nullptr, g_s_out = nullptr;
 cudaEvent_t g_ev_in[kHostChunks] = {}, g_ev_k[kHostChunks] = {};
 
-// Chunks per call: enough that the un-overlapped head (first upload) and tail (last download) are small,
-// few enough that per-copy set-up does not show.  WBMM_HOST_CHUNKS overrides (1..32) for experiments.
-int host_chunks()
-{
-    static int n = [] {
-        const char* e = getenv("WBMM_HOST_CHUNKS");
-        int v = e ? atoi(e) : 8;
-        return v < 1 ? 1 : (v > kHostChunks ? kHostChunks : v);
-    }();
-    return n;
-}
+// Chunks per call: enough that the un-overlapped head (first upload) and tail (last download) are small, few enough
+// that per-copy set-up does not show.
+int host_chunks() { return 8; }
 
 cudaError_t host_pipeline_init()
 {
@@ -601,7 +624,7 @@ void wbmm_release(void)
     g_sx.release(); g_sT.release(); g_sy.release(); g_sdy.release(); g_sdT.release();
     if (g_host_stream) { cudaStreamDestroy(g_host_stream); g_host_stream = nullptr; }
     host_pipeline_release();
-    wbmm::tc_release();
+    scratch_pools_release();
 }
 
 int wbmm_last_path(void) { return t_last_path; }

@@ -54,23 +54,7 @@ __device__ __forceinline__ bool mbar_test_wait(uint32_t bar, uint32_t parity)
     return ok != 0;
 }
 #ifdef WBMM_WATCHDOG
-// Debug build only: a wait that gives up after 20 ms and records who was stuck.
-__device__ unsigned long long g_watchdog[64];
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
-{
-    if (mbar_try_wait(bar, parity)) return;
-    long long t0, t1;
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
-    for (;;) {
-        if (mbar_try_wait(bar, parity)) return;
-        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
-        if (t1 - t0 > 20000000ll) break;
-    }
-    unsigned slot = atomicAdd((unsigned*)&g_watchdog[0], 1u);
-    if (slot < 60)
-        g_watchdog[2 + slot] = ((unsigned long long)blockIdx.x << 48) | ((unsigned long long)threadIdx.x << 36) |
-                               ((unsigned long long)(bar & 0xfffff) << 8) | parity;
-}
+#include "wbmm_debug.cuh"      // debug build only: a wait that times out and records the waiter
 #else
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
 {

@@ -200,9 +200,6 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
     __shared__ uint32_t tmem_base_s;
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-#ifdef WBMM_TRACE
-    if (tid == 0 && blockIdx.x < 148) { g_blk[blockIdx.x * 4] = gtime(); unsigned sm; asm("mov.u32 %0, %smid;" : "=r"(sm)); g_blk[blockIdx.x * 4 + 3] = sm; }
-#endif
     const uint32_t bar0 = ptx::smem_u32(bars);
     auto FULL = [&](int s) { return bar0 + 8u * s; };
     auto EMPTY = [&](int s) { return bar0 + 8u * (kMaxSlots + s); };
@@ -216,8 +213,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
     // Output hand-off groups: the smallest runs of whole epilogue warps that cover whole frame images
     // (lanes are image-major), so a group's images can be stored as soon as ITS warps are done.
     const OutGroups og = out_groups(tl, wpf);
-    TRACE(0, 15);
-    if (warp == 1) { ptx::tmem_alloc(ptx::smem_u32(&tmem_base_s), 512); if (lane == 0) TRACE(1, 15); }
+    if (warp == 1) { ptx::tmem_alloc(ptx::smem_u32(&tmem_base_s), 512); }
     if (tid >= 64 && tid < 64 + nslot) {
         ptx::mbar_init(FULL(tid - 64), 1);
         ptx::mbar_init(EMPTY(tid - 64), box ? box * wpf : wpf);   // box mode: one barrier pair per group of `box` images
@@ -237,7 +233,6 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
             ptx::mbar_init(OUT_EMPTY + 8 * ob, 1);
         }
         ptx::fence_mbar_init();
-        TRACE(2, 15);
     }
     if constexpr (Bc::TOEP) {
         // build_lib14 never writes the padding rows ci = 14, 15 of the blocks: zero the library once
@@ -246,17 +241,12 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
     for (int i = tid; i < Sm::TAB_BYTES / 4; i += kThreadsB) reinterpret_cast<uint32_t*>(tab)[i] = 0u;
     ptx::fence_proxy_async_smem();
     ptx::tc_fence_before_sync();
-    if (tid == 64) TRACE(3, 15);
     __syncthreads();
-    if (tid == 64) TRACE(4, 15);
     ptx::tc_fence_after_sync();
     // Programmatic dependent launch: everything above overlapped the previous kernel's tail; no
     // global memory is touched before this point.
     asm volatile("griddepcontrol.wait;" ::: "memory");
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-#ifdef WBMM_TRACE
-    if (tid == 0 && blockIdx.x < 148) g_blk[blockIdx.x * 4 + 1] = gtime();
-#endif
     const uint32_t tmem = tmem_base_s;
     constexpr uint32_t A_STRIDE = (Bc::A_COLS + 31) / 32 * 32;
     const uint32_t tmem_d = tmem + 2 * A_STRIDE;
@@ -308,7 +298,6 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                     const int slot = kk % nslot;            // first slot of the group (nslot, k, p are multiples of box)
                     ptx::mbar_wait(EMPTY(slot), ((kk / nslot) & 1) ^ 1);
                     ptx::mbar_arrive_expect_tx(FULL(slot), bytes * box);
-                    if (p == 0) TRACE(0, (t - t0));
                     // (the box starts on a 16-byte boundary at or below the plane: the plane sits poff bytes into the slot)
                     ptx::tma_load_4d(ptx::smem_u32(ring + (size_t)slot * tl.S), &mx, sbox == 2 ? (c * (int)plane_elems) & ~7 : 0, 0,
                                      sbox == 2 ? 0 : c, b0 + p, FULL(slot));
@@ -330,7 +319,6 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                     continue;
                 }
                 ptx::mbar_arrive_expect_tx(FULL(slot), bytes);
-                if (p == 0) TRACE(0, (t - t0));
                 const uint16_t* src = x + ((long long)(b0 + p) * g.C + c) * plane_elems + (long long)wy0 * WS * g.W;
                 ptx::bulk_g2s(ptx::smem_u32(ring + (size_t)slot * tl.S), src, bytes, FULL(slot));
             }
@@ -351,12 +339,10 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
             for (int t = t0; t < t1; ++t, ++lt) {
                 const uint32_t buf = lt & 1;
                 ptx::mbar_wait(A_FULL + 8 * buf, (lt >> 1) & 1);
-                if (lane == 0) TRACE(1, lt);
                 const uint32_t tmem_a = tmem + buf * A_STRIDE;
 #pragma unroll
                 for (int h = 0; h < Hs::NH; ++h) {
                     ptx::mbar_wait(D_EMPTY + 8 * h, (lt & 1) ^ 1);      // the epilogue has drained this half of tile lt-1
-                    if (h == 0 && lane == 0) TRACE(2, lt);
                     ptx::tc_fence_after_sync();
                     if (ptx::elect_one()) {
                         const uint32_t idesc = ptx::idesc_f16(BF16 ? 1 : 0, 128, Hs::ncols(h));
@@ -383,7 +369,6 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                     }
                     __syncwarp();
                 }
-                if (lane == 0) TRACE(3, lt);
             }
         }
     } else if (warp < 6) {
@@ -406,7 +391,6 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
             if (c != cur_c) {
                 if (lt > 0) ptx::mbar_wait(A_EMPTY + 8 * ((lt - 1) & 1), ((lt - 1) >> 1) & 1);   // MMA(lt-1) done with W_c
                 const uint16_t* Tc = T + (long long)c * Cf::NB;
-                if (rt == 0) TRACE(12, lt);
                 if constexpr (WS == 14) {
                     if (!tabv_ready) table_to_regs14(Tc, reverse != 0, rt, tabv);
                     build_lib14(tabv, tab, tab + Sm::TAB_ONE / 2, Wc, rt, bias ? (uint32_t)bias[c] : 0u);
@@ -461,7 +445,6 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
             // after every repack thread had finished tile lt-2, and the slot's previous fill is that old.
             if (nslot < 2 * tl.NP) ptx::named_bar_sync(2, 128);
             ptx::mbar_wait(A_EMPTY + 8 * buf, ((lt >> 1) & 1) ^ 1);   // MMA(lt-2) has consumed A[buf]
-            if (rt == 0) TRACE(4, lt);
             const bool part = wl < wpf && pl < np_eff;               // this thread's frame image was loaded
             const bool valid = part && wy0 + wyl < g.nwh;
             if constexpr (STRIP) {
@@ -471,10 +454,8 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
             const int slot = kk % nslot;
             const int poff = sbox == 2 ? ((c * (int)plane_elems) & 7) * 2 : 0;    // plane boxes: offset of the plane in its slot
             if (lt == 0) rebuild_weight(c, lt);   // first tile: build while its loads are in flight
-            if (rt == 0) TRACE(5, lt);
             const int bslot = box ? slot - slot % box : slot;      // the barrier pair that covers this image
             if (part) ptx::mbar_wait(FULL(bslot), (kk / nslot) & 1);
-            if (rt == 0) TRACE(6, lt);
             if constexpr (WG)
             {
                 const uint32_t ta = tmem + buf * A_STRIDE + ((uint32_t)(q * 32) << 16);
@@ -494,7 +475,6 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
             if (lt > 0) rebuild_weight(c, lt);
             ptx::tc_fence_before_sync();
             ptx::mbar_arrive(A_FULL + 8 * buf);
-            if (rt == 0) TRACE(7, lt);
             k += np_eff;
             if constexpr (WS == 14) {
                 // the next tile starts a new channel: have its table row in flight during the next copy
@@ -533,7 +513,6 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                 constexpr int h = decltype(hc)::value;
                 uint32_t pk[Hs::TOEP ? 49 : Hs::ncols(h) / 2];
                 ptx::mbar_wait(D_FULL + 8 * h, lt & 1);
-                if (m == 0 && h == 0) TRACE(8, lt);
                 ptx::tc_fence_after_sync();
                 accum_half_to_packed<WS, BF16, h>(tmem_d + Hs::col0(h) + ((uint32_t)(q * 32) << 16), pk);
                 ptx::tc_fence_before_sync();
@@ -563,7 +542,6 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
             if constexpr (Hs::NH > 1) drain_half(std::integral_constant<int, 1>{});
             ptx::fence_proxy_async_smem();      // generic-proxy writes -> the bulk store's async-proxy reads
             ptx::mbar_arrive(OUT_FULL + 8 * ob);
-            if (m == 0) TRACE(9, lt);
         }
     } else {
         // ------------------------------------------------------------------ store
@@ -625,7 +603,6 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                 if (lt % depth != frame) continue;
                 const uint32_t bytes = (uint32_t)rows_eff * rowB;
                 ptx::mbar_wait(OUT_FULL + 8 * lane, (lt / depth) & 1);
-                if (lane == 0) TRACE(10, lt);
                 const int p_first = gq * og.images, p_end = min(p_first + og.images, np_eff);
                 if (sbox) {
                     if (p_first < p_end) ptx::tma_store_4d(&my, 0, 0, c, b0 + p_first, ptx::smem_u32(outb + (size_t)lane * out_bytes));
@@ -644,7 +621,6 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                 }
                 ptx::bulk_commit();
                 ptx::bulk_wait_read<0>();
-                if (lane == 0) TRACE(11, lt);
                 ptx::mbar_arrive(OUT_EMPTY + 8 * lane);
             }
             ptx::bulk_wait_read<0>();   // the sources are in this CTA's shared memory: reads must finish before it exits
@@ -653,9 +629,6 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
     ptx::tc_fence_before_sync();
     __syncthreads();
     if (warp == 1) ptx::tmem_dealloc(tmem, 512);
-#ifdef WBMM_TRACE
-    if (tid == 0 && blockIdx.x < 148) g_blk[blockIdx.x * 4 + 2] = gtime();
-#endif
 }
 
 // Shared memory left after the weights / tables / barriers is cut into frame-image slots: an output
@@ -840,7 +813,7 @@ cudaError_t launch_bulk(const Geom& g, const TcTiles& tl_in, const void* x, cons
     }
     if (!box && !bulk_slots<WS>(tl, wpf, &nslot, &nout)) return cudaErrorInvalidConfiguration;
     const size_t smem = (size_t)BulkSmem<WS>::FIXED + (size_t)(nslot + nout * out_groups(tl, wpf).images) * tl.S;
-    static SmemOptIn smem_state = {0, 0};
+    static SmemOptIn smem_state;
     cudaError_t e = ensure_dynamic_smem(reinterpret_cast<const void*>(k), smem, &smem_state);
     if (e != cudaSuccess) return e;
     int grid = (int)(tl.ntiles < num_sms() ? tl.ntiles : num_sms());
@@ -886,7 +859,7 @@ cudaError_t launch_generic(const Geom& g, const TcTiles& tl, const void* x, cons
 {
     auto k = tc_generic_kernel<WS, BF16>;
     const size_t smem = generic_smem<WS>(tl);
-    static SmemOptIn smem_state = {0, 0};
+    static SmemOptIn smem_state;
     cudaError_t e = ensure_dynamic_smem(reinterpret_cast<const void*>(k), smem, &smem_state);
     if (e != cudaSuccess) return e;
     const int grid = (int)(tl.ntiles < num_sms() ? tl.ntiles : num_sms());
@@ -902,23 +875,27 @@ cudaError_t ensure_dynamic_smem(const void* kernel, size_t bytes, SmemOptIn* sta
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
-    if (state->dev_plus1 == dev + 1 && (size_t)state->bytes >= bytes) return cudaSuccess;
+    const bool cached = dev >= 0 && dev < kMaxDevices;
+    if (cached && (size_t)state->bytes[dev].load(std::memory_order_acquire) >= bytes) return cudaSuccess;
+    static std::mutex mu;      // the attribute is per (kernel, device): raise it once, monotonically
+    std::lock_guard<std::mutex> lock(mu);
+    if (cached && (size_t)state->bytes[dev].load(std::memory_order_relaxed) >= bytes) return cudaSuccess;
     e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
-    if (e == cudaSuccess) {
-        state->dev_plus1 = dev + 1;
-        state->bytes = (int)bytes;
-    }
+    if (e == cudaSuccess && cached) state->bytes[dev].store((int)bytes, std::memory_order_release);
     return e;
 }
 
+// Multiprocessors of the CURRENT device (cached per device).
 int num_sms()
 {
-    static int n = 0;
+    static std::atomic<int> cache[kMaxDevices];
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return 148;
+    const bool cached = dev >= 0 && dev < kMaxDevices;
+    int n = cached ? cache[dev].load(std::memory_order_relaxed) : 0;
     if (n == 0) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
-        if (n <= 0) n = 148;
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
+        if (cached) cache[dev].store(n, std::memory_order_relaxed);
     }
     return n;
 }
@@ -1085,17 +1062,5 @@ cudaError_t tc_forward_matrix(const Geom& g, int dtype, const void* x, const voi
               : launch_generic<14, false>(g, tl, x, nullptr, y, transpose, stream, M, bias);
 }
 
-void tc_release() {}
-
-#ifdef WBMM_TRACE
-extern "C" __attribute__((visibility("default"))) int wbmm_debug_trace(long long* out)
-{
-    return (int)cudaMemcpyFromSymbol(out, g_trace, sizeof(long long) * 256);
-}
-extern "C" __attribute__((visibility("default"))) int wbmm_debug_blocks(long long* out)
-{
-    return (int)cudaMemcpyFromSymbol(out, g_blk, sizeof(long long) * 148 * 4);
-}
-#endif
 
 }  // namespace wbmm

@@ -60,6 +60,4 @@ bool image_box_map(const Geom& g, int dtype, const void* base, int images, void*
 int plane_box_images(const Geom& g, const TcTiles& tl);
 bool plane_box_map(const Geom& g, int dtype, const void* base, int images, void* map);
 
-void tc_release();
-
 }  // namespace wbmm

@@ -3,6 +3,8 @@
 // TMEM transfer helpers, the static tile schedule.  Not part of the C ABI.
 #pragma once
 
+#include <atomic>
+
 #include "wbmm_ptx.cuh"
 #include "wbmm_tc.cuh"
 
@@ -687,23 +689,16 @@ struct TilePart {
 };
 
 
-#ifdef WBMM_TRACE
-// Debug build only: per-tile event timestamps of block 0 (read back with wbmm_debug_trace()).
-__device__ long long g_trace[16 * 16];
-__device__ long long g_blk[148 * 4];
-__device__ __forceinline__ long long gtime() { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
-#define TRACE(ev, lt) do { if (blockIdx.x == 1 && (lt) < 16) g_trace[(lt) * 16 + (ev)] = gtime(); } while (0)
-#else
-#define TRACE(ev, lt) do { } while (0)
-#endif
 
 }  // namespace tcdev
 
 // Host helpers defined in wbmm_tc.cu.
 int num_sms();
-// Opts a kernel in to `bytes` of dynamic shared memory unless an earlier call already allowed as much
-// on this device (`state`: one static per kernel instantiation, zero-initialised).
-struct SmemOptIn { int dev_plus1, bytes; };
+// Opts a kernel in to `bytes` of dynamic shared memory unless an earlier call already allowed as much on the
+// CURRENT device (`state`: one static per kernel instantiation, zero-initialised; per device, safe to use from
+// several host threads).
+constexpr int kMaxDevices = 64;
+struct SmemOptIn { std::atomic<int> bytes[kMaxDevices]; };
 cudaError_t ensure_dynamic_smem(const void* kernel, size_t bytes, SmemOptIn* state);
 // Greedy contiguous partition of the tile sequence over `grid` CTAs minimising the largest cost,
 // cost = tiles + switch_cost per channel boundary strictly inside a CTA's range.  Returns the

@@ -163,7 +163,6 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
                 for (int hf = 0; hf < 2; ++hf) {
                     const uint32_t a_addr = stage_addr + hf * Dc::HALF, b_addr = a_addr + Dc::OP_BYTES;
                     ptx::mbar_wait(STAGE_FULL + 8 * hf, lt & 1);
-                    if (hf == 0) TRACE(1, lt);
                     ptx::tc_fence_after_sync();
 #pragma unroll
                     for (int mt = 0; mt < Dc::MT; ++mt) {
@@ -176,7 +175,6 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
                     }
                     ptx::mma_commit(STAGE_EMPTY + 8 * hf);
                 }
-                TRACE(3, lt);
                 cur_c = c;
             }
         }
@@ -211,16 +209,13 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
             // After this barrier every repack thread has passed its waits of the previous tile, and a
             // slot's previous fill always belongs to an earlier tile (nslot > copies per tile).
             ptx::named_bar_sync(1, 256);
-            if (ot == 0) TRACE(4, lt);
             const bool part = pl < tl.NP && pl < np_eff;
             const bool valid = part && wy0 + wyl < g.nwh;
             const uint32_t kk = box ? k + 2 * box * (pl / box) + box * o + pl % box : k + 2 * pl + o;
             const int slot = kk % nslot;
             const int bslot = box ? slot - slot % box : slot;      // the barrier pair that covers this image
             if (part) ptx::mbar_wait(FULL(bslot), (kk / nslot) & 1);
-            if (ot == 0) TRACE(5, lt);
             ptx::mbar_wait(STAGE_EMPTY + 8 * hf, (lt & 1) ^ 1);      // the MMAs of tile lt-1 have read this half
-            if (ot == 0) TRACE(6, lt);
             const uint8_t* img = ring + (size_t)slot * tl.S + (pbox ? ((c * (int)plane_elems) & 7) * 2 : 0);
             {
                 uint32_t wv[Dc::NV * 4];
@@ -243,7 +238,6 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
             ptx::fence_proxy_async_smem();
             ptx::mbar_arrive(STAGE_FULL + 8 * hf);
             if (part) ptx::mbar_arrive(EMPTY(bslot));
-            if (ot == 0) TRACE(7, lt);
             k += 2 * np_eff;
 
             const bool seg_end = t + 1 == t1 || (t + 1) - c * tl.tiles_per_c == tl.tiles_per_c;
@@ -251,7 +245,6 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
                 // ---- S (TMEM) -> bins -> dT[c]
                 ptx::mbar_wait(STAGE_EMPTY, lt & 1);        // every MMA of this channel segment has completed
                 ptx::mbar_wait(STAGE_EMPTY + 8, lt & 1);
-                if (ot == 0) TRACE(8, lt);
                 ptx::tc_fence_after_sync();
                 for (int b = lane; b < Dc::BN; b += 32) bw[b] = 0.f;
                 if constexpr (HIER)
@@ -275,7 +268,6 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
                         for (int u = 0; u < NU; ++u)
                             if (g0 + u * RJ_STRIDE < WS) ptx::tmem_ld_n<WS>(taddr + (g0 + u * RJ_STRIDE) * WS, v[u]);
                         ptx::tmem_wait_ld();
-                        if (ot == 0 && g0 == 0) TRACE(13, lt);
 #pragma unroll
                         for (int cj = 0; cj < WS; ++cj) {
                             float old[NU];
@@ -301,13 +293,10 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
                                 __syncwarp();
                             }
                         }
-                        if (ot == 0 && g0 == 0) TRACE(14, lt);
                     }
                 }
-                if (ot == 0) TRACE(10, lt);
                 ptx::tc_fence_before_sync();
                 ptx::named_bar_sync(1, 256);
-                if (ot == 0) TRACE(11, lt);
                 for (int b = ot; b < Cf::NB; b += 256) {
                     float sacc = 0.f;
                     const int bp = (b / Cf::TW) * Dc::BP + b % Cf::TW;
@@ -326,13 +315,11 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
                     }
                 }
                 ptx::named_bar_sync(1, 256);
-                if (ot == 0) TRACE(12, lt);
                 // the bins aliased the operand stage: restore the zero padding vectors
                 for (int i = ot; i < 8 * (Dc::BN + Dc::LBN) * 4 / 16 + 1; i += 256)
                     if (i * 16 < Dc::STAGE) reinterpret_cast<uint4*>(stage)[i] = make_uint4(0, 0, 0, 0);
                 ptx::fence_proxy_async_smem();
                 ptx::named_bar_sync(1, 256);
-                if (ot == 0) TRACE(9, lt);
             }
         }
     }
@@ -452,7 +439,7 @@ cudaError_t launch_dt(const Geom& g, const TcTiles& tl_in, const void* x, const 
         }
     }
     const size_t smem = (size_t)DtCfg<WS>::FIXED + (size_t)nslot * tl.S;
-    static SmemOptIn smem_state = {0, 0};
+    static SmemOptIn smem_state;
     cudaError_t e = ensure_dynamic_smem(reinterpret_cast<const void*>(k), smem, &smem_state);
     if (e != cudaSuccess) return e;
     int grid = (int)(tl.ntiles < num_sms() ? tl.ntiles : num_sms());
@@ -528,18 +515,6 @@ cudaError_t tc_grad_table(const Geom& g, int dtype, const void* x, const void* d
 }
 
 
-#ifdef WBMM_TRACE
-extern "C" __attribute__((visibility("default"))) int wbmm_debug_trace_dt(long long* out)
-{
-    return (int)cudaMemcpyFromSymbol(out, tcdev::g_trace, sizeof(long long) * 256);
-}
-#endif
 
-#ifdef WBMM_WATCHDOG
-extern "C" __attribute__((visibility("default"))) int wbmm_debug_watchdog(unsigned long long* out)
-{
-    return (int)cudaMemcpyFromSymbol(out, ptx::g_watchdog, sizeof(unsigned long long) * 64);
-}
-#endif
 
 }  // namespace wbmm

@@ -608,7 +608,7 @@ cudaError_t launch_f32(const Geom& g, const TcTiles& tl, int nslot, const void* 
     auto k = tc_f32_kernel<WS, GEN>;
     const int out_bytes = f32_out_bytes<WS>(g, tl);
     const size_t smem = (size_t)F32Smem<WS>::FIXED + (size_t)nslot * tl.S + 2 * (size_t)out_bytes;
-    static SmemOptIn smem_state = {0, 0};
+    static SmemOptIn smem_state;
     static std::mutex mu;
     static TilePart cached;
     static long long key_n = -1;

@@ -185,8 +185,6 @@ tc_nhwc_kernel(Geom g, NhwcTiles nt, const uint16_t* __restrict__ x, const uint1
         const uint16_t* xg = x + cg * kCG;
         uint16_t* yg = y + cg * kCG;
 
-        const int ltile = (int)(t - t0);
-        if (tid == 0) TRACE(0, ltile);
         // ---- 1. gather + transpose: planar frame kc, pixel idx <- x[b0+p, h, v, cg*8 + kc]
         for (int i0 = tid; i0 < npx; i0 += kThreadsN * PB) {
             uint4 px[PB];
@@ -213,7 +211,6 @@ tc_nhwc_kernel(Geom g, NhwcTiles nt, const uint16_t* __restrict__ x, const uint1
         }
         __syncthreads();
 
-        if (tid == 0) TRACE(1, ltile);
         const bool valid = pl < np_eff && wy0 + wyl < g.nwh;
         for (int kc = 0; kc < kCG; ++kc) {
             const int c = cg * kCG + kc;
@@ -239,7 +236,6 @@ tc_nhwc_kernel(Geom g, NhwcTiles nt, const uint16_t* __restrict__ x, const uint1
                 ptx::tc_fence_before_sync();
             }
             __syncthreads();
-            if (tid == 0 && kc == 0) TRACE(2, ltile);
             // ---- 2c. contraction
             if (warp == 4 && lane == 0) {
                 ptx::tc_fence_after_sync();
@@ -258,7 +254,6 @@ tc_nhwc_kernel(Geom g, NhwcTiles nt, const uint16_t* __restrict__ x, const uint1
             ptx::mbar_wait(bar, phase);
             phase ^= 1;
             ptx::tc_fence_after_sync();
-            if (tid == 0 && kc == 0) TRACE(3, ltile);
             // ---- 2d. rounded results back into the channel's planar frame, in place
             if (warp < 4) {
                 auto drain_half = [&](auto hc) {
@@ -275,9 +270,7 @@ tc_nhwc_kernel(Geom g, NhwcTiles nt, const uint16_t* __restrict__ x, const uint1
                 ptx::tc_fence_before_sync();
             }
             __syncthreads();
-            if (tid == 0 && kc == 0) TRACE(4, ltile);
         }
-        if (tid == 0) TRACE(5, ltile);
 
         // ---- 3. transpose back + scatter: y[b0+p, h, v, cg*8 ..] <- the 8 planar frames (un-shift, crop)
         for (int idx = tid; idx < npx; idx += kThreadsN) {
@@ -295,7 +288,6 @@ tc_nhwc_kernel(Geom g, NhwcTiles nt, const uint16_t* __restrict__ x, const uint1
             }
         }
         __syncthreads();
-        if (tid == 0) TRACE(6, ltile);
     }
     ptx::tc_fence_before_sync();
     __syncthreads();
@@ -395,8 +387,6 @@ tc_nhwc_tma_kernel(Geom g, NhwcTiles nt, const __grid_constant__ CUtensorMap mx,
         const int b0 = gb * nt.NP, wy0 = strip * nt.NSY;
         const int np_eff = min(nt.NP, g.B - b0);
 
-        const int ltile = (int)(t - t0);
-        if (tid == 0) TRACE(0, ltile);
         // ---- 1. the frame: one tensor-map box per image
         if (tid == 0) {
             ptx::mbar_arrive_expect_tx(load_bar, (uint32_t)np_eff * img_bytes);
@@ -405,7 +395,6 @@ tc_nhwc_tma_kernel(Geom g, NhwcTiles nt, const __grid_constant__ CUtensorMap mx,
         }
         ptx::mbar_wait(load_bar, load_phase);
         load_phase ^= 1;
-        if (tid == 0) TRACE(1, ltile);
 
         const bool valid = pl < np_eff && pl < nt.NP && wy0 + wyl < g.nwh;
         const uint8_t* wsrc = frame + (valid ? win_byte : 0u);
@@ -428,7 +417,6 @@ tc_nhwc_tma_kernel(Geom g, NhwcTiles nt, const __grid_constant__ CUtensorMap mx,
                 }
                 ptx::tc_fence_before_sync();
             }
-            if (tid == 0 && kp == 0) TRACE(2, ltile);
             uint32_t keep[Bc::NH * NWH];                 // channel 2kp's rounded results, until 2kp+1's are there
 #pragma unroll
             for (int q = 0; q < 2; ++q) {
@@ -462,11 +450,9 @@ tc_nhwc_tma_kernel(Geom g, NhwcTiles nt, const __grid_constant__ CUtensorMap mx,
                     }
                     ptx::mma_commit(mma_bar);
                 }
-                if (tid == 0 && kp == 0 && q == 0) TRACE(7, ltile);
                 ptx::mbar_wait(mma_bar, mma_phase);
                 mma_phase ^= 1;
                 ptx::tc_fence_after_sync();
-                if (tid == 0 && kp == 0 && q == 0) TRACE(3, ltile);
                 // ---- 2d. results: keep channel 2kp in registers, interleave with 2kp+1 and store 32 bits per pixel
                 if (warp < 4) {
                     auto drain_half = [&](auto hc) {
@@ -493,10 +479,8 @@ tc_nhwc_tma_kernel(Geom g, NhwcTiles nt, const __grid_constant__ CUtensorMap mx,
                     ptx::tc_fence_before_sync();
                 }
                 __syncthreads();
-                if (tid == 0 && kp == 0 && q == 0) TRACE(4, ltile);
             }
         }
-        if (tid == 0) TRACE(5, ltile);
 
         // ---- 3. the frame back to y: one tensor-map box per image (padding clipped by the copy engine)
         ptx::fence_proxy_async_smem();
@@ -508,7 +492,6 @@ tc_nhwc_tma_kernel(Geom g, NhwcTiles nt, const __grid_constant__ CUtensorMap mx,
             ptx::bulk_wait_read<0>();
         }
         __syncthreads();
-        if (tid == 0) TRACE(6, ltile);
     }
     ptx::tc_fence_before_sync();
     __syncthreads();
@@ -568,7 +551,7 @@ cudaError_t launch_nhwc_tma(const Geom& g, const NhwcTiles& nt, const CUtensorMa
 {
     auto k = tc_nhwc_tma_kernel<WS, BF16>;
     const size_t smem = (size_t)NhwcTmaSmem<WS>::FIXED + (size_t)nt.NP * (((size_t)nt.frame_px * 16 + 127) / 128 * 128);
-    static SmemOptIn smem_state = {0, 0};
+    static SmemOptIn smem_state;
     cudaError_t e = ensure_dynamic_smem(reinterpret_cast<const void*>(k), smem, &smem_state);
     if (e != cudaSuccess) return e;
     const int grid = (int)(nt.ntiles < num_sms() ? nt.ntiles : num_sms());
@@ -582,7 +565,7 @@ cudaError_t launch_nhwc(const Geom& g, const NhwcTiles& nt, const void* x, const
 {
     auto k = tc_nhwc_kernel<WS, BF16>;
     const size_t smem = (size_t)NhwcSmem<WS>::FIXED + (size_t)nt.NP * nt.frame_px * 16;
-    static SmemOptIn smem_state = {0, 0};
+    static SmemOptIn smem_state;
     cudaError_t e = ensure_dynamic_smem(reinterpret_cast<const void*>(k), smem, &smem_state);
     if (e != cudaSuccess) return e;
     const int grid = (int)(nt.ntiles < num_sms() ? nt.ntiles : num_sms());
@@ -592,12 +575,6 @@ cudaError_t launch_nhwc(const Geom& g, const NhwcTiles& nt, const void* x, const
 
 }  // namespace
 
-#ifdef WBMM_TRACE
-extern "C" __attribute__((visibility("default"))) int wbmm_debug_trace_nhwc(long long* out)
-{
-    return (int)cudaMemcpyFromSymbol(out, tcdev::g_trace, sizeof(long long) * 256);
-}
-#endif
 
 bool tc_nhwc_supported(const Geom& g, int dtype, const void* x, const void* y)
 {
