@@ -174,8 +174,15 @@ struct BulkSmem {
 
 // STRIP (with GEN): general addressing on strips of window rows in rolled row order (maps with more than 128
 // windows per image); a template flag so that the whole-image general form pays nothing for it.
+// CTAs per SM: two for the aligned w = 7 form (96 registers, 128 TMEM columns, tiles of 12.5 KB: the hand-off
+// latencies of one CTA's pipeline are hidden by the other's), one otherwise.
+template <int WS, bool GEN>
+constexpr int bulk_ctas_per_sm() { return (WS == 7 && !GEN) ? 2 : 1; }
+template <int WS>
+constexpr int bulk_tmem_cols() { return (2 * ((BulkCfg<WS>::A_COLS + 31) / 32 * 32) + BulkCfg<WS>::D_COLS) <= 128 ? 128 : 512; }
+
 template <int WS, bool BF16, bool GEN, bool STRIP>
-__global__ void __launch_bounds__(kThreadsB, 1)
+__global__ void __launch_bounds__(kThreadsB, bulk_ctas_per_sm<WS, GEN>())
 tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const uint16_t* __restrict__ x, const uint16_t* __restrict__ T,
                const uint16_t* __restrict__ Tl, uint16_t* __restrict__ y, int reverse, int box, int sbox,
                const __grid_constant__ CUtensorMap mx, const __grid_constant__ CUtensorMap my,
@@ -213,7 +220,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
     // Output hand-off groups: the smallest runs of whole epilogue warps that cover whole frame images
     // (lanes are image-major), so a group's images can be stored as soon as ITS warps are done.
     const OutGroups og = out_groups(tl, wpf);
-    if (warp == 1) { ptx::tmem_alloc(ptx::smem_u32(&tmem_base_s), 512); }
+    if (warp == 1) ptx::tmem_alloc(ptx::smem_u32(&tmem_base_s), bulk_tmem_cols<WS>());
     if (tid >= 64 && tid < 64 + nslot) {
         ptx::mbar_init(FULL(tid - 64), 1);
         ptx::mbar_init(EMPTY(tid - 64), box ? box * wpf : wpf);   // box mode: one barrier pair per group of `box` images
@@ -628,7 +635,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
     }
     ptx::tc_fence_before_sync();
     __syncthreads();
-    if (warp == 1) ptx::tmem_dealloc(tmem, 512);
+    if (warp == 1) ptx::tmem_dealloc(tmem, bulk_tmem_cols<WS>());
 }
 
 // Shared memory left after the weights / tables / barriers is cut into frame-image slots: an output
@@ -640,12 +647,12 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
 // DESIGN.md section 7.7); less starves small tiles (w = 7: 12.5 KB per tile).
 // Returns false when a tile of output plus a tile + 1 of input does not fit.
 template <int WS>
-bool bulk_slots(const TcTiles& tl, int wpf, int* nslot, int* nout)
+bool bulk_slots(const TcTiles& tl, int wpf, int* nslot, int* nout, int ctas = 1)
 {
     const OutGroups og = out_groups(tl, wpf);
-    const long long room = 227ll * 1024 - 1024 - BulkSmem<WS>::FIXED;
+    const long long room = (ctas == 1 ? 227ll * 1024 : 113ll * 1024) - 1024 - BulkSmem<WS>::FIXED;
     const long long total = room / tl.S, out_tile = (long long)og.n * og.images;
-    constexpr long long kSide = 96 * 1024;
+    const long long kSide = 96 * 1024 / ctas;
     long long depth = (kSide + out_tile * tl.S / 2) / (out_tile * tl.S);
     if (depth > kMaxOutBufs / og.n) depth = kMaxOutBufs / og.n;
     while (depth > 1 && total - depth * out_tile < tl.NP + 1) --depth;
@@ -792,31 +799,41 @@ cudaError_t launch_bulk(const Geom& g, const TcTiles& tl_in, const void* x, cons
     memset(&my, 0, sizeof(my));
     int sbox = 0, box = 0;
     const int wpf = tl.NSY * g.nww;
-    if (((long long)g.H * g.W * 2) % 16 != 0) {
-        // plane boxes (see plane_box_images): loads by tensor map, stores by the store warp's own 8-byte stores
-        box = plane_box_images(g, tl_in);
-        if (box == 0 || !plane_box_map(g, BF16 ? WBMM_DTYPE_BF16 : WBMM_DTYPE_F16, x, box, &mx)) return cudaErrorInvalidConfiguration;
-        sbox = 2;
-        tl.S = (int)(((long long)g.H * g.W + 14) / 8 * 8 * 2);
-        if (!bulk_slots<WS>(tl, wpf, &nslot, &nout)) return cudaErrorInvalidConfiguration;
-        nslot -= nslot % box;
-        if (nslot < tl.NP + box) return cudaErrorInvalidConfiguration;
-    } else {
+    // shared-memory plan for `ctas` CTAs per SM; false when nothing fits
+    auto configure = [&](int ctas) -> bool {
+        tl = tl_in;
+        sbox = box = 0;
+        if (((long long)g.H * g.W * 2) % 16 != 0) {
+            // plane boxes (see plane_box_images): loads by tensor map, stores by the store warp's own 8-byte stores
+            box = plane_box_images(g, tl_in);
+            if (box == 0 || !plane_box_map(g, BF16 ? WBMM_DTYPE_BF16 : WBMM_DTYPE_F16, x, box, &mx)) return false;
+            sbox = 2;
+            tl.S = (int)(((long long)g.H * g.W + 14) / 8 * 8 * 2);
+            if (!bulk_slots<WS>(tl, wpf, &nslot, &nout, ctas)) return false;
+            nslot -= nslot % box;
+            return nslot >= tl.NP + box;
+        }
         box = bulk_box_mode(g, tl_in, BF16 ? WBMM_DTYPE_BF16 : WBMM_DTYPE_F16, x, y, &tl.S, &sbox, &mx, &my);
         if (box) {
-            if (bulk_slots<WS>(tl, wpf, &nslot, &nout)) nslot -= nslot % box;      // groups never wrap around the ring
-            if (nslot < tl.NP + box) {                                            // (does not fit: one copy per image)
-                box = sbox = 0;
-                tl = tl_in;
-            }
+            nslot = 0;
+            if (bulk_slots<WS>(tl, wpf, &nslot, &nout, ctas)) nslot -= nslot % box;      // groups never wrap around the ring
+            if (nslot >= tl.NP + box) return true;
+            box = sbox = 0;                                                             // (does not fit: one copy per image)
+            tl = tl_in;
         }
+        return bulk_slots<WS>(tl, wpf, &nslot, &nout, ctas);
+    };
+    int ctas = bulk_ctas_per_sm<WS, GEN>();
+    if (!configure(ctas)) {
+        if (ctas == 1) return cudaErrorInvalidConfiguration;
+        ctas = 1;
+        if (!configure(ctas)) return cudaErrorInvalidConfiguration;
     }
-    if (!box && !bulk_slots<WS>(tl, wpf, &nslot, &nout)) return cudaErrorInvalidConfiguration;
     const size_t smem = (size_t)BulkSmem<WS>::FIXED + (size_t)(nslot + nout * out_groups(tl, wpf).images) * tl.S;
     static SmemOptIn smem_state;
     cudaError_t e = ensure_dynamic_smem(reinterpret_cast<const void*>(k), smem, &smem_state);
     if (e != cudaSuccess) return e;
-    int grid = (int)(tl.ntiles < num_sms() ? tl.ntiles : num_sms());
+    int grid = (int)(tl.ntiles < (long long)num_sms() * ctas ? tl.ntiles : (long long)num_sms() * ctas);
     if (grid > kMaxGrid) grid = kMaxGrid;
     // the schedule depends on (tiles, tiles per channel, grid) only: keep the last one
     static std::mutex mu;

@@ -663,7 +663,7 @@ __device__ __forceinline__ void build_lib14_local(const uint8_t* lib, const uint
 
 constexpr int kThreadsB = 352;
 constexpr int kMaxSlots = 96;
-constexpr int kMaxGrid = 160;
+constexpr int kMaxGrid = 320;     // up to two CTAs per SM (w = 7)
 constexpr int kMaxOutBufs = 16;  // output group buffers of the bulk kernel
 
 // Output hand-off groups of the bulk kernel: the smallest runs of whole epilogue warps that cover
