@@ -817,3 +817,92 @@ def test_table_gradient_exact_on_small_integers(wb, oracle, name, case, layout):
     torch.cuda.synchronize()
     _, rdT = oracle.backward(widen(x), np.zeros((C, case.bins)), widen(dy), case.w, case.shift, layout, need_dx=False)
     assert np.array_equal(widen(dT), rdT), float(np.abs(widen(dT) - rdT).max())
+
+
+# ------------------------------------------------------------------ soak: thousands of launches, many shapes, two streams
+SOAK = [
+    si.Case("k_w14_56", 19, 5, 56, 56, 14, seed=401, backward=True),
+    si.Case("k_w14_28_boxes", 40, 12, 28, 28, 14, seed=402, backward=True),
+    si.Case("k_w14_28_shift", 24, 9, 28, 28, 14, shift=(7, 7), seed=403, backward=True),
+    si.Case("k_w14_shift_even", 9, 7, 28, 56, 14, shift=(3, 4), seed=404, backward=True),
+    si.Case("k_w14_ragged", 7, 6, 60, 60, 14, seed=405, backward=True),
+    si.Case("k_w14_ragged_shift", 6, 5, 36, 40, 14, shift=(5, 9), seed=406, backward=True),
+    si.Case("k_w14_112", 5, 4, 112, 112, 14, seed=407, backward=True),
+    si.Case("k_w14_112_shift", 3, 3, 112, 112, 14, shift=(7, 7), seed=408, backward=True),
+    si.Case("k_w14_224", 2, 3, 224, 224, 14, seed=409, backward=True),
+    si.Case("k_w14_14_planes", 72, 6, 14, 14, 14, seed=410, backward=True),
+    si.Case("k_w14_f16", 10, 9, 42, 56, 14, dtype="f16", shift=(0, 7), seed=411, backward=True),
+    si.Case("k_w7_56", 21, 6, 56, 56, 7, seed=412, backward=True),
+    si.Case("k_w7_28_shift", 13, 7, 28, 28, 7, shift=(3, 2), seed=413, backward=True),
+    si.Case("k_w7_ragged", 6, 4, 30, 60, 7, seed=414, backward=True),
+    si.Case("k_w7_112", 3, 5, 112, 112, 7, seed=415, backward=True),
+    si.Case("k_w7_112_shift", 3, 4, 112, 112, 7, shift=(3, 4), seed=416, backward=True),
+    si.Case("k_w7_14_planes", 24, 6, 14, 14, 7, shift=(3, 0), seed=417, backward=True),
+    si.Case("k_nhwc_w14", 6, 16, 28, 56, 14, layout=NHWC, shift=(0, 7), seed=418, backward=True),
+    si.Case("k_nhwc_w7", 9, 8, 28, 28, 7, layout=NHWC, seed=419, backward=True),
+    si.Case("k_f32_w14", 9, 5, 28, 56, 14, dtype="f32", seed=420, backward=True),
+    si.Case("k_f32_w7_shift", 5, 7, 28, 28, 7, dtype="f32", shift=(3, 2), seed=421, backward=True),
+    si.Case("k_many_channels", 8, 300, 28, 28, 14, seed=422, backward=True),        # > 148 tiles, several channels per CTA
+]
+
+
+def test_soak_many_shapes_two_streams(wb, oracle):
+    """>= 5000 launches cycling through 22 shapes x {forward, dX, dT, hierarchical forward} from two host threads on two
+    streams, every result checked on the device against ONE oracle evaluation per shape.  The pipelined kernels hand
+    work between warps through mbarrier phase parities; a protocol slip shows up as a hang or as a stale tile only
+    under the right timing, which single calls with a synchronise after each do not produce."""
+    import threading
+    items = []
+    for c in SOAK:
+        d = si.make(c, device="cuda")
+        xw, Tw, gw = widen(d["x"]), widen(d["T"]), widen(d["dy"])
+        ry = oracle.forward(xw, Tw, c.w, c.shift, c.layout)
+        rdx, rdT = oracle.backward(xw, Tw, gw, c.w, c.shift, c.layout)
+        ref = {"y": torch.from_numpy(ry).cuda(), "dx": torch.from_numpy(rdx).cuda(), "dT": torch.from_numpy(rdT).cuda()}
+        Tl = None
+        if c.w == 14 and c.layout == NCHW and c.dtype != "f32":
+            Tl = (torch.randn((c.C, 169), generator=torch.Generator().manual_seed(c.seed)) * 0.02).to(d["T"].dtype).cuda()
+            ref["hy"] = torch.from_numpy(oracle.hier_forward(xw, Tw, widen(Tl), c.w, c.shift, c.layout, "train")).cuda()
+        nwin = c.B * (-(-c.H // c.w)) * (-(-c.W // c.w))
+        items.append((c, d, Tl, ref, float(np.sqrt(nwin * c.w * c.w))))
+    torch.cuda.synchronize()
+    n_per_thread = 2600
+    fails, counts = [], [0, 0]
+
+    def err(got, ref, tol, scale=1.0):      # stays on the device: launches of different kernels run back to back
+        return ((got.double() - ref).abs() / (tol * (scale + ref.abs()))).max()
+
+    def work(tid):
+        st = torch.cuda.Stream()
+        with torch.cuda.stream(st):
+            worst = torch.zeros((), dtype=torch.float64, device="cuda")
+            for it in range(n_per_thread):
+                c, d, Tl, ref, dscale = items[(it * 7 + tid * 11) % len(items)]
+                op = (it // len(items) + tid) % 4
+                tol = TOL[c.dtype]
+                if op == 0:
+                    e = err(wb.wbmm_forward(d["x"], d["T"], c.w, c.shift, c.layout), ref["y"], tol)
+                elif op == 1:
+                    e = err(wb.wbmm_backward(None, d["T"], d["dy"], c.w, c.shift, c.layout, need_dT=False)[0], ref["dx"], tol)
+                elif op == 2:
+                    e = err(wb.wbmm_backward(d["x"], None, d["dy"], c.w, c.shift, c.layout, need_dx=False)[1], ref["dT"], 1e-4, dscale)
+                elif Tl is not None:
+                    e = err(wb.wbmm_hier_forward(d["x"], d["T"], Tl, c.w, c.shift, c.layout), ref["hy"], tol)
+                else:
+                    e = err(wb.wbmm_forward(d["x"], d["T"], c.w, c.shift, c.layout), ref["y"], tol)
+                worst = torch.maximum(worst, torch.nan_to_num(e, nan=1e30))
+                counts[tid] += 1
+                if it % 200 == 199 and not float(worst) <= 1.0:
+                    fails.append((tid, it, c.name, float(worst)))
+                    return
+            if not float(worst) <= 1.0:
+                fails.append((tid, "end", float(worst)))
+        st.synchronize()
+
+    th = [threading.Thread(target=work, args=(i,)) for i in range(2)]
+    for t in th:
+        t.start()
+    for t in th:
+        t.join()
+    assert not fails, fails
+    assert sum(counts) >= 5000
