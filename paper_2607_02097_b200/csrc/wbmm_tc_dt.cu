@@ -57,7 +57,10 @@ struct DtCfg {
 
 // HIER: S is folded a second time, onto the bins of the local (w/2 x w/2) sub-window table -- only pairs
 // (i, j) inside the same sub-window count (Eq. 9: diag_blocks(M_l)).
-template <int WS, bool BF16, bool GEN, bool HIER>
+// STRIP (with GEN): general addressing on strips of window rows held in ROLLED row order (shifted / ragged maps
+// whose whole frame images do not fit, or with more than 128 windows per image): the producer moves a strip as up
+// to two runs of image rows, so rows never wrap inside the frame and only the columns do (as in tc_bulk_kernel).
+template <int WS, bool BF16, bool GEN, bool HIER, bool STRIP = false>
 __global__ void __launch_bounds__(kThreadsD, 1)
 tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __restrict__ x,
              const uint16_t* __restrict__ dy, float* __restrict__ dT, float* __restrict__ dTl, int box, int pbox,
@@ -113,7 +116,7 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
         b0 = gb * tl.NP;
         wy0 = strip * tl.NSY;
         np_eff = min(tl.NP, g.B - b0);
-        rows_eff = GEN ? g.H : min(tl.frame_rows, g.H - wy0 * WS);
+        rows_eff = GEN ? (!STRIP ? g.H : min(tl.frame_rows, g.Hp - wy0 * WS)) : min(tl.frame_rows, g.H - wy0 * WS);
     };
 
     if (warp == 0) {
@@ -136,6 +139,29 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
                     ptx::tma_load_4d(ptx::smem_u32(ring + (size_t)slot * tl.S), (j & 1) ? &mg : &mx, pbox ? (c * (int)plane_elems) & ~7 : 0, 0,
                                      pbox ? 0 : c, b0 + (j >> 1) * box, FULL(slot));
                 }
+            } else if constexpr (STRIP) {
+                // The strip's rolled rows are up to two runs of image rows (none when it lies in the padding: the barrier
+                // then completes on the arrival alone).  One bulk copy per lane and pass: run A with the byte count of
+                // both runs, then run B.  (Two copies issued by the same lane inside one divergent loop body lost copies
+                // as soon as four lanes were active -- the reason the first strip variant of this kernel hung.)
+                const StripRuns sr = strip_runs(g, wy0 * WS, rows_eff);
+                for (int j = lane; j < 2 * np_eff; j += 32) {
+                    const uint32_t kk = k + j;
+                    const int slot = kk % nslot;
+                    ptx::mbar_wait(EMPTY(slot), ((kk / nslot) & 1) ^ 1);
+                    const uint16_t* pl0 = ((j & 1) ? dy : x) + ((long long)(b0 + (j >> 1)) * g.C + c) * plane_elems;
+                    ptx::mbar_arrive_expect_tx(FULL(slot), (uint32_t)(sr.nA + sr.nB) * rowB);
+                    if (sr.nA > 0)
+                        ptx::bulk_g2s(ptx::smem_u32(ring + (size_t)slot * tl.S), pl0 + (long long)sr.a0 * g.W, (uint32_t)sr.nA * rowB, FULL(slot));
+                }
+                __syncwarp();
+                if (sr.nB > 0)
+                    for (int j = lane; j < 2 * np_eff; j += 32) {
+                        const uint32_t kk = k + j;
+                        const int slot = kk % nslot;
+                        const uint16_t* pl0 = ((j & 1) ? dy : x) + ((long long)(b0 + (j >> 1)) * g.C + c) * plane_elems;
+                        ptx::bulk_g2s(ptx::smem_u32(ring + (size_t)slot * tl.S) + sr.n1 * rowB, pl0, (uint32_t)sr.nB * rowB, FULL(slot));
+                    }
             } else
             for (int j = lane; j < 2 * np_eff; j += 32) {
                 const uint32_t kk = k + j;
@@ -190,7 +216,8 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
         uint8_t* dst = stage + hf * Dc::HALF + (o ? 0 : Dc::OP_BYTES) + (m & 63) * 16;
         constexpr bool WG = GEN || (WS % 2 == 1);   // word-granular window addressing (GenAddr)
         GenAddr<WG ? WS : 1> ga;
-        if constexpr (GEN) gen_addr_init<WS>(ga, g, wyl, wx);
+        if constexpr (STRIP) gen_addr_init_strip<WS>(ga, g, wyl, wx);
+        else if constexpr (GEN) gen_addr_init<WS>(ga, g, wyl, wx);
         else if constexpr (WG) gen_addr_init_plain<WS>(ga, g.W, wyl, wx);
         float* bins = reinterpret_cast<float*>(stage);
         float* bw = bins + (ot >> 5) * Dc::BN;          // this warp's private copy of the bins
@@ -211,6 +238,9 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
             ptx::named_bar_sync(1, 256);
             const bool part = pl < tl.NP && pl < np_eff;
             const bool valid = part && wy0 + wyl < g.nwh;
+            if constexpr (STRIP) {
+                if (ragged) ga.rowmask = gen_strip_rowmask<WS>(g, wy0 + wyl);
+            }
             const uint32_t kk = box ? k + 2 * box * (pl / box) + box * o + pl % box : k + 2 * pl + o;
             const int slot = kk % nslot;
             const int bslot = box ? slot - slot % box : slot;      // the barrier pair that covers this image
@@ -352,7 +382,9 @@ int dt_mode(const Geom& g, const TcTiles& tl, const void* x, const void* dy)
     if (plain && (pb || (tl.frame_rows * g.W * 2) % 16 == 0) && (WS % 2 == 0 || g.W % 2 == 0)) return 1;   // odd w: rows must be word-aligned
     // general form: whole images in natural layout, word-granular window addressing (W, W' even)
     // (an odd W' -- ragged maps at odd w -- is fine without a column shift: nothing wraps)
-    return (tl.nstrips == 1 && g.W % 2 == 0 && (g.Wp % 2 == 0 || g.sw == 0)) ? 2 : 0;
+    // strips of window rows (maps with more than 128 windows per image, or whose whole images do not fit): rolled-order
+    // frames loaded as runs of whole image rows -- rows of 16-byte multiples
+    return ((tl.nstrips == 1 || (g.W * 2) % 16 == 0) && g.W % 2 == 0 && (g.Wp % 2 == 0 || g.sw == 0)) ? 2 : 0;
 }
 
 // Tiling of the table-gradient kernel.  Its ring holds x AND dy and shares the SM with the 106 KB operand stage,
@@ -364,28 +396,31 @@ bool dt_tiles(const Geom& g, TcTiles* t)
 {
     if (!tc_tiles(g, t)) return false;
     const bool plain = g.sh == 0 && g.sw == 0 && g.H == g.Hp && g.W == g.Wp;
+    const bool strip_ok = plain || (g.W * 2) % 16 == 0;     // general form on strips: runs of whole image rows
     if (dt_slots<WS>(*t) >= 2 * t->NP + 1) return true;
-    if (!plain || (t->nstrips == 1 && t->S <= 8192)) {
-        if (t->nstrips != 1) return true;
-        // shifted / ragged maps need whole images (general addressing), and tiny maps have more images per tile than
-        // the ring has slots for x and dy: fewer images per tile instead; the windows a tile then lacks are zero
-        // columns of the contraction
+    auto fewer_images = [&]() {
+        // whole images (general addressing without row runs), and tiny maps with more images per tile than the ring has
+        // slots for x and dy: fewer images per tile; the windows a tile then lacks are zero columns of the contraction
         TcTiles c = *t;
         while (c.NP > 1 && dt_slots<WS>(c) < 2 * c.NP + 1) c.NP /= 2;
         c.ngb = (g.B + c.NP - 1) / c.NP;
         c.tiles_per_c = c.ngb * c.nstrips;
         c.ntiles = (long long)g.C * c.tiles_per_c;
         if (dt_slots<WS>(c) >= 2 * c.NP + 1) *t = c;
+    };
+    if (!strip_ok || (t->nstrips == 1 && t->S <= 8192)) {
+        if (t->nstrips == 1) fewer_images();
         return true;
     }
     for (int nsy = t->NSY - 1; nsy >= 1; --nsy) {
-        if (g.nwh % nsy != 0 || (nsy * g.w * g.W * 2) % 16 != 0) continue;
+        // aligned form: whole strips of a window-multiple map, as one copy; general form: any strip, row by row runs
+        if (plain && (g.nwh % nsy != 0 || (nsy * g.w * g.W * 2) % 16 != 0)) continue;
         TcTiles c = *t;
         c.NSY = nsy;
         c.NP = 128 / (nsy * g.nww);
         if (c.NP > g.B) c.NP = g.B;
         if (c.NP < 1) continue;
-        c.nstrips = g.nwh / nsy;
+        c.nstrips = (g.nwh + nsy - 1) / nsy;
         c.ngb = (g.B + c.NP - 1) / c.NP;
         c.tiles_per_c = c.ngb * c.nstrips;
         c.frame_rows = nsy * g.w;
@@ -398,14 +433,15 @@ bool dt_tiles(const Geom& g, TcTiles* t)
             return true;
         }
     }
+    if (!plain && t->nstrips == 1) fewer_images();
     return true;    // nothing fits: dt_mode() rejects the original tiling
 }
 
-template <int WS, bool BF16, bool GEN, bool HIER = false>
+template <int WS, bool BF16, bool GEN, bool HIER = false, bool STRIP = false>
 cudaError_t launch_dt(const Geom& g, const TcTiles& tl_in, const void* x, const void* dy, float* dT, cudaStream_t s,
                       float* dTl = nullptr)
 {
-    auto k = tc_dt_kernel<WS, BF16, GEN, HIER>;
+    auto k = tc_dt_kernel<WS, BF16, GEN, HIER, STRIP>;
     TcTiles tl = tl_in;
     CUtensorMap mx, mg;
     memset(&mx, 0, sizeof(mx));
@@ -490,12 +526,20 @@ cudaError_t tc_grad_table(const Geom& g, int dtype, const void* x, const void* d
     if (tl.ntiles == 0) return cudaSuccess;
     const int mode = g.w == 7 ? dt_mode<7>(g, tl, x, dy) : dt_mode<14>(g, tl, x, dy);
     if (mode == 0) return cudaErrorNotSupported;
+    if (dTl && g.w != 14) return cudaErrorNotSupported;
     *launches += 1;
     *path = WBMM_PATH_TC_TMA;
     const bool bf = dtype == WBMM_DTYPE_BF16;
+    if (mode == 2 && tl.nstrips > 1) {      // general addressing on strips of window rows
+        if (dTl) return bf ? launch_dt<14, true, true, true, true>(g, tl, x, dy, dT, stream, dTl)
+                           : launch_dt<14, false, true, true, true>(g, tl, x, dy, dT, stream, dTl);
+        if (g.w == 7) return bf ? launch_dt<7, true, true, false, true>(g, tl, x, dy, dT, stream)
+                                : launch_dt<7, false, true, false, true>(g, tl, x, dy, dT, stream);
+        return bf ? launch_dt<14, true, true, false, true>(g, tl, x, dy, dT, stream)
+                  : launch_dt<14, false, true, false, true>(g, tl, x, dy, dT, stream);
+    }
     if (dTl) {
         // hierarchical: both table gradients from one pass over (x, dy)
-        if (g.w != 14) return cudaErrorNotSupported;
         if (mode == 2) return bf ? launch_dt<14, true, true, true>(g, tl, x, dy, dT, stream, dTl)
                                  : launch_dt<14, false, true, true>(g, tl, x, dy, dT, stream, dTl);
         return bf ? launch_dt<14, true, false, true>(g, tl, x, dy, dT, stream, dTl)
@@ -518,3 +562,11 @@ cudaError_t tc_grad_table(const Geom& g, int dtype, const void* x, const void* d
 
 
 }  // namespace wbmm
+
+#ifdef WBMM_WATCHDOG
+// debug build only (wbmm_debug.cuh): the waiters this translation unit's kernels gave up on
+extern "C" __attribute__((visibility("default"))) int wbmm_debug_watchdog_dt(unsigned long long* out)
+{
+    return (int)cudaMemcpyFromSymbol(out, wbmm::ptx::g_watchdog, sizeof(unsigned long long) * 64);
+}
+#endif
