@@ -696,6 +696,36 @@ def run_paper_shapes(args):
                 torch.cuda.empty_cache()
 
 
+PROFILE_CASES = {
+    "cfg3_fwd": (si.CFG3, "fwd"), "cfg2_fwd": (si.CFG2, "fwd"),
+    "cfg5_fwd": (si.with_(si.CFG5, backward=False), "fwd"), "cfg5_dX": (si.CFG5, "dX"), "cfg5_dT": (si.CFG5, "dT"),
+    "cfg3_shape_dT": (si.with_(si.CFG3, backward=True), "dT"),
+    "fp32_w14_fwd": (si.with_(si.CFG3, dtype="f32"), "fwd"),
+    "fp32_w7_fwd": (si.Case("f32w7", 128, 96, 56, 56, 7, dtype="f32", seed=86), "fwd"),
+    "nhwc_cfg3_fwd": (si.with_(si.CFG3, layout=si.NHWC), "fwd"),
+}
+
+
+def run_profile_case(name: str):
+    """--profile-case NAME: five launches of one kernel on one named workload and nothing else -- the command the
+    `ncu --set full` captures under profiles/ are taken with (a number printed under a profiler is never a result)."""
+    import paper_2607_02097_b200 as wb
+    case, op = PROFILE_CASES[name]
+    torch.cuda.set_device(0)
+    d = si.make(case, device="cuda")
+    y = torch.empty_like(d["x"])
+    dT = torch.empty((case.C, case.bins), dtype=torch.float32, device="cuda")
+    for _ in range(5):
+        if op == "fwd":
+            wb.wbmm_forward(d["x"], d["T"], case.w, case.shift, case.layout, out=y)
+        elif op == "dX":
+            wb.wbmm_backward(None, d["T"], d["dy"], case.w, case.shift, case.layout, need_dT=False, dx=y)
+        else:
+            wb.wbmm_backward(d["x"], None, d["dy"], case.w, case.shift, case.layout, need_dx=False, dT=dT)
+    torch.cuda.synchronize()
+    print(json.dumps({"profile_case": name, "op": op, "path": wb.wbmm_path_string(wb.wbmm_last_path())}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -706,7 +736,11 @@ def main():
     ap.add_argument("--ref-seconds", type=float, default=100.0, help="--impl reference: CPU seconds for the whole run")
     ap.add_argument("--paper-shapes", action="store_true",
                     help="time the shapes of the paper's Table 13 (B=128, C=256) in bf16 and fp32 (one JSON line per case)")
+    ap.add_argument("--profile-case", choices=sorted(PROFILE_CASES), help="five launches of one kernel on one workload (for ncu)")
     args = ap.parse_args()
+    if args.profile_case:
+        run_profile_case(args.profile_case)
+        return
     if args.sweep:
         run_sweep(args)
         return
