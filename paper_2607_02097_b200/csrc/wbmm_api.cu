@@ -132,6 +132,14 @@ int apply(const wbmm_desc_t* d, const wbmm::Geom& g, const void* x, const void* 
 {
     int launches = 0;
     cudaError_t e;
+    if (g.layout == WBMM_LAYOUT_NHWC && !(d->flags & WBMM_FLAG_FORCE_SIMT) && wbmm::tc_nhwc_pipe_supported(g, d->dtype, x, y)) {
+        // w = 7: one pass straight from NHWC memory, no scratch
+        e = wbmm::tc_nhwc_pipe_forward(g, d->dtype, x, T, y, reverse, stream, &launches);
+        g_launches += launches;
+        if (e != cudaSuccess) return set_cuda_error(e, "tc_nhwc_pipe_forward");
+        t_last_path = WBMM_PATH_TC_TMA;
+        return WBMM_STATUS_OK;
+    }
     if (nhwc_scratch_candidate(d, g)) {
         wbmm::Geom gn = g;
         gn.layout = WBMM_LAYOUT_NCHW;

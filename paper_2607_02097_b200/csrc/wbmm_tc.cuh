@@ -42,6 +42,11 @@ bool tc_f32_supported(const Geom& g, const void* x, const void* y);
 cudaError_t tc_f32_forward(const Geom& g, const void* x, const void* T, void* y, bool reverse, cudaStream_t stream,
                            int* launches);
 
+// NHWC forward / dX, w = 7, one pass straight from NHWC memory on the pipelined skeleton (wbmm_tc_nhwc7.cu): no shift.
+bool tc_nhwc_pipe_supported(const Geom& g, int dtype, const void* x, const void* y);
+cudaError_t tc_nhwc_pipe_forward(const Geom& g, int dtype, const void* x, const void* T, void* y, bool reverse,
+                                 cudaStream_t stream, int* launches);
+
 // NHWC forward / dX: 8-channel groups gathered with 16-byte cp.async (wbmm_tc_nhwc.cu).
 bool tc_nhwc_supported(const Geom& g, int dtype, const void* x, const void* y);
 cudaError_t tc_nhwc_forward(const Geom& g, int dtype, const void* x, const void* T, void* y, bool reverse,

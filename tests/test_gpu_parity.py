@@ -135,8 +135,11 @@ PIPE = [
 
 
 def _nhwc_path(wb, case, flags):
-    """NHWC: transposition scratch around the NCHW kernels when C and H*W are multiples of 8, else (or with
-    FLAG_NO_SCRATCH) the in-kernel 8-channel-group kernels."""
+    """NHWC forward / dX: w = 7 without a shift runs in one pass straight from NHWC memory (pipelined 8-channel-group
+    kernel); otherwise transposition scratch around the NCHW kernels when C and H*W are multiples of 8, else (or with
+    FLAG_NO_SCRATCH) the block-synchronous 8-channel-group kernels."""
+    if case.w == 7 and tuple(case.shift) == (0, 0) and case.C % 8 == 0:
+        return wb.PATH_TC_TMA
     via_scratch = not (flags & wb.FLAG_NO_SCRATCH) and case.C % 8 == 0 and (case.H * case.W) % 8 == 0
     return wb.PATH_TC_TRANSPOSED if via_scratch else wb.PATH_TC_GATHER
 
@@ -470,6 +473,54 @@ def test_hier_unsupported_shapes_fail_loudly(wb):
     with pytest.raises(wb.WbmmError):       # w = 7 has no hierarchical tensor-core path
         wb.wbmm_hier_forward(x, torch.zeros((4, 169), dtype=torch.bfloat16, device="cuda"),
                              torch.zeros((4, 36), dtype=torch.bfloat16, device="cuda"), 7)
+
+
+# ------------------------------------------------------------------ NHWC in one pass (w = 7)
+NHWC7 = [
+    si.Case("n7_oct4_56", 21, 32, 56, 56, 7, layout=NHWC, seed=501),                # 32-channel groups, strips of 3 window rows
+    si.Case("n7_oct4_28_many", 40, 96, 28, 28, 7, layout=NHWC, seed=502),           # 2 images per tile, 3 groups, > 148 tiles
+    si.Case("n7_oct4_112", 3, 64, 112, 112, 7, layout=NHWC, seed=503),              # 16 windows per row: 2 rows per tile
+    si.Case("n7_oct4_ragged", 6, 32, 30, 60, 7, layout=NHWC, seed=504),             # W' = 63, H' = 35: zero fill / clipping by the copy engine
+    si.Case("n7_oct2_56", 21, 16, 56, 56, 7, layout=NHWC, seed=505),                # 16-channel groups (C = 16)
+    si.Case("n7_oct2_ragged_f16", 5, 48, 26, 30, 7, layout=NHWC, dtype="f16", seed=506),
+    si.Case("n7_oct1_28", 33, 8, 28, 56, 7, layout=NHWC, seed=507),                 # 8-channel groups
+    si.Case("n7_oct1_c24", 5, 24, 26, 30, 7, layout=NHWC, seed=508),
+    si.Case("n7_tiny_maps", 50, 32, 14, 14, 7, layout=NHWC, seed=509),              # 4 windows per image, 8 images per tile
+    si.Case("n7_one_window_maps", 70, 64, 7, 7, 7, layout=NHWC, seed=510),          # the S4 stage: one window per image
+]
+
+
+@pytest.mark.parametrize("case", NHWC7, ids=lambda c: c.name)
+def test_nhwc_one_pass_w7(wb, oracle, case):
+    """NHWC forward and dX straight from NHWC memory (tensor-map boxes of 32 / 16 / 8 channels per pixel, swizzled
+    frames, channel octets on the TMEM lane quarters): the path BASELINE.json north_star (a) asks for."""
+    d = si.make(case, device="cuda")
+    y = wb.wbmm_forward(d["x"], d["T"], case.w, case.shift, case.layout)
+    assert wb.wbmm_last_path() == wb.PATH_TC_TMA, wb.wbmm_path_string(wb.wbmm_last_path())
+    dx, _ = wb.wbmm_backward(None, d["T"], d["x"], case.w, case.shift, case.layout, need_dT=False)
+    assert wb.wbmm_last_path() == wb.PATH_TC_TMA
+    ry = oracle.forward(widen(d["x"]), widen(d["T"]), case.w, case.shift, case.layout)
+    rdx, _ = oracle.backward(widen(d["x"]), widen(d["T"]), widen(d["x"]), case.w, case.shift, case.layout, need_dT=False)
+    tol = TOL[case.dtype]
+    assert max_err_over_tol(y, ry, tol) <= 1.0 and max_err_over_tol(dx, rdx, tol) <= 1.0
+
+
+def test_nhwc_one_pass_w7_one_hot_bins_bitwise(wb, oracle):
+    """Every one of the 169 bins as a one-hot table, one bin per channel (C = 192: six 32-channel groups), on a ragged
+    map: the result must equal the oracle's bitwise -- the Toeplitz blocks, the two-rows-per-K-step operand order,
+    the swizzled addressing and the channel interleave of the in-place epilogue."""
+    C = 192
+    case = si.Case("n7_onehot", 3, C, 30, 44, 7, layout=NHWC, seed=511)
+    d = si.make(case, device="cuda")
+    T = torch.zeros_like(d["T"])
+    bins = torch.arange(C) % 169
+    T[torch.arange(C), bins.to(T.device)] = 1.0
+    y = wb.wbmm_forward(d["x"], T, 7, layout=NHWC)
+    assert wb.wbmm_last_path() == wb.PATH_TC_TMA
+    assert np.array_equal(widen(y), oracle.forward(widen(d["x"]), widen(T), 7, layout=NHWC))
+    dx, _ = wb.wbmm_backward(None, T, d["x"], 7, layout=NHWC, need_dT=False)
+    rdx, _ = oracle.backward(widen(d["x"]), widen(T), widen(d["x"]), 7, layout=NHWC, need_dT=False)
+    assert np.array_equal(widen(dx), rdx)
 
 
 def test_config1_fp32_tiny(wb, oracle):
