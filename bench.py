@@ -703,6 +703,7 @@ PROFILE_CASES = {
     "fp32_w14_fwd": (si.with_(si.CFG3, dtype="f32"), "fwd"),
     "fp32_w7_fwd": (si.Case("f32w7", 128, 96, 56, 56, 7, dtype="f32", seed=86), "fwd"),
     "nhwc_cfg3_fwd": (si.with_(si.CFG3, layout=si.NHWC), "fwd"),
+    "nhwc_cfg2_shape_B128_fwd": (si.Case("nhwc_w7", 128, 96, 56, 56, 7, layout=si.NHWC, seed=87), "fwd"),
 }
 
 
