@@ -168,7 +168,12 @@ int apply(const wbmm_desc_t* d, const wbmm::Geom& g, const void* x, const void* 
         t_last_path = WBMM_PATH_TC_GATHER;
         return WBMM_STATUS_OK;
     }
-    if (!(d->flags & WBMM_FLAG_FORCE_SIMT) && wbmm::tc_forward_supported(g, d->dtype, x, y)) {
+    // The pipelined kernel where it applies.  Shapes only the block-synchronous gather kernel could take (planes that no
+    // copy scheme addresses: 7 x 7, 30 x 30, odd W) go to the FFMA kernels instead when those fit: measured 1.4-2.3x
+    // faster there (B128 C256 7x7 w7: 41.8 vs 21.3 us; B64 C96 30x30 w14: 226 vs 164 us).
+    const bool pipelined = g.layout == WBMM_LAYOUT_NCHW && wbmm::tc_bulk_supported(g, d->dtype, x, y);
+    if (!(d->flags & WBMM_FLAG_FORCE_SIMT) && wbmm::tc_forward_supported(g, d->dtype, x, y) &&
+        (pipelined || !wbmm::simt_supported(g))) {
         int path = WBMM_PATH_NONE;
         e = wbmm::tc_forward(g, d->dtype, x, T, nullptr, y, reverse, stream, &launches, &path);
         g_launches += launches;

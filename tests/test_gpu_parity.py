@@ -135,13 +135,17 @@ PIPE = [
 
 
 def _nhwc_path(wb, case, flags):
-    """NHWC forward / dX: w = 7 without a shift runs in one pass straight from NHWC memory (pipelined 8-channel-group
+    """NHWC forward / dX: w = 7 without a shift runs in one pass straight from NHWC memory (pipelined channel-group
     kernel); otherwise transposition scratch around the NCHW kernels when C and H*W are multiples of 8, else (or with
-    FLAG_NO_SCRATCH) the block-synchronous 8-channel-group kernels."""
+    FLAG_NO_SCRATCH) the block-synchronous 8-channel-group kernels -- which need an even W' at odd w; what is left
+    (here: W' = 63) takes the FFMA kernels."""
     if case.w == 7 and tuple(case.shift) == (0, 0) and case.C % 8 == 0:
         return wb.PATH_TC_TMA
     via_scratch = not (flags & wb.FLAG_NO_SCRATCH) and case.C % 8 == 0 and (case.H * case.W) % 8 == 0
-    return wb.PATH_TC_TRANSPOSED if via_scratch else wb.PATH_TC_GATHER
+    if via_scratch:
+        return wb.PATH_TC_TRANSPOSED
+    Wp = -(-case.W // case.w) * case.w
+    return wb.PATH_SIMT if (case.w % 2 == 1 and Wp % 2 == 1) else wb.PATH_TC_GATHER
 
 
 @pytest.mark.parametrize("case", PIPE, ids=lambda c: c.name)
