@@ -279,6 +279,11 @@ int wbmm_backward(const wbmm_desc_t* desc, const void* x, const void* T, const v
             g_launches += launches;
             if (e != cudaSuccess) return set_cuda_error(e, "tc_grad_table");
             t_last_path = path;
+        } else if (desc->dtype == WBMM_DTYPE_F32 && !(desc->flags & WBMM_FLAG_FORCE_SIMT) && wbmm::tc_f32_grad_table_supported(g, x, dy)) {
+            e = wbmm::tc_f32_grad_table(g, x, dy, dT, stream, &launches);
+            g_launches += launches;
+            if (e != cudaSuccess) return set_cuda_error(e, "tc_f32_grad_table");
+            t_last_path = WBMM_PATH_TC_TMA;
         } else {
             if (!wbmm::simt_supported(g)) return WBMM_STATUS_UNSUPPORTED;
             e = wbmm::simt_grad_table(g, desc->dtype, x, dy, dT, stream, &launches);

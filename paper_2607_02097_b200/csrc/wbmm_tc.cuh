@@ -42,6 +42,10 @@ bool tc_f32_supported(const Geom& g, const void* x, const void* y);
 cudaError_t tc_f32_forward(const Geom& g, const void* x, const void* T, void* y, bool reverse, cudaStream_t stream,
                            int* launches);
 
+// FP32 table gradient on the tensor cores: split operands, 3 (w = 14) / 6 (w = 7) passes (wbmm_tc_f32_dt.cu).  Adds into dT.
+bool tc_f32_grad_table_supported(const Geom& g, const void* x, const void* dy);
+cudaError_t tc_f32_grad_table(const Geom& g, const void* x, const void* dy, float* dT, cudaStream_t stream, int* launches);
+
 // NHWC forward / dX, w = 7, one pass straight from NHWC memory on the pipelined skeleton (wbmm_tc_nhwc7.cu): no shift.
 bool tc_nhwc_pipe_supported(const Geom& g, int dtype, const void* x, const void* y);
 cudaError_t tc_nhwc_pipe_forward(const Geom& g, int dtype, const void* x, const void* T, void* y, bool reverse,
