@@ -359,6 +359,21 @@ def other_rooflines(wb, dev, stream, hbm_peak):
                       "note": "includes the dT zeroing launch"}
     del xs, gs, dxs, d
     torch.cuda.empty_cache()
+
+    # float32 table gradient (3-way / 2-way bf16 split on the tensor cores): reads x and dy once
+    for name, cf in (("fp32_B128_C96_56x56_w14_dT", si.with_(si.CFG3, dtype="f32", backward=True)),
+                     ("fp32_B128_C96_56x56_w7_dT", si.Case("f32w7", 128, 96, 56, 56, 7, dtype="f32", backward=True, seed=86))):
+        d = si.make(cf, device=dev)
+        ns = buffer_sets(2.0 * cf.n_elem * 4)
+        xs = [d["x"]] + [d["x"].clone() for _ in range(ns - 1)]
+        gs = [d["dy"]] + [d["dy"].clone() for _ in range(ns - 1)]
+        dT = torch.empty((cf.C, cf.bins), dtype=torch.float32, device=dev)
+        ms = region_ms_rot(lambda i: wb.wbmm_backward(xs[i % ns], None, gs[i % ns], cf.w, cf.shift, need_dx=False, dT=dT), 10, stream)
+        by = 2 * cf.n_elem * 4 + cf.C * cf.bins * 4
+        out[name] = {"ms": round(ms, 5), "gbs": round(by / ms / 1e6, 1), "frac": round(by / (hbm_peak * 1e9) * 1e3 / ms, 4),
+                     "path": wb.wbmm_path_string(wb.wbmm_last_path()), "buffer_sets": ns, "note": "includes the dT zeroing launch"}
+        del xs, gs, d
+        torch.cuda.empty_cache()
     return out
 
 
@@ -517,6 +532,10 @@ def run_wbmm(args, rank, world, local):
     Tl = (torch.randn((case.C, (case.w - 1) ** 2), generator=g_l) * 0.02).to(T.dtype).to(dev)
     hier_ms = region_ms(lambda: wb.wbmm_hier_forward(xs[0], T, Tl, case.w, out=ys[0]))
     train_step["hier_forward_cfg3_ms"] = hier_ms
+    # cached-M mode (WBMM-C) on the headline shape: given matrices through the gather kernel -- context
+    Mc = wb.wbmm_materialize_weight(T, case.w)
+    train_step["cached_matrix_forward_cfg3_ms"] = region_ms(lambda: wb.wbmm_forward_matrix(xs[0], Mc, case.w, out=ys[0]))
+    del Mc
     # ... and its backward on the config-5 shape: dX (transposed fused operator) + both table gradients in one pass
     g_l5 = torch.Generator(device="cpu").manual_seed(78)
     Tl5 = (torch.randn((c5.C, (c5.w - 1) ** 2), generator=g_l5) * 0.02).to(d5["T"].dtype).to(dev)
@@ -702,6 +721,8 @@ PROFILE_CASES = {
     "cfg3_shape_dT": (si.with_(si.CFG3, backward=True), "dT"),
     "fp32_w14_fwd": (si.with_(si.CFG3, dtype="f32"), "fwd"),
     "fp32_w7_fwd": (si.Case("f32w7", 128, 96, 56, 56, 7, dtype="f32", seed=86), "fwd"),
+    "fp32_w14_dT": (si.with_(si.CFG3, dtype="f32", backward=True), "dT"),
+    "fp32_w7_dT": (si.Case("f32w7", 128, 96, 56, 56, 7, dtype="f32", backward=True, seed=86), "dT"),
     "nhwc_cfg3_fwd": (si.with_(si.CFG3, layout=si.NHWC), "fwd"),
     "nhwc_cfg2_shape_B128_fwd": (si.Case("nhwc_w7", 128, 96, 56, 56, 7, layout=si.NHWC, seed=87), "fwd"),
 }

@@ -24,10 +24,15 @@
  *     do: they return after the result is in host memory).
  *   - Return value: a wbmm_status_t.  Nothing throws or aborts across the ABI.  On a non-zero
  *     status no output buffer has been written.
- *   - NHWC activations (bf16/fp16, C and H*W multiples of 8) are served by transposing to NCHW and back around
- *     the NCHW kernels; the two temporaries come from cudaMallocAsync / cudaFreeAsync on the caller's stream
- *     (stream-ordered, capturable in CUDA graphs) and never outlive the call's work.  WBMM_FLAG_NO_SCRATCH
- *     selects the scratch-free in-kernel NHWC path instead.  Every other path allocates nothing.
+ *   - NHWC activations (bf16/fp16): w = 7 without shift and C a multiple of 8 is served straight from NHWC memory
+ *     by one pipelined kernel (forward and dX; no temporaries).  Other NHWC problems with C and H*W multiples of 8
+ *     are served by transposing to NCHW and back around the NCHW kernels; the two temporaries come from a memory
+ *     pool the library owns (cudaMallocFromPoolAsync / cudaFreeAsync on the caller's stream: stream-ordered,
+ *     capturable in CUDA graphs, released by wbmm_release()) and never outlive the call's work.
+ *     WBMM_FLAG_NO_SCRATCH forbids the temporaries; the call is then served by the slower scratch-free kernels.
+ *     Every other path allocates nothing.
+ *   - float32 activations with w in {7, 14} run on the tensor cores too, each operand split exactly into three
+ *     bf16 parts (error <= 1e-6 relative to sum |W||x|); other w use the FFMA kernels.
  *   - There is no CPU fallback.  Without a CUDA device of compute capability 10.x every compute
  *     entry point returns WBMM_STATUS_NO_DEVICE.
  */
@@ -65,16 +70,19 @@ typedef enum { WBMM_LAYOUT_NCHW = 0, WBMM_LAYOUT_NHWC = 1 } wbmm_layout_t;
 typedef enum {
     WBMM_PATH_NONE = 0,
     WBMM_PATH_SIMT = 1,      /* general fp32-FFMA kernels: any w, dtype, layout, shift, ragged size */
-    WBMM_PATH_TC_TMA = 2,    /* tcgen05/TMEM tensor-core kernels fed by TMA window loads (bf16/fp16) */
-    WBMM_PATH_TC_GATHER = 3, /* tcgen05/TMEM kernels fed by a predicated gather loader (bf16/fp16) */
+    WBMM_PATH_TC_TMA = 2,    /* pipelined tcgen05/TMEM tensor-core kernels fed by TMA (bf16/fp16 NCHW, NHWC w = 7,
+                                and float32 through the 3-way bf16 split) */
+    WBMM_PATH_TC_GATHER = 3, /* block-synchronous tcgen05/TMEM kernels fed by a predicated gather loader (bf16/fp16):
+                                wbmm_forward_matrix, and shapes the FFMA kernels cannot take */
     WBMM_PATH_TC_TRANSPOSED = 4 /* NHWC: transposition passes through stream-ordered scratch around the TC_TMA kernels */
 } wbmm_path_t;
 
 enum {
     WBMM_FLAG_ACCUMULATE_DT = 1u, /* wbmm_backward: add into dT instead of overwriting it */
     WBMM_FLAG_FORCE_SIMT = 2u,    /* never take a tensor-core path (testing / cross-checks) */
-    WBMM_FLAG_NO_SCRATCH = 4u     /* NHWC: never allocate transposition scratch (cudaMallocAsync on the stream); use the
-                                     in-kernel NHWC kernels, which are 2.5-20x slower */
+    WBMM_FLAG_NO_SCRATCH = 4u     /* NHWC: never allocate transposition scratch from the library's pool; problems the
+                                     one-pass NHWC kernel (w = 7, no shift) does not take then run on the
+                                     scratch-free gather / FFMA kernels, which are several times slower */
 };
 
 /* Problem descriptor (plain data, passed by pointer, read during the call only). */
@@ -121,8 +129,9 @@ WBMM_API int wbmm_backward(const wbmm_desc_t *desc, const void *x, const void *T
  *   Tg [in] C*(2w-1)^2, Tl [in] C*(w-1)^2 elements of desc->dtype.  x, y, padding, shift as wbmm_forward.
  *   transpose != 0 applies the transposed fused matrix: dX of the operator for dy in `x`.
  * Gradients: wbmm_hier_backward.
- * Supported where the pipelined tensor-core kernel is: w = 14, bf16/fp16, NCHW, 16-byte aligned planes
- * (H*W even ... see wbmm_last_path); otherwise WBMM_STATUS_UNSUPPORTED.
+ * Supported where the pipelined tensor-core kernel is: w = 14, bf16/fp16, NCHW with 16-byte aligned planes
+ * (H*W even ... see wbmm_last_path), or NHWC through the transposition scratch (C and H*W multiples of 8, no
+ * WBMM_FLAG_NO_SCRATCH); otherwise WBMM_STATUS_UNSUPPORTED.
  */
 WBMM_API int wbmm_hier_forward(const wbmm_desc_t *desc, const void *x, const void *Tg, const void *Tl, void *y,
                       int transpose, void *cuda_stream);
@@ -138,8 +147,8 @@ WBMM_API int wbmm_hier_forward(const wbmm_desc_t *desc, const void *x, const voi
  *                       folded onto both sets of bins.  Overwritten unless WBMM_FLAG_ACCUMULATE_DT.
  *   x may be NULL when the table gradients are not requested; Tg, Tl may be NULL when dx is NULL.
  * Padding, shift and the zero extension of dy as in wbmm_backward.  Supported where the pipelined
- * tensor-core kernels are (w = 14, bf16/fp16, NCHW, 16-byte aligned planes); otherwise
- * WBMM_STATUS_UNSUPPORTED, with nothing launched.
+ * tensor-core kernels are (w = 14, bf16/fp16, NCHW with 16-byte aligned planes, or NHWC through the
+ * transposition scratch); otherwise WBMM_STATUS_UNSUPPORTED, with nothing launched.
  */
 WBMM_API int wbmm_hier_backward(const wbmm_desc_t *desc, const void *x, const void *Tg, const void *Tl, const void *dy,
                        void *dx, float *dTg, float *dTl, void *cuda_stream);

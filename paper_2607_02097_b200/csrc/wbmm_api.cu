@@ -307,8 +307,31 @@ int wbmm_hier_forward(const wbmm_desc_t* desc, const void* x, const void* Tg, co
     if (!aligned(x, es) || !aligned(Tg, es) || !aligned(Tl, es) || !aligned(y, es)) return WBMM_STATUS_MISALIGNED;
     if (device_state() < 0) return WBMM_STATUS_NO_DEVICE;
     wbmm::Geom g = wbmm::make_geom(*desc);
-    if (!wbmm::tc_hier_supported(g, desc->dtype, x, y)) return WBMM_STATUS_UNSUPPORTED;
     int launches = 0, path = WBMM_PATH_NONE;
+    if (g.layout == WBMM_LAYOUT_NHWC) {
+        // the transposition route of wbmm_forward around the same kernel
+        cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+        wbmm::Geom gn = g;
+        gn.layout = WBMM_LAYOUT_NCHW;
+        void* const aligned16 = reinterpret_cast<void*>(256);
+        if (!nhwc_scratch_candidate(desc, g) || !wbmm::tc_hier_supported(gn, desc->dtype, aligned16, aligned16) ||
+            !wbmm::transpose16_supported((long long)g.H * g.W, g.C, x, y))
+            return WBMM_STATUS_UNSUPPORTED;
+        const size_t nbytes = (size_t)g.B * g.C * g.H * g.W * 2;
+        AsyncScratch xt(stream), yt(stream);
+        if (xt.alloc(nbytes) != cudaSuccess || yt.alloc(nbytes) != cudaSuccess) {
+            cudaGetLastError();
+            return WBMM_STATUS_UNSUPPORTED;
+        }
+        cudaError_t e = wbmm::transpose16(x, xt.p, g.B, g.H * g.W, g.C, stream, &launches);
+        if (e == cudaSuccess) e = wbmm::tc_forward(gn, desc->dtype, xt.p, Tg, Tl, yt.p, transpose != 0, stream, &launches, &path);
+        if (e == cudaSuccess) e = wbmm::transpose16(yt.p, y, g.B, g.C, g.H * g.W, stream, &launches);
+        g_launches += launches;
+        if (e != cudaSuccess) return set_cuda_error(e, "hierarchical forward, NHWC via NCHW scratch");
+        t_last_path = WBMM_PATH_TC_TRANSPOSED;
+        return WBMM_STATUS_OK;
+    }
+    if (!wbmm::tc_hier_supported(g, desc->dtype, x, y)) return WBMM_STATUS_UNSUPPORTED;
     cudaError_t e = wbmm::tc_forward(g, desc->dtype, x, Tg, Tl, y, transpose != 0, static_cast<cudaStream_t>(cuda_stream),
                                      &launches, &path);
     g_launches += launches;
@@ -348,13 +371,41 @@ int wbmm_hier_backward(const wbmm_desc_t* desc, const void* x, const void* Tg, c
     if (device_state() < 0) return WBMM_STATUS_NO_DEVICE;
     wbmm::Geom g = wbmm::make_geom(*desc);
     // check both halves before launching either
-    if (dx && !wbmm::tc_hier_supported(g, desc->dtype, dy, dx)) return WBMM_STATUS_UNSUPPORTED;
-    if (dTg && (g.w != 14 || !wbmm::tc_grad_table_supported(g, desc->dtype, x, dy))) return WBMM_STATUS_UNSUPPORTED;
+    const bool nhwc = g.layout == WBMM_LAYOUT_NHWC;
+    wbmm::Geom gn = g;
+    gn.layout = WBMM_LAYOUT_NCHW;
+    void* const aligned16 = reinterpret_cast<void*>(256);
+    if (nhwc) {
+        if (!nhwc_scratch_candidate(desc, g)) return WBMM_STATUS_UNSUPPORTED;
+        if (dx && (!wbmm::tc_hier_supported(gn, desc->dtype, aligned16, aligned16) ||
+                   !wbmm::transpose16_supported((long long)g.H * g.W, g.C, dy, dx)))
+            return WBMM_STATUS_UNSUPPORTED;
+        if (dTg && (g.w != 14 || !wbmm::tc_grad_table_supported(gn, desc->dtype, aligned16, aligned16) ||
+                    !wbmm::transpose16_supported((long long)g.H * g.W, g.C, x, dy)))
+            return WBMM_STATUS_UNSUPPORTED;
+    } else {
+        if (dx && !wbmm::tc_hier_supported(g, desc->dtype, dy, dx)) return WBMM_STATUS_UNSUPPORTED;
+        if (dTg && (g.w != 14 || !wbmm::tc_grad_table_supported(g, desc->dtype, x, dy))) return WBMM_STATUS_UNSUPPORTED;
+    }
     if (dx) {
         st = wbmm_hier_forward(desc, dy, Tg, Tl, dx, 1, cuda_stream);
         if (st != WBMM_STATUS_OK) return st;
     }
-    if (dTg) {
+    if (dTg && nhwc) {
+        const size_t nbytes = (size_t)g.B * g.C * g.H * g.W * 2;
+        AsyncScratch xt(stream), gt(stream);
+        if (xt.alloc(nbytes) != cudaSuccess || gt.alloc(nbytes) != cudaSuccess) {
+            cudaGetLastError();
+            return WBMM_STATUS_UNSUPPORTED;
+        }
+        int launches = 0, path = WBMM_PATH_NONE;
+        cudaError_t e = wbmm::transpose16(x, xt.p, g.B, g.H * g.W, g.C, stream, &launches);
+        if (e == cudaSuccess) e = wbmm::transpose16(dy, gt.p, g.B, g.H * g.W, g.C, stream, &launches);
+        if (e == cudaSuccess) e = wbmm::tc_grad_table(gn, desc->dtype, xt.p, gt.p, dTg, stream, &launches, &path, dTl);
+        g_launches += launches;
+        if (e != cudaSuccess) return set_cuda_error(e, "hierarchical table gradients, NHWC via NCHW scratch");
+        t_last_path = WBMM_PATH_TC_TRANSPOSED;
+    } else if (dTg) {
         int launches = 0, path = WBMM_PATH_NONE;
         cudaError_t e = wbmm::tc_grad_table(g, desc->dtype, x, dy, dTg, stream, &launches, &path, dTl);
         g_launches += launches;

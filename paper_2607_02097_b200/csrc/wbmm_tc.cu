@@ -86,19 +86,35 @@ tc_generic_kernel(Geom g, TcTiles tl, const uint16_t* __restrict__ x, const uint
             else build_weight<WS>(T + (long long)c * Cf::NB, reverse != 0, Ts, Wc, tid, kThreadsG);
             cur_c = c;
         }
-        // frame <- x (padded + shifted coordinates)
-        for (int idx = tid; idx < np_eff * frame_elems; idx += kThreadsG) {
-            const int p = idx / frame_elems, r2 = idx % frame_elems;
-            const int hh = r2 / g.Wp, vv = r2 % g.Wp;
+        // frame <- x (padded + shifted coordinates); eight loads in flight per thread
+        auto src_offset = [&](int idx) -> long long {
+            const int p = idx / frame_elems, r2 = idx - p * frame_elems;
+            const int hh = r2 / g.Wp, vv = r2 - hh * g.Wp;
             const int hp = wy0 * WS + hh;
-            uint16_t val = 0;
-            if (hp < g.Hp) {
-                int h = hp + g.sh, v = vv + g.sw;
-                if (h >= g.Hp) h -= g.Hp;
-                if (v >= g.Wp) v -= g.Wp;
-                if (h < g.H && v < g.W) val = x[act_offset(g, b0 + p, c, h, v)];
+            if (hp >= g.Hp) return -1;
+            int h = hp + g.sh, v = vv + g.sw;
+            if (h >= g.Hp) h -= g.Hp;
+            if (v >= g.Wp) v -= g.Wp;
+            return h < g.H && v < g.W ? act_offset(g, b0 + p, c, h, v) : -1;
+        };
+        auto frame_at = [&](int idx) -> uint16_t* {
+            const int p = idx / frame_elems, r2 = idx - p * frame_elems;
+            return reinterpret_cast<uint16_t*>(frame + p * tl.S + r2 * 2);
+        };
+        const int nfe = np_eff * frame_elems;
+        for (int base = tid; base < nfe; base += 8 * kThreadsG) {
+            uint16_t val[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const int idx = base + u * kThreadsG;
+                const long long off = idx < nfe ? src_offset(idx) : -1;
+                val[u] = off >= 0 ? x[off] : (uint16_t)0;
             }
-            *reinterpret_cast<uint16_t*>(frame + p * tl.S + r2 * 2) = val;
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const int idx = base + u * kThreadsG;
+                if (idx < nfe) *frame_at(idx) = val[u];
+            }
         }
         ptx::fence_proxy_async_smem();   // W_c (generic-proxy stores) -> tcgen05.mma operand reads
         __syncthreads();
@@ -130,17 +146,9 @@ tc_generic_kernel(Geom g, TcTiles tl, const uint16_t* __restrict__ x, const uint
         }
         __syncthreads();
         // y <- frame (un-shift, crop)
-        for (int idx = tid; idx < np_eff * frame_elems; idx += kThreadsG) {
-            const int p = idx / frame_elems, r2 = idx % frame_elems;
-            const int hh = r2 / g.Wp, vv = r2 % g.Wp;
-            const int hp = wy0 * WS + hh;
-            if (hp < g.Hp) {
-                int h = hp + g.sh, v = vv + g.sw;
-                if (h >= g.Hp) h -= g.Hp;
-                if (v >= g.Wp) v -= g.Wp;
-                if (h < g.H && v < g.W)
-                    y[act_offset(g, b0 + p, c, h, v)] = *reinterpret_cast<const uint16_t*>(frame + p * tl.S + r2 * 2);
-            }
+        for (int idx = tid; idx < nfe; idx += kThreadsG) {
+            const long long off = src_offset(idx);
+            if (off >= 0) y[off] = *frame_at(idx);
         }
         __syncthreads();
     }
@@ -412,6 +420,15 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                         for (int qq = rt; qq < 169; qq += 128) FL[qq] = Tlc[reverse ? qq : 168 - qq];
                         ptx::named_bar_sync(2, 128);          // the global library and FL are complete
                         build_lib14_local<BF16>(Wc, FL, hier, rt);
+                    }
+                } else if (Tl) {
+                    // cached-M mode (w = 7 only: `Tl` carries the given matrices [C][N][N]) -- the same
+                    // operand layout, loaded instead of built; the bias row meets the column of ones at K index N + 1
+                    load_weight<WS>(Tl + (long long)c * Cf::N * Cf::N, reverse != 0, Wc, rt, 128);
+                    if (bias) {
+                        ptx::named_bar_sync(2, 128);
+                        for (int i = rt; i < Cf::N; i += 128)
+                            *reinterpret_cast<uint16_t*>(Wc + ((Cf::N + 1) / 8) * Cf::LBO + i * 16 + ((Cf::N + 1) % 8) * 2) = bias[c];
                     }
                 } else {
                     for (int kk = rt; kk < Cf::NB; kk += 128) tab[kk] = Tc[reverse ? Cf::NB - 1 - kk : kk];
@@ -1070,8 +1087,23 @@ cudaError_t tc_forward_matrix(const Geom& g, int dtype, const void* x, const voi
     if (!tc_tiles(g, &tl)) return cudaErrorNotSupported;
     if (tl.ntiles == 0) return cudaSuccess;
     *launches += 1;
-    *path = WBMM_PATH_TC_GATHER;
     const bool bf = dtype == WBMM_DTYPE_BF16;
+    if (g.w == 7) {
+        // w = 7: the pipelined kernel holds the whole 8 KB W_c in shared memory anyway -- the given matrix takes its place
+        const int mode = bulk_mode<7>(g, tl, x, y);
+        if (mode != 0) {
+            *path = WBMM_PATH_TC_TMA;
+            if (mode == 2 && tl.nstrips > 1)
+                return bf ? launch_bulk<7, true, true, true>(g, tl, x, nullptr, M, y, transpose, stream, bias, 0u)
+                          : launch_bulk<7, false, true, true>(g, tl, x, nullptr, M, y, transpose, stream, bias, 0u);
+            if (mode == 2)
+                return bf ? launch_bulk<7, true, true>(g, tl, x, nullptr, M, y, transpose, stream, bias, 0u)
+                          : launch_bulk<7, false, true>(g, tl, x, nullptr, M, y, transpose, stream, bias, 0u);
+            return bf ? launch_bulk<7, true, false>(g, tl, x, nullptr, M, y, transpose, stream, bias, 0u)
+                      : launch_bulk<7, false, false>(g, tl, x, nullptr, M, y, transpose, stream, bias, 0u);
+        }
+    }
+    *path = WBMM_PATH_TC_GATHER;
     if (g.w == 7)
         return bf ? launch_generic<7, true>(g, tl, x, nullptr, y, transpose, stream, M, bias)
                   : launch_generic<7, false>(g, tl, x, nullptr, y, transpose, stream, M, bias);

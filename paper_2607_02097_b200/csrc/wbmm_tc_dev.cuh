@@ -174,17 +174,20 @@ __device__ __forceinline__ void load_weight(const uint16_t* __restrict__ Mc, boo
 {
     using Cf = WinCfg<WS>;
     constexpr int NCHUNK = (Cf::K_PAD / 8) * Cf::N_PAD;
+    constexpr int NKC = Cf::K_PAD / 8;
     for (int id = tid; id < NCHUNK; id += nthreads) {
-        const int kc = id / Cf::N_PAD, i = id % Cf::N_PAD;
+        // neighbouring threads read neighbouring addresses: along a row of M_c, or (transposed) along a column
+        const int kc = transpose ? id / Cf::N_PAD : id % NKC, i = transpose ? id % Cf::N_PAD : id / NKC;
         uint32_t pk[4] = {0u, 0u, 0u, 0u};
         if (i < Cf::N) {
+            uint32_t v[8];
 #pragma unroll
             for (int e = 0; e < 8; ++e) {
                 const int j = kc * 8 + e;
-                uint32_t v = 0;
-                if (j < Cf::N) v = transpose ? Mc[j * Cf::N + i] : Mc[i * Cf::N + j];
-                pk[e >> 1] |= v << ((e & 1) * 16);
+                v[e] = j < Cf::N ? (uint32_t)(transpose ? Mc[j * Cf::N + i] : Mc[i * Cf::N + j]) : 0u;
             }
+#pragma unroll
+            for (int e = 0; e < 8; ++e) pk[e >> 1] |= v[e] << ((e & 1) * 16);
         }
         *reinterpret_cast<uint4*>(Wc + kc * Cf::LBO + i * 16) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
     }

@@ -144,6 +144,39 @@ tc_nhwc7_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const __grid_cons
         wx = wl - wyl * g.nww;
     };
 
+    // The libraries of a channel group (Eq. 6-8): block 1 + (dr + 6), row ci, 8 values cj = 0..7,
+    //     Z[dr][ci][cj] = T[c, (dr + 6) * 13 + (ci - cj + 6)], zero for ci = 7 or cj = 7.
+    // One thread per (channel, dr): the 13 table entries of that row offset are loaded once (all loads in flight
+    // together) and shifted through the seven rows of the block.
+    auto build_lib = [&](int cg, int first, int nthreads) {
+        for (int id = first; id < Pc::CGT * 13; id += nthreads) {
+            const int ch = id / 13, d = id - ch * 13;
+            const uint16_t* Tc = T + (long long)(cg * Pc::CGT + ch) * kNB;
+            uint32_t e[13];
+#pragma unroll
+            for (int j = 0; j < 13; ++j) {
+                const int idx = d * 13 + j;
+                e[j] = Tc[reverse ? kNB - 1 - idx : idx];
+            }
+            uint8_t* blk = lib + ch * kLibBytes + (d + 1) * 128;
+#pragma unroll
+            for (int ci = 0; ci < 7; ++ci) {
+                uint32_t pk[4] = {0u, 0u, 0u, 0u};
+#pragma unroll
+                for (int cj = 0; cj < 7; ++cj) pk[cj >> 1] |= e[ci - cj + 6] << ((cj & 1) * 16);
+                *reinterpret_cast<uint4*>(blk + ci * 16) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+            }
+        }
+    };
+    // the first group's libraries: every warp but the producer, while the first boxes are on their way
+    int first_cg = -1;
+    if (t0 < t1) first_cg = t0 / tl.tiles_per_c;
+    if (warp >= 1 && first_cg >= 0) {
+        build_lib(first_cg, tid - 32, kThreadsP - 32);
+        ptx::fence_proxy_async_smem();
+        ptx::named_bar_sync(1, kThreadsP - 32);
+    }
+
     if (warp == 0) {
         // ------------------------------------------------------------------ producer: one box per window row of an image
         uint32_t k = 0;
@@ -210,7 +243,7 @@ tc_nhwc7_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const __grid_cons
         for (int c = 0; c < WS; ++c) coff[c] = px_addr<NOCT>(p0 + (uint32_t)c, (uint32_t)oct);
         const uint32_t rowB = (uint32_t)g.Wp * Pc::PX;
         uint32_t k = 0, lt = 0;
-        int cur_cg = -1;
+        int cur_cg = first_cg;
         for (int t = t0; t < t1; ++t, ++lt) {
             int cg, b0, wy0, np_eff;
             tile_decode(t, cg, b0, wy0, np_eff);
@@ -220,20 +253,9 @@ tc_nhwc7_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const __grid_cons
             // test of this tile's fill unambiguous.
             ptx::mbar_wait(A_EMPTY, (lt & 1) ^ 1);
             if (cg != cur_cg) {
-                // ---- the libraries of this channel group (Eq. 6-8): block 1 + (dr + 6), row ci, 8 values cj = 0..7
-                //      Z[dr][ci][cj] = T[c, (dr + 6) * 13 + (ci - cj + 6)], zero for ci = 7 or cj = 7
-                for (int id = rt; id < Pc::CGT * 13 * 7; id += 128) {
-                    const int ch = id / 91, rem = id - ch * 91, d = rem / 7, ci = rem - d * 7;
-                    const uint16_t* Tc = T + (long long)(cg * Pc::CGT + ch) * kNB;
-                    uint32_t pk[4] = {0u, 0u, 0u, 0u};
-#pragma unroll
-                    for (int cj = 0; cj < 7; ++cj) {
-                        const int idx = d * 13 + ci - cj + 6;
-                        const uint32_t v = Tc[reverse ? kNB - 1 - idx : idx];
-                        pk[cj >> 1] |= v << ((cj & 1) * 16);
-                    }
-                    *reinterpret_cast<uint4*>(lib + ch * kLibBytes + (d + 1) * 128 + ci * 16) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
-                }
+                // half 1 of the previous tile still reads the old libraries until its MMAs have completed
+                ptx::mbar_wait(A_EMPTY + 8, (lt & 1) ^ 1);
+                build_lib(cg, rt, 128);
                 ptx::fence_proxy_async_smem();
                 cur_cg = cg;
             }
@@ -401,7 +423,9 @@ EncodeTiledFn encode_fn()
     return fn;
 }
 
-// x or y viewed as (C, W, H, B), box {CGT channels, W', 7 rows, 1 image}, swizzled over the pixel's 16-byte chunks
+// x or y viewed as (C, W, H, B), box {CGT channels, W', 7 rows, 1 image}, swizzled over the pixel's 16-byte chunks.
+// 64-byte pixels are fetched as 64-byte L2 requests: with 128-byte promotion the other half of each line (the
+// neighbouring channel group) came along and was fetched again later (97 MB read for a 77 MB input, 2-5 % slower).
 template <int NOCT>
 bool make_map(const Geom& g, int dtype, const void* base, CUtensorMap* map)
 {
@@ -414,7 +438,7 @@ bool make_map(const Geom& g, int dtype, const void* base, CUtensorMap* map)
     const CUtensorMapSwizzle swz = NOCT == 4 ? CU_TENSOR_MAP_SWIZZLE_64B : (NOCT == 2 ? CU_TENSOR_MAP_SWIZZLE_32B : CU_TENSOR_MAP_SWIZZLE_NONE);
     return fn(map, dtype == WBMM_DTYPE_BF16 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 4,
               const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, swz,
-              CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+              NOCT == 4 ? CU_TENSOR_MAP_L2_PROMOTION_L2_64B : CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 // <= 128 / NOCT windows of one channel group per tile: whole frame images, else strips of window rows; a slot is one

@@ -262,6 +262,8 @@ def _hier_case(case):
     si.Case("h_ragged", 7, 6, 60, 60, 14, seed=44),
     si.Case("h_strips", 2, 3, 224, 224, 14, seed=45),
     si.Case("h_f16", 10, 9, 42, 56, 14, dtype="f16", shift=(0, 7), seed=46),
+    si.Case("h_nhwc_shift", 6, 16, 28, 56, 14, shift=(7, 3), layout=NHWC, seed=58),      # transposition route around the same kernel
+    si.Case("h_nhwc_ragged", 5, 24, 60, 60, 14, layout=NHWC, seed=59),
 ], ids=lambda c: c.name)
 @pytest.mark.parametrize("transpose", [False, True])
 def test_hier_forward_matches_oracle(wb, oracle, case, transpose):
@@ -269,7 +271,7 @@ def test_hier_forward_matches_oracle(wb, oracle, case, transpose):
     d, Tl = _hier_case(case)
     y = wb.wbmm_hier_forward(d["x"], d["T"], Tl, case.w, case.shift, case.layout, transpose)
     torch.cuda.synchronize()
-    assert wb.wbmm_last_path() == wb.PATH_TC_TMA
+    assert wb.wbmm_last_path() == (wb.PATH_TC_TRANSPOSED if case.layout == NHWC else wb.PATH_TC_TMA)
     ref = oracle.hier_forward(widen(d["x"]), widen(d["T"]), widen(Tl), case.w, case.shift, case.layout, "train", transpose)
     # |y| is ~2|x| here (two identity shortcuts): same bound form, |ref| carries the scale
     assert max_err_over_tol(y, ref, TOL[case.dtype]) <= 1.0
@@ -314,6 +316,7 @@ def test_hier_one_hot_tables_bitwise(wb, oracle, which):
     si.Case("hb_shift", 9, 7, 28, 56, 14, shift=(7, 3), seed=53, backward=True),
     si.Case("hb_ragged_shift", 7, 6, 60, 60, 14, shift=(5, 9), seed=54, backward=True),
     si.Case("hb_f16", 10, 9, 42, 56, 14, dtype="f16", shift=(0, 7), seed=56, backward=True),
+    si.Case("hb_nhwc_shift", 6, 16, 28, 56, 14, shift=(7, 3), layout=NHWC, seed=60, backward=True),
 ], ids=lambda c: c.name)
 def test_hier_backward_matches_oracle(wb, oracle, case):
     """dx, dTg, dTl of the hierarchical operator: one transposed fused forward and ONE pass of the
@@ -321,7 +324,7 @@ def test_hier_backward_matches_oracle(wb, oracle, case):
     d, Tl = _hier_case(case)
     dx, dTg, dTl = wb.wbmm_hier_backward(d["x"], d["T"], Tl, d["dy"], case.w, case.shift, case.layout)
     torch.cuda.synchronize()
-    assert wb.wbmm_last_path() == wb.PATH_TC_TMA
+    assert wb.wbmm_last_path() == (wb.PATH_TC_TRANSPOSED if case.layout == NHWC else wb.PATH_TC_TMA)
     rdx, rg, rl = oracle.hier_backward(widen(d["x"]), widen(d["T"]), widen(Tl), widen(d["dy"]), case.w, case.shift, case.layout)
     tol = TOL[case.dtype]
     errs = (max_err_over_tol(dx, rdx, tol), max_err_over_tol(dTg, rg, tol), max_err_over_tol(dTl, rl, tol))
@@ -354,6 +357,8 @@ def test_hier_backward_local_bins_exact_on_integers(wb, oracle):
     si.Case("m_w7_shift", 9, 7, 28, 42, 7, shift=(3, 4), seed=62),
     si.Case("m_ragged_nhwc", 3, 8, 30, 45, 14, shift=(7, 2), layout=NHWC, seed=63),
     si.Case("m_f16", 4, 3, 21, 21, 7, dtype="f16", seed=64),
+    si.Case("m_w7_many", 70, 40, 56, 56, 7, seed=68),                    # pipelined kernel, several channels per CTA
+    si.Case("m_w7_strips_shift", 3, 4, 112, 112, 7, shift=(2, 5), seed=69),
 ], ids=lambda c: c.name)
 def test_cached_matrix_mode_equals_the_table_mode(wb, oracle, case):
     """WBMM-C and WBMM-NC "produce identical outputs": forward and dX through
@@ -363,7 +368,9 @@ def test_cached_matrix_mode_equals_the_table_mode(wb, oracle, case):
     M = wb.wbmm_materialize_weight(d["T"], case.w)
     for transpose in (False, True):
         y = wb.wbmm_forward_matrix(d["x"], M, case.w, case.shift, case.layout, transpose=transpose)
-        assert wb.wbmm_last_path() == wb.PATH_TC_GATHER
+        # w = 7 on planes the pipelined kernel takes: the given matrix replaces the W_c it would have built
+        pipelined = case.w == 7 and case.layout == NCHW and case.W % 2 == 0
+        assert wb.wbmm_last_path() == (wb.PATH_TC_TMA if pipelined else wb.PATH_TC_GATHER)
         if transpose:
             ref, _ = wb.wbmm_backward(None, d["T"], d["x"], case.w, case.shift, case.layout, need_dT=False)
             rdx, _ = oracle.backward(widen(d["x"]), widen(d["T"]), widen(d["x"]), case.w, case.shift, case.layout, need_dT=False)
@@ -377,12 +384,17 @@ def test_cached_matrix_mode_equals_the_table_mode(wb, oracle, case):
         assert bool((diff <= ulp * ref.float().abs() + 1e-6).all())
 
 
-def test_cached_matrix_mode_arbitrary_matrix_and_bias(wb, oracle):
+@pytest.mark.parametrize("case", [
+    si.Case("m_any", 5, 6, 30, 44, 14, shift=(2, 9), seed=65),
+    si.Case("m_any_w7", 37, 12, 28, 56, 7, seed=70),                     # pipelined kernel: bias row at K index N + 1
+    si.Case("m_any_w7_ragged_shift", 9, 5, 30, 44, 7, shift=(2, 5), seed=71),
+], ids=lambda c: c.name)
+def test_cached_matrix_mode_arbitrary_matrix_and_bias(wb, oracle, case):
     """A matrix that is NOT table-generated, plus a bias, against the oracle's Algorithm 1."""
-    case = si.Case("m_any", 5, 6, 30, 44, 14, shift=(2, 9), seed=65)
     d = si.make(case, device="cuda")
     g = torch.Generator().manual_seed(66)
-    M = (torch.randn((case.C, 196, 196), generator=g) * 0.05).to(torch.bfloat16).cuda()
+    N = case.w * case.w
+    M = (torch.randn((case.C, N, N), generator=g) * 0.05).to(torch.bfloat16).cuda()
     bias = torch.randn((case.C,), generator=g).to(torch.bfloat16).cuda()
     for transpose in (False, True):
         y = wb.wbmm_forward_matrix(d["x"], M, case.w, case.shift, case.layout, bias, transpose)
