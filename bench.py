@@ -724,6 +724,9 @@ PROFILE_CASES = {
     "fp32_w14_dT": (si.with_(si.CFG3, dtype="f32", backward=True), "dT"),
     "fp32_w7_dT": (si.Case("f32w7", 128, 96, 56, 56, 7, dtype="f32", backward=True, seed=86), "dT"),
     "nhwc_cfg3_fwd": (si.with_(si.CFG3, layout=si.NHWC), "fwd"),
+    "s3_B128_C256_14x14_w14_fwd": (si.Case("s3w14", 128, 256, 14, 14, 14, seed=88), "fwd"),
+    "s3_B128_C256_14x14_w7_fwd": (si.Case("s3w7", 128, 256, 14, 14, 7, seed=89), "fwd"),
+    "s4_B128_C256_7x7_w7_fwd": (si.Case("s4w7", 128, 256, 7, 7, 7, seed=90), "fwd"),
     "nhwc_cfg2_shape_B128_fwd": (si.Case("nhwc_w7", 128, 96, 56, 56, 7, layout=si.NHWC, seed=87), "fwd"),
 }
 

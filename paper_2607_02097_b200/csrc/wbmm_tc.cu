@@ -431,7 +431,12 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                             *reinterpret_cast<uint16_t*>(Wc + ((Cf::N + 1) / 8) * Cf::LBO + i * 16 + ((Cf::N + 1) % 8) * 2) = bias[c];
                     }
                 } else {
-                    for (int kk = rt; kk < Cf::NB; kk += 128) tab[kk] = Tc[reverse ? Cf::NB - 1 - kk : kk];
+                    static_assert(WS == 14 || Cf::NB <= 2 * 128, "two table entries per repack thread");
+                    if (!tabv_ready) table_to_regs7(Tc, reverse != 0, rt, tabv);
+#pragma unroll
+                    for (int u = 0; u < 2; ++u)
+                        if (rt + u * 128 < Cf::NB) tab[rt + u * 128] = tabv[u];
+                    tabv_ready = false;
                     ptx::named_bar_sync(2, 128);
                     constexpr int NCHUNK = (Cf::K_PAD / 8) * Cf::N_PAD;
                     for (int id = rt; id < NCHUNK; id += 128) {
@@ -500,10 +505,13 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
             ptx::tc_fence_before_sync();
             ptx::mbar_arrive(A_FULL + 8 * buf);
             k += np_eff;
-            if constexpr (WS == 14) {
-                // the next tile starts a new channel: have its table row in flight during the next copy
-                if (t + 1 < t1 && (t + 1) - c * tl.tiles_per_c == tl.tiles_per_c) {
+            // the next tile starts a new channel: have its table row in flight during the next copy
+            if (t + 1 < t1 && (t + 1) - c * tl.tiles_per_c == tl.tiles_per_c) {
+                if constexpr (WS == 14) {
                     table_to_regs14(T + (long long)(c + 1) * Cf::NB, reverse != 0, rt, tabv);
+                    tabv_ready = true;
+                } else if (!Tl) {
+                    table_to_regs7(T + (long long)(c + 1) * Cf::NB, reverse != 0, rt, tabv);
                     tabv_ready = true;
                 }
             }

@@ -597,6 +597,17 @@ __device__ __forceinline__ void table_to_regs14(const uint16_t* __restrict__ Tc,
     }
 }
 
+// w = 7: the table row (169 entries) in the order the W_c builder reads it, two entries per thread.
+__device__ __forceinline__ void table_to_regs7(const uint16_t* __restrict__ Tc, bool reverse, int tid, uint16_t* v)
+{
+    using Cf = WinCfg<7>;
+#pragma unroll
+    for (int u = 0; u < 2; ++u) {
+        const int q = tid + u * 128;
+        v[u] = q < Cf::NB ? Tc[reverse ? Cf::NB - 1 - q : q] : (uint16_t)0;
+    }
+}
+
 // Block-Toeplitz library for w = 14 (BulkCfg<14>) from the two staged copies of the reversed table
 // (see build_weight14): chunk (d, ci, kc) = Z[d-13][ci][8kc .. 8kc+7] = F[(26-d)*27 + 13-ci + 8kc + e].
 // 128 threads (the repack warps); rows ci = 14, 15 of every block stay zero from the kernel prologue.
