@@ -727,6 +727,7 @@ PROFILE_CASES = {
     "s3_B128_C256_14x14_w14_fwd": (si.Case("s3w14", 128, 256, 14, 14, 14, seed=88), "fwd"),
     "s3_B128_C256_14x14_w7_fwd": (si.Case("s3w7", 128, 256, 14, 14, 7, seed=89), "fwd"),
     "s4_B128_C256_7x7_w7_fwd": (si.Case("s4w7", 128, 256, 7, 7, 7, seed=90), "fwd"),
+    "s3_B128_C592_14x14_w14_fwd": (si.Case("s3w14big", 128, 592, 14, 14, 14, seed=91), "fwd"),
     "nhwc_cfg2_shape_B128_fwd": (si.Case("nhwc_w7", 128, 96, 56, 56, 7, layout=si.NHWC, seed=87), "fwd"),
 }
 

@@ -189,6 +189,32 @@ constexpr int bulk_ctas_per_sm() { return (WS == 7 && !GEN) ? 2 : 1; }
 template <int WS>
 constexpr int bulk_tmem_cols() { return (2 * ((BulkCfg<WS>::A_COLS + 31) / 32 * 32) + BulkCfg<WS>::D_COLS) <= 128 ? 128 : 512; }
 
+// `np` planes of `chunks` units U each, shared memory (pitch `spitch`) -> global (pitch `dpitch`), by one warp.
+template <typename U>
+__device__ __forceinline__ void copy_planes_out(const uint8_t* src, uint8_t* dst, int np, int spitch, long long dpitch,
+                                                int chunks, int lane)
+{
+    for (int ch = lane; ch < chunks; ch += 32) {
+        const uint8_t* s0 = src + (size_t)ch * sizeof(U);
+        uint8_t* d0 = dst + (size_t)ch * sizeof(U);
+        int p = 0;
+        for (; p + 8 <= np; p += 8) {
+            U v[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) v[u] = *reinterpret_cast<const U*>(s0 + (size_t)u * spitch);
+#pragma unroll
+            for (int u = 0; u < 8; ++u) *reinterpret_cast<U*>(d0 + u * dpitch) = v[u];
+            s0 += 8 * (size_t)spitch;
+            d0 += 8 * dpitch;
+        }
+        for (; p < np; ++p) {
+            *reinterpret_cast<U*>(d0) = *reinterpret_cast<const U*>(s0);
+            s0 += spitch;
+            d0 += dpitch;
+        }
+    }
+}
+
 template <int WS, bool BF16, bool GEN, bool STRIP>
 __global__ void __launch_bounds__(kThreadsB, bulk_ctas_per_sm<WS, GEN>())
 tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const uint16_t* __restrict__ x, const uint16_t* __restrict__ T,
@@ -549,7 +575,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                 accum_half_to_packed<WS, BF16, h>(tmem_d + Hs::col0(h) + ((uint32_t)(q * 32) << 16), pk);
                 ptx::tc_fence_before_sync();
                 ptx::mbar_arrive(D_EMPTY + 8 * h);                                 // the MMAs of the next tile may overwrite this half
-                if (h == 0) ptx::mbar_wait(OUT_EMPTY + 8 * ob, (use & 1) ^ 1);     // the buffer's previous contents have been read out
+                if (h == 0 && sbox != 2) ptx::mbar_wait(OUT_EMPTY + 8 * ob, (use & 1) ^ 1);     // the buffer's previous contents have been read out
                 if (valid) {
                     if constexpr (WG) {
                         if constexpr (GEN && WS % 2 == 0) {
@@ -572,6 +598,23 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
             };
             drain_half(std::integral_constant<int, 0>{});
             if constexpr (Hs::NH > 1) drain_half(std::integral_constant<int, 1>{});
+            if (sbox == 2) {
+                // plane boxes: a plane is not a multiple of 16 bytes, so no bulk store can write it.  A group is this
+                // warp's own images (a warp always covers whole images here), so the warp copies them out itself with
+                // 8-byte stores (4-byte when H*W is not a multiple of 4), lane = chunk of a plane, eight planes in
+                // flight: four warps in parallel instead of the one store warp (which ran at 3 bytes per cycle, bound by
+                // its own instruction latencies: 11 us per tile of 128 14 x 14 planes).
+                __syncwarp();
+                const int p_first = gq * og.images, np = min(og.images, np_eff - p_first);
+                if (np > 0) {
+                    const uint8_t* src = outb + (size_t)ob * out_bytes;
+                    uint8_t* dst = reinterpret_cast<uint8_t*>(y + ((long long)(b0 + p_first) * g.C + c) * plane_elems);
+                    if (plane_elems % 4 == 0) copy_planes_out<uint2>(src, dst, np, tl.S, (long long)g.C * plane_elems * 2, (int)(plane_elems / 4), lane);
+                    else copy_planes_out<uint32_t>(src, dst, np, tl.S, (long long)g.C * plane_elems * 2, (int)(plane_elems / 2), lane);
+                }
+                __syncwarp();
+                continue;
+            }
             ptx::fence_proxy_async_smem();      // generic-proxy writes -> the bulk store's async-proxy reads
             ptx::mbar_arrive(OUT_FULL + 8 * ob);
         }
@@ -585,40 +628,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                 asm volatile("prefetch.global.L2 [%0];" ::"l"(base + off));
         }
         if (sbox == 2) {
-            // plane boxes: a plane is not a multiple of 16 bytes, so no bulk store can write it -- the whole warp
-            // copies the group's planes with 8-byte stores (these maps are small: a few KB per tile)
-            const uint32_t depth = nout / og.n;
-            const uint32_t out_bytes = (uint32_t)og.images * tl.S;
-            const int chunks = (int)(plane_elems * 2 / 8);
-            uint32_t lt = 0;
-            for (int t = t0; t < t1; ++t, ++lt) {
-                int c, b0, wy0, np_eff, rows_eff;
-                tile_decode(t, c, b0, wy0, np_eff, rows_eff);
-                for (int gq = 0; gq < og.n; ++gq) {
-                    const uint32_t ob = (lt % depth) * og.n + gq;
-                    ptx::mbar_wait(OUT_FULL + 8 * ob, (lt / depth) & 1);
-                    const int p_first = gq * og.images, p_end = min(p_first + og.images, np_eff);
-                    // lane = 8-byte chunk of a plane, four planes in flight per step (no division, loads batched)
-                    const uint8_t* src = outb + (size_t)ob * out_bytes;
-                    uint8_t* dst = reinterpret_cast<uint8_t*>(y + ((long long)(b0 + p_first) * g.C + c) * plane_elems);
-                    const long long dstep = (long long)g.C * plane_elems * 2;
-                    const int np = p_end - p_first;
-                    for (int ch = lane; ch < chunks; ch += 32) {
-                        int p = 0;
-                        for (; p + 4 <= np; p += 4) {
-                            uint2 v[4];
-#pragma unroll
-                            for (int u = 0; u < 4; ++u) v[u] = *reinterpret_cast<const uint2*>(src + (size_t)(p + u) * tl.S + ch * 8);
-#pragma unroll
-                            for (int u = 0; u < 4; ++u) *reinterpret_cast<uint2*>(dst + (p + u) * dstep + ch * 8) = v[u];
-                        }
-                        for (; p < np; ++p)
-                            *reinterpret_cast<uint2*>(dst + p * dstep + ch * 8) = *reinterpret_cast<const uint2*>(src + (size_t)p * tl.S + ch * 8);
-                    }
-                    __syncwarp();
-                    if (lane == 0) ptx::mbar_arrive(OUT_EMPTY + 8 * ob);
-                }
-            }
+            // plane boxes: the epilogue warps store their own groups
         } else if (lane < nout) {
             // Lane ob = (frame, gq) owns output buffer ob: group gq of the tiles lt = frame mod depth.  It
             // bulk-stores the group's images and releases the buffer once the copy engine has read it.

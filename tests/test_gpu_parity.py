@@ -247,6 +247,28 @@ def test_planes_that_are_not_multiples_of_16_bytes(wb, oracle, case):
     assert max(errs) <= 1.0, errs
 
 
+@pytest.mark.parametrize("case", [
+    si.Case("pb_7x14_w7", 16, 8, 7, 14, 7, seed=97, backward=True),                  # 196-byte planes: 4-byte store units
+    si.Case("pb_7x14_w7_many", 66, 24, 7, 14, 7, seed=98, backward=True),
+    si.Case("pb_14_w14_many", 130, 40, 14, 14, 14, seed=99, backward=True),          # ragged last tile, several tiles per CTA
+], ids=lambda c: c.name)
+def test_plane_box_store_units(wb, oracle, case):
+    """Planes of 196 bytes (H*W = 98: a multiple of 2 but not of 4) are stored in 4-byte units, 392-byte planes in
+    8-byte units, both by the flat (plane, chunk) walk of the store warp; canaries around the output."""
+    d = si.make(case, device="cuda")
+    n = d["x"].numel()
+    buf = torch.full((n + 64,), 7.0, dtype=d["x"].dtype, device="cuda")
+    y = buf[32:32 + n].view_as(d["x"])
+    wb.wbmm_forward(d["x"], d["T"], case.w, case.shift, out=y)
+    dx, _ = wb.wbmm_backward(None, d["T"], d["dy"], case.w, case.shift, need_dT=False)
+    torch.cuda.synchronize()
+    assert bool((buf[:32] == 7.0).all()) and bool((buf[32 + n:] == 7.0).all())
+    ry = oracle.forward(widen(d["x"]), widen(d["T"]), case.w, case.shift)
+    rdx, _ = oracle.backward(widen(d["x"]), widen(d["T"]), widen(d["dy"]), case.w, case.shift, need_dT=False)
+    tol = TOL[case.dtype]
+    assert max_err_over_tol(y, ry, tol) <= 1.0 and max_err_over_tol(dx, rdx, tol) <= 1.0
+
+
 # ------------------------------------------------------------------ hierarchical reparameterisation (NEXT-1)
 def _hier_case(case):
     d = si.make(case, device="cuda")
