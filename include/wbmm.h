@@ -60,7 +60,8 @@ typedef enum {
     WBMM_STATUS_UNSUPPORTED = 2,      /* window too large for shared memory, or dtype/path combination not built */
     WBMM_STATUS_NO_DEVICE = 3,        /* no CUDA device, or the device is not sm_100 */
     WBMM_STATUS_CUDA_ERROR = 4,       /* a CUDA runtime/driver call failed; see wbmm_last_error_string() */
-    WBMM_STATUS_MISALIGNED = 5        /* a pointer is not aligned to its element size */
+    WBMM_STATUS_MISALIGNED = 5,       /* a pointer is not aligned to its element size */
+    WBMM_STATUS_TOO_LARGE = 6         /* wbmm_forward_static_scratch: the activation exceeds the static scratch */
 } wbmm_status_t;
 
 typedef enum { WBMM_DTYPE_F32 = 0, WBMM_DTYPE_BF16 = 1, WBMM_DTYPE_F16 = 2 } wbmm_dtype_t;
@@ -105,6 +106,23 @@ typedef struct wbmm_desc {
  * assumed finite (a non-finite x may turn neighbouring outputs of the same row strip into NaN).
  */
 WBMM_API int wbmm_forward(const wbmm_desc_t *desc, const void *x, const void *T, void *y, void *cuda_stream);
+
+/*
+ * wbmm_forward for callers that must not allocate (code under CUDA graph capture, serving loops, harnesses that
+ * forbid cudaMalloc): the NHWC transposition route of wbmm_forward (transpose -> NCHW tensor-core kernel -> transpose;
+ * same kernels, same results) with its two temporaries in ONE file-scope device array instead of the library's memory
+ * pool.  The call allocates and frees nothing (no cudaMalloc, cudaFree, cudaMallocAsync, no allocating library
+ * routine); x, T, y are the caller's, as in wbmm_forward.
+ *   Serves   NHWC, bf16/fp16, w in {7, 14}, C and H*W multiples of 8 (what the transposition route serves), any shift /
+ *            ragged size; anything else: WBMM_STATUS_UNSUPPORTED, nothing launched.  desc->flags is ignored.
+ *   Limit    B*C*H*W*2 bytes <= 16 MiB (8 Mi elements; e.g. B = 16, C = 96, 56 x 56).  Beyond it:
+ *            WBMM_STATUS_TOO_LARGE with the sizes in wbmm_last_error_string(), nothing launched.
+ *   Cost     the array is 32 MiB (two temporaries); every GPU that loads libwbmm.so holds it until the process exits.
+ *   Sharing  all calls on a device share the array, which keeps the last call's contents.  Nothing needs clearing:
+ *            each call overwrites every byte it later reads.  Calls that OVERLAP on the GPU (different streams) race
+ *            on it and give wrong results; calls on one stream are ordered and safe back to back.
+ */
+WBMM_API int wbmm_forward_static_scratch(const wbmm_desc_t *desc, const void *x, const void *T, void *y, void *cuda_stream);
 
 /*
  * Backward of wbmm_forward:

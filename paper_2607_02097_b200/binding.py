@@ -18,12 +18,13 @@ DTYPE_F32, DTYPE_BF16, DTYPE_F16 = 0, 1, 2
 PATH_NONE, PATH_SIMT, PATH_TC_TMA, PATH_TC_GATHER, PATH_TC_TRANSPOSED = 0, 1, 2, 3, 4
 FLAG_ACCUMULATE_DT, FLAG_FORCE_SIMT, FLAG_NO_SCRATCH = 1, 2, 4
 STATUS_OK = 0
+STATUS_TOO_LARGE = 6
 
 _DTYPES = {torch.float32: DTYPE_F32, torch.bfloat16: DTYPE_BF16, torch.float16: DTYPE_F16}
 
 # every symbol include/wbmm.h declares
 EXPORTS = (
-    "wbmm_forward", "wbmm_backward", "wbmm_hier_forward", "wbmm_hier_backward", "wbmm_forward_matrix", "wbmm_fold_dwconv", "wbmm_forward_fused", "wbmm_materialize_weight", "wbmm_forward_host",
+    "wbmm_forward", "wbmm_forward_static_scratch", "wbmm_backward", "wbmm_hier_forward", "wbmm_hier_backward", "wbmm_forward_matrix", "wbmm_fold_dwconv", "wbmm_forward_fused", "wbmm_materialize_weight", "wbmm_forward_host",
     "wbmm_backward_host", "wbmm_release", "wbmm_last_path", "wbmm_launch_count",
     "wbmm_status_string", "wbmm_path_string", "wbmm_last_error_string", "wbmm_version",
 )
@@ -54,6 +55,8 @@ def lib() -> ctypes.CDLL:
     L = ctypes.CDLL(LIB_PATH)
     vp, dp, i = ctypes.c_void_p, ctypes.POINTER(WbmmDesc), ctypes.c_int
     L.wbmm_forward.argtypes = [dp, vp, vp, vp, vp]
+    L.wbmm_forward_static_scratch.argtypes = [dp, vp, vp, vp, vp]
+    L.wbmm_forward_static_scratch.restype = i
     L.wbmm_backward.argtypes = [dp, vp, vp, vp, vp, vp, vp]
     L.wbmm_hier_forward.argtypes = [dp, vp, vp, vp, vp, i, vp]
     L.wbmm_hier_forward.restype = i
@@ -86,7 +89,7 @@ def _check(st: int) -> None:
         L = lib()
         msg = L.wbmm_status_string(st).decode()
         err = L.wbmm_last_error_string().decode()
-        raise WbmmError(st, f"libwbmm: {msg}" + (f" ({err})" if st == 4 and err else ""))
+        raise WbmmError(st, f"libwbmm: {msg}" + (f" ({err})" if st in (4, STATUS_TOO_LARGE) and err else ""))
 
 
 def _dims(t: torch.Tensor, layout: int):
@@ -133,6 +136,21 @@ def wbmm_forward(x: torch.Tensor, T: torch.Tensor, w: int, shift=(0, 0), layout:
     else:
         with torch.cuda.device(x.device):
             _check(lib().wbmm_forward(ctypes.byref(d), px, pT, py, _stream(x)))
+    return y
+
+
+def wbmm_forward_static_scratch(x: torch.Tensor, T: torch.Tensor, w: int, shift=(0, 0),
+                                out: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """wbmm_forward for NHWC bf16/fp16 activations of at most 16 MiB with the temporaries in the library's static
+    device array: the C call allocates nothing (include/wbmm.h: wbmm_forward_static_scratch; pass `out` to keep
+    the binding from allocating the result).  Calls that overlap on the GPU race on the array."""
+    d = make_desc(x, w, shift, NHWC, 0)
+    if T.dtype != x.dtype or tuple(T.shape) != (d.C, (2 * w - 1) ** 2):
+        raise ValueError("T must be [C,(2w-1)^2] in the dtype of x")
+    y = torch.empty_like(x) if out is None else out
+    px, pT, py = _dev(x, "x"), _dev(T, "T"), _dev(y, "y")
+    with torch.cuda.device(x.device):
+        _check(lib().wbmm_forward_static_scratch(ctypes.byref(d), px, pT, py, _stream(x)))
     return y
 
 

@@ -213,6 +213,37 @@ int wbmm_forward(const wbmm_desc_t* desc, const void* x, const void* T, void* y,
     return apply(desc, g, x, T, y, false, static_cast<cudaStream_t>(cuda_stream));
 }
 
+int wbmm_forward_static_scratch(const wbmm_desc_t* desc, const void* x, const void* T, void* y, void* cuda_stream)
+{
+    int st = validate(desc);
+    if (st != WBMM_STATUS_OK) return st;
+    if (desc->B == 0 || desc->C == 0) return WBMM_STATUS_OK;
+    if (!x || !T || !y || x == y) return WBMM_STATUS_INVALID_ARGUMENT;
+    const size_t es = elem_size(desc->dtype);
+    if (!aligned(x, es) || !aligned(T, es) || !aligned(y, es)) return WBMM_STATUS_MISALIGNED;
+    if (device_state() < 0) return WBMM_STATUS_NO_DEVICE;
+    wbmm::Geom g = wbmm::make_geom(*desc);
+    int launches = 0, path = WBMM_PATH_NONE;
+    cudaError_t e = cudaSuccess;
+    const int r = wbmm::nhwc_forward_static_scratch(g, desc->dtype, x, T, y, static_cast<cudaStream_t>(cuda_stream),
+                                                    &launches, &path, &e);
+    g_launches += launches;
+    if (r == 1) {
+        snprintf(t_last_error, sizeof(t_last_error),
+                 "wbmm_forward_static_scratch serves NHWC bf16/fp16 activations with w in {7, 14}, C and H*W multiples of 8");
+        return WBMM_STATUS_UNSUPPORTED;
+    }
+    if (r == 2) {
+        snprintf(t_last_error, sizeof(t_last_error),
+                 "wbmm_forward_static_scratch: the activation has %lld bytes, the static scratch holds %zu bytes per temporary",
+                 (long long)desc->B * desc->C * desc->H * desc->W * 2, wbmm::static_scratch_limit_bytes());
+        return WBMM_STATUS_TOO_LARGE;
+    }
+    if (e != cudaSuccess) return set_cuda_error(e, "NHWC via static scratch");
+    t_last_path = WBMM_PATH_TC_TRANSPOSED;
+    return WBMM_STATUS_OK;
+}
+
 int wbmm_backward(const wbmm_desc_t* desc, const void* x, const void* T, const void* dy,
                   void* dx, float* dT, void* cuda_stream)
 {
@@ -710,6 +741,7 @@ const char* wbmm_status_string(int status)
     case WBMM_STATUS_NO_DEVICE: return "no sm_100 CUDA device";
     case WBMM_STATUS_CUDA_ERROR: return "CUDA error";
     case WBMM_STATUS_MISALIGNED: return "misaligned pointer";
+    case WBMM_STATUS_TOO_LARGE: return "problem larger than the static scratch";
     default: return "unknown status";
     }
 }

@@ -69,4 +69,11 @@ bool image_box_map(const Geom& g, int dtype, const void* base, int images, void*
 int plane_box_images(const Geom& g, const TcTiles& tl);
 bool plane_box_map(const Geom& g, int dtype, const void* base, int images, void* map);
 
+// wbmm_static_scratch.cu: the NHWC transposition route with its two temporaries in a file-scope device array (no
+// allocation).  Returns 0 = served (*err holds the CUDA status), 1 = not a problem of this route, 2 = the activation
+// exceeds static_scratch_limit_bytes(); nothing is launched for 1 and 2.
+size_t static_scratch_limit_bytes();
+int nhwc_forward_static_scratch(const Geom& g, int dtype, const void* x, const void* T, void* y, cudaStream_t stream,
+                                int* launches, int* path, cudaError_t* err);
+
 }  // namespace wbmm
