@@ -60,8 +60,16 @@ struct DtCfg {
 // STRIP (with GEN): general addressing on strips of window rows held in ROLLED row order (shifted / ragged maps
 // whose whole frame images do not fit, or with more than 128 windows per image): the producer moves a strip as up
 // to two runs of image rows, so rows never wrap inside the frame and only the columns do (as in tc_bulk_kernel).
+// CTAs per SM: two at w = 7 (S is 64 TMEM columns, the operand stage 32 KB, <= 96 registers): the repack / MMA /
+// fold latencies of one CTA are hidden by the other's, as in the forward kernel (wbmm_tc.cu).  w = 14 keeps S in
+// 416 of the 512 columns: one CTA.
+template <int WS>
+constexpr int dt_ctas_per_sm() { return WS == 7 ? 2 : 1; }
+template <int WS>
+constexpr int dt_tmem_cols() { return DtCfg<WS>::MT * 256 <= 256 && WinCfg<WS>::N_PAD <= 128 ? 128 : 512; }
+
 template <int WS, bool BF16, bool GEN, bool HIER, bool STRIP = false>
-__global__ void __launch_bounds__(kThreadsD, 1)
+__global__ void __launch_bounds__(kThreadsD, dt_ctas_per_sm<WS>())
 tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __restrict__ x,
              const uint16_t* __restrict__ dy, float* __restrict__ dT, float* __restrict__ dTl, int box, int pbox,
              const __grid_constant__ CUtensorMap mx, const __grid_constant__ CUtensorMap mg)
@@ -81,7 +89,7 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
     const uint32_t STAGE_FULL = bar0 + 8u * (2 * kMaxSlots), STAGE_EMPTY = STAGE_FULL + 16;   // [2 halves] each
     const int wpf = tl.NSY * g.nww;
 
-    if (warp == 1) ptx::tmem_alloc(ptx::smem_u32(&tmem_base_s), 512);
+    if (warp == 1) ptx::tmem_alloc(ptx::smem_u32(&tmem_base_s), dt_tmem_cols<WS>());
     if (tid >= 64 && tid < 64 + nslot) {
         ptx::mbar_init(FULL(tid - 64), 1);
         ptx::mbar_init(EMPTY(tid - 64), box ? box * wpf : wpf);   // box mode: one barrier pair per group of `box` images
@@ -355,13 +363,13 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
     }
     ptx::tc_fence_before_sync();
     __syncthreads();
-    if (warp == 1) ptx::tmem_dealloc(tmem, 512);
+    if (warp == 1) ptx::tmem_dealloc(tmem, dt_tmem_cols<WS>());
 }
 
 template <int WS>
-int dt_slots(const TcTiles& tl)
+int dt_slots(const TcTiles& tl, int ctas = 1)
 {
-    const long long room = 227ll * 1024 - 1024 - DtCfg<WS>::FIXED;
+    const long long room = (ctas == 1 ? 227ll * 1024 : 113ll * 1024) - 1024 - DtCfg<WS>::FIXED;
     long long n = room / tl.S;
     if (n > 6 * tl.NP) n = 6 * tl.NP;
     if (n > kMaxSlots) n = kMaxSlots;
@@ -464,13 +472,21 @@ cudaError_t launch_dt(const Geom& g, const TcTiles& tl_in, const void* x, const 
             tl.S = (int)ib;
         }
     }
-    int nslot = dt_slots<WS>(tl);
+    // two CTAs per SM (w = 7) when half the shared memory still holds a tile and a half of x and dy
+    int ctas = dt_ctas_per_sm<WS>();
+    if (ctas > 1) {
+        int n2 = dt_slots<WS>(tl, ctas);
+        if (box) n2 -= n2 % (2 * box);
+        if (n2 < 3 * tl.NP) ctas = 1;
+    }
+    int nslot = dt_slots<WS>(tl, ctas);
     if (box) {
         nslot -= nslot % (2 * box);
         if (nslot < 2 * tl.NP) {
             if (pbox) return cudaErrorInvalidConfiguration;
             box = 0;
             tl = tl_in;
+            ctas = 1;
             nslot = dt_slots<WS>(tl);
         }
     }
@@ -478,7 +494,7 @@ cudaError_t launch_dt(const Geom& g, const TcTiles& tl_in, const void* x, const 
     static SmemOptIn smem_state;
     cudaError_t e = ensure_dynamic_smem(reinterpret_cast<const void*>(k), smem, &smem_state);
     if (e != cudaSuccess) return e;
-    int grid = (int)(tl.ntiles < num_sms() ? tl.ntiles : num_sms());
+    int grid = (int)(tl.ntiles < (long long)num_sms() * ctas ? tl.ntiles : (long long)num_sms() * ctas);
     if (grid > kMaxGrid) grid = kMaxGrid;
     static std::mutex mu;
     static TilePart cached;
