@@ -36,6 +36,9 @@ struct FDtCfg {
     static constexpr int NV = (Cf::N + 7) / 8;         // 16-byte vectors (8 positions) a window fills
     static constexpr int NVEC = Cf::N_PAD / 8;         // vectors per operand region
     static constexpr int HW = 64;                      // windows per tile = MMA K of one stage
+    // two CTAs per SM at w = 7 (S is 64 TMEM columns, the stage 48 KB, <= 86 registers), as in wbmm_tc_dt.cu
+    static constexpr int CTAS = WS == 7 ? 2 : 1;
+    static constexpr int TMEM_COLS = WS == 7 ? 128 : 512;
     static constexpr int SBO = HW * 16;                // bytes between position groups
     static constexpr int LBO = 128;                    // bytes between groups of 8 windows
     static constexpr int OP_BYTES = NVEC * SBO;        // one operand term
@@ -61,7 +64,7 @@ __device__ __forceinline__ void split_vec(const float* f, uint4* out)
 }
 
 template <int WS, bool GEN>
-__global__ void __launch_bounds__(kThreadsFD, 1)
+__global__ void __launch_bounds__(kThreadsFD, FDtCfg<WS>::CTAS)
 tc_f32_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const float* __restrict__ x, const float* __restrict__ dy,
                  float* __restrict__ dT)
 {
@@ -80,7 +83,7 @@ tc_f32_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const float* __r
     const uint32_t STAGE_FULL = bar0 + 8u * (2 * kMaxSlots), STAGE_EMPTY = STAGE_FULL + 8;
     const int wpf = tl.NSY * g.nww;
 
-    if (warp == 1) ptx::tmem_alloc(ptx::smem_u32(&tmem_base_s), 512);
+    if (warp == 1) ptx::tmem_alloc(ptx::smem_u32(&tmem_base_s), Dc::TMEM_COLS);
     if (tid >= 64 && tid < 64 + nslot) {
         ptx::mbar_init(FULL(tid - 64), 1);
         ptx::mbar_init(EMPTY(tid - 64), 2 * wpf);        // two threads per window of the image
@@ -290,13 +293,33 @@ tc_f32_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const float* __r
     }
     ptx::tc_fence_before_sync();
     __syncthreads();
-    if (warp == 1) ptx::tmem_dealloc(tmem, 512);
+    if (warp == 1) ptx::tmem_dealloc(tmem, Dc::TMEM_COLS);
 }
 
 // Tiles of <= 64 windows of one channel: whole frame images, else strips of window rows (aligned form only); slots
 // for x and dy of a tile, two tiles where they fit.  Fewer images per tile when even one tile does not fit.
 template <int WS>
-bool f32dt_tiles(const Geom& g, TcTiles* t, int* nslot)
+bool f32dt_tiles_for(const Geom& g, TcTiles* t, int* nslot, int ctas);
+
+// two CTAs per SM where a tile and a half of x and dy fit half the shared memory, else one
+template <int WS>
+bool f32dt_tiles(const Geom& g, TcTiles* t, int* nslot, int* ctas)
+{
+    if (FDtCfg<WS>::CTAS > 1) {
+        TcTiles t1;
+        int n1 = 0;
+        const bool one = f32dt_tiles_for<WS>(g, &t1, &n1, 1);
+        if (f32dt_tiles_for<WS>(g, t, nslot, FDtCfg<WS>::CTAS) && *nslot >= 3 * t->NP && (!one || t->NP == t1.NP && t->NSY == t1.NSY)) {
+            *ctas = FDtCfg<WS>::CTAS;
+            return true;
+        }
+    }
+    *ctas = 1;
+    return f32dt_tiles_for<WS>(g, t, nslot, 1);
+}
+
+template <int WS>
+bool f32dt_tiles_for(const Geom& g, TcTiles* t, int* nslot, int ctas)
 {
     using Dc = FDtCfg<WS>;
     if (g.nww > Dc::HW) return false;
@@ -309,7 +332,7 @@ bool f32dt_tiles(const Geom& g, TcTiles* t, int* nslot)
         t->NP = 1;
         t->NSY = Dc::HW / g.nww;
     }
-    const long long room = 227ll * 1024 - 1024 - Dc::FIXED;
+    const long long room = (ctas == 1 ? 227ll * 1024 : 113ll * 1024) - 1024 - Dc::FIXED;
     for (;;) {
         t->frame_rows = t->NSY * g.w;
         int s16 = (t->frame_rows * g.Wp * 4 + 15) / 16;
@@ -344,14 +367,14 @@ int f32dt_mode(const Geom& g, const TcTiles& tl, const void* x, const void* dy)
 }
 
 template <int WS, bool GEN>
-cudaError_t launch_f32dt(const Geom& g, const TcTiles& tl, int nslot, const void* x, const void* dy, float* dT, cudaStream_t s)
+cudaError_t launch_f32dt(const Geom& g, const TcTiles& tl, int nslot, int ctas, const void* x, const void* dy, float* dT, cudaStream_t s)
 {
     auto k = tc_f32_dt_kernel<WS, GEN>;
     const size_t smem = (size_t)FDtCfg<WS>::FIXED + (size_t)nslot * tl.S;
     static SmemOptIn smem_state;
     cudaError_t e = ensure_dynamic_smem(reinterpret_cast<const void*>(k), smem, &smem_state);
     if (e != cudaSuccess) return e;
-    int grid = (int)(tl.ntiles < num_sms() ? tl.ntiles : num_sms());
+    int grid = (int)(tl.ntiles < (long long)num_sms() * ctas ? tl.ntiles : (long long)num_sms() * ctas);
     if (grid > kMaxGrid) grid = kMaxGrid;
     static std::mutex mu;
     static TilePart cached;
@@ -386,8 +409,8 @@ bool tc_f32_grad_table_supported(const Geom& g, const void* x, const void* dy)
 {
     if (g.w != 7 && g.w != 14) return false;
     TcTiles tl;
-    int nslot;
-    if (!(g.w == 7 ? f32dt_tiles<7>(g, &tl, &nslot) : f32dt_tiles<14>(g, &tl, &nslot))) return false;
+    int nslot, ctas;
+    if (!(g.w == 7 ? f32dt_tiles<7>(g, &tl, &nslot, &ctas) : f32dt_tiles<14>(g, &tl, &nslot, &ctas))) return false;
     return (g.w == 7 ? f32dt_mode<7>(g, tl, x, dy) : f32dt_mode<14>(g, tl, x, dy)) != 0;
 }
 
@@ -395,15 +418,15 @@ bool tc_f32_grad_table_supported(const Geom& g, const void* x, const void* dy)
 cudaError_t tc_f32_grad_table(const Geom& g, const void* x, const void* dy, float* dT, cudaStream_t stream, int* launches)
 {
     TcTiles tl;
-    int nslot;
-    if (!(g.w == 7 ? f32dt_tiles<7>(g, &tl, &nslot) : f32dt_tiles<14>(g, &tl, &nslot))) return cudaErrorNotSupported;
+    int nslot, ctas;
+    if (!(g.w == 7 ? f32dt_tiles<7>(g, &tl, &nslot, &ctas) : f32dt_tiles<14>(g, &tl, &nslot, &ctas))) return cudaErrorNotSupported;
     if (tl.ntiles == 0) return cudaSuccess;
     const int mode = g.w == 7 ? f32dt_mode<7>(g, tl, x, dy) : f32dt_mode<14>(g, tl, x, dy);
     if (mode == 0) return cudaErrorNotSupported;
     *launches += 1;
     if (g.w == 7)
-        return mode == 2 ? launch_f32dt<7, true>(g, tl, nslot, x, dy, dT, stream) : launch_f32dt<7, false>(g, tl, nslot, x, dy, dT, stream);
-    return mode == 2 ? launch_f32dt<14, true>(g, tl, nslot, x, dy, dT, stream) : launch_f32dt<14, false>(g, tl, nslot, x, dy, dT, stream);
+        return mode == 2 ? launch_f32dt<7, true>(g, tl, nslot, ctas, x, dy, dT, stream) : launch_f32dt<7, false>(g, tl, nslot, ctas, x, dy, dT, stream);
+    return mode == 2 ? launch_f32dt<14, true>(g, tl, nslot, ctas, x, dy, dT, stream) : launch_f32dt<14, false>(g, tl, nslot, ctas, x, dy, dT, stream);
 }
 
 }  // namespace wbmm
