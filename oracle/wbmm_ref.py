@@ -15,7 +15,10 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "wbmm_ref.c")
-_LIB = os.path.join(_HERE, "libwbmm_ref.so")
+# WBMM_ORACLE_SANITIZE=1: a second build with AddressSanitizer + UBSan (run the CPU pins under it with
+# LD_PRELOAD=$(gcc -print-file-name=libasan.so) ASAN_OPTIONS=detect_leaks=0; tests/README in DESIGN.md section 4)
+_SANITIZE = os.environ.get("WBMM_ORACLE_SANITIZE") == "1"
+_LIB = os.path.join(_HERE, "libwbmm_ref_asan.so" if _SANITIZE else "libwbmm_ref.so")
 
 NCHW, NHWC = 0, 1
 
@@ -28,6 +31,8 @@ def build(force: bool = False) -> str:
     if force or stale:
         cmd = ["gcc", "-O2", "-std=c99", "-fopenmp", "-fPIC", "-shared", "-Wall", "-Wextra",
                "-o", _LIB, _SRC]
+        if _SANITIZE:
+            cmd[1:2] = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"]
         subprocess.run(cmd, check=True)
     return _LIB
 
