@@ -340,8 +340,9 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                     ptx::mbar_wait(EMPTY(slot), ((kk / nslot) & 1) ^ 1);
                     ptx::mbar_arrive_expect_tx(FULL(slot), bytes * box);
                     // (the box starts on a 16-byte boundary at or below the plane: the plane sits poff bytes into the slot)
-                    ptx::tma_load_4d(ptx::smem_u32(ring + (size_t)slot * tl.S), &mx, sbox == 2 ? (c * (int)plane_elems) & ~7 : 0, 0,
-                                     sbox == 2 ? 0 : c, b0 + p, FULL(slot));
+                    const int pe0 = c * (int)plane_elems;
+                    ptx::tma_load_4d(ptx::smem_u32(ring + (size_t)slot * tl.S), &mx, sbox == 2 ? (plane_box_2d(plane_elems) ? 0 : pe0 & ~7) : 0,
+                                     sbox == 2 && plane_box_2d(plane_elems) ? pe0 >> 3 : 0, sbox == 2 ? 0 : c, b0 + p, FULL(slot));
                 }
             } else
             for (int p = lane; p < np_eff; p += 32) {
@@ -755,11 +756,13 @@ EncodeTiledFn bulk_encode_fn()
 // channel dimension can address one plane, but a map over [B][C*H*W] can: a box of `images` rows x (H*W + 7 rounded up
 // to 8) elements starting at the 16-byte boundary at or below element c*H*W (it also reads a few elements of the
 // neighbouring planes; the slot pitch is the padded size and the plane sits (c*H*W mod 8) elements into its slot).  Returns the images per box (8, 4 or 2), 0 when the shape does not allow it.
+constexpr long long kPlaneBoxMax = 2048;        // padded plane elements: 256 box rows of 8
+
 int plane_box_images(const Geom& g, const TcTiles& tl)
 {
     const long long hw = (long long)g.H * g.W;
     const long long hwp = (hw + 14) / 8 * 8;       // the box starts up to 7 elements before the plane (16-byte boundary)
-    if (tl.nstrips != 1 || hw % 2 != 0 || hwp > 256 || (g.C * hw * 2) % 16 != 0 || g.C * hw > 0x7fffffffll) return 0;
+    if (tl.nstrips != 1 || hw % 2 != 0 || hwp > kPlaneBoxMax || (g.C * hw * 2) % 16 != 0 || g.C * hw > 0x7fffffffll) return 0;
     for (int cand = 8; cand >= 2; cand >>= 1)
         if (tl.NP % cand == 0 && g.B % cand == 0 && (cand * hwp * 2) % 128 == 0) return cand;
     return 0;
@@ -769,11 +772,15 @@ bool plane_box_map(const Geom& g, int dtype, const void* base, int images, void*
 {
     const long long hw = (long long)g.H * g.W, hwp = (hw + 14) / 8 * 8;
     EncodeTiledFn fn = bulk_encode_fn();
-    if (!fn || images < 1 || images > 256 || hwp > 256) return false;
+    if (!fn || images < 1 || images > 256 || hwp > kPlaneBoxMax) return false;
     const cuuint64_t row = (cuuint64_t)g.C * hw;
-    const cuuint64_t dims[4] = {row, 1, 1, (cuuint64_t)g.B};
-    const cuuint64_t strides[3] = {row * 2, row * 2, row * 2};
-    const cuuint32_t boxd[4] = {(cuuint32_t)hwp, 1, 1, (cuuint32_t)images};
+    // planes of more than 256 elements (30 x 30: 900): a box dimension holds at most 256 elements, so the row of an image
+    // is viewed as (8 elements, C*H*W / 8) and the box is {8, padded plane / 8}: the same dense bytes in shared memory,
+    // box start (0, c*H*W / 8) -- see plane_box_2d()
+    const bool two_d = hwp > 256;
+    const cuuint64_t dims[4] = {two_d ? 8 : row, two_d ? row / 8 : 1, 1, (cuuint64_t)g.B};
+    const cuuint64_t strides[3] = {two_d ? 16 : row * 2, row * 2, row * 2};
+    const cuuint32_t boxd[4] = {(cuuint32_t)(two_d ? 8 : hwp), (cuuint32_t)(two_d ? hwp / 8 : 1), 1, (cuuint32_t)images};
     const cuuint32_t estr[4] = {1, 1, 1, 1};
     const CUtensorMapDataType dt = dtype == WBMM_DTYPE_BF16 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT16;
     return fn(static_cast<CUtensorMap*>(map), dt, 4, const_cast<void*>(base), dims, strides, boxd, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
@@ -1016,6 +1023,15 @@ bool tc_tiles(const Geom& g, TcTiles* t)
         if (t->NP > 64) t->NP = 64;      // one window per image (14 x 14 at w = 14): half-filled tiles, so that the ring's
                                          // slot count (one frame image each) stays within kMaxSlots
         if (t->NP > g.B) t->NP = g.B;
+        // planes that only tensor-map "plane boxes" can move (H*W*2 not a multiple of 16): the images of a tile come in
+        // boxes of 8, 4 or 2 -- take the largest tile that is whole boxes (30 x 30 at w = 14: 14 -> 12 images)
+        const long long hw = (long long)g.H * g.W, hwp = (hw + 14) / 8 * 8;
+        if (g.layout == WBMM_LAYOUT_NCHW && (hw * 2) % 16 != 0 && hw % 2 == 0 && hwp <= kPlaneBoxMax && (g.C * hw * 2) % 16 == 0) {
+            int best = 0;
+            for (int cand = 8; cand >= 2; cand >>= 1)
+                if (g.B % cand == 0 && (cand * hwp * 2) % 128 == 0 && t->NP / cand * cand > best) best = t->NP / cand * cand;
+            if (best > 0) t->NP = best;
+        }
     } else {
         t->NP = 1;
         t->NSY = 128 / g.nww;

@@ -677,6 +677,8 @@ __device__ __forceinline__ void build_lib14_local(const uint8_t* lib, const uint
 
 constexpr int kThreadsB = 352;
 constexpr int kMaxSlots = 96;
+// plane boxes (wbmm_tc.cu: plane_box_map) of more than 256 padded elements use the two-dimensional view of the row
+__host__ __device__ __forceinline__ bool plane_box_2d(long long plane_elems) { return (plane_elems + 14) / 8 * 8 > 256; }
 constexpr int kMaxGrid = 320;     // up to two CTAs per SM (w = 7)
 constexpr int kMaxOutBufs = 16;  // output group buffers of the bulk kernel
 

@@ -144,8 +144,9 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
                     const int slot = kk % nslot;
                     ptx::mbar_wait(EMPTY(slot), ((kk / nslot) & 1) ^ 1);
                     ptx::mbar_arrive_expect_tx(FULL(slot), bytes * box);
-                    ptx::tma_load_4d(ptx::smem_u32(ring + (size_t)slot * tl.S), (j & 1) ? &mg : &mx, pbox ? (c * (int)plane_elems) & ~7 : 0, 0,
-                                     pbox ? 0 : c, b0 + (j >> 1) * box, FULL(slot));
+                    const int pe0 = c * (int)plane_elems;
+                    ptx::tma_load_4d(ptx::smem_u32(ring + (size_t)slot * tl.S), (j & 1) ? &mg : &mx, pbox ? (plane_box_2d(plane_elems) ? 0 : pe0 & ~7) : 0,
+                                     pbox && plane_box_2d(plane_elems) ? pe0 >> 3 : 0, pbox ? 0 : c, b0 + (j >> 1) * box, FULL(slot));
                 }
             } else if constexpr (STRIP) {
                 // The strip's rolled rows are up to two runs of image rows (none when it lies in the padding: the barrier
@@ -381,8 +382,8 @@ template <int WS>
 int dt_mode(const Geom& g, const TcTiles& tl, const void* x, const void* dy)
 {
     if (g.layout != WBMM_LAYOUT_NCHW) return 0;
-    const bool pb = ((long long)g.H * g.W * 2) % 16 != 0;       // plane boxes (wbmm_tc.cu), 8 images per box here
-    if (pb && (plane_box_images(g, tl) != 8)) return 0;
+    const bool pb = ((long long)g.H * g.W * 2) % 16 != 0;       // plane boxes (wbmm_tc.cu), 8, 4 or 2 images per box
+    if (pb && plane_box_images(g, tl) == 0) return 0;
     if (reinterpret_cast<uintptr_t>(x) % 16 != 0 || reinterpret_cast<uintptr_t>(dy) % 16 != 0) return 0;
     if (tl.ntiles > 0x3fffffffll) return 0;
     if (dt_slots<WS>(tl) < 2 * tl.NP + 1) return 0;
@@ -458,9 +459,9 @@ cudaError_t launch_dt(const Geom& g, const TcTiles& tl_in, const void* x, const 
     int box = 0, pbox = 0;
     if (((long long)g.H * g.W * 2) % 16 != 0) {
         const int dtype = BF16 ? WBMM_DTYPE_BF16 : WBMM_DTYPE_F16;
-        if (plane_box_images(g, tl) != 8 || !plane_box_map(g, dtype, x, 8, &mx) || !plane_box_map(g, dtype, dy, 8, &mg))
+        box = plane_box_images(g, tl);
+        if (box == 0 || !plane_box_map(g, dtype, x, box, &mx) || !plane_box_map(g, dtype, dy, box, &mg))
             return cudaErrorInvalidConfiguration;
-        box = 8;
         pbox = 1;
         tl.S = (int)(((long long)g.H * g.W + 14) / 8 * 8 * 2);
     } else {

@@ -229,6 +229,13 @@ def test_table_gradient_of_large_maps_stays_on_the_tensor_cores(wb, oracle, B, C
     si.Case("pb_14_w14_shift", 16, 6, 14, 14, 14, shift=(7, 4), seed=94, backward=True),
     si.Case("pb_14_f16", 8, 10, 14, 14, 14, dtype="f16", seed=95, backward=True),
     si.Case("pb_7x28_w7", 16, 4, 7, 28, 7, seed=96, backward=True),                  # 392-byte planes again, 1 x 4 windows
+    # planes of more than 256 elements: the row of an image is viewed as (8, C*H*W/8) and the box is {8, plane/8}
+    si.Case("pb2_30_w14", 24, 16, 30, 30, 14, seed=101, backward=True),              # ragged (42 x 42 padded), 12 images per tile
+    si.Case("pb2_30_w14_shift", 16, 24, 30, 30, 14, shift=(7, 3), seed=102, backward=True),
+    si.Case("pb2_30_w7", 12, 8, 30, 30, 7, seed=103, backward=True),                 # 25 windows per image: 4 images per tile
+    si.Case("pb2_18_w7", 40, 8, 18, 18, 7, seed=104, backward=True),
+    si.Case("pb2_22x38_w14_f16", 20, 12, 22, 38, 14, dtype="f16", seed=105, backward=True),
+    si.Case("pb2_42_w14_many", 36, 40, 42, 42, 14, seed=106, backward=True),         # 3528-byte planes, several tiles per CTA
 ], ids=lambda c: c.name)
 def test_planes_that_are_not_multiples_of_16_bytes(wb, oracle, case):
     """14 x 14 and 7 x 7 maps: neither a bulk copy nor a tensor map with a channel dimension can address one plane;
@@ -902,6 +909,8 @@ DT_EXACT = [
     ("one_image_w14_112_shift", si.Case("dte", 5, 3, 112, 112, 14, shift=(7, 7), seed=309)),
     ("plane_boxes_w14_14", si.Case("dte", 72, 6, 14, 14, 14, seed=310)),                # 392-byte planes
     ("plane_boxes_w7_14_shift", si.Case("dte", 24, 6, 14, 14, 7, shift=(3, 0), seed=311)),
+    ("plane_boxes_2d_w14_30", si.Case("dte", 24, 8, 30, 30, 14, seed=322)),            # 1800-byte planes: (8, n) boxes, 12 images / tile
+    ("plane_boxes_2d_w7_30_rowshift", si.Case("dte", 12, 8, 30, 30, 7, shift=(3, 0), seed=323)),   # W' = 35 is odd: rows may roll, columns not
     ("aligned_w7_56", si.Case("dte", 21, 6, 56, 56, 7, seed=312)),
     ("boxes_w7_28", si.Case("dte", 40, 10, 28, 28, 7, seed=313)),
     ("gen_shift_w7_28", si.Case("dte", 13, 7, 28, 28, 7, shift=(3, 2), seed=314)),
