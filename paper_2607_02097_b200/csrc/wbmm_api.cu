@@ -589,6 +589,8 @@ cudaEvent_t g_ev_in[kHostChunks] = {}, g_ev_k[kHostChunks] = {};
 
 // Chunks per call: enough that the un-overlapped head (first upload) and tail (last download) are small, few enough
 // that per-copy set-up does not show.
+// Measured on cfg3 (77 MB each way, pinned buffers), ms per call: 2 chunks 2.21, 4: 1.96, 8: 1.91-1.97, 12: 1.99,
+// 16: 2.04, 32: 2.41.
 int host_chunks() { return 8; }
 
 cudaError_t host_pipeline_init()
