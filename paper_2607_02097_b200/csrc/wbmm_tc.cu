@@ -183,9 +183,10 @@ struct BulkSmem {
 // STRIP (with GEN): general addressing on strips of window rows in rolled row order (maps with more than 128
 // windows per image); a template flag so that the whole-image general form pays nothing for it.
 // CTAs per SM: two for the aligned w = 7 form (96 registers, 128 TMEM columns, tiles of 12.5 KB: the hand-off
-// latencies of one CTA's pipeline are hidden by the other's), one otherwise.
-template <int WS, bool GEN>
-constexpr int bulk_ctas_per_sm() { return (WS == 7 && !GEN) ? 2 : 1; }
+// latencies of one CTA's pipeline are hidden by the other's) and for its strip form (B32 C96 112x112 shift: 40.3 ->
+// 34.8 us); one otherwise -- the whole-image general form spills at 80 registers and loses (ragged 60x60: 52 -> 70 us).
+template <int WS, bool GEN, bool STRIP = false>
+constexpr int bulk_ctas_per_sm() { return (WS == 7 && (!GEN || STRIP)) ? 2 : 1; }
 template <int WS>
 constexpr int bulk_tmem_cols() { return (2 * ((BulkCfg<WS>::A_COLS + 31) / 32 * 32) + BulkCfg<WS>::D_COLS) <= 128 ? 128 : 512; }
 
@@ -216,7 +217,7 @@ __device__ __forceinline__ void copy_planes_out(const uint8_t* src, uint8_t* dst
 }
 
 template <int WS, bool BF16, bool GEN, bool STRIP>
-__global__ void __launch_bounds__(kThreadsB, bulk_ctas_per_sm<WS, GEN>())
+__global__ void __launch_bounds__(kThreadsB, bulk_ctas_per_sm<WS, GEN, STRIP>())
 tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const uint16_t* __restrict__ x, const uint16_t* __restrict__ T,
                const uint16_t* __restrict__ Tl, uint16_t* __restrict__ y, int reverse, int box, int sbox,
                const __grid_constant__ CUtensorMap mx, const __grid_constant__ CUtensorMap my,
@@ -865,7 +866,7 @@ cudaError_t launch_bulk(const Geom& g, const TcTiles& tl_in, const void* x, cons
         }
         return bulk_slots<WS>(tl, wpf, &nslot, &nout, ctas);
     };
-    int ctas = bulk_ctas_per_sm<WS, GEN>();
+    int ctas = bulk_ctas_per_sm<WS, GEN, STRIP>();
     if (!configure(ctas)) {
         if (ctas == 1) return cudaErrorInvalidConfiguration;
         ctas = 1;
