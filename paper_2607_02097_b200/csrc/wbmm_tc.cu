@@ -237,6 +237,8 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
     // K index: a column of ones in the A operand's padding against a weight row that holds bias_c.
     const bool use_I = Bc::TOEP && (is_hier || ident_bits != 0u);
     const uint32_t pad0 = bias ? (BF16 ? 0x3F80u : 0x3C00u) : 0u;     // 1.0
+    // 7 x 7 maps at w = 7: one window = one plane of 49 contiguous elements (plane boxes; see window_to_tmem_flat7)
+    const bool flat7 = WS == 7 && !GEN && sbox == 2 && g.W == WS && g.H == WS;
     uint8_t* ring = smem + Sm::FIXED;                       // input ring: nslot frame-image slots
     uint8_t* outb = ring + (size_t)nslot * tl.S;            // output ring: nout group buffers of og.images frame images
     __shared__ uint32_t tmem_base_s;
@@ -513,7 +515,10 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
             if (lt == 0) rebuild_weight(c, lt);   // first tile: build while its loads are in flight
             const int bslot = box ? slot - slot % box : slot;      // the barrier pair that covers this image
             if (part) ptx::mbar_wait(FULL(bslot), (kk / nslot) & 1);
-            if constexpr (WG)
+            if (WS == 7 && flat7) {
+                if constexpr (WS == 7)
+                    window_to_tmem_flat7(ring + (size_t)slot * tl.S, poff, valid, tmem + buf * A_STRIDE + ((uint32_t)(q * 32) << 16), pad0);
+            } else if constexpr (WG)
             {
                 const uint32_t ta = tmem + buf * A_STRIDE + ((uint32_t)(q * 32) << 16);
                 if constexpr (GEN && WS % 2 == 0) {      // even w: every window starts on the parity of the column shift
@@ -578,7 +583,11 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                 ptx::tc_fence_before_sync();
                 ptx::mbar_arrive(D_EMPTY + 8 * h);                                 // the MMAs of the next tile may overwrite this half
                 if (h == 0 && sbox != 2) ptx::mbar_wait(OUT_EMPTY + 8 * ob, (use & 1) ^ 1);     // the buffer's previous contents have been read out
-                if (valid) {
+                if (WS == 7 && flat7) {
+                    if constexpr (WS == 7) {
+                        if (valid) packed_to_flat7(img, pk);
+                    }
+                } else if (valid) {
                     if constexpr (WG) {
                         if constexpr (GEN && WS % 2 == 0) {
                             if (g.sw & 1) {
@@ -612,7 +621,8 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                     const uint8_t* src = outb + (size_t)ob * out_bytes;
                     uint8_t* dst = reinterpret_cast<uint8_t*>(y + ((long long)(b0 + p_first) * g.C + c) * plane_elems);
                     if (plane_elems % 4 == 0) copy_planes_out<uint2>(src, dst, np, tl.S, (long long)g.C * plane_elems * 2, (int)(plane_elems / 4), lane);
-                    else copy_planes_out<uint32_t>(src, dst, np, tl.S, (long long)g.C * plane_elems * 2, (int)(plane_elems / 2), lane);
+                    else if (plane_elems % 2 == 0) copy_planes_out<uint32_t>(src, dst, np, tl.S, (long long)g.C * plane_elems * 2, (int)(plane_elems / 2), lane);
+                    else copy_planes_out<uint16_t>(src, dst, np, tl.S, (long long)g.C * plane_elems * 2, (int)plane_elems, lane);   // 7 x 7: planes start on odd elements
                 }
                 __syncwarp();
                 continue;
@@ -717,7 +727,7 @@ int bulk_mode(const Geom& g, const TcTiles& tl, const void* x, const void* y)
     int nslot_, nout_;
     if (!bulk_slots<WS>(tl, tl.NSY * g.nww, &nslot_, &nout_)) return 0;
     const bool plain = g.sh == 0 && g.sw == 0 && g.H == g.Hp && g.W == g.Wp;
-    if (plain && (pb || (tl.frame_rows * g.W * 2) % 16 == 0) && (WS % 2 == 0 || g.W % 2 == 0)) return 1;   // odd w: rows must be word-aligned
+    if (plain && (pb || (tl.frame_rows * g.W * 2) % 16 == 0) && (WS % 2 == 0 || g.W % 2 == 0 || (pb && g.H == WS && g.W == WS))) return 1;   // odd w: rows must be word-aligned (7 x 7 maps: the flat form)
     // general form: whole images in natural layout, word-granular window addressing (W, W' even)
     // (an odd W' -- ragged maps at odd w -- is fine without a column shift: nothing wraps)
     // maps cut into strips of window rows (more than 128 windows per image): rolled-order frames, rows of 16-byte multiples
@@ -763,7 +773,8 @@ int plane_box_images(const Geom& g, const TcTiles& tl)
 {
     const long long hw = (long long)g.H * g.W;
     const long long hwp = (hw + 14) / 8 * 8;       // the box starts up to 7 elements before the plane (16-byte boundary)
-    if (tl.nstrips != 1 || hw % 2 != 0 || hwp > kPlaneBoxMax || (g.C * hw * 2) % 16 != 0 || g.C * hw > 0x7fffffffll) return 0;
+    const bool flat7 = g.w == 7 && g.H == 7 && g.W == 7 && g.sh == 0 && g.sw == 0;      // the plane is one window (window_to_tmem_flat7)
+    if (tl.nstrips != 1 || (hw % 2 != 0 && !flat7) || hwp > kPlaneBoxMax || (g.C * hw * 2) % 16 != 0 || g.C * hw > 0x7fffffffll) return 0;
     for (int cand = 8; cand >= 2; cand >>= 1)
         if (tl.NP % cand == 0 && g.B % cand == 0 && (cand * hwp * 2) % 128 == 0) return cand;
     return 0;
@@ -1027,7 +1038,7 @@ bool tc_tiles(const Geom& g, TcTiles* t)
         // planes that only tensor-map "plane boxes" can move (H*W*2 not a multiple of 16): the images of a tile come in
         // boxes of 8, 4 or 2 -- take the largest tile that is whole boxes (30 x 30 at w = 14: 14 -> 12 images)
         const long long hw = (long long)g.H * g.W, hwp = (hw + 14) / 8 * 8;
-        if (g.layout == WBMM_LAYOUT_NCHW && (hw * 2) % 16 != 0 && hw % 2 == 0 && hwp <= kPlaneBoxMax && (g.C * hw * 2) % 16 == 0) {
+        if (g.layout == WBMM_LAYOUT_NCHW && (hw * 2) % 16 != 0 && (hw % 2 == 0 || (g.w == 7 && hw == 49)) && hwp <= kPlaneBoxMax && (g.C * hw * 2) % 16 == 0) {
             int best = 0;
             for (int cand = 8; cand >= 2; cand >>= 1)
                 if (g.B % cand == 0 && (cand * hwp * 2) % 128 == 0 && t->NP / cand * cand > best) best = t->NP / cand * cand;

@@ -505,6 +505,31 @@ __device__ __forceinline__ void window_to_tmem_gen(const uint8_t* img, const Gen
     packed_window_to_tmem<WS>(v, taddr, pad0);
 }
 
+// 7 x 7 maps at w = 7 (the S4 stage): the window IS the plane -- 49 contiguous elements, 98 bytes, so
+// planes start on odd elements for every other (image, channel).  The plane sits `off` bytes (a multiple of 2) into
+// its plane-box slot; its 25 packed words come from 26 aligned words through one funnel shift by the parity.
+__device__ __forceinline__ void window_to_tmem_flat7(const uint8_t* slot, int off, bool valid, uint32_t taddr, uint32_t pad0 = 0u)
+{
+    constexpr int NW = WinCfg<7>::NW;
+    const uint32_t sh = (uint32_t)(off & 2) * 8u;
+    const uint32_t* p = reinterpret_cast<const uint32_t*>(slot + (off & ~3));
+    uint32_t w[NW + 1], v[NW];
+#pragma unroll
+    for (int k = 0; k <= NW; ++k) w[k] = p[k];          // (word NW may lie in the next slot: a legal address, used for odd planes only)
+#pragma unroll
+    for (int k = 0; k < NW; ++k) v[k] = valid ? __funnelshift_r(w[k], w[k + 1], sh) : 0u;
+    v[NW - 1] &= 0xffffu;                               // there is no element 49
+    packed_window_to_tmem<7>(v, taddr, pad0);
+}
+
+// ... and the result: 25 packed words to the start of the window's output slot (the plane is copied out from there
+// element by element; the high half of the last word falls into the slot's padding)
+__device__ __forceinline__ void packed_to_flat7(uint8_t* slot, const uint32_t* pk)
+{
+#pragma unroll
+    for (int k = 0; k < WinCfg<7>::NW; ++k) reinterpret_cast<uint32_t*>(slot)[k] = pk[k];
+}
+
 // Packed words [W0, W1) of a window (pk[0] = word W0; the range covers whole window rows, or the
 // whole window) -> the window's place in the natural-layout frame.
 template <int WS, int W0, int W1, bool RAGGED, int PAR = -1>

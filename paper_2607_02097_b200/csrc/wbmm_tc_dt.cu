@@ -383,7 +383,7 @@ int dt_mode(const Geom& g, const TcTiles& tl, const void* x, const void* dy)
 {
     if (g.layout != WBMM_LAYOUT_NCHW) return 0;
     const bool pb = ((long long)g.H * g.W * 2) % 16 != 0;       // plane boxes (wbmm_tc.cu), 8, 4 or 2 images per box
-    if (pb && plane_box_images(g, tl) == 0) return 0;
+    if (pb && (plane_box_images(g, tl) == 0 || ((long long)g.H * g.W) % 2 != 0)) return 0;      // (7 x 7 planes: forward / dX only)
     if (reinterpret_cast<uintptr_t>(x) % 16 != 0 || reinterpret_cast<uintptr_t>(dy) % 16 != 0) return 0;
     if (tl.ntiles > 0x3fffffffll) return 0;
     if (dt_slots<WS>(tl) < 2 * tl.NP + 1) return 0;

@@ -196,6 +196,40 @@ def test_pipelined_kernels_one_hot_bins_bitwise(wb, oracle, w, shift, H, W, layo
     assert np.array_equal(widen(dx), rdx)
 
 
+@pytest.mark.parametrize("B,C,dtype", [(16, 8, "bf16"), (128, 40, "bf16"), (72, 24, "f16")])
+def test_one_window_7x7_planes_on_the_pipelined_kernel(wb, oracle, B, C, dtype):
+    """7 x 7 maps at w = 7 (the S4 stage): the window is the plane, 49 contiguous elements that start
+    on odd elements for every other (image, channel) -- plane boxes + one funnel shift by the plane's parity
+    (window_to_tmem_flat7), 2-byte stores.  One-hot tables (pure data movement: bitwise), then a dense table;
+    forward and dX; canaries around the output."""
+    case = si.Case("flat7", B, C, 7, 7, 7, dtype=dtype, seed=130 + C, backward=True)
+    d = si.make(case, device="cuda")
+    g = torch.Generator().manual_seed(C)
+    bins = torch.randint(0, 169, (C,), generator=g)
+    bins[0], bins[1], bins[2] = 0, 168, 84
+    T1 = torch.zeros_like(d["T"])
+    T1[torch.arange(C), bins.to(T1.device)] = 1.0
+    n = d["x"].numel()
+    buf = torch.full((n + 64,), 7.0, dtype=d["x"].dtype, device="cuda")
+    y = buf[32:32 + n].view_as(d["x"])
+    wb.wbmm_forward(d["x"], T1, 7, out=y)
+    assert wb.wbmm_last_path() == wb.PATH_TC_TMA, wb.wbmm_path_string(wb.wbmm_last_path())
+    torch.cuda.synchronize()
+    assert bool((buf[:32] == 7.0).all()) and bool((buf[32 + n:] == 7.0).all())
+    assert np.array_equal(widen(y), oracle.forward(widen(d["x"]), widen(T1), 7))
+    dx, _ = wb.wbmm_backward(None, T1, d["dy"], 7, need_dT=False)
+    assert wb.wbmm_last_path() == wb.PATH_TC_TMA
+    rdx, _ = oracle.backward(widen(d["dy"]), widen(T1), widen(d["dy"]), 7, need_dT=False)
+    assert np.array_equal(widen(dx), rdx)
+    y2 = wb.wbmm_forward(d["x"], d["T"], 7)
+    dx2, dT2 = wb.wbmm_backward(d["x"], d["T"], d["dy"], 7)
+    ry = oracle.forward(widen(d["x"]), widen(d["T"]), 7)
+    rdx2, rdT = oracle.backward(widen(d["x"]), widen(d["T"]), widen(d["dy"]), 7)
+    tol = TOL[dtype]
+    errs = (max_err_over_tol(y2, ry, tol), max_err_over_tol(dx2, rdx2, tol), max_err_over_tol(dT2, rdT, tol))
+    assert max(errs) <= 1.0, errs
+
+
 @pytest.mark.parametrize("H,W,shift", [(112, 112, (7, 7)), (112, 112, (3, 8)), (106, 112, (0, 0))])
 def test_table_gradient_of_large_shifted_maps_stays_on_the_tensor_cores(wb, oracle, H, W, shift):
     """Shifted / ragged 112-row maps need whole frame images (general addressing): the dT kernel then takes one
