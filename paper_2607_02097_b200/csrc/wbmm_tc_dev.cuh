@@ -508,17 +508,23 @@ __device__ __forceinline__ void window_to_tmem_gen(const uint8_t* img, const Gen
 // 7 x 7 maps at w = 7 (the S4 stage): the window IS the plane -- 49 contiguous elements, 98 bytes, so
 // planes start on odd elements for every other (image, channel).  The plane sits `off` bytes (a multiple of 2) into
 // its plane-box slot; its 25 packed words come from 26 aligned words through one funnel shift by the parity.
-__device__ __forceinline__ void window_to_tmem_flat7(const uint8_t* slot, int off, bool valid, uint32_t taddr, uint32_t pad0 = 0u)
+__device__ __forceinline__ void window_to_regs_flat7(const uint8_t* slot, int off, bool valid, uint32_t* v)
 {
     constexpr int NW = WinCfg<7>::NW;
     const uint32_t sh = (uint32_t)(off & 2) * 8u;
     const uint32_t* p = reinterpret_cast<const uint32_t*>(slot + (off & ~3));
-    uint32_t w[NW + 1], v[NW];
+    uint32_t w[NW + 1];
 #pragma unroll
-    for (int k = 0; k <= NW; ++k) w[k] = p[k];          // (word NW may lie in the next slot: a legal address, used for odd planes only)
+    for (int k = 0; k < NW; ++k) w[k] = p[k];           // the 49 elements end inside word NW - 1 for either parity
+    w[NW] = 0u;
 #pragma unroll
     for (int k = 0; k < NW; ++k) v[k] = valid ? __funnelshift_r(w[k], w[k + 1], sh) : 0u;
     v[NW - 1] &= 0xffffu;                               // there is no element 49
+}
+__device__ __forceinline__ void window_to_tmem_flat7(const uint8_t* slot, int off, bool valid, uint32_t taddr, uint32_t pad0 = 0u)
+{
+    uint32_t v[WinCfg<7>::NW];
+    window_to_regs_flat7(slot, off, valid, v);
     packed_window_to_tmem<7>(v, taddr, pad0);
 }
 

@@ -116,6 +116,7 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
     const int rowB = g.W * 2;
     const long long plane_elems = (long long)g.H * g.W;
     const bool ragged = g.H != g.Hp || g.W != g.Wp;
+    const bool flat7 = WS == 7 && !GEN && pbox && g.W == WS && g.H == WS;      // 7 x 7 maps: the plane is the window (wbmm_tc_dev.cuh)
 
     auto tile_decode = [&](int t, int& c, int& b0, int& wy0, int& np_eff, int& rows_eff) {
         c = t / tl.tiles_per_c;
@@ -258,7 +259,9 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
             const uint8_t* img = ring + (size_t)slot * tl.S + (pbox ? ((c * (int)plane_elems) & 7) * 2 : 0);
             {
                 uint32_t wv[Dc::NV * 4];
-                if constexpr (WG) {
+                if (WS == 7 && flat7) {
+                    if constexpr (WS == 7) window_to_regs_flat7(ring + (size_t)slot * tl.S, ((c * (int)plane_elems) & 7) * 2, valid, wv);
+                } else if constexpr (WG) {
                     if (GEN && ragged) window_to_regs_gen<WS, true>(img, ga, valid, wv);
                     else window_to_regs_gen<WS, false>(img, ga, valid, wv);
                 } else {
@@ -383,12 +386,12 @@ int dt_mode(const Geom& g, const TcTiles& tl, const void* x, const void* dy)
 {
     if (g.layout != WBMM_LAYOUT_NCHW) return 0;
     const bool pb = ((long long)g.H * g.W * 2) % 16 != 0;       // plane boxes (wbmm_tc.cu), 8, 4 or 2 images per box
-    if (pb && (plane_box_images(g, tl) == 0 || ((long long)g.H * g.W) % 2 != 0)) return 0;      // (7 x 7 planes: forward / dX only)
+    if (pb && plane_box_images(g, tl) == 0) return 0;      // (odd planes: 7 x 7 at w = 7 only -- the flat form)
     if (reinterpret_cast<uintptr_t>(x) % 16 != 0 || reinterpret_cast<uintptr_t>(dy) % 16 != 0) return 0;
     if (tl.ntiles > 0x3fffffffll) return 0;
     if (dt_slots<WS>(tl) < 2 * tl.NP + 1) return 0;
     const bool plain = g.sh == 0 && g.sw == 0 && g.H == g.Hp && g.W == g.Wp;
-    if (plain && (pb || (tl.frame_rows * g.W * 2) % 16 == 0) && (WS % 2 == 0 || g.W % 2 == 0)) return 1;   // odd w: rows must be word-aligned
+    if (plain && (pb || (tl.frame_rows * g.W * 2) % 16 == 0) && (WS % 2 == 0 || g.W % 2 == 0 || (pb && g.H == WS && g.W == WS))) return 1;   // odd w: rows must be word-aligned (7 x 7 maps: flat form)
     // general form: whole images in natural layout, word-granular window addressing (W, W' even)
     // (an odd W' -- ragged maps at odd w -- is fine without a column shift: nothing wraps)
     // strips of window rows (maps with more than 128 windows per image, or whose whole images do not fit): rolled-order

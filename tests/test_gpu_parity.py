@@ -945,6 +945,7 @@ DT_EXACT = [
     ("plane_boxes_w7_14_shift", si.Case("dte", 24, 6, 14, 14, 7, shift=(3, 0), seed=311)),
     ("plane_boxes_2d_w14_30", si.Case("dte", 24, 8, 30, 30, 14, seed=322)),            # 1800-byte planes: (8, n) boxes, 12 images / tile
     ("plane_boxes_2d_w7_30_rowshift", si.Case("dte", 12, 8, 30, 30, 7, shift=(3, 0), seed=323)),   # W' = 35 is odd: rows may roll, columns not
+    ("flat_planes_w7_7", si.Case("dte", 24, 8, 7, 7, 7, seed=324)),                     # 98-byte planes: the plane is the window
     ("aligned_w7_56", si.Case("dte", 21, 6, 56, 56, 7, seed=312)),
     ("boxes_w7_28", si.Case("dte", 40, 10, 28, 28, 7, seed=313)),
     ("gen_shift_w7_28", si.Case("dte", 13, 7, 28, 28, 7, shift=(3, 2), seed=314)),
