@@ -465,13 +465,14 @@ def test_cached_matrix_mode_arbitrary_matrix_and_bias(wb, oracle, case):
         assert max_err_over_tol(y, ref, TOL["bf16"]) <= 1.0
 
 
+@pytest.mark.parametrize("B", [33, 64])                  # 64: whole plane boxes -- the pipelined kernel in its flat 7 x 7 form
 @pytest.mark.parametrize("dtype", ["bf16", "f32"])
-def test_multi_kernel_fusion_on_a_one_window_map(wb, oracle, dtype):
+def test_multi_kernel_fusion_on_a_one_window_map(wb, oracle, dtype, B):
     """Section 3.7 on a 7 x 7 map: Y = WBMM(X) + BN1(DW5(X)) + BN2(DW3(X)) as ONE operator -- tables folded on
     the device (wbmm_fold_dwconv), then the cached-M forward with the BatchNorm shifts as bias (16-bit) or the
     table forward (fp32, bias added by the caller).  Reference: the oracle's fold + Algorithm 1, itself pinned
     against a library conv2d."""
-    w, B, C = 7, 33, 24
+    w, C = 7, 24
     td = {"bf16": torch.bfloat16, "f32": torch.float32}[dtype]
     g = torch.Generator().manual_seed(67)
     x = torch.randn((B, C, w, w), generator=g).to(td).cuda()
@@ -492,6 +493,7 @@ def test_multi_kernel_fusion_on_a_one_window_map(wb, oracle, dtype):
     assert torch.equal(Tf[:, far], T[:, far])
     if dtype == "bf16":
         y = wb.wbmm_forward_matrix(x, wb.wbmm_materialize_weight(Tf, w), w, bias=bias)
+        assert wb.wbmm_last_path() == (wb.PATH_TC_TMA if B % 8 == 0 else wb.PATH_TC_GATHER)
     else:
         y = wb.wbmm_forward(x, Tf, w) + bias.view(1, C, 1, 1)
     ref = oracle.apply_matrix(widen(x), oracle.weight_matrix(widen(Tf), w), w, bias=widen(bias))
