@@ -255,7 +255,6 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
             const int slot = kk % nslot;
             const int bslot = box ? slot - slot % box : slot;      // the barrier pair that covers this image
             if (part) ptx::mbar_wait(FULL(bslot), (kk / nslot) & 1);
-            ptx::mbar_wait(STAGE_EMPTY + 8 * hf, (lt & 1) ^ 1);      // the MMAs of tile lt-1 have read this half
             const uint8_t* img = ring + (size_t)slot * tl.S + (pbox ? ((c * (int)plane_elems) & 7) * 2 : 0);
             {
                 uint32_t wv[Dc::NV * 4];
@@ -273,13 +272,16 @@ tc_dt_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, const uint16_t* __re
                 }
 #pragma unroll
                 for (int e = Cf::NW; e < Dc::NV * 4; ++e) wv[e] = 0u;
+                // The window is in registers: its frame image can be refilled, and only the vector stores below have to
+                // wait for the MMAs of the previous tile -- the frame reads (the larger part of the repack) overlap them.
+                if (part) ptx::mbar_arrive(EMPTY(bslot));
+                ptx::mbar_wait(STAGE_EMPTY + 8 * hf, (lt & 1) ^ 1);      // the MMAs of tile lt-1 have read this half
 #pragma unroll
                 for (int v = 0; v < Dc::NV; ++v)
                     *reinterpret_cast<uint4*>(dst + v * Dc::SBO) = make_uint4(wv[4 * v], wv[4 * v + 1], wv[4 * v + 2], wv[4 * v + 3]);
             }
             ptx::fence_proxy_async_smem();
             ptx::mbar_arrive(STAGE_FULL + 8 * hf);
-            if (part) ptx::mbar_arrive(EMPTY(bslot));
             k += 2 * np_eff;
 
             const bool seg_end = t + 1 == t1 || (t + 1) - c * tl.tiles_per_c == tl.tiles_per_c;
