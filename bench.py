@@ -342,6 +342,10 @@ def other_rooflines(wb, dev, stream, hbm_peak):
     fwd_row("nhwc_cfg2_shape_fwd_w7", si.with_(si.CFG2, layout=si.NHWC))
     fwd_row("fp32_B128_C96_56x56_w14_fwd", si.with_(si.CFG3, dtype="f32"), n=10)
     fwd_row("fp32_B128_C96_56x56_w7_fwd", si.Case("f32w7", 128, 96, 56, 56, 7, dtype="f32", seed=86), n=10)
+    # small planes (the paper's S3 / S4 stages and a 30 x 30 map): plane boxes; launch-latency-bound
+    fwd_row("s3_B128_C256_14x14_w14_fwd", si.Case("s3w14", 128, 256, 14, 14, 14, seed=88))
+    fwd_row("s4_B128_C256_7x7_w7_fwd", si.Case("s4w7", 128, 256, 7, 7, 7, seed=90))
+    fwd_row("B64_C96_30x30_w14_fwd", si.Case("r30", 64, 96, 30, 30, 14, seed=92))
 
     # backward of config 5, each kernel alone, rotating (x, dy, dx) sets
     c5 = si.CFG5
@@ -358,6 +362,19 @@ def other_rooflines(wb, dev, stream, hbm_peak):
     out["cfg5_dT"] = {"ms": round(ms, 5), "frac": round(by / (hbm_peak * 1e9) * 1e3 / ms, 4), "buffer_sets": ns,
                       "note": "includes the dT zeroing launch"}
     del xs, gs, dxs, d
+    torch.cuda.empty_cache()
+
+    # table gradient at w = 7 (two CTAs per SM) on the config-2 shape
+    c2 = si.with_(si.CFG2, backward=True)
+    d = si.make(c2, device=dev)
+    ns = buffer_sets(2.0 * c2.n_elem * 2)
+    xs = [d["x"]] + [d["x"].clone() for _ in range(ns - 1)]
+    gs = [d["dy"]] + [d["dy"].clone() for _ in range(ns - 1)]
+    dT = torch.empty((c2.C, c2.bins), dtype=torch.float32, device=dev)
+    ms = region_ms_rot(lambda i: wb.wbmm_backward(xs[i % ns], None, gs[i % ns], c2.w, c2.shift, need_dx=False, dT=dT), 30, stream)
+    out["cfg2_shape_dT_w7"] = {"ms": round(ms, 5), "frac": round(bytes_of(c2) / (hbm_peak * 1e9) * 1e3 / ms, 4), "buffer_sets": ns,
+                               "path": wb.wbmm_path_string(wb.wbmm_last_path()), "note": "includes the dT zeroing launch"}
+    del xs, gs, d
     torch.cuda.empty_cache()
 
     # float32 table gradient (3-way / 2-way bf16 split on the tensor cores): reads x and dy once
@@ -728,6 +745,8 @@ PROFILE_CASES = {
     "s3_B128_C256_14x14_w7_fwd": (si.Case("s3w7", 128, 256, 14, 14, 7, seed=89), "fwd"),
     "s4_B128_C256_7x7_w7_fwd": (si.Case("s4w7", 128, 256, 7, 7, 7, seed=90), "fwd"),
     "s3_B128_C592_14x14_w14_fwd": (si.Case("s3w14big", 128, 592, 14, 14, 14, seed=91), "fwd"),
+    "B64_C96_30x30_w14_fwd": (si.Case("r30", 64, 96, 30, 30, 14, seed=92), "fwd"),
+    "cfg2_shape_dT": (si.with_(si.CFG2, backward=True), "dT"),
     "nhwc_cfg2_shape_B128_fwd": (si.Case("nhwc_w7", 128, 96, 56, 56, 7, layout=si.NHWC, seed=87), "fwd"),
 }
 
