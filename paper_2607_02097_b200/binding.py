@@ -102,14 +102,31 @@ def _dims(t: torch.Tensor, layout: int):
     return B, C, H, W
 
 
+_desc_cache = {}
+
+
 def make_desc(x: torch.Tensor, w: int, shift=(0, 0), layout: int = NCHW, flags: int = 0) -> WbmmDesc:
-    B, C, H, W = _dims(x, layout)
-    if x.dtype not in _DTYPES:
-        raise TypeError(f"unsupported dtype {x.dtype}")
-    return WbmmDesc(B, C, H, W, int(w), int(shift[0]), int(shift[1]), _DTYPES[x.dtype], int(layout), int(flags))
+    """The problem descriptor of a call (read-only on the C side, so descriptors are cached by their fields:
+    an eager call costs the host ~7 us, of which building a ctypes structure was one)."""
+    key = (x.shape, x.dtype, w, shift[0], shift[1], layout, flags)
+    d = _desc_cache.get(key)
+    if d is None:
+        B, C, H, W = _dims(x, layout)
+        if x.dtype not in _DTYPES:
+            raise TypeError(f"unsupported dtype {x.dtype}")
+        d = WbmmDesc(B, C, H, W, int(w), int(shift[0]), int(shift[1]), _DTYPES[x.dtype], int(layout), int(flags))
+        if len(_desc_cache) < 4096:
+            _desc_cache[key] = d
+    return d
+
+
+_raw_stream = getattr(torch._C, "_cuda_getCurrentRawStream", None)
 
 
 def _stream(t: torch.Tensor) -> int:
+    """cudaStream_t of torch's current stream on the tensor's device."""
+    if _raw_stream is not None:
+        return _raw_stream(t.device.index)
     return torch.cuda.current_stream(t.device).cuda_stream
 
 
