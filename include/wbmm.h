@@ -206,10 +206,11 @@ WBMM_API int wbmm_forward_fused(const wbmm_desc_t *desc, const void *x, const vo
  *   transpose != 0 applies M_c^T (the dX of the cached operator; the bias is still added if given).
  * x, y, padding, shift, layout as wbmm_forward.  With M = wbmm_materialize_weight(T) and no bias the result is
  * wbmm_forward's ("identical outputs") up to the fp32 summation order of the kernel that serves it
- * (at most one 16-bit ulp).  Served by the gather tensor-core kernel
- * (w in {7, 14}, bf16/fp16, any layout / shift / ragged size); otherwise WBMM_STATUS_UNSUPPORTED.  On this design
- * the cached mode is NOT the fast one: the table path rebuilds its weights in shared memory from 1.4 KB per
- * channel while M costs 75 KB per channel of HBM traffic -- it exists for matrices that are not table-generated.
+ * (at most one 16-bit ulp).  Served by the pipelined tensor-core kernels where wbmm_forward is (NCHW; the matrix takes
+ * the place of the weights built from the table), else by the gather tensor-core kernel (w in {7, 14}, bf16/fp16, any
+ * layout / shift / ragged size); otherwise WBMM_STATUS_UNSUPPORTED.  On this design the cached mode is NOT the fast
+ * one: the table path rebuilds its weights in shared memory from 1.4 KB per channel while M costs 75 KB per channel
+ * of HBM traffic and ~9 us per channel change at w = 14 -- it exists for matrices that are not table-generated.
  */
 WBMM_API int wbmm_forward_matrix(const wbmm_desc_t *desc, const void *x, const void *M, const void *bias, void *y,
                         int transpose, void *cuda_stream);

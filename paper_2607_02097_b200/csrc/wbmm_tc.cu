@@ -177,7 +177,12 @@ struct BulkSmem {
     static constexpr int TAB_ONE = ((Cf::NB + 2) * 2 + 15) / 16 * 16;
     static constexpr int TAB_BYTES = 2 * TAB_ONE;                              // F0 and F1 (or Ts for the generic builder)
     static constexpr int BAR_BYTES = (2 * kMaxSlots + 8 + 2 * kMaxOutBufs) * 8;
-    static constexpr int FIXED = (BulkCfg<WS>::WC_BYTES + BulkCfg<WS>::HIER_BYTES + TAB_BYTES + BAR_BYTES + 127) / 128 * 128;   // tensor-map boxes land 128-byte aligned
+    // layout: barriers | staged table | weights (W_c or the Toeplitz library) | hierarchical libraries | ring ...
+    static constexpr int OFF_TAB = (BAR_BYTES + 15) / 16 * 16;
+    static constexpr int OFF_WC = (OFF_TAB + TAB_BYTES + 127) / 128 * 128;
+    static constexpr int FIXED = (OFF_WC + BulkCfg<WS>::WC_BYTES + BulkCfg<WS>::HIER_BYTES + 127) / 128 * 128;   // tensor-map boxes land 128-byte aligned
+    // cached-M mode at w = 14: the 100 KB matrix starts where the library would (which it replaces) and pushes the ring back
+    static constexpr int FULL_EXTRA = (OFF_WC + kFullBytes + 1023) / 1024 * 1024 - FIXED;
 };
 
 // STRIP (with GEN): general addressing on strips of window rows in rolled row order (maps with more than 128
@@ -221,16 +226,16 @@ __global__ void __launch_bounds__(kThreadsB, bulk_ctas_per_sm<WS, GEN, STRIP>())
 tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const uint16_t* __restrict__ x, const uint16_t* __restrict__ T,
                const uint16_t* __restrict__ Tl, uint16_t* __restrict__ y, int reverse, int box, int sbox,
                const __grid_constant__ CUtensorMap mx, const __grid_constant__ CUtensorMap my,
-               const uint16_t* __restrict__ bias, uint32_t ident_bits)
+               const uint16_t* __restrict__ bias, uint32_t ident_bits, const uint16_t* __restrict__ Mfull)
 {
     using Cf = WinCfg<WS>;
     using Sm = BulkSmem<WS>;
     extern __shared__ __align__(1024) uint8_t smem[];
-    uint8_t* Wc = smem;
+    uint8_t* Wc = smem + Sm::OFF_WC;
     using Bc = BulkCfg<WS>;
-    uint8_t* hier = smem + Bc::WC_BYTES;                    // w = 14: libA | libI | local table (hierarchical operator)
-    uint16_t* tab = reinterpret_cast<uint16_t*>(smem + Bc::WC_BYTES + Bc::HIER_BYTES);
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + Bc::WC_BYTES + Bc::HIER_BYTES + Sm::TAB_BYTES);
+    uint8_t* hier = Wc + Bc::WC_BYTES;                      // w = 14: libA | libI | local table (hierarchical operator)
+    uint16_t* tab = reinterpret_cast<uint16_t*>(smem + Sm::OFF_TAB);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem);
     const bool is_hier = Bc::TOEP && Tl != nullptr;
     // Epilogue fusions without an epilogue: y = W_c x + ident * x + bias_c.  The identity term is the 16 x 16 block
     // ident * I applied by 14 extra N = 16 MMAs (w = 14; 2 * I for the hierarchical operator); the bias is one more
@@ -239,7 +244,10 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
     const uint32_t pad0 = bias ? (BF16 ? 0x3F80u : 0x3C00u) : 0u;     // 1.0
     // 7 x 7 maps at w = 7: one window = one plane of 49 contiguous elements (plane boxes; see window_to_tmem_flat7)
     const bool flat7 = WS == 7 && !GEN && sbox == 2 && g.W == WS && g.H == WS;
-    uint8_t* ring = smem + Sm::FIXED;                       // input ring: nslot frame-image slots
+    // cached-M mode at w = 14: the given matrix of the current channel, 100 KB between the fixed area and the ring
+    const bool fullw = WS == 14 && Mfull != nullptr;
+    uint8_t* wfull = Wc;
+    uint8_t* ring = smem + Sm::FIXED + (fullw ? Sm::FULL_EXTRA : 0);  // input ring: nslot frame-image slots
     uint8_t* outb = ring + (size_t)nslot * tl.S;            // output ring: nout group buffers of og.images frame images
     __shared__ uint32_t tmem_base_s;
 
@@ -378,7 +386,8 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
         // descriptors differ from a base value by compile-time constants in their 14-bit address field.
         {
             const uint32_t wc_addr = ptx::smem_u32(Wc);
-            const uint64_t bd0 = ptx::smem_desc_kmajor_noswz(wc_addr, Bc::LBO, 128);
+            const uint64_t bd0 = fullw ? ptx::smem_desc_kmajor_noswz(ptx::smem_u32(wfull), kFullLbo, 128)
+                                       : ptx::smem_desc_kmajor_noswz(wc_addr, Bc::LBO, 128);
             const uint32_t b_hi = (uint32_t)(bd0 >> 32), b_lo = (uint32_t)bd0;
             uint32_t lt = 0;
             for (int t = t0; t < t1; ++t, ++lt) {
@@ -393,7 +402,9 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                         const uint32_t idesc = ptx::idesc_f16(BF16 ? 1 : 0, 128, Hs::ncols(h));
 #pragma unroll
                         for (int ks = 0; ks < Bc::KSTEPS; ++ks) {
-                            uint64_t bdesc = ((uint64_t)b_hi << 32) | (b_lo + (uint32_t)(Bc::b_off(ks, h) >> 4));
+                            const uint32_t boff = (WS == 14 && fullw) ? (uint32_t)((2 * ks * kFullLbo + h * 112 * 16) >> 4)
+                                                                      : (uint32_t)(Bc::b_off(ks, h) >> 4);
+                            uint64_t bdesc = ((uint64_t)b_hi << 32) | (b_lo + boff);
                             if constexpr (Bc::TOEP) {
                                 if (is_hier && ks / 7 == h)     // input and output rows in the same half: global + local blocks
                                     bdesc = ptx::smem_desc_kmajor_noswz(wc_addr + Bc::WC_BYTES + Bc::b_off_a(ks, h), Bc::LBO_A, 128);
@@ -436,7 +447,10 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
             if (c != cur_c) {
                 if (lt > 0) ptx::mbar_wait(A_EMPTY + 8 * ((lt - 1) & 1), ((lt - 1) >> 1) & 1);   // MMA(lt-1) done with W_c
                 const uint16_t* Tc = T + (long long)c * Cf::NB;
-                if constexpr (WS == 14) {
+                if (WS == 14 && fullw) {
+                    if constexpr (WS == 14)
+                        load_weight14_full(Mfull + (long long)c * Cf::N * Cf::N, reverse != 0, wfull, rt, bias ? (uint32_t)bias[c] : 0u);
+                } else if constexpr (WS == 14) {
                     if (!tabv_ready) table_to_regs14(Tc, reverse != 0, rt, tabv);
                     build_lib14(tabv, tab, tab + Sm::TAB_ONE / 2, Wc, rt, bias ? (uint32_t)bias[c] : 0u);
                     tabv_ready = false;
@@ -541,8 +555,10 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
             // the next tile starts a new channel: have its table row in flight during the next copy
             if (t + 1 < t1 && (t + 1) - c * tl.tiles_per_c == tl.tiles_per_c) {
                 if constexpr (WS == 14) {
-                    table_to_regs14(T + (long long)(c + 1) * Cf::NB, reverse != 0, rt, tabv);
-                    tabv_ready = true;
+                    if (!fullw) {
+                        table_to_regs14(T + (long long)(c + 1) * Cf::NB, reverse != 0, rt, tabv);
+                        tabv_ready = true;
+                    }
                 } else if (!Tl) {
                     table_to_regs7(T + (long long)(c + 1) * Cf::NB, reverse != 0, rt, tabv);
                     tabv_ready = true;
@@ -632,7 +648,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
         }
     } else {
         // ------------------------------------------------------------------ store
-        if (t1 > t0) {   // pull this CTA's table rows into L2 ahead of the W_c builds
+        if (t1 > t0 && T) {   // pull this CTA's table rows into L2 ahead of the W_c builds
             const int c_first = t0 / tl.tiles_per_c, c_last = (t1 - 1) / tl.tiles_per_c;
             const char* base = reinterpret_cast<const char*>(T + (long long)c_first * Cf::NB);
             const long long nbytes = (long long)(c_last - c_first + 1) * Cf::NB * 2;
@@ -694,10 +710,10 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
 // DESIGN.md section 7.7); less starves small tiles (w = 7: 12.5 KB per tile).
 // Returns false when a tile of output plus a tile + 1 of input does not fit.
 template <int WS>
-bool bulk_slots(const TcTiles& tl, int wpf, int* nslot, int* nout, int ctas = 1)
+bool bulk_slots(const TcTiles& tl, int wpf, int* nslot, int* nout, int ctas = 1, int extra = 0)
 {
     const OutGroups og = out_groups(tl, wpf);
-    const long long room = (ctas == 1 ? 227ll * 1024 : 113ll * 1024) - 1024 - BulkSmem<WS>::FIXED;
+    const long long room = (ctas == 1 ? 227ll * 1024 : 113ll * 1024) - 1024 - BulkSmem<WS>::FIXED - extra;
     const long long total = room / tl.S, out_tile = (long long)og.n * og.images;
     const long long kSide = 96 * 1024 / ctas;
     long long depth = (kSide + out_tile * tl.S / 2) / (out_tile * tl.S);
@@ -843,8 +859,9 @@ int bulk_box_mode(const Geom& g, const TcTiles& tl, int dtype, const void* x, co
 
 template <int WS, bool BF16, bool GEN, bool STRIP = false>
 cudaError_t launch_bulk(const Geom& g, const TcTiles& tl_in, const void* x, const void* T, const void* Tl, void* y,
-                        bool reverse, cudaStream_t s, const void* bias, uint32_t ident_bits)
+                        bool reverse, cudaStream_t s, const void* bias, uint32_t ident_bits, const void* Mfull = nullptr)
 {
+    const int extra = (WS == 14 && Mfull) ? BulkSmem<WS>::FULL_EXTRA : 0;      // cached-M mode at w = 14: the given matrix pushes the ring back
     auto k = tc_bulk_kernel<WS, BF16, GEN, STRIP>;
     int nslot = 0, nout = 0;
     TcTiles tl = tl_in;
@@ -863,19 +880,19 @@ cudaError_t launch_bulk(const Geom& g, const TcTiles& tl_in, const void* x, cons
             if (box == 0 || !plane_box_map(g, BF16 ? WBMM_DTYPE_BF16 : WBMM_DTYPE_F16, x, box, &mx)) return false;
             sbox = 2;
             tl.S = (int)(((long long)g.H * g.W + 14) / 8 * 8 * 2);
-            if (!bulk_slots<WS>(tl, wpf, &nslot, &nout, ctas)) return false;
+            if (!bulk_slots<WS>(tl, wpf, &nslot, &nout, ctas, extra)) return false;
             nslot -= nslot % box;
             return nslot >= tl.NP + box;
         }
         box = bulk_box_mode(g, tl_in, BF16 ? WBMM_DTYPE_BF16 : WBMM_DTYPE_F16, x, y, &tl.S, &sbox, &mx, &my);
         if (box) {
             nslot = 0;
-            if (bulk_slots<WS>(tl, wpf, &nslot, &nout, ctas)) nslot -= nslot % box;      // groups never wrap around the ring
+            if (bulk_slots<WS>(tl, wpf, &nslot, &nout, ctas, extra)) nslot -= nslot % box;      // groups never wrap around the ring
             if (nslot >= tl.NP + box) return true;
             box = sbox = 0;                                                             // (does not fit: one copy per image)
             tl = tl_in;
         }
-        return bulk_slots<WS>(tl, wpf, &nslot, &nout, ctas);
+        return bulk_slots<WS>(tl, wpf, &nslot, &nout, ctas, extra);
     };
     int ctas = bulk_ctas_per_sm<WS, GEN, STRIP>();
     if (!configure(ctas)) {
@@ -883,7 +900,7 @@ cudaError_t launch_bulk(const Geom& g, const TcTiles& tl_in, const void* x, cons
         ctas = 1;
         if (!configure(ctas)) return cudaErrorInvalidConfiguration;
     }
-    const size_t smem = (size_t)BulkSmem<WS>::FIXED + (size_t)(nslot + nout * out_groups(tl, wpf).images) * tl.S;
+    const size_t smem = (size_t)BulkSmem<WS>::FIXED + extra + (size_t)(nslot + nout * out_groups(tl, wpf).images) * tl.S;
     static SmemOptIn smem_state;
     cudaError_t e = ensure_dynamic_smem(reinterpret_cast<const void*>(k), smem, &smem_state);
     if (e != cudaSuccess) return e;
@@ -915,7 +932,7 @@ cudaError_t launch_bulk(const Geom& g, const TcTiles& tl_in, const void* x, cons
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     return cudaLaunchKernelEx(&cfg, k, g, tl, part, nslot, nout, (const uint16_t*)x, (const uint16_t*)T, (const uint16_t*)Tl,
-                              (uint16_t*)y, reverse ? 1 : 0, box, sbox, mx, my, (const uint16_t*)bias, ident_bits);
+                              (uint16_t*)y, reverse ? 1 : 0, box, sbox, mx, my, (const uint16_t*)bias, ident_bits, (const uint16_t*)Mfull);
 }
 
 template <int WS>
@@ -1147,6 +1164,24 @@ cudaError_t tc_forward_matrix(const Geom& g, int dtype, const void* x, const voi
                           : launch_bulk<7, false, true>(g, tl, x, nullptr, M, y, transpose, stream, bias, 0u);
             return bf ? launch_bulk<7, true, false>(g, tl, x, nullptr, M, y, transpose, stream, bias, 0u)
                       : launch_bulk<7, false, false>(g, tl, x, nullptr, M, y, transpose, stream, bias, 0u);
+        }
+    }
+    if (g.w == 14) {
+        // w = 14: the given matrix (100 KB in the row-padded operand layout) takes the place of the Toeplitz library in
+        // the same pipelined kernel, where a tile and a half of input plus a tile of output still fit beside it
+        const int mode = bulk_mode<14>(g, tl, x, y);
+        int ns_ = 0, no_ = 0;
+        if (mode != 0 && !(mode == 2 && tl.nstrips > 1) && bulk_slots<14>(tl, tl.NSY * g.nww, &ns_, &no_, 1, BulkSmem<14>::FULL_EXTRA)) {
+            *path = WBMM_PATH_TC_TMA;
+            cudaError_t e;
+            if (mode == 2)
+                e = bf ? launch_bulk<14, true, true>(g, tl, x, nullptr, nullptr, y, transpose, stream, bias, 0u, M)
+                       : launch_bulk<14, false, true>(g, tl, x, nullptr, nullptr, y, transpose, stream, bias, 0u, M);
+            else
+                e = bf ? launch_bulk<14, true, false>(g, tl, x, nullptr, nullptr, y, transpose, stream, bias, 0u, M)
+                       : launch_bulk<14, false, false>(g, tl, x, nullptr, nullptr, y, transpose, stream, bias, 0u, M);
+            if (e != cudaErrorInvalidConfiguration) return e;
+            cudaGetLastError();          // (the ring did not fit after all: the gather kernel below)
         }
     }
     *path = WBMM_PATH_TC_GATHER;

@@ -667,6 +667,40 @@ __device__ __forceinline__ void build_lib14(const uint16_t* v, uint16_t* F0, uin
 }
 
 
+// Cached-M mode at w = 14: the GIVEN matrix M_c [196][196] as the B operand of the same MMAs, in
+// the row-padded index space the Toeplitz form uses on both GEMM axes (K = rj*16 + cj, N = ri*16 + ci; pads are zero):
+// 28 K chunks of 8 x 224 rows x 16 bytes = 100 KB, chunk (kc, n) at byte kc * kFullLbo + n * 16.  K-step ks reads
+// chunks 2ks, 2ks + 1; output half h rows 112h ...  The A operand and the accumulator keep the Toeplitz form's
+// layout, so repack and epilogue are unchanged.  transpose: M_c^T.  bias_bits sits at K index (row 0, cj = 14), where
+// the repack puts the column of ones.  128 threads; a warp reads 8 rows x 56 contiguous bytes of M_c per step.
+constexpr int kFullLbo = 224 * 16;
+constexpr int kFullBytes = 28 * kFullLbo;          // 100352
+__device__ __forceinline__ void load_weight14_full(const uint16_t* __restrict__ Mc, bool transpose, uint8_t* wfull, int tid,
+                                                   uint32_t bias_bits)
+{
+    for (int q = tid; q < 28 * 224; q += 128) {
+        const int r = q >> 5, kcg = r % 7, kc = 4 * kcg + (q & 3), n = 8 * (r / 7) + ((q >> 2) & 7);
+        const int ri = n >> 4, ci = n & 15, rj = kc >> 1, cj0 = (kc & 1) * 8;
+        uint32_t w[4] = {0u, 0u, 0u, 0u};
+        if (ci < 14) {
+            const int i = ri * 14 + ci, j0 = rj * 14 + cj0;
+            if (!transpose) {
+                const uint32_t* src = reinterpret_cast<const uint32_t*>(Mc + i * 196 + j0);      // even element offset
+                w[0] = src[0]; w[1] = src[1]; w[2] = src[2];
+                if (cj0 == 0) w[3] = src[3];
+            } else {
+                uint32_t v[8];
+#pragma unroll
+                for (int e = 0; e < 8; ++e) v[e] = cj0 + e < 14 ? (uint32_t)Mc[(j0 + e) * 196 + i] : 0u;
+#pragma unroll
+                for (int e = 0; e < 8; ++e) w[e >> 1] |= v[e] << ((e & 1) * 16);
+            }
+            if (kc == 1) w[3] = bias_bits;           // K index (row 0, cj 14)
+        }
+        *reinterpret_cast<uint4*>(wfull + kc * kFullLbo + n * 16) = make_uint4(w[0], w[1], w[2], w[3]);
+    }
+}
+
 // Second library of the hierarchical operator (BulkCfg<14>): libA[da] = lib[da + 7] + Z_l'[da - 6], da = 0..12,
 // Z_l'[dr][ci][cj] = [ci/7 == cj/7] * T_l[(dr+6)*13 + (ci-cj+6)]; FL = the local table staged reversed
 // (FL[q] = T_l[168 - q], or T_l[q] for the transposed operator).  Sums are rounded (RNE) to the 16-bit type.

@@ -421,6 +421,9 @@ def test_hier_backward_local_bins_exact_on_integers(wb, oracle):
     si.Case("m_ragged_nhwc", 3, 8, 30, 45, 14, shift=(7, 2), layout=NHWC, seed=63),
     si.Case("m_f16", 4, 3, 21, 21, 7, dtype="f16", seed=64),
     si.Case("m_w7_many", 70, 40, 56, 56, 7, seed=68),                    # pipelined kernel, several channels per CTA
+    si.Case("m_w14_many", 37, 40, 56, 56, 14, seed=72),                  # w = 14: the 100 KB matrix beside the ring, channel changes
+    si.Case("m_w14_boxes_shift", 40, 24, 28, 28, 14, shift=(7, 5), seed=73),
+    si.Case("m_w14_f16_ragged", 6, 5, 60, 60, 14, dtype="f16", seed=74),
     si.Case("m_w7_strips_shift", 3, 4, 112, 112, 7, shift=(2, 5), seed=69),
 ], ids=lambda c: c.name)
 def test_cached_matrix_mode_equals_the_table_mode(wb, oracle, case):
@@ -431,8 +434,8 @@ def test_cached_matrix_mode_equals_the_table_mode(wb, oracle, case):
     M = wb.wbmm_materialize_weight(d["T"], case.w)
     for transpose in (False, True):
         y = wb.wbmm_forward_matrix(d["x"], M, case.w, case.shift, case.layout, transpose=transpose)
-        # w = 7 on planes the pipelined kernel takes: the given matrix replaces the W_c it would have built
-        pipelined = case.w == 7 and case.layout == NCHW and case.W % 2 == 0
+        # NCHW planes the pipelined kernel takes: the given matrix replaces the W_c (w = 7) / the Toeplitz library (w = 14)
+        pipelined = case.layout == NCHW and case.W % 2 == 0
         assert wb.wbmm_last_path() == (wb.PATH_TC_TMA if pipelined else wb.PATH_TC_GATHER)
         if transpose:
             ref, _ = wb.wbmm_backward(None, d["T"], d["x"], case.w, case.shift, case.layout, need_dT=False)
@@ -449,6 +452,7 @@ def test_cached_matrix_mode_equals_the_table_mode(wb, oracle, case):
 
 @pytest.mark.parametrize("case", [
     si.Case("m_any", 5, 6, 30, 44, 14, shift=(2, 9), seed=65),
+    si.Case("m_any_w14_plain", 21, 10, 56, 56, 14, seed=75),             # pipelined kernel: bias at K index (row 0, column 14)
     si.Case("m_any_w7", 37, 12, 28, 56, 7, seed=70),                     # pipelined kernel: bias row at K index N + 1
     si.Case("m_any_w7_ragged_shift", 9, 5, 30, 44, 7, shift=(2, 5), seed=71),
 ], ids=lambda c: c.name)
