@@ -678,26 +678,37 @@ constexpr int kFullBytes = 28 * kFullLbo;          // 100352
 __device__ __forceinline__ void load_weight14_full(const uint16_t* __restrict__ Mc, bool transpose, uint8_t* wfull, int tid,
                                                    uint32_t bias_bits)
 {
-    for (int q = tid; q < 28 * 224; q += 128) {
-        const int r = q >> 5, kcg = r % 7, kc = 4 * kcg + (q & 3), n = 8 * (r / 7) + ((q >> 2) & 7);
-        const int ri = n >> 4, ci = n & 15, rj = kc >> 1, cj0 = (kc & 1) * 8;
-        uint32_t w[4] = {0u, 0u, 0u, 0u};
-        if (ci < 14) {
-            const int i = ri * 14 + ci, j0 = rj * 14 + cj0;
-            if (!transpose) {
-                const uint32_t* src = reinterpret_cast<const uint32_t*>(Mc + i * 196 + j0);      // even element offset
-                w[0] = src[0]; w[1] = src[1]; w[2] = src[2];
-                if (cj0 == 0) w[3] = src[3];
-            } else {
-                uint32_t v[8];
+    // 49 chunks per thread, seven at a time: all their loads are issued before the first store
+    for (int q0 = tid; q0 < 28 * 224; q0 += 7 * 128) {
+        uint32_t w[7][4];
 #pragma unroll
-                for (int e = 0; e < 8; ++e) v[e] = cj0 + e < 14 ? (uint32_t)Mc[(j0 + e) * 196 + i] : 0u;
+        for (int u = 0; u < 7; ++u) {
+            const int q = q0 + u * 128;
+            const int r = q >> 5, kcg = r % 7, kc = 4 * kcg + (q & 3), n = 8 * (r / 7) + ((q >> 2) & 7);
+            const int ri = n >> 4, ci = n & 15, rj = kc >> 1, cj0 = (kc & 1) * 8;
+            w[u][0] = w[u][1] = w[u][2] = w[u][3] = 0u;
+            if (ci < 14) {
+                const int i = ri * 14 + ci, j0 = rj * 14 + cj0;
+                if (!transpose) {
+                    const uint32_t* src = reinterpret_cast<const uint32_t*>(Mc + i * 196 + j0);      // even element offset
+                    w[u][0] = src[0]; w[u][1] = src[1]; w[u][2] = src[2];
+                    if (cj0 == 0) w[u][3] = src[3];
+                } else {
+                    uint32_t v[8];
 #pragma unroll
-                for (int e = 0; e < 8; ++e) w[e >> 1] |= v[e] << ((e & 1) * 16);
+                    for (int e = 0; e < 8; ++e) v[e] = cj0 + e < 14 ? (uint32_t)Mc[(j0 + e) * 196 + i] : 0u;
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) w[u][e >> 1] |= v[e] << ((e & 1) * 16);
+                }
+                if (kc == 1) w[u][3] = bias_bits;           // K index (row 0, cj 14)
             }
-            if (kc == 1) w[3] = bias_bits;           // K index (row 0, cj 14)
         }
-        *reinterpret_cast<uint4*>(wfull + kc * kFullLbo + n * 16) = make_uint4(w[0], w[1], w[2], w[3]);
+#pragma unroll
+        for (int u = 0; u < 7; ++u) {
+            const int q = q0 + u * 128;
+            const int r = q >> 5, kcg = r % 7, kc = 4 * kcg + (q & 3), n = 8 * (r / 7) + ((q >> 2) & 7);
+            *reinterpret_cast<uint4*>(wfull + kc * kFullLbo + n * 16) = make_uint4(w[u][0], w[u][1], w[u][2], w[u][3]);
+        }
     }
 }
 
