@@ -5,7 +5,7 @@ thin Python binding with the same names.  Importing the package does not load th
 the first call does, and raises if it has not been built (no CPU fallback).
 """
 from .binding import (  # noqa: F401
-    NCHW, NHWC, FLAG_ACCUMULATE_DT, FLAG_FORCE_SIMT, FLAG_NO_SCRATCH,
+    NCHW, NHWC, FLAG_ACCUMULATE_DT, FLAG_FORCE_SIMT, FLAG_NO_SCRATCH, FLAG_NO_FORK,
     PATH_NONE, PATH_SIMT, PATH_TC_TMA, PATH_TC_GATHER, PATH_TC_TRANSPOSED,
     WbmmDesc, WbmmError,
     wbmm_forward, wbmm_forward_static_scratch, STATUS_TOO_LARGE, wbmm_backward, wbmm_hier_forward, wbmm_hier_backward, wbmm_forward_matrix, wbmm_fold_dwconv, wbmm_forward_fused, wbmm_materialize_weight,

@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(HERE, "libwbmm.so")
 NCHW, NHWC = 0, 1
 DTYPE_F32, DTYPE_BF16, DTYPE_F16 = 0, 1, 2
 PATH_NONE, PATH_SIMT, PATH_TC_TMA, PATH_TC_GATHER, PATH_TC_TRANSPOSED = 0, 1, 2, 3, 4
-FLAG_ACCUMULATE_DT, FLAG_FORCE_SIMT, FLAG_NO_SCRATCH = 1, 2, 4
+FLAG_ACCUMULATE_DT, FLAG_FORCE_SIMT, FLAG_NO_SCRATCH, FLAG_NO_FORK = 1, 2, 4, 8
 STATUS_OK = 0
 STATUS_TOO_LARGE = 6
 

@@ -196,6 +196,99 @@ int apply(const wbmm_desc_t* d, const wbmm::Geom& g, const void* x, const void* 
     return WBMM_STATUS_OK;
 }
 
+// The table gradient of wbmm_backward on `stream` (clearing included): returns a wbmm_status_t.
+int grad_table_on(const wbmm_desc_t* desc, const wbmm::Geom& g, const void* x, const void* dy, float* dT, cudaStream_t stream)
+{
+    if (!(desc->flags & WBMM_FLAG_ACCUMULATE_DT) && g.C > 0) {
+        int zl = 0;
+        cudaError_t e = wbmm::simt_zero_f32(dT, (long long)g.C * g.nb, stream, &zl);
+        g_launches += zl;
+        if (e != cudaSuccess) return set_cuda_error(e, "zero dT");
+    }
+    int launches = 0;
+    cudaError_t e;
+    bool done = false;
+    if (nhwc_scratch_candidate(desc, g) && wbmm::transpose16_supported((long long)g.H * g.W, g.C, x, dy)) {
+        wbmm::Geom gn = g;
+        gn.layout = WBMM_LAYOUT_NCHW;
+        void* const aligned16 = reinterpret_cast<void*>(256);
+        if (wbmm::tc_grad_table_supported(gn, desc->dtype, aligned16, aligned16)) {
+            const size_t nbytes = (size_t)g.B * g.C * g.H * g.W * 2;
+            AsyncScratch xt(stream), gt(stream);
+            if (xt.alloc(nbytes) == cudaSuccess && gt.alloc(nbytes) == cudaSuccess) {
+                int path = WBMM_PATH_NONE;
+                e = wbmm::transpose16(x, xt.p, g.B, g.H * g.W, g.C, stream, &launches);
+                if (e == cudaSuccess) e = wbmm::transpose16(dy, gt.p, g.B, g.H * g.W, g.C, stream, &launches);
+                if (e == cudaSuccess) e = wbmm::tc_grad_table(gn, desc->dtype, xt.p, gt.p, dT, stream, &launches, &path);
+                g_launches += launches;
+                if (e != cudaSuccess) return set_cuda_error(e, "NHWC dT via NCHW scratch");
+                t_last_path = WBMM_PATH_TC_TRANSPOSED;
+                done = true;
+            } else {
+                cudaGetLastError();
+            }
+        }
+    }
+    if (done) {
+    } else if (!(desc->flags & WBMM_FLAG_FORCE_SIMT) && wbmm::tc_grad_table_supported(g, desc->dtype, x, dy)) {
+        int path = WBMM_PATH_NONE;
+        e = wbmm::tc_grad_table(g, desc->dtype, x, dy, dT, stream, &launches, &path);
+        g_launches += launches;
+        if (e != cudaSuccess) return set_cuda_error(e, "tc_grad_table");
+        t_last_path = path;
+    } else if (desc->dtype == WBMM_DTYPE_F32 && !(desc->flags & WBMM_FLAG_FORCE_SIMT) && wbmm::tc_f32_grad_table_supported(g, x, dy)) {
+        e = wbmm::tc_f32_grad_table(g, x, dy, dT, stream, &launches);
+        g_launches += launches;
+        if (e != cudaSuccess) return set_cuda_error(e, "tc_f32_grad_table");
+        t_last_path = WBMM_PATH_TC_TMA;
+    } else {
+        if (!wbmm::simt_supported(g)) return WBMM_STATUS_UNSUPPORTED;
+        e = wbmm::simt_grad_table(g, desc->dtype, x, dy, dT, stream, &launches);
+        g_launches += launches;
+        if (e != cudaSuccess) return set_cuda_error(e, "simt_grad_table");
+        t_last_path = WBMM_PATH_SIMT;
+    }
+    return WBMM_STATUS_OK;
+}
+
+// wbmm_backward with both gradients: dX and dT do not depend on each other, so the table gradient runs on an internal
+// stream forked from the caller's and joined back into it -- its CTAs fill the SMs the dX kernel leaves idle at its ramp
+// and tail, and at w = 7 one CTA of each kernel shares an SM (cfg5: 61.1 -> 56.2 us for dX + dT, replayed from a
+// graph).  One side stream and event pair per host thread and device, created on first use outside stream capture.
+struct SideStream {
+    cudaStream_t s = nullptr;
+    cudaEvent_t fork = nullptr, join = nullptr;
+};
+thread_local SideStream t_side[kMaxDevices];
+
+SideStream* side_stream(cudaStream_t user)
+{
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) {
+        cudaGetLastError();
+        return nullptr;
+    }
+    SideStream& ss = t_side[dev];
+    if (ss.s) return &ss;
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(user, &cap) != cudaSuccess || cap != cudaStreamCaptureStatusNone) {
+        cudaGetLastError();
+        return nullptr;              // never create resources under capture: this call runs dX and dT in sequence
+    }
+    cudaStream_t st = nullptr;
+    cudaEvent_t a = nullptr, b = nullptr;
+    if (cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&a, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&b, cudaEventDisableTiming) != cudaSuccess) {
+        cudaGetLastError();
+        if (a) cudaEventDestroy(a);
+        if (st) cudaStreamDestroy(st);
+        return nullptr;
+    }
+    ss.s = st; ss.fork = a; ss.join = b;
+    return &ss;
+}
+
 }  // namespace
 
 extern "C" {
@@ -267,61 +360,31 @@ int wbmm_backward(const wbmm_desc_t* desc, const void* x, const void* T, const v
     if (device_state() < 0) return WBMM_STATUS_NO_DEVICE;
     wbmm::Geom g = wbmm::make_geom(*desc);
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    if (dx && dT && !(desc->flags & WBMM_FLAG_NO_FORK)) {
+        SideStream* ss = side_stream(stream);
+        if (ss && cudaEventRecord(ss->fork, stream) == cudaSuccess && cudaStreamWaitEvent(ss->s, ss->fork, 0) == cudaSuccess) {
+            const int st_dt = grad_table_on(desc, g, x, dy, dT, ss->s);
+            const int path_dt = t_last_path;
+            // dX = W_c^T dY on the caller's stream, then the join -- whatever the two returned
+            const int st_dx = apply(desc, g, dy, T, dx, true, stream);
+            cudaError_t e = cudaEventRecord(ss->join, ss->s);
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(stream, ss->join, 0);
+            if (st_dx != WBMM_STATUS_OK) return st_dx;
+            if (st_dt != WBMM_STATUS_OK) return st_dt;
+            if (e != cudaSuccess) return set_cuda_error(e, "join of the table-gradient stream");
+            t_last_path = path_dt;
+            return WBMM_STATUS_OK;
+        }
+        cudaGetLastError();          // no side stream: one after the other below
+    }
     if (dx) {
         // dX = W_c^T dY: the forward operator with the table index reversed (k -> nb-1-k)
         st = apply(desc, g, dy, T, dx, true, stream);
         if (st != WBMM_STATUS_OK) return st;
     }
     if (dT) {
-        if (!(desc->flags & WBMM_FLAG_ACCUMULATE_DT) && g.C > 0) {
-            int zl = 0;
-            cudaError_t e = wbmm::simt_zero_f32(dT, (long long)g.C * g.nb, stream, &zl);
-            g_launches += zl;
-            if (e != cudaSuccess) return set_cuda_error(e, "zero dT");
-        }
-        int launches = 0;
-        cudaError_t e;
-        bool done = false;
-        if (nhwc_scratch_candidate(desc, g) && wbmm::transpose16_supported((long long)g.H * g.W, g.C, x, dy)) {
-            wbmm::Geom gn = g;
-            gn.layout = WBMM_LAYOUT_NCHW;
-            void* const aligned16 = reinterpret_cast<void*>(256);
-            if (wbmm::tc_grad_table_supported(gn, desc->dtype, aligned16, aligned16)) {
-                const size_t nbytes = (size_t)g.B * g.C * g.H * g.W * 2;
-                AsyncScratch xt(stream), gt(stream);
-                if (xt.alloc(nbytes) == cudaSuccess && gt.alloc(nbytes) == cudaSuccess) {
-                    int path = WBMM_PATH_NONE;
-                    e = wbmm::transpose16(x, xt.p, g.B, g.H * g.W, g.C, stream, &launches);
-                    if (e == cudaSuccess) e = wbmm::transpose16(dy, gt.p, g.B, g.H * g.W, g.C, stream, &launches);
-                    if (e == cudaSuccess) e = wbmm::tc_grad_table(gn, desc->dtype, xt.p, gt.p, dT, stream, &launches, &path);
-                    g_launches += launches;
-                    if (e != cudaSuccess) return set_cuda_error(e, "NHWC dT via NCHW scratch");
-                    t_last_path = WBMM_PATH_TC_TRANSPOSED;
-                    done = true;
-                } else {
-                    cudaGetLastError();
-                }
-            }
-        }
-        if (done) {
-        } else if (!(desc->flags & WBMM_FLAG_FORCE_SIMT) && wbmm::tc_grad_table_supported(g, desc->dtype, x, dy)) {
-            int path = WBMM_PATH_NONE;
-            e = wbmm::tc_grad_table(g, desc->dtype, x, dy, dT, stream, &launches, &path);
-            g_launches += launches;
-            if (e != cudaSuccess) return set_cuda_error(e, "tc_grad_table");
-            t_last_path = path;
-        } else if (desc->dtype == WBMM_DTYPE_F32 && !(desc->flags & WBMM_FLAG_FORCE_SIMT) && wbmm::tc_f32_grad_table_supported(g, x, dy)) {
-            e = wbmm::tc_f32_grad_table(g, x, dy, dT, stream, &launches);
-            g_launches += launches;
-            if (e != cudaSuccess) return set_cuda_error(e, "tc_f32_grad_table");
-            t_last_path = WBMM_PATH_TC_TMA;
-        } else {
-            if (!wbmm::simt_supported(g)) return WBMM_STATUS_UNSUPPORTED;
-            e = wbmm::simt_grad_table(g, desc->dtype, x, dy, dT, stream, &launches);
-            g_launches += launches;
-            if (e != cudaSuccess) return set_cuda_error(e, "simt_grad_table");
-            t_last_path = WBMM_PATH_SIMT;
-        }
+        st = grad_table_on(desc, g, x, dy, dT, stream);
+        if (st != WBMM_STATUS_OK) return st;
     }
     return WBMM_STATUS_OK;
 }
@@ -727,6 +790,14 @@ void wbmm_release(void)
     if (g_host_stream) { cudaStreamDestroy(g_host_stream); g_host_stream = nullptr; }
     host_pipeline_release();
     scratch_pools_release();
+    // the calling thread's fork / join streams of wbmm_backward (other host threads keep theirs until they exit)
+    for (int d = 0; d < kMaxDevices; ++d)
+        if (t_side[d].s) {
+            cudaEventDestroy(t_side[d].fork);
+            cudaEventDestroy(t_side[d].join);
+            cudaStreamDestroy(t_side[d].s);
+            t_side[d] = SideStream();
+        }
 }
 
 int wbmm_last_path(void) { return t_last_path; }

@@ -196,6 +196,41 @@ def test_pipelined_kernels_one_hot_bins_bitwise(wb, oracle, w, shift, H, W, layo
     assert np.array_equal(widen(dx), rdx)
 
 
+@pytest.mark.parametrize("case", [
+    si.Case("fork_w14_shift", 24, 12, 28, 28, 14, shift=(7, 7), seed=140, backward=True),
+    si.Case("fork_w7", 21, 10, 56, 56, 7, seed=141, backward=True),
+    si.Case("fork_nhwc_w14", 6, 16, 28, 56, 14, layout=NHWC, seed=142, backward=True),      # scratch allocated on the internal stream
+    si.Case("fork_f32", 5, 3, 56, 56, 14, dtype="f32", seed=143, backward=True),
+], ids=lambda c: c.name)
+def test_backward_forks_the_table_gradient_and_joins(wb, oracle, case):
+    """wbmm_backward with dx and dT runs the table gradient on an internal stream forked from / joined into the
+    caller's (WBMM_FLAG_NO_FORK: one after the other).  Same results either way; work queued behind the call on the
+    caller's stream sees both outputs; the call can be captured into a CUDA graph and replayed."""
+    d = si.make(case, device="cuda")
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        dx0, dT0 = wb.wbmm_backward(d["x"], d["T"], d["dy"], case.w, case.shift, case.layout, wb.FLAG_NO_FORK)
+        dx1, dT1 = wb.wbmm_backward(d["x"], d["T"], d["dy"], case.w, case.shift, case.layout)
+        after = dT1.clone()                      # queued behind the call on the caller's stream: must see the joined dT
+        dxg, dTg = torch.empty_like(dx1), torch.empty_like(dT1)
+        torch.cuda.synchronize()
+        gr = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(gr, stream=s):
+            wb.wbmm_backward(d["x"], d["T"], d["dy"], case.w, case.shift, case.layout, dx=dxg, dT=dTg)
+        dxg.fill_(7.0); dTg.fill_(7.0)
+        gr.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(dx0, dx1) and torch.equal(dx0, dxg)
+    assert torch.equal(after, dT1)
+    rdx, rdT = oracle.backward(widen(d["x"]), widen(d["T"]), widen(d["dy"]), case.w, case.shift, case.layout)
+    for got in (dT0, dT1, dTg):
+        if case.dtype == "f32":
+            assert dT_err_over_tol(got, rdT, case, 1e-4) <= 1.0
+        else:
+            assert max_err_over_tol(got, rdT, TOL[case.dtype]) <= 1.0
+    assert max_err_over_tol(dx1, rdx, TOL[case.dtype]) <= 1.0
+
+
 @pytest.mark.parametrize("B,C,dtype", [(16, 8, "bf16"), (128, 40, "bf16"), (72, 24, "f16")])
 def test_one_window_7x7_planes_on_the_pipelined_kernel(wb, oracle, B, C, dtype):
     """7 x 7 maps at w = 7 (the S4 stage): the window is the plane, 49 contiguous elements that start
