@@ -481,30 +481,55 @@ int wbmm_hier_backward(const wbmm_desc_t* desc, const void* x, const void* Tg, c
         if (dx && !wbmm::tc_hier_supported(g, desc->dtype, dy, dx)) return WBMM_STATUS_UNSUPPORTED;
         if (dTg && (g.w != 14 || !wbmm::tc_grad_table_supported(g, desc->dtype, x, dy))) return WBMM_STATUS_UNSUPPORTED;
     }
+    // both table gradients on `sdt` (dTg, dTl were cleared on the caller's stream above)
+    auto table_gradients = [&](cudaStream_t sdt) -> int {
+        if (dTg && nhwc) {
+            const size_t nbytes = (size_t)g.B * g.C * g.H * g.W * 2;
+            AsyncScratch xt(sdt), gt(sdt);
+            if (xt.alloc(nbytes) != cudaSuccess || gt.alloc(nbytes) != cudaSuccess) {
+                cudaGetLastError();
+                return WBMM_STATUS_UNSUPPORTED;
+            }
+            int launches = 0, path = WBMM_PATH_NONE;
+            cudaError_t e = wbmm::transpose16(x, xt.p, g.B, g.H * g.W, g.C, sdt, &launches);
+            if (e == cudaSuccess) e = wbmm::transpose16(dy, gt.p, g.B, g.H * g.W, g.C, sdt, &launches);
+            if (e == cudaSuccess) e = wbmm::tc_grad_table(gn, desc->dtype, xt.p, gt.p, dTg, sdt, &launches, &path, dTl);
+            g_launches += launches;
+            if (e != cudaSuccess) return set_cuda_error(e, "hierarchical table gradients, NHWC via NCHW scratch");
+            t_last_path = WBMM_PATH_TC_TRANSPOSED;
+        } else if (dTg) {
+            int launches = 0, path = WBMM_PATH_NONE;
+            cudaError_t e = wbmm::tc_grad_table(g, desc->dtype, x, dy, dTg, sdt, &launches, &path, dTl);
+            g_launches += launches;
+            if (e != cudaSuccess) return set_cuda_error(e, "tc_grad_table (hierarchical)");
+            t_last_path = path;
+        }
+        return WBMM_STATUS_OK;
+    };
+    if (dx && dTg && !(desc->flags & WBMM_FLAG_NO_FORK)) {
+        // as wbmm_backward: the table gradients on the internal stream, forked from and joined into the caller's
+        SideStream* ss = side_stream(stream);
+        if (ss && cudaEventRecord(ss->fork, stream) == cudaSuccess && cudaStreamWaitEvent(ss->s, ss->fork, 0) == cudaSuccess) {
+            const int st_dt = table_gradients(ss->s);
+            const int path_dt = t_last_path;
+            const int st_dx = wbmm_hier_forward(desc, dy, Tg, Tl, dx, 1, cuda_stream);
+            cudaError_t e = cudaEventRecord(ss->join, ss->s);
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(stream, ss->join, 0);
+            if (st_dx != WBMM_STATUS_OK) return st_dx;
+            if (st_dt != WBMM_STATUS_OK) return st_dt;
+            if (e != cudaSuccess) return set_cuda_error(e, "join of the table-gradient stream");
+            t_last_path = path_dt;
+            return WBMM_STATUS_OK;
+        }
+        cudaGetLastError();
+    }
     if (dx) {
         st = wbmm_hier_forward(desc, dy, Tg, Tl, dx, 1, cuda_stream);
         if (st != WBMM_STATUS_OK) return st;
     }
-    if (dTg && nhwc) {
-        const size_t nbytes = (size_t)g.B * g.C * g.H * g.W * 2;
-        AsyncScratch xt(stream), gt(stream);
-        if (xt.alloc(nbytes) != cudaSuccess || gt.alloc(nbytes) != cudaSuccess) {
-            cudaGetLastError();
-            return WBMM_STATUS_UNSUPPORTED;
-        }
-        int launches = 0, path = WBMM_PATH_NONE;
-        cudaError_t e = wbmm::transpose16(x, xt.p, g.B, g.H * g.W, g.C, stream, &launches);
-        if (e == cudaSuccess) e = wbmm::transpose16(dy, gt.p, g.B, g.H * g.W, g.C, stream, &launches);
-        if (e == cudaSuccess) e = wbmm::tc_grad_table(gn, desc->dtype, xt.p, gt.p, dTg, stream, &launches, &path, dTl);
-        g_launches += launches;
-        if (e != cudaSuccess) return set_cuda_error(e, "hierarchical table gradients, NHWC via NCHW scratch");
-        t_last_path = WBMM_PATH_TC_TRANSPOSED;
-    } else if (dTg) {
-        int launches = 0, path = WBMM_PATH_NONE;
-        cudaError_t e = wbmm::tc_grad_table(g, desc->dtype, x, dy, dTg, stream, &launches, &path, dTl);
-        g_launches += launches;
-        if (e != cudaSuccess) return set_cuda_error(e, "tc_grad_table (hierarchical)");
-        t_last_path = path;
+    if (dTg) {
+        st = table_gradients(stream);
+        if (st != WBMM_STATUS_OK) return st;
     }
     return WBMM_STATUS_OK;
 }
