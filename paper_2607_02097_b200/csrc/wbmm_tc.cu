@@ -221,7 +221,7 @@ __device__ __forceinline__ void copy_planes_out(const uint8_t* src, uint8_t* dst
     }
 }
 
-template <int WS, bool BF16, bool GEN, bool STRIP>
+template <int WS, bool BF16, bool GEN, bool STRIP, bool FULLW>
 __global__ void __launch_bounds__(kThreadsB, bulk_ctas_per_sm<WS, GEN, STRIP>())
 tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const uint16_t* __restrict__ x, const uint16_t* __restrict__ T,
                const uint16_t* __restrict__ Tl, uint16_t* __restrict__ y, int reverse, int box, int sbox,
@@ -245,7 +245,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
     // 7 x 7 maps at w = 7: one window = one plane of 49 contiguous elements (plane boxes; see window_to_tmem_flat7)
     const bool flat7 = WS == 7 && !GEN && sbox == 2 && g.W == WS && g.H == WS;
     // cached-M mode at w = 14: the given matrix of the current channel, 100 KB between the fixed area and the ring
-    const bool fullw = WS == 14 && Mfull != nullptr;
+    constexpr bool fullw = WS == 14 && FULLW;      // a template flag: the table kernels pay nothing for this mode
     uint8_t* wfull = Wc;
     uint8_t* ring = smem + Sm::FIXED + (fullw ? Sm::FULL_EXTRA : 0);  // input ring: nslot frame-image slots
     uint8_t* outb = ring + (size_t)nslot * tl.S;            // output ring: nout group buffers of og.images frame images
@@ -857,12 +857,12 @@ int bulk_box_mode(const Geom& g, const TcTiles& tl, int dtype, const void* x, co
     return LB;
 }
 
-template <int WS, bool BF16, bool GEN, bool STRIP = false>
+template <int WS, bool BF16, bool GEN, bool STRIP = false, bool FULLW = false>
 cudaError_t launch_bulk(const Geom& g, const TcTiles& tl_in, const void* x, const void* T, const void* Tl, void* y,
                         bool reverse, cudaStream_t s, const void* bias, uint32_t ident_bits, const void* Mfull = nullptr)
 {
-    const int extra = (WS == 14 && Mfull) ? BulkSmem<WS>::FULL_EXTRA : 0;      // cached-M mode at w = 14: the given matrix pushes the ring back
-    auto k = tc_bulk_kernel<WS, BF16, GEN, STRIP>;
+    const int extra = (WS == 14 && FULLW) ? BulkSmem<WS>::FULL_EXTRA : 0;      // cached-M mode at w = 14: the given matrix pushes the ring back
+    auto k = tc_bulk_kernel<WS, BF16, GEN, STRIP, FULLW>;
     int nslot = 0, nout = 0;
     TcTiles tl = tl_in;
     CUtensorMap mx, my;
@@ -1175,11 +1175,11 @@ cudaError_t tc_forward_matrix(const Geom& g, int dtype, const void* x, const voi
             *path = WBMM_PATH_TC_TMA;
             cudaError_t e;
             if (mode == 2)
-                e = bf ? launch_bulk<14, true, true>(g, tl, x, nullptr, nullptr, y, transpose, stream, bias, 0u, M)
-                       : launch_bulk<14, false, true>(g, tl, x, nullptr, nullptr, y, transpose, stream, bias, 0u, M);
+                e = bf ? launch_bulk<14, true, true, false, true>(g, tl, x, nullptr, nullptr, y, transpose, stream, bias, 0u, M)
+                       : launch_bulk<14, false, true, false, true>(g, tl, x, nullptr, nullptr, y, transpose, stream, bias, 0u, M);
             else
-                e = bf ? launch_bulk<14, true, false>(g, tl, x, nullptr, nullptr, y, transpose, stream, bias, 0u, M)
-                       : launch_bulk<14, false, false>(g, tl, x, nullptr, nullptr, y, transpose, stream, bias, 0u, M);
+                e = bf ? launch_bulk<14, true, false, false, true>(g, tl, x, nullptr, nullptr, y, transpose, stream, bias, 0u, M)
+                       : launch_bulk<14, false, false, false, true>(g, tl, x, nullptr, nullptr, y, transpose, stream, bias, 0u, M);
             if (e != cudaErrorInvalidConfiguration) return e;
             cudaGetLastError();          // (the ring did not fit after all: the gather kernel below)
         }
