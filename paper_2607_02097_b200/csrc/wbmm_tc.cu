@@ -221,6 +221,8 @@ __device__ __forceinline__ void copy_planes_out(const uint8_t* src, uint8_t* dst
     }
 }
 
+// FULLW: the variant flag -- w = 14: cached-M mode (the given matrix instead of the Toeplitz library); w = 7: the flat
+// form of 7 x 7 maps (one window = one plane).  Template flags, so that the table kernels pay nothing for either.
 template <int WS, bool BF16, bool GEN, bool STRIP, bool FULLW>
 __global__ void __launch_bounds__(kThreadsB, bulk_ctas_per_sm<WS, GEN, STRIP>())
 tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const uint16_t* __restrict__ x, const uint16_t* __restrict__ T,
@@ -243,7 +245,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
     const bool use_I = Bc::TOEP && (is_hier || ident_bits != 0u);
     const uint32_t pad0 = bias ? (BF16 ? 0x3F80u : 0x3C00u) : 0u;     // 1.0
     // 7 x 7 maps at w = 7: one window = one plane of 49 contiguous elements (plane boxes; see window_to_tmem_flat7)
-    const bool flat7 = WS == 7 && !GEN && sbox == 2 && g.W == WS && g.H == WS;
+    constexpr bool flat7 = WS == 7 && !GEN && FULLW;      // (the variant flag of the w = 7 kernel: launched for 7 x 7 maps only)
     // cached-M mode at w = 14: the given matrix of the current channel, 100 KB between the fixed area and the ring
     constexpr bool fullw = WS == 14 && FULLW;      // a template flag: the table kernels pay nothing for this mode
     uint8_t* wfull = Wc;
@@ -529,8 +531,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
             if (lt == 0) rebuild_weight(c, lt);   // first tile: build while its loads are in flight
             const int bslot = box ? slot - slot % box : slot;      // the barrier pair that covers this image
             if (part) ptx::mbar_wait(FULL(bslot), (kk / nslot) & 1);
-            if (WS == 7 && flat7) {
-                if constexpr (WS == 7)
+            if constexpr (flat7) {
                     window_to_tmem_flat7(ring + (size_t)slot * tl.S, poff, valid, tmem + buf * A_STRIDE + ((uint32_t)(q * 32) << 16), pad0);
             } else if constexpr (WG)
             {
@@ -599,10 +600,8 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                 ptx::tc_fence_before_sync();
                 ptx::mbar_arrive(D_EMPTY + 8 * h);                                 // the MMAs of the next tile may overwrite this half
                 if (h == 0 && sbox != 2) ptx::mbar_wait(OUT_EMPTY + 8 * ob, (use & 1) ^ 1);     // the buffer's previous contents have been read out
-                if (WS == 7 && flat7) {
-                    if constexpr (WS == 7) {
-                        if (valid) packed_to_flat7(img, pk);
-                    }
+                if constexpr (flat7) {
+                    if (valid) packed_to_flat7(img, pk);
                 } else if (valid) {
                     if constexpr (WG) {
                         if constexpr (GEN && WS % 2 == 0) {
@@ -1121,6 +1120,9 @@ cudaError_t tc_forward(const Geom& g, int dtype, const void* x, const void* T, c
             return bf ? launch_bulk<14, true, true, true>(g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits)
                       : launch_bulk<14, false, true, true>(g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
         }
+        if (g.w == 7 && mode == 1 && g.H == 7 && g.W == 7)       // one-window maps: the flat-plane variant
+            return bf ? launch_bulk<7, true, false, false, true>(g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits)
+                      : launch_bulk<7, false, false, false, true>(g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
         const int sel = (g.w == 7 ? 0 : 4) + (bf ? 2 : 0) + (mode == 2 ? 1 : 0);
         switch (sel) {
         case 0: return launch_bulk<7, false, false>(g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
@@ -1162,6 +1164,9 @@ cudaError_t tc_forward_matrix(const Geom& g, int dtype, const void* x, const voi
             if (mode == 2)
                 return bf ? launch_bulk<7, true, true>(g, tl, x, nullptr, M, y, transpose, stream, bias, 0u)
                           : launch_bulk<7, false, true>(g, tl, x, nullptr, M, y, transpose, stream, bias, 0u);
+            if (g.H == 7 && g.W == 7)
+                return bf ? launch_bulk<7, true, false, false, true>(g, tl, x, nullptr, M, y, transpose, stream, bias, 0u)
+                          : launch_bulk<7, false, false, false, true>(g, tl, x, nullptr, M, y, transpose, stream, bias, 0u);
             return bf ? launch_bulk<7, true, false>(g, tl, x, nullptr, M, y, transpose, stream, bias, 0u)
                       : launch_bulk<7, false, false>(g, tl, x, nullptr, M, y, transpose, stream, bias, 0u);
         }
