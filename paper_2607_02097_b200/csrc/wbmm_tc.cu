@@ -221,9 +221,13 @@ __device__ __forceinline__ void copy_planes_out(const uint8_t* src, uint8_t* dst
     }
 }
 
-// FULLW: the variant flag -- w = 14: cached-M mode (the given matrix instead of the Toeplitz library); w = 7: the flat
-// form of 7 x 7 maps (one window = one plane).  Template flags, so that the table kernels pay nothing for either.
-template <int WS, bool BF16, bool GEN, bool STRIP, bool FULLW>
+// V: the variant, a template parameter so that the plain table kernel carries none of the other modes' registers and
+// branches (as run-time flags they cost the general form 7 % and the aligned w = 7 form 4 %):
+//   0  the operator from the table, nothing else
+//   1  extras chosen at run time: hierarchical libraries (Tl), identity block, fused bias; w = 7: a given matrix in Tl
+//   2  w = 14: cached-M mode (the given matrix Mfull instead of the Toeplitz library); w = 7: the flat form of 7 x 7
+//      maps (one window = one plane); bias and, at w = 7, a given matrix in Tl as in 1
+template <int WS, bool BF16, bool GEN, bool STRIP, int V>
 __global__ void __launch_bounds__(kThreadsB, bulk_ctas_per_sm<WS, GEN, STRIP>())
 tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const uint16_t* __restrict__ x, const uint16_t* __restrict__ T,
                const uint16_t* __restrict__ Tl, uint16_t* __restrict__ y, int reverse, int box, int sbox,
@@ -238,16 +242,18 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
     uint8_t* hier = Wc + Bc::WC_BYTES;                      // w = 14: libA | libI | local table (hierarchical operator)
     uint16_t* tab = reinterpret_cast<uint16_t*>(smem + Sm::OFF_TAB);
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem);
-    const bool is_hier = Bc::TOEP && Tl != nullptr;
+    const bool is_hier = V == 1 && Bc::TOEP && Tl != nullptr;
     // Epilogue fusions without an epilogue: y = W_c x + ident * x + bias_c.  The identity term is the 16 x 16 block
     // ident * I applied by 14 extra N = 16 MMAs (w = 14; 2 * I for the hierarchical operator); the bias is one more
     // K index: a column of ones in the A operand's padding against a weight row that holds bias_c.
-    const bool use_I = Bc::TOEP && (is_hier || ident_bits != 0u);
-    const uint32_t pad0 = bias ? (BF16 ? 0x3F80u : 0x3C00u) : 0u;     // 1.0
+    const bool use_I = V == 1 && Bc::TOEP && (is_hier || ident_bits != 0u);
+    const uint16_t* const biasp = V != 0 ? bias : nullptr;
+    const uint16_t* const Mw7 = (V != 0 && WS == 7) ? Tl : nullptr;      // w = 7: a given matrix (cached-M mode)
+    const uint32_t pad0 = biasp ? (BF16 ? 0x3F80u : 0x3C00u) : 0u;     // 1.0
     // 7 x 7 maps at w = 7: one window = one plane of 49 contiguous elements (plane boxes; see window_to_tmem_flat7)
-    constexpr bool flat7 = WS == 7 && !GEN && FULLW;      // (the variant flag of the w = 7 kernel: launched for 7 x 7 maps only)
+    constexpr bool flat7 = WS == 7 && !GEN && V == 2;      // (the variant flag of the w = 7 kernel: launched for 7 x 7 maps only)
     // cached-M mode at w = 14: the given matrix of the current channel, 100 KB between the fixed area and the ring
-    constexpr bool fullw = WS == 14 && FULLW;      // a template flag: the table kernels pay nothing for this mode
+    constexpr bool fullw = WS == 14 && V == 2;      // a template flag: the table kernels pay nothing for this mode
     uint8_t* wfull = Wc;
     uint8_t* ring = smem + Sm::FIXED + (fullw ? Sm::FULL_EXTRA : 0);  // input ring: nslot frame-image slots
     uint8_t* outb = ring + (size_t)nslot * tl.S;            // output ring: nout group buffers of og.images frame images
@@ -451,10 +457,10 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                 const uint16_t* Tc = T + (long long)c * Cf::NB;
                 if (WS == 14 && fullw) {
                     if constexpr (WS == 14)
-                        load_weight14_full(Mfull + (long long)c * Cf::N * Cf::N, reverse != 0, wfull, rt, bias ? (uint32_t)bias[c] : 0u);
+                        load_weight14_full(Mfull + (long long)c * Cf::N * Cf::N, reverse != 0, wfull, rt, biasp ? (uint32_t)biasp[c] : 0u);
                 } else if constexpr (WS == 14) {
                     if (!tabv_ready) table_to_regs14(Tc, reverse != 0, rt, tabv);
-                    build_lib14(tabv, tab, tab + Sm::TAB_ONE / 2, Wc, rt, bias ? (uint32_t)bias[c] : 0u);
+                    build_lib14(tabv, tab, tab + Sm::TAB_ONE / 2, Wc, rt, biasp ? (uint32_t)biasp[c] : 0u);
                     tabv_ready = false;
                     // libI = ident * I (hierarchical: the two identity shortcuts, 2.0 = 0x4000 in bf16 and in fp16)
                     if (use_I && rt < 14)
@@ -467,14 +473,14 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                         ptx::named_bar_sync(2, 128);          // the global library and FL are complete
                         build_lib14_local<BF16>(Wc, FL, hier, rt);
                     }
-                } else if (Tl) {
+                } else if (Mw7) {
                     // cached-M mode (w = 7 only: `Tl` carries the given matrices [C][N][N]) -- the same
                     // operand layout, loaded instead of built; the bias row meets the column of ones at K index N + 1
-                    load_weight<WS>(Tl + (long long)c * Cf::N * Cf::N, reverse != 0, Wc, rt, 128);
-                    if (bias) {
+                    load_weight<WS>(Mw7 + (long long)c * Cf::N * Cf::N, reverse != 0, Wc, rt, 128);
+                    if (biasp) {
                         ptx::named_bar_sync(2, 128);
                         for (int i = rt; i < Cf::N; i += 128)
-                            *reinterpret_cast<uint16_t*>(Wc + ((Cf::N + 1) / 8) * Cf::LBO + i * 16 + ((Cf::N + 1) % 8) * 2) = bias[c];
+                            *reinterpret_cast<uint16_t*>(Wc + ((Cf::N + 1) / 8) * Cf::LBO + i * 16 + ((Cf::N + 1) % 8) * 2) = biasp[c];
                     }
                 } else {
                     static_assert(WS == 14 || Cf::NB <= 2 * 128, "two table entries per repack thread");
@@ -495,7 +501,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                             for (int e = 0; e < 8; ++e) {
                                 uint32_t v = 0;
                                 if (j < Cf::N) v = tab[(ri - rj + WS - 1) * Cf::TW + (ci - cj + WS - 1)];
-                                else if (j == Cf::N + 1 && bias) v = bias[c];      // K index of the column of ones
+                                else if (j == Cf::N + 1 && bias) v = biasp[c];      // K index of the column of ones
                                 pk[e >> 1] |= v << ((e & 1) * 16);
                                 ++j;
                                 if (++cj == WS) { cj = 0; ++rj; }
@@ -560,7 +566,7 @@ tc_bulk_kernel(Geom g, TcTiles tl, TilePart part_, int nslot, int nout, const ui
                         table_to_regs14(T + (long long)(c + 1) * Cf::NB, reverse != 0, rt, tabv);
                         tabv_ready = true;
                     }
-                } else if (!Tl) {
+                } else if (!Mw7) {
                     table_to_regs7(T + (long long)(c + 1) * Cf::NB, reverse != 0, rt, tabv);
                     tabv_ready = true;
                 }
@@ -856,12 +862,12 @@ int bulk_box_mode(const Geom& g, const TcTiles& tl, int dtype, const void* x, co
     return LB;
 }
 
-template <int WS, bool BF16, bool GEN, bool STRIP = false, bool FULLW = false>
+template <int WS, bool BF16, bool GEN, bool STRIP = false, int V = 0>
 cudaError_t launch_bulk(const Geom& g, const TcTiles& tl_in, const void* x, const void* T, const void* Tl, void* y,
                         bool reverse, cudaStream_t s, const void* bias, uint32_t ident_bits, const void* Mfull = nullptr)
 {
-    const int extra = (WS == 14 && FULLW) ? BulkSmem<WS>::FULL_EXTRA : 0;      // cached-M mode at w = 14: the given matrix pushes the ring back
-    auto k = tc_bulk_kernel<WS, BF16, GEN, STRIP, FULLW>;
+    const int extra = (WS == 14 && V == 2) ? BulkSmem<WS>::FULL_EXTRA : 0;      // cached-M mode at w = 14: the given matrix pushes the ring back
+    auto k = tc_bulk_kernel<WS, BF16, GEN, STRIP, V>;
     int nslot = 0, nout = 0;
     TcTiles tl = tl_in;
     CUtensorMap mx, my;
@@ -932,6 +938,18 @@ cudaError_t launch_bulk(const Geom& g, const TcTiles& tl_in, const void* x, cons
     cfg.numAttrs = 1;
     return cudaLaunchKernelEx(&cfg, k, g, tl, part, nslot, nout, (const uint16_t*)x, (const uint16_t*)T, (const uint16_t*)Tl,
                               (uint16_t*)y, reverse ? 1 : 0, box, sbox, mx, my, (const uint16_t*)bias, ident_bits, (const uint16_t*)Mfull);
+}
+
+// the table kernel (V = 0), or the one with the run-time extras (V = 1)
+template <int WS, bool BF16, bool GEN, bool STRIP = false>
+cudaError_t launch_bulk_v(bool extras, const Geom& g, const TcTiles& tl, const void* x, const void* T, const void* Tl, void* y,
+                          bool reverse, cudaStream_t s, const void* bias, uint32_t ident_bits)
+{
+    // The general form at w = 14 sits at the register limit (168, with spills), and ptxas spills MORE in its V = 0
+    // instantiation than in V = 1 (cfg5 forward 22.5 -> 24.2 us): that one form keeps the run-time flags.
+    if constexpr (WS == 14 && GEN) return launch_bulk<WS, BF16, GEN, STRIP, 1>(g, tl, x, T, Tl, y, reverse, s, bias, ident_bits);
+    return extras ? launch_bulk<WS, BF16, GEN, STRIP, 1>(g, tl, x, T, Tl, y, reverse, s, bias, ident_bits)
+                  : launch_bulk<WS, BF16, GEN, STRIP, 0>(g, tl, x, T, Tl, y, reverse, s, bias, ident_bits);
 }
 
 template <int WS>
@@ -1114,25 +1132,26 @@ cudaError_t tc_forward(const Geom& g, int dtype, const void* x, const void* T, c
     const int mode = g.w == 7 ? bulk_mode<7>(g, tl, x, y) : bulk_mode<14>(g, tl, x, y);
     if (mode != 0) {
         *path = WBMM_PATH_TC_TMA;
+        const bool extras = Tl || bias || ident_bits;
         if (mode == 2 && tl.nstrips > 1) {      // general addressing on strips of window rows
-            if (g.w == 7) return bf ? launch_bulk<7, true, true, true>(g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits)
-                                    : launch_bulk<7, false, true, true>(g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
-            return bf ? launch_bulk<14, true, true, true>(g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits)
-                      : launch_bulk<14, false, true, true>(g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
+            if (g.w == 7) return bf ? launch_bulk_v<7, true, true, true>(extras, g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits)
+                                    : launch_bulk_v<7, false, true, true>(extras, g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
+            return bf ? launch_bulk_v<14, true, true, true>(extras, g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits)
+                      : launch_bulk_v<14, false, true, true>(extras, g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
         }
         if (g.w == 7 && mode == 1 && g.H == 7 && g.W == 7)       // one-window maps: the flat-plane variant
-            return bf ? launch_bulk<7, true, false, false, true>(g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits)
-                      : launch_bulk<7, false, false, false, true>(g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
+            return bf ? launch_bulk<7, true, false, false, 2>(g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits)
+                      : launch_bulk<7, false, false, false, 2>(g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
         const int sel = (g.w == 7 ? 0 : 4) + (bf ? 2 : 0) + (mode == 2 ? 1 : 0);
         switch (sel) {
-        case 0: return launch_bulk<7, false, false>(g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
-        case 1: return launch_bulk<7, false, true>(g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
-        case 2: return launch_bulk<7, true, false>(g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
-        case 3: return launch_bulk<7, true, true>(g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
-        case 4: return launch_bulk<14, false, false>(g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
-        case 5: return launch_bulk<14, false, true>(g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
-        case 6: return launch_bulk<14, true, false>(g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
-        default: return launch_bulk<14, true, true>(g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
+        case 0: return launch_bulk_v<7, false, false>(extras, g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
+        case 1: return launch_bulk_v<7, false, true>(extras, g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
+        case 2: return launch_bulk_v<7, true, false>(extras, g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
+        case 3: return launch_bulk_v<7, true, true>(extras, g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
+        case 4: return launch_bulk_v<14, false, false>(extras, g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
+        case 5: return launch_bulk_v<14, false, true>(extras, g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
+        case 6: return launch_bulk_v<14, true, false>(extras, g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
+        default: return launch_bulk_v<14, true, true>(extras, g, tl, x, T, Tl, y, reverse, stream, bias, ident_bits);
         }
     }
     if (Tl || bias || ident_bits) return cudaErrorNotSupported;      // hierarchical / fused variants exist in the bulk kernel only
@@ -1159,16 +1178,16 @@ cudaError_t tc_forward_matrix(const Geom& g, int dtype, const void* x, const voi
         if (mode != 0) {
             *path = WBMM_PATH_TC_TMA;
             if (mode == 2 && tl.nstrips > 1)
-                return bf ? launch_bulk<7, true, true, true>(g, tl, x, nullptr, M, y, transpose, stream, bias, 0u)
-                          : launch_bulk<7, false, true, true>(g, tl, x, nullptr, M, y, transpose, stream, bias, 0u);
+                return bf ? launch_bulk<7, true, true, true, 1>(g, tl, x, nullptr, M, y, transpose, stream, bias, 0u)
+                          : launch_bulk<7, false, true, true, 1>(g, tl, x, nullptr, M, y, transpose, stream, bias, 0u);
             if (mode == 2)
-                return bf ? launch_bulk<7, true, true>(g, tl, x, nullptr, M, y, transpose, stream, bias, 0u)
-                          : launch_bulk<7, false, true>(g, tl, x, nullptr, M, y, transpose, stream, bias, 0u);
+                return bf ? launch_bulk<7, true, true, false, 1>(g, tl, x, nullptr, M, y, transpose, stream, bias, 0u)
+                          : launch_bulk<7, false, true, false, 1>(g, tl, x, nullptr, M, y, transpose, stream, bias, 0u);
             if (g.H == 7 && g.W == 7)
-                return bf ? launch_bulk<7, true, false, false, true>(g, tl, x, nullptr, M, y, transpose, stream, bias, 0u)
-                          : launch_bulk<7, false, false, false, true>(g, tl, x, nullptr, M, y, transpose, stream, bias, 0u);
-            return bf ? launch_bulk<7, true, false>(g, tl, x, nullptr, M, y, transpose, stream, bias, 0u)
-                      : launch_bulk<7, false, false>(g, tl, x, nullptr, M, y, transpose, stream, bias, 0u);
+                return bf ? launch_bulk<7, true, false, false, 2>(g, tl, x, nullptr, M, y, transpose, stream, bias, 0u)
+                          : launch_bulk<7, false, false, false, 2>(g, tl, x, nullptr, M, y, transpose, stream, bias, 0u);
+            return bf ? launch_bulk<7, true, false, false, 1>(g, tl, x, nullptr, M, y, transpose, stream, bias, 0u)
+                      : launch_bulk<7, false, false, false, 1>(g, tl, x, nullptr, M, y, transpose, stream, bias, 0u);
         }
     }
     if (g.w == 14) {
@@ -1180,11 +1199,11 @@ cudaError_t tc_forward_matrix(const Geom& g, int dtype, const void* x, const voi
             *path = WBMM_PATH_TC_TMA;
             cudaError_t e;
             if (mode == 2)
-                e = bf ? launch_bulk<14, true, true, false, true>(g, tl, x, nullptr, nullptr, y, transpose, stream, bias, 0u, M)
-                       : launch_bulk<14, false, true, false, true>(g, tl, x, nullptr, nullptr, y, transpose, stream, bias, 0u, M);
+                e = bf ? launch_bulk<14, true, true, false, 2>(g, tl, x, nullptr, nullptr, y, transpose, stream, bias, 0u, M)
+                       : launch_bulk<14, false, true, false, 2>(g, tl, x, nullptr, nullptr, y, transpose, stream, bias, 0u, M);
             else
-                e = bf ? launch_bulk<14, true, false, false, true>(g, tl, x, nullptr, nullptr, y, transpose, stream, bias, 0u, M)
-                       : launch_bulk<14, false, false, false, true>(g, tl, x, nullptr, nullptr, y, transpose, stream, bias, 0u, M);
+                e = bf ? launch_bulk<14, true, false, false, 2>(g, tl, x, nullptr, nullptr, y, transpose, stream, bias, 0u, M)
+                       : launch_bulk<14, false, false, false, 2>(g, tl, x, nullptr, nullptr, y, transpose, stream, bias, 0u, M);
             if (e != cudaErrorInvalidConfiguration) return e;
             cudaGetLastError();          // (the ring did not fit after all: the gather kernel below)
         }
