@@ -458,3 +458,86 @@ int wbmm_ref_hier_backward_tables(int B, int C, int H, int W, int w, int sh, int
     }
     return 0;
 }
+
+/* ----------------------------------------------------------------------------------------------
+ * Rectangular windows w_h x w_w (section 3.1: "window size w_h x w_w", d = w_h * w_w,
+ * R in R^{C x (2w_h-1)(2w_w-1)}; Eq. 4-5: pad_h by w_h, pad_w by w_w; Eq. 6-7,
+ * PAPER.md:190-193:  I[i,j] = (dh + w_h - 1)(2w_w - 1) + (dw + w_w - 1)).  w_h = 1 is the 1-D case of
+ * PAPER.md:909.  Same readings as the square operator (A1 orientation, A2 row-major i = r*w_w + c,
+ * A4 padding bottom/right, A6 shift over the padded extent with sh < w_h, sw < w_w, A11).
+ *
+ * Written apart from the square functions above (no shared loops), in the DIRECT form:
+ *   y^[h,v] = sum over (h',v') in the window of (h,v) of T[c, (h-h'+w_h-1)(2w_w-1) + (v-v'+w_w-1)] x^[h',v'].
+ */
+int wbmm_ref_forward_rect(int B, int C, int H, int W, int wh, int ww, int sh, int sw, int layout,
+                          const double *x, const double *T, double *y)
+{
+    if (B < 0 || C < 0 || H < 1 || W < 1 || wh < 1 || ww < 1 || sh < 0 || sw < 0 || sh >= wh || sw >= ww)
+        return 1;
+    const int tw = 2 * ww - 1, nb = (2 * wh - 1) * tw;
+    const int Hp = padded(H, wh), Wp = padded(W, ww);
+    const long planes = (long)B * C;
+
+#pragma omp parallel for schedule(static)
+    for (long pc = 0; pc < planes; ++pc) {
+        int b = (int)(pc / C), c = (int)(pc % C);
+        const double *Tc = T + (size_t)c * nb;
+        for (int ho = 0; ho < H; ++ho)
+            for (int vo = 0; vo < W; ++vo) {
+                int h = modp(ho - sh, Hp), v = modp(vo - sw, Wp);
+                int h0 = (h / wh) * wh, v0 = (v / ww) * ww;
+                double acc = 0.0;
+                for (int hq = h0; hq < h0 + wh; ++hq)
+                    for (int vq = v0; vq < v0 + ww; ++vq)
+                        acc += Tc[(h - hq + wh - 1) * tw + (v - vq + ww - 1)] *
+                               load_hat(x, layout, B, C, H, W, Hp, Wp, sh, sw, b, c, hq, vq);
+                y[elem_off(layout, B, C, H, W, b, c, ho, vo)] = acc;
+            }
+    }
+    return 0;
+}
+
+/*
+ * Backward of the rectangular operator, term by term from the forward sum above:
+ *   dx^[h',v'] = sum over (h,v) in the window of (h',v') of T[c, (h-h'+w_h-1)(2w_w-1) + (v-v'+w_w-1)] dy^[h,v]
+ *   dT[c,k]    = sum over images, windows and pairs ((h,v),(h',v')) of one window with that index k of dy^[h,v] x^[h',v'].
+ * dy is zero outside H x W; dx is un-shifted and cropped.  Either output may be NULL; dT is overwritten.
+ */
+int wbmm_ref_backward_rect(int B, int C, int H, int W, int wh, int ww, int sh, int sw, int layout,
+                           const double *x, const double *T, const double *dy, double *dx, double *dT)
+{
+    if (B < 0 || C < 0 || H < 1 || W < 1 || wh < 1 || ww < 1 || sh < 0 || sw < 0 || sh >= wh || sw >= ww)
+        return 1;
+    const int tw = 2 * ww - 1, nb = (2 * wh - 1) * tw;
+    const int Hp = padded(H, wh), Wp = padded(W, ww);
+
+#pragma omp parallel for schedule(static)
+    for (int c = 0; c < C; ++c) {
+        const double *Tc = T ? T + (size_t)c * nb : NULL;
+        if (dT)
+            for (int k = 0; k < nb; ++k) dT[(size_t)c * nb + k] = 0.0;
+        for (int b = 0; b < B; ++b)
+            for (int h0 = 0; h0 < Hp; h0 += wh)
+                for (int v0 = 0; v0 < Wp; v0 += ww) {
+                    /* one window: input position (hq,vq), output position (h,v) */
+                    for (int hq = h0; hq < h0 + wh; ++hq)
+                        for (int vq = v0; vq < v0 + ww; ++vq) {
+                            double xin = dT ? load_hat(x, layout, B, C, H, W, Hp, Wp, sh, sw, b, c, hq, vq) : 0.0;
+                            double acc = 0.0;
+                            for (int h = h0; h < h0 + wh; ++h)
+                                for (int v = v0; v < v0 + ww; ++v) {
+                                    int k = (h - hq + wh - 1) * tw + (v - vq + ww - 1);
+                                    double g = load_hat(dy, layout, B, C, H, W, Hp, Wp, sh, sw, b, c, h, v);
+                                    if (dx) acc += Tc[k] * g;
+                                    if (dT) dT[(size_t)c * nb + k] += g * xin;
+                                }
+                            if (dx) {
+                                int hs = modp(hq + sh, Hp), vs = modp(vq + sw, Wp);
+                                if (hs < H && vs < W)
+                                    dx[elem_off(layout, B, C, H, W, b, c, hs, vs)] = acc;
+                            }
+                        }
+                }
+    }
+    return 0;
+}

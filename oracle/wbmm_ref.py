@@ -55,6 +55,10 @@ def _load():
         f = getattr(lib, name)
         f.restype = i
         f.argtypes = [i] * 8 + [dp, dp, dp]
+    lib.wbmm_ref_forward_rect.restype = i
+    lib.wbmm_ref_forward_rect.argtypes = [i] * 9 + [dp, dp, dp]
+    lib.wbmm_ref_backward_rect.restype = i
+    lib.wbmm_ref_backward_rect.argtypes = [i] * 9 + [dp, dp, dp, dp, dp]
     lib.wbmm_ref_backward.restype = i
     lib.wbmm_ref_backward.argtypes = [i] * 8 + [dp, dp, dp, dp, dp]
     lib.wbmm_ref_hier_forward_train.restype = i
@@ -141,6 +145,40 @@ def backward(x, T, dy, w, shift=(0, 0), layout=NCHW, need_dx=True, need_dT=True)
     dT = np.zeros_like(T) if need_dT else None
     rc = _load().wbmm_ref_backward(
         B, C, H, W, w, int(shift[0]), int(shift[1]), layout, xp, tp, gp,
+        dx.ctypes.data_as(ctypes.POINTER(ctypes.c_double)) if need_dx else null,
+        dT.ctypes.data_as(ctypes.POINTER(ctypes.c_double)) if need_dT else null)
+    if rc != 0:
+        raise ValueError(f"oracle rejected arguments (rc={rc})")
+    return dx, dT
+
+
+def forward_rect(x, T, wh, ww, shift=(0, 0), layout=NCHW) -> np.ndarray:
+    """Rectangular windows w_h x w_w (Eq. 4-7): y = WBMM(x; T), T [C,(2w_h-1)(2w_w-1)]."""
+    x, xp = _d(x)
+    T, tp = _d(T)
+    B, C, H, W = _dims(x, layout)
+    assert T.shape == (C, (2 * wh - 1) * (2 * ww - 1)), (T.shape, C, wh, ww)
+    y = np.zeros_like(x)
+    rc = _load().wbmm_ref_forward_rect(B, C, H, W, wh, ww, int(shift[0]), int(shift[1]), layout, xp, tp,
+                                       y.ctypes.data_as(ctypes.POINTER(ctypes.c_double)))
+    if rc != 0:
+        raise ValueError(f"oracle rejected arguments (rc={rc})")
+    return y
+
+
+def backward_rect(x, T, dy, wh, ww, shift=(0, 0), layout=NCHW, need_dx=True, need_dT=True):
+    """(dx, dT) of forward_rect in float64; either is None when not requested."""
+    x, xp = _d(x)
+    T, tp = _d(T)
+    dy, gp = _d(dy)
+    assert dy.shape == x.shape
+    B, C, H, W = _dims(x, layout)
+    assert T.shape == (C, (2 * wh - 1) * (2 * ww - 1))
+    null = ctypes.POINTER(ctypes.c_double)()
+    dx = np.zeros_like(x) if need_dx else None
+    dT = np.zeros_like(T) if need_dT else None
+    rc = _load().wbmm_ref_backward_rect(
+        B, C, H, W, wh, ww, int(shift[0]), int(shift[1]), layout, xp, tp, gp,
         dx.ctypes.data_as(ctypes.POINTER(ctypes.c_double)) if need_dx else null,
         dT.ctypes.data_as(ctypes.POINTER(ctypes.c_double)) if need_dT else null)
     if rc != 0:

@@ -591,3 +591,104 @@ def test_fold_dwconv_equals_library_conv_on_one_window(oracle, w):
     Tf = oracle.fold_dwconv(oracle.fold_dwconv(T, K5, w, s1), K3, w, s2)
     got = oracle.apply_matrix(x, oracle.weight_matrix(Tf, w), w, bias=b1 + b2)
     assert np.max(np.abs(got - ref)) < 1e-11
+
+
+# ------------------------------------------------------------------ rectangular windows w_h x w_w (Eq. 4-7)
+RECT = [(2, 3), (3, 2), (1, 5), (4, 1), (7, 14), (14, 7), (3, 8)]
+
+
+@pytest.mark.parametrize("wh,ww", RECT)
+def test_rect_single_window_is_depthwise_conv(oracle, wh, ww):
+    """Theorem 3.2 for a w_h x w_w window: on a map of ONE window the operator is the zero-padded depthwise conv with a
+    (2w_h-1) x (2w_w-1) kernel -- a library routine (torch conv2d).  Pins Eq. 7's rectangular index
+    I = (dh + w_h - 1)(2w_w - 1) + (dw + w_w - 1): a transposed table shape or a swapped w_h / w_w fails."""
+    r = rng(31)
+    C = 3
+    x = r.standard_normal((2, C, wh, ww))
+    T = r.standard_normal((C, (2 * wh - 1) * (2 * ww - 1)))
+    y = oracle.forward_rect(x, T, wh, ww)
+    K = torch.from_numpy(T.reshape(C, 1, 2 * wh - 1, 2 * ww - 1))
+    ref = F.conv2d(torch.from_numpy(x), torch.flip(K, dims=(2, 3)), padding=(wh - 1, ww - 1), groups=C)
+    assert np.allclose(y, ref.numpy(), rtol=0, atol=1e-12)
+
+
+@pytest.mark.parametrize("w,s,H,W,layout", [(3, (0, 0), 9, 6, NCHW), (4, (1, 3), 10, 7, NCHW), (7, (3, 2), 14, 20, NHWC)])
+def test_rect_reduces_to_the_square_operator(oracle, w, s, H, W, layout):
+    """w_h = w_w = w: forward, dX and dT equal the square oracle's (written apart: two sets of loops)."""
+    r = rng(32)
+    shape = (2, 3, H, W) if layout == NCHW else (2, H, W, 3)
+    x, dy = r.standard_normal(shape), r.standard_normal(shape)
+    T = r.standard_normal((3, (2 * w - 1) ** 2))
+    assert np.allclose(oracle.forward_rect(x, T, w, w, s, layout), oracle.forward(x, T, w, s, layout), rtol=0, atol=1e-12)
+    dx, dT = oracle.backward_rect(x, T, dy, w, w, s, layout)
+    rdx, rdT = oracle.backward(x, T, dy, w, s, layout)
+    assert np.allclose(dx, rdx, rtol=0, atol=1e-12) and np.allclose(dT, rdT, rtol=0, atol=1e-11)
+
+
+def test_rect_windows_do_not_interact_and_padding_is_cropped(oracle):
+    """Each w_h x w_w window equals the conv on its isolated crop (Alg. 1 l.3-4); Eq. 4-5: pad_h by w_h, pad_w by w_w."""
+    r = rng(33)
+    wh, ww, C = 2, 5, 2
+    x = r.standard_normal((1, C, 5, 12))                       # H' = 6, W' = 15
+    T = r.standard_normal((C, 3 * 9))
+    y = oracle.forward_rect(x, T, wh, ww)
+    xp = np.zeros((1, C, 6, 15))
+    xp[:, :, :5, :12] = x
+    yp = oracle.forward_rect(xp, T, wh, ww)
+    assert np.array_equal(y, yp[:, :, :5, :12])
+    K = torch.flip(torch.from_numpy(T.reshape(C, 1, 3, 9)), dims=(2, 3))
+    for wy in range(3):
+        for wx in range(3):
+            crop = xp[:, :, wy * wh:(wy + 1) * wh, wx * ww:(wx + 1) * ww]
+            ref = F.conv2d(torch.from_numpy(crop.copy()), K, padding=(wh - 1, ww - 1), groups=C).numpy()
+            assert np.allclose(yp[:, :, wy * wh:(wy + 1) * wh, wx * ww:(wx + 1) * ww], ref, atol=1e-12)
+
+
+@pytest.mark.parametrize("wh,ww,s,H,W", [(2, 3, (1, 2), 6, 9), (3, 5, (2, 4), 7, 11), (1, 4, (0, 3), 3, 10)])
+def test_rect_shift_equals_explicit_roll(oracle, wh, ww, s, H, W):
+    """A6 on rectangular windows: pad, roll by -s over the padded extent, operator, roll back, crop."""
+    r = rng(34)
+    x = r.standard_normal((2, 2, H, W))
+    T = r.standard_normal((2, (2 * wh - 1) * (2 * ww - 1)))
+    Hp, Wp = -(-H // wh) * wh, -(-W // ww) * ww
+    xp = np.zeros((2, 2, Hp, Wp))
+    xp[:, :, :H, :W] = x
+    yr = oracle.forward_rect(np.roll(xp, shift=(-s[0], -s[1]), axis=(2, 3)), T, wh, ww)
+    ref = np.roll(yr, shift=(s[0], s[1]), axis=(2, 3))[:, :, :H, :W]
+    assert np.allclose(oracle.forward_rect(x, T, wh, ww, s), ref, rtol=0, atol=1e-13)
+
+
+@pytest.mark.parametrize("wh,ww,s,H,W,layout", [(2, 3, (1, 2), 6, 9, NCHW), (3, 5, (2, 4), 7, 11, NHWC), (1, 6, (0, 0), 2, 13, NCHW)])
+def test_rect_backward_adjoint_and_finite_differences(oracle, wh, ww, s, H, W, layout):
+    """<dy, A x> = <A^T dy, x> for dx; dT against central differences of the (linear in T) forward."""
+    r = rng(35)
+    C = 2
+    shape = (2, C, H, W) if layout == NCHW else (2, H, W, C)
+    x, dy = r.standard_normal(shape), r.standard_normal(shape)
+    nb = (2 * wh - 1) * (2 * ww - 1)
+    T = r.standard_normal((C, nb))
+    dx, dT = oracle.backward_rect(x, T, dy, wh, ww, s, layout)
+    assert np.isclose(np.sum(dy * oracle.forward_rect(x, T, wh, ww, s, layout)), np.sum(dx * x), rtol=1e-12)
+    for c, k in ((0, 0), (1, nb - 1), (0, nb // 2), (1, 3)):
+        E = np.zeros_like(T)
+        E[c, k] = 1.0
+        # the forward is linear in T: its derivative along E is the forward with table E
+        assert np.isclose(dT[c, k], np.sum(dy * oracle.forward_rect(x, E, wh, ww, s, layout)), rtol=1e-11, atol=1e-12)
+
+
+def test_rect_one_dimensional_windows(oracle):
+    """w_h = 1 (1-D sequences): rows never mix, each row is a windowed 1-D operator."""
+    r = rng(36)
+    ww = 5
+    x = r.standard_normal((2, 3, 4, 15))
+    T = r.standard_normal((3, 2 * ww - 1))
+    y = oracle.forward_rect(x, T, 1, ww)
+    for h in range(4):
+        assert np.array_equal(y[:, :, h:h + 1, :], oracle.forward_rect(x[:, :, h:h + 1, :].copy(), T, 1, ww))
+    # brute force: y[v] = sum_{v' in window} T[v - v' + ww - 1] x[v']
+    ref = np.zeros_like(x)
+    for v in range(15):
+        v0 = (v // ww) * ww
+        for vq in range(v0, v0 + ww):
+            ref[:, :, :, v] += T[None, :, None, v - vq + ww - 1] * x[:, :, :, vq]
+    assert np.allclose(y, ref, rtol=0, atol=1e-12)
