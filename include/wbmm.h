@@ -145,6 +145,20 @@ WBMM_API int wbmm_backward(const wbmm_desc_t *desc, const void *x, const void *T
                   void *dx, float *dT, void *cuda_stream);
 
 /*
+ * Rectangular windows w_h x w_w (section 3.1 states the method for a "window size w_h x w_w": d = w_h*w_w
+ * positions, table [C][(2w_h-1)(2w_w-1)] row-major; Eq. 4-5 pad H to a multiple of w_h and W to a multiple of w_w;
+ * Eq. 6-7  I[i,j] = (dh + w_h - 1)(2w_w - 1) + (dw + w_w - 1)).  w_h = 1 gives the 1-D windows of PAPER.md:909.
+ *   desc->w is w_h, w_w is passed beside it; desc->shift_h in [0, w_h), desc->shift_w in [0, w_w).
+ *   x, T, y / dy, dx, dT: as wbmm_forward / wbmm_backward with the rectangular table shape.
+ * w_w == desc->w is the square operator and is served by wbmm_forward / wbmm_backward (tensor cores).  Other shapes run on
+ * FFMA kernels (any dtype / layout / shift / ragged size; wbmm_last_path() = WBMM_PATH_SIMT); w_h*w_w <= 1024 and
+ * (2w_h-1)(2w_w-1) <= 4096, else WBMM_STATUS_UNSUPPORTED.  dT: cleared first unless WBMM_FLAG_ACCUMULATE_DT; atomics.
+ */
+WBMM_API int wbmm_forward_rect(const wbmm_desc_t *desc, int32_t w_w, const void *x, const void *T, void *y, void *cuda_stream);
+WBMM_API int wbmm_backward_rect(const wbmm_desc_t *desc, int32_t w_w, const void *x, const void *T, const void *dy,
+                       void *dx, float *dT, void *cuda_stream);
+
+/*
  * Hierarchical window reparameterisation, fused (section 3.6, Eq. 9; PAPER.md:862-887
  * Algorithm 3; identical in value to the training form, Algorithm 2):
  *     y_win = (M_g + diag_blocks(M_l) + 2 I) * x_win

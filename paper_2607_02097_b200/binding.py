@@ -24,7 +24,7 @@ _DTYPES = {torch.float32: DTYPE_F32, torch.bfloat16: DTYPE_BF16, torch.float16: 
 
 # every symbol include/wbmm.h declares
 EXPORTS = (
-    "wbmm_forward", "wbmm_forward_static_scratch", "wbmm_backward", "wbmm_hier_forward", "wbmm_hier_backward", "wbmm_forward_matrix", "wbmm_fold_dwconv", "wbmm_forward_fused", "wbmm_materialize_weight", "wbmm_forward_host",
+    "wbmm_forward", "wbmm_forward_static_scratch", "wbmm_forward_rect", "wbmm_backward_rect", "wbmm_backward", "wbmm_hier_forward", "wbmm_hier_backward", "wbmm_forward_matrix", "wbmm_fold_dwconv", "wbmm_forward_fused", "wbmm_materialize_weight", "wbmm_forward_host",
     "wbmm_backward_host", "wbmm_release", "wbmm_last_path", "wbmm_launch_count",
     "wbmm_status_string", "wbmm_path_string", "wbmm_last_error_string", "wbmm_version",
 )
@@ -57,6 +57,10 @@ def lib() -> ctypes.CDLL:
     L.wbmm_forward.argtypes = [dp, vp, vp, vp, vp]
     L.wbmm_forward_static_scratch.argtypes = [dp, vp, vp, vp, vp]
     L.wbmm_forward_static_scratch.restype = i
+    L.wbmm_forward_rect.argtypes = [dp, ctypes.c_int32, vp, vp, vp, vp]
+    L.wbmm_forward_rect.restype = i
+    L.wbmm_backward_rect.argtypes = [dp, ctypes.c_int32, vp, vp, vp, vp, vp, vp]
+    L.wbmm_backward_rect.restype = i
     L.wbmm_backward.argtypes = [dp, vp, vp, vp, vp, vp, vp]
     L.wbmm_hier_forward.argtypes = [dp, vp, vp, vp, vp, i, vp]
     L.wbmm_hier_forward.restype = i
@@ -169,6 +173,35 @@ def wbmm_forward_static_scratch(x: torch.Tensor, T: torch.Tensor, w: int, shift=
     with torch.cuda.device(x.device):
         _check(lib().wbmm_forward_static_scratch(ctypes.byref(d), px, pT, py, _stream(x)))
     return y
+
+
+def wbmm_forward_rect(x: torch.Tensor, T: torch.Tensor, wh: int, ww: int, shift=(0, 0), layout: int = NCHW,
+                      out: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """Rectangular windows w_h x w_w (include/wbmm.h: wbmm_forward_rect); T is [C, (2w_h-1)(2w_w-1)]."""
+    d = make_desc(x, wh, shift, layout, 0)
+    if T.dtype != x.dtype or tuple(T.shape) != (d.C, (2 * wh - 1) * (2 * ww - 1)):
+        raise ValueError("T must be [C,(2w_h-1)(2w_w-1)] in the dtype of x")
+    y = torch.empty_like(x) if out is None else out
+    px, pT, py = _dev(x, "x"), _dev(T, "T"), _dev(y, "y")
+    with torch.cuda.device(x.device):
+        _check(lib().wbmm_forward_rect(ctypes.byref(d), int(ww), px, pT, py, _stream(x)))
+    return y
+
+
+def wbmm_backward_rect(x: Optional[torch.Tensor], T: Optional[torch.Tensor], dy: torch.Tensor, wh: int, ww: int,
+                       shift=(0, 0), layout: int = NCHW, flags: int = 0, need_dx: bool = True, need_dT: bool = True,
+                       dT: Optional[torch.Tensor] = None):
+    """(dx, dT) of wbmm_forward_rect; dT is float32 [C, (2w_h-1)(2w_w-1)]."""
+    d = make_desc(dy, wh, shift, layout, flags)
+    dx = torch.empty_like(dy) if need_dx else None
+    if need_dT and dT is None:
+        dT = torch.empty((d.C, (2 * wh - 1) * (2 * ww - 1)), dtype=torch.float32, device=dy.device)
+    if not need_dT:
+        dT = None
+    with torch.cuda.device(dy.device):
+        _check(lib().wbmm_backward_rect(ctypes.byref(d), int(ww), _dev(x, "x"), _dev(T, "T"), _dev(dy, "dy"),
+                                        _dev(dx, "dx"), _dev(dT, "dT"), _stream(dy)))
+    return dx, dT
 
 
 def wbmm_hier_forward(x: torch.Tensor, Tg: torch.Tensor, Tl: torch.Tensor, w: int, shift=(0, 0),

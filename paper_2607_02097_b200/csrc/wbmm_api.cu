@@ -389,6 +389,67 @@ int wbmm_backward(const wbmm_desc_t* desc, const void* x, const void* T, const v
     return WBMM_STATUS_OK;
 }
 
+// Rectangular windows: desc->w is w_h, w_w is passed beside it.
+static int validate_rect(const wbmm_desc_t* d, int w_w)
+{
+    if (!d) return WBMM_STATUS_INVALID_ARGUMENT;
+    if (d->B < 0 || d->C < 0 || d->H < 1 || d->W < 1 || d->w < 1 || w_w < 1) return WBMM_STATUS_INVALID_ARGUMENT;
+    if (d->shift_h < 0 || d->shift_w < 0 || d->shift_h >= d->w || d->shift_w >= w_w) return WBMM_STATUS_INVALID_ARGUMENT;
+    if (d->dtype != WBMM_DTYPE_F32 && d->dtype != WBMM_DTYPE_BF16 && d->dtype != WBMM_DTYPE_F16) return WBMM_STATUS_INVALID_ARGUMENT;
+    if (d->layout != WBMM_LAYOUT_NCHW && d->layout != WBMM_LAYOUT_NHWC) return WBMM_STATUS_INVALID_ARGUMENT;
+    long long n = (long long)d->B * d->C;
+    if (n > (1ll << 40) / ((long long)d->H * d->W)) return WBMM_STATUS_UNSUPPORTED;
+    return WBMM_STATUS_OK;
+}
+
+int wbmm_forward_rect(const wbmm_desc_t* desc, int32_t w_w, const void* x, const void* T, void* y, void* cuda_stream)
+{
+    if (desc && w_w == desc->w) return wbmm_forward(desc, x, T, y, cuda_stream);      // square: the tensor-core kernels
+    int st = validate_rect(desc, w_w);
+    if (st != WBMM_STATUS_OK) return st;
+    if (desc->B == 0 || desc->C == 0) return WBMM_STATUS_OK;
+    if (!x || !T || !y || x == y) return WBMM_STATUS_INVALID_ARGUMENT;
+    const size_t es = elem_size(desc->dtype);
+    if (!aligned(x, es) || !aligned(T, es) || !aligned(y, es)) return WBMM_STATUS_MISALIGNED;
+    if (device_state() < 0) return WBMM_STATUS_NO_DEVICE;
+    if (!wbmm::rect_supported(*desc, w_w)) return WBMM_STATUS_UNSUPPORTED;
+    int launches = 0;
+    cudaError_t e = wbmm::rect_forward(*desc, w_w, x, T, y, false, static_cast<cudaStream_t>(cuda_stream), &launches);
+    g_launches += launches;
+    if (e != cudaSuccess) return set_cuda_error(e, "rect_forward");
+    t_last_path = WBMM_PATH_SIMT;
+    return WBMM_STATUS_OK;
+}
+
+int wbmm_backward_rect(const wbmm_desc_t* desc, int32_t w_w, const void* x, const void* T, const void* dy,
+                       void* dx, float* dT, void* cuda_stream)
+{
+    if (desc && w_w == desc->w) return wbmm_backward(desc, x, T, dy, dx, dT, cuda_stream);
+    int st = validate_rect(desc, w_w);
+    if (st != WBMM_STATUS_OK) return st;
+    if (desc->C == 0) return WBMM_STATUS_OK;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    const long long nb = (2ll * desc->w - 1) * (2ll * w_w - 1);
+    if (dT && !aligned(dT, 4)) return WBMM_STATUS_MISALIGNED;
+    if (desc->B > 0 && (!dy || (dx && !T) || (dT && !x) || (dx && dx == dy))) return WBMM_STATUS_INVALID_ARGUMENT;
+    const size_t es = elem_size(desc->dtype);
+    if (desc->B > 0 && (!aligned(dy, es) || (x && !aligned(x, es)) || (T && !aligned(T, es)) || (dx && !aligned(dx, es))))
+        return WBMM_STATUS_MISALIGNED;
+    if (device_state() < 0) return WBMM_STATUS_NO_DEVICE;
+    if (desc->B > 0 && !wbmm::rect_supported(*desc, w_w)) return WBMM_STATUS_UNSUPPORTED;
+    int launches = 0;
+    cudaError_t e = cudaSuccess;
+    if (dT && !(desc->flags & WBMM_FLAG_ACCUMULATE_DT)) e = wbmm::simt_zero_f32(dT, (long long)desc->C * nb, stream, &launches);
+    if (desc->B > 0) {
+        if (e == cudaSuccess && dx) e = wbmm::rect_forward(*desc, w_w, dy, T, dx, true, stream, &launches);
+        if (e == cudaSuccess && dT) e = wbmm::rect_grad_table(*desc, w_w, x, dy, dT, stream, &launches);
+    }
+    g_launches += launches;
+    if (e != cudaSuccess) return set_cuda_error(e, "rect backward");
+    t_last_path = WBMM_PATH_SIMT;
+    return WBMM_STATUS_OK;
+}
+
 int wbmm_hier_forward(const wbmm_desc_t* desc, const void* x, const void* Tg, const void* Tl, void* y,
                       int transpose, void* cuda_stream)
 {

@@ -72,5 +72,9 @@ bool transpose16_supported(long long R, long long Cc, const void* in, const void
 cudaError_t transpose16(const void* in, void* out, int batch, int R, int Cc, cudaStream_t stream, int* launches);
 // Largest window the SIMT kernels can stage in shared memory for this layout.
 bool simt_supported(const Geom& g);
+// Rectangular windows w_h x w_w (wbmm_rect.cu): d.w is w_h, `ww` is w_w; shifts in [0, w_h) x [0, w_w).
+bool rect_supported(const wbmm_desc_t& d, int ww);
+cudaError_t rect_forward(const wbmm_desc_t& d, int ww, const void* x, const void* T, void* y, bool reverse, cudaStream_t stream, int* launches);
+cudaError_t rect_grad_table(const wbmm_desc_t& d, int ww, const void* x, const void* dy, float* dT, cudaStream_t stream, int* launches);
 
 }  // namespace wbmm

@@ -1,0 +1,234 @@
+// WBMM with RECTANGULAR windows w_h x w_w (section 3.1: "window size w_h x w_w", d = w_h * w_w positions,
+// table R in R^{C x (2w_h-1)(2w_w-1)}; Eq. 4-5 pad H by w_h and W by w_w; Eq. 6-7:
+//     I[i,j] = (dh + w_h - 1)(2w_w - 1) + (dw + w_w - 1),   dh = h_i - h_j, dw = w_i - w_j).
+// w_h = 1 (or w_w = 1) is the 1-D case the paper names as an extension.  SURVEY.md 8(f) NEXT-4.
+//
+// FFMA kernels (fp32 accumulate), any layout / shift / ragged size / dtype: the general statement of the operator.
+// The square sizes 7 and 14 have the tensor-core kernels; nothing here is on their path.
+//   forward / dX   a block = one channel x G windows: the table row and the windows staged in shared memory as fp32,
+//                  a thread per (output position, four windows) walks the w_h x w_w inputs of its windows
+//   dT             a block = one channel x a run of window groups: a thread per bin (dr, dc) sums dy[p] * x[p - (dr, dc)]
+//                  over the staged windows, one atomicAdd per bin and block at the end
+#include "wbmm_common.cuh"
+
+namespace wbmm {
+
+namespace {
+
+constexpr int kThreadsR = 256;
+
+struct RectGeom {
+    int B, C, H, W, wh, ww, sh, sw, layout;
+    int Hp, Wp, nwh, nww, N, tw, nb;
+    long long nwin;
+};
+
+__device__ __forceinline__ long long rect_offset(const RectGeom& g, int b, int c, int h, int v)
+{
+    if (g.layout == WBMM_LAYOUT_NCHW) return (((long long)b * g.C + c) * g.H + h) * g.W + v;
+    return (((long long)b * g.H + h) * g.W + v) * g.C + c;
+}
+
+// element of the zero-extended, cyclically shifted frame that window `win` holds at in-window position p; -1 = padding
+__device__ __forceinline__ long long rect_window_elem(const RectGeom& g, long long win, int p, int c)
+{
+    const int wpi = g.nwh * g.nww;
+    const int b = (int)(win / wpi), wl = (int)(win - (long long)b * wpi);
+    const int wy = wl / g.nww, wx = wl - wy * g.nww;
+    int h = wy * g.wh + p / g.ww + g.sh, v = wx * g.ww + p % g.ww + g.sw;
+    if (h >= g.Hp) h -= g.Hp;
+    if (v >= g.Wp) v -= g.Wp;
+    if (h >= g.H || v >= g.W) return -1;
+    return rect_offset(g, b, c, h, v);
+}
+
+template <typename E>
+__global__ void __launch_bounds__(kThreadsR)
+rect_forward_kernel(RectGeom g, const E* __restrict__ x, const E* __restrict__ T, E* __restrict__ y, int G, int reverse)
+{
+    // G is a multiple of 4; windows are staged position-major, xs[q][G], so that a thread -- one output position of
+    // FOUR windows -- reads the four inputs it needs with one 16-byte load (the same address for every thread of its
+    // window quad: a broadcast) and one table entry per input position: 2 shared-memory loads per 4 FFMA.
+    extern __shared__ __align__(16) float smem[];
+    float* xs = smem;                    // [N][G]
+    float* Ts = smem + g.N * G;          // [nb]
+    const int c = blockIdx.y;
+    const long long win0 = (long long)blockIdx.x * G;
+    for (int k = threadIdx.x; k < g.nb; k += kThreadsR)
+        Ts[k] = to_f32(T[(long long)c * g.nb + (reverse ? g.nb - 1 - k : k)]);
+    for (int idx = threadIdx.x; idx < G * g.N; idx += kThreadsR) {
+        const int gw = idx / g.N, p = idx - gw * g.N;
+        float val = 0.f;
+        if (win0 + gw < g.nwin) {
+            const long long off = rect_window_elem(g, win0 + gw, p, c);
+            if (off >= 0) val = to_f32(x[off]);
+        }
+        xs[p * G + gw] = val;
+    }
+    __syncthreads();
+    const int nq = G / 4;
+    for (int idx = threadIdx.x; idx < nq * g.N; idx += kThreadsR) {
+        const int gq = idx / g.N, p = idx - gq * g.N;
+        const int r = p / g.ww, cc = p - r * g.ww;
+        // Eq. 7 with i = p (output), j = q (input): k = (r - rq + w_h - 1)(2w_w - 1) + (cc - cq + w_w - 1)
+        const float* Tr = Ts + (r + g.wh - 1) * g.tw + cc + g.ww - 1;
+        const float4* xq = reinterpret_cast<const float4*>(xs) + gq;
+        float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
+        for (int rq = 0; rq < g.wh; ++rq) {
+            const float* Trr = Tr - rq * g.tw;
+            const float4* xr = xq + (long long)rq * g.ww * nq;
+            for (int cq = 0; cq < g.ww; ++cq) {
+                const float t = Trr[-cq];
+                const float4 v = xr[cq * nq];
+                a0 = fmaf(t, v.x, a0); a1 = fmaf(t, v.y, a1); a2 = fmaf(t, v.z, a2); a3 = fmaf(t, v.w, a3);
+            }
+        }
+        const float acc[4] = {a0, a1, a2, a3};
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const long long win = win0 + gq * 4 + u;
+            if (win >= g.nwin) break;
+            const long long off = rect_window_elem(g, win, p, c);
+            if (off >= 0) y[off] = from_f32<E>(acc[u]);          // padding is cropped (Eq. 4-5)
+        }
+    }
+}
+
+template <typename E>
+__global__ void __launch_bounds__(kThreadsR)
+rect_grad_table_kernel(RectGeom g, const E* __restrict__ x, const E* __restrict__ dy, float* __restrict__ dT, int G, int groups_per_block)
+{
+    extern __shared__ __align__(16) float smem[];
+    float* xs = smem;                    // [G][N]
+    float* gs = smem + G * g.N;          // [G][N]
+    const int c = blockIdx.y;
+    const long long ngroups = (g.nwin + G - 1) / G;
+    const long long grp0 = (long long)blockIdx.x * groups_per_block;
+    // bins owned by this thread: k = threadIdx.x + i * kThreadsR, at most kMaxOwn of them
+    constexpr int kMaxOwn = 16;          // nb <= 4096
+    float acc[kMaxOwn];
+#pragma unroll
+    for (int i = 0; i < kMaxOwn; ++i) acc[i] = 0.f;
+    for (long long grp = grp0; grp < grp0 + groups_per_block && grp < ngroups; ++grp) {
+        __syncthreads();
+        for (int idx = threadIdx.x; idx < G * g.N; idx += kThreadsR) {
+            const int gw = idx / g.N, p = idx - gw * g.N;
+            float xv = 0.f, gv = 0.f;
+            if (grp * G + gw < g.nwin) {
+                const long long off = rect_window_elem(g, grp * G + gw, p, c);
+                if (off >= 0) { xv = to_f32(x[off]); gv = to_f32(dy[off]); }      // dy is zero outside H x W (A11)
+            }
+            xs[idx] = xv;
+            gs[idx] = gv;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int i = 0; i < kMaxOwn; ++i) {
+            const int k = threadIdx.x + i * kThreadsR;
+            if (k >= g.nb) break;
+            // bin k = (dr + w_h - 1)(2w_w - 1) + (dc + w_w - 1): pairs p = (rp, cp), q = (rp - dr, cp - dc) inside the window
+            const int dr = k / g.tw - (g.wh - 1), dc = k % g.tw - (g.ww - 1);
+            const int r0 = max(0, dr), r1 = min(g.wh, g.wh + dr), c0 = max(0, dc), c1 = min(g.ww, g.ww + dc);
+            float a = 0.f;
+            for (int gw = 0; gw < G; ++gw) {
+                const float* xw = xs + gw * g.N;
+                const float* gw_ = gs + gw * g.N;
+                for (int rp = r0; rp < r1; ++rp)
+                    for (int cp = c0; cp < c1; ++cp) a = fmaf(gw_[rp * g.ww + cp], xw[(rp - dr) * g.ww + cp - dc], a);
+            }
+            acc[i] += a;
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < kMaxOwn; ++i) {
+        const int k = threadIdx.x + i * kThreadsR;
+        if (k < g.nb) atomicAdd(dT + (long long)c * g.nb + k, acc[i]);
+    }
+}
+
+RectGeom make_rect(const wbmm_desc_t& d, int ww)
+{
+    RectGeom g;
+    g.B = d.B; g.C = d.C; g.H = d.H; g.W = d.W; g.wh = d.w; g.ww = ww;
+    g.sh = d.shift_h; g.sw = d.shift_w; g.layout = d.layout;
+    g.Hp = (d.H + g.wh - 1) / g.wh * g.wh;
+    g.Wp = (d.W + g.ww - 1) / g.ww * g.ww;
+    g.nwh = g.Hp / g.wh; g.nww = g.Wp / g.ww;
+    g.N = g.wh * g.ww;
+    g.tw = 2 * g.ww - 1; g.nb = (2 * g.wh - 1) * g.tw;
+    g.nwin = (long long)d.B * g.nwh * g.nww;
+    return g;
+}
+
+int rect_group(const RectGeom& g) { int G = (2048 / g.N) & ~3; return G < 4 ? 4 : (G > 32 ? 32 : G); }      // a multiple of 4
+
+template <typename E>
+cudaError_t rect_forward_t(const RectGeom& g, const E* x, const E* T, E* y, bool reverse, cudaStream_t s)
+{
+    const int G = rect_group(g);
+    const size_t smem = sizeof(float) * ((size_t)g.nb + (size_t)G * g.N);
+    auto k = rect_forward_kernel<E>;
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    dim3 grid((unsigned)((g.nwin + G - 1) / G), (unsigned)g.C);
+    k<<<grid, kThreadsR, smem, s>>>(g, x, T, y, G, reverse ? 1 : 0);
+    return cudaGetLastError();
+}
+
+template <typename E>
+cudaError_t rect_grad_table_t(const RectGeom& g, const E* x, const E* dy, float* dT, cudaStream_t s)
+{
+    const int G = rect_group(g);
+    const size_t smem = sizeof(float) * 2 * (size_t)G * g.N;
+    auto k = rect_grad_table_kernel<E>;
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    const long long ngroups = (g.nwin + G - 1) / G;
+    long long want = (8ll * 148 + g.C - 1) / g.C;          // about 8 waves of blocks
+    if (want < 1) want = 1;
+    long long nsplit = ngroups < want ? ngroups : want;
+    const int gpb = (int)((ngroups + nsplit - 1) / nsplit);
+    nsplit = (ngroups + gpb - 1) / gpb;
+    dim3 grid((unsigned)nsplit, (unsigned)g.C);
+    k<<<grid, kThreadsR, smem, s>>>(g, x, dy, dT, G, gpb);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+// window area and table size the kernels stage in shared memory / registers
+bool rect_supported(const wbmm_desc_t& d, int ww)
+{
+    if (ww < 1 || d.w < 1 || d.w > 1024 || ww > 1024) return false;
+    const long long N = (long long)d.w * ww, nb = (2ll * d.w - 1) * (2ll * ww - 1);
+    if (N > 1024 || nb > 4096 || d.C > 65535) return false;
+    const RectGeom g = make_rect(d, ww);
+    return (g.nwin + rect_group(g) - 1) / rect_group(g) <= 0x7fffffffll;
+}
+
+cudaError_t rect_forward(const wbmm_desc_t& d, int ww, const void* x, const void* T, void* y, bool reverse, cudaStream_t s, int* launches)
+{
+    const RectGeom g = make_rect(d, ww);
+    if (g.nwin == 0 || g.C == 0) return cudaSuccess;
+    *launches += 1;
+    switch (d.dtype) {
+    case WBMM_DTYPE_F32: return rect_forward_t<float>(g, (const float*)x, (const float*)T, (float*)y, reverse, s);
+    case WBMM_DTYPE_BF16: return rect_forward_t<__nv_bfloat16>(g, (const __nv_bfloat16*)x, (const __nv_bfloat16*)T, (__nv_bfloat16*)y, reverse, s);
+    default: return rect_forward_t<__half>(g, (const __half*)x, (const __half*)T, (__half*)y, reverse, s);
+    }
+}
+
+// adds into dT (the caller clears it)
+cudaError_t rect_grad_table(const wbmm_desc_t& d, int ww, const void* x, const void* dy, float* dT, cudaStream_t s, int* launches)
+{
+    const RectGeom g = make_rect(d, ww);
+    if (g.nwin == 0 || g.C == 0) return cudaSuccess;
+    *launches += 1;
+    switch (d.dtype) {
+    case WBMM_DTYPE_F32: return rect_grad_table_t<float>(g, (const float*)x, (const float*)dy, dT, s);
+    case WBMM_DTYPE_BF16: return rect_grad_table_t<__nv_bfloat16>(g, (const __nv_bfloat16*)x, (const __nv_bfloat16*)dy, dT, s);
+    default: return rect_grad_table_t<__half>(g, (const __half*)x, (const __half*)dy, dT, s);
+    }
+}
+
+}  // namespace wbmm
