@@ -32,7 +32,8 @@
  *     WBMM_FLAG_NO_SCRATCH forbids the temporaries; the call is then served by the slower scratch-free kernels.
  *     Every other path allocates nothing.
  *   - float32 activations with w in {7, 14} run on the tensor cores too, each operand split exactly into three
- *     bf16 parts (error <= 1e-6 relative to sum |W||x|); other w use the FFMA kernels.
+ *     bf16 parts (error <= 1e-6 relative to sum |W||x|); other w use the FFMA kernels.  float32 NHWC
+ *     (C and H*W multiples of 4) takes the transposition route with temporaries from the library's pool, as above.
  *   - There is no CPU fallback.  Without a CUDA device of compute capability 10.x every compute
  *     entry point returns WBMM_STATUS_NO_DEVICE.
  */

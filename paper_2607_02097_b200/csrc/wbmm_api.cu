@@ -161,6 +161,27 @@ int apply(const wbmm_desc_t* d, const wbmm::Geom& g, const void* x, const void* 
             cudaGetLastError();      // no stream-ordered allocator / out of memory: in-kernel NHWC path below
         }
     }
+    if (g.layout == WBMM_LAYOUT_NHWC && d->dtype == WBMM_DTYPE_F32 && !(d->flags & (WBMM_FLAG_FORCE_SIMT | WBMM_FLAG_NO_SCRATCH)) &&
+        wbmm::transpose32_supported((long long)g.H * g.W, g.C, x, y)) {
+        // fp32 NHWC: the transposition route around the fp32 tensor-core kernel (the FFMA kernel is 3-5x slower)
+        wbmm::Geom gn = g;
+        gn.layout = WBMM_LAYOUT_NCHW;
+        void* const aligned16 = reinterpret_cast<void*>(256);
+        if (wbmm::tc_f32_supported(gn, aligned16, aligned16)) {
+            const size_t nbytes = (size_t)g.B * g.C * g.H * g.W * 4;
+            AsyncScratch xt(stream), yt(stream);
+            if (xt.alloc(nbytes) == cudaSuccess && yt.alloc(nbytes) == cudaSuccess) {
+                e = wbmm::transpose32(x, xt.p, g.B, g.H * g.W, g.C, stream, &launches);
+                if (e == cudaSuccess) e = wbmm::tc_f32_forward(gn, xt.p, T, yt.p, reverse, stream, &launches);
+                if (e == cudaSuccess) e = wbmm::transpose32(yt.p, y, g.B, g.C, g.H * g.W, stream, &launches);
+                g_launches += launches;
+                if (e != cudaSuccess) return set_cuda_error(e, "fp32 NHWC via NCHW scratch");
+                t_last_path = WBMM_PATH_TC_TRANSPOSED;
+                return WBMM_STATUS_OK;
+            }
+            cudaGetLastError();
+        }
+    }
     if (!(d->flags & WBMM_FLAG_FORCE_SIMT) && wbmm::tc_nhwc_supported(g, d->dtype, x, y)) {
         e = wbmm::tc_nhwc_forward(g, d->dtype, x, T, y, reverse, stream, &launches);
         g_launches += launches;
@@ -222,6 +243,27 @@ int grad_table_on(const wbmm_desc_t* desc, const wbmm::Geom& g, const void* x, c
                 if (e == cudaSuccess) e = wbmm::tc_grad_table(gn, desc->dtype, xt.p, gt.p, dT, stream, &launches, &path);
                 g_launches += launches;
                 if (e != cudaSuccess) return set_cuda_error(e, "NHWC dT via NCHW scratch");
+                t_last_path = WBMM_PATH_TC_TRANSPOSED;
+                done = true;
+            } else {
+                cudaGetLastError();
+            }
+        }
+    }
+    if (!done && g.layout == WBMM_LAYOUT_NHWC && desc->dtype == WBMM_DTYPE_F32 &&
+        !(desc->flags & (WBMM_FLAG_FORCE_SIMT | WBMM_FLAG_NO_SCRATCH)) && wbmm::transpose32_supported((long long)g.H * g.W, g.C, x, dy)) {
+        wbmm::Geom gn = g;
+        gn.layout = WBMM_LAYOUT_NCHW;
+        void* const aligned16 = reinterpret_cast<void*>(256);
+        if (wbmm::tc_f32_grad_table_supported(gn, aligned16, aligned16)) {
+            const size_t nbytes = (size_t)g.B * g.C * g.H * g.W * 4;
+            AsyncScratch xt(stream), gt(stream);
+            if (xt.alloc(nbytes) == cudaSuccess && gt.alloc(nbytes) == cudaSuccess) {
+                e = wbmm::transpose32(x, xt.p, g.B, g.H * g.W, g.C, stream, &launches);
+                if (e == cudaSuccess) e = wbmm::transpose32(dy, gt.p, g.B, g.H * g.W, g.C, stream, &launches);
+                if (e == cudaSuccess) e = wbmm::tc_f32_grad_table(gn, xt.p, gt.p, dT, stream, &launches);
+                g_launches += launches;
+                if (e != cudaSuccess) return set_cuda_error(e, "fp32 NHWC dT via NCHW scratch");
                 t_last_path = WBMM_PATH_TC_TRANSPOSED;
                 done = true;
             } else {

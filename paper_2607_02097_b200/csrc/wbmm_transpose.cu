@@ -45,7 +45,53 @@ __global__ void __launch_bounds__(256) transpose16_kernel(const uint16_t* __rest
     }
 }
 
+// The same for 32-bit elements (fp32 activations): 32 x 32 tiles, 16-byte global accesses both ways.
+__global__ void __launch_bounds__(256) transpose32_kernel(const uint32_t* __restrict__ in, uint32_t* __restrict__ out, int R, int Cc)
+{
+    __shared__ uint32_t tileT[32 * 33];      // [c][r]
+    const long long base = (long long)blockIdx.z * R * Cc;
+    const int r0 = blockIdx.y * 32, c0 = blockIdx.x * 32;
+    const int t = threadIdx.x;
+    {
+        const int r = t >> 3, ch = (t & 7) * 4;
+        if (r0 + r < R && c0 + ch < Cc) {
+            const uint4 v = __ldg(reinterpret_cast<const uint4*>(in + base + (long long)(r0 + r) * Cc + c0 + ch));
+            tileT[(ch + 0) * 33 + r] = v.x;
+            tileT[(ch + 1) * 33 + r] = v.y;
+            tileT[(ch + 2) * 33 + r] = v.z;
+            tileT[(ch + 3) * 33 + r] = v.w;
+        }
+    }
+    __syncthreads();
+    {
+        const int c = t >> 3, r4 = (t & 7) * 4;
+        if (c0 + c < Cc && r0 + r4 < R) {
+            const uint32_t* src = tileT + c * 33 + r4;
+            *reinterpret_cast<uint4*>(out + base + (long long)(c0 + c) * R + r0 + r4) = make_uint4(src[0], src[1], src[2], src[3]);
+        }
+    }
+}
+
 }  // namespace
+
+bool transpose32_supported(long long R, long long Cc, const void* in, const void* out)
+{
+    return R % 4 == 0 && Cc % 4 == 0 && R <= 0x7fffffff && Cc <= 0x7fffffff &&
+           reinterpret_cast<uintptr_t>(in) % 16 == 0 && reinterpret_cast<uintptr_t>(out) % 16 == 0;
+}
+
+cudaError_t transpose32(const void* in, void* out, int batch, int R, int Cc, cudaStream_t stream, int* launches)
+{
+    if (batch == 0 || R == 0 || Cc == 0) return cudaSuccess;
+    for (int b0 = 0; b0 < batch; b0 += 65535) {          // gridDim.z limit
+        const int nb = batch - b0 < 65535 ? batch - b0 : 65535;
+        dim3 grid((Cc + 31) / 32, (R + 31) / 32, nb);
+        const long long off = (long long)b0 * R * Cc;
+        transpose32_kernel<<<grid, 256, 0, stream>>>((const uint32_t*)in + off, (uint32_t*)out + off, R, Cc);
+        *launches += 1;
+    }
+    return cudaGetLastError();
+}
 
 bool transpose16_supported(long long R, long long Cc, const void* in, const void* out)
 {

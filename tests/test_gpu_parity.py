@@ -231,6 +231,29 @@ def test_backward_forks_the_table_gradient_and_joins(wb, oracle, case):
     assert max_err_over_tol(dx1, rdx, TOL[case.dtype]) <= 1.0
 
 
+@pytest.mark.parametrize("case", [
+    si.Case("f32_nhwc_w14", 6, 12, 56, 56, 14, dtype="f32", layout=NHWC, seed=150, backward=True),
+    si.Case("f32_nhwc_w14_shift_ragged", 5, 8, 30, 44, 14, dtype="f32", layout=NHWC, shift=(7, 5), seed=151, backward=True),
+    si.Case("f32_nhwc_w7", 9, 20, 28, 56, 7, dtype="f32", layout=NHWC, seed=152, backward=True),
+], ids=lambda c: c.name)
+def test_fp32_nhwc_through_the_transposition_route(wb, oracle, case):
+    """fp32 NHWC: 32-bit transposition passes around the fp32 tensor-core kernels (forward, dX, dT); with
+    WBMM_FLAG_NO_SCRATCH the FFMA kernels serve it.  Forward held to 1e-6 (the split is exact), dT to the sqrt(L*N) bound."""
+    d = si.make(case, device="cuda")
+    y = wb.wbmm_forward(d["x"], d["T"], case.w, case.shift, case.layout)
+    assert wb.wbmm_last_path() == wb.PATH_TC_TRANSPOSED, wb.wbmm_path_string(wb.wbmm_last_path())
+    dx, dT = wb.wbmm_backward(d["x"], d["T"], d["dy"], case.w, case.shift, case.layout)
+    assert wb.wbmm_last_path() == wb.PATH_TC_TRANSPOSED
+    y_simt = wb.wbmm_forward(d["x"], d["T"], case.w, case.shift, case.layout, wb.FLAG_NO_SCRATCH)
+    assert wb.wbmm_last_path() == wb.PATH_SIMT
+    torch.cuda.synchronize()
+    ry = oracle.forward(widen(d["x"]), widen(d["T"]), case.w, case.shift, case.layout)
+    rdx, rdT = oracle.backward(widen(d["x"]), widen(d["T"]), widen(d["dy"]), case.w, case.shift, case.layout)
+    assert max_err_over_tol(y, ry, 1e-6) <= 1.0 and max_err_over_tol(dx, rdx, 1e-6) <= 1.0
+    assert max_err_over_tol(y_simt, ry, 1e-4) <= 1.0
+    assert dT_err_over_tol(dT, rdT, case, 1e-4) <= 1.0
+
+
 @pytest.mark.parametrize("B,C,dtype", [(16, 8, "bf16"), (128, 40, "bf16"), (72, 24, "f16")])
 def test_one_window_7x7_planes_on_the_pipelined_kernel(wb, oracle, B, C, dtype):
     """7 x 7 maps at w = 7 (the S4 stage): the window is the plane, 49 contiguous elements that start
