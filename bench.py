@@ -364,6 +364,20 @@ def other_rooflines(wb, dev, stream, hbm_peak):
     del xs, gs, dxs, d
     torch.cuda.empty_cache()
 
+    fwd_row("fp32_nhwc_B128_C96_56x56_w14_fwd", si.with_(si.CFG3, dtype="f32", layout=si.NHWC), n=5)
+
+    # rectangular windows 7 x 14 (FFMA kernels, section 7.10 of DESIGN.md) on the config-2 shape: context
+    cr = si.CFG2
+    dr = si.make(cr, device=dev)
+    Tr = (torch.randn((cr.C, 13 * 27), generator=torch.Generator().manual_seed(93)) * 0.02).to(dr["x"].dtype).to(dev)
+    yr = torch.empty_like(dr["x"])
+    ms = region_ms_rot(lambda i: wb.wbmm_forward_rect(dr["x"], Tr, 7, 14, out=yr), 5, stream)
+    out["rect_7x14_B64_C96_56x56_fwd"] = {"ms": round(ms, 5), "tflops": round(2.0 * 98 * cr.n_elem / ms / 1e9, 2),
+                                         "frac": round(bytes_of(cr) / (hbm_peak * 1e9) * 1e3 / ms, 4),
+                                         "path": wb.wbmm_path_string(wb.wbmm_last_path())}
+    del dr, Tr, yr
+    torch.cuda.empty_cache()
+
     # table gradient at w = 7 (two CTAs per SM) on the config-2 shape
     c2 = si.with_(si.CFG2, backward=True)
     d = si.make(c2, device=dev)
