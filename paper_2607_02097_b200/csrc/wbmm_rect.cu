@@ -99,8 +99,8 @@ __global__ void __launch_bounds__(kThreadsR)
 rect_grad_table_kernel(RectGeom g, const E* __restrict__ x, const E* __restrict__ dy, float* __restrict__ dT, int G, int groups_per_block)
 {
     extern __shared__ __align__(16) float smem[];
-    float* xs = smem;                    // [G][N]
-    float* gs = smem + G * g.N;          // [G][N]
+    float* xs = smem;                    // [N][G]
+    float* gs = smem + G * g.N;          // [N][G]
     const int c = blockIdx.y;
     const long long ngroups = (g.nwin + G - 1) / G;
     const long long grp0 = (long long)blockIdx.x * groups_per_block;
@@ -118,10 +118,13 @@ rect_grad_table_kernel(RectGeom g, const E* __restrict__ x, const E* __restrict_
                 const long long off = rect_window_elem(g, grp * G + gw, p, c);
                 if (off >= 0) { xv = to_f32(x[off]); gv = to_f32(dy[off]); }      // dy is zero outside H x W (A11)
             }
-            xs[idx] = xv;
-            gs[idx] = gv;
+            xs[p * G + gw] = xv;          // position-major: four windows per 16-byte load (G is a multiple of 4)
+            gs[p * G + gw] = gv;
         }
         __syncthreads();
+        const int nq = G / 4;
+        const float4* x4 = reinterpret_cast<const float4*>(xs);
+        const float4* g4 = reinterpret_cast<const float4*>(gs);
 #pragma unroll
         for (int i = 0; i < kMaxOwn; ++i) {
             const int k = threadIdx.x + i * kThreadsR;
@@ -129,14 +132,17 @@ rect_grad_table_kernel(RectGeom g, const E* __restrict__ x, const E* __restrict_
             // bin k = (dr + w_h - 1)(2w_w - 1) + (dc + w_w - 1): pairs p = (rp, cp), q = (rp - dr, cp - dc) inside the window
             const int dr = k / g.tw - (g.wh - 1), dc = k % g.tw - (g.ww - 1);
             const int r0 = max(0, dr), r1 = min(g.wh, g.wh + dr), c0 = max(0, dc), c1 = min(g.ww, g.ww + dc);
-            float a = 0.f;
-            for (int gw = 0; gw < G; ++gw) {
-                const float* xw = xs + gw * g.N;
-                const float* gw_ = gs + gw * g.N;
-                for (int rp = r0; rp < r1; ++rp)
-                    for (int cp = c0; cp < c1; ++cp) a = fmaf(gw_[rp * g.ww + cp], xw[(rp - dr) * g.ww + cp - dc], a);
-            }
-            acc[i] += a;
+            float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
+            for (int rp = r0; rp < r1; ++rp)
+                for (int cp = c0; cp < c1; ++cp) {
+                    const float4* gp = g4 + (rp * g.ww + cp) * nq;
+                    const float4* xp = x4 + ((rp - dr) * g.ww + cp - dc) * nq;
+                    for (int q = 0; q < nq; ++q) {
+                        const float4 gv = gp[q], xv = xp[q];
+                        a0 = fmaf(gv.x, xv.x, a0); a1 = fmaf(gv.y, xv.y, a1); a2 = fmaf(gv.z, xv.z, a2); a3 = fmaf(gv.w, xv.w, a3);
+                    }
+                }
+            acc[i] += (a0 + a1) + (a2 + a3);
         }
     }
 #pragma unroll
@@ -160,7 +166,7 @@ RectGeom make_rect(const wbmm_desc_t& d, int ww)
     return g;
 }
 
-int rect_group(const RectGeom& g) { int G = (2048 / g.N) & ~3; return G < 4 ? 4 : (G > 32 ? 32 : G); }      // a multiple of 4
+int rect_group(const RectGeom& g, int budget = 2048) { int G = (budget / g.N) & ~3; return G < 4 ? 4 : (G > 32 ? 32 : G); }      // a multiple of 4
 
 template <typename E>
 cudaError_t rect_forward_t(const RectGeom& g, const E* x, const E* T, E* y, bool reverse, cudaStream_t s)
@@ -178,7 +184,7 @@ cudaError_t rect_forward_t(const RectGeom& g, const E* x, const E* T, E* y, bool
 template <typename E>
 cudaError_t rect_grad_table_t(const RectGeom& g, const E* x, const E* dy, float* dT, cudaStream_t s)
 {
-    const int G = rect_group(g);
+    const int G = rect_group(g, g.nb >= kThreadsR ? 2048 : 1024);      // few bins (1-D windows): smaller groups, more blocks
     const size_t smem = sizeof(float) * 2 * (size_t)G * g.N;
     auto k = rect_grad_table_kernel<E>;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
