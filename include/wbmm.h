@@ -170,9 +170,11 @@ WBMM_API int wbmm_backward_rect(const wbmm_desc_t *desc, int32_t w_w, const void
  *   Tg [in] C*(2w-1)^2, Tl [in] C*(w-1)^2 elements of desc->dtype.  x, y, padding, shift as wbmm_forward.
  *   transpose != 0 applies the transposed fused matrix: dX of the operator for dy in `x`.
  * Gradients: wbmm_hier_backward.
- * Supported where the pipelined tensor-core kernel is: w = 14, bf16/fp16, NCHW with 16-byte aligned planes
+ * Served by the pipelined tensor-core kernel where it applies: w = 14, bf16/fp16, NCHW with 16-byte aligned planes
  * (H*W even ... see wbmm_last_path), or NHWC through the transposition scratch (C and H*W multiples of 8, no
- * WBMM_FLAG_NO_SCRATCH); otherwise WBMM_STATUS_UNSUPPORTED.
+ * WBMM_FLAG_NO_SCRATCH).  Everything else (float32 -- the paper's precision --, other even w, WBMM_FLAG_FORCE_SIMT)
+ * runs on FFMA kernels that apply the same fused operator in one pass (wbmm_last_path() = WBMM_PATH_SIMT);
+ * w*w > 1024: WBMM_STATUS_UNSUPPORTED.
  */
 WBMM_API int wbmm_hier_forward(const wbmm_desc_t *desc, const void *x, const void *Tg, const void *Tl, void *y,
                       int transpose, void *cuda_stream);
@@ -187,9 +189,9 @@ WBMM_API int wbmm_hier_forward(const wbmm_desc_t *desc, const void *x, const voi
  *                       come from ONE pass over (x, dy): S = dY^T X is accumulated once in tensor memory and
  *                       folded onto both sets of bins.  Overwritten unless WBMM_FLAG_ACCUMULATE_DT.
  *   x may be NULL when the table gradients are not requested; Tg, Tl may be NULL when dx is NULL.
- * Padding, shift and the zero extension of dy as in wbmm_backward.  Supported where the pipelined
- * tensor-core kernels are (w = 14, bf16/fp16, NCHW with 16-byte aligned planes, or NHWC through the
- * transposition scratch); otherwise WBMM_STATUS_UNSUPPORTED, with nothing launched.
+ * Padding, shift and the zero extension of dy as in wbmm_backward.  Tensor-core kernels where wbmm_hier_forward
+ * uses them, FFMA kernels otherwise (the local-table gradient is then the table gradient of the (w/2)-window
+ * operator on the extent padded for the global window).
  */
 WBMM_API int wbmm_hier_backward(const wbmm_desc_t *desc, const void *x, const void *Tg, const void *Tl, const void *dy,
                        void *dx, float *dTg, float *dTl, void *cuda_stream);

@@ -205,10 +205,11 @@ def wbmm_backward_rect(x: Optional[torch.Tensor], T: Optional[torch.Tensor], dy:
 
 
 def wbmm_hier_forward(x: torch.Tensor, Tg: torch.Tensor, Tl: torch.Tensor, w: int, shift=(0, 0),
-                      layout: int = NCHW, transpose: bool = False, out: Optional[torch.Tensor] = None) -> torch.Tensor:
+                      layout: int = NCHW, transpose: bool = False, out: Optional[torch.Tensor] = None,
+                      flags: int = 0) -> torch.Tensor:
     """Fused hierarchical operator y = (M_g + diag_blocks(M_l) + 2I) x per w x w window
     (include/wbmm.h: wbmm_hier_forward); transpose=True gives dX for dy passed as x."""
-    d = make_desc(x, w, shift, layout, 0)
+    d = make_desc(x, w, shift, layout, flags)
     if Tg.dtype != x.dtype or Tl.dtype != x.dtype or tuple(Tg.shape) != (d.C, (2 * w - 1) ** 2) \
             or tuple(Tl.shape) != (d.C, (w - 1) ** 2):
         raise ValueError("Tg must be [C,(2w-1)^2] and Tl [C,(w-1)^2] in the dtype of x")

@@ -505,6 +505,18 @@ int wbmm_hier_forward(const wbmm_desc_t* desc, const void* x, const void* Tg, co
     if (device_state() < 0) return WBMM_STATUS_NO_DEVICE;
     wbmm::Geom g = wbmm::make_geom(*desc);
     int launches = 0, path = WBMM_PATH_NONE;
+    // what the tensor-core kernel does not take (fp32, w != 14, planes no copy scheme moves, NHWC without scratch): the
+    // FFMA kernel of wbmm_rect.cu, the same operator in one pass
+    auto ffma = [&]() -> int {
+        if (!wbmm::hier_simt_supported(*desc)) return WBMM_STATUS_UNSUPPORTED;
+        int l = 0;
+        cudaError_t e = wbmm::hier_simt_forward(*desc, x, Tg, Tl, y, transpose != 0, static_cast<cudaStream_t>(cuda_stream), &l);
+        g_launches += l;
+        if (e != cudaSuccess) return set_cuda_error(e, "hier_simt_forward");
+        t_last_path = WBMM_PATH_SIMT;
+        return WBMM_STATUS_OK;
+    };
+    if (desc->flags & WBMM_FLAG_FORCE_SIMT) return ffma();
     if (g.layout == WBMM_LAYOUT_NHWC) {
         // the transposition route of wbmm_forward around the same kernel
         cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
@@ -513,12 +525,12 @@ int wbmm_hier_forward(const wbmm_desc_t* desc, const void* x, const void* Tg, co
         void* const aligned16 = reinterpret_cast<void*>(256);
         if (!nhwc_scratch_candidate(desc, g) || !wbmm::tc_hier_supported(gn, desc->dtype, aligned16, aligned16) ||
             !wbmm::transpose16_supported((long long)g.H * g.W, g.C, x, y))
-            return WBMM_STATUS_UNSUPPORTED;
+            return ffma();
         const size_t nbytes = (size_t)g.B * g.C * g.H * g.W * 2;
         AsyncScratch xt(stream), yt(stream);
         if (xt.alloc(nbytes) != cudaSuccess || yt.alloc(nbytes) != cudaSuccess) {
             cudaGetLastError();
-            return WBMM_STATUS_UNSUPPORTED;
+            return ffma();
         }
         cudaError_t e = wbmm::transpose16(x, xt.p, g.B, g.H * g.W, g.C, stream, &launches);
         if (e == cudaSuccess) e = wbmm::tc_forward(gn, desc->dtype, xt.p, Tg, Tl, yt.p, transpose != 0, stream, &launches, &path);
@@ -528,7 +540,7 @@ int wbmm_hier_forward(const wbmm_desc_t* desc, const void* x, const void* Tg, co
         t_last_path = WBMM_PATH_TC_TRANSPOSED;
         return WBMM_STATUS_OK;
     }
-    if (!wbmm::tc_hier_supported(g, desc->dtype, x, y)) return WBMM_STATUS_UNSUPPORTED;
+    if (!wbmm::tc_hier_supported(g, desc->dtype, x, y)) return ffma();
     cudaError_t e = wbmm::tc_forward(g, desc->dtype, x, Tg, Tl, y, transpose != 0, static_cast<cudaStream_t>(cuda_stream),
                                      &launches, &path);
     g_launches += launches;
@@ -572,17 +584,30 @@ int wbmm_hier_backward(const wbmm_desc_t* desc, const void* x, const void* Tg, c
     wbmm::Geom gn = g;
     gn.layout = WBMM_LAYOUT_NCHW;
     void* const aligned16 = reinterpret_cast<void*>(256);
+    bool tc_ok = !(desc->flags & WBMM_FLAG_FORCE_SIMT);
     if (nhwc) {
-        if (!nhwc_scratch_candidate(desc, g)) return WBMM_STATUS_UNSUPPORTED;
+        if (!nhwc_scratch_candidate(desc, g)) tc_ok = false;
         if (dx && (!wbmm::tc_hier_supported(gn, desc->dtype, aligned16, aligned16) ||
                    !wbmm::transpose16_supported((long long)g.H * g.W, g.C, dy, dx)))
-            return WBMM_STATUS_UNSUPPORTED;
+            tc_ok = false;
         if (dTg && (g.w != 14 || !wbmm::tc_grad_table_supported(gn, desc->dtype, aligned16, aligned16) ||
                     !wbmm::transpose16_supported((long long)g.H * g.W, g.C, x, dy)))
-            return WBMM_STATUS_UNSUPPORTED;
+            tc_ok = false;
     } else {
-        if (dx && !wbmm::tc_hier_supported(g, desc->dtype, dy, dx)) return WBMM_STATUS_UNSUPPORTED;
-        if (dTg && (g.w != 14 || !wbmm::tc_grad_table_supported(g, desc->dtype, x, dy))) return WBMM_STATUS_UNSUPPORTED;
+        if (dx && !wbmm::tc_hier_supported(g, desc->dtype, dy, dx)) tc_ok = false;
+        if (dTg && (g.w != 14 || !wbmm::tc_grad_table_supported(g, desc->dtype, x, dy))) tc_ok = false;
+    }
+    if (!tc_ok) {
+        // the FFMA kernels of wbmm_rect.cu: dx = the transposed operator, both table gradients as windowed correlations
+        if (!wbmm::hier_simt_supported(*desc)) return WBMM_STATUS_UNSUPPORTED;
+        int l = 0;
+        cudaError_t e = cudaSuccess;
+        if (dx) e = wbmm::hier_simt_forward(*desc, dy, Tg, Tl, dx, true, stream, &l);
+        if (e == cudaSuccess && dTg) e = wbmm::hier_simt_grad_tables(*desc, x, dy, dTg, dTl, stream, &l);
+        g_launches += l;
+        if (e != cudaSuccess) return set_cuda_error(e, "hierarchical backward (FFMA)");
+        t_last_path = WBMM_PATH_SIMT;
+        return WBMM_STATUS_OK;
     }
     // both table gradients on `sdt` (dTg, dTl were cleared on the caller's stream above)
     auto table_gradients = [&](cudaStream_t sdt) -> int {

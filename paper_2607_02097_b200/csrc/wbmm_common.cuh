@@ -79,5 +79,11 @@ bool simt_supported(const Geom& g);
 bool rect_supported(const wbmm_desc_t& d, int ww);
 cudaError_t rect_forward(const wbmm_desc_t& d, int ww, const void* x, const void* T, void* y, bool reverse, cudaStream_t stream, int* launches);
 cudaError_t rect_grad_table(const wbmm_desc_t& d, int ww, const void* x, const void* dy, float* dT, cudaStream_t stream, int* launches);
+// Hierarchical operator on FFMA kernels (wbmm_rect.cu): any dtype / layout / shift / ragged size, w even.
+bool hier_simt_supported(const wbmm_desc_t& d);
+cudaError_t hier_simt_forward(const wbmm_desc_t& d, const void* x, const void* Tg, const void* Tl, void* y, bool transpose,
+                              cudaStream_t stream, int* launches);
+cudaError_t hier_simt_grad_tables(const wbmm_desc_t& d, const void* x, const void* dy, float* dTg, float* dTl, cudaStream_t stream,
+                                  int* launches);
 
 }  // namespace wbmm

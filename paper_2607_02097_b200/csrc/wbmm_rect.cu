@@ -42,9 +42,13 @@ __device__ __forceinline__ long long rect_window_elem(const RectGeom& g, long lo
     return rect_offset(g, b, c, h, v);
 }
 
-template <typename E>
+// HIER (square windows, w even): the hierarchical operator of PAPER.md:216-227 (Eq. 9) / Algorithm 2 in one pass,
+//     y_win = (M_g + diag_blocks(M_l) + 2 I) x_win,
+// M_l from the second table Tl [C][(w-1)^2] applied inside each of the 2 x 2 sub-windows of side w/2, 2 I = the two identity
+// shortcuts.  The FFMA fallback of wbmm_hier_forward for what the tensor-core kernel does not take (fp32, ...).
+template <typename E, bool HIER>
 __global__ void __launch_bounds__(kThreadsR)
-rect_forward_kernel(RectGeom g, const E* __restrict__ x, const E* __restrict__ T, E* __restrict__ y, int G, int reverse)
+rect_forward_kernel(RectGeom g, const E* __restrict__ x, const E* __restrict__ T, const E* __restrict__ Tl, E* __restrict__ y, int G, int reverse)
 {
     // G is a multiple of 4; windows are staged position-major, xs[q][G], so that a thread -- one output position of
     // FOUR windows -- reads the four inputs it needs with one 16-byte load (the same address for every thread of its
@@ -56,6 +60,12 @@ rect_forward_kernel(RectGeom g, const E* __restrict__ x, const E* __restrict__ T
     const long long win0 = (long long)blockIdx.x * G;
     for (int k = threadIdx.x; k < g.nb; k += kThreadsR)
         Ts[k] = to_f32(T[(long long)c * g.nb + (reverse ? g.nb - 1 - k : k)]);
+    const int wl = g.wh / 2, twl = 2 * wl - 1, nbl = twl * twl;      // HIER: the local table
+    float* Tls = Ts + g.nb;
+    if constexpr (HIER) {
+        for (int k = threadIdx.x; k < nbl; k += kThreadsR)
+            Tls[k] = to_f32(Tl[(long long)c * nbl + (reverse ? nbl - 1 - k : k)]);
+    }
     for (int idx = threadIdx.x; idx < G * g.N; idx += kThreadsR) {
         const int gw = idx / g.N, p = idx - gw * g.N;
         float val = 0.f;
@@ -78,7 +88,11 @@ rect_forward_kernel(RectGeom g, const E* __restrict__ x, const E* __restrict__ T
             const float* Trr = Tr - rq * g.tw;
             const float4* xr = xq + (long long)rq * g.ww * nq;
             for (int cq = 0; cq < g.ww; ++cq) {
-                const float t = Trr[-cq];
+                float t = Trr[-cq];
+                if constexpr (HIER) {
+                    if (rq / wl == r / wl && cq / wl == cc / wl) t += Tls[(r - rq + wl - 1) * twl + (cc - cq + wl - 1)];
+                    if (rq == r && cq == cc) t += 2.f;
+                }
                 const float4 v = xr[cq * nq];
                 a0 = fmaf(t, v.x, a0); a1 = fmaf(t, v.y, a1); a2 = fmaf(t, v.z, a2); a3 = fmaf(t, v.w, a3);
             }
@@ -152,13 +166,17 @@ rect_grad_table_kernel(RectGeom g, const E* __restrict__ x, const E* __restrict_
     }
 }
 
-RectGeom make_rect(const wbmm_desc_t& d, int ww)
+// pad_h, pad_w: the padded extents are multiples of these (default: of the window -- Eq. 4-5; the local sub-windows of the
+// hierarchical operator live on the extent padded for the GLOBAL window)
+RectGeom make_rect(const wbmm_desc_t& d, int ww, int wh = 0, int pad_h = 0, int pad_w = 0)
 {
     RectGeom g;
-    g.B = d.B; g.C = d.C; g.H = d.H; g.W = d.W; g.wh = d.w; g.ww = ww;
+    g.B = d.B; g.C = d.C; g.H = d.H; g.W = d.W; g.wh = wh ? wh : d.w; g.ww = ww;
     g.sh = d.shift_h; g.sw = d.shift_w; g.layout = d.layout;
-    g.Hp = (d.H + g.wh - 1) / g.wh * g.wh;
-    g.Wp = (d.W + g.ww - 1) / g.ww * g.ww;
+    if (pad_h == 0) pad_h = g.wh;
+    if (pad_w == 0) pad_w = g.ww;
+    g.Hp = (d.H + pad_h - 1) / pad_h * pad_h;
+    g.Wp = (d.W + pad_w - 1) / pad_w * pad_w;
     g.nwh = g.Hp / g.wh; g.nww = g.Wp / g.ww;
     g.N = g.wh * g.ww;
     g.tw = 2 * g.ww - 1; g.nb = (2 * g.wh - 1) * g.tw;
@@ -168,16 +186,17 @@ RectGeom make_rect(const wbmm_desc_t& d, int ww)
 
 int rect_group(const RectGeom& g, int budget = 2048) { int G = (budget / g.N) & ~3; return G < 4 ? 4 : (G > 32 ? 32 : G); }      // a multiple of 4
 
-template <typename E>
-cudaError_t rect_forward_t(const RectGeom& g, const E* x, const E* T, E* y, bool reverse, cudaStream_t s)
+template <typename E, bool HIER>
+cudaError_t rect_forward_t(const RectGeom& g, const E* x, const E* T, const E* Tl, E* y, bool reverse, cudaStream_t s)
 {
     const int G = rect_group(g);
-    const size_t smem = sizeof(float) * ((size_t)g.nb + (size_t)G * g.N);
-    auto k = rect_forward_kernel<E>;
+    const int nbl = (g.wh - 1) * (g.wh - 1);
+    const size_t smem = sizeof(float) * ((size_t)g.nb + (HIER ? nbl : 0) + (size_t)G * g.N);
+    auto k = rect_forward_kernel<E, HIER>;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     dim3 grid((unsigned)((g.nwin + G - 1) / G), (unsigned)g.C);
-    k<<<grid, kThreadsR, smem, s>>>(g, x, T, y, G, reverse ? 1 : 0);
+    k<<<grid, kThreadsR, smem, s>>>(g, x, T, Tl, y, G, reverse ? 1 : 0);
     return cudaGetLastError();
 }
 
@@ -218,9 +237,9 @@ cudaError_t rect_forward(const wbmm_desc_t& d, int ww, const void* x, const void
     if (g.nwin == 0 || g.C == 0) return cudaSuccess;
     *launches += 1;
     switch (d.dtype) {
-    case WBMM_DTYPE_F32: return rect_forward_t<float>(g, (const float*)x, (const float*)T, (float*)y, reverse, s);
-    case WBMM_DTYPE_BF16: return rect_forward_t<__nv_bfloat16>(g, (const __nv_bfloat16*)x, (const __nv_bfloat16*)T, (__nv_bfloat16*)y, reverse, s);
-    default: return rect_forward_t<__half>(g, (const __half*)x, (const __half*)T, (__half*)y, reverse, s);
+    case WBMM_DTYPE_F32: return rect_forward_t<float, false>(g, (const float*)x, (const float*)T, nullptr, (float*)y, reverse, s);
+    case WBMM_DTYPE_BF16: return rect_forward_t<__nv_bfloat16, false>(g, (const __nv_bfloat16*)x, (const __nv_bfloat16*)T, nullptr, (__nv_bfloat16*)y, reverse, s);
+    default: return rect_forward_t<__half, false>(g, (const __half*)x, (const __half*)T, nullptr, (__half*)y, reverse, s);
     }
 }
 
@@ -234,6 +253,41 @@ cudaError_t rect_grad_table(const wbmm_desc_t& d, int ww, const void* x, const v
     case WBMM_DTYPE_F32: return rect_grad_table_t<float>(g, (const float*)x, (const float*)dy, dT, s);
     case WBMM_DTYPE_BF16: return rect_grad_table_t<__nv_bfloat16>(g, (const __nv_bfloat16*)x, (const __nv_bfloat16*)dy, dT, s);
     default: return rect_grad_table_t<__half>(g, (const __half*)x, (const __half*)dy, dT, s);
+    }
+}
+
+// ---- hierarchical operator, FFMA fallback (wbmm_hier_forward / wbmm_hier_backward on what the tensor-core kernels do not take)
+bool hier_simt_supported(const wbmm_desc_t& d)
+{
+    return d.w >= 2 && d.w % 2 == 0 && rect_supported(d, d.w);
+}
+
+cudaError_t hier_simt_forward(const wbmm_desc_t& d, const void* x, const void* Tg, const void* Tl, void* y, bool transpose,
+                              cudaStream_t s, int* launches)
+{
+    const RectGeom g = make_rect(d, d.w);
+    if (g.nwin == 0 || g.C == 0) return cudaSuccess;
+    *launches += 1;
+    switch (d.dtype) {
+    case WBMM_DTYPE_F32: return rect_forward_t<float, true>(g, (const float*)x, (const float*)Tg, (const float*)Tl, (float*)y, transpose, s);
+    case WBMM_DTYPE_BF16: return rect_forward_t<__nv_bfloat16, true>(g, (const __nv_bfloat16*)x, (const __nv_bfloat16*)Tg, (const __nv_bfloat16*)Tl, (__nv_bfloat16*)y, transpose, s);
+    default: return rect_forward_t<__half, true>(g, (const __half*)x, (const __half*)Tg, (const __half*)Tl, (__half*)y, transpose, s);
+    }
+}
+
+// adds into dTg and dTl (the caller clears them).  dTl: the table gradient of the (w/2 x w/2)-window operator on the extent
+// padded for the GLOBAL window, with the same shift -- its windows are exactly the local sub-windows.
+cudaError_t hier_simt_grad_tables(const wbmm_desc_t& d, const void* x, const void* dy, float* dTg, float* dTl, cudaStream_t s, int* launches)
+{
+    cudaError_t e = rect_grad_table(d, d.w, x, dy, dTg, s, launches);
+    if (e != cudaSuccess) return e;
+    const RectGeom g = make_rect(d, d.w / 2, d.w / 2, d.w, d.w);
+    if (g.nwin == 0 || g.C == 0) return cudaSuccess;
+    *launches += 1;
+    switch (d.dtype) {
+    case WBMM_DTYPE_F32: return rect_grad_table_t<float>(g, (const float*)x, (const float*)dy, dTl, s);
+    case WBMM_DTYPE_BF16: return rect_grad_table_t<__nv_bfloat16>(g, (const __nv_bfloat16*)x, (const __nv_bfloat16*)dy, dTl, s);
+    default: return rect_grad_table_t<__half>(g, (const __half*)x, (const __half*)dy, dTl, s);
     }
 }
 

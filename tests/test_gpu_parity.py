@@ -611,6 +611,35 @@ def test_fused_unsupported_combinations_fail_loudly(wb):
         wb.wbmm_forward_fused(x.float(), T7.float(), 7, bias=torch.zeros(4, device="cuda"))
 
 
+@pytest.mark.parametrize("case,flags", [
+    (si.Case("hf_f32", 5, 6, 56, 56, 14, dtype="f32", seed=160, backward=True), 0),                      # the paper's precision
+    (si.Case("hf_f32_shift_ragged", 3, 4, 30, 44, 14, dtype="f32", shift=(9, 4), seed=161, backward=True), 0),
+    (si.Case("hf_f32_nhwc", 4, 5, 28, 42, 14, dtype="f32", layout=NHWC, shift=(7, 7), seed=162, backward=True), 0),
+    (si.Case("hf_bf16_forced", 6, 7, 28, 56, 14, shift=(7, 3), seed=163, backward=True), 2),             # WBMM_FLAG_FORCE_SIMT
+    (si.Case("hf_w8", 4, 3, 20, 24, 8, dtype="f32", shift=(5, 2), seed=164, backward=True), 0),          # w = 8: 4 x 4 sub-windows
+], ids=lambda v: v.name if hasattr(v, "name") else str(v))
+def test_hier_ffma_fallback_matches_oracle(wb, oracle, case, flags):
+    """The hierarchical operator where the tensor-core kernel does not apply (fp32, w != 14, forced): FFMA kernels
+    (csrc/wbmm_rect.cu) against the oracle's TRAINING form (Alg. 2) and its table gradients."""
+    d, Tl = _hier_case(case)
+    tol = TOL[case.dtype]
+    for transpose in (False, True):
+        y = wb.wbmm_hier_forward(d["x"], d["T"], Tl, case.w, case.shift, case.layout, transpose, flags=flags)
+        torch.cuda.synchronize()
+        assert wb.wbmm_last_path() == wb.PATH_SIMT
+        ref = oracle.hier_forward(widen(d["x"]), widen(d["T"]), widen(Tl), case.w, case.shift, case.layout, "train", transpose)
+        assert max_err_over_tol(y, ref, tol) <= 1.0
+    dx, dTg, dTl = wb.wbmm_hier_backward(d["x"], d["T"], Tl, d["dy"], case.w, case.shift, case.layout, flags)
+    torch.cuda.synchronize()
+    assert wb.wbmm_last_path() == wb.PATH_SIMT
+    rdx, rg, rl = oracle.hier_backward(widen(d["x"]), widen(d["T"]), widen(Tl), widen(d["dy"]), case.w, case.shift, case.layout)
+    assert max_err_over_tol(dx, rdx, tol) <= 1.0
+    if case.dtype == "f32":
+        assert dT_err_over_tol(dTg, rg, case, 1e-4) <= 1.0 and dT_err_over_tol(dTl, rl, case, 1e-4) <= 1.0
+    else:
+        assert max_err_over_tol(dTg, rg, tol) <= 1.0 and max_err_over_tol(dTl, rl, tol) <= 1.0
+
+
 def test_hier_unsupported_shapes_fail_loudly(wb):
     x = torch.zeros((2, 4, 14, 14), dtype=torch.bfloat16, device="cuda")
     with pytest.raises(wb.WbmmError):       # w = 7 has no hierarchical tensor-core path
