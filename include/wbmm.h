@@ -214,9 +214,10 @@ WBMM_API int wbmm_materialize_weight(const wbmm_desc_t *desc, const void *T, voi
  *            16 x 16 block identity * I of the w = 14 weight library (14 extra N = 16 MMAs per tile), never summed
  *            into the 16-bit table values.  w = 14 only.
  *   transpose != 0 applies W_c^T + identity * I (the dX of the fused operator for dy in `x`; pass bias = NULL).
- * Served by the pipelined tensor-core kernel only (bf16/fp16, w in {7, 14}, NCHW planes 16-byte aligned, or NHWC
- * through the transposition scratch); otherwise WBMM_STATUS_UNSUPPORTED with nothing launched -- the caller then
- * uses wbmm_forward and its own elementwise pass.
+ * Served by the pipelined tensor-core kernel where it applies (bf16/fp16, w in {7, 14} -- identity: w = 14 --, NCHW
+ * planes the copy schemes move, or NHWC through the transposition scratch); everything else (float32, identity at
+ * other w, other window sizes) by an FFMA kernel that applies the same fused operator in one pass
+ * (wbmm_last_path() = WBMM_PATH_SIMT); w*w > 1024: WBMM_STATUS_UNSUPPORTED.
  */
 WBMM_API int wbmm_forward_fused(const wbmm_desc_t *desc, const void *x, const void *T, const void *bias, float identity,
                        void *y, int transpose, void *cuda_stream);
@@ -233,7 +234,8 @@ WBMM_API int wbmm_forward_fused(const wbmm_desc_t *desc, const void *x, const vo
  * wbmm_forward's ("identical outputs") up to the fp32 summation order of the kernel that serves it
  * (at most one 16-bit ulp).  Served by the pipelined tensor-core kernels where wbmm_forward is (NCHW; the matrix takes
  * the place of the weights built from the table), else by the gather tensor-core kernel (w in {7, 14}, bf16/fp16, any
- * layout / shift / ragged size); otherwise WBMM_STATUS_UNSUPPORTED.  On this design the cached mode is NOT the fast
+ * layout / shift / ragged size), else (float32, other w with w*w <= 1024) by an FFMA kernel that reads M_c from
+ * global memory; otherwise WBMM_STATUS_UNSUPPORTED.  On this design the cached mode is NOT the fast
  * one: the table path rebuilds its weights in shared memory from 1.4 KB per channel while M costs 75 KB per channel
  * of HBM traffic and ~9 us per channel change at w = 14 -- it exists for matrices that are not table-generated.
  */

@@ -673,13 +673,24 @@ int wbmm_forward_fused(const wbmm_desc_t* desc, const void* x, const void* T, co
     const size_t es = elem_size(desc->dtype);
     if (!aligned(x, es) || !aligned(T, es) || !aligned(y, es) || (bias && !aligned(bias, es))) return WBMM_STATUS_MISALIGNED;
     if (device_state() < 0) return WBMM_STATUS_NO_DEVICE;
-    if (desc->dtype != WBMM_DTYPE_BF16 && desc->dtype != WBMM_DTYPE_F16) return WBMM_STATUS_UNSUPPORTED;
+    // identity rounded to the dtype, as the tensor-core path holds it
     uint32_t ident_bits = 0;
-    if (identity != 0.f) {
-        if (desc->w != 14) return WBMM_STATUS_UNSUPPORTED;            // the identity block exists in the w = 14 library only
-        if (desc->dtype == WBMM_DTYPE_BF16) { __nv_bfloat16 h = __float2bfloat16_rn(identity); memcpy(&ident_bits, &h, 2); }
-        else { __half h = __float2half_rn(identity); memcpy(&ident_bits, &h, 2); }
-    }
+    float ident_f = identity;
+    if (identity != 0.f && desc->dtype == WBMM_DTYPE_BF16) { __nv_bfloat16 h = __float2bfloat16_rn(identity); memcpy(&ident_bits, &h, 2); ident_f = __bfloat162float(h); }
+    if (identity != 0.f && desc->dtype == WBMM_DTYPE_F16) { __half h = __float2half_rn(identity); memcpy(&ident_bits, &h, 2); ident_f = __half2float(h); }
+    // what the pipelined kernel does not take (float32, identity at w != 14, planes no copy scheme moves, NHWC without
+    // scratch): the FFMA kernel of wbmm_rect.cu, same operator, one pass
+    auto ffma = [&]() -> int {
+        if (!wbmm::rect_supported(*desc, desc->w)) return WBMM_STATUS_UNSUPPORTED;
+        int l = 0;
+        cudaError_t e2 = wbmm::fused_simt_forward(*desc, x, T, bias, ident_f, y, transpose != 0, static_cast<cudaStream_t>(cuda_stream), &l);
+        g_launches += l;
+        if (e2 != cudaSuccess) return set_cuda_error(e2, "fused_simt_forward");
+        t_last_path = WBMM_PATH_SIMT;
+        return WBMM_STATUS_OK;
+    };
+    if ((desc->flags & WBMM_FLAG_FORCE_SIMT) || (desc->dtype != WBMM_DTYPE_BF16 && desc->dtype != WBMM_DTYPE_F16)) return ffma();
+    if (identity != 0.f && desc->w != 14) return ffma();              // the identity block exists in the w = 14 library only
     wbmm::Geom g = wbmm::make_geom(*desc);
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     int launches = 0, path = WBMM_PATH_NONE;
@@ -691,12 +702,12 @@ int wbmm_forward_fused(const wbmm_desc_t* desc, const void* x, const void* T, co
         void* const aligned16 = reinterpret_cast<void*>(256);
         if (!nhwc_scratch_candidate(desc, g) || !wbmm::tc_bulk_supported(gn, desc->dtype, aligned16, aligned16) ||
             !wbmm::transpose16_supported((long long)g.H * g.W, g.C, x, y))
-            return WBMM_STATUS_UNSUPPORTED;
+            return ffma();
         const size_t nbytes = (size_t)g.B * g.C * g.H * g.W * 2;
         AsyncScratch xt(stream), yt(stream);
         if (xt.alloc(nbytes) != cudaSuccess || yt.alloc(nbytes) != cudaSuccess) {
             cudaGetLastError();
-            return WBMM_STATUS_UNSUPPORTED;
+            return ffma();
         }
         e = wbmm::transpose16(x, xt.p, g.B, g.H * g.W, g.C, stream, &launches);
         if (e == cudaSuccess)
@@ -707,7 +718,7 @@ int wbmm_forward_fused(const wbmm_desc_t* desc, const void* x, const void* T, co
         t_last_path = WBMM_PATH_TC_TRANSPOSED;
         return WBMM_STATUS_OK;
     }
-    if (!wbmm::tc_bulk_supported(g, desc->dtype, x, y)) return WBMM_STATUS_UNSUPPORTED;
+    if (!wbmm::tc_bulk_supported(g, desc->dtype, x, y)) return ffma();
     e = wbmm::tc_forward(g, desc->dtype, x, T, nullptr, y, transpose != 0, stream, &launches, &path, bias, ident_bits);
     g_launches += launches;
     if (e != cudaSuccess) return set_cuda_error(e, "tc_forward (fused)");
@@ -726,7 +737,16 @@ int wbmm_forward_matrix(const wbmm_desc_t* desc, const void* x, const void* M, c
     if (!aligned(x, es) || !aligned(M, es) || !aligned(y, es) || (bias && !aligned(bias, es))) return WBMM_STATUS_MISALIGNED;
     if (device_state() < 0) return WBMM_STATUS_NO_DEVICE;
     wbmm::Geom g = wbmm::make_geom(*desc);
-    if (!wbmm::tc_forward_supported(g, desc->dtype, x, y)) return WBMM_STATUS_UNSUPPORTED;
+    if ((desc->flags & WBMM_FLAG_FORCE_SIMT) || !wbmm::tc_forward_supported(g, desc->dtype, x, y)) {
+        // float32, window sizes without a tensor-core kernel: the FFMA kernel of wbmm_rect.cu reads M_c from global memory
+        if (!wbmm::rect_supported(*desc, desc->w)) return WBMM_STATUS_UNSUPPORTED;
+        int l = 0;
+        cudaError_t e2 = wbmm::matrix_simt_forward(*desc, x, M, bias, y, transpose != 0, static_cast<cudaStream_t>(cuda_stream), &l);
+        g_launches += l;
+        if (e2 != cudaSuccess) return set_cuda_error(e2, "matrix_simt_forward");
+        t_last_path = WBMM_PATH_SIMT;
+        return WBMM_STATUS_OK;
+    }
     int launches = 0, path = WBMM_PATH_NONE;
     cudaError_t e = wbmm::tc_forward_matrix(g, desc->dtype, x, M, bias, y, transpose != 0,
                                             static_cast<cudaStream_t>(cuda_stream), &launches, &path);

@@ -80,6 +80,10 @@ bool rect_supported(const wbmm_desc_t& d, int ww);
 cudaError_t rect_forward(const wbmm_desc_t& d, int ww, const void* x, const void* T, void* y, bool reverse, cudaStream_t stream, int* launches);
 cudaError_t rect_grad_table(const wbmm_desc_t& d, int ww, const void* x, const void* dy, float* dT, cudaStream_t stream, int* launches);
 // Hierarchical operator on FFMA kernels (wbmm_rect.cu): any dtype / layout / shift / ragged size, w even.
+cudaError_t fused_simt_forward(const wbmm_desc_t& d, const void* x, const void* T, const void* bias, float ident, void* y, bool transpose,
+                               cudaStream_t stream, int* launches);
+cudaError_t matrix_simt_forward(const wbmm_desc_t& d, const void* x, const void* M, const void* bias, void* y, bool transpose,
+                                cudaStream_t stream, int* launches);
 bool hier_simt_supported(const wbmm_desc_t& d);
 cudaError_t hier_simt_forward(const wbmm_desc_t& d, const void* x, const void* Tg, const void* Tl, void* y, bool transpose,
                               cudaStream_t stream, int* launches);

@@ -46,10 +46,18 @@ __device__ __forceinline__ long long rect_window_elem(const RectGeom& g, long lo
 //     y_win = (M_g + diag_blocks(M_l) + 2 I) x_win,
 // M_l from the second table Tl [C][(w-1)^2] applied inside each of the 2 x 2 sub-windows of side w/2, 2 I = the two identity
 // shortcuts.  The FFMA fallback of wbmm_hier_forward for what the tensor-core kernel does not take (fp32, ...).
-template <typename E, bool HIER>
+// MODE 0: the operator from the table.  1 (HIER): see above.  2 (fused, square windows): y = W_c x + ident * x + bias_c --
+// wbmm_forward_fused where the pipelined kernel does not apply; `Tl` carries the bias [C] (nullable).  3 (cached-M,
+// PAPER.md:208-210): the GIVEN matrices M [C][N][N] in `T` (reverse = apply M_c^T), bias in `Tl` -- wbmm_forward_matrix
+// for float32 and for window sizes without a tensor-core kernel.
+enum { kModeTable = 0, kModeHier = 1, kModeFused = 2, kModeMatrix = 3 };
+
+template <typename E, int MODE>
 __global__ void __launch_bounds__(kThreadsR)
-rect_forward_kernel(RectGeom g, const E* __restrict__ x, const E* __restrict__ T, const E* __restrict__ Tl, E* __restrict__ y, int G, int reverse)
+rect_forward_kernel(RectGeom g, const E* __restrict__ x, const E* __restrict__ T, const E* __restrict__ Tl, E* __restrict__ y, int G, int reverse,
+                    float ident)
 {
+    constexpr bool HIER = MODE == kModeHier;
     // G is a multiple of 4; windows are staged position-major, xs[q][G], so that a thread -- one output position of
     // FOUR windows -- reads the four inputs it needs with one 16-byte load (the same address for every thread of its
     // window quad: a broadcast) and one table entry per input position: 2 shared-memory loads per 4 FFMA.
@@ -58,8 +66,10 @@ rect_forward_kernel(RectGeom g, const E* __restrict__ x, const E* __restrict__ T
     float* Ts = smem + g.N * G;          // [nb]
     const int c = blockIdx.y;
     const long long win0 = (long long)blockIdx.x * G;
-    for (int k = threadIdx.x; k < g.nb; k += kThreadsR)
-        Ts[k] = to_f32(T[(long long)c * g.nb + (reverse ? g.nb - 1 - k : k)]);
+    if constexpr (MODE != kModeMatrix) {
+        for (int k = threadIdx.x; k < g.nb; k += kThreadsR)
+            Ts[k] = to_f32(T[(long long)c * g.nb + (reverse ? g.nb - 1 - k : k)]);
+    }
     const int wl = g.wh / 2, twl = 2 * wl - 1, nbl = twl * twl;      // HIER: the local table
     float* Tls = Ts + g.nb;
     if constexpr (HIER) {
@@ -84,11 +94,21 @@ rect_forward_kernel(RectGeom g, const E* __restrict__ x, const E* __restrict__ T
         const float* Tr = Ts + (r + g.wh - 1) * g.tw + cc + g.ww - 1;
         const float4* xq = reinterpret_cast<const float4*>(xs) + gq;
         float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
+        const E* Mc = T + (long long)c * g.N * g.N;                 // MODE 3: this channel's matrix
         for (int rq = 0; rq < g.wh; ++rq) {
             const float* Trr = Tr - rq * g.tw;
             const float4* xr = xq + (long long)rq * g.ww * nq;
             for (int cq = 0; cq < g.ww; ++cq) {
-                float t = Trr[-cq];
+                float t;
+                if constexpr (MODE == kModeMatrix) {
+                    const int q = rq * g.ww + cq;
+                    t = to_f32(reverse ? Mc[(long long)q * g.N + p] : Mc[(long long)p * g.N + q]);
+                } else {
+                    t = Trr[-cq];
+                }
+                if constexpr (MODE == kModeFused) {
+                    if (rq == r && cq == cc) t += ident;
+                }
                 if constexpr (HIER) {
                     if (rq / wl == r / wl && cq / wl == cc / wl) t += Tls[(r - rq + wl - 1) * twl + (cc - cq + wl - 1)];
                     if (rq == r && cq == cc) t += 2.f;
@@ -97,7 +117,11 @@ rect_forward_kernel(RectGeom g, const E* __restrict__ x, const E* __restrict__ T
                 a0 = fmaf(t, v.x, a0); a1 = fmaf(t, v.y, a1); a2 = fmaf(t, v.z, a2); a3 = fmaf(t, v.w, a3);
             }
         }
-        const float acc[4] = {a0, a1, a2, a3};
+        float bc = 0.f;
+        if constexpr (MODE == kModeFused || MODE == kModeMatrix) {
+            if (Tl) bc = to_f32(Tl[c]);
+        }
+        const float acc[4] = {a0 + bc, a1 + bc, a2 + bc, a3 + bc};
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
             const long long win = win0 + gq * 4 + u;
@@ -186,17 +210,17 @@ RectGeom make_rect(const wbmm_desc_t& d, int ww, int wh = 0, int pad_h = 0, int 
 
 int rect_group(const RectGeom& g, int budget = 2048) { int G = (budget / g.N) & ~3; return G < 4 ? 4 : (G > 32 ? 32 : G); }      // a multiple of 4
 
-template <typename E, bool HIER>
-cudaError_t rect_forward_t(const RectGeom& g, const E* x, const E* T, const E* Tl, E* y, bool reverse, cudaStream_t s)
+template <typename E, int MODE>
+cudaError_t rect_forward_t(const RectGeom& g, const E* x, const E* T, const E* Tl, E* y, bool reverse, cudaStream_t s, float ident = 0.f)
 {
     const int G = rect_group(g);
     const int nbl = (g.wh - 1) * (g.wh - 1);
-    const size_t smem = sizeof(float) * ((size_t)g.nb + (HIER ? nbl : 0) + (size_t)G * g.N);
-    auto k = rect_forward_kernel<E, HIER>;
+    const size_t smem = sizeof(float) * ((size_t)g.nb + (MODE == kModeHier ? nbl : 0) + (size_t)G * g.N);
+    auto k = rect_forward_kernel<E, MODE>;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     dim3 grid((unsigned)((g.nwin + G - 1) / G), (unsigned)g.C);
-    k<<<grid, kThreadsR, smem, s>>>(g, x, T, Tl, y, G, reverse ? 1 : 0);
+    k<<<grid, kThreadsR, smem, s>>>(g, x, T, Tl, y, G, reverse ? 1 : 0, ident);
     return cudaGetLastError();
 }
 
@@ -237,9 +261,9 @@ cudaError_t rect_forward(const wbmm_desc_t& d, int ww, const void* x, const void
     if (g.nwin == 0 || g.C == 0) return cudaSuccess;
     *launches += 1;
     switch (d.dtype) {
-    case WBMM_DTYPE_F32: return rect_forward_t<float, false>(g, (const float*)x, (const float*)T, nullptr, (float*)y, reverse, s);
-    case WBMM_DTYPE_BF16: return rect_forward_t<__nv_bfloat16, false>(g, (const __nv_bfloat16*)x, (const __nv_bfloat16*)T, nullptr, (__nv_bfloat16*)y, reverse, s);
-    default: return rect_forward_t<__half, false>(g, (const __half*)x, (const __half*)T, nullptr, (__half*)y, reverse, s);
+    case WBMM_DTYPE_F32: return rect_forward_t<float, kModeTable>(g, (const float*)x, (const float*)T, nullptr, (float*)y, reverse, s);
+    case WBMM_DTYPE_BF16: return rect_forward_t<__nv_bfloat16, kModeTable>(g, (const __nv_bfloat16*)x, (const __nv_bfloat16*)T, nullptr, (__nv_bfloat16*)y, reverse, s);
+    default: return rect_forward_t<__half, kModeTable>(g, (const __half*)x, (const __half*)T, nullptr, (__half*)y, reverse, s);
     }
 }
 
@@ -269,9 +293,9 @@ cudaError_t hier_simt_forward(const wbmm_desc_t& d, const void* x, const void* T
     if (g.nwin == 0 || g.C == 0) return cudaSuccess;
     *launches += 1;
     switch (d.dtype) {
-    case WBMM_DTYPE_F32: return rect_forward_t<float, true>(g, (const float*)x, (const float*)Tg, (const float*)Tl, (float*)y, transpose, s);
-    case WBMM_DTYPE_BF16: return rect_forward_t<__nv_bfloat16, true>(g, (const __nv_bfloat16*)x, (const __nv_bfloat16*)Tg, (const __nv_bfloat16*)Tl, (__nv_bfloat16*)y, transpose, s);
-    default: return rect_forward_t<__half, true>(g, (const __half*)x, (const __half*)Tg, (const __half*)Tl, (__half*)y, transpose, s);
+    case WBMM_DTYPE_F32: return rect_forward_t<float, kModeHier>(g, (const float*)x, (const float*)Tg, (const float*)Tl, (float*)y, transpose, s);
+    case WBMM_DTYPE_BF16: return rect_forward_t<__nv_bfloat16, kModeHier>(g, (const __nv_bfloat16*)x, (const __nv_bfloat16*)Tg, (const __nv_bfloat16*)Tl, (__nv_bfloat16*)y, transpose, s);
+    default: return rect_forward_t<__half, kModeHier>(g, (const __half*)x, (const __half*)Tg, (const __half*)Tl, (__half*)y, transpose, s);
     }
 }
 
@@ -289,6 +313,33 @@ cudaError_t hier_simt_grad_tables(const wbmm_desc_t& d, const void* x, const voi
     case WBMM_DTYPE_BF16: return rect_grad_table_t<__nv_bfloat16>(g, (const __nv_bfloat16*)x, (const __nv_bfloat16*)dy, dTl, s);
     default: return rect_grad_table_t<__half>(g, (const __half*)x, (const __half*)dy, dTl, s);
     }
+}
+
+// ---- wbmm_forward_fused / wbmm_forward_matrix on FFMA kernels (square windows; what the tensor-core kernels do not take)
+template <int MODE>
+static cudaError_t square_mode_forward(const wbmm_desc_t& d, const void* x, const void* T, const void* bias, void* y, bool transpose,
+                                       float ident, cudaStream_t s, int* launches)
+{
+    const RectGeom g = make_rect(d, d.w);
+    if (g.nwin == 0 || g.C == 0) return cudaSuccess;
+    *launches += 1;
+    switch (d.dtype) {
+    case WBMM_DTYPE_F32: return rect_forward_t<float, MODE>(g, (const float*)x, (const float*)T, (const float*)bias, (float*)y, transpose, s, ident);
+    case WBMM_DTYPE_BF16: return rect_forward_t<__nv_bfloat16, MODE>(g, (const __nv_bfloat16*)x, (const __nv_bfloat16*)T, (const __nv_bfloat16*)bias, (__nv_bfloat16*)y, transpose, s, ident);
+    default: return rect_forward_t<__half, MODE>(g, (const __half*)x, (const __half*)T, (const __half*)bias, (__half*)y, transpose, s, ident);
+    }
+}
+
+cudaError_t fused_simt_forward(const wbmm_desc_t& d, const void* x, const void* T, const void* bias, float ident, void* y, bool transpose,
+                               cudaStream_t s, int* launches)
+{
+    return square_mode_forward<kModeFused>(d, x, T, bias, y, transpose, ident, s, launches);
+}
+
+cudaError_t matrix_simt_forward(const wbmm_desc_t& d, const void* x, const void* M, const void* bias, void* y, bool transpose,
+                                cudaStream_t s, int* launches)
+{
+    return square_mode_forward<kModeMatrix>(d, x, M, bias, y, transpose, 0.f, s, launches);
 }
 
 }  // namespace wbmm

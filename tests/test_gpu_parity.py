@@ -602,13 +602,38 @@ def test_fused_bias_exact_with_zero_table(wb):
     assert torch.equal(y7, bias.view(1, -1, 1, 1).expand_as(d["x"]).contiguous())
 
 
-def test_fused_unsupported_combinations_fail_loudly(wb):
-    x = torch.zeros((2, 4, 14, 14), dtype=torch.bfloat16, device="cuda")
-    T7 = torch.zeros((4, 169), dtype=torch.bfloat16, device="cuda")
-    with pytest.raises(wb.WbmmError):       # the identity block exists in the w = 14 library only
-        wb.wbmm_forward_fused(x, T7, 7, identity=1.0)
-    with pytest.raises(wb.WbmmError):       # fp32 has no pipelined kernel
-        wb.wbmm_forward_fused(x.float(), T7.float(), 7, bias=torch.zeros(4, device="cuda"))
+@pytest.mark.parametrize("case,identity", [
+    (si.Case("ff_f32_w14", 5, 6, 56, 56, 14, dtype="f32", seed=170), 1.0),                      # float32: no pipelined fused kernel
+    (si.Case("ff_f32_w7_shift", 7, 5, 28, 42, 7, dtype="f32", shift=(3, 2), seed=171), 2.0),
+    (si.Case("ff_bf16_w7_identity", 9, 6, 28, 28, 7, seed=172), 1.0),                           # identity at w = 7
+    (si.Case("ff_f16_w5_nhwc", 4, 8, 22, 31, 5, dtype="f16", layout=NHWC, shift=(1, 4), seed=173), 0.5),
+], ids=lambda v: v.name if hasattr(v, "name") else str(v))
+def test_fused_and_cached_matrix_on_the_ffma_kernels(wb, oracle, case, identity):
+    """wbmm_forward_fused and wbmm_forward_matrix where no tensor-core kernel applies (float32, identity at w != 14, other
+    window sizes): FFMA kernels (csrc/wbmm_rect.cu) against the oracle's Algorithm 1 with M = R[:, I] + identity I and a
+    bias; then the same matrix GIVEN (cached-M mode), forward and transposed."""
+    d = si.make(case, device="cuda")
+    td = d["x"].dtype
+    g = torch.Generator().manual_seed(case.seed)
+    bias = torch.randn((case.C,), generator=g).to(td).cuda()
+    N = case.w * case.w
+    Mref = oracle.weight_matrix(widen(d["T"]), case.w) + float(torch.tensor(identity).to(td)) * np.eye(N)[None]
+    tol = TOL[case.dtype]
+    y = wb.wbmm_forward_fused(d["x"], d["T"], case.w, case.shift, case.layout, bias=bias, identity=identity)
+    assert wb.wbmm_last_path() == wb.PATH_SIMT
+    ref = oracle.apply_matrix(widen(d["x"]), Mref, case.w, case.shift, case.layout, False, widen(bias))
+    assert max_err_over_tol(y, ref, tol) <= 1.0
+    yt = wb.wbmm_forward_fused(d["x"], d["T"], case.w, case.shift, case.layout, identity=identity, transpose=True)
+    reft = oracle.apply_matrix(widen(d["x"]), Mref, case.w, case.shift, case.layout, True)
+    assert max_err_over_tol(yt, reft, tol) <= 1.0
+    if case.dtype == "f32" or case.w not in (7, 14):
+        gm = torch.Generator().manual_seed(case.seed + 1)
+        M = (torch.randn((case.C, N, N), generator=gm) * 0.05).to(td).cuda()
+        for transpose in (False, True):
+            ym = wb.wbmm_forward_matrix(d["x"], M, case.w, case.shift, case.layout, bias, transpose)
+            assert wb.wbmm_last_path() == wb.PATH_SIMT
+            refm = oracle.apply_matrix(widen(d["x"]), widen(M), case.w, case.shift, case.layout, transpose, widen(bias))
+            assert max_err_over_tol(ym, refm, tol) <= 1.0
 
 
 @pytest.mark.parametrize("case,flags", [
