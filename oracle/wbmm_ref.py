@@ -30,7 +30,7 @@ def build(force: bool = False) -> str:
     stale = (not os.path.exists(_LIB)) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC)
     if force or stale:
         cmd = ["gcc", "-O2", "-std=c99", "-fopenmp", "-fPIC", "-shared", "-Wall", "-Wextra",
-               "-o", _LIB, _SRC]
+               "-o", _LIB, _SRC, "-lm"]
         if _SANITIZE:
             cmd[1:2] = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"]
         subprocess.run(cmd, check=True)
@@ -61,6 +61,8 @@ def _load():
     lib.wbmm_ref_backward_rect.argtypes = [i] * 9 + [dp, dp, dp, dp, dp]
     lib.wbmm_ref_backward.restype = i
     lib.wbmm_ref_backward.argtypes = [i] * 8 + [dp, dp, dp, dp, dp]
+    lib.wbmm_ref_forward_int8.argtypes = [i] * 8 + [ctypes.c_void_p] * 5
+    lib.wbmm_ref_forward_int8.restype = i
     lib.wbmm_ref_hier_forward_train.restype = i
     lib.wbmm_ref_hier_forward_train.argtypes = [i] * 9 + [dp, dp, dp, dp]
     lib.wbmm_ref_hier_forward_fused.restype = i
@@ -161,6 +163,28 @@ def forward_rect(x, T, wh, ww, shift=(0, 0), layout=NCHW) -> np.ndarray:
     y = np.zeros_like(x)
     rc = _load().wbmm_ref_forward_rect(B, C, H, W, wh, ww, int(shift[0]), int(shift[1]), layout, xp, tp,
                                        y.ctypes.data_as(ctypes.POINTER(ctypes.c_double)))
+    if rc != 0:
+        raise ValueError(f"oracle rejected arguments (rc={rc})")
+    return y
+
+
+def forward_int8(x, T, w, shift=(0, 0), layout=NCHW, scale=None) -> np.ndarray:
+    """INT8 forward (NEXT-4): x, T int8, exact integer sums.  scale None: the int32 sums; scale [C]
+    float32: int8 values sat_s8(rne(fp32(sum) * scale[c])) (reading A21)."""
+    x = np.ascontiguousarray(x, dtype=np.int8)
+    T = np.ascontiguousarray(T, dtype=np.int8)
+    B, C, H, W = _dims(x, layout)
+    assert T.shape == (C, (2 * w - 1) ** 2), (T.shape, C, w)
+    if scale is None:
+        y = np.zeros(x.shape, dtype=np.int32)
+        rc = _load().wbmm_ref_forward_int8(B, C, H, W, w, int(shift[0]), int(shift[1]), layout, x.ctypes.data,
+                                           T.ctypes.data, None, y.ctypes.data, None)
+    else:
+        scale = np.ascontiguousarray(scale, dtype=np.float32)
+        assert scale.shape == (C,) and np.isfinite(scale).all()
+        y = np.zeros(x.shape, dtype=np.int8)
+        rc = _load().wbmm_ref_forward_int8(B, C, H, W, w, int(shift[0]), int(shift[1]), layout, x.ctypes.data,
+                                           T.ctypes.data, scale.ctypes.data, None, y.ctypes.data)
     if rc != 0:
         raise ValueError(f"oracle rejected arguments (rc={rc})")
     return y

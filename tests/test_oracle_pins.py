@@ -692,3 +692,95 @@ def test_rect_one_dimensional_windows(oracle):
         for vq in range(v0, v0 + ww):
             ref[:, :, :, v] += T[None, :, None, v - vq + ww - 1] * x[:, :, :, vq]
     assert np.allclose(y, ref, rtol=0, atol=1e-12)
+
+
+# ----------------------------------------------------------------------------- NEXT-4: INT8 forward
+def _int8_brute(x, T, w, s, scale=None):
+    """Pure-Python restatement of Alg. 1 on integers (NCHW): pad, roll by -s, windows, W_c[i,j] = T[rel(i,j)], roll back."""
+    B, C, H, W = x.shape
+    Hp, Wp = -(-H // w) * w, -(-W // w) * w
+    tw = 2 * w - 1
+    xp = np.zeros((B, C, Hp, Wp), dtype=np.int64)
+    xp[:, :, :H, :W] = x
+    xh = np.roll(xp, (-s[0], -s[1]), axis=(2, 3))
+    yh = np.zeros_like(xh)
+    for b in range(B):
+        for c in range(C):
+            for h0 in range(0, Hp, w):
+                for v0 in range(0, Wp, w):
+                    for i in range(w * w):
+                        acc = 0
+                        for j in range(w * w):
+                            k = (i // w - j // w + w - 1) * tw + (i % w - j % w + w - 1)
+                            acc += int(T[c, k]) * int(xh[b, c, h0 + j // w, v0 + j % w])
+                        yh[b, c, h0 + i // w, v0 + i % w] = acc
+    y = np.roll(yh, (s[0], s[1]), axis=(2, 3))[:, :, :H, :W]
+    if scale is None:
+        return y
+    q = np.rint(y.astype(np.float32) * scale.astype(np.float32)[None, :, None, None])
+    return np.clip(q, -128, 127).astype(np.int8)
+
+
+@pytest.mark.parametrize("w,H,W,s", [(2, 4, 4, (0, 0)), (3, 7, 8, (1, 2)), (4, 9, 6, (3, 0))])
+def test_int8_forward_is_the_brute_force_sum(oracle, w, H, W, s):
+    """Catches: a wrong bin index, padding treated as non-zero, shift direction, sign extension of the 8-bit values."""
+    r = rng(700 + w)
+    x = r.integers(-128, 128, (2, 3, H, W), dtype=np.int8)
+    T = r.integers(-128, 128, (3, (2 * w - 1) ** 2), dtype=np.int8)
+    want = _int8_brute(x, T, w, s)
+    assert np.array_equal(oracle.forward_int8(x, T, w, s).astype(np.int64), want)
+    xn = np.ascontiguousarray(x.transpose(0, 2, 3, 1))
+    got = oracle.forward_int8(xn, T, w, s, layout=NHWC).transpose(0, 3, 1, 2)
+    assert np.array_equal(got.astype(np.int64), want)
+
+
+@pytest.mark.parametrize("w,H,W,s,layout", [(7, 16, 20, (3, 5), NCHW), (14, 28, 30, (7, 2), NHWC), (5, 10, 10, (0, 0), NCHW)])
+def test_int8_forward_equals_the_float64_operator_on_integers(oracle, w, H, W, s, layout):
+    """Integer inputs are exact in float64 (|sum| < 2^53): the pinned float64 forward gives the same numbers.
+    Catches: any disagreement between the 8-bit routine and the operator pinned above (extreme values included)."""
+    r = rng(710 + w)
+    shape = (2, 4, H, W) if layout == NCHW else (2, H, W, 4)
+    x = r.integers(-128, 128, shape, dtype=np.int8)
+    T = r.integers(-128, 128, (4, (2 * w - 1) ** 2), dtype=np.int8)
+    x.flat[:7] = -128
+    T[0, :] = -128                                    # the largest products: (-128) * (-128)
+    want = oracle.forward(x.astype(np.float64), T.astype(np.float64), w, s, layout)
+    assert np.array_equal(oracle.forward_int8(x, T, w, s, layout).astype(np.float64), want)
+
+
+def test_int8_requantisation_rounds_to_even_and_saturates(oracle):
+    """Identity table (centre bin 1): the sum is x itself, so q = sat(rne(x * scale)) has a closed form.
+    Catches: truncation or round-half-away instead of ties-to-even, missing saturation, scale taken from the wrong channel."""
+    w = 3
+    x = np.arange(-128, 128, dtype=np.int8).reshape(1, 1, 16, 16).repeat(3, axis=1).copy()
+    T = np.zeros((3, 25), dtype=np.int8)
+    T[:, 12] = 1
+    scale = np.array([0.5, 1.5, -2.0], dtype=np.float32)
+    q = oracle.forward_int8(x, T, w, scale=scale)
+    xi = np.arange(-128, 128).reshape(16, 16)
+    # ties to even written out: v/2 is a tie when v is odd; the even neighbour is chosen
+    def rne(a):
+        f = np.floor(a)
+        d = a - f
+        return np.where(d > 0.5, f + 1, np.where(d < 0.5, f, np.where(f % 2 == 0, f, f + 1)))
+    assert np.array_equal(q[0, 0], np.clip(rne(xi * 0.5), -128, 127).astype(np.int8))
+    assert np.array_equal(q[0, 1], np.clip(rne(xi * 1.5), -128, 127).astype(np.int8))      # saturates beyond |x| > 85
+    assert np.array_equal(q[0, 2], np.clip(rne(xi * -2.0), -128, 127).astype(np.int8))     # sign, saturation at +127 / -128
+    assert q[0, 0, 8, 1] == 0 and q[0, 0, 8, 3] == 2 and q[0, 0, 8, 5] == 2                # 0.5 -> 0, 1.5 -> 2, 2.5 -> 2
+    assert q[0, 1].max() == 127 and q[0, 1].min() == -128
+
+
+def test_int8_requantisation_uses_binary32_products(oracle):
+    """The largest sum of a 14 x 14 window (196 * 127 * 127 = 3 161 284) times scales that are not binary fractions:
+    the quantised value is the one numpy gets with every intermediate held in binary32 (conversion, one product,
+    round-to-nearest-even).  Catches: a float64 product, a fused multiply-add, a wrong clamp order."""
+    w = 14
+    T = np.zeros((1, 729), dtype=np.int8)
+    T[0, :] = 127
+    x = np.full((1, 1, 14, 14), 127, dtype=np.int8)
+    s = int(oracle.forward_int8(x, T, w)[0, 0, 7, 7])
+    assert s == 196 * 127 * 127
+    for sc in (np.float32(1e-4), np.float32(3.3e-5), np.nextafter(np.float32(4e-5), np.float32(0))):
+        q = int(oracle.forward_int8(x, T, w, scale=np.array([sc], dtype=np.float32))[0, 0, 7, 7])
+        want = int(np.clip(np.rint(np.float32(np.float32(s) * sc)), -128, 127))
+        assert q == want, (sc, q, want)
