@@ -243,6 +243,23 @@ WBMM_API int wbmm_forward_matrix(const wbmm_desc_t *desc, const void *x, const v
                         int transpose, void *cuda_stream);
 
 /*
+ * INT8 forward (PAPER.md:749 reports INT8 deployments of the operator; reading A21):
+ * Algorithm 1 on signed 8-bit activations and tables with exact 32-bit integer sums (|sum| <= w*w*128*128 < 2^31),
+ * on the tensor cores (tcgen05.mma kind::i8, accumulator in tensor memory; wbmm_last_path() = WBMM_PATH_TC_GATHER).
+ *   x     [in]  B*C*H*W int8 in desc->layout.  T [in] C*(2w-1)^2 int8.  Device pointers, read-only.
+ *   scale [in, nullable] float32 [C], device, finite.
+ *   y     [out] scale == NULL: int32, the raw sums (4-byte aligned), same shape / layout as x;
+ *               scale != NULL: int8, q = sat_s8(rne(fp32(sum) * scale[c])) -- the sum converted to binary32 (RNE), ONE
+ *               binary32 product, rounded to the nearest integer with ties to even, clamped to [-128, 127].
+ *               Every element is overwritten, nothing outside it; y must not alias x.
+ * desc->dtype and desc->flags are not read (the element types are fixed by this entry point).  Serves w in {7, 14},
+ * any shift / ragged size / layout, with at most 128 windows across (W' / w <= 128); anything else:
+ * WBMM_STATUS_UNSUPPORTED, nothing launched.  Results are bit-exact against the integer definition.
+ */
+WBMM_API int wbmm_forward_int8(const wbmm_desc_t *desc, const int8_t *x, const int8_t *T, const float *scale, void *y,
+                      void *cuda_stream);
+
+/*
  * Multi-kernel fusion for one-window maps (section 3.7): a zero-padded ksize x ksize depthwise
  * conv (Eq. 1, cross-correlation) on an H = W = w map is the WBMM operator with the conv kernel written around
  * the centre of the table, so  Y = WBMM(X) + BN1(DW5(X)) + BN2(DW3(X))  folds into ONE table plus a bias:

@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libwbmm.so")
-SOURCES = ["wbmm_api.cu", "wbmm_simt.cu", "wbmm_tc.cu", "wbmm_tc_dt.cu", "wbmm_tc_nhwc.cu", "wbmm_tc_nhwc7.cu", "wbmm_tc_f32.cu", "wbmm_tc_f32_dt.cu", "wbmm_transpose.cu", "wbmm_static_scratch.cu", "wbmm_rect.cu"]
+SOURCES = ["wbmm_api.cu", "wbmm_simt.cu", "wbmm_tc.cu", "wbmm_tc_dt.cu", "wbmm_tc_nhwc.cu", "wbmm_tc_nhwc7.cu", "wbmm_tc_f32.cu", "wbmm_tc_f32_dt.cu", "wbmm_transpose.cu", "wbmm_static_scratch.cu", "wbmm_rect.cu", "wbmm_tc_i8.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--expt-relaxed-constexpr",

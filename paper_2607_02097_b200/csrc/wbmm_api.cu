@@ -756,6 +756,31 @@ int wbmm_forward_matrix(const wbmm_desc_t* desc, const void* x, const void* M, c
     return WBMM_STATUS_OK;
 }
 
+int wbmm_forward_int8(const wbmm_desc_t* desc, const int8_t* x, const int8_t* T, const float* scale, void* y, void* cuda_stream)
+{
+    if (!desc) return WBMM_STATUS_INVALID_ARGUMENT;
+    wbmm_desc_t d = *desc;
+    d.dtype = WBMM_DTYPE_F32;          // the element type is fixed by this entry point: desc->dtype is not read
+    int st = validate(&d);
+    if (st != WBMM_STATUS_OK) return st;
+    if (d.B == 0 || d.C == 0) return WBMM_STATUS_OK;
+    if (!x || !T || !y || static_cast<const void*>(x) == y) return WBMM_STATUS_INVALID_ARGUMENT;
+    if ((scale && !aligned(scale, 4)) || (!scale && !aligned(y, 4))) return WBMM_STATUS_MISALIGNED;
+    if (device_state() < 0) return WBMM_STATUS_NO_DEVICE;
+    wbmm::Geom g = wbmm::make_geom(d);
+    if (!wbmm::tc_i8_supported(g)) {
+        snprintf(t_last_error, sizeof(t_last_error),
+                 "wbmm_forward_int8: w must be 7 or 14 with at most 128 windows across (w = %d, %d windows across)", g.w, g.nww);
+        return WBMM_STATUS_UNSUPPORTED;
+    }
+    int launches = 0;
+    cudaError_t e = wbmm::tc_i8_forward(g, x, T, scale, y, static_cast<cudaStream_t>(cuda_stream), &launches);
+    g_launches += launches;
+    if (e != cudaSuccess) return set_cuda_error(e, "tc_i8_forward");
+    t_last_path = WBMM_PATH_TC_GATHER;
+    return WBMM_STATUS_OK;
+}
+
 int wbmm_fold_dwconv(const wbmm_desc_t* desc, const void* T, const void* K, int ksize, const float* scale,
                      void* Tout, void* cuda_stream)
 {

@@ -1,0 +1,377 @@
+// INT8 forward on the tensor cores (PAPER.md:749 reports INT8 deployments): signed 8-bit x and
+// table, exact 32-bit sums (tcgen05.mma kind::i8, accumulator in TMEM), output either the raw sums (int32) or
+// requantised 8-bit values q = sat_s8(rne(fp32(sum) * scale[c])) (reading A21).
+//
+// Per channel the GEMM is the one of wbmm_tc.cu:  D[m, i] = sum_j X[m, j] * W_c[i, j],  m = window, i = output
+// position, j = input position (Alg. 1 l.15).
+//   * A = X from TMEM ("TS" form): lane m holds window m's N bytes in row-major in-window order, four per 32-bit
+//     column; K = 32 per instruction = 8 columns.
+//   * B = W_c built in shared memory from the (2w-1)^2 table (Eq. 6-8), K-major no-swizzle core
+//     matrices of 8 rows x 16 bytes (16 values); never in HBM.
+//   * D: 128 lanes x N_PAD int32 columns, read back with tcgen05.ld.
+// The kernel is block-synchronous (one tile of up to 128 windows at a time: gather -> TMEM -> MMA -> epilogue ->
+// scatter), any layout / shift / ragged size by index arithmetic, with 32-bit copies where rows allow it.
+#include <cuda.h>
+
+#include "wbmm_common.cuh"
+#include "wbmm_ptx.cuh"
+#include "wbmm_tc.cuh"
+
+namespace wbmm {
+
+namespace {
+
+constexpr int kThreadsI = 256;   // 8 warps; warps 0-3 own the 128 TMEM lanes
+
+template <int WS>
+struct I8Cfg {
+    static constexpr int N = WS * WS;
+    static constexpr int K_PAD = (N + 31) / 32 * 32;     // MMA K: 32 per instruction
+    static constexpr int N_PAD = (N + 15) / 16 * 16;     // MMA N: multiple of 16 at M = 128
+    static constexpr int KSTEPS = K_PAD / 32;
+    static constexpr int NW = (N + 3) / 4;               // 32-bit words per window
+    static constexpr int A_COLS = K_PAD / 4;
+    static constexpr int TW = 2 * WS - 1;
+    static constexpr int NB = TW * TW;
+    static constexpr int LBO = N_PAD * 16;               // bytes between K chunks (16 values) of W_c
+    static constexpr int WC_BYTES = (K_PAD / 16) * LBO;
+    static constexpr int D_COL = (A_COLS + 31) / 32 * 32;
+    static constexpr int TMEM_COLS = (D_COL + N_PAD) <= 128 ? 128 : ((D_COL + N_PAD) <= 256 ? 256 : 512);
+    static constexpr int TS_BYTES = (NB + 15) / 16 * 16;
+    static constexpr int FRAME_BYTES = 128 * N + 128 * 16;   // <= 128 windows, plane stride rounded up to 16 bytes
+};
+
+struct I8Tiles {
+    int NP, NSY, nstrips, tiles_per_c;
+    int frame_rows, S;       // rows of one frame plane; plane stride in bytes (multiple of 16)
+    long long ntiles;
+    int vec;                 // rows can move as aligned 32-bit words (NCHW, no column shift, W' = W, W % 4 == 0)
+};
+
+__host__ __device__ constexpr uint32_t idesc_i8(int M, int N)
+{
+    // c_format S32 (2) | a, b signed 8-bit (1) | K-major both | N >> 3 | M >> 4
+    return (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
+}
+
+__device__ __forceinline__ void mma_ts_i8(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t accumulate)
+{
+    asm volatile(
+        "{ .reg .pred p; setp.ne.b32 p, %4, 0; tcgen05.mma.cta_group::1.kind::i8 [%0], [%1], %2, %3, p; }" ::"r"(d_tmem),
+        "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+
+// W_c[i][j] = T[c, rel(i, j)] (Eq. 7) in the K-major core-matrix layout: value (i, j) at byte (j/16)*LBO + i*16 + j%16.
+template <int WS>
+__device__ __forceinline__ void build_weight_i8(const int8_t* __restrict__ Tc, uint8_t* Ts, uint8_t* Wc, int tid)
+{
+    using Cf = I8Cfg<WS>;
+    for (int k = tid; k < Cf::NB; k += kThreadsI) Ts[k] = (uint8_t)Tc[k];
+    __syncthreads();
+    constexpr int NCHUNK = (Cf::K_PAD / 16) * Cf::N_PAD;
+    for (int id = tid; id < NCHUNK; id += kThreadsI) {
+        const int kc = id / Cf::N_PAD, i = id % Cf::N_PAD;
+        uint32_t pk[4] = {0u, 0u, 0u, 0u};
+        if (i < Cf::N) {
+            const int ri = i / WS, ci = i % WS;
+            int j = kc * 16;
+            int rj = j / WS, cj = j % WS;
+#pragma unroll
+            for (int e = 0; e < 16; ++e) {
+                uint32_t v = 0;
+                if (j < Cf::N) v = Ts[(ri - rj + WS - 1) * Cf::TW + (ci - cj + WS - 1)];
+                pk[e >> 2] |= v << ((e & 3) * 8);
+                ++j;
+                if (++cj == WS) { cj = 0; ++rj; }
+            }
+        }
+        *reinterpret_cast<uint4*>(Wc + kc * Cf::LBO + i * 16) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+    }
+}
+
+// Window -> TMEM A (warp-collective): the N bytes in row-major order, four per column; lanes without a window and
+// the K padding write zeros.
+template <int WS>
+__device__ __forceinline__ void window_to_tmem_i8(const uint8_t* win, bool valid, int rowB, uint32_t taddr)
+{
+    using Cf = I8Cfg<WS>;
+    constexpr int NV = (Cf::A_COLS + 7) / 8 * 8;
+    uint32_t v[NV];
+#pragma unroll
+    for (int k = 0; k < NV; ++k) v[k] = 0u;
+    if (valid) {
+        if constexpr (WS % 2 == 0) {
+            // a window row is WS/2 aligned halfwords; halfword q = r*(WS/2) + k of the window lands in word q/2
+#pragma unroll
+            for (int r = 0; r < WS; ++r)
+#pragma unroll
+                for (int k = 0; k < WS / 2; ++k) {
+                    const int q = r * (WS / 2) + k;
+                    const uint32_t h = *reinterpret_cast<const uint16_t*>(win + r * rowB + 2 * k);
+                    v[q >> 1] |= h << ((q & 1) * 16);
+                }
+        } else {
+#pragma unroll
+            for (int r = 0; r < WS; ++r)
+#pragma unroll
+                for (int k = 0; k < WS; ++k) {
+                    const int q = r * WS + k;
+                    v[q >> 2] |= (uint32_t)win[r * rowB + k] << ((q & 3) * 8);
+                }
+        }
+    }
+#pragma unroll
+    for (int ch = 0; ch < NV / 8; ++ch) ptx::tmem_st8(taddr + ch * 8, v + ch * 8);
+    ptx::tmem_wait_st();
+}
+
+__device__ __forceinline__ uint32_t requant(uint32_t acc_bits, float scale)
+{
+    const float r = __fmul_rn(__int2float_rn((int)acc_bits), scale);   // binary32 conversion and ONE product (no fma)
+    const int q = __float2int_rn(r);                                   // ties to even; saturates at the int32 range
+    return (uint32_t)min(127, max(-128, q)) & 0xffu;
+}
+
+template <int WS, bool OUT8>
+__global__ void __launch_bounds__(kThreadsI, 1)
+tc_i8_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t* __restrict__ T, const float* __restrict__ scale,
+             void* __restrict__ yv)
+{
+    using Cf = I8Cfg<WS>;
+    extern __shared__ __align__(1024) uint8_t smem[];
+    uint8_t* Wc = smem;
+    uint8_t* Ts = smem + Cf::WC_BYTES;
+    uint8_t* frame = smem + Cf::WC_BYTES + Cf::TS_BYTES;
+    int32_t* oframe = reinterpret_cast<int32_t*>(frame + Cf::FRAME_BYTES);   // int32 output staging (OUT8: unused)
+    __shared__ __align__(8) uint64_t mma_bar;
+    __shared__ uint32_t tmem_base_s;
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const uint32_t bar = ptx::smem_u32(&mma_bar);
+    if (warp == 0) ptx::tmem_alloc(ptx::smem_u32(&tmem_base_s), Cf::TMEM_COLS);
+    if (tid == 32) {
+        ptx::mbar_init(bar, 1);
+        ptx::fence_mbar_init();
+    }
+    ptx::tc_fence_before_sync();
+    __syncthreads();
+    ptx::tc_fence_after_sync();
+    const uint32_t tmem = tmem_base_s;
+    const uint32_t tmem_a = tmem, tmem_d = tmem + Cf::D_COL;
+    constexpr uint32_t idesc = idesc_i8(128, Cf::N_PAD);
+
+    const long long t0 = tl.ntiles * blockIdx.x / gridDim.x, t1 = tl.ntiles * (blockIdx.x + 1) / gridDim.x;
+    const int rowB = g.Wp;
+    const int frame_elems = tl.frame_rows * g.Wp;
+    int cur_c = -1;
+    uint32_t phase = 0;
+
+    // this thread's window (warps 0-3 only): m = wl * NP + pl
+    const int m = tid & 127;
+    const int wl = m / tl.NP, pl = m % tl.NP;
+    const int wyl = wl / g.nww, wx = wl % g.nww;
+    const int win_off = (wyl * WS) * g.Wp + wx * WS;
+    uint8_t* win = frame + pl * tl.S + win_off;
+
+    int8_t* y8 = static_cast<int8_t*>(yv);
+    int32_t* y32 = static_cast<int32_t*>(yv);
+
+    for (long long t = t0; t < t1; ++t) {
+        const int c = (int)(t / tl.tiles_per_c);
+        const int rem = (int)(t % tl.tiles_per_c);
+        const int gb = rem / tl.nstrips, strip = rem % tl.nstrips;
+        const int b0 = gb * tl.NP, wy0 = strip * tl.NSY;
+        const int np_eff = min(tl.NP, g.B - b0);
+
+        if (c != cur_c) {   // (the previous tile's MMAs have completed: every thread waited on mma_bar)
+            build_weight_i8<WS>(T + (long long)c * Cf::NB, Ts, Wc, tid);
+            cur_c = c;
+        }
+        // element `idx` of the frame (plane p, row hh, column vv in padded + shifted coordinates) -> offset in x / y
+        auto src_offset = [&](int p, int r2) -> long long {
+            const int hh = r2 / g.Wp, vv = r2 - hh * g.Wp;
+            const int hp = wy0 * WS + hh;
+            if (hp >= g.Hp) return -1;
+            int h = hp + g.sh, v = vv + g.sw;
+            if (h >= g.Hp) h -= g.Hp;
+            if (v >= g.Wp) v -= g.Wp;
+            return h < g.H && v < g.W ? act_offset(g, b0 + p, c, h, v) : -1;
+        };
+        if (tl.vec) {
+            const int fw = frame_elems >> 2, nfw = np_eff * fw;
+            for (int base = tid; base < nfw; base += 8 * kThreadsI) {
+                uint32_t val[8];
+#pragma unroll
+                for (int u = 0; u < 8; ++u) {
+                    const int idx = base + u * kThreadsI;
+                    long long off = -1;
+                    if (idx < nfw) { const int p = idx / fw; off = src_offset(p, (idx - p * fw) * 4); }
+                    val[u] = off >= 0 ? *reinterpret_cast<const uint32_t*>(x + off) : 0u;
+                }
+#pragma unroll
+                for (int u = 0; u < 8; ++u) {
+                    const int idx = base + u * kThreadsI;
+                    if (idx < nfw) { const int p = idx / fw; *reinterpret_cast<uint32_t*>(frame + p * tl.S + (idx - p * fw) * 4) = val[u]; }
+                }
+            }
+        } else {
+            const int nfe = np_eff * frame_elems;
+            for (int base = tid; base < nfe; base += 8 * kThreadsI) {
+                uint8_t val[8];
+#pragma unroll
+                for (int u = 0; u < 8; ++u) {
+                    const int idx = base + u * kThreadsI;
+                    long long off = -1;
+                    if (idx < nfe) { const int p = idx / frame_elems; off = src_offset(p, idx - p * frame_elems); }
+                    val[u] = off >= 0 ? (uint8_t)x[off] : (uint8_t)0;
+                }
+#pragma unroll
+                for (int u = 0; u < 8; ++u) {
+                    const int idx = base + u * kThreadsI;
+                    if (idx < nfe) { const int p = idx / frame_elems; frame[p * tl.S + (idx - p * frame_elems)] = val[u]; }
+                }
+            }
+        }
+        ptx::fence_proxy_async_smem();   // W_c (generic-proxy stores) -> tcgen05.mma operand reads
+        __syncthreads();
+
+        const bool valid = wl < tl.NSY * g.nww && pl < np_eff && wy0 + wyl < g.nwh;
+        if (warp < 4) {
+            window_to_tmem_i8<WS>(win, valid, rowB, tmem_a + ((uint32_t)(warp * 32) << 16));
+            ptx::tc_fence_before_sync();
+        }
+        __syncthreads();
+        if (warp == 4 && lane == 0) {
+            ptx::tc_fence_after_sync();
+            const uint32_t wc_addr = ptx::smem_u32(Wc);
+#pragma unroll
+            for (int ks = 0; ks < Cf::KSTEPS; ++ks) {
+                const uint64_t bdesc = ptx::smem_desc_kmajor_noswz(wc_addr + ks * 2 * Cf::LBO, Cf::LBO, 128);
+                mma_ts_i8(tmem_d, tmem_a + ks * 8, bdesc, idesc, ks > 0 ? 1u : 0u);
+            }
+            ptx::mma_commit(bar);
+        }
+        ptx::mbar_wait(bar, phase);
+        phase ^= 1;
+        ptx::tc_fence_after_sync();
+        if (warp < 4) {
+            const uint32_t td = tmem_d + ((uint32_t)(warp * 32) << 16);
+            const float sc = OUT8 ? scale[c] : 0.f;
+            int32_t* owin = oframe + pl * frame_elems + win_off;
+#pragma unroll
+            for (int ch = 0; ch < Cf::N_PAD / 16; ++ch) {
+                uint32_t v[16];
+                ptx::tmem_ld16(td + ch * 16, v);
+                ptx::tmem_wait_ld();
+                if (valid) {
+#pragma unroll
+                    for (int e = 0; e < 16; ++e) {
+                        const int i = ch * 16 + e;
+                        if (i < Cf::N) {
+                            const int r = i / WS, k = i % WS;
+                            if constexpr (!OUT8) {
+                                owin[r * rowB + k] = (int32_t)v[e];
+                            } else if constexpr (WS % 2 == 0) {
+                                if ((k & 1) == 0)   // (i and i+1 are in the same chunk: 16 and WS are even)
+                                    *reinterpret_cast<uint16_t*>(win + r * rowB + k) =
+                                        (uint16_t)(requant(v[e], sc) | (requant(v[e + 1], sc) << 8));
+                            } else {
+                                win[r * rowB + k] = (uint8_t)requant(v[e], sc);
+                            }
+                        }
+                    }
+                }
+            }
+            ptx::tc_fence_before_sync();
+        }
+        __syncthreads();
+        // y <- frame (un-shift, crop)
+        if constexpr (OUT8) {
+            if (tl.vec) {
+                const int fw = frame_elems >> 2, nfw = np_eff * fw;
+                for (int idx = tid; idx < nfw; idx += kThreadsI) {
+                    const int p = idx / fw, r2 = (idx - p * fw) * 4;
+                    const long long off = src_offset(p, r2);
+                    if (off >= 0) *reinterpret_cast<uint32_t*>(y8 + off) = *reinterpret_cast<const uint32_t*>(frame + p * tl.S + r2);
+                }
+            } else {
+                const int nfe = np_eff * frame_elems;
+                for (int idx = tid; idx < nfe; idx += kThreadsI) {
+                    const int p = idx / frame_elems, r2 = idx - p * frame_elems;
+                    const long long off = src_offset(p, r2);
+                    if (off >= 0) y8[off] = (int8_t)frame[p * tl.S + r2];
+                }
+            }
+        } else {
+            const int nfe = np_eff * frame_elems;
+            for (int idx = tid; idx < nfe; idx += kThreadsI) {
+                const int p = idx / frame_elems, r2 = idx - p * frame_elems;
+                const long long off = src_offset(p, r2);
+                if (off >= 0) y32[off] = oframe[p * frame_elems + r2];
+            }
+        }
+        __syncthreads();
+    }
+    ptx::tc_fence_before_sync();
+    __syncthreads();
+    if (warp == 0) ptx::tmem_dealloc(tmem, Cf::TMEM_COLS);
+}
+
+bool i8_tiles(const Geom& g, const void* x, const void* y, bool out8, I8Tiles* t)
+{
+    if (g.nww > 128 || g.nww < 1) return false;
+    t->NSY = g.nwh < 128 / g.nww ? g.nwh : 128 / g.nww;
+    t->NP = t->NSY == g.nwh ? 128 / (g.nwh * g.nww) : 1;
+    if (t->NP < 1) t->NP = 1;
+    if (t->NP > g.B) t->NP = g.B > 0 ? g.B : 1;
+    t->nstrips = (g.nwh + t->NSY - 1) / t->NSY;
+    t->tiles_per_c = (g.B + t->NP - 1) / t->NP * t->nstrips;
+    t->frame_rows = t->NSY * g.w;
+    t->S = (t->frame_rows * g.Wp + 15) / 16 * 16;
+    t->ntiles = (long long)g.C * t->tiles_per_c;
+    const bool al = reinterpret_cast<uintptr_t>(x) % 4 == 0 && (!out8 || reinterpret_cast<uintptr_t>(y) % 4 == 0);
+    t->vec = (g.layout == WBMM_LAYOUT_NCHW && g.sw == 0 && g.Wp == g.W && g.W % 4 == 0 && al) ? 1 : 0;
+    return true;
+}
+
+template <int WS, bool OUT8>
+cudaError_t launch_i8(const Geom& g, const I8Tiles& tl, const int8_t* x, const int8_t* T, const float* scale, void* y,
+                      cudaStream_t stream, int* launches)
+{
+    using Cf = I8Cfg<WS>;
+    const size_t smem = Cf::WC_BYTES + Cf::TS_BYTES + Cf::FRAME_BYTES + (OUT8 ? 0 : 128 * Cf::N * 4);
+    auto kern = tc_i8_kernel<WS, OUT8>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const long long grid = tl.ntiles < sms ? tl.ntiles : sms;
+    kern<<<(unsigned)grid, kThreadsI, smem, stream>>>(g, tl, x, T, scale, y);
+    ++*launches;
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+bool tc_i8_supported(const Geom& g)
+{
+    if (g.w != 7 && g.w != 14) return false;
+    I8Tiles tl;
+    return i8_tiles(g, nullptr, nullptr, false, &tl);
+}
+
+cudaError_t tc_i8_forward(const Geom& g, const int8_t* x, const int8_t* T, const float* scale, void* y, cudaStream_t stream,
+                          int* launches)
+{
+    I8Tiles tl;
+    if (!i8_tiles(g, x, y, scale != nullptr, &tl)) return cudaErrorInvalidValue;
+    if (tl.ntiles == 0) return cudaSuccess;
+    if (g.w == 14) return scale ? launch_i8<14, true>(g, tl, x, T, scale, y, stream, launches)
+                                : launch_i8<14, false>(g, tl, x, T, scale, y, stream, launches);
+    return scale ? launch_i8<7, true>(g, tl, x, T, scale, y, stream, launches)
+                 : launch_i8<7, false>(g, tl, x, T, scale, y, stream, launches);
+}
+
+}  // namespace wbmm

@@ -108,3 +108,28 @@ def make(case: Case, device: str = "cpu", pin: bool = False):
         return t.to(device) if device != "cpu" else t
 
     return {"x": fin(x, True), "T": fin(T, False), "dy": fin(dy, True)}
+
+
+def make_int8(case: Case, device: str = "cpu", extreme: bool = False):
+    """dict(x=, T=, scale=) for the INT8 forward: activations as symmetric 8-bit quantisation of a normal map
+    (round(x / 3 sigma * 127), clipped), the table likewise from the case's table recipe, per-channel float32
+    requantisation scales that put the sums' spread at about a third of the int8 range.  extreme: a few -128 / 127
+    runs and one all -128 table row (the largest products)."""
+    f = make(with_(case, dtype="f32", layout=NCHW), device="cpu")
+    x = torch.clamp(torch.round(f["x"] / 3.0 * 127.0), -128, 127).to(torch.int8)
+    T = f["T"]
+    T = torch.clamp(torch.round(T / T.abs().amax(dim=1, keepdim=True) * 127.0), -128, 127).to(torch.int8)
+    if extreme:
+        x.view(-1)[: min(x.numel(), 3 * case.w * case.w)] = -128
+        x.view(-1)[-min(x.numel(), 2 * case.w * case.w):] = 127
+        T[0, :] = -128
+        if case.C > 1:
+            T[1, :] = 127
+    g = torch.Generator(device="cpu").manual_seed(case.seed + 77)
+    sigma = 42.0 * 42.0 * case.w                       # ~ std of a sum of w*w products of such values
+    scale = (40.0 / sigma) * (0.5 + torch.rand((case.C,), generator=g, dtype=torch.float32))
+    if case.layout == NHWC:
+        x = x.permute(0, 2, 3, 1).contiguous()
+    if device != "cpu":
+        x, T, scale = x.to(device), T.to(device), scale.to(device)
+    return {"x": x, "T": T, "scale": scale}
