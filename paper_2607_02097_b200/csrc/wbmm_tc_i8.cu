@@ -9,7 +9,8 @@
 //   * B = W_c built in shared memory from the (2w-1)^2 table (Eq. 6-8), K-major no-swizzle core
 //     matrices of 8 rows x 16 bytes (16 values); never in HBM.
 //   * D: 128 lanes x N_PAD int32 columns, read back with tcgen05.ld.
-// The kernel is block-synchronous (one tile of up to 128 windows at a time: gather -> TMEM -> MMA -> epilogue ->
+// Two kernels: tc_i8_bulk_kernel (NCHW, no shift, aligned sizes: bulk copies, two or three CTAs per SM, see there) and
+// tc_i8_kernel, block-synchronous (one tile of up to 128 windows at a time: gather -> TMEM -> MMA -> epilogue ->
 // scatter), any layout / shift / ragged size by index arithmetic, with 32-bit copies where rows allow it.
 #include <cuda.h>
 
@@ -29,7 +30,6 @@ struct I8Cfg {
     static constexpr int K_PAD = (N + 31) / 32 * 32;     // MMA K: 32 per instruction
     static constexpr int N_PAD = (N + 15) / 16 * 16;     // MMA N: multiple of 16 at M = 128
     static constexpr int KSTEPS = K_PAD / 32;
-    static constexpr int NW = (N + 3) / 4;               // 32-bit words per window
     static constexpr int A_COLS = K_PAD / 4;
     static constexpr int TW = 2 * WS - 1;
     static constexpr int NB = TW * TW;
@@ -38,7 +38,11 @@ struct I8Cfg {
     static constexpr int D_COL = (A_COLS + 31) / 32 * 32;
     static constexpr int TMEM_COLS = (D_COL + N_PAD) <= 128 ? 128 : ((D_COL + N_PAD) <= 256 ? 256 : 512);
     static constexpr int TS_BYTES = (NB + 15) / 16 * 16;
-    static constexpr int FRAME_BYTES = 128 * N + 128 * 16;   // <= 128 windows, plane stride rounded up to 16 bytes
+    static constexpr int FRAME_BYTES = 128 * N + 128 * 32;   // <= 128 windows, plane stride rounded up to 16 * odd bytes
+    // pipelined form: A in shared memory (K-major core matrices, 128 rows), D alone in tensor memory
+    static constexpr int A_LBO = 128 * 16;
+    static constexpr int A_BYTES = (K_PAD / 16) * A_LBO;
+    static constexpr int D_COLS_ALLOC = N_PAD <= 32 ? 32 : (N_PAD <= 64 ? 64 : (N_PAD <= 128 ? 128 : 256));
 };
 
 struct I8Tiles {
@@ -46,6 +50,7 @@ struct I8Tiles {
     int frame_rows, S;       // rows of one frame plane; plane stride in bytes (multiple of 16)
     long long ntiles;
     int vec;                 // rows can move as aligned 32-bit words (NCHW, no column shift, W' = W, W % 4 == 0)
+    int bulk;                // plane strips are contiguous 16-byte aligned runs: the bulk-copy kernel serves (see i8_tiles)
 };
 
 __host__ __device__ constexpr uint32_t idesc_i8(int M, int N)
@@ -59,6 +64,14 @@ __device__ __forceinline__ void mma_ts_i8(uint32_t d_tmem, uint32_t a_tmem, uint
     asm volatile(
         "{ .reg .pred p; setp.ne.b32 p, %4, 0; tcgen05.mma.cta_group::1.kind::i8 [%0], [%1], %2, %3, p; }" ::"r"(d_tmem),
         "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+
+__device__ __forceinline__ void mma_ss_i8(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate)
+{
+    asm volatile(
+        "{ .reg .pred p; setp.ne.b32 p, %4, 0; tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p; }" ::"r"(d_tmem),
+        "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
         : "memory");
 }
 
@@ -318,6 +331,193 @@ tc_i8_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t* __r
     if (warp == 0) ptx::tmem_dealloc(tmem, Cf::TMEM_COLS);
 }
 
+// ------------------------------------------------------------------------------------------------
+// Bulk-copy form: NCHW, no shift, H and W multiples of w, plane strips that are 16-byte aligned runs.  A plane strip
+// moves global <-> shared memory as ONE 1-D bulk copy (cp.async.bulk, TMA engine); the next tile's planes are in
+// flight while the current tile is multiplied and requantised.  A is staged in shared memory (tcgen05.mma "SS" form)
+// so that tensor memory holds D only (208 columns at w = 14 -> 256 allocated): two CTAs share an SM (three at w = 7)
+// and fill each other's barrier waits.  Per tile:
+//   wait full | windows: frame -> registers -> A (16-byte chunks, conflict-free) | sync | load of tile t+1 starts
+//   7 (w = 14) / 2 (w = 7) MMAs | tcgen05.ld -> requantise -> output planes (over the A tile) | sync | bulk stores
+template <int WS, bool OUT8>
+constexpr int i8_ctas() { return WS == 7 ? 3 : (OUT8 ? 2 : 1); }
+
+template <int WS, bool OUT8>
+struct I8Fast {
+    using Cf = I8Cfg<WS>;
+    static constexpr int OUT_BYTES = OUT8 ? Cf::FRAME_BYTES : 128 * Cf::N * 4;
+    static constexpr int AO_BYTES = (Cf::A_BYTES > OUT_BYTES ? Cf::A_BYTES : OUT_BYTES);
+    static constexpr int OFF_TS = Cf::WC_BYTES;
+    static constexpr int OFF_FRAME = (OFF_TS + Cf::TS_BYTES + 127) / 128 * 128;
+    static constexpr int OFF_AO = (OFF_FRAME + Cf::FRAME_BYTES + 127) / 128 * 128;
+    static constexpr int SMEM = OFF_AO + AO_BYTES;
+};
+
+template <int WS, bool OUT8>
+__global__ void __launch_bounds__(kThreadsI, i8_ctas<WS, OUT8>())
+tc_i8_bulk_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t* __restrict__ T,
+                  const float* __restrict__ scale, void* __restrict__ yv)
+{
+    using Cf = I8Cfg<WS>;
+    using Sm = I8Fast<WS, OUT8>;
+    extern __shared__ __align__(1024) uint8_t smem[];
+    uint8_t* Wc = smem;
+    uint8_t* Ts = smem + Sm::OFF_TS;
+    uint8_t* frame = smem + Sm::OFF_FRAME;
+    uint8_t* ao = smem + Sm::OFF_AO;          // the A tile, then the tile's output planes
+    __shared__ __align__(8) uint64_t bars[2];
+    __shared__ uint32_t tmem_base_s;
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const uint32_t mma_bar = ptx::smem_u32(&bars[0]), full_bar = ptx::smem_u32(&bars[1]);
+    if (warp == 0) ptx::tmem_alloc(ptx::smem_u32(&tmem_base_s), Cf::D_COLS_ALLOC);
+    if (tid == 32) {
+        ptx::mbar_init(mma_bar, 1);
+        ptx::mbar_init(full_bar, 1);
+        ptx::fence_mbar_init();
+    }
+    ptx::tc_fence_before_sync();
+    __syncthreads();
+    ptx::tc_fence_after_sync();
+    const uint32_t tmem_d = tmem_base_s;
+    constexpr uint32_t idesc = idesc_i8(128, Cf::N_PAD);
+
+    const long long t0 = tl.ntiles * blockIdx.x / gridDim.x, t1 = tl.ntiles * (blockIdx.x + 1) / gridDim.x;
+    const int rowB = g.W;
+    const int frame_elems = tl.frame_rows * g.W;
+    const long long plane = (long long)g.H * g.W;
+    const int So = OUT8 ? tl.S : frame_elems * 4;        // output plane stride in shared memory (bytes)
+    int cur_c = -1;
+    uint32_t phase = 0;
+
+    const int m = tid & 127;
+    const int wl = m / tl.NP, pl = m % tl.NP;
+    const int wyl = wl / g.nww, wx = wl % g.nww;
+    const bool in_frame = wl < tl.NSY * g.nww;
+    const int win_off = in_frame ? (wyl * WS) * g.W + wx * WS : 0;
+    const uint8_t* win = frame + pl * tl.S + win_off;
+
+    struct Tile { int c, b0, wy0, np, bytes; };
+    auto tile_at = [&](long long t) -> Tile {
+        Tile q;
+        q.c = (int)(t / tl.tiles_per_c);
+        const int rem = (int)(t % tl.tiles_per_c);
+        const int gb = rem / tl.nstrips, strip = rem % tl.nstrips;
+        q.b0 = gb * tl.NP;
+        q.wy0 = strip * tl.NSY;
+        q.np = min(tl.NP, g.B - q.b0);
+        q.bytes = min(tl.NSY, g.nwh - q.wy0) * WS * g.W;
+        return q;
+    };
+    auto load_tile = [&](const Tile& q) {    // one thread
+        ptx::mbar_arrive_expect_tx(full_bar, (uint32_t)(q.np * q.bytes));
+        const int8_t* src = x + ((long long)q.b0 * g.C + q.c) * plane + (long long)q.wy0 * WS * g.W;
+        for (int p = 0; p < q.np; ++p)
+            ptx::bulk_g2s(ptx::smem_u32(frame + p * tl.S), src + (long long)p * g.C * plane, (uint32_t)q.bytes, full_bar);
+    };
+    if (tid == 0 && t0 < t1) load_tile(tile_at(t0));
+
+    for (long long t = t0; t < t1; ++t) {
+        const Tile q = tile_at(t);
+        if (q.c != cur_c) {   // (the previous tile's MMAs have completed: every thread waited on mma_bar)
+            build_weight_i8<WS>(T + (long long)q.c * Cf::NB, Ts, Wc, tid);
+            cur_c = q.c;
+        }
+        ptx::mbar_wait(full_bar, phase);
+        if (warp < 4) {
+            // this thread's window -> registers (row-major bytes, four per word) -> row m of A, 16 bytes per K chunk
+            constexpr int NV = Cf::K_PAD / 4;
+            uint32_t v[NV];
+#pragma unroll
+            for (int k = 0; k < NV; ++k) v[k] = 0u;
+            if constexpr (WS % 2 == 0) {
+#pragma unroll
+                for (int r = 0; r < WS; ++r)
+#pragma unroll
+                    for (int k = 0; k < WS / 2; ++k) {
+                        const int h = r * (WS / 2) + k;
+                        const uint32_t u = *reinterpret_cast<const uint16_t*>(win + r * rowB + 2 * k);
+                        v[h >> 1] |= u << ((h & 1) * 16);
+                    }
+            } else {
+#pragma unroll
+                for (int r = 0; r < WS; ++r)
+#pragma unroll
+                    for (int k = 0; k < WS; ++k) {
+                        const int h = r * WS + k;
+                        v[h >> 2] |= (uint32_t)win[r * rowB + k] << ((h & 3) * 8);
+                    }
+            }
+#pragma unroll
+            for (int kc = 0; kc < Cf::K_PAD / 16; ++kc)
+                *reinterpret_cast<uint4*>(ao + kc * Cf::A_LBO + m * 16) = make_uint4(v[4 * kc], v[4 * kc + 1], v[4 * kc + 2], v[4 * kc + 3]);
+        }
+        ptx::fence_proxy_async_smem();   // A and W_c (generic-proxy stores) -> tcgen05.mma operand reads
+        __syncthreads();                 // the frame has been read: the next tile may land in it
+        if (tid == 0 && t + 1 < t1) load_tile(tile_at(t + 1));
+        if (warp == 4 && lane == 0) {
+            ptx::tc_fence_after_sync();
+            const uint32_t wc_addr = ptx::smem_u32(Wc), a_addr = ptx::smem_u32(ao);
+#pragma unroll
+            for (int ks = 0; ks < Cf::KSTEPS; ++ks) {
+                const uint64_t adesc = ptx::smem_desc_kmajor_noswz(a_addr + ks * 2 * Cf::A_LBO, Cf::A_LBO, 128);
+                const uint64_t bdesc = ptx::smem_desc_kmajor_noswz(wc_addr + ks * 2 * Cf::LBO, Cf::LBO, 128);
+                mma_ss_i8(tmem_d, adesc, bdesc, idesc, ks > 0 ? 1u : 0u);
+            }
+            ptx::mma_commit(mma_bar);
+        }
+        ptx::mbar_wait(mma_bar, phase);
+        phase ^= 1;
+        ptx::tc_fence_after_sync();
+        if (warp < 4) {
+            const bool valid = in_frame && pl < q.np && q.wy0 + wyl < g.nwh;
+            const uint32_t td = tmem_d + ((uint32_t)(warp * 32) << 16);
+            const float sc = OUT8 ? scale[q.c] : 0.f;
+            uint8_t* owin = ao + pl * So + win_off * (OUT8 ? 1 : 4);
+#pragma unroll
+            for (int ch = 0; ch < Cf::N_PAD / 16; ++ch) {
+                uint32_t v[16];
+                ptx::tmem_ld16(td + ch * 16, v);
+                ptx::tmem_wait_ld();
+                if (valid) {
+#pragma unroll
+                    for (int e = 0; e < 16; ++e) {
+                        const int i = ch * 16 + e;
+                        if (i < Cf::N) {
+                            const int r = i / WS, k = i % WS;
+                            if constexpr (!OUT8) {
+                                *reinterpret_cast<uint32_t*>(owin + (r * rowB + k) * 4) = v[e];
+                            } else if constexpr (WS % 2 == 0) {
+                                if ((k & 1) == 0)
+                                    *reinterpret_cast<uint16_t*>(owin + r * rowB + k) =
+                                        (uint16_t)(requant(v[e], sc) | (requant(v[e + 1], sc) << 8));
+                            } else {
+                                owin[r * rowB + k] = (uint8_t)requant(v[e], sc);
+                            }
+                        }
+                    }
+                }
+            }
+            ptx::tc_fence_before_sync();
+        }
+        ptx::fence_proxy_async_smem();   // output planes (generic-proxy stores) -> bulk-copy reads
+        __syncthreads();
+        if (tid == 0) {
+            constexpr int ES = OUT8 ? 1 : 4;
+            uint8_t* dst = static_cast<uint8_t*>(yv) + (((long long)q.b0 * g.C + q.c) * plane + (long long)q.wy0 * WS * g.W) * ES;
+            for (int p = 0; p < q.np; ++p)
+                ptx::bulk_s2g(dst + (long long)p * g.C * plane * ES, ptx::smem_u32(ao + p * So), (uint32_t)(q.bytes * ES));
+            ptx::bulk_commit();
+            ptx::bulk_wait_read<0>();    // the A tile of the next iteration overwrites these planes
+        }
+        __syncthreads();
+    }
+    if (tid == 0) ptx::bulk_wait_all<0>();
+    ptx::tc_fence_before_sync();
+    __syncthreads();
+    if (warp == 0) ptx::tmem_dealloc(tmem_d, Cf::D_COLS_ALLOC);
+}
+
 bool i8_tiles(const Geom& g, const void* x, const void* y, bool out8, I8Tiles* t)
 {
     if (g.nww > 128 || g.nww < 1) return false;
@@ -329,9 +529,15 @@ bool i8_tiles(const Geom& g, const void* x, const void* y, bool out8, I8Tiles* t
     t->tiles_per_c = (g.B + t->NP - 1) / t->NP * t->nstrips;
     t->frame_rows = t->NSY * g.w;
     t->S = (t->frame_rows * g.Wp + 15) / 16 * 16;
+    if ((t->S / 16) % 2 == 0) t->S += 16;          // 16 * odd: planes start on different banks
     t->ntiles = (long long)g.C * t->tiles_per_c;
     const bool al = reinterpret_cast<uintptr_t>(x) % 4 == 0 && (!out8 || reinterpret_cast<uintptr_t>(y) % 4 == 0);
     t->vec = (g.layout == WBMM_LAYOUT_NCHW && g.sw == 0 && g.Wp == g.W && g.W % 4 == 0 && al) ? 1 : 0;
+    // bulk-copy kernel: every plane strip is one contiguous run whose address and size are multiples of 16 bytes
+    const bool al16 = reinterpret_cast<uintptr_t>(x) % 16 == 0 && reinterpret_cast<uintptr_t>(y) % 16 == 0;
+    const long long plane = (long long)g.H * g.W;
+    t->bulk = (g.layout == WBMM_LAYOUT_NCHW && g.sh == 0 && g.sw == 0 && g.Hp == g.H && g.Wp == g.W && al16 && plane % 16 == 0 &&
+               (t->nstrips == 1 || (g.w * g.W) % 16 == 0) && x != nullptr) ? 1 : 0;
     return true;
 }
 
@@ -340,13 +546,24 @@ cudaError_t launch_i8(const Geom& g, const I8Tiles& tl, const int8_t* x, const i
                       cudaStream_t stream, int* launches)
 {
     using Cf = I8Cfg<WS>;
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (tl.bulk) {
+        const size_t smem = I8Fast<WS, OUT8>::SMEM;
+        auto kern = tc_i8_bulk_kernel<WS, OUT8>;
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        const long long cap = (long long)sms * i8_ctas<WS, OUT8>();
+        const long long grid = tl.ntiles < cap ? tl.ntiles : cap;
+        kern<<<(unsigned)grid, kThreadsI, smem, stream>>>(g, tl, x, T, scale, y);
+        ++*launches;
+        return cudaGetLastError();
+    }
     const size_t smem = Cf::WC_BYTES + Cf::TS_BYTES + Cf::FRAME_BYTES + (OUT8 ? 0 : 128 * Cf::N * 4);
     auto kern = tc_i8_kernel<WS, OUT8>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    int dev = 0, sms = 148;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     const long long grid = tl.ntiles < sms ? tl.ntiles : sms;
     kern<<<(unsigned)grid, kThreadsI, smem, stream>>>(g, tl, x, T, scale, y);
     ++*launches;

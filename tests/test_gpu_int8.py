@@ -96,6 +96,40 @@ def test_int8_output_is_fully_overwritten_and_nothing_else(wb, oracle):
         assert np.array_equal(out.cpu().numpy(), want)
 
 
+@pytest.mark.parametrize("off", [0, 1, 4, 16])
+def test_int8_pointer_alignment_picks_a_kernel_that_fits(wb, oracle, off):
+    """x and y at byte offsets 0 / 1 / 4 / 16 inside larger buffers: bulk copies need 16, 32-bit copies 4, else bytes."""
+    case = si.Case("i8_align", 9, 3, 56, 56, 14, seed=840)
+    d = si.make_int8(case, device="cuda")
+    n = d["x"].numel()
+    xb = torch.zeros(n + 64, dtype=torch.int8, device="cuda")
+    xs = xb[off:off + n].view(d["x"].shape)
+    xs.copy_(d["x"])
+    yb = torch.full((n + 64,), 55, dtype=torch.int8, device="cuda")
+    ys = yb[off:off + n].view(d["x"].shape)
+    wb.wbmm_forward_int8(xs, d["T"], case.w, scale=d["scale"], out=ys)
+    want = oracle.forward_int8(d["x"].cpu().numpy(), d["T"].cpu().numpy(), case.w, scale=d["scale"].cpu().numpy())
+    assert np.array_equal(ys.cpu().numpy(), want)
+    assert bool((yb[:off] == 55).all()) and bool((yb[off + n:] == 55).all())
+    y32 = wb.wbmm_forward_int8(xs, d["T"], case.w)
+    assert np.array_equal(y32.cpu().numpy(), oracle.forward_int8(d["x"].cpu().numpy(), d["T"].cpu().numpy(), case.w))
+
+
+def test_int8_full_size_headline_shape(wb, oracle):
+    """B128 C96 56x56 w=14 (the headline shape of BASELINE.json in int8), whole tensor, both outputs."""
+    case = si.Case("i8_cfg3", 128, 96, 56, 56, 14, seed=850)
+    d = si.make_int8(case, device="cuda")
+    xh, Th, sh = d["x"].cpu().numpy(), d["T"].cpu().numpy(), d["scale"].cpu().numpy()
+    y8 = wb.wbmm_forward_int8(d["x"], d["T"], 14, scale=d["scale"])
+    assert np.array_equal(y8.cpu().numpy(), oracle.forward_int8(xh, Th, 14, scale=sh))
+    y32 = wb.wbmm_forward_int8(d["x"], d["T"], 14)
+    assert np.array_equal(y32.cpu().numpy(), oracle.forward_int8(xh, Th, 14))
+    case = si.Case("i8_cfg2", 128, 96, 56, 56, 7, seed=851)
+    d = si.make_int8(case, device="cuda")
+    y8 = wb.wbmm_forward_int8(d["x"], d["T"], 7, scale=d["scale"])
+    assert np.array_equal(y8.cpu().numpy(), oracle.forward_int8(d["x"].cpu().numpy(), d["T"].cpu().numpy(), 7, scale=d["scale"].cpu().numpy()))
+
+
 def test_int8_unsupported_and_argument_errors(wb):
     x = torch.zeros((1, 2, 10, 10), dtype=torch.int8, device="cuda")
     n0 = wb.wbmm_launch_count()
