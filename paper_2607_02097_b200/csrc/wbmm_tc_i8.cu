@@ -76,31 +76,59 @@ __device__ __forceinline__ void mma_ss_i8(uint32_t d_tmem, uint64_t a_desc, uint
 }
 
 // W_c[i][j] = T[c, rel(i, j)] (Eq. 7) in the K-major core-matrix layout: value (i, j) at byte (j/16)*LBO + i*16 + j%16.
+// The table row is staged REVERSED (F[q] = T[NB-1-q]): then rel(i, j) reads F at (w-1-ri+rj)*(2w-1) + (w-1-ci+cj), which
+// is one per-thread base plus a compile-time constant of j -- thread i builds row i, all K chunks unrolled, two
+// instructions per byte.  Rows i >= N and columns j >= N are zero.
 template <int WS>
 __device__ __forceinline__ void build_weight_i8(const int8_t* __restrict__ Tc, uint8_t* Ts, uint8_t* Wc, int tid)
 {
     using Cf = I8Cfg<WS>;
-    for (int k = tid; k < Cf::NB; k += kThreadsI) Ts[k] = (uint8_t)Tc[k];
+    for (int k = tid; k < Cf::NB; k += kThreadsI) Ts[k] = (uint8_t)Tc[Cf::NB - 1 - k];
     __syncthreads();
-    constexpr int NCHUNK = (Cf::K_PAD / 16) * Cf::N_PAD;
-    for (int id = tid; id < NCHUNK; id += kThreadsI) {
-        const int kc = id / Cf::N_PAD, i = id % Cf::N_PAD;
-        uint32_t pk[4] = {0u, 0u, 0u, 0u};
-        if (i < Cf::N) {
-            const int ri = i / WS, ci = i % WS;
-            int j = kc * 16;
-            int rj = j / WS, cj = j % WS;
+    if (tid < Cf::N_PAD) {
+        const int i = tid;
+        const int ri = i / WS, ci = i % WS;
+        const uint8_t* f = Ts + (i < Cf::N ? (WS - 1 - ri) * Cf::TW + (WS - 1 - ci) : 0);
 #pragma unroll
-            for (int e = 0; e < 16; ++e) {
-                uint32_t v = 0;
-                if (j < Cf::N) v = Ts[(ri - rj + WS - 1) * Cf::TW + (ci - cj + WS - 1)];
-                pk[e >> 2] |= v << ((e & 3) * 8);
-                ++j;
-                if (++cj == WS) { cj = 0; ++rj; }
+        for (int kc = 0; kc < Cf::K_PAD / 16; ++kc) {
+            uint32_t pk[4] = {0u, 0u, 0u, 0u};
+            if (i < Cf::N) {
+#pragma unroll
+                for (int e = 0; e < 16; ++e) {
+                    const int j = kc * 16 + e;
+                    if (j < Cf::N) pk[e >> 2] |= (uint32_t)f[(j / WS) * Cf::TW + (j % WS)] << ((e & 3) * 8);
+                }
             }
+            *reinterpret_cast<uint4*>(Wc + kc * Cf::LBO + i * 16) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
         }
-        *reinterpret_cast<uint4*>(Wc + kc * Cf::LBO + i * 16) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
     }
+}
+
+// Bytes [16*KC0, 16*KC1) of a window (row-major order) from the frame into row m of the A tile, 16 bytes per K chunk.
+template <int WS, int KC0, int KC1>
+__device__ __forceinline__ void stage_window_i8(const uint8_t* win, int rowB, uint8_t* arow)
+{
+    using Cf = I8Cfg<WS>;
+    constexpr int NV = (KC1 - KC0) * 4;
+    uint32_t v[NV];
+#pragma unroll
+    for (int k = 0; k < NV; ++k) v[k] = 0u;
+    if constexpr (WS % 2 == 0) {
+#pragma unroll
+        for (int h = KC0 * 8; h < KC1 * 8; ++h)          // halfword h = bytes 2h, 2h+1 (a row is WS/2 aligned halfwords)
+            if (2 * h < Cf::N) {
+                const uint32_t u = *reinterpret_cast<const uint16_t*>(win + (h / (WS / 2)) * rowB + 2 * (h % (WS / 2)));
+                v[(h >> 1) - KC0 * 4] |= u << ((h & 1) * 16);
+            }
+    } else {
+#pragma unroll
+        for (int b = KC0 * 16; b < KC1 * 16; ++b)
+            if (b < Cf::N) v[(b >> 2) - KC0 * 4] |= (uint32_t)win[(b / WS) * rowB + (b % WS)] << ((b & 3) * 8);
+    }
+#pragma unroll
+    for (int kc = KC0; kc < KC1; ++kc)
+        *reinterpret_cast<uint4*>(arow + kc * Cf::A_LBO) =
+            make_uint4(v[4 * (kc - KC0)], v[4 * (kc - KC0) + 1], v[4 * (kc - KC0) + 2], v[4 * (kc - KC0) + 3]);
 }
 
 // Window -> TMEM A (warp-collective): the N bytes in row-major order, four per column; lanes without a window and
@@ -139,12 +167,19 @@ __device__ __forceinline__ void window_to_tmem_i8(const uint8_t* win, bool valid
     ptx::tmem_wait_st();
 }
 
+// q = sat_s8(rne(fp32(sum) * scale)) without the conversion unit (I2F / F2I issue at a quarter of the FP32 rate and were
+// the floor of the epilogue): |sum| <= 196 * 128 * 128 < 2^22, so  fp32(sum) = as_float(0x4B400000 + sum) - 1.5 * 2^23
+// exactly; one binary32 product (no fma); clamping to [-128, 127] BEFORE rounding gives the same integer as after
+// (the bounds are integers, rounding is monotone); adding 1.5 * 2^23 rounds to the nearest integer, ties to even, and
+// leaves the two's-complement value in the low mantissa bits.  The low byte of the result is q.
 __device__ __forceinline__ uint32_t requant(uint32_t acc_bits, float scale)
 {
-    const float r = __fmul_rn(__int2float_rn((int)acc_bits), scale);   // binary32 conversion and ONE product (no fma)
-    const int q = __float2int_rn(r);                                   // ties to even; saturates at the int32 range
-    return (uint32_t)min(127, max(-128, q)) & 0xffu;
+    const float f = __fsub_rn(__uint_as_float(0x4B400000u + acc_bits), 12582912.0f);
+    float r = __fmul_rn(f, scale);
+    r = fminf(fmaxf(r, -128.0f), 127.0f);
+    return __float_as_uint(__fadd_rn(r, 12582912.0f));
 }
+__device__ __forceinline__ uint32_t pack_q2(uint32_t a, uint32_t b) { return __byte_perm(a, b, 0x0040) & 0xffffu; }
 
 template <int WS, bool OUT8>
 __global__ void __launch_bounds__(kThreadsI, 1)
@@ -288,7 +323,7 @@ tc_i8_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t* __r
                             } else if constexpr (WS % 2 == 0) {
                                 if ((k & 1) == 0)   // (i and i+1 are in the same chunk: 16 and WS are even)
                                     *reinterpret_cast<uint16_t*>(win + r * rowB + k) =
-                                        (uint16_t)(requant(v[e], sc) | (requant(v[e + 1], sc) << 8));
+                                        (uint16_t)pack_q2(requant(v[e], sc), requant(v[e + 1], sc));
                             } else {
                                 win[r * rowB + k] = (uint8_t)requant(v[e], sc);
                             }
@@ -338,7 +373,8 @@ tc_i8_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t* __r
 // so that tensor memory holds D only (208 columns at w = 14 -> 256 allocated): two CTAs share an SM (three at w = 7)
 // and fill each other's barrier waits.  Per tile:
 //   wait full | windows: frame -> registers -> A (16-byte chunks, conflict-free) | sync | load of tile t+1 starts
-//   7 (w = 14) / 2 (w = 7) MMAs | tcgen05.ld -> requantise -> output planes (over the A tile) | sync | bulk stores
+//   7 (w = 14) / 2 (w = 7) MMAs | tcgen05.ld -> requantise -> output planes (over the A tile) | sync | 16-byte stores
+// (A bulk store would have to be waited for before the next A tile overwrites its source: measured 2.5 us per tile.)
 template <int WS, bool OUT8>
 constexpr int i8_ctas() { return WS == 7 ? 3 : (OUT8 ? 2 : 1); }
 
@@ -424,33 +460,12 @@ tc_i8_bulk_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t
             cur_c = q.c;
         }
         ptx::mbar_wait(full_bar, phase);
-        if (warp < 4) {
-            // this thread's window -> registers (row-major bytes, four per word) -> row m of A, 16 bytes per K chunk
-            constexpr int NV = Cf::K_PAD / 4;
-            uint32_t v[NV];
-#pragma unroll
-            for (int k = 0; k < NV; ++k) v[k] = 0u;
-            if constexpr (WS % 2 == 0) {
-#pragma unroll
-                for (int r = 0; r < WS; ++r)
-#pragma unroll
-                    for (int k = 0; k < WS / 2; ++k) {
-                        const int h = r * (WS / 2) + k;
-                        const uint32_t u = *reinterpret_cast<const uint16_t*>(win + r * rowB + 2 * k);
-                        v[h >> 1] |= u << ((h & 1) * 16);
-                    }
-            } else {
-#pragma unroll
-                for (int r = 0; r < WS; ++r)
-#pragma unroll
-                    for (int k = 0; k < WS; ++k) {
-                        const int h = r * WS + k;
-                        v[h >> 2] |= (uint32_t)win[r * rowB + k] << ((h & 3) * 8);
-                    }
-            }
-#pragma unroll
-            for (int kc = 0; kc < Cf::K_PAD / 16; ++kc)
-                *reinterpret_cast<uint4*>(ao + kc * Cf::A_LBO + m * 16) = make_uint4(v[4 * kc], v[4 * kc + 1], v[4 * kc + 2], v[4 * kc + 3]);
+        // this thread's window -> registers (row-major bytes, four per word) -> row m of A; warps 0-3 take the first
+        // half of the K chunks, warps 4-7 the rest
+        {
+            constexpr int KCH = (Cf::K_PAD / 16 + 1) / 2;
+            if (warp < 4) stage_window_i8<WS, 0, KCH>(win, rowB, ao + m * 16);
+            else stage_window_i8<WS, KCH, Cf::K_PAD / 16>(win, rowB, ao + m * 16);
         }
         ptx::fence_proxy_async_smem();   // A and W_c (generic-proxy stores) -> tcgen05.mma operand reads
         __syncthreads();                 // the frame has been read: the next tile may land in it
@@ -469,13 +484,15 @@ tc_i8_bulk_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t
         ptx::mbar_wait(mma_bar, phase);
         phase ^= 1;
         ptx::tc_fence_after_sync();
-        if (warp < 4) {
+        {   // all 8 warps: warp w and warp w+4 share the TMEM lanes of windows 32(w%4) .. +31 and take half the columns each
             const bool valid = in_frame && pl < q.np && q.wy0 + wyl < g.nwh;
-            const uint32_t td = tmem_d + ((uint32_t)(warp * 32) << 16);
+            const uint32_t td = tmem_d + ((uint32_t)((warp & 3) * 32) << 16);
             const float sc = OUT8 ? scale[q.c] : 0.f;
             uint8_t* owin = ao + pl * So + win_off * (OUT8 ? 1 : 4);
+            constexpr int NCH = Cf::N_PAD / 16, CH_SPLIT = (NCH + 1) / 2;
 #pragma unroll
-            for (int ch = 0; ch < Cf::N_PAD / 16; ++ch) {
+            for (int ch = 0; ch < NCH; ++ch) {
+                if ((ch < CH_SPLIT) != (warp < 4)) continue;
                 uint32_t v[16];
                 ptx::tmem_ld16(td + ch * 16, v);
                 ptx::tmem_wait_ld();
@@ -490,7 +507,7 @@ tc_i8_bulk_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t
                             } else if constexpr (WS % 2 == 0) {
                                 if ((k & 1) == 0)
                                     *reinterpret_cast<uint16_t*>(owin + r * rowB + k) =
-                                        (uint16_t)(requant(v[e], sc) | (requant(v[e + 1], sc) << 8));
+                                        (uint16_t)pack_q2(requant(v[e], sc), requant(v[e + 1], sc));
                             } else {
                                 owin[r * rowB + k] = (uint8_t)requant(v[e], sc);
                             }
@@ -500,19 +517,30 @@ tc_i8_bulk_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t
             }
             ptx::tc_fence_before_sync();
         }
-        ptx::fence_proxy_async_smem();   // output planes (generic-proxy stores) -> bulk-copy reads
         __syncthreads();
-        if (tid == 0) {
+        {   // output planes -> y: every plane strip is one 16-byte aligned run; all threads, 16 bytes each
             constexpr int ES = OUT8 ? 1 : 4;
             uint8_t* dst = static_cast<uint8_t*>(yv) + (((long long)q.b0 * g.C + q.c) * plane + (long long)q.wy0 * WS * g.W) * ES;
-            for (int p = 0; p < q.np; ++p)
-                ptx::bulk_s2g(dst + (long long)p * g.C * plane * ES, ptx::smem_u32(ao + p * So), (uint32_t)(q.bytes * ES));
-            ptx::bulk_commit();
-            ptx::bulk_wait_read<0>();    // the A tile of the next iteration overwrites these planes
+            const int per = q.bytes * ES / 16;                  // 16-byte units per plane strip
+            const long long dpitch = (long long)g.C * plane * ES;
+            int p = tid / per, off = tid - p * per;              // unit `off` of plane p; advanced by 256 units per step
+            while (p < q.np) {
+                uint4 val[4];
+                int pp[4], oo[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    pp[u] = p; oo[u] = off;
+                    if (p < q.np) val[u] = *reinterpret_cast<const uint4*>(ao + p * So + off * 16);
+                    off += kThreadsI;
+                    while (off >= per) { off -= per; ++p; }
+                }
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+                    if (pp[u] < q.np) *reinterpret_cast<uint4*>(dst + pp[u] * dpitch + oo[u] * 16) = val[u];
+            }
         }
-        __syncthreads();
+        __syncthreads();   // the A tile of the next iteration overwrites these planes
     }
-    if (tid == 0) ptx::bulk_wait_all<0>();
     ptx::tc_fence_before_sync();
     __syncthreads();
     if (warp == 0) ptx::tmem_dealloc(tmem_d, Cf::D_COLS_ALLOC);
