@@ -180,6 +180,23 @@ __device__ __forceinline__ uint32_t requant(uint32_t acc_bits, float scale)
     return __float_as_uint(__fadd_rn(r, 12582912.0f));
 }
 __device__ __forceinline__ uint32_t pack_q2(uint32_t a, uint32_t b) { return __byte_perm(a, b, 0x0040) & 0xffffu; }
+// Two values at once with the packed binary32 instructions of sm_100 (sub / mul / add .f32x2: each lane is the scalar
+// operation, same rounding); returns q(a0) | q(a1) << 8.
+__device__ __forceinline__ uint64_t pack_f2(float lo, float hi)
+{
+    return (uint64_t)__float_as_uint(lo) | ((uint64_t)__float_as_uint(hi) << 32);
+}
+__device__ __forceinline__ uint32_t requant2(uint32_t a0, uint32_t a1, uint64_t scale2)
+{
+    const uint64_t magic2 = pack_f2(12582912.0f, 12582912.0f);
+    uint64_t x = (uint64_t)(0x4B400000u + a0) | ((uint64_t)(0x4B400000u + a1) << 32);
+    asm("sub.rn.f32x2 %0, %0, %1;\n\tmul.rn.f32x2 %0, %0, %2;" : "+l"(x) : "l"(magic2), "l"(scale2));
+    const float r0 = fminf(fmaxf(__uint_as_float((uint32_t)x), -128.0f), 127.0f);
+    const float r1 = fminf(fmaxf(__uint_as_float((uint32_t)(x >> 32)), -128.0f), 127.0f);
+    uint64_t t = pack_f2(r0, r1);
+    asm("add.rn.f32x2 %0, %0, %1;" : "+l"(t) : "l"(magic2));
+    return __byte_perm((uint32_t)t, (uint32_t)(t >> 32), 0x0040) & 0xffffu;
+}
 
 template <int WS, bool OUT8>
 __global__ void __launch_bounds__(kThreadsI, 1)
@@ -488,6 +505,7 @@ tc_i8_bulk_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t
             const bool valid = in_frame && pl < q.np && q.wy0 + wyl < g.nwh;
             const uint32_t td = tmem_d + ((uint32_t)((warp & 3) * 32) << 16);
             const float sc = OUT8 ? scale[q.c] : 0.f;
+            const uint64_t sc2 = pack_f2(sc, sc);
             uint8_t* owin = ao + pl * So + win_off * (OUT8 ? 1 : 4);
             constexpr int NCH = Cf::N_PAD / 16, CH_SPLIT = (NCH + 1) / 2;
 #pragma unroll
@@ -506,8 +524,7 @@ tc_i8_bulk_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t
                                 *reinterpret_cast<uint32_t*>(owin + (r * rowB + k) * 4) = v[e];
                             } else if constexpr (WS % 2 == 0) {
                                 if ((k & 1) == 0)
-                                    *reinterpret_cast<uint16_t*>(owin + r * rowB + k) =
-                                        (uint16_t)pack_q2(requant(v[e], sc), requant(v[e + 1], sc));
+                                    *reinterpret_cast<uint16_t*>(owin + r * rowB + k) = (uint16_t)requant2(v[e], v[e + 1], sc2);
                             } else {
                                 owin[r * rowB + k] = (uint8_t)requant(v[e], sc);
                             }
@@ -523,20 +540,18 @@ tc_i8_bulk_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t
             uint8_t* dst = static_cast<uint8_t*>(yv) + (((long long)q.b0 * g.C + q.c) * plane + (long long)q.wy0 * WS * g.W) * ES;
             const int per = q.bytes * ES / 16;                  // 16-byte units per plane strip
             const long long dpitch = (long long)g.C * plane * ES;
-            int p = tid / per, off = tid - p * per;              // unit `off` of plane p; advanced by 256 units per step
-            while (p < q.np) {
-                uint4 val[4];
-                int pp[4], oo[4];
+            for (int p = warp; p < q.np; p += kThreadsI / 32) {    // a warp per plane, four units in flight per lane
+                const uint8_t* sp = ao + p * So;
+                uint8_t* dp = dst + p * dpitch;
+                for (int o = lane; o < per; o += 128) {
+                    uint4 val[4];
 #pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    pp[u] = p; oo[u] = off;
-                    if (p < q.np) val[u] = *reinterpret_cast<const uint4*>(ao + p * So + off * 16);
-                    off += kThreadsI;
-                    while (off >= per) { off -= per; ++p; }
+                    for (int u = 0; u < 4; ++u)
+                        if (o + 32 * u < per) val[u] = *reinterpret_cast<const uint4*>(sp + (o + 32 * u) * 16);
+#pragma unroll
+                    for (int u = 0; u < 4; ++u)
+                        if (o + 32 * u < per) *reinterpret_cast<uint4*>(dp + (o + 32 * u) * 16) = val[u];
                 }
-#pragma unroll
-                for (int u = 0; u < 4; ++u)
-                    if (pp[u] < q.np) *reinterpret_cast<uint4*>(dst + pp[u] * dpitch + oo[u] * 16) = val[u];
             }
         }
         __syncthreads();   // the A tile of the next iteration overwrites these planes
