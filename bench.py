@@ -378,6 +378,24 @@ def other_rooflines(wb, dev, stream, hbm_peak):
     del dr, Tr, yr
     torch.cuda.empty_cache()
 
+    # INT8 forward (tcgen05 kind::i8, section 7.11 of DESIGN.md) on the shapes of configs 3 and 2: int8 in, int8 out
+    # (requantised): 2 bytes per element of algorithmic traffic; int32 out: 5 bytes
+    for name, ci in (("int8_B128_C96_56x56_w14_fwd", si.with_(si.CFG3, backward=False)), ("int8_B128_C96_56x56_w7_fwd", si.with_(si.CFG2, backward=False))):
+        d8 = si.make_int8(ci, device=dev)
+        ns = buffer_sets(2.0 * ci.n_elem)
+        xs = [d8["x"]] + [d8["x"].clone() for _ in range(ns - 1)]
+        y8 = [torch.empty_like(d8["x"]) for _ in range(ns)]
+        ms = region_ms_rot(lambda i: wb.wbmm_forward_int8(xs[i % ns], d8["T"], ci.w, scale=d8["scale"], out=y8[i % ns]), 30, stream)
+        by8 = 2.0 * ci.n_elem + ci.C * ci.bins + 4 * ci.C
+        out[name] = {"ms": round(ms, 5), "gbs": round(by8 / ms / 1e6, 1), "frac": round(by8 / (hbm_peak * 1e9) * 1e3 / ms, 4),
+                     "tops": round(2.0 * ci.w * ci.w * ci.n_elem / ms / 1e9, 2), "path": wb.wbmm_path_string(wb.wbmm_last_path()),
+                     "buffer_sets": ns}
+        y32 = [torch.empty(d8["x"].shape, dtype=torch.int32, device=dev) for _ in range(2)]
+        ms = region_ms_rot(lambda i: wb.wbmm_forward_int8(xs[i % ns], d8["T"], ci.w, out=y32[i % 2]), 10, stream)
+        out[name.replace("_fwd", "_fwd_int32_out")] = {"ms": round(ms, 5), "frac": round((5.0 * ci.n_elem) / (hbm_peak * 1e9) * 1e3 / ms, 4)}
+        del xs, y8, y32, d8
+        torch.cuda.empty_cache()
+
     # table gradient at w = 7 (two CTAs per SM) on the config-2 shape
     c2 = si.with_(si.CFG2, backward=True)
     d = si.make(c2, device=dev)
@@ -762,6 +780,7 @@ PROFILE_CASES = {
     "B64_C96_30x30_w14_fwd": (si.Case("r30", 64, 96, 30, 30, 14, seed=92), "fwd"),
     "cfg2_shape_dT": (si.with_(si.CFG2, backward=True), "dT"),
     "nhwc_cfg2_shape_B128_fwd": (si.Case("nhwc_w7", 128, 96, 56, 56, 7, layout=si.NHWC, seed=87), "fwd"),
+    "int8_w14_fwd": (si.with_(si.CFG3, backward=False), "int8"), "int8_w7_fwd": (si.with_(si.CFG2, backward=False), "int8"),
 }
 
 
@@ -771,6 +790,14 @@ def run_profile_case(name: str):
     import paper_2607_02097_b200 as wb
     case, op = PROFILE_CASES[name]
     torch.cuda.set_device(0)
+    if op == "int8":
+        d = si.make_int8(case, device="cuda")
+        y = torch.empty_like(d["x"])
+        for _ in range(5):
+            wb.wbmm_forward_int8(d["x"], d["T"], case.w, scale=d["scale"], out=y)
+        torch.cuda.synchronize()
+        print(json.dumps({"profile_case": name, "op": op, "path": wb.wbmm_path_string(wb.wbmm_last_path())}))
+        return
     d = si.make(case, device="cuda")
     y = torch.empty_like(d["x"])
     dT = torch.empty((case.C, case.bins), dtype=torch.float32, device="cuda")
