@@ -380,7 +380,8 @@ def other_rooflines(wb, dev, stream, hbm_peak):
 
     # INT8 forward (tcgen05 kind::i8, section 7.11 of DESIGN.md) on the shapes of configs 3 and 2: int8 in, int8 out
     # (requantised): 2 bytes per element of algorithmic traffic; int32 out: 5 bytes
-    for name, ci in (("int8_B128_C96_56x56_w14_fwd", si.with_(si.CFG3, backward=False)), ("int8_B128_C96_56x56_w7_fwd", si.with_(si.CFG2, backward=False))):
+    for ci in (si.with_(si.CFG3, backward=False), si.with_(si.CFG2, backward=False)):
+        name = f"int8_B{ci.B}_C{ci.C}_{ci.H}x{ci.W}_w{ci.w}_fwd"
         d8 = si.make_int8(ci, device=dev)
         ns = buffer_sets(2.0 * ci.n_elem)
         xs = [d8["x"]] + [d8["x"].clone() for _ in range(ns - 1)]

@@ -309,7 +309,7 @@ def wbmm_forward_matrix(x: torch.Tensor, M: torch.Tensor, w: int, shift=(0, 0), 
 
 
 def wbmm_forward_int8(x: torch.Tensor, T: torch.Tensor, w: int, shift=(0, 0), layout: int = NCHW,
-                      scale: Optional[torch.Tensor] = None, out: Optional[torch.Tensor] = None) -> torch.Tensor:
+                      scale: Optional[torch.Tensor] = None, out: Optional[torch.Tensor] = None, flags: int = 0) -> torch.Tensor:
     """INT8 forward with exact int32 sums; scale [C] float32 requantises to int8 (include/wbmm.h: wbmm_forward_int8)."""
     if x.dtype != torch.int8 or T.dtype != torch.int8:
         raise TypeError("x and T must be int8")
@@ -318,7 +318,7 @@ def wbmm_forward_int8(x: torch.Tensor, T: torch.Tensor, w: int, shift=(0, 0), la
         raise ValueError("T must be [C, (2w-1)^2]")
     if scale is not None and (scale.dtype != torch.float32 or tuple(scale.shape) != (C,)):
         raise ValueError("scale must be float32 [C]")
-    d = WbmmDesc(B, C, H, W, int(w), int(shift[0]), int(shift[1]), DTYPE_F32, int(layout), 0)
+    d = WbmmDesc(B, C, H, W, int(w), int(shift[0]), int(shift[1]), DTYPE_F32, int(layout), int(flags))
     odt = torch.int32 if scale is None else torch.int8
     y = torch.empty(x.shape, dtype=odt, device=x.device) if out is None else out
     if y.dtype != odt or y.shape != x.shape:

@@ -73,6 +73,9 @@ cudaError_t transpose16(const void* in, void* out, int batch, int R, int Cc, cud
 // ... and of 32-bit elements (R and Cc multiples of 4).
 bool transpose32_supported(long long R, long long Cc, const void* in, const void* out);
 cudaError_t transpose32(const void* in, void* out, int batch, int R, int Cc, cudaStream_t stream, int* launches);
+// ... and of 8-bit elements (R and Cc multiples of 16).
+bool transpose8_supported(long long R, long long Cc, const void* in, const void* out);
+cudaError_t transpose8(const void* in, void* out, int batch, int R, int Cc, cudaStream_t stream, int* launches);
 // Largest window the SIMT kernels can stage in shared memory for this layout.
 bool simt_supported(const Geom& g);
 // Rectangular windows w_h x w_w (wbmm_rect.cu): d.w is w_h, `ww` is w_w; shifts in [0, w_h) x [0, w_w).

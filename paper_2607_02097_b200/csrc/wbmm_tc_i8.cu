@@ -623,10 +623,11 @@ bool tc_i8_supported(const Geom& g)
 }
 
 cudaError_t tc_i8_forward(const Geom& g, const int8_t* x, const int8_t* T, const float* scale, void* y, cudaStream_t stream,
-                          int* launches)
+                          int* launches, int* path)
 {
     I8Tiles tl;
     if (!i8_tiles(g, x, y, scale != nullptr, &tl)) return cudaErrorInvalidValue;
+    *path = tl.bulk ? WBMM_PATH_TC_TMA : WBMM_PATH_TC_GATHER;
     if (tl.ntiles == 0) return cudaSuccess;
     if (g.w == 14) return scale ? launch_i8<14, true>(g, tl, x, T, scale, y, stream, launches)
                                 : launch_i8<14, false>(g, tl, x, T, scale, y, stream, launches);

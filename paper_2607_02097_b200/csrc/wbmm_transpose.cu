@@ -72,7 +72,53 @@ __global__ void __launch_bounds__(256) transpose32_kernel(const uint32_t* __rest
     }
 }
 
+// The same for 8-bit elements (INT8 activations): 64 x 64 tiles, 16-byte global accesses both ways.
+__global__ void __launch_bounds__(256) transpose8_kernel(const uint8_t* __restrict__ in, uint8_t* __restrict__ out, int R, int Cc)
+{
+    constexpr int kP = 68;                       // tile row pitch in bytes (17 words)
+    __shared__ __align__(16) uint8_t tileT[64 * kP];   // [c][r]
+    const long long base = (long long)blockIdx.z * R * Cc;
+    const int r0 = blockIdx.y * 64, c0 = blockIdx.x * 64;
+    const int t = threadIdx.x;
+    {
+        const int r = t >> 2, ch = (t & 3) * 16;
+        if (r0 + r < R && c0 + ch < Cc) {
+            const uint4 v = __ldg(reinterpret_cast<const uint4*>(in + base + (long long)(r0 + r) * Cc + c0 + ch));
+            const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+            for (int k = 0; k < 16; ++k) tileT[(ch + k) * kP + r] = (uint8_t)(w[k >> 2] >> ((k & 3) * 8));
+        }
+    }
+    __syncthreads();
+    {
+        const int c = t >> 2, r16 = (t & 3) * 16;
+        if (c0 + c < Cc && r0 + r16 < R) {
+            const uint32_t* src = reinterpret_cast<const uint32_t*>(tileT + c * kP + r16);
+            *reinterpret_cast<uint4*>(out + base + (long long)(c0 + c) * R + r0 + r16) = make_uint4(src[0], src[1], src[2], src[3]);
+        }
+    }
+}
+
 }  // namespace
+
+bool transpose8_supported(long long R, long long Cc, const void* in, const void* out)
+{
+    return R % 16 == 0 && Cc % 16 == 0 && R <= 0x7fffffff && Cc <= 0x7fffffff &&
+           reinterpret_cast<uintptr_t>(in) % 16 == 0 && reinterpret_cast<uintptr_t>(out) % 16 == 0;
+}
+
+cudaError_t transpose8(const void* in, void* out, int batch, int R, int Cc, cudaStream_t stream, int* launches)
+{
+    if (batch == 0 || R == 0 || Cc == 0) return cudaSuccess;
+    for (int b0 = 0; b0 < batch; b0 += 65535) {          // gridDim.z limit
+        const int nb = batch - b0 < 65535 ? batch - b0 : 65535;
+        dim3 grid((Cc + 63) / 64, (R + 63) / 64, nb);
+        const long long off = (long long)b0 * R * Cc;
+        transpose8_kernel<<<grid, 256, 0, stream>>>((const uint8_t*)in + off, (uint8_t*)out + off, R, Cc);
+        *launches += 1;
+    }
+    return cudaGetLastError();
+}
 
 bool transpose32_supported(long long R, long long Cc, const void* in, const void* out)
 {

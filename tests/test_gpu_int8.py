@@ -33,6 +33,9 @@ CASES = [
     si.Case("i8_w7_one_window", 131, 3, 7, 7, 7, seed=811),
     si.Case("i8_w7_wide", 1, 2, 7, 896, 7, seed=812),                                 # 128 windows across
     si.Case("i8_odd_width", 2, 3, 28, 54, 14, seed=813),                              # W' != W: byte copies
+    si.Case("i8_w14_nhwc_t", 5, 32, 28, 56, 14, layout=NHWC, seed=814),               # NHWC through the transposition route
+    si.Case("i8_w14_nhwc_t_shift", 3, 96, 56, 56, 14, shift=(7, 5), layout=NHWC, seed=815),
+    si.Case("i8_w7_nhwc_t", 4, 80, 28, 28, 7, layout=NHWC, seed=816),                 # C = 64 + 16: a partial tile
 ]
 
 
@@ -44,7 +47,11 @@ def test_int8_forward_bit_exact(wb, oracle, case, extreme):
     want32 = oracle.forward_int8(xh, Th, case.w, case.shift, case.layout)
     out = torch.full(d["x"].shape, -77, dtype=torch.int32, device="cuda")
     y32 = wb.wbmm_forward_int8(d["x"], d["T"], case.w, case.shift, case.layout, out=out)
-    assert wb.wbmm_last_path() == wb.PATH_TC_GATHER
+    assert wb.wbmm_last_path() in (wb.PATH_TC_GATHER, wb.PATH_TC_TMA, wb.PATH_TC_TRANSPOSED)
+    if case.name.startswith("i8_w14_nhwc_t") or case.name == "i8_w7_nhwc_t":
+        assert wb.wbmm_last_path() == wb.PATH_TC_TRANSPOSED
+        yn = wb.wbmm_forward_int8(d["x"], d["T"], case.w, case.shift, case.layout, flags=wb.FLAG_NO_SCRATCH)
+        assert wb.wbmm_last_path() == wb.PATH_TC_GATHER and np.array_equal(yn.cpu().numpy(), want32)
     assert np.array_equal(y32.cpu().numpy(), want32), case.name
     want8 = oracle.forward_int8(xh, Th, case.w, case.shift, case.layout, scale=sh)
     y8 = wb.wbmm_forward_int8(d["x"], d["T"], case.w, case.shift, case.layout, scale=d["scale"])
@@ -111,6 +118,7 @@ def test_int8_pointer_alignment_picks_a_kernel_that_fits(wb, oracle, off):
     want = oracle.forward_int8(d["x"].cpu().numpy(), d["T"].cpu().numpy(), case.w, scale=d["scale"].cpu().numpy())
     assert np.array_equal(ys.cpu().numpy(), want)
     assert bool((yb[:off] == 55).all()) and bool((yb[off + n:] == 55).all())
+    assert wb.wbmm_last_path() == (wb.PATH_TC_TMA if off % 16 == 0 else wb.PATH_TC_GATHER)
     y32 = wb.wbmm_forward_int8(xs, d["T"], case.w)
     assert np.array_equal(y32.cpu().numpy(), oracle.forward_int8(d["x"].cpu().numpy(), d["T"].cpu().numpy(), case.w))
 
