@@ -190,6 +190,31 @@ def forward_int8(x, T, w, shift=(0, 0), layout=NCHW, scale=None) -> np.ndarray:
     return y
 
 
+def e4m3_decode(codes) -> np.ndarray:
+    """FP8 E4M3 ("fn" flavour: no infinities, 0x7f / 0xff are NaN; bias 7) byte codes -> float64, from the format's
+    definition: sign (1) | exponent (4) | mantissa (3); exponent 0: subnormal m/8 * 2^-6; else (1 + m/8) * 2^(e-7)."""
+    c = np.asarray(codes).astype(np.uint8).astype(np.int64)
+    sign = np.where(c & 0x80, -1.0, 1.0)
+    e = (c >> 3) & 0xF
+    m = (c & 0x7).astype(np.float64)
+    val = np.where(e == 0, m / 8.0 * 2.0 ** -6, (1.0 + m / 8.0) * np.exp2((e - 7).astype(np.float64)))
+    val = np.where((e == 15) & ((c & 7) == 7), np.nan, val)
+    return sign * val
+
+
+def forward_fp8(x_codes, T_codes, w, shift=(0, 0), layout=NCHW, scale=None) -> np.ndarray:
+    """FP8 (E4M3) forward, NEXT-4: the operator of `forward` on the decoded values, in float64 (every product of two
+    E4M3 numbers and every sum of w*w of them is exact in float64), times scale[c] when given.  What the kernel stores
+    (float32 sums, or E4M3 codes of sum * scale) is compared against THIS real number: DESIGN.md reading A22."""
+    x = e4m3_decode(x_codes)
+    T = e4m3_decode(T_codes)
+    y = forward(x, T, w, shift, layout, form="direct")
+    if scale is not None:
+        sc = np.asarray(scale, dtype=np.float64)
+        y = y * (sc[None, :, None, None] if layout == NCHW else sc[None, None, None, :])
+    return y
+
+
 def backward_rect(x, T, dy, wh, ww, shift=(0, 0), layout=NCHW, need_dx=True, need_dT=True):
     """(dx, dT) of forward_rect in float64; either is None when not requested."""
     x, xp = _d(x)

@@ -784,3 +784,37 @@ def test_int8_requantisation_uses_binary32_products(oracle):
         q = int(oracle.forward_int8(x, T, w, scale=np.array([sc], dtype=np.float32))[0, 0, 7, 7])
         want = int(np.clip(np.rint(np.float32(np.float32(s) * sc)), -128, 127))
         assert q == want, (sc, q, want)
+
+
+# ----------------------------------------------------------------------------- NEXT-4: FP8 (E4M3) decode
+def test_e4m3_decode_matches_the_format_and_the_library(oracle):
+    """All 256 codes against torch's float8_e4m3fn conversion (a library routine) and the facts of the format: 0x38 = 1,
+    largest finite 448 (0x7e), smallest subnormal 2^-9 (0x01), 0x7f / 0xff NaN, 0x80 = -0.
+    Catches: wrong bias, subnormals treated as normals, the 'fnuz' or IEEE-like flavour with infinities."""
+    codes = np.arange(256, dtype=np.uint8)
+    got = oracle.e4m3_decode(codes)
+    lib = torch.from_numpy(codes.copy()).view(torch.float8_e4m3fn).to(torch.float64).numpy()
+    assert np.array_equal(np.isnan(got), np.isnan(lib)) and np.array_equal(got[~np.isnan(got)], lib[~np.isnan(lib)])
+    assert got[0x38] == 1.0 and got[0x7e] == 448.0 and got[0x01] == 2.0 ** -9 and got[0x08] == 2.0 ** -6
+    assert np.isnan(got[0x7f]) and np.isnan(got[0xff]) and got[0x80] == 0.0 and np.signbit(got[0x80])
+    assert got[0xb8] == -1.0 and got[0x3c] == 1.5
+
+
+def test_fp8_forward_is_the_operator_on_decoded_values(oracle):
+    """Identity table (code 0x38 = 1.0 at the centre bin) returns the decoded input; an all-ones table the window sums.
+    Catches: codes used as integers, scale applied to the wrong axis in NHWC."""
+    r = rng(900)
+    w = 4
+    codes = r.integers(0, 256, (2, 3, 8, 8)).astype(np.uint8)
+    codes[(codes & 0x7f) == 0x7f] = 0x38                      # no NaN
+    T = np.zeros((3, 49), dtype=np.uint8)
+    T[:, 24] = 0x38
+    x = oracle.e4m3_decode(codes)
+    assert np.array_equal(oracle.forward_fp8(codes, T, w), x)
+    T1 = np.full((3, 49), 0x38, dtype=np.uint8)
+    y = oracle.forward_fp8(codes, T1, w)
+    want = x.reshape(2, 3, 2, 4, 2, 4).sum(axis=(3, 5), keepdims=True).repeat(4, axis=3).repeat(4, axis=5).reshape(2, 3, 8, 8)
+    assert np.array_equal(y, want)
+    sc = np.array([0.5, 2.0, -1.0])
+    yn = oracle.forward_fp8(np.ascontiguousarray(codes.transpose(0, 2, 3, 1)), T1, w, layout=NHWC, scale=sc)
+    assert np.array_equal(yn.transpose(0, 3, 1, 2), want * sc[None, :, None, None])
