@@ -264,6 +264,21 @@ WBMM_API int wbmm_forward_int8(const wbmm_desc_t *desc, const int8_t *x, const i
                       void *cuda_stream);
 
 /*
+ * FP8 forward (reading A22): Algorithm 1 on E4M3 activations and tables ("fn" flavour:
+ * bias 7, no infinities, 0x7f / 0xff NaN), products accumulated in float32 by the tensor cores (tcgen05.mma
+ * kind::f8f6f4); the kernels, routes, limits and wbmm_last_path() values of wbmm_forward_int8.
+ *   x, T  [in]  E4M3 bytes, shapes as in wbmm_forward_int8.  Inputs are assumed finite (no NaN codes).
+ *   scale [in, nullable] float32 [C], device, finite.
+ *   y     [out] scale == NULL: float32, the sums (4-byte aligned);
+ *               scale != NULL: E4M3 bytes of sum * scale[c] (one binary32 product, round-to-nearest-even, saturating
+ *               at +-448).  Every element is overwritten; y must not alias x.
+ * The float32 sums agree with the exact real sums to float32 accumulation accuracy (the tensor core's summation order
+ * is not specified); a stored code is the nearest E4M3 number to sum * scale except within that error of a midpoint.
+ */
+WBMM_API int wbmm_forward_fp8(const wbmm_desc_t *desc, const void *x, const void *T, const float *scale, void *y,
+                     void *cuda_stream);
+
+/*
  * Multi-kernel fusion for one-window maps (section 3.7): a zero-padded ksize x ksize depthwise
  * conv (Eq. 1, cross-correlation) on an H = W = w map is the WBMM operator with the conv kernel written around
  * the centre of the table, so  Y = WBMM(X) + BN1(DW5(X)) + BN2(DW3(X))  folds into ONE table plus a bias:

@@ -24,7 +24,7 @@ _DTYPES = {torch.float32: DTYPE_F32, torch.bfloat16: DTYPE_BF16, torch.float16: 
 
 # every symbol include/wbmm.h declares
 EXPORTS = (
-    "wbmm_forward", "wbmm_forward_static_scratch", "wbmm_forward_rect", "wbmm_backward_rect", "wbmm_backward", "wbmm_hier_forward", "wbmm_hier_backward", "wbmm_forward_matrix", "wbmm_forward_int8", "wbmm_fold_dwconv", "wbmm_forward_fused", "wbmm_materialize_weight", "wbmm_forward_host",
+    "wbmm_forward", "wbmm_forward_static_scratch", "wbmm_forward_rect", "wbmm_backward_rect", "wbmm_backward", "wbmm_hier_forward", "wbmm_hier_backward", "wbmm_forward_matrix", "wbmm_forward_int8", "wbmm_forward_fp8", "wbmm_fold_dwconv", "wbmm_forward_fused", "wbmm_materialize_weight", "wbmm_forward_host",
     "wbmm_backward_host", "wbmm_release", "wbmm_last_path", "wbmm_launch_count",
     "wbmm_status_string", "wbmm_path_string", "wbmm_last_error_string", "wbmm_version",
 )
@@ -71,6 +71,8 @@ def lib() -> ctypes.CDLL:
     L.wbmm_forward_matrix.restype = i
     L.wbmm_forward_int8.argtypes = [dp, vp, vp, vp, vp, vp]
     L.wbmm_forward_int8.restype = i
+    L.wbmm_forward_fp8.argtypes = [dp, vp, vp, vp, vp, vp]
+    L.wbmm_forward_fp8.restype = i
     L.wbmm_fold_dwconv.argtypes = [dp, vp, vp, i, vp, vp, vp]
     L.wbmm_fold_dwconv.restype = i
     L.wbmm_forward_fused.argtypes = [dp, vp, vp, vp, ctypes.c_float, vp, i, vp]
@@ -326,6 +328,28 @@ def wbmm_forward_int8(x: torch.Tensor, T: torch.Tensor, w: int, shift=(0, 0), la
     with torch.cuda.device(x.device):
         _check(lib().wbmm_forward_int8(ctypes.byref(d), _dev(x, "x"), _dev(T, "T"), _dev(scale, "scale"), _dev(y, "y"),
                                        _stream(x)))
+    return y
+
+
+def wbmm_forward_fp8(x: torch.Tensor, T: torch.Tensor, w: int, shift=(0, 0), layout: int = NCHW,
+                     scale: Optional[torch.Tensor] = None, out: Optional[torch.Tensor] = None, flags: int = 0) -> torch.Tensor:
+    """FP8 (E4M3) forward with float32 sums; scale [C] float32 gives E4M3 output (include/wbmm.h: wbmm_forward_fp8)."""
+    f8 = torch.float8_e4m3fn
+    if x.dtype != f8 or T.dtype != f8:
+        raise TypeError("x and T must be torch.float8_e4m3fn")
+    B, C, H, W = _dims(x, layout)
+    if tuple(T.shape) != (C, (2 * w - 1) ** 2):
+        raise ValueError("T must be [C, (2w-1)^2]")
+    if scale is not None and (scale.dtype != torch.float32 or tuple(scale.shape) != (C,)):
+        raise ValueError("scale must be float32 [C]")
+    d = WbmmDesc(B, C, H, W, int(w), int(shift[0]), int(shift[1]), DTYPE_F32, int(layout), int(flags))
+    odt = torch.float32 if scale is None else f8
+    y = torch.empty(x.shape, dtype=odt, device=x.device) if out is None else out
+    if y.dtype != odt or y.shape != x.shape:
+        raise ValueError(f"out must be {odt} with the shape of x")
+    with torch.cuda.device(x.device):
+        _check(lib().wbmm_forward_fp8(ctypes.byref(d), _dev(x, "x"), _dev(T, "T"), _dev(scale, "scale"), _dev(y, "y"),
+                                      _stream(x)))
     return y
 
 

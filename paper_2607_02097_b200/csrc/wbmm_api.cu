@@ -756,7 +756,8 @@ int wbmm_forward_matrix(const wbmm_desc_t* desc, const void* x, const void* M, c
     return WBMM_STATUS_OK;
 }
 
-int wbmm_forward_int8(const wbmm_desc_t* desc, const int8_t* x, const int8_t* T, const float* scale, void* y, void* cuda_stream)
+// INT8 / FP8 (E4M3) forward: the same kernels and routes, 8-bit elements either way.
+static int forward_8bit(const wbmm_desc_t* desc, const int8_t* x, const int8_t* T, const float* scale, void* y, void* cuda_stream, bool fp8)
 {
     if (!desc) return WBMM_STATUS_INVALID_ARGUMENT;
     wbmm_desc_t d = *desc;
@@ -770,7 +771,7 @@ int wbmm_forward_int8(const wbmm_desc_t* desc, const int8_t* x, const int8_t* T,
     wbmm::Geom g = wbmm::make_geom(d);
     if (!wbmm::tc_i8_supported(g)) {
         snprintf(t_last_error, sizeof(t_last_error),
-                 "wbmm_forward_int8: w must be 7 or 14 with at most 128 windows across (w = %d, %d windows across)", g.w, g.nww);
+                 "8-bit forward: w must be 7 or 14 with at most 128 windows across (w = %d, %d windows across)", g.w, g.nww);
         return WBMM_STATUS_UNSUPPORTED;
     }
     int launches = 0, path = WBMM_PATH_NONE;
@@ -787,7 +788,7 @@ int wbmm_forward_int8(const wbmm_desc_t* desc, const int8_t* x, const int8_t* T,
             AsyncScratch xt(stream), yt(stream);
             if (xt.alloc(n) == cudaSuccess && yt.alloc(n * (scale ? 1 : 4)) == cudaSuccess) {
                 cudaError_t e = wbmm::transpose8(x, xt.p, g.B, (int)hw, g.C, stream, &launches);
-                if (e == cudaSuccess) e = wbmm::tc_i8_forward(gn, static_cast<const int8_t*>(xt.p), T, scale, yt.p, stream, &launches, &path);
+                if (e == cudaSuccess) e = wbmm::tc_i8_forward(gn, static_cast<const int8_t*>(xt.p), T, scale, yt.p, stream, &launches, &path, fp8);
                 if (e == cudaSuccess)
                     e = scale ? wbmm::transpose8(yt.p, y, g.B, g.C, (int)hw, stream, &launches)
                               : wbmm::transpose32(yt.p, y, g.B, g.C, (int)hw, stream, &launches);
@@ -799,11 +800,21 @@ int wbmm_forward_int8(const wbmm_desc_t* desc, const int8_t* x, const int8_t* T,
             cudaGetLastError();      // no stream-ordered allocator / out of memory: the gather kernel below
         }
     }
-    cudaError_t e = wbmm::tc_i8_forward(g, x, T, scale, y, stream, &launches, &path);
+    cudaError_t e = wbmm::tc_i8_forward(g, x, T, scale, y, stream, &launches, &path, fp8);
     g_launches += launches;
     if (e != cudaSuccess) return set_cuda_error(e, "tc_i8_forward");
     t_last_path = path;
     return WBMM_STATUS_OK;
+}
+
+int wbmm_forward_int8(const wbmm_desc_t* desc, const int8_t* x, const int8_t* T, const float* scale, void* y, void* cuda_stream)
+{
+    return forward_8bit(desc, x, T, scale, y, cuda_stream, false);
+}
+
+int wbmm_forward_fp8(const wbmm_desc_t* desc, const void* x, const void* T, const float* scale, void* y, void* cuda_stream)
+{
+    return forward_8bit(desc, static_cast<const int8_t*>(x), static_cast<const int8_t*>(T), scale, y, cuda_stream, true);
 }
 
 int wbmm_fold_dwconv(const wbmm_desc_t* desc, const void* T, const void* K, int ksize, const float* scale,

@@ -72,8 +72,9 @@ bool plane_box_map(const Geom& g, int dtype, const void* base, int images, void*
 // INT8 forward on the tensor cores (wbmm_tc_i8.cu): kind::i8, exact int32 sums; scale == nullptr: y is int32, else y is
 // int8 = sat(rne(fp32(sum) * scale[c])).  w in {7, 14}, any layout / shift / ragged size with at most 128 windows across.
 bool tc_i8_supported(const Geom& g);
+// fp8: the same kernels with E4M3 operands (kind::f8f6f4, fp32 sums; scale != nullptr: y is E4M3 = rn_satfinite(sum * scale[c])).
 cudaError_t tc_i8_forward(const Geom& g, const int8_t* x, const int8_t* T, const float* scale, void* y, cudaStream_t stream,
-                          int* launches, int* path);
+                          int* launches, int* path, bool fp8 = false);
 
 // wbmm_static_scratch.cu: the NHWC transposition route with its two temporaries in a file-scope device array (no
 // allocation).  Returns 0 = served (*err holds the CUDA status), 1 = not a problem of this route, 2 = the activation

@@ -14,6 +14,8 @@
 // scatter), any layout / shift / ragged size by index arithmetic, with 32-bit copies where rows allow it.
 #include <cuda.h>
 
+#include <type_traits>
+
 #include "wbmm_common.cuh"
 #include "wbmm_ptx.cuh"
 #include "wbmm_tc.cuh"
@@ -53,26 +55,33 @@ struct I8Tiles {
     int bulk;                // plane strips are contiguous 16-byte aligned runs: the bulk-copy kernel serves (see i8_tiles)
 };
 
-__host__ __device__ constexpr uint32_t idesc_i8(int M, int N)
+// kind::i8: c_format S32 (2), a / b signed 8-bit (1).  kind::f8f6f4: c_format F32 (1), a / b E4M3 (0).  K-major both.
+template <bool F8>
+__host__ __device__ constexpr uint32_t idesc_8bit(int M, int N)
 {
-    // c_format S32 (2) | a, b signed 8-bit (1) | K-major both | N >> 3 | M >> 4
-    return (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
+    return (F8 ? (1u << 4) : ((2u << 4) | (1u << 7) | (1u << 10))) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
 }
 
+template <bool F8>
 __device__ __forceinline__ void mma_ts_i8(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t accumulate)
 {
-    asm volatile(
-        "{ .reg .pred p; setp.ne.b32 p, %4, 0; tcgen05.mma.cta_group::1.kind::i8 [%0], [%1], %2, %3, p; }" ::"r"(d_tmem),
-        "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate)
-        : "memory");
+    if constexpr (F8)
+        asm volatile("{ .reg .pred p; setp.ne.b32 p, %4, 0; tcgen05.mma.cta_group::1.kind::f8f6f4 [%0], [%1], %2, %3, p; }" ::"r"(d_tmem),
+                     "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
+    else
+        asm volatile("{ .reg .pred p; setp.ne.b32 p, %4, 0; tcgen05.mma.cta_group::1.kind::i8 [%0], [%1], %2, %3, p; }" ::"r"(d_tmem),
+                     "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
 }
 
+template <bool F8>
 __device__ __forceinline__ void mma_ss_i8(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate)
 {
-    asm volatile(
-        "{ .reg .pred p; setp.ne.b32 p, %4, 0; tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p; }" ::"r"(d_tmem),
-        "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
-        : "memory");
+    if constexpr (F8)
+        asm volatile("{ .reg .pred p; setp.ne.b32 p, %4, 0; tcgen05.mma.cta_group::1.kind::f8f6f4 [%0], %1, %2, %3, p; }" ::"r"(d_tmem),
+                     "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
+    else
+        asm volatile("{ .reg .pred p; setp.ne.b32 p, %4, 0; tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p; }" ::"r"(d_tmem),
+                     "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
 }
 
 // W_c[i][j] = T[c, rel(i, j)] (Eq. 7) in the K-major core-matrix layout: value (i, j) at byte (j/16)*LBO + i*16 + j%16.
@@ -198,7 +207,24 @@ __device__ __forceinline__ uint32_t requant2(uint32_t a0, uint32_t a1, uint64_t 
     return __byte_perm((uint32_t)t, (uint32_t)(t >> 32), 0x0040) & 0xffffu;
 }
 
-template <int WS, bool OUT8>
+// FP8 output: E4M3 codes of (sum * scale), round-to-nearest-even, saturating at +-448 (cvt.rn.satfinite.e4m3x2.f32: the
+// first source lands in the HIGH byte).  Returns code(a0) | code(a1) << 8.
+__device__ __forceinline__ uint32_t to_e4m3x2(uint32_t a0, uint32_t a1, float scale)
+{
+    const float r0 = __fmul_rn(__uint_as_float(a0), scale), r1 = __fmul_rn(__uint_as_float(a1), scale);
+    uint16_t d;
+    asm("cvt.rn.satfinite.e4m3x2.f32 %0, %1, %2;" : "=h"(d) : "f"(r1), "f"(r0));
+    return d;
+}
+// One pair of outputs as two 8-bit codes (int8: requantised; fp8: E4M3), low byte = the first.
+template <bool F8>
+__device__ __forceinline__ uint32_t out_pair(uint32_t a0, uint32_t a1, float sc, uint64_t sc2)
+{
+    if constexpr (F8) return to_e4m3x2(a0, a1, sc);
+    else return requant2(a0, a1, sc2);
+}
+
+template <int WS, bool OUT8, bool F8>
 __global__ void __launch_bounds__(kThreadsI, 1)
 tc_i8_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t* __restrict__ T, const float* __restrict__ scale,
              void* __restrict__ yv)
@@ -224,7 +250,7 @@ tc_i8_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t* __r
     ptx::tc_fence_after_sync();
     const uint32_t tmem = tmem_base_s;
     const uint32_t tmem_a = tmem, tmem_d = tmem + Cf::D_COL;
-    constexpr uint32_t idesc = idesc_i8(128, Cf::N_PAD);
+    constexpr uint32_t idesc = idesc_8bit<F8>(128, Cf::N_PAD);
 
     const long long t0 = tl.ntiles * blockIdx.x / gridDim.x, t1 = tl.ntiles * (blockIdx.x + 1) / gridDim.x;
     const int rowB = g.Wp;
@@ -313,7 +339,7 @@ tc_i8_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t* __r
 #pragma unroll
             for (int ks = 0; ks < Cf::KSTEPS; ++ks) {
                 const uint64_t bdesc = ptx::smem_desc_kmajor_noswz(wc_addr + ks * 2 * Cf::LBO, Cf::LBO, 128);
-                mma_ts_i8(tmem_d, tmem_a + ks * 8, bdesc, idesc, ks > 0 ? 1u : 0u);
+                mma_ts_i8<F8>(tmem_d, tmem_a + ks * 8, bdesc, idesc, ks > 0 ? 1u : 0u);
             }
             ptx::mma_commit(bar);
         }
@@ -340,9 +366,9 @@ tc_i8_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t* __r
                             } else if constexpr (WS % 2 == 0) {
                                 if ((k & 1) == 0)   // (i and i+1 are in the same chunk: 16 and WS are even)
                                     *reinterpret_cast<uint16_t*>(win + r * rowB + k) =
-                                        (uint16_t)pack_q2(requant(v[e], sc), requant(v[e + 1], sc));
+                                        (uint16_t)out_pair<F8>(v[e], v[e + 1], sc, pack_f2(sc, sc));
                             } else {
-                                win[r * rowB + k] = (uint8_t)requant(v[e], sc);
+                                win[r * rowB + k] = (uint8_t)(F8 ? to_e4m3x2(v[e], 0u, sc) : requant(v[e], sc));
                             }
                         }
                     }
@@ -406,7 +432,7 @@ struct I8Fast {
     static constexpr int SMEM = OFF_AO + AO_BYTES;
 };
 
-template <int WS, bool OUT8>
+template <int WS, bool OUT8, bool F8>
 __global__ void __launch_bounds__(kThreadsI, i8_ctas<WS, OUT8>())
 tc_i8_bulk_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t* __restrict__ T,
                   const float* __restrict__ scale, void* __restrict__ yv)
@@ -433,7 +459,7 @@ tc_i8_bulk_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t
     __syncthreads();
     ptx::tc_fence_after_sync();
     const uint32_t tmem_d = tmem_base_s;
-    constexpr uint32_t idesc = idesc_i8(128, Cf::N_PAD);
+    constexpr uint32_t idesc = idesc_8bit<F8>(128, Cf::N_PAD);
 
     const long long t0 = tl.ntiles * blockIdx.x / gridDim.x, t1 = tl.ntiles * (blockIdx.x + 1) / gridDim.x;
     const int rowB = g.W;
@@ -494,7 +520,7 @@ tc_i8_bulk_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t
             for (int ks = 0; ks < Cf::KSTEPS; ++ks) {
                 const uint64_t adesc = ptx::smem_desc_kmajor_noswz(a_addr + ks * 2 * Cf::A_LBO, Cf::A_LBO, 128);
                 const uint64_t bdesc = ptx::smem_desc_kmajor_noswz(wc_addr + ks * 2 * Cf::LBO, Cf::LBO, 128);
-                mma_ss_i8(tmem_d, adesc, bdesc, idesc, ks > 0 ? 1u : 0u);
+                mma_ss_i8<F8>(tmem_d, adesc, bdesc, idesc, ks > 0 ? 1u : 0u);
             }
             ptx::mma_commit(mma_bar);
         }
@@ -524,9 +550,9 @@ tc_i8_bulk_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t
                                 *reinterpret_cast<uint32_t*>(owin + (r * rowB + k) * 4) = v[e];
                             } else if constexpr (WS % 2 == 0) {
                                 if ((k & 1) == 0)
-                                    *reinterpret_cast<uint16_t*>(owin + r * rowB + k) = (uint16_t)requant2(v[e], v[e + 1], sc2);
+                                    *reinterpret_cast<uint16_t*>(owin + r * rowB + k) = (uint16_t)out_pair<F8>(v[e], v[e + 1], sc, sc2);
                             } else {
-                                owin[r * rowB + k] = (uint8_t)requant(v[e], sc);
+                                owin[r * rowB + k] = (uint8_t)(F8 ? to_e4m3x2(v[e], 0u, sc) : requant(v[e], sc));
                             }
                         }
                     }
@@ -584,7 +610,7 @@ bool i8_tiles(const Geom& g, const void* x, const void* y, bool out8, I8Tiles* t
     return true;
 }
 
-template <int WS, bool OUT8>
+template <int WS, bool OUT8, bool F8>
 cudaError_t launch_i8(const Geom& g, const I8Tiles& tl, const int8_t* x, const int8_t* T, const float* scale, void* y,
                       cudaStream_t stream, int* launches)
 {
@@ -594,7 +620,7 @@ cudaError_t launch_i8(const Geom& g, const I8Tiles& tl, const int8_t* x, const i
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     if (tl.bulk) {
         const size_t smem = I8Fast<WS, OUT8>::SMEM;
-        auto kern = tc_i8_bulk_kernel<WS, OUT8>;
+        auto kern = tc_i8_bulk_kernel<WS, OUT8, F8>;
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         const long long cap = (long long)sms * i8_ctas<WS, OUT8>();
@@ -604,7 +630,7 @@ cudaError_t launch_i8(const Geom& g, const I8Tiles& tl, const int8_t* x, const i
         return cudaGetLastError();
     }
     const size_t smem = Cf::WC_BYTES + Cf::TS_BYTES + Cf::FRAME_BYTES + (OUT8 ? 0 : 128 * Cf::N * 4);
-    auto kern = tc_i8_kernel<WS, OUT8>;
+    auto kern = tc_i8_kernel<WS, OUT8, F8>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const long long grid = tl.ntiles < sms ? tl.ntiles : sms;
@@ -623,16 +649,22 @@ bool tc_i8_supported(const Geom& g)
 }
 
 cudaError_t tc_i8_forward(const Geom& g, const int8_t* x, const int8_t* T, const float* scale, void* y, cudaStream_t stream,
-                          int* launches, int* path)
+                          int* launches, int* path, bool fp8)
 {
     I8Tiles tl;
     if (!i8_tiles(g, x, y, scale != nullptr, &tl)) return cudaErrorInvalidValue;
     *path = tl.bulk ? WBMM_PATH_TC_TMA : WBMM_PATH_TC_GATHER;
     if (tl.ntiles == 0) return cudaSuccess;
-    if (g.w == 14) return scale ? launch_i8<14, true>(g, tl, x, T, scale, y, stream, launches)
-                                : launch_i8<14, false>(g, tl, x, T, scale, y, stream, launches);
-    return scale ? launch_i8<7, true>(g, tl, x, T, scale, y, stream, launches)
-                 : launch_i8<7, false>(g, tl, x, T, scale, y, stream, launches);
+    auto go = [&](auto ws, auto f8) -> cudaError_t {
+        constexpr int WS = decltype(ws)::value;
+        constexpr bool F8 = decltype(f8)::value;
+        return scale ? launch_i8<WS, true, F8>(g, tl, x, T, scale, y, stream, launches)
+                     : launch_i8<WS, false, F8>(g, tl, x, T, scale, y, stream, launches);
+    };
+    using I14 = std::integral_constant<int, 14>;
+    using I7 = std::integral_constant<int, 7>;
+    if (g.w == 14) return fp8 ? go(I14{}, std::true_type{}) : go(I14{}, std::false_type{});
+    return fp8 ? go(I7{}, std::true_type{}) : go(I7{}, std::false_type{});
 }
 
 }  // namespace wbmm

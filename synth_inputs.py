@@ -133,3 +133,19 @@ def make_int8(case: Case, device: str = "cpu", extreme: bool = False):
     if device != "cpu":
         x, T, scale = x.to(device), T.to(device), scale.to(device)
     return {"x": x, "T": T, "scale": scale}
+
+
+def make_fp8(case: Case, device: str = "cpu"):
+    """dict(x=, T=, scale=) for the FP8 forward: the case's normal activations and table recipe (table scaled to unit
+    row maximum) rounded to E4M3 by torch's conversion, per-channel float32 scales that put sum * scale at O(1-100)."""
+    f = make(with_(case, dtype="f32", layout=NCHW), device="cpu")
+    x = f["x"].to(torch.float8_e4m3fn)
+    T = f["T"]
+    T = (T / T.abs().amax(dim=1, keepdim=True)).to(torch.float8_e4m3fn)
+    g = torch.Generator(device="cpu").manual_seed(case.seed + 78)
+    scale = (32.0 / case.w) * (0.5 + torch.rand((case.C,), generator=g, dtype=torch.float32))
+    if case.layout == NHWC:
+        x = x.permute(0, 2, 3, 1).contiguous()
+    if device != "cpu":
+        x, T, scale = x.to(device), T.to(device), scale.to(device)
+    return {"x": x, "T": T, "scale": scale}
