@@ -396,6 +396,16 @@ def other_rooflines(wb, dev, stream, hbm_peak):
         out[name.replace("_fwd", "_fwd_int32_out")] = {"ms": round(ms, 5), "frac": round((5.0 * ci.n_elem) / (hbm_peak * 1e9) * 1e3 / ms, 4)}
         del xs, y8, y32, d8
         torch.cuda.empty_cache()
+        # FP8 (E4M3 in, E4M3 out with per-channel scale) on the same kernels (kind::f8f6f4)
+        f8 = si.make_fp8(ci, device=dev)
+        xs = [f8["x"]] + [f8["x"].clone() for _ in range(ns - 1)]
+        yf = [torch.empty_like(f8["x"]) for _ in range(ns)]
+        ms = region_ms_rot(lambda i: wb.wbmm_forward_fp8(xs[i % ns], f8["T"], ci.w, scale=f8["scale"], out=yf[i % ns]), 30, stream)
+        out[name.replace("int8_", "fp8_")] = {"ms": round(ms, 5), "gbs": round(by8 / ms / 1e6, 1), "frac": round(by8 / (hbm_peak * 1e9) * 1e3 / ms, 4),
+                                              "tflops": round(2.0 * ci.w * ci.w * ci.n_elem / ms / 1e9, 2),
+                                              "path": wb.wbmm_path_string(wb.wbmm_last_path()), "buffer_sets": ns}
+        del xs, yf, f8
+        torch.cuda.empty_cache()
 
     # table gradient at w = 7 (two CTAs per SM) on the config-2 shape
     c2 = si.with_(si.CFG2, backward=True)
