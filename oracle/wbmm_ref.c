@@ -603,3 +603,104 @@ int wbmm_ref_forward_int8(int B, int C, int H, int W, int w, int sh, int sw, int
     }
     return bad ? 2 : 0;
 }
+
+/*
+ * 3-D windows w_d x w_h x w_w on [B, C, D, H, W] volumes (the extension PAPER.md:909 names).
+ * The paper gives no formula; reading A23 takes Eq. 4-7 with one more axis:
+ *   pad D, H, W at the far end to multiples of w_d, w_h, w_w; cyclic shift (s_d, s_h, s_w) on the padded volume (A6);
+ *   table T [C][(2w_d-1)(2w_h-1)(2w_w-1)],  I = ((dz + w_d - 1)(2w_h - 1) + (dh + w_h - 1))(2w_w - 1) + (dw + w_w - 1),
+ *   (dz, dh, dw) = output position - input position inside the window.
+ * layout 0: [B][C][D][H][W];  1: [B][D][H][W][C].
+ */
+static inline size_t elem_off3(int layout, int C, int D, int H, int W, int b, int c, int z, int h, int v)
+{
+    if (layout == 0)
+        return ((((size_t)b * C + c) * D + z) * H + h) * W + v;
+    return ((((size_t)b * D + z) * H + h) * W + v) * C + c;
+}
+
+static inline double load_hat3(const double *x, int layout, int C, int D, int H, int W, int Dp, int Hp, int Wp,
+                               int sd, int sh, int sw, int b, int c, int z, int h, int v)
+{
+    int zs = modp(z + sd, Dp), hs = modp(h + sh, Hp), vs = modp(v + sw, Wp);
+    if (zs >= D || hs >= H || vs >= W)
+        return 0.0;
+    return x[elem_off3(layout, C, D, H, W, b, c, zs, hs, vs)];
+}
+
+int wbmm_ref_forward_3d(int B, int C, int D, int H, int W, int wd, int wh, int ww, int sd, int sh, int sw, int layout,
+                        const double *x, const double *T, double *y)
+{
+    if (B < 0 || C < 0 || D < 1 || H < 1 || W < 1 || wd < 1 || wh < 1 || ww < 1 || sd < 0 || sh < 0 || sw < 0 ||
+        sd >= wd || sh >= wh || sw >= ww)
+        return 1;
+    const int tw = 2 * ww - 1, th = 2 * wh - 1, nb = (2 * wd - 1) * th * tw;
+    const int Dp = padded(D, wd), Hp = padded(H, wh), Wp = padded(W, ww);
+    const long planes = (long)B * C;
+
+#pragma omp parallel for schedule(static)
+    for (long pc = 0; pc < planes; ++pc) {
+        int b = (int)(pc / C), c = (int)(pc % C);
+        const double *Tc = T + (size_t)c * nb;
+        for (int zo = 0; zo < D; ++zo)
+            for (int ho = 0; ho < H; ++ho)
+                for (int vo = 0; vo < W; ++vo) {
+                    int z = modp(zo - sd, Dp), h = modp(ho - sh, Hp), v = modp(vo - sw, Wp);
+                    int z0 = (z / wd) * wd, h0 = (h / wh) * wh, v0 = (v / ww) * ww;
+                    double acc = 0.0;
+                    for (int zq = z0; zq < z0 + wd; ++zq)
+                        for (int hq = h0; hq < h0 + wh; ++hq)
+                            for (int vq = v0; vq < v0 + ww; ++vq)
+                                acc += Tc[((z - zq + wd - 1) * th + (h - hq + wh - 1)) * tw + (v - vq + ww - 1)] *
+                                       load_hat3(x, layout, C, D, H, W, Dp, Hp, Wp, sd, sh, sw, b, c, zq, hq, vq);
+                    y[elem_off3(layout, C, D, H, W, b, c, zo, ho, vo)] = acc;
+                }
+    }
+    return 0;
+}
+
+/* Backward of wbmm_ref_forward_3d: dx = W_c^T dy per window, dT[c,k] = sum over windows and pairs with I = k of
+ * dy[out] * x[in]; dy is zero outside the volume (A11).  Either output may be NULL; dT is overwritten. */
+int wbmm_ref_backward_3d(int B, int C, int D, int H, int W, int wd, int wh, int ww, int sd, int sh, int sw, int layout,
+                         const double *x, const double *T, const double *dy, double *dx, double *dT)
+{
+    if (B < 0 || C < 0 || D < 1 || H < 1 || W < 1 || wd < 1 || wh < 1 || ww < 1 || sd < 0 || sh < 0 || sw < 0 ||
+        sd >= wd || sh >= wh || sw >= ww)
+        return 1;
+    if ((dx && !T) || (dT && !x))
+        return 1;
+    const int tw = 2 * ww - 1, th = 2 * wh - 1, nb = (2 * wd - 1) * th * tw;
+    const int Dp = padded(D, wd), Hp = padded(H, wh), Wp = padded(W, ww);
+
+#pragma omp parallel for schedule(static)
+    for (int c = 0; c < C; ++c) {
+        const double *Tc = T ? T + (size_t)c * nb : NULL;
+        if (dT)
+            for (int k = 0; k < nb; ++k) dT[(size_t)c * nb + k] = 0.0;
+        for (int b = 0; b < B; ++b)
+            for (int z0 = 0; z0 < Dp; z0 += wd)
+                for (int h0 = 0; h0 < Hp; h0 += wh)
+                    for (int v0 = 0; v0 < Wp; v0 += ww)
+                        /* one window: input position (zq,hq,vq), output position (z,h,v) */
+                        for (int zq = z0; zq < z0 + wd; ++zq)
+                            for (int hq = h0; hq < h0 + wh; ++hq)
+                                for (int vq = v0; vq < v0 + ww; ++vq) {
+                                    double xin = dT ? load_hat3(x, layout, C, D, H, W, Dp, Hp, Wp, sd, sh, sw, b, c, zq, hq, vq) : 0.0;
+                                    double acc = 0.0;
+                                    for (int z = z0; z < z0 + wd; ++z)
+                                        for (int h = h0; h < h0 + wh; ++h)
+                                            for (int v = v0; v < v0 + ww; ++v) {
+                                                int k = ((z - zq + wd - 1) * th + (h - hq + wh - 1)) * tw + (v - vq + ww - 1);
+                                                double g = load_hat3(dy, layout, C, D, H, W, Dp, Hp, Wp, sd, sh, sw, b, c, z, h, v);
+                                                if (dx) acc += Tc[k] * g;
+                                                if (dT) dT[(size_t)c * nb + k] += g * xin;
+                                            }
+                                    if (dx) {
+                                        int zs = modp(zq + sd, Dp), hs = modp(hq + sh, Hp), vs = modp(vq + sw, Wp);
+                                        if (zs < D && hs < H && vs < W)
+                                            dx[elem_off3(layout, C, D, H, W, b, c, zs, hs, vs)] = acc;
+                                    }
+                                }
+    }
+    return 0;
+}

@@ -61,6 +61,10 @@ def _load():
     lib.wbmm_ref_backward_rect.argtypes = [i] * 9 + [dp, dp, dp, dp, dp]
     lib.wbmm_ref_backward.restype = i
     lib.wbmm_ref_backward.argtypes = [i] * 8 + [dp, dp, dp, dp, dp]
+    lib.wbmm_ref_forward_3d.argtypes = [i] * 12 + [dp, dp, dp]
+    lib.wbmm_ref_forward_3d.restype = i
+    lib.wbmm_ref_backward_3d.argtypes = [i] * 12 + [dp, dp, dp, dp, dp]
+    lib.wbmm_ref_backward_3d.restype = i
     lib.wbmm_ref_forward_int8.argtypes = [i] * 8 + [ctypes.c_void_p] * 5
     lib.wbmm_ref_forward_int8.restype = i
     lib.wbmm_ref_hier_forward_train.restype = i
@@ -188,6 +192,52 @@ def forward_int8(x, T, w, shift=(0, 0), layout=NCHW, scale=None) -> np.ndarray:
     if rc != 0:
         raise ValueError(f"oracle rejected arguments (rc={rc})")
     return y
+
+
+def _dims3(x, layout):
+    if x.ndim != 5:
+        raise ValueError("volume must be 5-D")
+    if layout == NCHW:
+        B, C, D, H, W = x.shape
+    else:
+        B, D, H, W, C = x.shape
+    return B, C, D, H, W
+
+
+def forward_3d(x, T, win, shift=(0, 0, 0), layout=NCHW) -> np.ndarray:
+    """3-D windows win = (w_d, w_h, w_w) on [B,C,D,H,W] (layout 0) / [B,D,H,W,C] (layout 1): DESIGN.md reading A23."""
+    x, xp = _d(x)
+    T, tp = _d(T)
+    B, C, D, H, W = _dims3(x, layout)
+    wd, wh, ww = win
+    assert T.shape == (C, (2 * wd - 1) * (2 * wh - 1) * (2 * ww - 1)), (T.shape, C, win)
+    y = np.zeros_like(x)
+    rc = _load().wbmm_ref_forward_3d(B, C, D, H, W, wd, wh, ww, int(shift[0]), int(shift[1]), int(shift[2]), layout, xp, tp,
+                                     y.ctypes.data_as(ctypes.POINTER(ctypes.c_double)))
+    if rc != 0:
+        raise ValueError(f"oracle rejected arguments (rc={rc})")
+    return y
+
+
+def backward_3d(x, T, dy, win, shift=(0, 0, 0), layout=NCHW, need_dx=True, need_dT=True):
+    """(dx, dT) of forward_3d in float64; either is None when not requested."""
+    x, xp = _d(x)
+    T, tp = _d(T)
+    dy, gp = _d(dy)
+    assert dy.shape == x.shape
+    B, C, D, H, W = _dims3(x, layout)
+    wd, wh, ww = win
+    assert T.shape == (C, (2 * wd - 1) * (2 * wh - 1) * (2 * ww - 1))
+    null = ctypes.POINTER(ctypes.c_double)()
+    dx = np.zeros_like(x) if need_dx else None
+    dT = np.zeros_like(T) if need_dT else None
+    rc = _load().wbmm_ref_backward_3d(
+        B, C, D, H, W, wd, wh, ww, int(shift[0]), int(shift[1]), int(shift[2]), layout, xp, tp, gp,
+        dx.ctypes.data_as(ctypes.POINTER(ctypes.c_double)) if need_dx else null,
+        dT.ctypes.data_as(ctypes.POINTER(ctypes.c_double)) if need_dT else null)
+    if rc != 0:
+        raise ValueError(f"oracle rejected arguments (rc={rc})")
+    return dx, dT
 
 
 def e4m3_decode(codes) -> np.ndarray:

@@ -818,3 +818,99 @@ def test_fp8_forward_is_the_operator_on_decoded_values(oracle):
     sc = np.array([0.5, 2.0, -1.0])
     yn = oracle.forward_fp8(np.ascontiguousarray(codes.transpose(0, 2, 3, 1)), T1, w, layout=NHWC, scale=sc)
     assert np.array_equal(yn.transpose(0, 3, 1, 2), want * sc[None, :, None, None])
+
+
+# ----------------------------------------------------------------------------- NEXT-4: 3-D windows (reading A23)
+WIN3 = [(2, 3, 4), (3, 2, 2), (1, 3, 3), (2, 1, 5)]
+
+
+@pytest.mark.parametrize("win", WIN3)
+def test_3d_single_window_is_depthwise_conv3d(oracle, win):
+    """Theorem 3.2 with one more axis: on a volume of ONE window the operator is the zero-padded depthwise conv3d with a
+    (2w_d-1) x (2w_h-1) x (2w_w-1) kernel (library routine).  Catches: a wrong stride in the 3-D index, swapped axes."""
+    wd, wh, ww = win
+    r = rng(950)
+    C = 3
+    x = r.standard_normal((2, C, wd, wh, ww))
+    T = r.standard_normal((C, (2 * wd - 1) * (2 * wh - 1) * (2 * ww - 1)))
+    y = oracle.forward_3d(x, T, win)
+    K = torch.from_numpy(T.reshape(C, 1, 2 * wd - 1, 2 * wh - 1, 2 * ww - 1))
+    ref = F.conv3d(torch.from_numpy(x), torch.flip(K, dims=(2, 3, 4)), padding=(wd - 1, wh - 1, ww - 1), groups=C)
+    assert np.allclose(y, ref.numpy(), rtol=0, atol=1e-12)
+
+
+@pytest.mark.parametrize("layout", [NCHW, NHWC])
+def test_3d_depth_one_windows_are_the_rectangular_operator_per_slice(oracle, layout):
+    """w_d = 1: every depth slice is an independent 2-D problem (depth acts as batch); forward, dX and dT equal the
+    pinned rectangular oracle's.  Catches: depth leaking between slices, layout strides."""
+    r = rng(951)
+    B, C, D, H, W, wh, ww, s = 2, 3, 4, 7, 9, 3, 4, (0, 2, 1)
+    x = r.standard_normal((B, C, D, H, W))
+    dy = r.standard_normal((B, C, D, H, W))
+    T = r.standard_normal((C, (2 * wh - 1) * (2 * ww - 1)))
+    to = (lambda a: np.ascontiguousarray(a.transpose(0, 2, 3, 4, 1))) if layout == NHWC else (lambda a: a)
+    back = (lambda a: a.transpose(0, 4, 1, 2, 3)) if layout == NHWC else (lambda a: a)
+    y = back(oracle.forward_3d(to(x), T, (1, wh, ww), s, layout))
+    dx, dT = oracle.backward_3d(to(x), T, to(dy), (1, wh, ww), s, layout)
+    x2 = x.transpose(0, 2, 1, 3, 4).reshape(B * D, C, H, W)
+    g2 = dy.transpose(0, 2, 1, 3, 4).reshape(B * D, C, H, W)
+    y2 = oracle.forward_rect(x2, T, wh, ww, s[1:])
+    dx2, dT2 = oracle.backward_rect(x2, T, g2, wh, ww, s[1:])
+    unfold = lambda a: a.reshape(B, D, C, H, W).transpose(0, 2, 1, 3, 4)
+    assert np.allclose(y, unfold(y2), rtol=0, atol=1e-12)
+    assert np.allclose(back(dx), unfold(dx2), rtol=0, atol=1e-12) and np.allclose(dT, dT2, rtol=0, atol=1e-11)
+
+
+def test_3d_axes_are_interchangeable(oracle):
+    """Transposing the volume's depth and height axes together with the window and the table's axes transposes the
+    result.  Catches: an axis handled differently from the others (padding, shift, index stride)."""
+    r = rng(952)
+    win, s = (2, 3, 2), (1, 2, 0)
+    x = r.standard_normal((2, 2, 5, 7, 4))
+    T = r.standard_normal((2, 3 * 5 * 3))
+    y = oracle.forward_3d(x, T, win, s)
+    xt = np.ascontiguousarray(x.transpose(0, 1, 3, 2, 4))
+    Tt = np.ascontiguousarray(T.reshape(2, 3, 5, 3).transpose(0, 2, 1, 3)).reshape(2, -1)
+    yt = oracle.forward_3d(xt, Tt, (3, 2, 2), (2, 1, 0))
+    assert np.allclose(y, yt.transpose(0, 1, 3, 2, 4), rtol=0, atol=1e-12)
+
+
+def test_3d_padding_shift_and_window_independence(oracle):
+    """Explicit zero padding + roll + per-window conv3d + roll back + crop (library pieces) equals the operator."""
+    r = rng(953)
+    win, s = (2, 3, 2), (1, 1, 1)
+    B, C, D, H, W = 1, 2, 3, 7, 5
+    x = r.standard_normal((B, C, D, H, W))
+    T = r.standard_normal((C, 3 * 5 * 3))
+    Dp, Hp, Wp = 4, 9, 6
+    xp = np.zeros((B, C, Dp, Hp, Wp))
+    xp[:, :, :D, :H, :W] = x
+    xh = np.roll(xp, (-s[0], -s[1], -s[2]), axis=(2, 3, 4))
+    yh = np.zeros_like(xh)
+    K = torch.flip(torch.from_numpy(T.reshape(C, 1, 3, 5, 3)), dims=(2, 3, 4))
+    for z0 in range(0, Dp, 2):
+        for h0 in range(0, Hp, 3):
+            for v0 in range(0, Wp, 2):
+                blk = torch.from_numpy(np.ascontiguousarray(xh[:, :, z0:z0 + 2, h0:h0 + 3, v0:v0 + 2]))
+                yh[:, :, z0:z0 + 2, h0:h0 + 3, v0:v0 + 2] = F.conv3d(blk, K, padding=(1, 2, 1), groups=C).numpy()
+    want = np.roll(yh, s, axis=(2, 3, 4))[:, :, :D, :H, :W]
+    assert np.allclose(oracle.forward_3d(x, T, win, s), want, rtol=0, atol=1e-12)
+
+
+@pytest.mark.parametrize("layout", [NCHW, NHWC])
+def test_3d_backward_adjoint_and_one_hot_derivative(oracle, layout):
+    """<dy, WBMM(x2;T)> = <dX, x2>, <dT, T2> = <dy, WBMM(x;T2)> (the operator is bilinear), and dT along a one-hot
+    table direction is the derivative of the pinned forward.  Catches: dX built from W instead of W^T, a bin offset."""
+    r = rng(954)
+    win, s = (2, 2, 3), (1, 0, 2)
+    shape = (2, 3, 3, 5, 7) if layout == NCHW else (2, 3, 5, 7, 3)
+    x, x2, dy = (r.standard_normal(shape) for _ in range(3))
+    nb = 3 * 3 * 5
+    T, T2 = r.standard_normal((3, nb)), r.standard_normal((3, nb))
+    dx, dT = oracle.backward_3d(x, T, dy, win, s, layout)
+    assert np.isclose(np.sum(dy * oracle.forward_3d(x2, T, win, s, layout)), np.sum(dx * x2), rtol=1e-12)
+    assert np.isclose(np.sum(dT * T2), np.sum(dy * oracle.forward_3d(x, T2, win, s, layout)), rtol=1e-12)
+    for (c, k) in [(0, 0), (1, nb // 2), (2, nb - 1), (1, 7)]:
+        E = np.zeros((3, nb))
+        E[c, k] = 1.0
+        assert np.isclose(dT[c, k], np.sum(dy * oracle.forward_3d(x, E, win, s, layout)), rtol=1e-12, atol=1e-12)
