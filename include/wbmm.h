@@ -243,6 +243,23 @@ WBMM_API int wbmm_forward_matrix(const wbmm_desc_t *desc, const void *x, const v
                         int transpose, void *cuda_stream);
 
 /*
+ * 3-D windows w_d x w_h x w_w on volumes (the extension PAPER.md:909 names; reading A23:
+ * Eq. 4-7 with one more axis).  desc gives B, C, H, W, w = w_h, shift_h, shift_w, dtype, layout and flags as for
+ * wbmm_forward_rect; D (depth), w_d, w_w and shift_d in [0, w_d) are arguments.
+ *   layout   WBMM_LAYOUT_NCHW: x, y, dy, dx are [B][C][D][H][W];  WBMM_LAYOUT_NHWC: [B][D][H][W][C].
+ *   T, dT    [C][(2w_d-1)(2w_h-1)(2w_w-1)], index ((dz + w_d - 1)(2w_h - 1) + (dh + w_h - 1))(2w_w - 1) + (dw + w_w - 1) with
+ *            (dz, dh, dw) = output position - input position inside the window; T in desc->dtype, dT float32.
+ *   D, H, W are zero-padded at the far end to multiples of the window; the cyclic shift acts on the padded volume.
+ * FFMA kernels with float32 accumulation (wbmm_last_path() = WBMM_PATH_SIMT), any dtype / layout / shift / ragged size;
+ * w_d*w_h*w_w <= 1024 and (2w_d-1)(2w_h-1)(2w_w-1) <= 4096, else WBMM_STATUS_UNSUPPORTED.  Pointer rules, nullable dx / dT,
+ * WBMM_FLAG_ACCUMULATE_DT as in wbmm_backward_rect.
+ */
+WBMM_API int wbmm_forward_win3d(const wbmm_desc_t *desc, int32_t D, int32_t w_d, int32_t w_w, int32_t shift_d, const void *x,
+                       const void *T, void *y, void *cuda_stream);
+WBMM_API int wbmm_backward_win3d(const wbmm_desc_t *desc, int32_t D, int32_t w_d, int32_t w_w, int32_t shift_d, const void *x,
+                        const void *T, const void *dy, void *dx, float *dT, void *cuda_stream);
+
+/*
  * INT8 forward (PAPER.md:749 reports INT8 deployments of the operator; reading A21):
  * Algorithm 1 on signed 8-bit activations and tables with exact 32-bit integer sums (|sum| <= w*w*128*128 < 2^31),
  * on the tensor cores (tcgen05.mma kind::i8, accumulator in tensor memory; wbmm_last_path() = WBMM_PATH_TC_TMA for

@@ -24,7 +24,7 @@ _DTYPES = {torch.float32: DTYPE_F32, torch.bfloat16: DTYPE_BF16, torch.float16: 
 
 # every symbol include/wbmm.h declares
 EXPORTS = (
-    "wbmm_forward", "wbmm_forward_static_scratch", "wbmm_forward_rect", "wbmm_backward_rect", "wbmm_backward", "wbmm_hier_forward", "wbmm_hier_backward", "wbmm_forward_matrix", "wbmm_forward_int8", "wbmm_forward_fp8", "wbmm_fold_dwconv", "wbmm_forward_fused", "wbmm_materialize_weight", "wbmm_forward_host",
+    "wbmm_forward", "wbmm_forward_static_scratch", "wbmm_forward_rect", "wbmm_backward_rect", "wbmm_forward_win3d", "wbmm_backward_win3d", "wbmm_backward", "wbmm_hier_forward", "wbmm_hier_backward", "wbmm_forward_matrix", "wbmm_forward_int8", "wbmm_forward_fp8", "wbmm_fold_dwconv", "wbmm_forward_fused", "wbmm_materialize_weight", "wbmm_forward_host",
     "wbmm_backward_host", "wbmm_release", "wbmm_last_path", "wbmm_launch_count",
     "wbmm_status_string", "wbmm_path_string", "wbmm_last_error_string", "wbmm_version",
 )
@@ -61,6 +61,11 @@ def lib() -> ctypes.CDLL:
     L.wbmm_forward_rect.restype = i
     L.wbmm_backward_rect.argtypes = [dp, ctypes.c_int32, vp, vp, vp, vp, vp, vp]
     L.wbmm_backward_rect.restype = i
+    i32 = ctypes.c_int32
+    L.wbmm_forward_win3d.argtypes = [dp, i32, i32, i32, i32, vp, vp, vp, vp]
+    L.wbmm_forward_win3d.restype = i
+    L.wbmm_backward_win3d.argtypes = [dp, i32, i32, i32, i32, vp, vp, vp, vp, vp, vp]
+    L.wbmm_backward_win3d.restype = i
     L.wbmm_backward.argtypes = [dp, vp, vp, vp, vp, vp, vp]
     L.wbmm_hier_forward.argtypes = [dp, vp, vp, vp, vp, i, vp]
     L.wbmm_hier_forward.restype = i
@@ -205,6 +210,48 @@ def wbmm_backward_rect(x: Optional[torch.Tensor], T: Optional[torch.Tensor], dy:
     with torch.cuda.device(dy.device):
         _check(lib().wbmm_backward_rect(ctypes.byref(d), int(ww), _dev(x, "x"), _dev(T, "T"), _dev(dy, "dy"),
                                         _dev(dx, "dx"), _dev(dT, "dT"), _stream(dy)))
+    return dx, dT
+
+
+def _desc3d(t: torch.Tensor, win, shift, layout: int, flags: int):
+    if t.dim() != 5:
+        raise ValueError("volume must be 5-D: [B,C,D,H,W] (NCHW) or [B,D,H,W,C] (NHWC)")
+    if layout == NCHW:
+        B, C, D, H, W = t.shape
+    else:
+        B, D, H, W, C = t.shape
+    if t.dtype not in _DTYPES:
+        raise TypeError(f"unsupported dtype {t.dtype}")
+    wd, wh, ww = (int(v) for v in win)
+    d = WbmmDesc(B, C, H, W, wh, int(shift[1]), int(shift[2]), _DTYPES[t.dtype], int(layout), int(flags))
+    return d, D, wd, ww, int(shift[0]), (C, (2 * wd - 1) * (2 * wh - 1) * (2 * ww - 1))
+
+
+def wbmm_forward_win3d(x: torch.Tensor, T: torch.Tensor, win, shift=(0, 0, 0), layout: int = NCHW,
+                       out: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """3-D windows win = (w_d, w_h, w_w) on a volume (include/wbmm.h: wbmm_forward_win3d)."""
+    d, D, wd, ww, sd, tshape = _desc3d(x, win, shift, layout, 0)
+    if T.dtype != x.dtype or tuple(T.shape) != tshape:
+        raise ValueError("T must be [C,(2w_d-1)(2w_h-1)(2w_w-1)] in the dtype of x")
+    y = torch.empty_like(x) if out is None else out
+    with torch.cuda.device(x.device):
+        _check(lib().wbmm_forward_win3d(ctypes.byref(d), D, wd, ww, sd, _dev(x, "x"), _dev(T, "T"), _dev(y, "y"), _stream(x)))
+    return y
+
+
+def wbmm_backward_win3d(x: Optional[torch.Tensor], T: Optional[torch.Tensor], dy: torch.Tensor, win, shift=(0, 0, 0),
+                        layout: int = NCHW, flags: int = 0, need_dx: bool = True, need_dT: bool = True,
+                        dT: Optional[torch.Tensor] = None):
+    """(dx, dT) of wbmm_forward_win3d; dT is float32 [C, (2w_d-1)(2w_h-1)(2w_w-1)]."""
+    d, D, wd, ww, sd, tshape = _desc3d(dy, win, shift, layout, flags)
+    dx = torch.empty_like(dy) if need_dx else None
+    if need_dT and dT is None:
+        dT = torch.empty(tshape, dtype=torch.float32, device=dy.device)
+    if not need_dT:
+        dT = None
+    with torch.cuda.device(dy.device):
+        _check(lib().wbmm_backward_win3d(ctypes.byref(d), D, wd, ww, sd, _dev(x, "x"), _dev(T, "T"), _dev(dy, "dy"),
+                                         _dev(dx, "dx"), _dev(dT, "dT"), _stream(dy)))
     return dx, dT
 
 

@@ -756,6 +756,63 @@ int wbmm_forward_matrix(const wbmm_desc_t* desc, const void* x, const void* M, c
     return WBMM_STATUS_OK;
 }
 
+// 3-D windows (reading A23): desc gives B, C, H, W, w = w_h, shift_h / shift_w, dtype, layout (NCHW = [B][C][D][H][W],
+// NHWC = [B][D][H][W][C]); depth, the other two window sides and the depth shift are arguments.
+static int validate_win3d(const wbmm_desc_t* d, int D, int w_d, int w_w, int shift_d)
+{
+    int st = validate_rect(d, w_w);
+    if (st != WBMM_STATUS_OK) return st;
+    if (D < 1 || w_d < 1 || shift_d < 0 || shift_d >= w_d) return WBMM_STATUS_INVALID_ARGUMENT;
+    return WBMM_STATUS_OK;
+}
+
+int wbmm_forward_win3d(const wbmm_desc_t* desc, int32_t D, int32_t w_d, int32_t w_w, int32_t shift_d, const void* x, const void* T,
+                       void* y, void* cuda_stream)
+{
+    int st = validate_win3d(desc, D, w_d, w_w, shift_d);
+    if (st != WBMM_STATUS_OK) return st;
+    if (desc->B == 0 || desc->C == 0) return WBMM_STATUS_OK;
+    if (!x || !T || !y || x == y) return WBMM_STATUS_INVALID_ARGUMENT;
+    const size_t es = elem_size(desc->dtype);
+    if (!aligned(x, es) || !aligned(T, es) || !aligned(y, es)) return WBMM_STATUS_MISALIGNED;
+    if (device_state() < 0) return WBMM_STATUS_NO_DEVICE;
+    if (!wbmm::win3d_supported(*desc, D, w_d, w_w)) return WBMM_STATUS_UNSUPPORTED;
+    int launches = 0;
+    cudaError_t e = wbmm::win3d_forward(*desc, D, w_d, w_w, shift_d, x, T, y, false, static_cast<cudaStream_t>(cuda_stream), &launches);
+    g_launches += launches;
+    if (e != cudaSuccess) return set_cuda_error(e, "win3d_forward");
+    t_last_path = WBMM_PATH_SIMT;
+    return WBMM_STATUS_OK;
+}
+
+int wbmm_backward_win3d(const wbmm_desc_t* desc, int32_t D, int32_t w_d, int32_t w_w, int32_t shift_d, const void* x, const void* T,
+                        const void* dy, void* dx, float* dT, void* cuda_stream)
+{
+    int st = validate_win3d(desc, D, w_d, w_w, shift_d);
+    if (st != WBMM_STATUS_OK) return st;
+    if (desc->C == 0) return WBMM_STATUS_OK;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    const long long nb = (2ll * w_d - 1) * (2ll * desc->w - 1) * (2ll * w_w - 1);
+    if (dT && !aligned(dT, 4)) return WBMM_STATUS_MISALIGNED;
+    if (desc->B > 0 && (!dy || (dx && !T) || (dT && !x) || (dx && dx == dy))) return WBMM_STATUS_INVALID_ARGUMENT;
+    const size_t es = elem_size(desc->dtype);
+    if (desc->B > 0 && (!aligned(dy, es) || (x && !aligned(x, es)) || (T && !aligned(T, es)) || (dx && !aligned(dx, es))))
+        return WBMM_STATUS_MISALIGNED;
+    if (device_state() < 0) return WBMM_STATUS_NO_DEVICE;
+    if (!wbmm::win3d_supported(*desc, D, w_d, w_w)) return WBMM_STATUS_UNSUPPORTED;
+    int launches = 0;
+    cudaError_t e = cudaSuccess;
+    if (dT && !(desc->flags & WBMM_FLAG_ACCUMULATE_DT)) e = wbmm::simt_zero_f32(dT, (long long)desc->C * nb, stream, &launches);
+    if (desc->B > 0) {
+        if (e == cudaSuccess && dx) e = wbmm::win3d_forward(*desc, D, w_d, w_w, shift_d, dy, T, dx, true, stream, &launches);
+        if (e == cudaSuccess && dT) e = wbmm::win3d_grad_table(*desc, D, w_d, w_w, shift_d, x, dy, dT, stream, &launches);
+    }
+    g_launches += launches;
+    if (e != cudaSuccess) return set_cuda_error(e, "win3d backward");
+    t_last_path = WBMM_PATH_SIMT;
+    return WBMM_STATUS_OK;
+}
+
 // INT8 / FP8 (E4M3) forward: the same kernels and routes, 8-bit elements either way.
 static int forward_8bit(const wbmm_desc_t* desc, const int8_t* x, const int8_t* T, const float* scale, void* y, void* cuda_stream, bool fp8)
 {

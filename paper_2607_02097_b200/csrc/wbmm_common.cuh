@@ -82,6 +82,12 @@ bool simt_supported(const Geom& g);
 bool rect_supported(const wbmm_desc_t& d, int ww);
 cudaError_t rect_forward(const wbmm_desc_t& d, int ww, const void* x, const void* T, void* y, bool reverse, cudaStream_t stream, int* launches);
 cudaError_t rect_grad_table(const wbmm_desc_t& d, int ww, const void* x, const void* dy, float* dT, cudaStream_t stream, int* launches);
+// 3-D windows w_d x w_h x w_w on volumes of depth D (wbmm_rect.cu with a depth axis): d.w is w_h, shift (sd, d.shift_h, d.shift_w).
+bool win3d_supported(const wbmm_desc_t& d, int D, int wd, int ww);
+cudaError_t win3d_forward(const wbmm_desc_t& d, int D, int wd, int ww, int sd, const void* x, const void* T, void* y, bool reverse,
+                          cudaStream_t stream, int* launches);
+cudaError_t win3d_grad_table(const wbmm_desc_t& d, int D, int wd, int ww, int sd, const void* x, const void* dy, float* dT,
+                             cudaStream_t stream, int* launches);
 // Hierarchical operator on FFMA kernels (wbmm_rect.cu): any dtype / layout / shift / ragged size, w even.
 cudaError_t fused_simt_forward(const wbmm_desc_t& d, const void* x, const void* T, const void* bias, float ident, void* y, bool transpose,
                                cudaStream_t stream, int* launches);

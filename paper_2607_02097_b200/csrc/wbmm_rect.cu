@@ -17,29 +17,36 @@ namespace {
 
 constexpr int kThreadsR = 256;
 
+// A depth axis makes the same kernels serve 3-D windows w_d x w_h x w_w on volumes [B][C][D][H][W] / [B][D][H][W][C]
+// (reading A23): in-window position p = (pz * w_h + pr) * w_w + pc, table index
+// ((dz + w_d - 1)(2w_h - 1) + (dh + w_h - 1))(2w_w - 1) + (dw + w_w - 1).  2-D problems have D = w_d = 1.
 struct RectGeom {
     int B, C, H, W, wh, ww, sh, sw, layout;
     int Hp, Wp, nwh, nww, N, tw, nb;
+    int D, wd, sd, Dp, nwd, th;
     long long nwin;
 };
 
-__device__ __forceinline__ long long rect_offset(const RectGeom& g, int b, int c, int h, int v)
+__device__ __forceinline__ long long rect_offset(const RectGeom& g, int b, int c, int z, int h, int v)
 {
-    if (g.layout == WBMM_LAYOUT_NCHW) return (((long long)b * g.C + c) * g.H + h) * g.W + v;
-    return (((long long)b * g.H + h) * g.W + v) * g.C + c;
+    if (g.layout == WBMM_LAYOUT_NCHW) return ((((long long)b * g.C + c) * g.D + z) * g.H + h) * g.W + v;
+    return ((((long long)b * g.D + z) * g.H + h) * g.W + v) * g.C + c;
 }
 
 // element of the zero-extended, cyclically shifted frame that window `win` holds at in-window position p; -1 = padding
 __device__ __forceinline__ long long rect_window_elem(const RectGeom& g, long long win, int p, int c)
 {
-    const int wpi = g.nwh * g.nww;
-    const int b = (int)(win / wpi), wl = (int)(win - (long long)b * wpi);
+    const int wps = g.nwh * g.nww, wpi = g.nwd * wps;
+    const int b = (int)(win / wpi), wv = (int)(win - (long long)b * wpi);
+    const int wz = wv / wps, wl = wv - wz * wps;
     const int wy = wl / g.nww, wx = wl - wy * g.nww;
-    int h = wy * g.wh + p / g.ww + g.sh, v = wx * g.ww + p % g.ww + g.sw;
+    const int area = g.wh * g.ww, pz = p / area, p2 = p - pz * area;
+    int z = wz * g.wd + pz + g.sd, h = wy * g.wh + p2 / g.ww + g.sh, v = wx * g.ww + p2 % g.ww + g.sw;
+    if (z >= g.Dp) z -= g.Dp;
     if (h >= g.Hp) h -= g.Hp;
     if (v >= g.Wp) v -= g.Wp;
-    if (h >= g.H || v >= g.W) return -1;
-    return rect_offset(g, b, c, h, v);
+    if (z >= g.D || h >= g.H || v >= g.W) return -1;
+    return rect_offset(g, b, c, z, h, v);
 }
 
 // HIER (square windows, w even): the hierarchical operator of PAPER.md:216-227 (Eq. 9) / Algorithm 2 in one pass,
@@ -89,29 +96,31 @@ rect_forward_kernel(RectGeom g, const E* __restrict__ x, const E* __restrict__ T
     const int nq = G / 4;
     for (int idx = threadIdx.x; idx < nq * g.N; idx += kThreadsR) {
         const int gq = idx / g.N, p = idx - gq * g.N;
-        const int r = p / g.ww, cc = p - r * g.ww;
-        // Eq. 7 with i = p (output), j = q (input): k = (r - rq + w_h - 1)(2w_w - 1) + (cc - cq + w_w - 1)
-        const float* Tr = Ts + (r + g.wh - 1) * g.tw + cc + g.ww - 1;
+        const int area = g.wh * g.ww, pz = p / area, p2 = p - pz * area;
+        const int r = p2 / g.ww, cc = p2 - r * g.ww;
+        // Eq. 7 with i = p (output), j = q (input): k = ((pz - zq + w_d - 1)(2w_h - 1) + (r - rq + w_h - 1))(2w_w - 1) + (cc - cq + w_w - 1)
+        const float* Tr = Ts + ((pz + g.wd - 1) * g.th + r + g.wh - 1) * g.tw + cc + g.ww - 1;
         const float4* xq = reinterpret_cast<const float4*>(xs) + gq;
         float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
         const E* Mc = T + (long long)c * g.N * g.N;                 // MODE 3: this channel's matrix
+        for (int zq = 0; zq < g.wd; ++zq)
         for (int rq = 0; rq < g.wh; ++rq) {
-            const float* Trr = Tr - rq * g.tw;
-            const float4* xr = xq + (long long)rq * g.ww * nq;
+            const float* Trr = Tr - (zq * g.th + rq) * g.tw;
+            const float4* xr = xq + (long long)(zq * g.wh + rq) * g.ww * nq;
             for (int cq = 0; cq < g.ww; ++cq) {
                 float t;
                 if constexpr (MODE == kModeMatrix) {
-                    const int q = rq * g.ww + cq;
+                    const int q = (zq * g.wh + rq) * g.ww + cq;
                     t = to_f32(reverse ? Mc[(long long)q * g.N + p] : Mc[(long long)p * g.N + q]);
                 } else {
                     t = Trr[-cq];
                 }
                 if constexpr (MODE == kModeFused) {
-                    if (rq == r && cq == cc) t += ident;
+                    if (zq == pz && rq == r && cq == cc) t += ident;
                 }
                 if constexpr (HIER) {
                     if (rq / wl == r / wl && cq / wl == cc / wl) t += Tls[(r - rq + wl - 1) * twl + (cc - cq + wl - 1)];
-                    if (rq == r && cq == cc) t += 2.f;
+                    if (zq == pz && rq == r && cq == cc) t += 2.f;
                 }
                 const float4 v = xr[cq * nq];
                 a0 = fmaf(t, v.x, a0); a1 = fmaf(t, v.y, a1); a2 = fmaf(t, v.z, a2); a3 = fmaf(t, v.w, a3);
@@ -167,14 +176,18 @@ rect_grad_table_kernel(RectGeom g, const E* __restrict__ x, const E* __restrict_
         for (int i = 0; i < kMaxOwn; ++i) {
             const int k = threadIdx.x + i * kThreadsR;
             if (k >= g.nb) break;
-            // bin k = (dr + w_h - 1)(2w_w - 1) + (dc + w_w - 1): pairs p = (rp, cp), q = (rp - dr, cp - dc) inside the window
-            const int dr = k / g.tw - (g.wh - 1), dc = k % g.tw - (g.ww - 1);
+            // bin k = ((dz + w_d - 1)(2w_h - 1) + (dr + w_h - 1))(2w_w - 1) + (dc + w_w - 1): pairs p = (zp, rp, cp),
+            // q = (zp - dz, rp - dr, cp - dc) inside the window
+            const int kz = k / (g.th * g.tw), k2 = k - kz * (g.th * g.tw);
+            const int dz = kz - (g.wd - 1), dr = k2 / g.tw - (g.wh - 1), dc = k2 % g.tw - (g.ww - 1);
+            const int z0 = max(0, dz), z1 = min(g.wd, g.wd + dz);
             const int r0 = max(0, dr), r1 = min(g.wh, g.wh + dr), c0 = max(0, dc), c1 = min(g.ww, g.ww + dc);
             float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
+            for (int zp = z0; zp < z1; ++zp)
             for (int rp = r0; rp < r1; ++rp)
                 for (int cp = c0; cp < c1; ++cp) {
-                    const float4* gp = g4 + (rp * g.ww + cp) * nq;
-                    const float4* xp = x4 + ((rp - dr) * g.ww + cp - dc) * nq;
+                    const float4* gp = g4 + ((zp * g.wh + rp) * g.ww + cp) * nq;
+                    const float4* xp = x4 + (((zp - dz) * g.wh + rp - dr) * g.ww + cp - dc) * nq;
                     for (int q = 0; q < nq; ++q) {
                         const float4 gv = gp[q], xv = xp[q];
                         a0 = fmaf(gv.x, xv.x, a0); a1 = fmaf(gv.y, xv.y, a1); a2 = fmaf(gv.z, xv.z, a2); a3 = fmaf(gv.w, xv.w, a3);
@@ -205,6 +218,20 @@ RectGeom make_rect(const wbmm_desc_t& d, int ww, int wh = 0, int pad_h = 0, int 
     g.N = g.wh * g.ww;
     g.tw = 2 * g.ww - 1; g.nb = (2 * g.wh - 1) * g.tw;
     g.nwin = (long long)d.B * g.nwh * g.nww;
+    g.D = 1; g.wd = 1; g.sd = 0; g.Dp = 1; g.nwd = 1; g.th = 2 * g.wh - 1;
+    return g;
+}
+
+// 3-D windows w_d x (d.w = w_h) x w_w on volumes of depth D, shift (sd, d.shift_h, d.shift_w)
+RectGeom make_win3d(const wbmm_desc_t& d, int D, int wd, int ww, int sd)
+{
+    RectGeom g = make_rect(d, ww);
+    g.D = D; g.wd = wd; g.sd = sd;
+    g.Dp = (D + wd - 1) / wd * wd;
+    g.nwd = g.Dp / wd;
+    g.N = wd * g.wh * g.ww;
+    g.nb = (2 * wd - 1) * g.th * g.tw;
+    g.nwin = (long long)d.B * g.nwd * g.nwh * g.nww;
     return g;
 }
 
@@ -271,6 +298,44 @@ cudaError_t rect_forward(const wbmm_desc_t& d, int ww, const void* x, const void
 cudaError_t rect_grad_table(const wbmm_desc_t& d, int ww, const void* x, const void* dy, float* dT, cudaStream_t s, int* launches)
 {
     const RectGeom g = make_rect(d, ww);
+    if (g.nwin == 0 || g.C == 0) return cudaSuccess;
+    *launches += 1;
+    switch (d.dtype) {
+    case WBMM_DTYPE_F32: return rect_grad_table_t<float>(g, (const float*)x, (const float*)dy, dT, s);
+    case WBMM_DTYPE_BF16: return rect_grad_table_t<__nv_bfloat16>(g, (const __nv_bfloat16*)x, (const __nv_bfloat16*)dy, dT, s);
+    default: return rect_grad_table_t<__half>(g, (const __half*)x, (const __half*)dy, dT, s);
+    }
+}
+
+// ---- 3-D windows (wbmm_forward_win3d / wbmm_backward_win3d)
+bool win3d_supported(const wbmm_desc_t& d, int D, int wd, int ww)
+{
+    if (D < 1 || wd < 1 || ww < 1 || d.w < 1 || wd > 1024 || d.w > 1024 || ww > 1024) return false;
+    const long long N = (long long)wd * d.w * ww, nb = (2ll * wd - 1) * (2ll * d.w - 1) * (2ll * ww - 1);
+    if (N > 1024 || nb > 4096 || d.C > 65535) return false;
+    if ((long long)d.B * d.C > (1ll << 40) / ((long long)D * d.H * d.W)) return false;
+    const RectGeom g = make_win3d(d, D, wd, ww, 0);
+    return (g.nwin + rect_group(g) - 1) / rect_group(g) <= 0x7fffffffll;
+}
+
+cudaError_t win3d_forward(const wbmm_desc_t& d, int D, int wd, int ww, int sd, const void* x, const void* T, void* y, bool reverse,
+                          cudaStream_t s, int* launches)
+{
+    const RectGeom g = make_win3d(d, D, wd, ww, sd);
+    if (g.nwin == 0 || g.C == 0) return cudaSuccess;
+    *launches += 1;
+    switch (d.dtype) {
+    case WBMM_DTYPE_F32: return rect_forward_t<float, kModeTable>(g, (const float*)x, (const float*)T, nullptr, (float*)y, reverse, s);
+    case WBMM_DTYPE_BF16: return rect_forward_t<__nv_bfloat16, kModeTable>(g, (const __nv_bfloat16*)x, (const __nv_bfloat16*)T, nullptr, (__nv_bfloat16*)y, reverse, s);
+    default: return rect_forward_t<__half, kModeTable>(g, (const __half*)x, (const __half*)T, nullptr, (__half*)y, reverse, s);
+    }
+}
+
+// adds into dT (the caller clears it)
+cudaError_t win3d_grad_table(const wbmm_desc_t& d, int D, int wd, int ww, int sd, const void* x, const void* dy, float* dT,
+                             cudaStream_t s, int* launches)
+{
+    const RectGeom g = make_win3d(d, D, wd, ww, sd);
     if (g.nwin == 0 || g.C == 0) return cudaSuccess;
     *launches += 1;
     switch (d.dtype) {
