@@ -378,6 +378,18 @@ def other_rooflines(wb, dev, stream, hbm_peak):
     del dr, Tr, yr
     torch.cuda.empty_cache()
 
+    # 3-D windows 2 x 7 x 7 (the FFMA kernels with a depth axis, section 7.10 of DESIGN.md) on a video-shaped volume: context
+    g3 = torch.Generator().manual_seed(94)
+    x3 = torch.randn((16, 96, 8, 56, 56), generator=g3).to(torch.bfloat16).to(dev)
+    T3 = (torch.randn((96, 3 * 13 * 13), generator=g3) * 0.02).to(torch.bfloat16).to(dev)
+    y3 = torch.empty_like(x3)
+    ms = region_ms_rot(lambda i: wb.wbmm_forward_win3d(x3, T3, (2, 7, 7), out=y3), 5, stream)
+    out["win3d_2x7x7_B16_C96_8x56x56_fwd"] = {"ms": round(ms, 5), "tflops": round(2.0 * 98 * x3.numel() / ms / 1e9, 2),
+                                             "frac": round(4.0 * x3.numel() / (hbm_peak * 1e9) * 1e3 / ms, 4),
+                                             "path": wb.wbmm_path_string(wb.wbmm_last_path())}
+    del x3, T3, y3
+    torch.cuda.empty_cache()
+
     # INT8 forward (tcgen05 kind::i8, section 7.11 of DESIGN.md) on the shapes of configs 3 and 2: int8 in, int8 out
     # (requantised): 2 bytes per element of algorithmic traffic; int32 out: 5 bytes
     for ci in (si.with_(si.CFG3, backward=False), si.with_(si.CFG2, backward=False)):
