@@ -34,14 +34,27 @@ __device__ __forceinline__ long long rect_offset(const RectGeom& g, int b, int c
 }
 
 // element of the zero-extended, cyclically shifted frame that window `win` holds at in-window position p; -1 = padding
+// (VOL = false: the 2-D problems, D = w_d = 1 -- the depth arithmetic compiles away)
+template <bool VOL>
 __device__ __forceinline__ long long rect_window_elem(const RectGeom& g, long long win, int p, int c)
 {
-    const int wps = g.nwh * g.nww, wpi = g.nwd * wps;
+    if constexpr (!VOL) {
+        const int wpi = g.nwh * g.nww;
+        const int b = (int)(win / wpi), wl = (int)(win - (long long)b * wpi);
+        const int wy = wl / g.nww, wx = wl - wy * g.nww;
+        int h = wy * g.wh + p / g.ww + g.sh, v = wx * g.ww + p % g.ww + g.sw;
+        if (h >= g.Hp) h -= g.Hp;
+        if (v >= g.Wp) v -= g.Wp;
+        if (h >= g.H || v >= g.W) return -1;
+        if (g.layout == WBMM_LAYOUT_NCHW) return (((long long)b * g.C + c) * g.H + h) * g.W + v;
+        return (((long long)b * g.H + h) * g.W + v) * g.C + c;
+    }
+    const int wps = g.nwh * g.nww, wpi = VOL ? g.nwd * wps : wps;
     const int b = (int)(win / wpi), wv = (int)(win - (long long)b * wpi);
-    const int wz = wv / wps, wl = wv - wz * wps;
+    const int wz = VOL ? wv / wps : 0, wl = wv - wz * wps;
     const int wy = wl / g.nww, wx = wl - wy * g.nww;
-    const int area = g.wh * g.ww, pz = p / area, p2 = p - pz * area;
-    int z = wz * g.wd + pz + g.sd, h = wy * g.wh + p2 / g.ww + g.sh, v = wx * g.ww + p2 % g.ww + g.sw;
+    const int area = g.wh * g.ww, pz = VOL ? p / area : 0, p2 = p - pz * area;
+    int z = VOL ? wz * g.wd + pz + g.sd : 0, h = wy * g.wh + p2 / g.ww + g.sh, v = wx * g.ww + p2 % g.ww + g.sw;
     if (z >= g.Dp) z -= g.Dp;
     if (h >= g.Hp) h -= g.Hp;
     if (v >= g.Wp) v -= g.Wp;
@@ -59,7 +72,7 @@ __device__ __forceinline__ long long rect_window_elem(const RectGeom& g, long lo
 // for float32 and for window sizes without a tensor-core kernel.
 enum { kModeTable = 0, kModeHier = 1, kModeFused = 2, kModeMatrix = 3 };
 
-template <typename E, int MODE>
+template <typename E, int MODE, bool VOL>
 __global__ void __launch_bounds__(kThreadsR)
 rect_forward_kernel(RectGeom g, const E* __restrict__ x, const E* __restrict__ T, const E* __restrict__ Tl, E* __restrict__ y, int G, int reverse,
                     float ident)
@@ -87,7 +100,7 @@ rect_forward_kernel(RectGeom g, const E* __restrict__ x, const E* __restrict__ T
         const int gw = idx / g.N, p = idx - gw * g.N;
         float val = 0.f;
         if (win0 + gw < g.nwin) {
-            const long long off = rect_window_elem(g, win0 + gw, p, c);
+            const long long off = rect_window_elem<VOL>(g, win0 + gw, p, c);
             if (off >= 0) val = to_f32(x[off]);
         }
         xs[p * G + gw] = val;
@@ -96,14 +109,16 @@ rect_forward_kernel(RectGeom g, const E* __restrict__ x, const E* __restrict__ T
     const int nq = G / 4;
     for (int idx = threadIdx.x; idx < nq * g.N; idx += kThreadsR) {
         const int gq = idx / g.N, p = idx - gq * g.N;
-        const int area = g.wh * g.ww, pz = p / area, p2 = p - pz * area;
+        const int area = g.wh * g.ww, pz = VOL ? p / area : 0, p2 = p - pz * area;
         const int r = p2 / g.ww, cc = p2 - r * g.ww;
+        const int wdn = VOL ? g.wd : 1;
         // Eq. 7 with i = p (output), j = q (input): k = ((pz - zq + w_d - 1)(2w_h - 1) + (r - rq + w_h - 1))(2w_w - 1) + (cc - cq + w_w - 1)
-        const float* Tr = Ts + ((pz + g.wd - 1) * g.th + r + g.wh - 1) * g.tw + cc + g.ww - 1;
+        const float* Tr = VOL ? Ts + ((pz + g.wd - 1) * g.th + r + g.wh - 1) * g.tw + cc + g.ww - 1
+                              : Ts + (r + g.wh - 1) * g.tw + cc + g.ww - 1;
         const float4* xq = reinterpret_cast<const float4*>(xs) + gq;
         float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
         const E* Mc = T + (long long)c * g.N * g.N;                 // MODE 3: this channel's matrix
-        for (int zq = 0; zq < g.wd; ++zq)
+        for (int zq = 0; zq < wdn; ++zq)
         for (int rq = 0; rq < g.wh; ++rq) {
             const float* Trr = Tr - (zq * g.th + rq) * g.tw;
             const float4* xr = xq + (long long)(zq * g.wh + rq) * g.ww * nq;
@@ -135,13 +150,13 @@ rect_forward_kernel(RectGeom g, const E* __restrict__ x, const E* __restrict__ T
         for (int u = 0; u < 4; ++u) {
             const long long win = win0 + gq * 4 + u;
             if (win >= g.nwin) break;
-            const long long off = rect_window_elem(g, win, p, c);
+            const long long off = rect_window_elem<VOL>(g, win, p, c);
             if (off >= 0) y[off] = from_f32<E>(acc[u]);          // padding is cropped (Eq. 4-5)
         }
     }
 }
 
-template <typename E>
+template <typename E, bool VOL>
 __global__ void __launch_bounds__(kThreadsR)
 rect_grad_table_kernel(RectGeom g, const E* __restrict__ x, const E* __restrict__ dy, float* __restrict__ dT, int G, int groups_per_block)
 {
@@ -162,7 +177,7 @@ rect_grad_table_kernel(RectGeom g, const E* __restrict__ x, const E* __restrict_
             const int gw = idx / g.N, p = idx - gw * g.N;
             float xv = 0.f, gv = 0.f;
             if (grp * G + gw < g.nwin) {
-                const long long off = rect_window_elem(g, grp * G + gw, p, c);
+                const long long off = rect_window_elem<VOL>(g, grp * G + gw, p, c);
                 if (off >= 0) { xv = to_f32(x[off]); gv = to_f32(dy[off]); }      // dy is zero outside H x W (A11)
             }
             xs[p * G + gw] = xv;          // position-major: four windows per 16-byte load (G is a multiple of 4)
@@ -178,9 +193,9 @@ rect_grad_table_kernel(RectGeom g, const E* __restrict__ x, const E* __restrict_
             if (k >= g.nb) break;
             // bin k = ((dz + w_d - 1)(2w_h - 1) + (dr + w_h - 1))(2w_w - 1) + (dc + w_w - 1): pairs p = (zp, rp, cp),
             // q = (zp - dz, rp - dr, cp - dc) inside the window
-            const int kz = k / (g.th * g.tw), k2 = k - kz * (g.th * g.tw);
-            const int dz = kz - (g.wd - 1), dr = k2 / g.tw - (g.wh - 1), dc = k2 % g.tw - (g.ww - 1);
-            const int z0 = max(0, dz), z1 = min(g.wd, g.wd + dz);
+            const int kz = VOL ? k / (g.th * g.tw) : 0, k2 = k - kz * (g.th * g.tw);
+            const int dz = VOL ? kz - (g.wd - 1) : 0, dr = k2 / g.tw - (g.wh - 1), dc = k2 % g.tw - (g.ww - 1);
+            const int z0 = VOL ? max(0, dz) : 0, z1 = VOL ? min(g.wd, g.wd + dz) : 1;
             const int r0 = max(0, dr), r1 = min(g.wh, g.wh + dr), c0 = max(0, dc), c1 = min(g.ww, g.ww + dc);
             float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
             for (int zp = z0; zp < z1; ++zp)
@@ -243,7 +258,8 @@ cudaError_t rect_forward_t(const RectGeom& g, const E* x, const E* T, const E* T
     const int G = rect_group(g);
     const int nbl = (g.wh - 1) * (g.wh - 1);
     const size_t smem = sizeof(float) * ((size_t)g.nb + (MODE == kModeHier ? nbl : 0) + (size_t)G * g.N);
-    auto k = rect_forward_kernel<E, MODE>;
+    auto k = rect_forward_kernel<E, MODE, false>;
+    if constexpr (MODE == kModeTable) { if (g.D > 1 || g.wd > 1) k = rect_forward_kernel<E, MODE, true>; }      // volumes: the table operator only
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     dim3 grid((unsigned)((g.nwin + G - 1) / G), (unsigned)g.C);
@@ -256,7 +272,7 @@ cudaError_t rect_grad_table_t(const RectGeom& g, const E* x, const E* dy, float*
 {
     const int G = rect_group(g, g.nb >= kThreadsR ? 2048 : 1024);      // few bins (1-D windows): smaller groups, more blocks
     const size_t smem = sizeof(float) * 2 * (size_t)G * g.N;
-    auto k = rect_grad_table_kernel<E>;
+    auto k = (g.D > 1 || g.wd > 1) ? rect_grad_table_kernel<E, true> : rect_grad_table_kernel<E, false>;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const long long ngroups = (g.nwin + G - 1) / G;
