@@ -53,6 +53,8 @@ struct I8Tiles {
     long long ntiles;
     int vec;                 // rows can move as aligned 32-bit words (NCHW, no column shift, W' = W, W % 4 == 0)
     int bulk;                // plane strips are contiguous 16-byte aligned runs: the bulk-copy kernel serves (see i8_tiles)
+    int flat;                // gather kernel: a plane strip is ONE contiguous run (NCHW, no shift, H and W multiples of w),
+                             // copied by a warp in units of `flat` bytes (4 or 1) without per-element index arithmetic
 };
 
 // kind::i8: c_format S32 (2), a / b signed 8-bit (1).  kind::f8f6f4: c_format F32 (1), a / b E4M3 (0).  K-major both.
@@ -289,7 +291,35 @@ tc_i8_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t* __r
             if (v >= g.Wp) v -= g.Wp;
             return h < g.H && v < g.W ? act_offset(g, b0 + p, c, h, v) : -1;
         };
-        if (tl.vec) {
+        const int strip_elems = min(tl.NSY, g.nwh - wy0) * WS * g.Wp;                 // flat mode: the strip's run
+        const long long strip_off = (long long)c * g.H * g.W + (long long)wy0 * WS * g.Wp;    // ... inside image b's block
+        const long long img_pitch = (long long)g.C * g.H * g.W;
+        if (tl.flat == 4) {
+            const int nu = strip_elems >> 2;
+            for (int p = warp; p < np_eff; p += kThreadsI / 32) {
+                const uint32_t* sp = reinterpret_cast<const uint32_t*>(x + (b0 + p) * img_pitch + strip_off);
+                uint32_t* dp = reinterpret_cast<uint32_t*>(frame + p * tl.S);
+                for (int u = lane; u < nu; u += 128) {
+                    uint32_t val[4];
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) if (u + 32 * k < nu) val[k] = sp[u + 32 * k];
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) if (u + 32 * k < nu) dp[u + 32 * k] = val[k];
+                }
+            }
+        } else if (tl.flat == 1) {
+            for (int p = warp; p < np_eff; p += kThreadsI / 32) {
+                const int8_t* sp = x + (b0 + p) * img_pitch + strip_off;
+                uint8_t* dp = frame + p * tl.S;
+                for (int u = lane; u < strip_elems; u += 128) {
+                    uint8_t val[4];
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) if (u + 32 * k < strip_elems) val[k] = (uint8_t)sp[u + 32 * k];
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) if (u + 32 * k < strip_elems) dp[u + 32 * k] = val[k];
+                }
+            }
+        } else if (tl.vec) {
             const int fw = frame_elems >> 2, nfw = np_eff * fw;
             for (int base = tid; base < nfw; base += 8 * kThreadsI) {
                 uint32_t val[8];
@@ -378,7 +408,20 @@ tc_i8_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t* __r
         }
         __syncthreads();
         // y <- frame (un-shift, crop)
-        if constexpr (OUT8) {
+        if (tl.flat) {
+            constexpr int ES = OUT8 ? 1 : 4;
+            const bool words = !OUT8 || tl.flat == 4;
+            const int nu = words ? strip_elems * ES / 4 : strip_elems;
+            for (int p = warp; p < np_eff; p += kThreadsI / 32) {
+                uint8_t* dp = static_cast<uint8_t*>(yv) + ((b0 + p) * img_pitch + strip_off) * ES;
+                const uint8_t* sp = OUT8 ? frame + p * tl.S : reinterpret_cast<const uint8_t*>(oframe + p * frame_elems);
+                if (words) {
+                    for (int u = lane; u < nu; u += 32) reinterpret_cast<uint32_t*>(dp)[u] = reinterpret_cast<const uint32_t*>(sp)[u];
+                } else {
+                    for (int u = lane; u < nu; u += 32) dp[u] = sp[u];
+                }
+            }
+        } else if constexpr (OUT8) {
             if (tl.vec) {
                 const int fw = frame_elems >> 2, nfw = np_eff * fw;
                 for (int idx = tid; idx < nfw; idx += kThreadsI) {
@@ -605,6 +648,8 @@ bool i8_tiles(const Geom& g, const void* x, const void* y, bool out8, I8Tiles* t
     // bulk-copy kernel: every plane strip is one contiguous run whose address and size are multiples of 16 bytes
     const bool al16 = reinterpret_cast<uintptr_t>(x) % 16 == 0 && reinterpret_cast<uintptr_t>(y) % 16 == 0;
     const long long plane = (long long)g.H * g.W;
+    const bool plain = g.layout == WBMM_LAYOUT_NCHW && g.sh == 0 && g.sw == 0 && g.Hp == g.H && g.Wp == g.W;
+    t->flat = !plain ? 0 : ((plane % 4 == 0 && (g.w * g.W) % 4 == 0 && al) ? 4 : 1);
     t->bulk = (g.layout == WBMM_LAYOUT_NCHW && g.sh == 0 && g.sw == 0 && g.Hp == g.H && g.Wp == g.W && al16 && plane % 16 == 0 &&
                (t->nstrips == 1 || (g.w * g.W) % 16 == 0) && x != nullptr) ? 1 : 0;
     return true;
