@@ -461,17 +461,24 @@ tc_i8_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t* __r
 //   wait full | windows: frame -> registers -> A (16-byte chunks, conflict-free) | sync | load of tile t+1 starts
 //   7 (w = 14) / 2 (w = 7) MMAs | tcgen05.ld -> requantise -> output planes (over the A tile) | sync | 16-byte stores
 // (A bulk store would have to be waited for before the next A tile overwrites its source: measured 2.5 us per tile.)
+// MT: 128-window sub-tiles per tile.  At w = 7 a 128-window tile is 6 KB and its fixed costs (barriers, MMA round trip,
+// tile arithmetic) dominate: four sub-tiles share them (4 x 64 TMEM columns, two CTAs per SM).
 template <int WS, bool OUT8>
-constexpr int i8_ctas() { return WS == 7 ? 3 : (OUT8 ? 2 : 1); }
+constexpr int i8_mt() { return (WS == 7 && OUT8) ? 4 : 1; }
+template <int WS, bool OUT8>
+constexpr int i8_ctas() { return WS == 7 ? (OUT8 ? 2 : 3) : (OUT8 ? 2 : 1); }
 
 template <int WS, bool OUT8>
 struct I8Fast {
     using Cf = I8Cfg<WS>;
-    static constexpr int OUT_BYTES = OUT8 ? Cf::FRAME_BYTES : 128 * Cf::N * 4;
-    static constexpr int AO_BYTES = (Cf::A_BYTES > OUT_BYTES ? Cf::A_BYTES : OUT_BYTES);
+    static constexpr int MT = i8_mt<WS, OUT8>();
+    static constexpr int FRAME_BYTES = MT * Cf::FRAME_BYTES;
+    static constexpr int OUT_BYTES = OUT8 ? FRAME_BYTES : MT * 128 * Cf::N * 4;
+    static constexpr int AO_BYTES = (MT * Cf::A_BYTES > OUT_BYTES ? MT * Cf::A_BYTES : OUT_BYTES);
+    static constexpr int D_COLS = MT * Cf::N_PAD <= 32 ? 32 : (MT * Cf::N_PAD <= 64 ? 64 : (MT * Cf::N_PAD <= 128 ? 128 : (MT * Cf::N_PAD <= 256 ? 256 : 512)));
     static constexpr int OFF_TS = Cf::WC_BYTES;
     static constexpr int OFF_FRAME = (OFF_TS + Cf::TS_BYTES + 127) / 128 * 128;
-    static constexpr int OFF_AO = (OFF_FRAME + Cf::FRAME_BYTES + 127) / 128 * 128;
+    static constexpr int OFF_AO = (OFF_FRAME + FRAME_BYTES + 127) / 128 * 128;
     static constexpr int SMEM = OFF_AO + AO_BYTES;
 };
 
@@ -492,7 +499,8 @@ tc_i8_bulk_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const uint32_t mma_bar = ptx::smem_u32(&bars[0]), full_bar = ptx::smem_u32(&bars[1]);
-    if (warp == 0) ptx::tmem_alloc(ptx::smem_u32(&tmem_base_s), Cf::D_COLS_ALLOC);
+    constexpr int MT = Sm::MT;
+    if (warp == 0) ptx::tmem_alloc(ptx::smem_u32(&tmem_base_s), Sm::D_COLS);
     if (tid == 32) {
         ptx::mbar_init(mma_bar, 1);
         ptx::mbar_init(full_bar, 1);
@@ -512,12 +520,21 @@ tc_i8_bulk_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t
     int cur_c = -1;
     uint32_t phase = 0;
 
+    // this thread's windows: row m of sub-tile s is window m + 128 s of the tile = (wl, pl) with m + 128 s = wl * NP + pl
+    // (recomputed where used: held in registers across the tile loop -- plain or packed -- they push the kernels with
+    // 80 or 128 registers into spills inside the hot loops: int32-out 59 -> 88 us at w = 7, 87 -> 97 us at w = 14)
     const int m = tid & 127;
-    const int wl = m / tl.NP, pl = m % tl.NP;
-    const int wyl = wl / g.nww, wx = wl % g.nww;
-    const bool in_frame = wl < tl.NSY * g.nww;
-    const int win_off = in_frame ? (wyl * WS) * g.W + wx * WS : 0;
-    const uint8_t* win = frame + pl * tl.S + win_off;
+    struct Win { int pl, wyl, off; bool in; };
+    auto window_of = [&](int s) -> Win {
+        const int ms = m + 128 * s;
+        const int wl = ms / tl.NP;
+        Win w;
+        w.pl = ms - wl * tl.NP;
+        w.wyl = wl / g.nww;
+        w.in = wl < tl.NSY * g.nww;
+        w.off = w.in ? (w.wyl * WS) * g.W + (wl - w.wyl * g.nww) * WS : 0;
+        return w;
+    };
 
     struct Tile { int c, b0, wy0, np, bytes; };
     auto tile_at = [&](long long t) -> Tile {
@@ -550,8 +567,13 @@ tc_i8_bulk_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t
         // half of the K chunks, warps 4-7 the rest
         {
             constexpr int KCH = (Cf::K_PAD / 16 + 1) / 2;
-            if (warp < 4) stage_window_i8<WS, 0, KCH>(win, rowB, ao + m * 16);
-            else stage_window_i8<WS, KCH, Cf::K_PAD / 16>(win, rowB, ao + m * 16);
+#pragma unroll
+            for (int s = 0; s < MT; ++s) {
+                const Win wn = window_of(s);
+                const uint8_t* win = frame + wn.pl * tl.S + wn.off;
+                if (warp < 4) stage_window_i8<WS, 0, KCH>(win, rowB, ao + s * Cf::A_BYTES + m * 16);
+                else stage_window_i8<WS, KCH, Cf::K_PAD / 16>(win, rowB, ao + s * Cf::A_BYTES + m * 16);
+            }
         }
         ptx::fence_proxy_async_smem();   // A and W_c (generic-proxy stores) -> tcgen05.mma operand reads
         __syncthreads();                 // the frame has been read: the next tile may land in it
@@ -560,22 +582,27 @@ tc_i8_bulk_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t
             ptx::tc_fence_after_sync();
             const uint32_t wc_addr = ptx::smem_u32(Wc), a_addr = ptx::smem_u32(ao);
 #pragma unroll
-            for (int ks = 0; ks < Cf::KSTEPS; ++ks) {
-                const uint64_t adesc = ptx::smem_desc_kmajor_noswz(a_addr + ks * 2 * Cf::A_LBO, Cf::A_LBO, 128);
-                const uint64_t bdesc = ptx::smem_desc_kmajor_noswz(wc_addr + ks * 2 * Cf::LBO, Cf::LBO, 128);
-                mma_ss_i8<F8>(tmem_d, adesc, bdesc, idesc, ks > 0 ? 1u : 0u);
-            }
+            for (int s = 0; s < MT; ++s)
+#pragma unroll
+                for (int ks = 0; ks < Cf::KSTEPS; ++ks) {
+                    const uint64_t adesc = ptx::smem_desc_kmajor_noswz(a_addr + s * Cf::A_BYTES + ks * 2 * Cf::A_LBO, Cf::A_LBO, 128);
+                    const uint64_t bdesc = ptx::smem_desc_kmajor_noswz(wc_addr + ks * 2 * Cf::LBO, Cf::LBO, 128);
+                    mma_ss_i8<F8>(tmem_d + s * Cf::N_PAD, adesc, bdesc, idesc, ks > 0 ? 1u : 0u);
+                }
             ptx::mma_commit(mma_bar);
         }
         ptx::mbar_wait(mma_bar, phase);
         phase ^= 1;
         ptx::tc_fence_after_sync();
-        {   // all 8 warps: warp w and warp w+4 share the TMEM lanes of windows 32(w%4) .. +31 and take half the columns each
-            const bool valid = in_frame && pl < q.np && q.wy0 + wyl < g.nwh;
-            const uint32_t td = tmem_d + ((uint32_t)((warp & 3) * 32) << 16);
+        // all 8 warps: warp w and warp w+4 share the TMEM lanes of windows 32(w%4) .. +31 and take half the columns each
+#pragma unroll
+        for (int s = 0; s < MT; ++s) {
+            const Win wn = window_of(s);
+            const bool valid = wn.in && wn.pl < q.np && q.wy0 + wn.wyl < g.nwh;
+            const uint32_t td = tmem_d + s * Cf::N_PAD + ((uint32_t)((warp & 3) * 32) << 16);
             const float sc = OUT8 ? scale[q.c] : 0.f;
             const uint64_t sc2 = pack_f2(sc, sc);
-            uint8_t* owin = ao + pl * So + win_off * (OUT8 ? 1 : 4);
+            uint8_t* owin = ao + wn.pl * So + wn.off * (OUT8 ? 1 : 4);
             constexpr int NCH = Cf::N_PAD / 16, CH_SPLIT = (NCH + 1) / 2;
 #pragma unroll
             for (int ch = 0; ch < NCH; ++ch) {
@@ -627,14 +654,15 @@ tc_i8_bulk_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t
     }
     ptx::tc_fence_before_sync();
     __syncthreads();
-    if (warp == 0) ptx::tmem_dealloc(tmem_d, Cf::D_COLS_ALLOC);
+    if (warp == 0) ptx::tmem_dealloc(tmem_d, Sm::D_COLS);
 }
 
-bool i8_tiles(const Geom& g, const void* x, const void* y, bool out8, I8Tiles* t)
+// cap: windows per tile (128, or 128 * MT for the bulk-copy kernel's sub-tiled form)
+bool i8_tiles(const Geom& g, const void* x, const void* y, bool out8, I8Tiles* t, int cap = 128)
 {
     if (g.nww > 128 || g.nww < 1) return false;
-    t->NSY = g.nwh < 128 / g.nww ? g.nwh : 128 / g.nww;
-    t->NP = t->NSY == g.nwh ? 128 / (g.nwh * g.nww) : 1;
+    t->NSY = g.nwh < cap / g.nww ? g.nwh : cap / g.nww;
+    t->NP = t->NSY == g.nwh ? cap / (g.nwh * g.nww) : 1;
     if (t->NP < 1) t->NP = 1;
     if (t->NP > g.B) t->NP = g.B > 0 ? g.B : 1;
     t->nstrips = (g.nwh + t->NSY - 1) / t->NSY;
@@ -698,6 +726,12 @@ cudaError_t tc_i8_forward(const Geom& g, const int8_t* x, const int8_t* T, const
 {
     I8Tiles tl;
     if (!i8_tiles(g, x, y, scale != nullptr, &tl)) return cudaErrorInvalidValue;
+    if (tl.bulk && g.w == 7) {          // the sub-tiled form: 4 (8-bit output) or 2 (32-bit output) x 128 windows per tile
+        I8Tiles t4;
+        const int mt = scale ? i8_mt<7, true>() : i8_mt<7, false>();
+        if (i8_tiles(g, x, y, scale != nullptr, &t4, 128 * mt) && t4.bulk) tl = t4;
+        else tl.bulk = 0;
+    }
     *path = tl.bulk ? WBMM_PATH_TC_TMA : WBMM_PATH_TC_GATHER;
     if (tl.ntiles == 0) return cudaSuccess;
     auto go = [&](auto ws, auto f8) -> cudaError_t {
