@@ -73,6 +73,22 @@ def test_fp8_forward_against_the_exact_operator(wb, oracle, case):
     assert np.abs(oracle.e4m3_decode(codes(q))).max() >= 16.0   # the scales exercise the range
 
 
+@pytest.mark.parametrize("w", [14, 7])
+def test_fp8_full_size_headline_shape(wb, oracle, w):
+    """B128 C96 56x56 (the headline shape of BASELINE.json in E4M3), whole tensor, in the launch configuration bench.py times."""
+    case = si.Case("f8_full", 128, 96, 56, 56, w, seed=950 + w)
+    d = si.make_fp8(case, device="cuda")
+    xc, Tc, sc = codes(d["x"]), codes(d["T"]), d["scale"].cpu().numpy().astype(np.float64)
+    ref = oracle.forward_fp8(xc, Tc, w)
+    mag = oracle.forward(np.abs(oracle.e4m3_decode(xc)), np.abs(oracle.e4m3_decode(Tc)), w)
+    y = wb.wbmm_forward_fp8(d["x"], d["T"], w).cpu().numpy().astype(np.float64)
+    assert wb.wbmm_last_path() == wb.PATH_TC_TMA
+    assert np.all(np.abs(y - ref) <= ACC_EPS * mag + 1e-30)
+    q = wb.wbmm_forward_fp8(d["x"], d["T"], w, scale=d["scale"])
+    scb = sc[None, :, None, None]
+    assert check_codes(codes(q), ref * scb, (ACC_EPS * mag + np.abs(ref) * 2.0 ** -23) * np.abs(scb), oracle) > 0.99
+
+
 @pytest.mark.parametrize("w", [7, 14])
 def test_fp8_one_hot_table_every_bin_is_exact(wb, oracle, w):
     """One bin = +-1 or +-2 per channel: every output is a signed, scaled copy of one input -- exact in float32."""

@@ -138,6 +138,23 @@ def test_int8_full_size_headline_shape(wb, oracle):
     assert np.array_equal(y8.cpu().numpy(), oracle.forward_int8(d["x"].cpu().numpy(), d["T"].cpu().numpy(), 7, scale=d["scale"].cpu().numpy()))
 
 
+def test_int8_full_size_shifted_and_nhwc(wb, oracle):
+    """Config 5's shape (B64 C192 28x28 w=14 shift 7,7) and the headline shape in NHWC, whole tensors: the gather kernel and the
+    transposition route at full size."""
+    case = si.Case("i8_cfg5", 64, 192, 28, 28, 14, shift=(7, 7), seed=860)
+    d = si.make_int8(case, device="cuda")
+    y8 = wb.wbmm_forward_int8(d["x"], d["T"], 14, case.shift, scale=d["scale"])
+    assert wb.wbmm_last_path() == wb.PATH_TC_GATHER
+    assert np.array_equal(y8.cpu().numpy(), oracle.forward_int8(d["x"].cpu().numpy(), d["T"].cpu().numpy(), 14, case.shift,
+                                                                 scale=d["scale"].cpu().numpy()))
+    case = si.Case("i8_cfg3_nhwc", 128, 96, 56, 56, 14, layout=NHWC, seed=861)
+    d = si.make_int8(case, device="cuda")
+    y8 = wb.wbmm_forward_int8(d["x"], d["T"], 14, layout=NHWC, scale=d["scale"])
+    assert wb.wbmm_last_path() == wb.PATH_TC_TRANSPOSED
+    assert np.array_equal(y8.cpu().numpy(), oracle.forward_int8(d["x"].cpu().numpy(), d["T"].cpu().numpy(), 14, layout=NHWC,
+                                                                 scale=d["scale"].cpu().numpy()))
+
+
 def test_int8_unsupported_and_argument_errors(wb):
     x = torch.zeros((1, 2, 10, 10), dtype=torch.int8, device="cuda")
     n0 = wb.wbmm_launch_count()
