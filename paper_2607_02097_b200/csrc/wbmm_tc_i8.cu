@@ -11,7 +11,7 @@
 //   * D: 128 lanes x N_PAD int32 columns, read back with tcgen05.ld.
 // Two kernels: tc_i8_bulk_kernel (NCHW, no shift, aligned sizes: bulk copies, two or three CTAs per SM, see there) and
 // tc_i8_kernel, block-synchronous (one tile of up to 128 windows at a time: gather -> TMEM -> MMA -> epilogue ->
-// scatter), any layout / shift / ragged size by index arithmetic, with 32-bit copies where rows allow it.
+// scatter), any layout / shift / ragged size: a warp per frame row, or one run per plane strip for aligned NCHW maps.
 #include <cuda.h>
 
 #include <type_traits>
@@ -44,14 +44,12 @@ struct I8Cfg {
     // pipelined form: A in shared memory (K-major core matrices, 128 rows), D alone in tensor memory
     static constexpr int A_LBO = 128 * 16;
     static constexpr int A_BYTES = (K_PAD / 16) * A_LBO;
-    static constexpr int D_COLS_ALLOC = N_PAD <= 32 ? 32 : (N_PAD <= 64 ? 64 : (N_PAD <= 128 ? 128 : 256));
 };
 
 struct I8Tiles {
     int NP, NSY, nstrips, tiles_per_c;
     int frame_rows, S;       // rows of one frame plane; plane stride in bytes (multiple of 16)
     long long ntiles;
-    int vec;                 // rows can move as aligned 32-bit words (NCHW, no column shift, W' = W, W % 4 == 0)
     int bulk;                // plane strips are contiguous 16-byte aligned runs: the bulk-copy kernel serves (see i8_tiles)
     int flat;                // gather kernel: a plane strip is ONE contiguous run (NCHW, no shift, H and W multiples of w),
                              // copied by a warp in units of `flat` bytes (4 or 1) without per-element index arithmetic
@@ -190,7 +188,6 @@ __device__ __forceinline__ uint32_t requant(uint32_t acc_bits, float scale)
     r = fminf(fmaxf(r, -128.0f), 127.0f);
     return __float_as_uint(__fadd_rn(r, 12582912.0f));
 }
-__device__ __forceinline__ uint32_t pack_q2(uint32_t a, uint32_t b) { return __byte_perm(a, b, 0x0040) & 0xffffu; }
 // Two values at once with the packed binary32 instructions of sm_100 (sub / mul / add .f32x2: each lane is the scalar
 // operation, same rounding); returns q(a0) | q(a1) << 8.
 __device__ __forceinline__ uint64_t pack_f2(float lo, float hi)
@@ -281,16 +278,6 @@ tc_i8_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t* __r
             build_weight_i8<WS>(T + (long long)c * Cf::NB, Ts, Wc, tid);
             cur_c = c;
         }
-        // element `idx` of the frame (plane p, row hh, column vv in padded + shifted coordinates) -> offset in x / y
-        auto src_offset = [&](int p, int r2) -> long long {
-            const int hh = r2 / g.Wp, vv = r2 - hh * g.Wp;
-            const int hp = wy0 * WS + hh;
-            if (hp >= g.Hp) return -1;
-            int h = hp + g.sh, v = vv + g.sw;
-            if (h >= g.Hp) h -= g.Hp;
-            if (v >= g.Wp) v -= g.Wp;
-            return h < g.H && v < g.W ? act_offset(g, b0 + p, c, h, v) : -1;
-        };
         const int strip_elems = min(tl.NSY, g.nwh - wy0) * WS * g.Wp;                 // flat mode: the strip's run
         const long long strip_off = (long long)c * g.H * g.W + (long long)wy0 * WS * g.Wp;    // ... inside image b's block
         const long long img_pitch = (long long)g.C * g.H * g.W;
@@ -319,38 +306,51 @@ tc_i8_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t* __r
                     for (int k = 0; k < 4; ++k) if (u + 32 * k < strip_elems) dp[u + 32 * k] = val[k];
                 }
             }
-        } else if (tl.vec) {
-            const int fw = frame_elems >> 2, nfw = np_eff * fw;
-            for (int base = tid; base < nfw; base += 8 * kThreadsI) {
-                uint32_t val[8];
-#pragma unroll
-                for (int u = 0; u < 8; ++u) {
-                    const int idx = base + u * kThreadsI;
-                    long long off = -1;
-                    if (idx < nfw) { const int p = idx / fw; off = src_offset(p, (idx - p * fw) * 4); }
-                    val[u] = off >= 0 ? *reinterpret_cast<const uint32_t*>(x + off) : 0u;
-                }
-#pragma unroll
-                for (int u = 0; u < 8; ++u) {
-                    const int idx = base + u * kThreadsI;
-                    if (idx < nfw) { const int p = idx / fw; *reinterpret_cast<uint32_t*>(frame + p * tl.S + (idx - p * fw) * 4) = val[u]; }
-                }
-            }
         } else {
-            const int nfe = np_eff * frame_elems;
-            for (int base = tid; base < nfe; base += 8 * kThreadsI) {
-                uint8_t val[8];
+            // general form: a warp per frame row -- the row's source (shifted row, padding) is worked out once, the lanes
+            // walk its columns (column shift and crop by a compare; NHWC by the element stride): no division per element
+            const int nrows = np_eff * tl.frame_rows;
+            const int estride = g.layout == WBMM_LAYOUT_NCHW ? 1 : g.C;
+            const long long rowstride = (long long)g.W * estride;
+            const int8_t* xb = x + act_offset(g, b0, c, 0, 0);           // element (b0 + p, c, h, v) = xb[p * img_pitch + h * rowstride + v * estride]
+            // eight consecutive rows per warp and step, all their loads issued before the first shared-memory store (a row
+            // at a time is one global-memory latency per row); (plane, row) advance by additions -- a division per row and
+            // the general offset arithmetic made this loop 100 M of the kernel's 174 M instructions
+            constexpr int RB = 8;
+            for (int r0 = warp * RB; r0 < nrows; r0 += RB * (kThreadsI / 32)) {
+                const int p0 = r0 / tl.frame_rows, hh0 = r0 - p0 * tl.frame_rows;
+                for (int vv0 = 0; vv0 < g.Wp; vv0 += 64) {
+                    uint8_t val[RB][2];
+                    int p = p0, hh = hh0;
 #pragma unroll
-                for (int u = 0; u < 8; ++u) {
-                    const int idx = base + u * kThreadsI;
-                    long long off = -1;
-                    if (idx < nfe) { const int p = idx / frame_elems; off = src_offset(p, idx - p * frame_elems); }
-                    val[u] = off >= 0 ? (uint8_t)x[off] : (uint8_t)0;
-                }
+                    for (int j = 0; j < RB; ++j) {
+                        const int hp = wy0 * WS + hh;
+                        int h = hp + g.sh;
+                        if (h >= g.Hp) h -= g.Hp;
+                        const bool rowok = r0 + j < nrows && hp < g.Hp && h < g.H;
+                        const int8_t* srow = xb + (rowok ? p * img_pitch + h * rowstride : 0);
 #pragma unroll
-                for (int u = 0; u < 8; ++u) {
-                    const int idx = base + u * kThreadsI;
-                    if (idx < nfe) { const int p = idx / frame_elems; frame[p * tl.S + (idx - p * frame_elems)] = val[u]; }
+                        for (int k = 0; k < 2; ++k) {
+                            const int vv = vv0 + lane + 32 * k;
+                            int v = vv + g.sw;
+                            if (v >= g.Wp) v -= g.Wp;
+                            val[j][k] = (rowok && vv < g.Wp && v < g.W) ? (uint8_t)srow[v * estride] : (uint8_t)0;
+                        }
+                        if (++hh == tl.frame_rows) { hh = 0; ++p; }
+                    }
+                    p = p0; hh = hh0;
+#pragma unroll
+                    for (int j = 0; j < RB; ++j) {
+                        if (r0 + j < nrows) {
+                            uint8_t* drow = frame + p * tl.S + hh * g.Wp;
+#pragma unroll
+                            for (int k = 0; k < 2; ++k) {
+                                const int vv = vv0 + lane + 32 * k;
+                                if (vv < g.Wp) drow[vv] = val[j][k];
+                            }
+                        }
+                        if (++hh == tl.frame_rows) { hh = 0; ++p; }
+                    }
                 }
             }
         }
@@ -421,28 +421,30 @@ tc_i8_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t* __r
                     for (int u = lane; u < nu; u += 32) dp[u] = sp[u];
                 }
             }
-        } else if constexpr (OUT8) {
-            if (tl.vec) {
-                const int fw = frame_elems >> 2, nfw = np_eff * fw;
-                for (int idx = tid; idx < nfw; idx += kThreadsI) {
-                    const int p = idx / fw, r2 = (idx - p * fw) * 4;
-                    const long long off = src_offset(p, r2);
-                    if (off >= 0) *reinterpret_cast<uint32_t*>(y8 + off) = *reinterpret_cast<const uint32_t*>(frame + p * tl.S + r2);
-                }
-            } else {
-                const int nfe = np_eff * frame_elems;
-                for (int idx = tid; idx < nfe; idx += kThreadsI) {
-                    const int p = idx / frame_elems, r2 = idx - p * frame_elems;
-                    const long long off = src_offset(p, r2);
-                    if (off >= 0) y8[off] = (int8_t)frame[p * tl.S + r2];
-                }
-            }
         } else {
-            const int nfe = np_eff * frame_elems;
-            for (int idx = tid; idx < nfe; idx += kThreadsI) {
-                const int p = idx / frame_elems, r2 = idx - p * frame_elems;
-                const long long off = src_offset(p, r2);
-                if (off >= 0) y32[off] = oframe[p * frame_elems + r2];
+            const int nrows = np_eff * tl.frame_rows;
+            const int estride = g.layout == WBMM_LAYOUT_NCHW ? 1 : g.C;
+            const long long rowstride = (long long)g.W * estride;
+            const long long yb = act_offset(g, b0, c, 0, 0);
+            int p = warp / tl.frame_rows, hh = warp - p * tl.frame_rows;       // row rr = warp, warp + 8, ...: (p, hh) by additions
+            for (int rr = warp; rr < nrows; rr += kThreadsI / 32) {
+                const int hp = wy0 * WS + hh;
+                int h = hp + g.sh;
+                if (h >= g.Hp) h -= g.Hp;
+                if (hp < g.Hp && h < g.H) {                                   // padding rows are cropped
+                    const long long rbase = yb + p * img_pitch + h * rowstride;
+                    const int fo = p * (OUT8 ? tl.S : frame_elems) + hh * g.Wp;
+                    for (int vv = lane; vv < g.Wp; vv += 32) {
+                        int v = vv + g.sw;
+                        if (v >= g.Wp) v -= g.Wp;
+                        if (v < g.W) {
+                            if constexpr (OUT8) y8[rbase + v * estride] = (int8_t)frame[fo + vv];
+                            else y32[rbase + v * estride] = oframe[fo + vv];
+                        }
+                    }
+                }
+                hh += kThreadsI / 32;
+                while (hh >= tl.frame_rows) { hh -= tl.frame_rows; ++p; }
             }
         }
         __syncthreads();
@@ -672,7 +674,6 @@ bool i8_tiles(const Geom& g, const void* x, const void* y, bool out8, I8Tiles* t
     if ((t->S / 16) % 2 == 0) t->S += 16;          // 16 * odd: planes start on different banks
     t->ntiles = (long long)g.C * t->tiles_per_c;
     const bool al = reinterpret_cast<uintptr_t>(x) % 4 == 0 && (!out8 || reinterpret_cast<uintptr_t>(y) % 4 == 0);
-    t->vec = (g.layout == WBMM_LAYOUT_NCHW && g.sw == 0 && g.Wp == g.W && g.W % 4 == 0 && al) ? 1 : 0;
     // bulk-copy kernel: every plane strip is one contiguous run whose address and size are multiples of 16 bytes
     const bool al16 = reinterpret_cast<uintptr_t>(x) % 16 == 0 && reinterpret_cast<uintptr_t>(y) % 16 == 0;
     const long long plane = (long long)g.H * g.W;
