@@ -51,6 +51,10 @@ struct I8Tiles {
     int frame_rows, S;       // rows of one frame plane; plane stride in bytes (multiple of 16)
     long long ntiles;
     int bulk;                // plane strips are contiguous 16-byte aligned runs: the bulk-copy kernel serves (see i8_tiles)
+    int rot;                 // gather kernel, NCHW with shift on maps without padding: frame rows hold the SOURCE row unrotated
+                             // (copied in units of `rot` bytes, 4 or 1); the windows read and write their columns rotated by the shift
+    int runs;                // (= rot != 0) a plane strip is TWO contiguous runs of source rows (before / after the row wrap),
+                             // copied like the flat form
     int flat;                // gather kernel: a plane strip is ONE contiguous run (NCHW, no shift, H and W multiples of w),
                              // copied by a warp in units of `flat` bytes (4 or 1) without per-element index arithmetic
 };
@@ -181,6 +185,34 @@ __device__ __forceinline__ void window_to_tmem_i8(const uint8_t* win, bool valid
 // exactly; one binary32 product (no fma); clamping to [-128, 127] BEFORE rounding gives the same integer as after
 // (the bounds are integers, rounding is monotone); adding 1.5 * 2^23 rounds to the nearest integer, ties to even, and
 // leaves the two's-complement value in the low mantissa bits.  The low byte of the result is q.
+// The same from a frame whose rows hold the source row unrotated: column k of the window is at byte v0 + k of the row, or
+// v0 + k - W' once that runs past the row's end (kw = W' - v0 columns come before the wrap; kw >= w: none).
+template <int WS>
+__device__ __forceinline__ void window_to_tmem_i8_rot(const uint8_t* rows, int v0, int kw, int rowB, bool valid, uint32_t taddr)
+{
+    using Cf = I8Cfg<WS>;
+    constexpr int NV = (Cf::A_COLS + 7) / 8 * 8;
+    uint32_t v[NV];
+#pragma unroll
+    for (int k = 0; k < NV; ++k) v[k] = 0u;
+    if (valid) {
+        const uint8_t* pa = rows + v0;
+        const uint8_t* pb = rows + v0 - rowB;
+#pragma unroll
+        for (int r = 0; r < WS; ++r) {
+#pragma unroll
+            for (int k = 0; k < WS; ++k) {
+                const int q = r * WS + k;
+                v[q >> 2] |= (uint32_t)(k < kw ? pa : pb)[r * rowB + k] << ((q & 3) * 8);
+            }
+            asm volatile("" ::: "memory");      // a row at a time: with all w*w loads hoisted the kernel spilled 764 bytes
+        }
+    }
+#pragma unroll
+    for (int ch = 0; ch < NV / 8; ++ch) ptx::tmem_st8(taddr + ch * 8, v + ch * 8);
+    ptx::tmem_wait_st();
+}
+
 __device__ __forceinline__ uint32_t requant(uint32_t acc_bits, float scale)
 {
     const float f = __fsub_rn(__uint_as_float(0x4B400000u + acc_bits), 12582912.0f);
@@ -223,7 +255,9 @@ __device__ __forceinline__ uint32_t out_pair(uint32_t a0, uint32_t a1, float sc,
     else return requant2(a0, a1, sc2);
 }
 
-template <int WS, bool OUT8, bool F8>
+// ROT: the rot / runs forms (NCHW with shift or ragged size) are their own instantiation -- in one kernel with the flat and
+// row forms the register allocation collapsed (255 registers, 892 bytes of spills)
+template <int WS, bool OUT8, bool F8, bool ROT>
 __global__ void __launch_bounds__(kThreadsI, 1)
 tc_i8_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t* __restrict__ T, const float* __restrict__ scale,
              void* __restrict__ yv)
@@ -263,6 +297,12 @@ tc_i8_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t* __r
     const int wyl = wl / g.nww, wx = wl % g.nww;
     const int win_off = (wyl * WS) * g.Wp + wx * WS;
     uint8_t* win = frame + pl * tl.S + win_off;
+    // rot mode: this window's rows start at row_off (bytes of the frame plane / elements of the int32 plane), its columns
+    // at v0 of the unrotated row, kw of them before the wrap
+    const int row_off = (wyl * WS) * g.Wp;
+    int v0 = wx * WS + g.sw;
+    if (v0 >= g.Wp) v0 -= g.Wp;
+    const int kw = g.Wp - v0;
 
     int8_t* y8 = static_cast<int8_t*>(yv);
     int32_t* y32 = static_cast<int32_t*>(yv);
@@ -281,7 +321,7 @@ tc_i8_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t* __r
         const int strip_elems = min(tl.NSY, g.nwh - wy0) * WS * g.Wp;                 // flat mode: the strip's run
         const long long strip_off = (long long)c * g.H * g.W + (long long)wy0 * WS * g.Wp;    // ... inside image b's block
         const long long img_pitch = (long long)g.C * g.H * g.W;
-        if (tl.flat == 4) {
+        if (!ROT && tl.flat == 4) {
             const int nu = strip_elems >> 2;
             for (int p = warp; p < np_eff; p += kThreadsI / 32) {
                 const uint32_t* sp = reinterpret_cast<const uint32_t*>(x + (b0 + p) * img_pitch + strip_off);
@@ -294,7 +334,7 @@ tc_i8_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t* __r
                     for (int k = 0; k < 4; ++k) if (u + 32 * k < nu) dp[u + 32 * k] = val[k];
                 }
             }
-        } else if (tl.flat == 1) {
+        } else if (!ROT && tl.flat == 1) {
             for (int p = warp; p < np_eff; p += kThreadsI / 32) {
                 const int8_t* sp = x + (b0 + p) * img_pitch + strip_off;
                 uint8_t* dp = frame + p * tl.S;
@@ -306,7 +346,36 @@ tc_i8_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t* __r
                     for (int k = 0; k < 4; ++k) if (u + 32 * k < strip_elems) dp[u + 32 * k] = val[k];
                 }
             }
-        } else {
+        } else if (ROT && tl.runs) {
+            // shift without padding: frame rows [0, lenA) <- source rows [s0, s0 + lenA), frame rows [lenA, R) <- source rows
+            // [0, R - lenA): two contiguous runs per plane, a warp per plane
+            const int R = strip_elems / g.W;
+            int s0 = wy0 * WS + g.sh;
+            if (s0 >= g.Hp) s0 -= g.Hp;
+            const int lenA = min(R, g.Hp - s0);
+            const int nA = lenA * g.W / tl.rot, nB = (R - lenA) * g.W / tl.rot;
+            for (int p = warp; p < np_eff; p += kThreadsI / 32) {
+                const int8_t* pb = x + (b0 + p) * img_pitch + (long long)c * g.H * g.W;
+#pragma unroll
+                for (int run = 0; run < 2; ++run) {
+                    const int nu = run ? nB : nA;
+                    const int8_t* sp = pb + (run ? 0 : (long long)s0 * g.W);
+                    uint8_t* dp = frame + p * tl.S + (run ? lenA * g.W : 0);
+                    for (int u = lane; u < nu; u += 128) {
+                        uint32_t val[4];
+#pragma unroll
+                        for (int k = 0; k < 4; ++k)
+                            if (u + 32 * k < nu) val[k] = tl.rot == 4 ? reinterpret_cast<const uint32_t*>(sp)[u + 32 * k] : (uint32_t)(uint8_t)sp[u + 32 * k];
+#pragma unroll
+                        for (int k = 0; k < 4; ++k)
+                            if (u + 32 * k < nu) {
+                                if (tl.rot == 4) reinterpret_cast<uint32_t*>(dp)[u + 32 * k] = val[k];
+                                else dp[u + 32 * k] = (uint8_t)val[k];
+                            }
+                    }
+                }
+            }
+        } else if (!ROT) {
             // general form: a warp per frame row -- the row's source (shifted row, padding) is worked out once, the lanes
             // walk its columns (column shift and crop by a compare; NHWC by the element stride): no division per element
             const int nrows = np_eff * tl.frame_rows;
@@ -359,7 +428,8 @@ tc_i8_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t* __r
 
         const bool valid = wl < tl.NSY * g.nww && pl < np_eff && wy0 + wyl < g.nwh;
         if (warp < 4) {
-            window_to_tmem_i8<WS>(win, valid, rowB, tmem_a + ((uint32_t)(warp * 32) << 16));
+            if constexpr (ROT) window_to_tmem_i8_rot<WS>(frame + pl * tl.S + row_off, v0, kw, rowB, valid, tmem_a + ((uint32_t)(warp * 32) << 16));
+            else window_to_tmem_i8<WS>(win, valid, rowB, tmem_a + ((uint32_t)(warp * 32) << 16));
             ptx::tc_fence_before_sync();
         }
         __syncthreads();
@@ -391,7 +461,11 @@ tc_i8_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t* __r
                         const int i = ch * 16 + e;
                         if (i < Cf::N) {
                             const int r = i / WS, k = i % WS;
-                            if constexpr (!OUT8) {
+                            if constexpr (ROT) {      // column k of the window sits at v0 + k of the unrotated row, wrapped
+                                const int col = r * rowB + k + (k < kw ? v0 : v0 - rowB);
+                                if constexpr (!OUT8) oframe[pl * frame_elems + row_off + col] = (int32_t)v[e];
+                                else frame[pl * tl.S + row_off + col] = (uint8_t)(F8 ? to_e4m3x2(v[e], 0u, sc) : requant(v[e], sc));
+                            } else if constexpr (!OUT8) {
                                 owin[r * rowB + k] = (int32_t)v[e];
                             } else if constexpr (WS % 2 == 0) {
                                 if ((k & 1) == 0)   // (i and i+1 are in the same chunk: 16 and WS are even)
@@ -408,7 +482,7 @@ tc_i8_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t* __r
         }
         __syncthreads();
         // y <- frame (un-shift, crop)
-        if (tl.flat) {
+        if (!ROT && tl.flat) {
             constexpr int ES = OUT8 ? 1 : 4;
             const bool words = !OUT8 || tl.flat == 4;
             const int nu = words ? strip_elems * ES / 4 : strip_elems;
@@ -421,7 +495,26 @@ tc_i8_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t* __r
                     for (int u = lane; u < nu; u += 32) dp[u] = sp[u];
                 }
             }
-        } else {
+        } else if (ROT && tl.runs) {
+            constexpr int ES = OUT8 ? 1 : 4;
+            const int R = strip_elems / g.W;
+            int s0 = wy0 * WS + g.sh;
+            if (s0 >= g.Hp) s0 -= g.Hp;
+            const int lenA = min(R, g.Hp - s0);
+            const bool words = !OUT8 || tl.rot == 4;
+            for (int p = warp; p < np_eff; p += kThreadsI / 32) {
+                uint8_t* pb = static_cast<uint8_t*>(yv) + ((b0 + p) * img_pitch + (long long)c * g.H * g.W) * ES;
+                const uint8_t* fb = OUT8 ? frame + p * tl.S : reinterpret_cast<const uint8_t*>(oframe + p * frame_elems);
+#pragma unroll
+                for (int run = 0; run < 2; ++run) {
+                    const int nbytes = (run ? R - lenA : lenA) * g.W * ES;
+                    uint8_t* dp = pb + (run ? 0 : (long long)s0 * g.W * ES);
+                    const uint8_t* sp = fb + (run ? lenA * g.W * ES : 0);
+                    if (words) for (int u = lane; u < nbytes / 4; u += 32) reinterpret_cast<uint32_t*>(dp)[u] = reinterpret_cast<const uint32_t*>(sp)[u];
+                    else for (int u = lane; u < nbytes; u += 32) dp[u] = sp[u];
+                }
+            }
+        } else if (!ROT) {
             const int nrows = np_eff * tl.frame_rows;
             const int estride = g.layout == WBMM_LAYOUT_NCHW ? 1 : g.C;
             const long long rowstride = (long long)g.W * estride;
@@ -679,6 +772,9 @@ bool i8_tiles(const Geom& g, const void* x, const void* y, bool out8, I8Tiles* t
     const long long plane = (long long)g.H * g.W;
     const bool plain = g.layout == WBMM_LAYOUT_NCHW && g.sh == 0 && g.sw == 0 && g.Hp == g.H && g.Wp == g.W;
     t->flat = !plain ? 0 : ((plane % 4 == 0 && (g.w * g.W) % 4 == 0 && al) ? 4 : 1);
+    // (ragged sizes stay on the row form: whole-row copies into an unrotated frame measured slower there, 366 vs 299 us)
+    t->rot = (plain || g.layout != WBMM_LAYOUT_NCHW || g.Hp != g.H || g.Wp != g.W) ? 0 : ((g.W % 4 == 0 && al) ? 4 : 1);
+    t->runs = t->rot ? 1 : 0;
     t->bulk = (g.layout == WBMM_LAYOUT_NCHW && g.sh == 0 && g.sw == 0 && g.Hp == g.H && g.Wp == g.W && al16 && plane % 16 == 0 &&
                (t->nstrips == 1 || (g.w * g.W) % 16 == 0) && x != nullptr) ? 1 : 0;
     return true;
@@ -704,7 +800,7 @@ cudaError_t launch_i8(const Geom& g, const I8Tiles& tl, const int8_t* x, const i
         return cudaGetLastError();
     }
     const size_t smem = Cf::WC_BYTES + Cf::TS_BYTES + Cf::FRAME_BYTES + (OUT8 ? 0 : 128 * Cf::N * 4);
-    auto kern = tc_i8_kernel<WS, OUT8, F8>;
+    auto kern = tl.rot ? tc_i8_kernel<WS, OUT8, F8, true> : tc_i8_kernel<WS, OUT8, F8, false>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const long long grid = tl.ntiles < sms ? tl.ntiles : sms;

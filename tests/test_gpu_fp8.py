@@ -36,6 +36,8 @@ CASES = [
     si.Case("f8_w7_aligned", 4, 6, 28, 28, 7, seed=907),
     si.Case("f8_w7_shift_ragged", 3, 5, 30, 33, 7, shift=(3, 6), seed=908),
     si.Case("f8_w7_one_window", 131, 3, 7, 7, 7, seed=909),
+    si.Case("f8_w14_shift_unpadded", 5, 4, 56, 56, 14, shift=(7, 7), seed=910),       # rotated-window form
+    si.Case("f8_w7_shift_bytes", 2, 3, 28, 21, 7, shift=(2, 5), seed=911),
 ]
 
 

@@ -33,6 +33,11 @@ CASES = [
     si.Case("i8_w7_one_window", 131, 3, 7, 7, 7, seed=811),
     si.Case("i8_w7_wide", 1, 2, 7, 896, 7, seed=812),                                 # 128 windows across
     si.Case("i8_odd_width", 2, 3, 28, 54, 14, seed=813),                              # W' != W: byte copies
+    si.Case("i8_w14_shift_strips", 2, 3, 224, 224, 14, shift=(5, 9), seed=817),       # two row runs per strip, several strips
+    si.Case("i8_w14_shift_bytes", 3, 4, 28, 42, 14, shift=(3, 11), seed=818),         # W % 4 != 0: byte units
+    si.Case("i8_w7_shift_bytes", 2, 3, 28, 21, 7, shift=(2, 5), seed=819),
+    si.Case("i8_w14_row_shift_only", 4, 3, 56, 28, 14, shift=(9, 0), seed=820),
+    si.Case("i8_w14_col_shift_only", 4, 3, 28, 56, 14, shift=(0, 13), seed=821),
     si.Case("i8_w14_nhwc_t", 5, 32, 28, 56, 14, layout=NHWC, seed=814),               # NHWC through the transposition route
     si.Case("i8_w14_nhwc_t_shift", 3, 96, 56, 56, 14, shift=(7, 5), layout=NHWC, seed=815),
     si.Case("i8_w7_nhwc_t", 4, 80, 28, 28, 7, layout=NHWC, seed=816),                 # C = 64 + 16: a partial tile
