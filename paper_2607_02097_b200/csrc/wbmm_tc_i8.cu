@@ -196,14 +196,16 @@ __device__ __forceinline__ void window_to_tmem_i8_rot(const uint8_t* rows, int v
 #pragma unroll
     for (int k = 0; k < NV; ++k) v[k] = 0u;
     if (valid) {
-        const uint8_t* pa = rows + v0;
-        const uint8_t* pb = rows + v0 - rowB;
+        int offk[WS];                      // byte of the row that holds the window's column k
+#pragma unroll
+        for (int k = 0; k < WS; ++k) offk[k] = k < kw ? v0 + k : v0 + k - rowB;
 #pragma unroll
         for (int r = 0; r < WS; ++r) {
+            const uint8_t* row = rows + r * rowB;
 #pragma unroll
             for (int k = 0; k < WS; ++k) {
                 const int q = r * WS + k;
-                v[q >> 2] |= (uint32_t)(k < kw ? pa : pb)[r * rowB + k] << ((q & 3) * 8);
+                v[q >> 2] |= (uint32_t)row[offk[k]] << ((q & 3) * 8);
             }
             asm volatile("" ::: "memory");      // a row at a time: with all w*w loads hoisted the kernel spilled 764 bytes
         }
@@ -450,6 +452,9 @@ tc_i8_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t* __r
             const uint32_t td = tmem_d + ((uint32_t)(warp * 32) << 16);
             const float sc = OUT8 ? scale[c] : 0.f;
             int32_t* owin = oframe + pl * frame_elems + win_off;
+            int offk[WS];                  // ROT: byte / element of the unrotated row that holds the window's column k
+#pragma unroll
+            for (int k = 0; k < WS; ++k) offk[k] = k < kw ? v0 + k : v0 + k - rowB;
 #pragma unroll
             for (int ch = 0; ch < Cf::N_PAD / 16; ++ch) {
                 uint32_t v[16];
@@ -462,7 +467,7 @@ tc_i8_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t* __r
                         if (i < Cf::N) {
                             const int r = i / WS, k = i % WS;
                             if constexpr (ROT) {      // column k of the window sits at v0 + k of the unrotated row, wrapped
-                                const int col = r * rowB + k + (k < kw ? v0 : v0 - rowB);
+                                const int col = r * rowB + offk[k];
                                 if constexpr (!OUT8) oframe[pl * frame_elems + row_off + col] = (int32_t)v[e];
                                 else frame[pl * tl.S + row_off + col] = (uint8_t)(F8 ? to_e4m3x2(v[e], 0u, sc) : requant(v[e], sc));
                             } else if constexpr (!OUT8) {
