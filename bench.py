@@ -419,6 +419,18 @@ def other_rooflines(wb, dev, stream, hbm_peak):
         del xs, yf, f8
         torch.cuda.empty_cache()
 
+    # INT8 on config 5's shape with its shift (7, 7): the gather kernel's rotated-window form
+    c5i = si.with_(si.CFG5, backward=False)
+    d8 = si.make_int8(c5i, device=dev)
+    ns = buffer_sets(2.0 * c5i.n_elem)
+    xs = [d8["x"]] + [d8["x"].clone() for _ in range(ns - 1)]
+    y8 = [torch.empty_like(d8["x"]) for _ in range(ns)]
+    ms = region_ms_rot(lambda i: wb.wbmm_forward_int8(xs[i % ns], d8["T"], c5i.w, c5i.shift, scale=d8["scale"], out=y8[i % ns]), 20, stream)
+    out["int8_cfg5_shape_shift7_fwd"] = {"ms": round(ms, 5), "frac": round(2.0 * c5i.n_elem / (hbm_peak * 1e9) * 1e3 / ms, 4),
+                                        "path": wb.wbmm_path_string(wb.wbmm_last_path()), "buffer_sets": ns}
+    del xs, y8, d8
+    torch.cuda.empty_cache()
+
     # table gradient at w = 7 (two CTAs per SM) on the config-2 shape
     c2 = si.with_(si.CFG2, backward=True)
     d = si.make(c2, device=dev)
