@@ -428,6 +428,20 @@ tc_i8_kernel(Geom g, I8Tiles tl, const int8_t* __restrict__ x, const int8_t* __r
         ptx::fence_proxy_async_smem();   // W_c (generic-proxy stores) -> tcgen05.mma operand reads
         __syncthreads();
 
+        // the next tile's planes -> L2 while this one is multiplied (one CTA per SM and plain loads: without it every tile
+        // waits out a DRAM round trip; whole-image tiles of the run-copy forms only)
+        if ((tl.flat || tl.runs) && tl.nstrips == 1 && t + 1 < t1) {
+            const int c2 = (int)((t + 1) / tl.tiles_per_c);
+            const int b2 = (int)((t + 1) % tl.tiles_per_c) * tl.NP;
+            const int np2 = min(tl.NP, g.B - b2);
+            const int pbytes = g.H * g.W, lines = (pbytes + 127) >> 7;
+            for (int i = tid; i < np2 * lines; i += kThreadsI) {
+                const int p = i / lines, l = i - p * lines;
+                const int8_t* a = x + (b2 + p) * img_pitch + (long long)c2 * pbytes + min(l << 7, pbytes - 1);
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(a));
+            }
+        }
+
         const bool valid = wl < tl.NSY * g.nww && pl < np_eff && wy0 + wyl < g.nwh;
         if (warp < 4) {
             if constexpr (ROT) window_to_tmem_i8_rot<WS>(frame + pl * tl.S + row_off, v0, kw, rowB, valid, tmem_a + ((uint32_t)(warp * 32) << 16));
